@@ -1,0 +1,528 @@
+// amp_oracle.cpp — TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, event-by-event CPU oracle (FP64; an 80-bit `long double` twin is
+// instantiated from the same template as a tie-breaker) of the per-event unbinned
+// negative log-likelihood of the 4D amplitude model of Sur et al., "A GPU based
+// multidimensional amplitude analysis to search for tetraquark candidates"
+// (PAPER.md, Methodology, Eqs. 1-12 and 14).
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+// legs may load this.  It shares no code, header, table or constant with the CUDA
+// path under paper_2007_14931_b200/csrc and neither includes the other.
+//
+// The method is exact inside one NLL evaluation, so every function below is the
+// paper's definition written out in the paper's order; where the paper is silent
+// the reading (A1..A18) is the one listed in DESIGN.md §"Readings".
+//
+// Parity pins: every function here is pinned by tests/test_oracle_pins.py EXCEPT the
+// orientation of theta_Z (reading A10: literal "angle between K and pi momenta in the
+// Z rest frame") — *parity unpinned* for that one sign convention: the
+// paper gives nothing that distinguishes it from its supplement.
+//
+// Units: MeV; Blatt-Weisskopf radius in MeV^-1.
+
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+enum Kind { KSTAR = 0, ZRES = 1, CONSTANT = 2 };
+
+template <typename T>
+struct Decay {
+    T MB, mpsi, mK, mpi;  // parent, J/psi, K, pi masses
+};
+
+template <typename T>
+struct Resonance {
+    int kind, J;
+    T mass, width, radius;
+};
+
+// ---------------------------------------------------------------------------------
+// O1. Two-body breakup momentum of M -> a b ("momenta ... calculated
+// from the running and pole mass").  Fully factored Kallen form, differences first.
+// Returns NaN below threshold.
+template <typename T>
+T breakup_momentum(T M, T a, T b) {
+    const T s = a + b, d = a - b;
+    const T k = (M - s) * (M + s) * (M - d) * (M + d);
+    if (!(M > 0) || k < 0) return std::numeric_limits<T>::quiet_NaN();
+    return std::sqrt(k) / (2 * M);
+}
+
+// ---------------------------------------------------------------------------------
+// O2. Blatt-Weisskopf barrier factor (ref. [35]; reading A2): z = (r p)^2,
+// F^(L)(p, p0) = sqrt(B_L(z0) / B_L(z)), normalised to 1 at the pole momentum p0.
+template <typename T>
+T barrier_polynomial(int L, T z) {
+    switch (L) {
+        case 0: return T(1);
+        case 1: return 1 + z;
+        case 2: return 9 + 3 * z + z * z;
+        case 3: return 225 + 45 * z + 6 * z * z + z * z * z;
+        case 4: return 11025 + 1575 * z + 135 * z * z + 10 * z * z * z + z * z * z * z;
+    }
+    return std::numeric_limits<T>::quiet_NaN();
+}
+
+template <typename T>
+T blatt_weisskopf(int L, T p, T p0, T r) {
+    const T z = (r * p) * (r * p), z0 = (r * p0) * (r * p0);
+    return std::sqrt(barrier_polynomial(L, z0) / barrier_polynomial(L, z));
+}
+
+// ---------------------------------------------------------------------------------
+// Orbital angular momenta ("lowest L_B is taken as the default"; readings A5, A6).
+inline void orbital_L(int kind, int J, int* LB, int* LR) {
+    if (kind == ZRES) { *LB = 1; *LR = 0; return; }   // 1+ Z: B -> Z K P-wave, Z -> psi pi S-wave
+    *LR = J;                                           // K* -> K pi
+    *LB = (J == 0) ? 1 : J - 1;                        // B(0-) -> psi(1-) K*(J): lowest allowed
+}
+
+// ---------------------------------------------------------------------------------
+// O3. Lineshape, Eqs. (2)-(3) (readings A1, A4).
+//   Gamma(m) = Gamma0 (pR/pR0)^(2LR+1) (MR/m) FR^2
+//   A^R(m)   = FB (pB/MB)^LB FR (pR/m)^LR / (MR^2 - m^2 - i MR Gamma(m))
+// m is the running mass of the resonance's daughters: m_Kpi for a K*, m_psipi for the Z.
+template <typename T>
+std::complex<T> lineshape(const Decay<T>& dk, const Resonance<T>& R, T m, T* gamma_out = nullptr) {
+    if (R.kind == CONSTANT) { if (gamma_out) *gamma_out = 0; return {T(1), T(0)}; }
+    int LB, LR;
+    orbital_L(R.kind, R.J, &LB, &LR);
+    T pB, pB0, pR, pR0;
+    if (R.kind == KSTAR) {
+        pB  = breakup_momentum(dk.MB, m, dk.mpsi);        // K* momentum in the B frame
+        pB0 = breakup_momentum(dk.MB, R.mass, dk.mpsi);
+        pR  = breakup_momentum(m, dk.mK, dk.mpi);         // K momentum in the K* frame
+        pR0 = breakup_momentum(R.mass, dk.mK, dk.mpi);
+    } else {
+        pB  = breakup_momentum(dk.MB, m, dk.mK);          // Z momentum in the B frame
+        pB0 = breakup_momentum(dk.MB, R.mass, dk.mK);
+        pR  = breakup_momentum(m, dk.mpsi, dk.mpi);       // pi momentum in the Z frame
+        pR0 = breakup_momentum(R.mass, dk.mpsi, dk.mpi);
+    }
+    const T FB = blatt_weisskopf(LB, pB, pB0, R.radius);
+    const T FR = blatt_weisskopf(LR, pR, pR0, R.radius);
+    const T gamma = R.width * std::pow(pR / pR0, 2 * LR + 1) * (R.mass / m) * FR * FR;   // Eq. (3)
+    if (gamma_out) *gamma_out = gamma;
+    const T num = FB * std::pow(pB / dk.MB, LB) * FR * std::pow(pR / m, LR);
+    const std::complex<T> den(R.mass * R.mass - m * m, -R.mass * gamma);
+    return std::complex<T>(num, 0) / den;                                                 // Eq. (2)
+}
+
+// ---------------------------------------------------------------------------------
+// O4. Wigner small-d, d^j_{m'm}(beta) = <j m'| exp(-i beta J_y) |j m>, Wigner's factorial sum
+// ("Wigner small-d functions").
+template <typename T>
+T factorial(int n) { T f = 1; for (int i = 2; i <= n; ++i) f *= i; return f; }
+
+template <typename T>
+T wigner_d(int j, int mp, int m, T beta) {
+    const T ch = std::cos(beta / 2), sh = std::sin(beta / 2);
+    T sum = 0;
+    for (int k = 0; k <= 2 * j; ++k) {
+        const int a = j + m - k, b = j - mp - k, c = k, d = k + mp - m;
+        if (a < 0 || b < 0 || c < 0 || d < 0) continue;
+        const T sign = ((k + mp - m) % 2 == 0) ? T(1) : T(-1);
+        sum += sign / (factorial<T>(a) * factorial<T>(b) * factorial<T>(c) * factorial<T>(d)) *
+               std::pow(ch, 2 * j - 2 * k + m - mp) * std::pow(sh, 2 * k - m + mp);
+    }
+    return sum * std::sqrt(factorial<T>(j + m) * factorial<T>(j - m) * factorial<T>(j + mp) * factorial<T>(j - mp));
+}
+
+// ---------------------------------------------------------------------------------
+// plain 4-vector algebra for O6 ("Lorentz boosts and rotations to go from one rest frame to
+// another")
+template <typename T> struct V3 { T x, y, z; };
+template <typename T> struct V4 { T E; V3<T> p; };
+template <typename T> T dot(V3<T> a, V3<T> b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+template <typename T> V3<T> cross(V3<T> a, V3<T> b) { return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x}; }
+template <typename T> V3<T> scale(T s, V3<T> a) { return {s * a.x, s * a.y, s * a.z}; }
+template <typename T> V3<T> add(V3<T> a, V3<T> b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+template <typename T> V3<T> sub(V3<T> a, V3<T> b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+template <typename T> T norm(V3<T> a) { return std::sqrt(dot(a, a)); }
+template <typename T> V3<T> unit(V3<T> a) { return scale(1 / norm(a), a); }
+template <typename T> V4<T> add4(V4<T> a, V4<T> b) { return {a.E + b.E, add(a.p, b.p)}; }
+
+// 4-momentum p seen from a frame that moves with velocity beta (|beta| < 1) relative to the
+// frame in which p is given.
+template <typename T>
+V4<T> boost_to_frame(V4<T> p, V3<T> beta) {
+    const T b2 = dot(beta, beta);
+    if (b2 == 0) return p;
+    const T g = 1 / std::sqrt(1 - b2);
+    const T bp = dot(beta, p.p);
+    V4<T> out;
+    out.E = g * (p.E - bp);
+    out.p = add(p.p, scale((g - 1) * bp / b2 - g * p.E, beta));
+    return out;
+}
+
+// signed dihedral angle about the unit axis a from the direction u to the direction v
+template <typename T>
+T dihedral(V3<T> a, V3<T> u, V3<T> v) {
+    const V3<T> up = sub(u, scale(dot(u, a), a)), vp = sub(v, scale(dot(v, a), a));
+    return std::atan2(dot(a, cross(up, vp)), dot(up, vp));
+}
+
+template <typename T>
+struct ZKinematics {
+    T mZ, cosZ, sinZ, cosT, sinT, phiT, alpha;   // m_psipi, theta_Z, theta~_psi, phi~, alpha
+    V4<T> K_B, pi_B, psi_B;                       // B-frame 4-momenta (diagnostics, pin P5)
+    V3<T> nK, npi, nKst, nmu;                     // unit vectors in the psi rest frame (pin P7)
+};
+
+// O6. Z-chain kinematics from (m_Kpi, cos theta_K*, cos theta_psi, phi)
+// (definitions; readings A7-A11).
+template <typename T>
+ZKinematics<T> z_kinematics(const Decay<T>& dk, T m, T cK, T cpsi, T phi) {
+    ZKinematics<T> k;
+    const T pB = breakup_momentum(dk.MB, m, dk.mpsi);
+    const T q = breakup_momentum(m, dk.mK, dk.mpi);
+    // 1. B rest frame, z along the K pi system
+    const T EKpi = (dk.MB * dk.MB + m * m - dk.mpsi * dk.mpsi) / (2 * dk.MB);
+    const V4<T> Kpi_B{EKpi, {0, 0, pB}};
+    k.psi_B = V4<T>{dk.MB - EKpi, {0, 0, -pB}};
+    // 2. K pi rest frame: theta_K* is the angle of the K from the K* flight direction
+    const T sK = std::sqrt((1 - cK) * (1 + cK));
+    const V4<T> K_R{std::sqrt(q * q + dk.mK * dk.mK), {q * sK, 0, q * cK}};
+    const V4<T> pi_R{std::sqrt(q * q + dk.mpi * dk.mpi), {-q * sK, 0, -q * cK}};
+    const V3<T> vKpi{0, 0, pB / EKpi};
+    k.K_B = boost_to_frame(K_R, scale(T(-1), vKpi));
+    k.pi_B = boost_to_frame(pi_R, scale(T(-1), vKpi));
+    // 3. J/psi rest frame
+    const V3<T> vpsi = scale(1 / k.psi_B.E, k.psi_B.p);
+    const V4<T> K_P = boost_to_frame(k.K_B, vpsi), pi_P = boost_to_frame(k.pi_B, vpsi), Kst_P = boost_to_frame(Kpi_B, vpsi);
+    k.nK = unit(K_P.p); k.npi = unit(pi_P.p); k.nKst = unit(Kst_P.p);
+    // 4. mu+ direction: polar angle theta_psi from n_K* (A7), azimuth phi about n_K* from the K side (A8)
+    const V3<T> ez = k.nKst;
+    const V3<T> ex = unit(sub(k.nK, scale(dot(k.nK, ez), ez)));
+    const V3<T> ey = cross(ez, ex);
+    const T spsi = std::sqrt((1 - cpsi) * (1 + cpsi));
+    k.nmu = add(add(scale(spsi * std::cos(phi), ex), scale(spsi * std::sin(phi), ey)), scale(cpsi, ez));
+    // 5. Z = psi pi; theta_Z = angle between K and pi momenta in the Z rest frame (A10)
+    const V4<T> Z_B = add4(k.psi_B, k.pi_B);
+    k.mZ = std::sqrt(Z_B.E * Z_B.E - dot(Z_B.p, Z_B.p));
+    const V3<T> vZ = scale(1 / Z_B.E, Z_B.p);
+    const V3<T> uK = unit(boost_to_frame(k.K_B, vZ).p), upi = unit(boost_to_frame(k.pi_B, vZ).p);
+    k.cosZ = dot(uK, upi);
+    k.sinZ = norm(cross(uK, upi));
+    // 6. theta~_psi = angle between mu+ and pi in the psi rest frame (A11)
+    k.cosT = dot(k.nmu, k.npi);
+    k.sinT = norm(cross(k.nmu, k.npi));
+    // 7. phi~: between the (mu, pi) and (K, pi) planes about n_pi; alpha: between the (mu+, pi) and
+    //    (mu+, K pi) planes about n_mu (A9)
+    k.phiT = dihedral(k.npi, k.nK, k.nmu);
+    k.alpha = dihedral(k.nmu, k.npi, k.nKst);
+    return k;
+}
+
+// ---------------------------------------------------------------------------------
+// Model = decay constants + resonance list; coupling slots in resonance order, lambda = -1,0,+1
+// for J >= 1 K* and for the Z, lambda = 0 only for J = 0 K* and the constant term.
+template <typename T>
+struct Model {
+    Decay<T> dk;
+    std::vector<Resonance<T>> res;
+    int num_couplings() const {
+        int K = 0;
+        for (auto& r : res) K += (r.kind == ZRES || (r.kind == KSTAR && r.J >= 1)) ? 3 : 1;
+        return K;
+    }
+};
+
+// O5 + O7. Basis terms B_{k,xi}(event): everything in Eqs. (4) and (10) except the coupling H.
+// out[k][0] is xi = +1, out[k][1] is xi = -1.
+template <typename T>
+void basis_terms(const Model<T>& M, const T x[4], std::complex<T>* out /* [K][2] */) {
+    using C = std::complex<T>;
+    const T m = x[0], cK = x[1], cpsi = x[2], phi = x[3];
+    const T thK = std::atan2(std::sqrt((1 - cK) * (1 + cK)), cK);
+    const T thpsi = std::atan2(std::sqrt((1 - cpsi) * (1 + cpsi)), cpsi);
+    bool haveZ = false;
+    ZKinematics<T> zk;
+    int k = 0;
+    const int xis[2] = {+1, -1};
+    for (const auto& R : M.res) {
+        if (R.kind == ZRES) {
+            if (!haveZ) { zk = z_kinematics(M.dk, m, cK, cpsi, phi); haveZ = true; }
+            const C A = lineshape(M.dk, R, zk.mZ);
+            const T thZ = std::atan2(zk.sinZ, zk.cosZ), thT = std::atan2(zk.sinT, zk.cosT);
+            for (int lp = -1; lp <= 1; ++lp, ++k)
+                for (int ix = 0; ix < 2; ++ix) {
+                    const int xi = xis[ix];
+                    // Eq. (10): A^Z d^J_{0 lambda'}(theta_Z) e^{i lambda' phi~} d^1_{lambda' xi}(theta~) e^{i xi alpha}
+                    out[2 * k + ix] = A * wigner_d<T>(R.J, 0, lp, thZ) * std::polar(T(1), lp * zk.phiT) *
+                                      wigner_d<T>(1, lp, xi, thT) * std::polar(T(1), xi * zk.alpha);
+                }
+        } else {
+            const C A = lineshape(M.dk, R, m);
+            const int lmax = (R.kind == KSTAR && R.J >= 1) ? 1 : 0;
+            for (int l = -lmax; l <= lmax; ++l, ++k)
+                for (int ix = 0; ix < 2; ++ix) {
+                    const int xi = xis[ix];
+                    // Eq. (4): A^K* d^J_{lambda 0}(theta_K*) e^{i lambda phi} d^1_{lambda xi}(theta_psi)
+                    out[2 * k + ix] = A * wigner_d<T>(R.J, l, 0, thK) * std::polar(T(1), l * phi) *
+                                      wigner_d<T>(1, l, xi, thpsi);
+                }
+        }
+    }
+}
+
+// O8. Signal density, Eq. (12): S = sum_xi | sum_k c_k B_{k xi} |^2
+template <typename T>
+T signal_density(const Model<T>& M, const std::complex<T>* c, const T x[4]) {
+    const int K = M.num_couplings();
+    std::vector<std::complex<T>> B(2 * K);
+    basis_terms(M, x, B.data());
+    T S = 0;
+    for (int ix = 0; ix < 2; ++ix) {
+        std::complex<T> A(0, 0);
+        for (int k = 0; k < K; ++k) A += c[k] * B[2 * k + ix];
+        S += std::norm(A);
+    }
+    return S;
+}
+
+// Neumaier-compensated running sum
+template <typename T>
+struct Neumaier {
+    T s = 0, c = 0;
+    void add(T v) { const T t = s + v; c += (std::fabs(s) >= std::fabs(v)) ? (s - t) + v : (v - t) + s; s = t; }
+    T value() const { return s + c; }
+};
+
+template <typename T>
+Model<T> make_model(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass,
+                    const double* width, const double* radius) {
+    Model<T> M;
+    M.dk = Decay<T>{T(decay[0]), T(decay[1]), T(decay[2]), T(decay[3])};
+    for (int r = 0; r < n_res; ++r) M.res.push_back(Resonance<T>{kinds[r], Js[r], T(mass[r]), T(width[r]), T(radius[r])});
+    return M;
+}
+
+template <typename T>
+std::vector<std::complex<T>> make_couplings(const double* c, int K) {
+    std::vector<std::complex<T>> v(K);
+    for (int k = 0; k < K; ++k) v[k] = std::complex<T>(T(c[2 * k]), T(c[2 * k + 1]));
+    return v;
+}
+
+// per-event v_i = eff_i * S_i (Eq. 14 with purity p = 1); x is SoA [4][n]
+template <typename T>
+void eval_events(const Model<T>& M, const std::complex<T>* c, const double* x, const double* eff, long long n, double* out) {
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < n; ++i) {
+        const T xi[4] = {T(x[i]), T(x[n + i]), T(x[2 * n + i]), T(x[3 * n + i])};
+        const T S = signal_density(M, c, xi);
+        out[i] = double((eff ? T(eff[i]) : T(1)) * S);
+    }
+}
+
+// O9 pieces.  Sum over events of w*S and of w (normalisation) or of log(eff*S) (data), each
+// Neumaier-compensated, in event order (per-thread chunks are contiguous and combined in
+// thread order, so the result does not depend on scheduling, only on the thread count).
+template <typename T>
+void weighted_sum(const Model<T>& M, const std::complex<T>* c, const double* x, const double* w, long long n,
+                  bool take_log, T* sum_out, T* wsum_out) {
+    int nt = 1;
+#ifdef _OPENMP
+    nt = omp_get_max_threads();
+#endif
+    std::vector<Neumaier<T>> acc(nt), wacc(nt);
+#pragma omp parallel num_threads(nt)
+    {
+        int t = 0;
+#ifdef _OPENMP
+        t = omp_get_thread_num();
+#endif
+        const long long lo = n * t / nt, hi = n * (t + 1) / nt;
+        for (long long i = lo; i < hi; ++i) {
+            const T xi[4] = {T(x[i]), T(x[n + i]), T(x[2 * n + i]), T(x[3 * n + i])};
+            const T S = signal_density(M, c, xi);
+            const T wi = w ? T(w[i]) : T(1);
+            acc[t].add(take_log ? std::log(wi * S) : wi * S);
+            wacc[t].add(wi);
+        }
+    }
+    Neumaier<T> tot, wtot;
+    for (int t = 0; t < nt; ++t) { tot.add(acc[t].s); tot.add(acc[t].c); wtot.add(wacc[t].s); wtot.add(wacc[t].c); }
+    *sum_out = tot.value();
+    *wsum_out = wtot.value();
+}
+
+template <typename T>
+int nll_impl(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass, const double* width,
+             const double* radius, int P, const double* couplings /*[P][K][2]*/, const double* mass_width /*[P][R][2] or null*/,
+             const double* x, const double* eff, long long n, const double* xn, const double* wn, long long mn,
+             double* nll_out, double* integral_out) {
+    for (int p = 0; p < P; ++p) {
+        Model<T> M = make_model<T>(decay, n_res, kinds, Js, mass, width, radius);
+        if (mass_width)
+            for (int r = 0; r < n_res; ++r) { M.res[r].mass = T(mass_width[(p * n_res + r) * 2]); M.res[r].width = T(mass_width[(p * n_res + r) * 2 + 1]); }
+        const int K = M.num_couplings();
+        auto c = make_couplings<T>(couplings + (size_t)p * K * 2, K);
+        T wS, wsum, slog, dummy;
+        weighted_sum(M, c.data(), xn, wn, mn, false, &wS, &wsum);
+        const T I = wS / wsum;                                   // MC integral (A15)
+        if (integral_out) integral_out[p] = double(I);
+        if (nll_out) {
+            weighted_sum(M, c.data(), x, eff, n, true, &slog, &dummy);
+            nll_out[p] = double(-(slog - T(n) * std::log(I)));   // -sum log(eff S / I)
+        }
+    }
+    return 0;
+}
+
+// Hermitian normalisation matrix M_kl = sum_j w_j sum_xi conj(B_k xi) B_l xi / sum_j w_j (pin P10,
+// fit fractions Eq. 13).  out is [K][K][2] row-major.
+template <typename T>
+void norm_matrix_impl(const Model<T>& M, const double* xn, const double* wn, long long mn, double* out) {
+    const int K = M.num_couplings();
+    std::vector<std::complex<T>> acc((size_t)K * K, std::complex<T>(0, 0));
+    std::vector<std::complex<T>> B(2 * K);
+    T wsum = 0;
+    for (long long j = 0; j < mn; ++j) {
+        const T xj[4] = {T(xn[j]), T(xn[mn + j]), T(xn[2 * mn + j]), T(xn[3 * mn + j])};
+        basis_terms(M, xj, B.data());
+        const T w = wn ? T(wn[j]) : T(1);
+        wsum += w;
+        for (int k = 0; k < K; ++k)
+            for (int l = 0; l < K; ++l)
+                for (int ix = 0; ix < 2; ++ix) acc[(size_t)k * K + l] += w * std::conj(B[2 * k + ix]) * B[2 * l + ix];
+    }
+    for (size_t i = 0; i < acc.size(); ++i) { out[2 * i] = double(acc[i].real() / wsum); out[2 * i + 1] = double(acc[i].imag() / wsum); }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------
+// C ABI for ctypes (tests and the bench's cpu_baseline leg).  `prec` = 0: double, 1: long double.
+#define DISPATCH(prec, CALL_D, CALL_L) do { if (prec) { CALL_L; } else { CALL_D; } } while (0)
+
+extern "C" {
+
+int orc_num_threads() {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+void orc_set_num_threads(int n) {
+#ifdef _OPENMP
+    omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+double orc_breakup_momentum(double M, double a, double b, int prec) {
+    if (prec) return double(breakup_momentum<long double>(M, a, b));
+    return breakup_momentum<double>(M, a, b);
+}
+double orc_barrier_polynomial(int L, double z) { return barrier_polynomial<double>(L, z); }
+double orc_blatt_weisskopf(int L, double p, double p0, double r) { return blatt_weisskopf<double>(L, p, p0, r); }
+double orc_wigner_d(int j, int mp, int m, double beta, int prec) {
+    if (prec) return double(wigner_d<long double>(j, mp, m, beta));
+    return wigner_d<double>(j, mp, m, beta);
+}
+void orc_orbital_L(int kind, int J, int* LB, int* LR) { orbital_L(kind, J, LB, LR); }
+
+// out[0..1] = A^R(m) (re, im), out[2] = Gamma(m)
+void orc_lineshape(const double* decay, int kind, int J, double mass, double width, double radius, double m, int prec, double* out) {
+    if (prec) {
+        Decay<long double> dk{decay[0], decay[1], decay[2], decay[3]};
+        Resonance<long double> R{kind, J, mass, width, radius};
+        long double g; auto A = lineshape<long double>(dk, R, m, &g);
+        out[0] = double(A.real()); out[1] = double(A.imag()); out[2] = double(g);
+    } else {
+        Decay<double> dk{decay[0], decay[1], decay[2], decay[3]};
+        Resonance<double> R{kind, J, mass, width, radius};
+        double g; auto A = lineshape<double>(dk, R, m, &g);
+        out[0] = A.real(); out[1] = A.imag(); out[2] = g;
+    }
+}
+
+// out[0..6] = mZ, cosZ, sinZ, cosT, sinT, phiT, alpha; out[7..18] = K_B, pi_B, psi_B (E,px,py,pz);
+// out[19..30] = nK, npi, nKst, nmu (unit 3-vectors in the psi rest frame)
+}  // extern "C"
+template <typename T>
+static void zkin_fill(const double* decay, const double* x, double* out) {
+    Decay<T> dk{T(decay[0]), T(decay[1]), T(decay[2]), T(decay[3])};
+    auto k = z_kinematics<T>(dk, T(x[0]), T(x[1]), T(x[2]), T(x[3]));
+    const T v[31] = {k.mZ, k.cosZ, k.sinZ, k.cosT, k.sinT, k.phiT, k.alpha,
+                     k.K_B.E, k.K_B.p.x, k.K_B.p.y, k.K_B.p.z, k.pi_B.E, k.pi_B.p.x, k.pi_B.p.y, k.pi_B.p.z,
+                     k.psi_B.E, k.psi_B.p.x, k.psi_B.p.y, k.psi_B.p.z,
+                     k.nK.x, k.nK.y, k.nK.z, k.npi.x, k.npi.y, k.npi.z, k.nKst.x, k.nKst.y, k.nKst.z, k.nmu.x, k.nmu.y, k.nmu.z};
+    for (int i = 0; i < 31; ++i) out[i] = double(v[i]);
+}
+extern "C" {
+void orc_z_kinematics(const double* decay, const double* x /*[4]*/, int prec, double* out /*[31]*/) {
+    DISPATCH(prec, zkin_fill<double>(decay, x, out), zkin_fill<long double>(decay, x, out));
+}
+
+int orc_num_couplings(int n_res, const int* kinds, const int* Js) {
+    int K = 0;
+    for (int r = 0; r < n_res; ++r) K += (kinds[r] == ZRES || (kinds[r] == KSTAR && Js[r] >= 1)) ? 3 : 1;
+    return K;
+}
+
+// basis terms of one event: out [K][2 (xi=+1,-1)][2 (re,im)]
+}  // extern "C"
+template <typename T>
+static void basis_fill(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass, const double* width,
+                       const double* radius, const double* x, double* out) {
+    auto M = make_model<T>(decay, n_res, kinds, Js, mass, width, radius);
+    const int K = M.num_couplings();
+    std::vector<std::complex<T>> B(2 * K);
+    const T xx[4] = {T(x[0]), T(x[1]), T(x[2]), T(x[3])};
+    basis_terms(M, xx, B.data());
+    for (int i = 0; i < 2 * K; ++i) { out[2 * i] = double(B[i].real()); out[2 * i + 1] = double(B[i].imag()); }
+}
+extern "C" {
+void orc_basis_terms(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass, const double* width,
+                     const double* radius, const double* x, int prec, double* out) {
+    DISPATCH(prec, basis_fill<double>(decay, n_res, kinds, Js, mass, width, radius, x, out),
+             basis_fill<long double>(decay, n_res, kinds, Js, mass, width, radius, x, out));
+}
+
+// v_i = eff_i S_i for n events, x SoA [4][n]; eff may be null (= 1)
+void orc_eval_events(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass, const double* width,
+                     const double* radius, const double* couplings, const double* x, const double* eff, long long n, int prec,
+                     double* out) {
+    if (prec) {
+        auto M = make_model<long double>(decay, n_res, kinds, Js, mass, width, radius);
+        auto c = make_couplings<long double>(couplings, M.num_couplings());
+        eval_events(M, c.data(), x, eff, n, out);
+    } else {
+        auto M = make_model<double>(decay, n_res, kinds, Js, mass, width, radius);
+        auto c = make_couplings<double>(couplings, M.num_couplings());
+        eval_events(M, c.data(), x, eff, n, out);
+    }
+}
+
+// NLL(p) = -sum_i log(eff_i S_i(p) / I(p)), I(p) = sum_j w_j S_j(p) / sum_j w_j, for P parameter points.
+// nll_out and/or integral_out may be null.
+int orc_nll(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass, const double* width,
+            const double* radius, int P, const double* couplings, const double* mass_width, const double* x, const double* eff,
+            long long n, const double* xn, const double* wn, long long mn, int prec, double* nll_out, double* integral_out) {
+    if (prec) return nll_impl<long double>(decay, n_res, kinds, Js, mass, width, radius, P, couplings, mass_width, x, eff, n, xn, wn, mn, nll_out, integral_out);
+    return nll_impl<double>(decay, n_res, kinds, Js, mass, width, radius, P, couplings, mass_width, x, eff, n, xn, wn, mn, nll_out, integral_out);
+}
+
+void orc_norm_matrix(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass, const double* width,
+                     const double* radius, const double* xn, const double* wn, long long mn, double* out) {
+    auto M = make_model<double>(decay, n_res, kinds, Js, mass, width, radius);
+    norm_matrix_impl(M, xn, wn, mn, out);
+}
+
+}  // extern "C"

@@ -1,0 +1,420 @@
+"""Pins of the CPU oracle (oracle/amp_oracle.cpp) against what the paper and the mathematics fix.
+
+None of these re-types an oracle formula: each compares against a library routine (sympy Wigner d,
+scipy spherical Bessel / quadrature / Legendre), a closed form, an invariant, or an identity that a
+dropped term, wrong sign, wrong index or transposed operand breaks.  Pin numbers P1..P12 are those of
+DESIGN.md §"Oracle pins".
+"""
+import math
+
+import numpy as np
+import pytest
+from numpy.polynomial import legendre as npleg
+from scipy import integrate, special
+
+from oracle import oracle as O
+from paper_2007_14931_b200 import workloads as W
+
+DEC = W.DECAY
+MB, MPSI, MK, MPI = DEC
+R16 = W.RADIUS
+
+
+def model(cfg):
+    return O.Model(DEC, W.resonances(cfg))
+
+
+# ------------------------------------------------------------------ P1: Wigner d closed forms / library
+def test_P1_wigner_d_matches_sympy_and_tables():
+    from sympy import N
+    from sympy.physics.quantum.spin import Rotation
+    for beta in (0.3, 1.1, 2.9):
+        for j in (1, 2, 3, 4):
+            for mp in range(-j, j + 1):
+                for m in (-1, 0, 1):
+                    ref = complex(N(Rotation.d(j, mp, m, beta).doit(), 30)).real
+                    assert abs(O.wigner_d(j, mp, m, beta) - ref) < 2e-15, (j, mp, m, beta)
+    # PDG table, j = 1 (valid for any beta, also negative)
+    for b in np.linspace(-3.0, 3.0, 13):
+        c, s = math.cos(b), math.sin(b)
+        assert abs(O.wigner_d(1, 1, 1, b) - (1 + c) / 2) < 1e-15
+        assert abs(O.wigner_d(1, -1, -1, b) - (1 + c) / 2) < 1e-15
+        assert abs(O.wigner_d(1, 1, -1, b) - (1 - c) / 2) < 1e-15
+        assert abs(O.wigner_d(1, -1, 1, b) - (1 - c) / 2) < 1e-15
+        assert abs(O.wigner_d(1, 1, 0, b) + s / math.sqrt(2)) < 1e-15
+        assert abs(O.wigner_d(1, 0, 1, b) - s / math.sqrt(2)) < 1e-15
+        assert abs(O.wigner_d(1, 0, -1, b) + s / math.sqrt(2)) < 1e-15
+        assert abs(O.wigner_d(1, 0, 0, b) - c) < 1e-15
+        assert abs(O.wigner_d(2, 1, 0, b) + math.sqrt(1.5) * s * c) < 1e-15
+        assert abs(O.wigner_d(2, 0, 0, b) - (3 * c * c - 1) / 2) < 1e-15
+    # d^J_00 = P_J(cos), d^J_{10} = -sin P_J'(cos)/sqrt(J(J+1)) (Legendre from numpy)
+    for J in range(0, 5):
+        PJ = npleg.Legendre.basis(J)
+        for b in (0.2, 1.3, 2.7):
+            assert abs(O.wigner_d(J, 0, 0, b) - PJ(math.cos(b))) < 2e-15
+            if J:
+                ref = -math.sin(b) * PJ.deriv()(math.cos(b)) / math.sqrt(J * (J + 1))
+                assert abs(O.wigner_d(J, 1, 0, b) - ref) < 4e-15
+                assert abs(O.wigner_d(J, -1, 0, b) + ref) < 4e-15
+    assert abs(O.wigner_d(3, 1, 0, 0.9, prec=1) - O.wigner_d(3, 1, 0, 0.9)) < 1e-15
+
+
+# ------------------------------------------------------------------ P2: orthogonality
+def test_P2_wigner_d_orthogonality():
+    xs, ws = npleg.leggauss(24)
+    for lam in (0, 1):
+        for J in range(lam, 5):
+            for Jp in range(lam, 5):
+                val = sum(w * O.wigner_d(J, lam, 0, math.acos(x)) * O.wigner_d(Jp, lam, 0, math.acos(x)) for x, w in zip(xs, ws))
+                assert abs(val - (2.0 / (2 * J + 1) if J == Jp else 0.0)) < 1e-13
+    for lam in (-1, 0, 1):
+        val = sum(w * sum(O.wigner_d(1, lam, xi, math.acos(x)) ** 2 for xi in (1, -1)) for x, w in zip(xs, ws))
+        assert abs(val - 4.0 / 3.0) < 1e-13
+
+
+# ------------------------------------------------------------------ P3: lineshape at the pole; optical-theorem identity
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_P3_lineshape_pole_and_phase(cfg):
+    M = model(cfg)
+    for r, (kind, J, mass, width, rad) in enumerate(W.resonances(cfg)):
+        A, gam = M.lineshape(r, mass)
+        assert abs(gam - width) < 1e-12 * width                       # Gamma(M_R) = Gamma0
+        LB, LR = O.orbital_L(kind, J)
+        if kind == O.KSTAR:
+            pB0, pR0 = O.breakup_momentum(MB, mass, MPSI), O.breakup_momentum(mass, MK, MPI)
+        else:
+            pB0, pR0 = O.breakup_momentum(MB, mass, MK), O.breakup_momentum(mass, MPSI, MPI)
+        # F = 1 at the pole, so A = i (pB0/MB)^LB (pR0/M)^LR / (M Gamma0): bare propagator modulus 1/(M Gamma0)
+        bare = A / ((pB0 / MB) ** LB * (pR0 / mass) ** LR)
+        assert abs(bare.real) < 1e-12 * abs(bare)
+        assert abs(bare.imag - 1.0 / (mass * width)) < 1e-12 / (mass * width)
+        # phase rises through pi/2 at the pole; imaginary part positive everywhere (Gamma > 0)
+        lo, hi = (MK + MPI + 1, MB - MPSI - 1) if kind == O.KSTAR else (MPSI + MPI + 1, MB - MK - 1)
+        ms = np.linspace(lo, hi, 400)
+        ph = np.unwrap([np.angle(M.lineshape(r, m)[0]) for m in ms])
+        assert np.all(np.diff(ph) > 0) and np.all((ph > 0) & (ph < np.pi))
+        assert (ph[ms < mass] < np.pi / 2).all() and (ph[ms > mass] > np.pi / 2).all()
+
+
+def test_P3b_running_width_scaling_from_optical_identity():
+    """Im(1/D) = M Gamma(m)/|D|^2 gives Gamma(m) from the complex output alone.  With r -> 0 the barrier
+    factors are 1, so Gamma(m) m / (M Gamma0) must be an exact power (2L+1) of the breakup momentum and the
+    numerator an exact power law — fixes the exponents and the M_R/m factor of Eq. 3 and the momentum powers
+    of Eq. 2 (reading A4)."""
+    for kind, J, mass, width in [(O.KSTAR, 0, 1425.0, 270.0), (O.KSTAR, 1, 895.55, 47.3), (O.KSTAR, 2, 1432.4, 109.0),
+                                 (O.KSTAR, 3, 1776.0, 159.0), (O.KSTAR, 4, 2045.0, 198.0), (O.ZRES, 1, 4196.0, 370.0)]:
+        M = O.Model(DEC, [(kind, J, mass, width, 0.0)])
+        LB, LR = O.orbital_L(kind, J)
+        assert (LB, LR) == ((1, 0) if kind == O.ZRES else (1 if J == 0 else J - 1, J))
+        mom = (lambda m: (O.breakup_momentum(MB, m, MPSI), O.breakup_momentum(m, MK, MPI))) if kind == O.KSTAR else \
+              (lambda m: (O.breakup_momentum(MB, m, MK), O.breakup_momentum(m, MPSI, MPI)))
+        pB0, pR0 = mom(mass)
+        for m in np.linspace(mass - 200, mass + 130, 7):
+            A, gam = M.lineshape(0, m)
+            pB, pR = mom(m)
+            num = (pB / MB) ** LB * (pR / m) ** LR                    # r = 0: |A| |D| = numerator
+            D = num / A                                               # M^2 - m^2 - i M Gamma
+            assert abs(D.real - (mass * mass - m * m)) < 1e-9 * mass * mass
+            g = -D.imag / mass
+            assert abs(g - gam) < 1e-10 * width
+            assert abs(g * m / (mass * width) - (pR / pR0) ** (2 * LR + 1)) < 1e-11 * (pR / pR0) ** (2 * LR + 1)
+
+
+# ------------------------------------------------------------------ P4: Blatt-Weisskopf polynomials = x^(2L+2) |h_L(x)|^2
+def test_P4_barrier_polynomials_are_spherical_hankel_moduli():
+    for L in range(5):
+        for x in (0.05, 0.4, 1.0, 2.5, 7.0):
+            h2 = special.spherical_jn(L, x) ** 2 + special.spherical_yn(L, x) ** 2
+            ref = x ** (2 * L + 2) * h2
+            assert abs(O.barrier_polynomial(L, x * x) - ref) < 1e-11 * ref, (L, x)
+    for L in range(5):
+        assert O.blatt_weisskopf(L, 321.0, 321.0, R16) == 1.0          # F(p0) = 1
+        assert O.blatt_weisskopf(0, 100.0, 300.0, R16) == 1.0          # F^(0) = 1
+        # monotone: F decreases with p for L > 0; limit F -> (p0/p)^L (B_L(z0)/z0^L)^(1/2) ... ratio check at r -> 0
+        if L:
+            assert O.blatt_weisskopf(L, 400.0, 300.0, R16) < 1.0 < O.blatt_weisskopf(L, 200.0, 300.0, R16)
+            assert abs(O.blatt_weisskopf(L, 400.0, 300.0, 1e-9) - 1.0) < 1e-9
+
+
+# ------------------------------------------------------------------ P5: kinematic invariants
+def test_P5_kinematic_invariants():
+    M = model(2)
+    rng = np.random.default_rng(5)
+    x = W.phase_space_events(rng, 300)
+    for i in range(x.shape[1]):
+        k = M.z_kinematics(x[:, i])
+        K, pi, psi = k["K_B"], k["pi_B"], k["psi_B"]
+        tot = K + pi + psi
+        assert abs(tot[0] - MB) < 1e-9 and np.abs(tot[1:]).max() < 1e-9          # 4-momentum conservation
+        m2 = lambda p: p[0] ** 2 - p[1:] @ p[1:]
+        assert abs(m2(K) - MK ** 2) < 1e-6 and abs(m2(pi) - MPI ** 2) < 1e-6 and abs(m2(psi) - MPSI ** 2) < 1e-5
+        assert abs(math.sqrt(m2(K + pi)) - x[0, i]) < 1e-9
+        s_kpi, s_psipi, s_psik = m2(K + pi), m2(psi + pi), m2(psi + K)
+        assert abs(s_kpi + s_psipi + s_psik - (MB ** 2 + MPSI ** 2 + MK ** 2 + MPI ** 2)) < 1e-6   # Dalitz identity
+        assert abs(k["mZ"] - math.sqrt(s_psipi)) < 1e-9
+        assert MPSI + MPI <= k["mZ"] <= MB - MK
+        assert abs(k["cosZ"] ** 2 + k["sinZ"] ** 2 - 1) < 1e-12 and k["sinZ"] >= 0
+        assert abs(k["cosT"] ** 2 + k["sinT"] ** 2 - 1) < 1e-12 and k["sinT"] >= 0
+        # the helicity angle of the K in the K pi frame is recovered from B-frame invariants:
+        # m_psipi^2 is linear in cos theta_K* with slope -2 q pB MB / m  (two-body kinematics)
+        pB, q = O.breakup_momentum(MB, x[0, i], MPSI), O.breakup_momentum(x[0, i], MK, MPI)
+        k0 = M.z_kinematics([x[0, i], 0.0, x[2, i], x[3, i]])
+        slope = (k["mZ"] ** 2 - k0["mZ"] ** 2) / x[1, i]
+        assert abs(slope + 2 * q * pB * MB / x[0, i]) < 1e-7 * abs(slope)
+    # independent of (cos theta_psi, phi): the Z mass and theta_Z only depend on the hadronic variables
+    a, b = M.z_kinematics([1200.0, 0.3, 0.5, 1.0]), M.z_kinematics([1200.0, 0.3, -0.7, -2.0])
+    assert abs(a["mZ"] - b["mZ"]) < 1e-10 and abs(a["cosZ"] - b["cosZ"]) < 1e-13
+
+
+# ------------------------------------------------------------------ P6: theta_Z from Lorentz invariants
+def test_P6_theta_Z_from_invariants():
+    """cos theta_Z via Lorentz invariants only (energies in the Z frame from two-body kinematics, p_K.p_pi
+    from m_Kpi) must agree with the oracle's explicit boosts; sin theta_Z via the Gram determinant."""
+    M = model(2)
+    x = W.phase_space_events(np.random.default_rng(6), 500)
+    for i in range(x.shape[1]):
+        m, cK = x[0, i], x[1, i]
+        k = M.z_kinematics(x[:, i])
+        mZ = k["mZ"]
+        EK, Epi = (MB ** 2 - mZ ** 2 - MK ** 2) / (2 * mZ), (mZ ** 2 + MPI ** 2 - MPSI ** 2) / (2 * mZ)
+        pK, ppi = math.sqrt(EK ** 2 - MK ** 2), math.sqrt(Epi ** 2 - MPI ** 2)
+        cZ = (EK * Epi - (m * m - MK ** 2 - MPI ** 2) / 2) / (pK * ppi)
+        assert abs(cZ - k["cosZ"]) < 5e-11
+        pB, q = O.breakup_momentum(MB, m, MPSI), O.breakup_momentum(m, MK, MPI)
+        sZ = MB * q * pB * math.sqrt((1 - cK) * (1 + cK)) / (mZ * pK * ppi)
+        assert abs(sZ - k["sinZ"]) < 5e-11
+
+
+# ------------------------------------------------------------------ P7: rotation-composition identity
+def test_P7_rotation_composition_pins_Z_angles():
+    """The J/psi helicity state quantised along n_K* (K* chain, Eq. 4) re-expressed along n_pi (Z chain, Eq. 10):
+    sum_l d^1_{l l'}(beta) e^{i l phi} d^1_{l xi}(theta_psi) = e^{i l' phi~} d^1_{l' xi}(theta~) e^{i xi alpha},
+    beta the rotation angle about y from n_K* to n_pi.  Fixes theta~, phi~, alpha and the sign in e^{+i xi alpha};
+    flipping any of those signs breaks it at O(1)."""
+    M = model(2)
+    x = W.phase_space_events(np.random.default_rng(7), 200)
+    d1 = lambda a, b, ang: O.wigner_d(1, a, b, ang)
+    worst, worst_flip = 0.0, [10.0, 10.0, 10.0]
+    for i in range(x.shape[1]):
+        m, cK, cpsi, phi = x[:, i]
+        k = M.z_kinematics(x[:, i])
+        # the frame (x, y, z = n_K*) of reading A7/A8: everything hadronic lies in the x-z plane, K on the +x side
+        ez = k["nKst"]
+        ex = k["nK"] - (k["nK"] @ ez) * ez
+        ex /= np.linalg.norm(ex)
+        ey = np.cross(ez, ex)
+        assert abs(k["npi"] @ ey) < 1e-12 and k["nK"] @ ex > 0
+        spsi = math.sqrt(1 - cpsi * cpsi)
+        assert np.allclose(k["nmu"], spsi * math.cos(phi) * ex + spsi * math.sin(phi) * ey + cpsi * ez, atol=1e-13)
+        beta = math.atan2(k["npi"] @ ex, k["npi"] @ ez)
+        th, tht = math.acos(cpsi), math.atan2(k["sinT"], k["cosT"])
+        for lp in (-1, 0, 1):
+            for xi in (-1, 1):
+                lhs = sum(d1(l, lp, beta) * np.exp(1j * l * phi) * d1(l, xi, th) for l in (-1, 0, 1))
+                f = lambda s1, s2: np.exp(1j * lp * s1 * k["phiT"]) * d1(lp, xi, tht) * np.exp(1j * xi * s2 * k["alpha"])
+                worst = max(worst, abs(lhs - f(1, 1)))
+                if lp:
+                    for j, (s1, s2) in enumerate([(-1, 1), (1, -1), (-1, -1)]):
+                        worst_flip[j] = min(worst_flip[j], 10.0) if abs(lhs - f(s1, s2)) > 0.05 else 0.0
+    assert worst < 1e-13
+    # the three other sign choices fail for (almost) every event
+    for j, (s1, s2) in enumerate([(-1, 1), (1, -1), (-1, -1)]):
+        bad = 0
+        for i in range(50):
+            m, cK, cpsi, phi = x[:, i]
+            k = M.z_kinematics(x[:, i])
+            beta = math.atan2(k["npi"][0], k["npi"][2])
+            th, tht = math.acos(cpsi), math.atan2(k["sinT"], k["cosT"])
+            lhs = sum(d1(l, 1, beta) * np.exp(1j * l * phi) * d1(l, 1, th) for l in (-1, 0, 1))
+            rhs = np.exp(1j * s1 * k["phiT"]) * d1(1, 1, tht) * np.exp(1j * s2 * k["alpha"])
+            bad += abs(lhs - rhs) > 1e-3
+        assert bad > 40
+
+
+# ------------------------------------------------------------------ helpers: tensor quadrature grid as weighted "norm events"
+def quadrature_events(nm, ncK, ncpsi, nphi, m_lo=None, m_hi=None):
+    m_lo = MK + MPI if m_lo is None else m_lo
+    m_hi = MB - MPSI if m_hi is None else m_hi
+    xm, wm = npleg.leggauss(nm)
+    mm = 0.5 * (m_hi - m_lo) * xm + 0.5 * (m_hi + m_lo)
+    wm = wm * 0.5 * (m_hi - m_lo)
+    pq = np.array([O.breakup_momentum(MB, m, MPSI) * O.breakup_momentum(m, MK, MPI) for m in mm])
+    xk, wk = npleg.leggauss(ncK)
+    xp, wp = npleg.leggauss(ncpsi)
+    ph = -np.pi + 2 * np.pi * (np.arange(nphi) + 0.5) / nphi
+    G = np.meshgrid(mm, xk, xp, ph, indexing="ij")
+    Wt = np.einsum("i,j,k,l->ijkl", wm * pq, wk, wp, np.full(nphi, 2 * np.pi / nphi))
+    return np.stack([g.ravel() for g in G]), Wt.ravel()
+
+
+# ------------------------------------------------------------------ P8: K*-only angular average; spin-0 normalisation
+def test_P8_kstar_angular_average_closed_form():
+    """<S>_angles = (2/3) sum_lambda sum_J |sum_{R in J} H^R_lambda A^R(m)|^2 / (2J+1) (orthogonality of the d's),
+    checked per mass point on a Gauss-Legendre x uniform grid — pins Eq. 4/5's angular structure, the slot order
+    and which sums are coherent."""
+    res = W.resonances(1)
+    M = model(1)
+    c = W.couplings(1)
+    slots = W.slot_table(res)
+    xk, wk = npleg.leggauss(8)
+    xp, wp = npleg.leggauss(4)
+    nphi = 8
+    ph = -np.pi + 2 * np.pi * (np.arange(nphi) + 0.5) / nphi
+    for m in (700.0, 895.55, 1432.0, 1800.0, 2100.0):
+        G = np.meshgrid([m], xk, xp, ph, indexing="ij")
+        x = np.stack([g.ravel() for g in G])
+        w = np.einsum("j,k,l->jkl", wk, wp, np.full(nphi, 2 * np.pi / nphi)).ravel()
+        avg = np.sum(w * M.eval_events(c, x)) / np.sum(w)
+        amp = {}
+        for k, (r, lam) in enumerate(slots):
+            amp[(res[r][1], lam)] = amp.get((res[r][1], lam), 0) + c[k] * M.lineshape(r, m)[0]
+        ref = (2.0 / 3.0) * sum(abs(a) ** 2 / (2 * J + 1) for (J, lam), a in amp.items())
+        assert abs(avg - ref) < 1e-13 * ref
+
+
+def test_P8b_spin0_normalisation_vs_quadrature():
+    """north_star pin: a single spin-0 resonance's MC normalisation against brute-force quadrature.
+    I = (2/3) |H|^2 int |A(m)|^2 pB q dm / int pB q dm (scipy.integrate.quad on the oracle's pinned 1D pieces)
+    against the oracle's weighted-event normalisation over a 4D tensor grid."""
+    res = [(O.KSTAR, 0, 1425.0, 270.0, R16)]
+    M = O.Model(DEC, res)
+    H = 0.7 - 1.1j
+    x, w = quadrature_events(512, 3, 3, 4)   # sqrt end-point behaviour of pB q: GL error ~ n^-3
+    I4d = M.norm_integral(np.array([H]), x, w)[0]
+    lo, hi = MK + MPI, MB - MPSI
+    pq = lambda m: O.breakup_momentum(MB, m, MPSI) * O.breakup_momentum(m, MK, MPI)
+    num = integrate.quad(lambda m: abs(M.lineshape(0, m)[0]) ** 2 * pq(m), lo, hi, epsabs=0, epsrel=1e-12, limit=400, points=[1425.0])[0]
+    den = integrate.quad(pq, lo, hi, epsabs=0, epsrel=1e-12, limit=400)[0]
+    ref = (2.0 / 3.0) * abs(H) ** 2 * num / den
+    assert abs(I4d - ref) < 5e-8 * ref
+    # and brute force: plain 4D midpoint rule in (m, cK, cpsi, phi), no Gauss weights
+    n = 24
+    mm = lo + (hi - lo) * (np.arange(400) + 0.5) / 400
+    cc = -1 + 2 * (np.arange(n) + 0.5) / n
+    G = np.meshgrid(mm, cc[::6], cc, [0.3], indexing="ij")
+    xb = np.stack([g.ravel() for g in G])
+    wb = np.array([pq(m) for m in xb[0]])
+    Ib = M.norm_integral(np.array([H]), xb, wb)[0]
+    assert abs(Ib - ref) < 2e-3 * ref
+
+
+# ------------------------------------------------------------------ P9: Z-only integral over K*-chain phase space
+def test_P9_z_only_phase_space_integral():
+    """Z-only density integrated over the (m_Kpi, cosK, cospsi, phi) phase space equals (2/9) sum|H|^2 times the
+    1D integral of |A^Z|^2 over m_psipi with the Z-chain phase-space weight — exercises m_psipi, theta~, phi~ and
+    |d(theta_Z)| through the change of variables; and Z-only S does not depend on alpha."""
+    res = [(O.ZRES, 1, 4196.0, 370.0, R16)]
+    M = O.Model(DEC, res)
+    H = np.array([0.8 * np.exp(0.4j), 1.3 * np.exp(-2.0j), 0.6 * np.exp(1.9j)])
+    x, w = quadrature_events(64, 64, 4, 8)
+    I = M.norm_integral(H, x, w)[0]
+    pqZ = lambda mz: O.breakup_momentum(MB, mz, MK) * O.breakup_momentum(mz, MPSI, MPI)
+    lo, hi = MPSI + MPI, MB - MK
+    num = integrate.quad(lambda mz: abs(M.lineshape(0, mz)[0]) ** 2 * pqZ(mz), lo, hi, epsabs=0, epsrel=1e-11, limit=400)[0]
+    den = integrate.quad(pqZ, lo, hi, epsabs=0, epsrel=1e-11, limit=400)[0]
+    ref = (2.0 / 9.0) * np.sum(np.abs(H) ** 2) * num / den
+    assert abs(I - ref) < 1e-5 * ref          # quadrature-limited (sqrt end points), converges with the grid
+    # each helicity separately (catches a d^1_{0 lambda'} / d^1_{lambda' xi} mix-up that the sum hides)
+    for l in range(3):
+        Hl = np.zeros(3, complex)
+        Hl[l] = 1.0
+        Il = M.norm_integral(Hl, x, w)[0]
+        assert abs(Il - (2.0 / 9.0) * num / den) < 1e-5 * Il
+
+
+# ------------------------------------------------------------------ P10: c^H M c = direct sum
+def test_P10_norm_matrix_quadratic_form():
+    M = model(2)
+    c = W.couplings(2)
+    xn, wn = W.norm_events(2, 3000)
+    Mat = M.norm_matrix(xn, wn)
+    assert np.abs(Mat - Mat.conj().T).max() < 1e-16 * np.abs(Mat).max() + 1e-30
+    assert np.linalg.eigvalsh(Mat).min() > -1e-14 * np.abs(Mat).max()
+    direct = M.norm_integral(c, xn, wn)[0]
+    quad = (c.conj() @ Mat @ c).real
+    assert abs(quad - direct) < 1e-13 * direct
+
+
+# ------------------------------------------------------------------ P11: invariances
+def test_P11_invariances():
+    M = model(2)
+    c = W.couplings(2)
+    xn, wn = W.norm_events(2, 2000)
+    x, eff = xn[:, :500].copy(), wn[:500].copy()
+    v = M.eval_events(c, x, eff)
+    assert np.all(v > 0)
+    assert np.allclose(M.eval_events(np.exp(0.77j) * c, x, eff), v, rtol=1e-13, atol=0)       # global phase
+    assert np.allclose(M.eval_events(3.0 * c, x, eff), 9.0 * v, rtol=1e-13, atol=0)
+    nll0 = M.nll(c, x, eff, xn, wn)[0][0]
+    nll1 = M.nll((0.3 - 2.0j) * c, x, eff, xn, wn)[0][0]
+    assert abs(nll0 - nll1) < 1e-12 * abs(nll0)
+    x2 = x.copy()
+    x2[3] += 2 * np.pi
+    assert np.allclose(M.eval_events(c, x2, eff), v, rtol=1e-12, atol=0)                      # periodic in phi
+    # K*-only with all H_{+-1} = 0: no phi dependence at all
+    M1, c1 = model(1), W.couplings(1).copy()
+    for k, (r, lam) in enumerate(W.slot_table(W.resonances(1))):
+        if lam:
+            c1[k] = 0
+    x3 = x.copy()
+    x3[3] = np.random.default_rng(1).uniform(-np.pi, np.pi, x.shape[1])
+    assert np.allclose(M1.eval_events(c1, x3), M1.eval_events(c1, x), rtol=1e-13, atol=0)
+    # Z-only: S independent of alpha is equivalent to: S(xi=+1)+S(xi=-1) unchanged under phi -> shifts that keep
+    # theta~, phi~ fixed — checked through the basis: |B_{k,xi}| carries no alpha
+    B = M.basis_terms(x[:, 0])
+    kZ = [k for k, (r, lam) in enumerate(W.slot_table(W.resonances(2))) if W.resonances(2)[r][0] == O.ZRES]
+    k0 = M.z_kinematics(x[:, 0])
+    for k, lp in zip(kZ, (-1, 0, 1)):
+        for ix, xi in enumerate((1, -1)):
+            expect = B[k, ix] * np.exp(-1j * xi * k0["alpha"]) * np.exp(-1j * lp * k0["phiT"])
+            ratio = expect / M.lineshape(10, k0["mZ"])[0]
+            assert abs(ratio.imag) < 1e-13                                # what is left is real: d * d
+
+
+# ------------------------------------------------------------------ P12: PDF properties, summation, closure
+def test_P12_normalisation_and_exact_summation():
+    M = model(1)
+    c = W.couplings(1)
+    xn, wn = W.norm_events(1, 4000)
+    I = M.norm_integral(c, xn, wn)[0]
+    S = M.eval_events(c, xn)                      # eff = 1 -> S_j
+    assert np.all(S >= 0)
+    assert abs(math.fsum(wn * S / I) / math.fsum(wn) - 1.0) < 1e-13
+    x, eff = xn[:, :1500], wn[:1500]
+    nll = M.nll(c, x, eff, xn, wn)[0][0]
+    v = M.eval_events(c, x, eff)
+    ref = -math.fsum(math.log(vi / I) for vi in v)   # exactly rounded sum of the same terms
+    assert abs(nll - ref) < 1e-13 * abs(ref)
+    # long double twin agrees
+    nllL = M.nll(c, x, eff, xn, wn, prec=1)[0][0]
+    assert abs(nll - nllL) < 1e-12 * abs(nll)
+
+
+def test_P12b_closure_true_parameters_beat_wrong_ones():
+    cfg = 0
+    M = model(cfg)
+    c = W.couplings(cfg)
+    xn, wn = W.norm_events(cfg, 20000)
+    x, eff = W.data_events(cfg, lambda xx, ee: M.eval_events(c, xx, ee), n=4000)
+    nll_true = M.nll(c, x, eff, xn, wn)[0][0]
+    rng = np.random.default_rng(3)
+    for _ in range(4):
+        c2 = c.copy()
+        c2[:3] *= 1 + 0.5 * rng.uniform(-1, 1, 3)
+        c2[:3] *= np.exp(1j * rng.uniform(-1, 1, 3))
+        assert M.nll(c2, x, eff, xn, wn)[0][0] > nll_true
+    # and a wrong mass: K*(892) moved by one width
+    mw = np.array([[[895.55 + 47.3, 47.3], [0, 0]]])
+    assert M.nll(c, x, eff, xn, wn, mass_width=mw)[0][0] > nll_true + 100
+
+
+def test_mass_width_override_equals_new_model():
+    res = W.resonances(2)
+    M = O.Model(DEC, res)
+    c = W.couplings(2)
+    xn, wn = W.norm_events(2, 500)
+    mw = W.step_mass_width(3, 1)
+    res2 = [(r[0], r[1], mw[i, 0], mw[i, 1], r[4]) for i, r in enumerate(res)]
+    a = M.nll(c, xn[:, :100], wn[:100], xn, wn, mass_width=mw[None])[0][0]
+    b = O.Model(DEC, res2).nll(c, xn[:, :100], wn[:100], xn, wn)[0][0]
+    assert a == b
