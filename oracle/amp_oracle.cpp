@@ -239,50 +239,93 @@ struct Model {
     }
 };
 
+// Parameter-independent part of one event: the angles of both decay chains and the Wigner d's and
+// phases Eqs. (4) and (10) need.  Computed once per event and reused for every parameter point
+// (hoisting only: each entry is the same call the equations spell out).
+template <typename T>
+struct EventAngles {
+    T m;                              // m_Kpi
+    T dK[5][3];                       // d^J_{lambda 0}(theta_K*), J = 0..4, lambda = -1,0,+1 (index lambda+1)
+    std::complex<T> ephi[3];          // e^{i lambda phi}
+    T dpsi[3][2];                     // d^1_{lambda xi}(theta_psi), xi = +1 (index 0), -1 (index 1)
+    bool haveZ = false;
+    T mZ;                             // m_psipi
+    T dZ[5][3];                       // d^J_{0 lambda'}(theta_Z)
+    std::complex<T> ephiT[3];         // e^{i lambda' phi~}
+    T dT[3][2];                       // d^1_{lambda' xi}(theta~_psi)
+    std::complex<T> ealpha[2];        // e^{i xi alpha}
+};
+
+template <typename T>
+EventAngles<T> event_angles(const Model<T>& M, const T x[4]) {
+    EventAngles<T> a;
+    const int xis[2] = {+1, -1};
+    const T m = x[0], cK = x[1], cpsi = x[2], phi = x[3];
+    a.m = m;
+    const T thK = std::atan2(std::sqrt((1 - cK) * (1 + cK)), cK);
+    const T thpsi = std::atan2(std::sqrt((1 - cpsi) * (1 + cpsi)), cpsi);
+    for (const auto& R : M.res) {
+        if (R.kind == ZRES) {
+            if (!a.haveZ) {
+                const ZKinematics<T> zk = z_kinematics(M.dk, m, cK, cpsi, phi);
+                const T thT = std::atan2(zk.sinT, zk.cosT);
+                a.haveZ = true;
+                a.mZ = zk.mZ;
+                for (int lp = -1; lp <= 1; ++lp) {
+                    a.ephiT[lp + 1] = std::polar(T(1), lp * zk.phiT);
+                    for (int ix = 0; ix < 2; ++ix) a.dT[lp + 1][ix] = wigner_d<T>(1, lp, xis[ix], thT);
+                }
+                for (int ix = 0; ix < 2; ++ix) a.ealpha[ix] = std::polar(T(1), xis[ix] * zk.alpha);
+                const T thZ = std::atan2(zk.sinZ, zk.cosZ);
+                for (int J = 0; J <= 4; ++J)
+                    for (int lp = -1; lp <= 1; ++lp) a.dZ[J][lp + 1] = (std::abs(lp) <= J) ? wigner_d<T>(J, 0, lp, thZ) : T(0);
+            }
+        }
+    }
+    for (int J = 0; J <= 4; ++J)
+        for (int l = -1; l <= 1; ++l) a.dK[J][l + 1] = (std::abs(l) <= J) ? wigner_d<T>(J, l, 0, thK) : T(0);
+    for (int l = -1; l <= 1; ++l) {
+        a.ephi[l + 1] = std::polar(T(1), l * phi);
+        for (int ix = 0; ix < 2; ++ix) a.dpsi[l + 1][ix] = wigner_d<T>(1, l, xis[ix], thpsi);
+    }
+    return a;
+}
+
 // O5 + O7. Basis terms B_{k,xi}(event): everything in Eqs. (4) and (10) except the coupling H.
 // out[k][0] is xi = +1, out[k][1] is xi = -1.
 template <typename T>
-void basis_terms(const Model<T>& M, const T x[4], std::complex<T>* out /* [K][2] */) {
+void basis_terms(const Model<T>& M, const EventAngles<T>& a, std::complex<T>* out /* [K][2] */) {
     using C = std::complex<T>;
-    const T m = x[0], cK = x[1], cpsi = x[2], phi = x[3];
-    const T thK = std::atan2(std::sqrt((1 - cK) * (1 + cK)), cK);
-    const T thpsi = std::atan2(std::sqrt((1 - cpsi) * (1 + cpsi)), cpsi);
-    bool haveZ = false;
-    ZKinematics<T> zk;
     int k = 0;
-    const int xis[2] = {+1, -1};
     for (const auto& R : M.res) {
         if (R.kind == ZRES) {
-            if (!haveZ) { zk = z_kinematics(M.dk, m, cK, cpsi, phi); haveZ = true; }
-            const C A = lineshape(M.dk, R, zk.mZ);
-            const T thZ = std::atan2(zk.sinZ, zk.cosZ), thT = std::atan2(zk.sinT, zk.cosT);
+            const C A = lineshape(M.dk, R, a.mZ);
             for (int lp = -1; lp <= 1; ++lp, ++k)
-                for (int ix = 0; ix < 2; ++ix) {
-                    const int xi = xis[ix];
+                for (int ix = 0; ix < 2; ++ix)
                     // Eq. (10): A^Z d^J_{0 lambda'}(theta_Z) e^{i lambda' phi~} d^1_{lambda' xi}(theta~) e^{i xi alpha}
-                    out[2 * k + ix] = A * wigner_d<T>(R.J, 0, lp, thZ) * std::polar(T(1), lp * zk.phiT) *
-                                      wigner_d<T>(1, lp, xi, thT) * std::polar(T(1), xi * zk.alpha);
-                }
+                    out[2 * k + ix] = A * a.dZ[R.J][lp + 1] * a.ephiT[lp + 1] * a.dT[lp + 1][ix] * a.ealpha[ix];
         } else {
-            const C A = lineshape(M.dk, R, m);
+            const C A = lineshape(M.dk, R, a.m);
             const int lmax = (R.kind == KSTAR && R.J >= 1) ? 1 : 0;
             for (int l = -lmax; l <= lmax; ++l, ++k)
-                for (int ix = 0; ix < 2; ++ix) {
-                    const int xi = xis[ix];
+                for (int ix = 0; ix < 2; ++ix)
                     // Eq. (4): A^K* d^J_{lambda 0}(theta_K*) e^{i lambda phi} d^1_{lambda xi}(theta_psi)
-                    out[2 * k + ix] = A * wigner_d<T>(R.J, l, 0, thK) * std::polar(T(1), l * phi) *
-                                      wigner_d<T>(1, l, xi, thpsi);
-                }
+                    out[2 * k + ix] = A * a.dK[R.J][l + 1] * a.ephi[l + 1] * a.dpsi[l + 1][ix];
         }
     }
 }
 
+template <typename T>
+void basis_terms(const Model<T>& M, const T x[4], std::complex<T>* out) {
+    basis_terms(M, event_angles(M, x), out);
+}
+
 // O8. Signal density, Eq. (12): S = sum_xi | sum_k c_k B_{k xi} |^2
 template <typename T>
-T signal_density(const Model<T>& M, const std::complex<T>* c, const T x[4]) {
+T signal_density(const Model<T>& M, const std::complex<T>* c, const EventAngles<T>& a) {
     const int K = M.num_couplings();
     std::vector<std::complex<T>> B(2 * K);
-    basis_terms(M, x, B.data());
+    basis_terms(M, a, B.data());
     T S = 0;
     for (int ix = 0; ix < 2; ++ix) {
         std::complex<T> A(0, 0);
@@ -290,6 +333,11 @@ T signal_density(const Model<T>& M, const std::complex<T>* c, const T x[4]) {
         S += std::norm(A);
     }
     return S;
+}
+
+template <typename T>
+T signal_density(const Model<T>& M, const std::complex<T>* c, const T x[4]) {
+    return signal_density(M, c, event_angles(M, x));
 }
 
 // Neumaier-compensated running sum
@@ -327,17 +375,20 @@ void eval_events(const Model<T>& M, const std::complex<T>* c, const double* x, c
     }
 }
 
-// O9 pieces.  Sum over events of w*S and of w (normalisation) or of log(eff*S) (data), each
-// Neumaier-compensated, in event order (per-thread chunks are contiguous and combined in
-// thread order, so the result does not depend on scheduling, only on the thread count).
+// O9 pieces.  For every parameter point p: sum over events of w*S_p and of w (normalisation) or of
+// log(eff*S_p) (data), each Neumaier-compensated, in event order (per-thread chunks are contiguous and
+// combined in thread order: the result depends on the thread count only, not on scheduling).  The
+// parameter loop sits inside the event loop so the angles of an event are computed once.
 template <typename T>
-void weighted_sum(const Model<T>& M, const std::complex<T>* c, const double* x, const double* w, long long n,
-                  bool take_log, T* sum_out, T* wsum_out) {
+void weighted_sums(const std::vector<Model<T>>& Ms, const std::vector<std::vector<std::complex<T>>>& cs, const double* x,
+                   const double* w, long long n, bool take_log, std::vector<T>& sum_out, T* wsum_out) {
+    const int P = (int)Ms.size();
     int nt = 1;
 #ifdef _OPENMP
     nt = omp_get_max_threads();
 #endif
-    std::vector<Neumaier<T>> acc(nt), wacc(nt);
+    std::vector<std::vector<Neumaier<T>>> acc(nt, std::vector<Neumaier<T>>(P));
+    std::vector<Neumaier<T>> wacc(nt);
 #pragma omp parallel num_threads(nt)
     {
         int t = 0;
@@ -347,15 +398,23 @@ void weighted_sum(const Model<T>& M, const std::complex<T>* c, const double* x, 
         const long long lo = n * t / nt, hi = n * (t + 1) / nt;
         for (long long i = lo; i < hi; ++i) {
             const T xi[4] = {T(x[i]), T(x[n + i]), T(x[2 * n + i]), T(x[3 * n + i])};
-            const T S = signal_density(M, c, xi);
+            const EventAngles<T> a = event_angles(Ms[0], xi);
             const T wi = w ? T(w[i]) : T(1);
-            acc[t].add(take_log ? std::log(wi * S) : wi * S);
+            for (int p = 0; p < P; ++p) {
+                const T S = signal_density(Ms[p], cs[p].data(), a);
+                acc[t][p].add(take_log ? std::log(wi * S) : wi * S);
+            }
             wacc[t].add(wi);
         }
     }
-    Neumaier<T> tot, wtot;
-    for (int t = 0; t < nt; ++t) { tot.add(acc[t].s); tot.add(acc[t].c); wtot.add(wacc[t].s); wtot.add(wacc[t].c); }
-    *sum_out = tot.value();
+    sum_out.assign(P, T(0));
+    for (int p = 0; p < P; ++p) {
+        Neumaier<T> tot;
+        for (int t = 0; t < nt; ++t) { tot.add(acc[t][p].s); tot.add(acc[t][p].c); }
+        sum_out[p] = tot.value();
+    }
+    Neumaier<T> wtot;
+    for (int t = 0; t < nt; ++t) { wtot.add(wacc[t].s); wtot.add(wacc[t].c); }
     *wsum_out = wtot.value();
 }
 
@@ -364,20 +423,24 @@ int nll_impl(const double* decay, int n_res, const int* kinds, const int* Js, co
              const double* radius, int P, const double* couplings /*[P][K][2]*/, const double* mass_width /*[P][R][2] or null*/,
              const double* x, const double* eff, long long n, const double* xn, const double* wn, long long mn,
              double* nll_out, double* integral_out) {
+    std::vector<Model<T>> Ms;
+    std::vector<std::vector<std::complex<T>>> cs;
     for (int p = 0; p < P; ++p) {
         Model<T> M = make_model<T>(decay, n_res, kinds, Js, mass, width, radius);
         if (mass_width)
             for (int r = 0; r < n_res; ++r) { M.res[r].mass = T(mass_width[(p * n_res + r) * 2]); M.res[r].width = T(mass_width[(p * n_res + r) * 2 + 1]); }
         const int K = M.num_couplings();
-        auto c = make_couplings<T>(couplings + (size_t)p * K * 2, K);
-        T wS, wsum, slog, dummy;
-        weighted_sum(M, c.data(), xn, wn, mn, false, &wS, &wsum);
-        const T I = wS / wsum;                                   // MC integral (A15)
+        cs.push_back(make_couplings<T>(couplings + (size_t)p * K * 2, K));
+        Ms.push_back(M);
+    }
+    std::vector<T> wS, slog;
+    T wsum, dummy;
+    weighted_sums(Ms, cs, xn, wn, mn, false, wS, &wsum);
+    if (nll_out) weighted_sums(Ms, cs, x, eff, n, true, slog, &dummy);
+    for (int p = 0; p < P; ++p) {
+        const T I = wS[p] / wsum;                                   // MC integral (A15)
         if (integral_out) integral_out[p] = double(I);
-        if (nll_out) {
-            weighted_sum(M, c.data(), x, eff, n, true, &slog, &dummy);
-            nll_out[p] = double(-(slog - T(n) * std::log(I)));   // -sum log(eff S / I)
-        }
+        if (nll_out) nll_out[p] = double(-(slog[p] - T(n) * std::log(I)));   // -sum_i log(eff_i S_i / I)
     }
     return 0;
 }
