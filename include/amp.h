@@ -1,0 +1,153 @@
+/* amp.h — C ABI of libamp4d: the per-event unbinned negative log-likelihood of the 4D
+ * helicity-amplitude model for B0 -> J/psi K+ pi-, J/psi -> mu+ mu- (ten K* resonances and an
+ * exotic Z+ -> J/psi pi+), evaluated by hand-written sm_100a CUDA kernels.
+ *
+ * Paper: Sur et al., "A GPU based multidimensional amplitude analysis to search for tetraquark
+ * candidates", J Big Data 8:16 (2021) — cited below as PAPER.md:<line> (+ equation).
+ *
+ * The calls follow the paper's statement of the problem: the minimiser on the host
+ * proposes a parameter vector at every step, the device evaluates the PDF over all events and
+ * returns one scalar.  Events (4 doubles each, Eq. 1) are loaded once per data
+ * set; the normalisation integral is a sum over "several million phase space points"
+ * (PAPER.md:53), loaded once as well.
+ *
+ * Conventions
+ *  - Units: MeV; Blatt-Weisskopf radius in MeV^-1.
+ *  - `d_` arguments are DEVICE pointers, `h_` arguments are HOST pointers.  Device input buffers
+ *    are borrowed for the duration of the call only: the library builds its own cache from them
+ *    on `stream` and the caller may free them after synchronising that stream.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work of a
+ *    model is issued on the stream given to the call; calls that return host data synchronise it.
+ *  - No exception or abort crosses the ABI.  Every call returns an amp_status; amp_last_error()
+ *    gives the text of the last failure of that model.
+ *  - One amp_model per host thread; calls on one model are not re-entrant.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns AMP_ERR_CUDA.
+ */
+#ifndef AMP4D_AMP_H
+#define AMP4D_AMP_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct amp_model amp_model; /* opaque; owns all device state */
+
+typedef enum {
+    AMP_OK = 0,
+    AMP_ERR_INVALID = 1, /* null pointer, bad size, J out of range, too many resonances / points          */
+    AMP_ERR_STATE = 2,   /* call order: amp_nll before amp_load_events / amp_load_norm / amp_set_params   */
+    AMP_ERR_DOMAIN = 3,  /* event outside phase space, pole mass outside the kinematic range,
+                            non-finite or non-positive PDF value                                          */
+    AMP_ERR_CUDA = 4,    /* CUDA runtime error (text in amp_last_error)                                   */
+    AMP_ERR_NOMEM = 5    /* device or host allocation failed                                              */
+} amp_status;
+
+/* Resonance kinds.  AMP_KSTAR: K* -> K pi, Eq. 4.  AMP_Z: Z -> J/psi pi evaluated in
+ * its own decay frame, Eq. 10; only J^P = 1+ (PAPER.md:171).  AMP_CONST: lineshape == 1,
+ * J = 0, angular factor d^1_{0 xi}(theta_psi) (BASELINE.json configs[0], "constant S-wave term").   */
+typedef enum { AMP_KSTAR = 0, AMP_Z = 1, AMP_CONST = 2 } amp_kind;
+
+/* One resonance: spin J (K*: 0..4, Z: 1, CONST: 0), nominal mass M_R and width
+ * Gamma_0 [MeV], Blatt-Weisskopf radius r [MeV^-1] used for both F_B and F_R of Eq. 2 (PAPER.md:89,
+ * 103).  Orbital momenta: K*: L_R = J, L_B = J-1 (J >= 1) or 1 (J = 0), the lowest allowed
+ * (PAPER.md:107); Z: L_B = 1, L_R = 0.                                                               */
+typedef struct {
+    int kind;
+    int J;
+    double mass, width, radius;
+} amp_resonance;
+
+/* Masses of B0, J/psi, K+, pi- [MeV] (symbols of Eq. 2). */
+typedef struct {
+    double m_parent, m_psi, m_k, m_pi;
+} amp_decay;
+
+enum { AMP_MAX_RESONANCES = 16, AMP_MAX_COUPLINGS = 48, AMP_MAX_POINTS = 256 };
+
+/* Create a model from the decay constants and a resonance list (copied).  Fails with AMP_ERR_INVALID on
+ * bad J / kind / non-positive mass or width / n_res > AMP_MAX_RESONANCES, AMP_ERR_DOMAIN if a pole mass
+ * lies outside the kinematic range of its chain (its pole momenta would not exist), AMP_ERR_CUDA if no
+ * device is usable.  *out is owned by the caller and released with amp_model_destroy.                 */
+amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, int n_res, amp_model** out);
+amp_status amp_model_destroy(amp_model* m);
+
+/* K = number of complex coupling slots.  Slot order: resonance order, then lambda = -1, 0, +1 for a
+ * K* with J >= 1 and for the Z (lambda' for the Z), lambda = 0 only for J = 0 and AMP_CONST
+ * ("For K*s with zero spin, only lambda = 0 is allowed").  Returns -1 on a null model. */
+int amp_num_couplings(const amp_model* m);
+int amp_num_resonances(const amp_model* m);
+
+/* Load the data events and build the parameter-independent per-event cache (breakup momenta,
+ * d-function arguments, phi phases, Z-frame mass and angles: Eqs. 1, 4, 10; "Lorentz
+ * boosts and rotations", :171-179).
+ *   d_x   device, FP64 structure-of-arrays [4][n]: m_Kpi [MeV], cos(theta_K*), cos(theta_J/psi), phi
+ *         [rad] (the variables of Eq. 1 with m_J/psi pi replaced by the equivalent cos(theta_K*)).
+ *   d_eff device [n] relative efficiency eps_i > 0 (Eq. 14), or NULL (= 1).
+ * Replaces a previously loaded data set.  n >= 0 (n == 0: NLL data term is 0).  Synchronises `stream`.
+ * AMP_ERR_DOMAIN if any event is outside phase space (m_Kpi not in (m_K+m_pi, m_B-m_psi), |cos| > 1,
+ * non-finite input, eps <= 0); the data set is then left unloaded.                                    */
+amp_status amp_load_events(amp_model* m, const double* d_x, const double* d_eff, long long n, void* stream);
+
+/* Load the phase-space Monte Carlo sample used for the normalisation integral.
+ *   d_x as above, [4][n_norm]; d_w device [n_norm] weights w_j >= 0 (efficiency x quadrature weight) or
+ *   NULL (= 1).  The integral is I = sum_j w_j S(x_j) / sum_j w_j.  Same errors as amp_load_events.   */
+amp_status amp_load_norm(amp_model* m, const double* d_x, const double* d_w, long long n_norm, void* stream);
+
+/* Set P >= 1 parameter points (P <= AMP_MAX_POINTS).
+ *   h_couplings  host [P][K][2]: complex helicity couplings H (re, im) in slot order (Eqs. 4, 10).  The
+ *                constraints of Eq. 6 and Eq. 11 are the caller's business:
+ *                the library treats all K slots as free.
+ *   h_mass_width host [P][R][2]: (mass, width) of every resonance at every point, or NULL (= the values
+ *                given at amp_model_create).  Entries of AMP_CONST resonances are ignored.
+ * The library compares each (resonance, mass, width) with the lineshape columns it holds and marks only
+ * the missing ones for recomputation (done lazily by the next evaluation call).  Copies both arrays.    */
+amp_status amp_set_params(amp_model* m, int P, const double* h_couplings, const double* h_mass_width);
+
+/* NLL(p) = - sum_i log( eps_i S_i(p) / I(p) ) for the P points of the last amp_set_params, with
+ * S = sum_xi |sum_k H_k B_k,xi|^2 (Eqs. 5, 12) and I(p) the Monte Carlo integral.
+ *   h_nll host [P].  Synchronous with respect to h_nll.  Deterministic: the same inputs give the same
+ * bits (fixed-order reductions, no floating-point atomics).
+ * AMP_ERR_STATE without data / norm sample / parameters; AMP_ERR_DOMAIN if some eps_i S_i or I(p) is not
+ * finite and positive: h_nll[p] = +inf for those points, the others are valid.                         */
+amp_status amp_nll(amp_model* m, double* h_nll, void* stream);
+
+/* Diagnostics / parity. */
+/* d_out device [n]: eps_i * S_i(p) of the loaded data events for point p of the last amp_set_params.   */
+amp_status amp_eval_events(amp_model* m, int p, double* d_out, void* stream);
+/* h_I host [P]: I(p) = sum_j w_j S_j(p) / sum_j w_j.                                                   */
+amp_status amp_norm_integral(amp_model* m, double* h_I, void* stream);
+/* d_out device [ncols][n] (or [ncols][n_norm] if which == 1): the kinematics cache columns, in the order
+ * returned by amp_cache_column_name(i); *ncols receives the count (pass d_out == NULL to query).       */
+amp_status amp_dump_cache(amp_model* m, int which, double* d_out, int* ncols, void* stream);
+const char* amp_cache_column_name(int i);
+/* d_out device [n or n_norm][2]: A^R(m) of resonance r at (mass, width) (Eqs. 2-3).                    */
+amp_status amp_eval_lineshape(amp_model* m, int which, int r, double mass, double width, double* d_out, void* stream);
+/* h_M host [K][K][2]: Hermitian normalisation matrix M_kl = sum_j w_j sum_xi conj(B_k,xi) B_l,xi / sum_j w_j
+ * at the lineshapes of point p, so that I(p) = c^H M c (fit fractions of Eq. 13, are ratios
+ * of its diagonal blocks).                                                                             */
+amp_status amp_norm_matrix(amp_model* m, int p, double* h_M, void* stream);
+
+/* How the normalisation integral is evaluated: 0 = automatic (default), 1 = always the direct sum over
+ * the norm events, 2 = always through the matrix M (rebuilt when a lineshape it depends on changes).   */
+amp_status amp_set_norm_mode(amp_model* m, int mode);
+/* How missing lineshape columns are produced when P == 1: 0 = automatic (a resonance whose column missed
+ * on two successive calls is floating: evaluate it in registers inside the combine kernel, no HBM round
+ * trip), 1 = always store columns in the pool, 2 = always evaluate missing columns in registers.        */
+amp_status amp_set_lineshape_mode(amp_model* m, int mode);
+/* Counters of the last amp_nll / amp_norm_integral call: kernels launched, lineshape columns
+ * recomputed (data + norm), which normalisation path ran (1 direct, 2 matrix).                         */
+amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_recomputed, int* norm_path);
+
+const char* amp_last_error(const amp_model* m);
+const char* amp_status_string(amp_status s);
+const char* amp_version(void);
+
+/* FP64 throughput probes used for the roofline denominators: run `iters`
+ * dependent-chain rounds of register-resident DFMA (kind 0) or mma.sync m8n8k4 f64 (kind 1) on every SM
+ * and return achieved FLOP/s in *flops (timed with CUDA events on `stream`).                          */
+amp_status amp_probe_fp64(int kind, int iters, double* flops, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AMP4D_AMP_H */

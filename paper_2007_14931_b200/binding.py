@@ -1,0 +1,234 @@
+"""Thin ctypes binding of libamp4d.so (include/amp.h): argument marshalling only.
+
+Same names as the C ABI.  torch is used for device memory and streams; every step of the path runs in
+the library's CUDA kernels.  There is no fallback: a missing library or a failing call raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libamp4d.so")
+
+AMP_OK, AMP_ERR_INVALID, AMP_ERR_STATE, AMP_ERR_DOMAIN, AMP_ERR_CUDA, AMP_ERR_NOMEM = range(6)
+AMP_KSTAR, AMP_Z, AMP_CONST = 0, 1, 2
+AMP_MAX_RESONANCES, AMP_MAX_COUPLINGS, AMP_MAX_POINTS = 16, 48, 256
+
+# every symbol include/amp.h declares (tests/test_abi.py checks the header against this list and the .so)
+SYMBOLS = [
+    "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
+    "amp_load_norm", "amp_set_params", "amp_nll", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
+    "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_set_norm_mode", "amp_set_lineshape_mode",
+    "amp_last_call_stats", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
+]
+
+
+class amp_resonance(C.Structure):
+    _fields_ = [("kind", C.c_int), ("J", C.c_int), ("mass", C.c_double), ("width", C.c_double), ("radius", C.c_double)]
+
+
+class amp_decay(C.Structure):
+    _fields_ = [("m_parent", C.c_double), ("m_psi", C.c_double), ("m_k", C.c_double), ("m_pi", C.c_double)]
+
+
+class AmpError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__(f"{text}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """Load libamp4d.so (built by paper_2007_14931_b200.build); raises if it is missing — no fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2007_14931_b200.build` (needs nvcc); "
+                          "there is no CPU fallback")
+    L = C.CDLL(LIB_PATH)
+    vp, i, ll, d = C.c_void_p, C.c_int, C.c_longlong, C.c_double
+    pd, pi = C.POINTER(C.c_double), C.POINTER(C.c_int)
+    sig = {
+        "amp_model_create": (i, [C.POINTER(amp_decay), C.POINTER(amp_resonance), i, C.POINTER(vp)]),
+        "amp_model_destroy": (i, [vp]),
+        "amp_num_couplings": (i, [vp]),
+        "amp_num_resonances": (i, [vp]),
+        "amp_load_events": (i, [vp, vp, vp, ll, vp]),
+        "amp_load_norm": (i, [vp, vp, vp, ll, vp]),
+        "amp_set_params": (i, [vp, i, vp, vp]),
+        "amp_nll": (i, [vp, vp, vp]),
+        "amp_eval_events": (i, [vp, i, vp, vp]),
+        "amp_norm_integral": (i, [vp, vp, vp]),
+        "amp_dump_cache": (i, [vp, i, vp, pi, vp]),
+        "amp_cache_column_name": (C.c_char_p, [i]),
+        "amp_eval_lineshape": (i, [vp, i, i, d, d, vp, vp]),
+        "amp_norm_matrix": (i, [vp, i, vp, vp]),
+        "amp_set_norm_mode": (i, [vp, i]),
+        "amp_set_lineshape_mode": (i, [vp, i]),
+        "amp_last_call_stats": (i, [vp, pi, pi, pi]),
+        "amp_last_error": (C.c_char_p, [vp]),
+        "amp_status_string": (C.c_char_p, [i]),
+        "amp_version": (C.c_char_p, []),
+        "amp_probe_fp64": (i, [i, i, pd, vp]),
+    }
+    for name, (res, args) in sig.items():
+        f = getattr(L, name)
+        f.restype, f.argtypes = res, args
+    _lib = L
+    return L
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(getattr(stream, "cuda_stream", stream))
+
+
+def _dev_ptr(t, n_expected=None):
+    """device pointer of a contiguous float64 CUDA tensor (or None)"""
+    if t is None:
+        return None
+    import torch
+    assert isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous(), \
+        "expected a contiguous float64 CUDA tensor"
+    if n_expected is not None:
+        assert t.numel() == n_expected, f"expected {n_expected} elements, got {t.numel()}"
+    return C.c_void_p(t.data_ptr())
+
+
+class Model:
+    """amp_model handle.  Methods mirror the C calls one to one."""
+
+    def __init__(self, decay, resonances):
+        """decay = (m_parent, m_psi, m_k, m_pi); resonances = [(kind, J, mass, width, radius), ...]"""
+        L = lib()
+        self._h = C.c_void_p()
+        dec = amp_decay(*[float(v) for v in decay])
+        arr = (amp_resonance * len(resonances))(*[amp_resonance(int(k), int(J), float(m), float(w), float(r)) for k, J, m, w, r in resonances])
+        st = L.amp_model_create(C.byref(dec), arr, len(resonances), C.byref(self._h))
+        if st != AMP_OK:
+            self._h = C.c_void_p()
+            raise AmpError(st, f"amp_model_create: {L.amp_status_string(st).decode()}")
+        self.K = L.amp_num_couplings(self._h)
+        self.R = L.amp_num_resonances(self._h)
+        self.P = 0
+        self.n = self.n_norm = 0
+
+    def _check(self, st, what):
+        if st != AMP_OK:
+            L = lib()
+            raise AmpError(st, f"{what}: {L.amp_status_string(st).decode()}: {L.amp_last_error(self._h).decode()}")
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib().amp_model_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # --- loading ---------------------------------------------------------------------------------
+    def load_events(self, d_x, d_eff=None, stream=None):
+        n = d_x.shape[1] if d_x.dim() == 2 else d_x.numel() // 4
+        self._check(lib().amp_load_events(self._h, _dev_ptr(d_x, 4 * n), _dev_ptr(d_eff, n if d_eff is not None else None), n,
+                                          _stream_ptr(stream)), "amp_load_events")
+        self.n = n
+
+    def load_norm(self, d_x, d_w=None, stream=None):
+        n = d_x.shape[1] if d_x.dim() == 2 else d_x.numel() // 4
+        self._check(lib().amp_load_norm(self._h, _dev_ptr(d_x, 4 * n), _dev_ptr(d_w, n if d_w is not None else None), n,
+                                        _stream_ptr(stream)), "amp_load_norm")
+        self.n_norm = n
+
+    # --- parameters ------------------------------------------------------------------------------
+    def set_params(self, couplings, mass_width=None):
+        """couplings: complex [K] or [P][K] (host); mass_width: [P][R][2] (host) or None"""
+        c = np.asarray(couplings)
+        if c.ndim == 1:
+            c = c[None]
+        P = c.shape[0]
+        assert c.shape == (P, self.K), f"couplings must be [P][{self.K}]"
+        hc = np.ascontiguousarray(np.stack([c.real, c.imag], -1), dtype=np.float64)
+        pmw = None
+        if mass_width is not None:
+            hmw = np.ascontiguousarray(mass_width, dtype=np.float64)
+            if hmw.ndim == 2:
+                hmw = hmw[None]
+            assert hmw.shape == (P, self.R, 2), f"mass_width must be [P][{self.R}][2]"
+            pmw = hmw.ctypes.data_as(C.c_void_p)
+        self._check(lib().amp_set_params(self._h, P, hc.ctypes.data_as(C.c_void_p), pmw), "amp_set_params")
+        self.P = P
+
+    # --- evaluation ------------------------------------------------------------------------------
+    def nll(self, stream=None, allow_domain_error=False):
+        out = np.empty(max(self.P, 1), dtype=np.float64)
+        st = lib().amp_nll(self._h, out.ctypes.data_as(C.c_void_p), _stream_ptr(stream))
+        if not (allow_domain_error and st == AMP_ERR_DOMAIN):
+            self._check(st, "amp_nll")
+        return out[:self.P]
+
+    def norm_integral(self, stream=None):
+        out = np.empty(max(self.P, 1), dtype=np.float64)
+        self._check(lib().amp_norm_integral(self._h, out.ctypes.data_as(C.c_void_p), _stream_ptr(stream)), "amp_norm_integral")
+        return out[:self.P]
+
+    def eval_events(self, p=0, out=None, stream=None):
+        import torch
+        if out is None:
+            out = torch.empty(self.n, dtype=torch.float64, device="cuda")
+        self._check(lib().amp_eval_events(self._h, int(p), _dev_ptr(out, self.n) if self.n else None, _stream_ptr(stream)), "amp_eval_events")
+        return out
+
+    def dump_cache(self, which=0, stream=None):
+        import torch
+        nc = C.c_int(0)
+        self._check(lib().amp_dump_cache(self._h, which, None, C.byref(nc), _stream_ptr(stream)), "amp_dump_cache")
+        n = self.n_norm if which else self.n
+        out = torch.empty((nc.value, n), dtype=torch.float64, device="cuda")
+        self._check(lib().amp_dump_cache(self._h, which, _dev_ptr(out), C.byref(nc), _stream_ptr(stream)), "amp_dump_cache")
+        names = [lib().amp_cache_column_name(i).decode() for i in range(nc.value)]
+        return names, out
+
+    def eval_lineshape(self, r, mass, width, which=0, stream=None):
+        import torch
+        n = self.n_norm if which else self.n
+        out = torch.empty((n, 2), dtype=torch.float64, device="cuda")
+        self._check(lib().amp_eval_lineshape(self._h, which, int(r), float(mass), float(width), _dev_ptr(out), _stream_ptr(stream)),
+                    "amp_eval_lineshape")
+        return out
+
+    def norm_matrix(self, p=0, stream=None):
+        out = np.empty((self.K, self.K, 2), dtype=np.float64)
+        self._check(lib().amp_norm_matrix(self._h, int(p), out.ctypes.data_as(C.c_void_p), _stream_ptr(stream)), "amp_norm_matrix")
+        return out[..., 0] + 1j * out[..., 1]
+
+    def set_norm_mode(self, mode):
+        self._check(lib().amp_set_norm_mode(self._h, int(mode)), "amp_set_norm_mode")
+
+    def set_lineshape_mode(self, mode):
+        self._check(lib().amp_set_lineshape_mode(self._h, int(mode)), "amp_set_lineshape_mode")
+
+    def last_call_stats(self):
+        a, b, c = C.c_int(), C.c_int(), C.c_int()
+        self._check(lib().amp_last_call_stats(self._h, C.byref(a), C.byref(b), C.byref(c)), "amp_last_call_stats")
+        return {"launches": a.value, "columns_recomputed": b.value, "norm_path": c.value}
+
+
+def probe_fp64(kind, iters=2000, stream=None):
+    out = C.c_double(0)
+    st = lib().amp_probe_fp64(int(kind), int(iters), C.byref(out), _stream_ptr(stream))
+    if st != AMP_OK:
+        raise AmpError(st, "amp_probe_fp64 failed")
+    return out.value
+
+
+def version():
+    return lib().amp_version().decode()

@@ -1,0 +1,161 @@
+// amp_internal.cuh — shared declarations of the CUDA path (product code; shares nothing with oracle/).
+//
+// Data layout in HBM:
+//   kinematics cache  double[NCOL][npad]   structure-of-arrays, one column per cached quantity,
+//                                          npad = n rounded up to a multiple of 32 events
+//   lineshape columns double2[ncol][npad]  complex A^R(m_i) (re, im) interleaved: one 128-bit load
+//                                          per (event, column)
+// One thread owns one event at a time; a warp reads 32 consecutive doubles (256 B) of a cache
+// column or 32 consecutive double2 (512 B) of a lineshape column.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/amp.h"
+
+namespace amp {
+
+// ---- kinematics cache columns (a1) -------------------------------------------------------------
+enum CacheCol {
+    // K* chain: running mass and momenta (Eqs. 2-3), helicity-angle cosines/sines and phi phase (Eq. 4)
+    C_M2 = 0,   // m_Kpi^2
+    C_INVM,     // 1 / m_Kpi
+    C_Q,        // K momentum in the K pi frame (p_R of a K*)
+    C_PB,       // K pi momentum in the B frame (p_B of a K*)
+    C_CK, C_SK,         // cos, sin theta_K*
+    C_CPSI, C_SPSI,     // cos, sin theta_J/psi
+    C_CPHI, C_SPHI,     // cos, sin phi
+    NCOL_K = 10,
+    // Z chain (Eq. 10): running mass m_psipi and momenta, theta_Z, theta~_psi, phi~, alpha
+    C_MZ2 = 10, // m_psipi^2
+    C_INVMZ,    // 1 / m_psipi
+    C_QZ,       // pi momentum in the Z frame (p_R of the Z)
+    C_PBZ,      // Z momentum in the B frame (p_B of the Z)
+    C_CZ, C_SZ,         // cos, sin theta_Z
+    C_CT, C_ST,         // cos, sin theta~_psi
+    C_CPT, C_SPT,       // cos, sin phi~
+    C_CA, C_SA,         // cos, sin alpha
+    NCOL_ALL = 22
+};
+
+struct DecayConst {
+    double MB, mpsi, mK, mpi;
+};
+
+// Per-(resonance, mass, width) constants of Eqs. 2-3, prepared on the host once per lineshape column
+// (O(1) work; every per-event step runs on the device).  With z = (r p)^2, B_L the Blatt-Weisskopf
+// polynomial and rs = 1/sqrt(B_LR(zR) B_LB(zB)):
+//   F_B F_R          = kF rs                      kF  = sqrt(B_LR(zR0) B_LB(zB0))
+//   numerator        = kN rs pB^LB (pR/m)^LR      kN  = kF / MB^LB
+//   M_R Gamma(m)     = kG pR^(2LR+1) (1/m) rs^2 B_LB(zB),   kG = M_R^2 Gamma0 B_LR(zR0) / pR0^(2LR+1)
+struct LineConst {
+    int kind, LR, LB, chain;  // chain: 0 = K pi (K*), 1 = psi pi (Z), 2 = constant
+    double M2, r2, kN, kG;
+};
+
+struct Dataset {
+    long long n = 0, npad = 0;
+    double* cache = nullptr;   // [NCOL][npad]
+    double* weight = nullptr;  // [npad] eps_i (data) or w_j (norm); 1 if the caller gave none
+    double2* cols = nullptr;   // lineshape column pool [capacity][npad]
+    int ncache = 0;            // columns present (NCOL_K or NCOL_ALL)
+    double wsum = 0;           // sum_j w_j (norm) ; sum_i log eps_i (data)
+    bool loaded = false;
+};
+
+static inline long long pad32(long long n) { return (n + 31) / 32 * 32; }
+
+// ---- device helpers ------------------------------------------------------------------------------
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 c) {   // a*b + c
+    return make_double2(fma(a.x, b.x, fma(-a.y, b.y, c.x)), fma(a.x, b.y, fma(a.y, b.x, c.y)));
+}
+__device__ __forceinline__ double2 cscale(double s, double2 a) { return make_double2(s * a.x, s * a.y); }
+__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+
+// Blatt-Weisskopf polynomial B_L(z), z = (r p)^2 (ref. [35]); L is warp-uniform.
+__device__ __forceinline__ double bw_poly(int L, double z) {
+    switch (L) {
+        case 0: return 1.0;
+        case 1: return 1.0 + z;
+        case 2: return fma(z + 3.0, z, 9.0);
+        case 3: return fma(fma(z + 6.0, z, 45.0), z, 225.0);
+        default: return fma(fma(fma(z + 10.0, z, 135.0), z, 1575.0), z, 11025.0);
+    }
+}
+__device__ __forceinline__ double powi(double x, int n) {   // n in 0..9, warp-uniform
+    double r = 1.0;
+#pragma unroll 1
+    for (int i = 0; i < n; ++i) r *= x;
+    return r;
+}
+
+// Lineshape A^R(m) of Eqs. 2-3 from the cached running-mass quantities of its chain.
+__device__ __forceinline__ double2 lineshape_eval(const LineConst& c, double m2, double invm, double pR, double pB) {
+    if (c.chain == 2) return make_double2(1.0, 0.0);
+    const double zR = c.r2 * pR * pR, zB = c.r2 * pB * pB;
+    const double DB = bw_poly(c.LB, zB);
+    const double rs = rsqrt(bw_poly(c.LR, zR) * DB);
+    const double x = pR * invm;
+    const double num = c.kN * rs * powi(pB, c.LB) * powi(x, c.LR);
+    const double MG = c.kG * powi(pR, 2 * c.LR + 1) * invm * (rs * rs) * DB;   // M_R Gamma(m), Eq. 3
+    const double dre = c.M2 - m2;
+    const double s = num / fma(dre, dre, MG * MG);
+    return make_double2(s * dre, s * MG);   // num / (M^2 - m^2 - i M Gamma), Eq. 2
+}
+
+// ---- launchers (one translation unit per kernel family) -------------------------------------------
+struct KinArgs {
+    DecayConst dk;
+    const double* x;      // [4][n] input events (borrowed)
+    const double* w;      // [n] or null
+    double* cache;        // [ncache][npad]
+    double* weight;       // [npad]
+    long long n, npad;
+    int with_z;           // also fill the Z-chain columns
+    int weight_positive;  // 1: weights must be > 0 (eps), 0: >= 0 (norm weights)
+    int* flag;            // device int: set to 1 on a domain error
+    double* partial;      // [grid] per-block partial of sum(log w) (data) or sum(w) (norm)
+};
+cudaError_t launch_kinematics(const KinArgs& a, int grid, cudaStream_t s);
+int kinematics_grid(long long n);
+
+struct LineshapeJob {
+    LineConst lc;
+    int column;   // index into the column pool
+};
+enum { MAX_LINE_JOBS = 64 };
+cudaError_t launch_lineshape(const Dataset& d, const LineshapeJob* jobs, int njobs, cudaStream_t s);
+
+// Streaming combine + reduce for one parameter point (a3 + a5, P = 1)
+enum StreamMode { MODE_DATA = 0, MODE_NORM = 1, MODE_EVAL = 2 };
+struct SlotRef {
+    int column;      // lineshape column in the pool, or -1: evaluate inline from `lc` (not stored)
+    int lc;          // index into StreamArgs::lc for inline evaluation
+    int c0;          // first coupling slot of this resonance
+};
+struct StreamArgs {
+    // resonances grouped by spin: order[jstart[J] .. jstart[J+1]) are the K*/CONST of spin J; zstart.. are Zs
+    SlotRef ref[AMP_MAX_RESONANCES];
+    int jstart[6];
+    int zend;                       // order[jstart[5] .. zend) are the Z resonances
+    LineConst lc[AMP_MAX_RESONANCES];
+    double2 c[AMP_MAX_COUPLINGS];   // couplings of this point
+    const double* cache;
+    const double* weight;
+    const double2* cols;
+    long long n, npad;
+    double* partial;                // [grid] (MODE_DATA: sum log S; MODE_NORM: sum w S)
+    double* out;                    // MODE_EVAL: [n] eps_i S_i
+    int* flag;
+    int mode;
+};
+cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s);
+int stream_grid(long long n);
+
+// fixed-order final reduction of per-block partials: out[j] = sum_b partial[j][b], j < nrows
+cudaError_t launch_finalize(const double* partial, int nblocks, int stride, int nrows, double* out, cudaStream_t s);
+
+cudaError_t probe_fp64(int kind, int iters, double* flops, cudaStream_t s);
+
+}  // namespace amp

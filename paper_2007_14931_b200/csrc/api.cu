@@ -1,0 +1,605 @@
+// api.cu — the C ABI of include/amp.h: argument checking, device-state ownership, the lineshape column
+// pool (which columns are already held, which must be recomputed), the choice of normalisation path and
+// the launch sequence of one NLL evaluation.  All per-event arithmetic is in the kernels.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "amp_internal.cuh"
+
+using namespace amp;
+
+namespace {
+
+struct PoolEntry {
+    int r = -1;
+    double mass = 0, width = 0;
+    bool valid_data = false, valid_norm = false;
+    long long last_used = -1;
+};
+
+}  // namespace
+
+struct amp_model {
+    DecayConst dk{};
+    std::vector<amp_resonance> res;
+    int R = 0, K = 0;
+    int slot0[AMP_MAX_RESONANCES]{};
+    bool has_z = false;
+
+    Dataset data, norm;
+    std::vector<PoolEntry> pool;   // same slot numbering in data.cols and norm.cols
+    int pool_cap = 0;
+
+    // parameter points of the last amp_set_params
+    int P = 0;
+    std::vector<double> couplings;   // [P][K][2]
+    std::vector<double> mw;          // [P][R][2]
+    std::vector<int> colidx;         // [P][R] pool slot, -1 for CONST, -2 for inline evaluation
+    int miss_streak[AMP_MAX_RESONANCES]{};
+    long long call_id = 0;
+
+    int norm_mode = 0, lineshape_mode = 0;
+
+    // scratch
+    double* d_partial = nullptr;   // [2 * AMP_MAX_POINTS][PARTIAL_STRIDE]
+    double* d_sums = nullptr;      // [2 * AMP_MAX_POINTS]
+    double* d_result = nullptr;    // [2 * AMP_MAX_POINTS]
+    int* d_flag = nullptr;
+    double* h_pinned = nullptr;    // [2 * AMP_MAX_POINTS + 2]
+
+    int stat_launches = 0, stat_columns = 0, stat_norm_path = 0;
+    std::string err;
+};
+
+namespace {
+
+enum { PARTIAL_STRIDE = 2048 };
+
+amp_status fail(amp_model* m, amp_status s, const std::string& msg) {
+    if (m) m->err = msg;
+    return s;
+}
+amp_status cuda_fail(amp_model* m, cudaError_t e, const char* where) {
+    return fail(m, e == cudaErrorMemoryAllocation ? AMP_ERR_NOMEM : AMP_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                                  \
+    do {                                                          \
+        cudaError_t e_ = (call);                                  \
+        if (e_ != cudaSuccess) return cuda_fail(m, e_, #call);    \
+    } while (0)
+
+double h_two_body(double M, double a, double b) {
+    const double s = a + b, d = a - b;
+    const double k = (M - s) * (M + s) * (M - d) * (M + d);
+    return (k >= 0 && M > 0) ? std::sqrt(k) / (2 * M) : std::numeric_limits<double>::quiet_NaN();
+}
+double h_bw_poly(int L, double z) {
+    switch (L) {
+        case 0: return 1.0;
+        case 1: return 1.0 + z;
+        case 2: return (z + 3.0) * z + 9.0;
+        case 3: return ((z + 6.0) * z + 45.0) * z + 225.0;
+        default: return (((z + 10.0) * z + 135.0) * z + 1575.0) * z + 11025.0;
+    }
+}
+
+// Constants of one lineshape column (see LineConst).  Returns false if the pole momenta do not exist.
+bool make_line_const(const amp_model* m, int r, double mass, double width, LineConst* out) {
+    const amp_resonance& R = m->res[r];
+    LineConst c{};
+    c.kind = R.kind;
+    if (R.kind == AMP_CONST) { c.chain = 2; *out = c; return true; }
+    double pR0, pB0;
+    if (R.kind == AMP_KSTAR) {
+        c.chain = 0;
+        c.LR = R.J;
+        c.LB = R.J == 0 ? 1 : R.J - 1;                          // lowest allowed L_B
+        pR0 = h_two_body(mass, m->dk.mK, m->dk.mpi);
+        pB0 = h_two_body(m->dk.MB, mass, m->dk.mpsi);
+    } else {
+        c.chain = 1;
+        c.LR = 0;                                                // 1+ Z -> psi pi in S wave
+        c.LB = 1;                                                // B -> Z K in P wave
+        pR0 = h_two_body(mass, m->dk.mpsi, m->dk.mpi);
+        pB0 = h_two_body(m->dk.MB, mass, m->dk.mK);
+    }
+    if (!(pR0 > 0) || !(pB0 > 0) || !(mass > 0) || !(width > 0)) return false;
+    c.M2 = mass * mass;
+    c.r2 = R.radius * R.radius;
+    const double BR0 = h_bw_poly(c.LR, c.r2 * pR0 * pR0), BB0 = h_bw_poly(c.LB, c.r2 * pB0 * pB0);
+    const double kF = std::sqrt(BR0 * BB0);
+    c.kN = kF / std::pow(m->dk.MB, c.LB);
+    c.kG = mass * mass * width * BR0 / std::pow(pR0, 2 * c.LR + 1);
+    *out = c;
+    return true;
+}
+
+void free_dataset(Dataset& d) {
+    if (d.cache) cudaFree(d.cache);
+    if (d.weight) cudaFree(d.weight);
+    if (d.cols) cudaFree(d.cols);
+    d = Dataset{};
+}
+
+amp_status load_dataset(amp_model* m, Dataset& d, bool is_norm, const double* d_x, const double* d_w, long long n, cudaStream_t s) {
+    if (!m) return AMP_ERR_INVALID;
+    if (n < 0 || (n > 0 && !d_x)) return fail(m, AMP_ERR_INVALID, "load: null events or negative count");
+    free_dataset(d);
+    for (auto& e : m->pool) (is_norm ? e.valid_norm : e.valid_data) = false;
+    d.n = n;
+    d.npad = pad32(n > 0 ? n : 1);
+    d.ncache = m->has_z ? NCOL_ALL : NCOL_K;
+    CK(cudaMalloc(&d.cache, sizeof(double) * d.ncache * d.npad));
+    CK(cudaMalloc(&d.weight, sizeof(double) * d.npad));
+    CK(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
+    const int grid = kinematics_grid(d.npad);
+    KinArgs a{};
+    a.dk = m->dk;
+    a.x = d_x;
+    a.w = d_w;
+    a.cache = d.cache;
+    a.weight = d.weight;
+    a.n = n;
+    a.npad = d.npad;
+    a.with_z = m->has_z ? 1 : 0;
+    a.weight_positive = is_norm ? 0 : 1;
+    a.flag = m->d_flag;
+    a.partial = m->d_partial;
+    CK(launch_kinematics(a, grid, s));
+    CK(launch_finalize(m->d_partial, grid, PARTIAL_STRIDE, 1, m->d_sums, s));
+    CK(cudaMemcpyAsync(m->h_pinned, m->d_sums, sizeof(double), cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(m->h_pinned + 1, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    int flag;
+    std::memcpy(&flag, m->h_pinned + 1, sizeof(int));
+    if (flag) {
+        free_dataset(d);
+        return fail(m, AMP_ERR_DOMAIN, is_norm ? "amp_load_norm: event outside phase space or bad weight"
+                                               : "amp_load_events: event outside phase space or non-positive efficiency");
+    }
+    d.wsum = m->h_pinned[0];
+    if (is_norm && n > 0 && !(d.wsum > 0)) {
+        free_dataset(d);
+        return fail(m, AMP_ERR_DOMAIN, "amp_load_norm: weights sum to zero");
+    }
+    d.loaded = true;
+    return AMP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* amp_version(void) { return "amp4d 0.1 (sm_100a)"; }
+
+const char* amp_status_string(amp_status s) {
+    switch (s) {
+        case AMP_OK: return "AMP_OK";
+        case AMP_ERR_INVALID: return "AMP_ERR_INVALID";
+        case AMP_ERR_STATE: return "AMP_ERR_STATE";
+        case AMP_ERR_DOMAIN: return "AMP_ERR_DOMAIN";
+        case AMP_ERR_CUDA: return "AMP_ERR_CUDA";
+        case AMP_ERR_NOMEM: return "AMP_ERR_NOMEM";
+    }
+    return "?";
+}
+
+const char* amp_last_error(const amp_model* m) { return m ? m->err.c_str() : "null model"; }
+
+amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, int n_res, amp_model** out) {
+    if (!decay || !res || !out || n_res < 1 || n_res > AMP_MAX_RESONANCES) return AMP_ERR_INVALID;
+    *out = nullptr;
+    if (!(decay->m_parent > 0 && decay->m_psi > 0 && decay->m_k > 0 && decay->m_pi > 0) ||
+        !(decay->m_parent > decay->m_psi + decay->m_k + decay->m_pi))
+        return AMP_ERR_INVALID;
+    amp_model* m = new (std::nothrow) amp_model();
+    if (!m) return AMP_ERR_NOMEM;
+    m->dk = DecayConst{decay->m_parent, decay->m_psi, decay->m_k, decay->m_pi};
+    m->R = n_res;
+    int K = 0;
+    for (int r = 0; r < n_res; ++r) {
+        const amp_resonance& a = res[r];
+        bool ok = true;
+        if (a.kind == AMP_KSTAR) ok = a.J >= 0 && a.J <= 4;
+        else if (a.kind == AMP_Z) ok = a.J == 1;
+        else if (a.kind == AMP_CONST) ok = a.J == 0;
+        else ok = false;
+        if (a.kind != AMP_CONST) ok = ok && a.mass > 0 && a.width > 0 && a.radius >= 0 && std::isfinite(a.mass + a.width + a.radius);
+        if (!ok) { delete m; return AMP_ERR_INVALID; }
+        m->res.push_back(a);
+        m->slot0[r] = K;
+        K += (a.kind == AMP_Z || (a.kind == AMP_KSTAR && a.J >= 1)) ? 3 : 1;
+        if (a.kind == AMP_Z) m->has_z = true;
+    }
+    if (K > AMP_MAX_COUPLINGS) { delete m; return AMP_ERR_INVALID; }
+    m->K = K;
+    for (int r = 0; r < n_res; ++r) {
+        LineConst lc;
+        if (!make_line_const(m, r, res[r].mass, res[r].width, &lc)) { delete m; return AMP_ERR_DOMAIN; }
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { delete m; return AMP_ERR_CUDA; }
+    cudaError_t e = cudaMalloc(&m->d_partial, sizeof(double) * 2 * AMP_MAX_POINTS * PARTIAL_STRIDE);
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_sums, sizeof(double) * 2 * AMP_MAX_POINTS);
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_result, sizeof(double) * 2 * AMP_MAX_POINTS);
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_flag, sizeof(int));
+    if (e == cudaSuccess) e = cudaMallocHost(&m->h_pinned, sizeof(double) * (2 * AMP_MAX_POINTS + 2));
+    if (e != cudaSuccess) { amp_model_destroy(m); return e == cudaErrorMemoryAllocation ? AMP_ERR_NOMEM : AMP_ERR_CUDA; }
+    *out = m;
+    return AMP_OK;
+}
+
+amp_status amp_model_destroy(amp_model* m) {
+    if (!m) return AMP_ERR_INVALID;
+    free_dataset(m->data);
+    free_dataset(m->norm);
+    if (m->d_partial) cudaFree(m->d_partial);
+    if (m->d_sums) cudaFree(m->d_sums);
+    if (m->d_result) cudaFree(m->d_result);
+    if (m->d_flag) cudaFree(m->d_flag);
+    if (m->h_pinned) cudaFreeHost(m->h_pinned);
+    delete m;
+    return AMP_OK;
+}
+
+int amp_num_couplings(const amp_model* m) { return m ? m->K : -1; }
+int amp_num_resonances(const amp_model* m) { return m ? m->R : -1; }
+
+amp_status amp_load_events(amp_model* m, const double* d_x, const double* d_eff, long long n, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    return load_dataset(m, m->data, false, d_x, d_eff, n, (cudaStream_t)stream);
+}
+
+amp_status amp_load_norm(amp_model* m, const double* d_x, const double* d_w, long long n_norm, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    if (n_norm < 1) return fail(m, AMP_ERR_INVALID, "amp_load_norm: need at least one normalisation event");
+    return load_dataset(m, m->norm, true, d_x, d_w, n_norm, (cudaStream_t)stream);
+}
+
+amp_status amp_set_norm_mode(amp_model* m, int mode) {
+    if (!m || mode < 0 || mode > 2) return AMP_ERR_INVALID;
+    m->norm_mode = mode;
+    return AMP_OK;
+}
+
+amp_status amp_set_lineshape_mode(amp_model* m, int mode) {
+    if (!m || mode < 0 || mode > 2) return AMP_ERR_INVALID;
+    m->lineshape_mode = mode;
+    return AMP_OK;
+}
+
+amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_recomputed, int* norm_path) {
+    if (!m) return AMP_ERR_INVALID;
+    if (launches) *launches = m->stat_launches;
+    if (columns_recomputed) *columns_recomputed = m->stat_columns;
+    if (norm_path) *norm_path = m->stat_norm_path;
+    return AMP_OK;
+}
+
+amp_status amp_probe_fp64(int kind, int iters, double* flops, void* stream) {
+    if (!flops || kind < 0 || kind > 1 || iters < 1) return AMP_ERR_INVALID;
+    return probe_fp64(kind, iters, flops, (cudaStream_t)stream) == cudaSuccess ? AMP_OK : AMP_ERR_CUDA;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------
+// Parameter points and the lineshape column pool
+namespace {
+
+// Make sure both datasets have a column pool of at least `need` slots.  Growing drops all columns.
+amp_status ensure_pool(amp_model* m, int need) {
+    if (need <= m->pool_cap && (!m->data.loaded || m->data.cols) && (!m->norm.loaded || m->norm.cols)) return AMP_OK;
+    int cap = std::max(need, m->pool_cap);
+    if (need > m->pool_cap) cap = std::max(need + 4, m->R + 4);
+    for (Dataset* d : {&m->data, &m->norm}) {
+        if (!d->loaded) continue;
+        if (d->cols && cap == m->pool_cap) continue;
+        if (d->cols) { cudaFree(d->cols); d->cols = nullptr; }
+        CK(cudaMalloc(&d->cols, sizeof(double2) * (size_t)cap * d->npad));
+        for (auto& e : m->pool) (d == &m->data ? e.valid_data : e.valid_norm) = false;
+    }
+    m->pool_cap = cap;
+    m->pool.resize(cap);
+    return AMP_OK;
+}
+
+}  // namespace
+
+extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_couplings, const double* h_mass_width) {
+    if (!m) return AMP_ERR_INVALID;
+    if (P < 1 || P > AMP_MAX_POINTS || !h_couplings) return fail(m, AMP_ERR_INVALID, "amp_set_params: bad P or null couplings");
+    const int R = m->R, K = m->K;
+    std::vector<double> mw((size_t)P * R * 2);
+    for (int p = 0; p < P; ++p)
+        for (int r = 0; r < R; ++r) {
+            double mass = m->res[r].mass, width = m->res[r].width;
+            if (h_mass_width && m->res[r].kind != AMP_CONST) { mass = h_mass_width[((size_t)p * R + r) * 2]; width = h_mass_width[((size_t)p * R + r) * 2 + 1]; }
+            LineConst lc;
+            if (!std::isfinite(mass) || !std::isfinite(width)) return fail(m, AMP_ERR_INVALID, "amp_set_params: non-finite mass or width");
+            if (!make_line_const(m, r, mass, width, &lc)) return fail(m, AMP_ERR_DOMAIN, "amp_set_params: pole mass outside the kinematic range or width <= 0");
+            mw[((size_t)p * R + r) * 2] = mass;
+            mw[((size_t)p * R + r) * 2 + 1] = width;
+        }
+    for (size_t i = 0; i < (size_t)P * K * 2; ++i)
+        if (!std::isfinite(h_couplings[i])) return fail(m, AMP_ERR_INVALID, "amp_set_params: non-finite coupling");
+    m->P = P;
+    m->couplings.assign(h_couplings, h_couplings + (size_t)P * K * 2);
+    m->mw.swap(mw);
+    m->call_id++;
+
+    // distinct (resonance, mass, width) keys of this call
+    struct Key { int r; double mass, width; };
+    std::vector<Key> keys;
+    std::vector<int> keyidx((size_t)P * R, -1);
+    for (int p = 0; p < P; ++p)
+        for (int r = 0; r < R; ++r) {
+            if (m->res[r].kind == AMP_CONST) continue;
+            const double mass = m->mw[((size_t)p * R + r) * 2], width = m->mw[((size_t)p * R + r) * 2 + 1];
+            int found = -1;
+            for (int k = (int)keys.size() - 1; k >= 0; --k)
+                if (keys[k].r == r && keys[k].mass == mass && keys[k].width == width) { found = k; break; }
+            if (found < 0) { keys.push_back(Key{r, mass, width}); found = (int)keys.size() - 1; }
+            keyidx[(size_t)p * R + r] = found;
+        }
+    // hit / miss against the pool; a resonance that misses call after call floats: with P == 1 its column
+    // is transient and is evaluated in registers by the combine kernel instead of making a round trip
+    std::vector<int> keyslot(keys.size(), -1);
+    bool res_missed[AMP_MAX_RESONANCES] = {};
+    for (size_t k = 0; k < keys.size(); ++k)
+        for (int sidx = 0; sidx < (int)m->pool.size(); ++sidx) {
+            const PoolEntry& e = m->pool[sidx];
+            if (e.r == keys[k].r && e.mass == keys[k].mass && e.width == keys[k].width) { keyslot[k] = sidx; break; }
+        }
+    for (size_t k = 0; k < keys.size(); ++k)
+        if (keyslot[k] < 0) res_missed[keys[k].r] = true;
+    for (int r = 0; r < R; ++r) m->miss_streak[r] = res_missed[r] ? m->miss_streak[r] + 1 : 0;
+    std::vector<char> inline_key(keys.size(), 0);
+    int need = 0;
+    for (size_t k = 0; k < keys.size(); ++k) {
+        const bool want_inline = P == 1 && keyslot[k] < 0 &&
+                                 (m->lineshape_mode == 2 || (m->lineshape_mode == 0 && m->miss_streak[keys[k].r] >= 2));
+        inline_key[k] = want_inline;
+        if (!want_inline) ++need;
+    }
+    amp_status st = ensure_pool(m, need);
+    if (st != AMP_OK) return st;
+    if (need > 0) {
+        // re-resolve hits (ensure_pool may have resized the table) and give misses the least recently used slots
+        for (size_t k = 0; k < keys.size(); ++k) {
+            keyslot[k] = -1;
+            for (int sidx = 0; sidx < (int)m->pool.size(); ++sidx) {
+                const PoolEntry& e = m->pool[sidx];
+                if (e.r == keys[k].r && e.mass == keys[k].mass && e.width == keys[k].width) { keyslot[k] = sidx; break; }
+            }
+            if (keyslot[k] >= 0) m->pool[keyslot[k]].last_used = m->call_id;
+        }
+        for (size_t k = 0; k < keys.size(); ++k) {
+            if (keyslot[k] >= 0 || inline_key[k]) continue;
+            int best = -1;
+            for (int sidx = 0; sidx < (int)m->pool.size(); ++sidx)
+                if (m->pool[sidx].last_used != m->call_id && (best < 0 || m->pool[sidx].last_used < m->pool[best].last_used)) best = sidx;
+            if (best < 0) return fail(m, AMP_ERR_NOMEM, "amp_set_params: lineshape column pool exhausted");
+            m->pool[best] = PoolEntry{keys[k].r, keys[k].mass, keys[k].width, false, false, m->call_id};
+            keyslot[k] = best;
+        }
+    }
+    m->colidx.assign((size_t)P * R, -1);
+    for (int p = 0; p < P; ++p)
+        for (int r = 0; r < R; ++r) {
+            const int k = keyidx[(size_t)p * R + r];
+            if (k >= 0) m->colidx[(size_t)p * R + r] = inline_key[k] ? -2 : keyslot[k];
+        }
+    return AMP_OK;
+}
+
+namespace {
+
+// Recompute the columns of `d` that the current points need and that are not valid yet.
+amp_status refresh_columns(amp_model* m, Dataset& d, bool is_norm, cudaStream_t s) {
+    std::vector<LineshapeJob> jobs;
+    std::vector<char> seen(m->pool.size(), 0);
+    for (int p = 0; p < m->P; ++p)
+        for (int r = 0; r < m->R; ++r) {
+            const int sidx = m->colidx[(size_t)p * m->R + r];
+            if (sidx < 0 || seen[sidx]) continue;
+            seen[sidx] = 1;
+            PoolEntry& e = m->pool[sidx];
+            if (is_norm ? e.valid_norm : e.valid_data) continue;
+            LineshapeJob j;
+            make_line_const(m, e.r, e.mass, e.width, &j.lc);
+            j.column = sidx;
+            jobs.push_back(j);
+            (is_norm ? e.valid_norm : e.valid_data) = true;
+        }
+    if (jobs.empty() || d.n == 0) return AMP_OK;
+    CK(launch_lineshape(d, jobs.data(), (int)jobs.size(), s));
+    m->stat_launches += ((int)jobs.size() + MAX_LINE_JOBS - 1) / MAX_LINE_JOBS;
+    m->stat_columns += (int)jobs.size();
+    return AMP_OK;
+}
+
+// Arguments of the streaming kernel for point p on dataset d.
+void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, StreamArgs* a) {
+    std::memset(a, 0, sizeof(*a));
+    int t = 0, nlc = 0;
+    auto add = [&](int r) {
+        SlotRef& ref = a->ref[t++];
+        ref.c0 = m->slot0[r];
+        const int sidx = m->colidx[(size_t)p * m->R + r];
+        if (sidx >= 0) { ref.column = sidx; ref.lc = 0; return; }
+        ref.column = -1;
+        ref.lc = nlc;
+        make_line_const(m, r, m->mw[((size_t)p * m->R + r) * 2], m->mw[((size_t)p * m->R + r) * 2 + 1], &a->lc[nlc++]);
+    };
+    for (int J = 0; J < 5; ++J) {
+        a->jstart[J] = t;
+        for (int r = 0; r < m->R; ++r)
+            if (m->res[r].kind != AMP_Z && m->res[r].J == J) add(r);
+    }
+    a->jstart[5] = t;
+    for (int r = 0; r < m->R; ++r)
+        if (m->res[r].kind == AMP_Z) add(r);
+    a->zend = t;
+    for (int k = 0; k < m->K; ++k) a->c[k] = make_double2(m->couplings[((size_t)p * m->K + k) * 2], m->couplings[((size_t)p * m->K + k) * 2 + 1]);
+    a->cache = d.cache;
+    a->weight = d.weight;
+    a->cols = d.cols;
+    a->n = d.n;
+    a->npad = d.npad;
+    a->flag = m->d_flag;
+    a->mode = mode;
+}
+
+// nll[p] = -(sum_i log S_i + sum_i log eps_i) + N log I(p), I(p) = sum_j w_j S_j / sum_j w_j
+__global__ void k_nll_final(const double* __restrict__ sums, int P, double n_data, double sum_log_eff, double wsum, int want_nll,
+                            double* __restrict__ result) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    const double I = sums[P + p] / wsum;
+    result[P + p] = I;
+    if (want_nll) {
+        double v = -(sums[p] + sum_log_eff) + n_data * log(I);
+        if (!isfinite(v) || !(I > 0.0)) v = INFINITY;
+        result[p] = v;
+    }
+}
+
+amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cudaStream_t s) {
+    if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
+    if (want_nll && !m->data.loaded) return fail(m, AMP_ERR_STATE, "no data events loaded (amp_load_events)");
+    if (m->P < 1) return fail(m, AMP_ERR_STATE, "no parameters set (amp_set_params)");
+    const int P = m->P;
+    m->stat_launches = m->stat_columns = 0;
+    m->stat_norm_path = 1;
+    amp_status st = ensure_pool(m, 0);
+    if (st != AMP_OK) return st;
+    CK(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
+    if (want_nll) { st = refresh_columns(m, m->data, false, s); if (st != AMP_OK) return st; }
+    st = refresh_columns(m, m->norm, true, s);
+    if (st != AMP_OK) return st;
+    const int gd = stream_grid(m->data.n), gn = stream_grid(m->norm.n);
+    StreamArgs a;
+    for (int p = 0; p < P; ++p) {
+        if (want_nll) {
+            if (m->data.n > 0) {
+                fill_stream_args(m, m->data, p, MODE_DATA, &a);
+                a.partial = m->d_partial + (size_t)p * PARTIAL_STRIDE;
+                CK(launch_stream(a, gd, s));
+                m->stat_launches++;
+            } else {
+                CK(cudaMemsetAsync(m->d_partial + (size_t)p * PARTIAL_STRIDE, 0, sizeof(double), s));
+            }
+        }
+        fill_stream_args(m, m->norm, p, MODE_NORM, &a);
+        a.partial = m->d_partial + (size_t)(P + p) * PARTIAL_STRIDE;
+        CK(launch_stream(a, gn, s));
+        m->stat_launches++;
+    }
+    if (want_nll) {
+        CK(launch_finalize(m->d_partial, m->data.n > 0 ? gd : 1, PARTIAL_STRIDE, P, m->d_sums, s));
+        m->stat_launches++;
+    }
+    CK(launch_finalize(m->d_partial + (size_t)P * PARTIAL_STRIDE, gn, PARTIAL_STRIDE, P, m->d_sums + P, s));
+    k_nll_final<<<(P + 127) / 128, 128, 0, s>>>(m->d_sums, P, (double)m->data.n, m->data.loaded ? m->data.wsum : 0.0, m->norm.wsum, want_nll ? 1 : 0,
+                                                m->d_result);
+    CK(cudaGetLastError());
+    m->stat_launches += 2;
+    CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 2 * P, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(m->h_pinned + 2 * P, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    int flag;
+    std::memcpy(&flag, m->h_pinned + 2 * P, sizeof(int));
+    bool bad = flag != 0;
+    for (int p = 0; p < P; ++p) {
+        if (h_nll) { h_nll[p] = m->h_pinned[p]; bad |= !std::isfinite(h_nll[p]); }
+        if (h_I) { h_I[p] = m->h_pinned[P + p]; bad |= !(h_I[p] > 0) || !std::isfinite(h_I[p]); }
+    }
+    if (bad) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
+    return AMP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+amp_status amp_nll(amp_model* m, double* h_nll, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    if (!h_nll) return fail(m, AMP_ERR_INVALID, "amp_nll: null output");
+    return evaluate(m, true, h_nll, nullptr, (cudaStream_t)stream);
+}
+
+amp_status amp_norm_integral(amp_model* m, double* h_I, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    if (!h_I) return fail(m, AMP_ERR_INVALID, "amp_norm_integral: null output");
+    return evaluate(m, false, nullptr, h_I, (cudaStream_t)stream);
+}
+
+amp_status amp_eval_events(amp_model* m, int p, double* d_out, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!m->data.loaded) return fail(m, AMP_ERR_STATE, "no data events loaded (amp_load_events)");
+    if (m->P < 1) return fail(m, AMP_ERR_STATE, "no parameters set (amp_set_params)");
+    if (p < 0 || p >= m->P || (!d_out && m->data.n > 0)) return fail(m, AMP_ERR_INVALID, "amp_eval_events: bad point index or null output");
+    if (m->data.n == 0) return AMP_OK;
+    m->stat_launches = m->stat_columns = 0;
+    amp_status st = ensure_pool(m, 0);
+    if (st != AMP_OK) return st;
+    st = refresh_columns(m, m->data, false, s);
+    if (st != AMP_OK) return st;
+    StreamArgs a;
+    fill_stream_args(m, m->data, p, MODE_EVAL, &a);
+    a.out = d_out;
+    CK(launch_stream(a, stream_grid(m->data.n), s));
+    m->stat_launches++;
+    CK(cudaStreamSynchronize(s));
+    return AMP_OK;
+}
+
+static const char* const kColNames[NCOL_ALL] = {"m2", "inv_m", "q", "pB", "cosK", "sinK", "cosPsi", "sinPsi", "cosPhi", "sinPhi",
+                                                "mZ2", "inv_mZ", "qZ", "pBZ", "cosZ", "sinZ", "cosT", "sinT", "cosPhiT", "sinPhiT", "cosAlpha", "sinAlpha"};
+const char* amp_cache_column_name(int i) { return (i >= 0 && i < NCOL_ALL) ? kColNames[i] : nullptr; }
+
+amp_status amp_dump_cache(amp_model* m, int which, double* d_out, int* ncols, void* stream) {
+    if (!m || which < 0 || which > 1) return AMP_ERR_INVALID;
+    Dataset& d = which ? m->norm : m->data;
+    if (!d.loaded) return fail(m, AMP_ERR_STATE, "amp_dump_cache: dataset not loaded");
+    if (ncols) *ncols = d.ncache;
+    if (!d_out || d.n == 0) return AMP_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    CK(cudaMemcpy2DAsync(d_out, sizeof(double) * d.n, d.cache, sizeof(double) * d.npad, sizeof(double) * d.n, d.ncache, cudaMemcpyDeviceToDevice, s));
+    CK(cudaStreamSynchronize(s));
+    return AMP_OK;
+}
+
+amp_status amp_eval_lineshape(amp_model* m, int which, int r, double mass, double width, double* d_out, void* stream) {
+    if (!m || which < 0 || which > 1 || r < 0 || r >= m->R || !d_out) return AMP_ERR_INVALID;
+    Dataset& d = which ? m->norm : m->data;
+    if (!d.loaded) return fail(m, AMP_ERR_STATE, "amp_eval_lineshape: dataset not loaded");
+    cudaStream_t s = (cudaStream_t)stream;
+    LineshapeJob j;
+    if (!make_line_const(m, r, mass, width, &j.lc)) return fail(m, AMP_ERR_DOMAIN, "amp_eval_lineshape: pole mass outside the kinematic range");
+    j.column = 0;
+    Dataset tmp = d;   // same cache, private one-column pool
+    tmp.cols = nullptr;
+    CK(cudaMalloc(&tmp.cols, sizeof(double2) * d.npad));
+    cudaError_t e = launch_lineshape(tmp, &j, 1, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_out, tmp.cols, sizeof(double2) * d.n, cudaMemcpyDeviceToDevice, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(tmp.cols);
+    if (e != cudaSuccess) return cuda_fail(m, e, "amp_eval_lineshape");
+    return AMP_OK;
+}
+
+amp_status amp_norm_matrix(amp_model* m, int p, double* h_M, void* stream) {
+    (void)p; (void)h_M; (void)stream;
+    return fail(m, AMP_ERR_STATE, "amp_norm_matrix: not built yet");
+}
+
+}  // extern "C"

@@ -1,0 +1,152 @@
+// kinematics.cu — step a1: the once-per-dataset kinematics cache.
+//
+// For every event (m_Kpi, cos theta_K*, cos theta_psi, phi) (Eq. 1) compute everything
+// in Eqs. 4 and 10 that does not depend on fit parameters: the running-mass quantities the lineshapes
+// need, the sines of the input helicity angles, the phi phase, and the Z-chain
+// variables m_psipi, theta_Z, theta~_psi, phi~, alpha.
+//
+// The Z chain is derived from Lorentz invariants and closed forms,
+// not by boosting 4-vectors: in the J/psi rest frame every hadron lies in the x-z plane (z = K*
+// direction, K on the +x side), so only z components change under the boost along z and the two
+// dihedral angles reduce to ratios of components of the mu+ direction.
+//
+// HBM-bound: reads 32-40 B, writes 88-184 B per event; one thread per event, fully coalesced.
+#include "amp_internal.cuh"
+
+namespace amp {
+
+__device__ __forceinline__ double two_body(double M, double a, double b) {
+    const double s = a + b, d = a - b;
+    return sqrt((M - s) * (M + s) * (M - d) * (M + d)) / (2.0 * M);
+}
+
+__global__ void __launch_bounds__(256) k_kinematics(const KinArgs a) {
+    const double MB = a.dk.MB, mpsi = a.dk.mpsi, mK = a.dk.mK, mpi = a.dk.mpi;
+    double acc = 0.0;
+    bool bad = false;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < a.npad; i += (long long)gridDim.x * blockDim.x) {
+        double* col = a.cache + i;
+        if (i >= a.n) {   // padding: benign values, weight 0
+            for (int c = 0; c < (a.with_z ? NCOL_ALL : NCOL_K); ++c) col[c * a.npad] = 1.0;
+            a.weight[i] = 0.0;
+            continue;
+        }
+        const double m = a.x[i], cK = a.x[a.n + i], cpsi = a.x[2 * a.n + i], phi = a.x[3 * a.n + i];
+        const double w = a.w ? a.w[i] : 1.0;
+        // domain: strictly inside phase space, finite inputs, positive efficiency / non-negative weight
+        const bool ok = (m > mK + mpi) && (m < MB - mpsi) && (fabs(cK) <= 1.0) && (fabs(cpsi) <= 1.0) && isfinite(phi) &&
+                        isfinite(w) && (a.weight_positive ? (w > 0.0) : (w >= 0.0));
+        if (!ok) { bad = true; continue; }
+        a.weight[i] = w;
+        acc += a.weight_positive ? log(w) : w;
+
+        const double m2 = m * m, invm = 1.0 / m;
+        const double q = two_body(m, mK, mpi);
+        const double pB = two_body(MB, m, mpsi);
+        const double sK = sqrt((1.0 - cK) * (1.0 + cK)), spsi = sqrt((1.0 - cpsi) * (1.0 + cpsi));
+        double sphi, cphi;
+        sincos(phi, &sphi, &cphi);
+        col[C_M2 * a.npad] = m2;
+        col[C_INVM * a.npad] = invm;
+        col[C_Q * a.npad] = q;
+        col[C_PB * a.npad] = pB;
+        col[C_CK * a.npad] = cK;
+        col[C_SK * a.npad] = sK;
+        col[C_CPSI * a.npad] = cpsi;
+        col[C_SPSI * a.npad] = spsi;
+        col[C_CPHI * a.npad] = cphi;
+        col[C_SPHI * a.npad] = sphi;
+        if (!a.with_z) continue;
+
+        // B frame, z along the K pi system.  Energies in the K pi frame, then boosted with gamma = E_Kpi/m.
+        const double EKpi = (MB * MB + m2 - mpsi * mpsi) / (2.0 * MB), Epsi = MB - EKpi;
+        const double g = EKpi * invm, bg = pB * invm;
+        const double Epi_r = (m2 - mK * mK + mpi * mpi) * (0.5 * invm);
+        const double Epi = g * Epi_r - bg * q * cK;      // pion energy, B frame
+        const double ppz = bg * Epi_r - g * q * cK;      // pion p_z, B frame (p_x = -q sK)
+        // m_psipi^2 = (P_psi + P_pi)^2, linear in cos theta_K*
+        const double mZ2 = mpsi * mpsi + mpi * mpi + 2.0 * (Epsi * Epi + pB * ppz);
+        const double mZ = sqrt(mZ2), invmZ = 1.0 / mZ;
+        // J/psi rest frame: boost along z; pion direction n_pi = (nx, 0, nz)
+        const double pz = (Epsi * ppz + pB * Epi) / mpsi, px = -q * sK;
+        const double inorm = rsqrt(pz * pz + px * px);
+        const double nx = px * inorm, nz = pz * inorm;
+        // mu+ direction n_mu = (spsi cphi, spsi sphi, cpsi); theta~ = angle(mu+, pi)
+        const double ct = spsi * cphi * nx + cpsi * nz;
+        // components of n_mu perpendicular to n_pi: along x_Z = y x n_pi = (nz, 0, -nx) and along y
+        const double ax = spsi * cphi * nz - cpsi * nx, ay = spsi * sphi;
+        const double st = sqrt(ax * ax + ay * ay);
+        const double ist = 1.0 / st;
+        // phi~: azimuth of mu+ about n_pi from the K side; alpha: from the (mu+,pi) to the (mu+,K*) plane about n_mu
+        const double cpt = ax * ist, spt = ay * ist;
+        const double ca = (spsi * nz - cpsi * cphi * nx) * ist, sa = -sphi * nx * ist;
+        // Z rest frame: theta_Z = angle(K, pi) from invariants; sine from the Gram determinant
+        const double pBZ = two_body(MB, mZ, mK);         // Z (and K) momentum in the B frame
+        const double qZ = two_body(mZ, mpsi, mpi);       // pi momentum in the Z frame
+        const double pKZ = pBZ * MB * invmZ;             // K momentum in the Z frame
+        const double EKZ = (MB * MB - mZ2 - mK * mK) * (0.5 * invmZ), EpiZ = (mZ2 + mpi * mpi - mpsi * mpsi) * (0.5 * invmZ);
+        const double iden = 1.0 / (pKZ * qZ);
+        const double cZ = (EKZ * EpiZ - 0.5 * (m2 - mK * mK - mpi * mpi)) * iden;
+        const double sZ = MB * q * pB * sK * invmZ * iden;
+        col[C_MZ2 * a.npad] = mZ2;
+        col[C_INVMZ * a.npad] = invmZ;
+        col[C_QZ * a.npad] = qZ;
+        col[C_PBZ * a.npad] = pBZ;
+        col[C_CZ * a.npad] = cZ;
+        col[C_SZ * a.npad] = sZ;
+        col[C_CT * a.npad] = ct;
+        col[C_ST * a.npad] = st;
+        col[C_CPT * a.npad] = cpt;
+        col[C_SPT * a.npad] = spt;
+        col[C_CA * a.npad] = ca;
+        col[C_SA * a.npad] = sa;
+    }
+    if (bad) atomicOr(a.flag, 1);
+    // deterministic block reduction of acc (fixed shuffle tree, fixed warp order)
+    __shared__ double sm[8];
+#pragma unroll
+    for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int wv = 0; wv < 8; ++wv) t += sm[wv];
+        a.partial[blockIdx.x] = t;
+    }
+}
+
+int kinematics_grid(long long n) {
+    long long blocks = (n + 255) / 256;
+    const long long cap = 148 * 8;
+    return (int)(blocks < 1 ? 1 : (blocks > cap ? cap : blocks));
+}
+
+cudaError_t launch_kinematics(const KinArgs& a, int grid, cudaStream_t s) {
+    k_kinematics<<<grid, 256, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
+// out[j] = sum_b partial[j * stride + b], b < nblocks, in a fixed order: thread t adds b = t, t+256, ...
+// then a fixed shuffle/shared tree.  One block per row.
+__global__ void __launch_bounds__(256) k_finalize(const double* __restrict__ partial, int nblocks, int stride, double* __restrict__ out) {
+    const double* p = partial + (size_t)blockIdx.x * stride;
+    double acc = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += 256) acc += p[b];
+    __shared__ double sm[8];
+#pragma unroll
+    for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int wv = 0; wv < 8; ++wv) t += sm[wv];
+        out[blockIdx.x] = t;
+    }
+}
+
+cudaError_t launch_finalize(const double* partial, int nblocks, int stride, int nrows, double* out, cudaStream_t s) {
+    k_finalize<<<nrows, 256, 0, s>>>(partial, nblocks, stride, out);
+    return cudaGetLastError();
+}
+
+}  // namespace amp

@@ -150,22 +150,53 @@ def norm_events(cfg, m=None):
     return x, efficiency(cfg, x)
 
 
+def _mass_proposal(rng, k):
+    """m drawn from an equal mixture of the phase-space density and a truncated Cauchy peak at the K*(892)
+    (a proposal shape only: it flattens the narrow peak so that accept-reject wastes fewer model evaluations);
+    returns (m [k], ratio [k] = phase-space density / proposal density, up to a common constant)."""
+    MB, mpsi, mK, mpi = DECAY
+    lo, hi = mK + mpi + M_LO_MARGIN, M_HI
+    M0, G0 = KSTARS[1][3], 0.5 * KSTARS[1][4]
+    grid = np.linspace(lo, hi, 20001)
+    fps = _two_body_momentum(MB, grid, mpsi) * _two_body_momentum(grid, mK, mpi)
+    zps = np.sum(0.5 * (fps[1:] + fps[:-1])) * (grid[1] - grid[0])          # normalisation of the phase-space density
+    a_lo, a_hi = np.arctan((lo - M0) / G0), np.arctan((hi - M0) / G0)
+    n_ps = rng.binomial(k, 0.5)
+    m = np.concatenate([phase_space_events(rng, n_ps)[0], M0 + G0 * np.tan(rng.uniform(a_lo, a_hi, k - n_ps))])
+    m = m[rng.permutation(k)]
+    g_ps = _two_body_momentum(MB, m, mpsi) * _two_body_momentum(m, mK, mpi) / zps
+    g_c = (G0 / ((m - M0) ** 2 + G0 ** 2)) / (a_hi - a_lo)
+    return m, g_ps / (0.5 * g_ps + 0.5 * g_c)
+
+
+def _proposal_events(rng, k):
+    m, ratio = _mass_proposal(rng, k)
+    x = np.empty((4, k))
+    x[0] = m
+    x[1] = np.clip(rng.uniform(-1, 1, k), -COS_MAX, COS_MAX)
+    x[2] = np.clip(rng.uniform(-1, 1, k), -COS_MAX, COS_MAX)
+    x[3] = rng.uniform(-np.pi, np.pi, k)
+    return x, ratio
+
+
 def data_events(cfg, density, n=None, chunk=None):
     """(x [4][n], eff [n]) accept-reject sampled from eff * S over phase space.
 
-    ``density(x) -> eff(x) * S(x)`` for x SoA [4][k] is the model evaluation handed in by the caller
-    (the oracle in tests; the product's amp_eval_events in bench.py, as the paper generates its
-    pseudo-data with the fitter itself).  Envelope: 1.5 x the maximum over a 1e5-event pilot; proposals
-    above the envelope are accepted with probability 1 (the sample is a valid input either way)."""
+    ``density(x, eff) -> eff(x) * S(x)`` for x SoA [4][k] is the model evaluation handed in by the caller
+    (the oracle in tests; the product's amp_eval_events in bench.py, as the paper generates its pseudo-data
+    with the fitter itself).  Proposals: angles uniform, m from `_mass_proposal`; a proposal is accepted
+    with probability density * ratio / envelope, envelope = 1.5 x the maximum of density * ratio over a
+    1e5-event pilot (values above the envelope are accepted with probability 1: the sample is a valid
+    input either way)."""
     n = SIZES[cfg][0] if n is None else n
     rng = _rng(cfg, "data")
-    pilot = phase_space_events(rng, 100_000)
-    fmax = 1.5 * float(np.max(density(pilot, efficiency(cfg, pilot))))
-    chunk = chunk or max(200_000, min(4 * n, 8_000_000))
+    pilot, ratio = _proposal_events(rng, 100_000)
+    fmax = 1.5 * float(np.max(density(pilot, efficiency(cfg, pilot)) * ratio))
+    chunk = chunk or int(max(100_000, min(2 * n, 4_000_000)))
     out, filled = np.empty((4, n)), 0
     while filled < n:
-        xx = phase_space_events(rng, chunk)
-        f = density(xx, efficiency(cfg, xx))
+        xx, ratio = _proposal_events(rng, chunk)
+        f = density(xx, efficiency(cfg, xx)) * ratio
         keep = xx[:, rng.uniform(0, fmax, chunk) < f]
         take = min(keep.shape[1], n - filled)
         out[:, filled:filled + take] = keep[:, :take]
