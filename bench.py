@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py — NLL evaluations per second of the 4D amplitude model on B200 (BASELINE.json metric).
+
+Workload (config.workload): BASELINE.json configs[3] at its headline point — the full K* + Z model
+(11 resonances, K = 27 couplings), 2M data events and 10M normalisation events, FP64 structure-of-arrays,
+every lineshape floating: each timed step is one `amp_set_params` (new masses and widths for all 11
+resonances, new couplings) + one `amp_nll` through the C ABI, i.e. one pass of the whole hot path
+(lineshapes -> combine -> normalisation -> -log L reduction) over the data and the normalisation sample.
+The kinematics cache is built once per dataset (step a1, outside the per-step metric, reported separately).
+
+One JSON line on stdout (rank 0).  `--impl reference` times the CPU oracle instead (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2007_14931_b200 import workloads as W  # noqa: E402
+
+METRIC = "4D amplitude NLL evals/sec at 2M events (FP64)"
+UNIT = "NLL evals/s"
+
+# Algorithmic work per event of the fused streaming kernel with all lineshapes evaluated in registers
+# (DESIGN.md "Rooflines"): 22 cached FP64 values read per event (+ the weight on the normalisation side);
+# flops: + - x once, FMA twice, / sqrt log once each.
+BYTES_PER_EVENT_DATA = 22 * 8
+BYTES_PER_EVENT_NORM = 23 * 8
+FLOP_PER_EVENT = 730.0
+FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # 148 SMs x 64 DFMA/clk x 2 flop x 1965 MHz
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured"
+    return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """SM clock and throttle reasons sampled through NVML (pynvml) in a thread DURING the timed region."""
+
+    def __init__(self, index):
+        self.index, self.rows, self.stop_flag, self.thread = index, [], False, None
+
+    def start(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            self.nv = nv
+            self.h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.smax = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+        except Exception as e:   # noqa: BLE001
+            self.nv = None
+            self.err = repr(e)
+            return
+        self.thread = threading.Thread(target=self._poll, daemon=True)
+        self.thread.start()
+
+    def _poll(self):
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1e3
+                self.rows.append((time.perf_counter(), sm, rs, pw))
+            except Exception:   # noqa: BLE001
+                pass
+            time.sleep(0.001)
+
+    def stop(self, t0=None, t1=None):
+        if not getattr(self, "nv", None):
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable: " + getattr(self, "err", "")]}
+        self.stop_flag = True
+        self.thread.join(timeout=2)
+        nv = self.nv
+        rows = [r for r in self.rows if (t0 is None or r[0] >= t0) and (t1 is None or r[0] <= t1)] or self.rows[-3:]
+        names = {"hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown, "hw_thermal_slowdown": nv.nvmlClocksEventReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksEventReasonSwThermalSlowdown, "sw_power_cap": nv.nvmlClocksEventReasonSwPowerCap}
+        reasons = sorted(k for k, bit in names.items() if any(r[2] & bit for r in rows))
+        return {"sm_mhz": float(np.median([r[1] for r in rows])) if rows else None, "sm_max_mhz": float(self.smax), "reasons": reasons,
+                "power_w_max": max(r[3] for r in rows) if rows else None, "samples": len(rows)}
+
+
+def build_workload(args, device):
+    """events on the device, model with data + norm loaded.  Data events: accept-reject driven by the product's
+    own amp_eval_events (toy generation with the fitter itself)."""
+    import torch
+    from paper_2007_14931_b200 import binding as B
+
+    cfg = args.cfg
+    res = W.resonances(cfg)
+    c = W.couplings(cfg)
+    dev = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=device)
+    gen = B.Model(W.DECAY, res)
+
+    def density(xx, ee):
+        gen.load_events(dev(xx), dev(ee))
+        gen.set_params(c)
+        return gen.eval_events(0).cpu().numpy()
+
+    t0 = time.time()
+    x, eff = W.data_events(cfg, density, n=args.n_data)
+    gen.close()
+    xn, wn = W.norm_events(cfg, args.n_norm)
+    t_gen = time.time() - t0
+    model = B.Model(W.DECAY, res)
+    d_x, d_e, d_xn, d_wn = dev(x), dev(eff), dev(xn), dev(wn)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    model.load_events(d_x, d_e)
+    model.load_norm(d_xn, d_wn)
+    e1.record()
+    torch.cuda.synchronize()
+    load_ms = e0.elapsed_time(e1)
+    del d_x, d_e, d_xn, d_wn
+    return model, c, {"gen_s": t_gen, "load_ms": load_ms}
+
+
+def step_params(cfg, c, step):
+    """parameters of timed call `step`: every mass and width moved by a seeded 1e-4 step (cfg 3 call pattern) and
+    the couplings rotated by a small seeded amount, so that successive calls genuinely differ."""
+    if cfg == 4:
+        return W.fit_points(cfg, step)
+    mw = W.step_mass_width(cfg, step)
+    rng = np.random.default_rng(np.random.SeedSequence([W.SEED, 99, int(step)]))
+    cc = c * (1.0 + 1e-3 * rng.uniform(-1, 1, c.size)) * np.exp(1e-3j * rng.uniform(-1, 1, c.size))
+    return cc[None], mw[None]
+
+
+def run_own(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+    from paper_2007_14931_b200 import binding as B
+
+    model, c, info = build_workload(args, device)
+    P = 121 if args.cfg == 4 else 1
+    params = [step_params(args.cfg, c, s) for s in range(args.warmup + args.steps)]
+    h2d = sum(a.nbytes for a in (np.zeros((P, model.K, 2)), np.zeros((P, model.R, 2))))
+    d2h = 8 * P
+
+    def one_step(s):
+        cs, mws = params[s]
+        model.set_params(cs, mws)
+        return model.nll()
+
+    for s in range(args.warmup):
+        one_step(s)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.02)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches, t_norm, t_data, t_line = 0, [], [], []
+    nll_last = None
+    t_wall0 = time.perf_counter()
+    ev0.record()
+    for s in range(args.warmup, args.warmup + args.steps):
+        nll_last = one_step(s)
+        launches += model.last_call_stats()["launches"]
+        tm = model.last_call_timing()
+        t_norm.append(tm["norm_ms"]); t_data.append(tm["data_ms"]); t_line.append(tm["lineshape_ms"])
+    ev1.record()
+    torch.cuda.synchronize()
+    t_wall = time.perf_counter() - t_wall0
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop(t_wall0, t_wall0 + t_wall) if rank == 0 else None
+    dev_ms = ev0.elapsed_time(ev1)
+    if world > 1:
+        t = torch.tensor([dev_ms, t_wall * 1e3], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dev_ms, t_wall = float(t[0]), float(t[1]) / 1e3
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    evals = P * args.steps * world          # replicas: every rank evaluates its own data set
+    value = evals / (dev_ms * 1e-3)
+    e2e = evals / t_wall
+    hbm_peak, peak_kind = measured_peaks()
+    norm_ms = float(np.mean(t_norm))
+    if args.cfg == 4:
+        roof = None
+    else:
+        ach = BYTES_PER_EVENT_NORM * args.n_norm / (norm_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "k_stream<MODE_NORM> (fused lineshape + combine + reduce over the norm sample)",
+                "achieved": ach, "peak": hbm_peak, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})", "unit": "GB/s",
+                "frac": ach / hbm_peak, "traffic": None,
+                "alu_frac_nominal": FLOP_PER_EVENT * args.n_norm / (norm_ms * 1e-3) / FP64_PEAK_NOMINAL,
+                "kernel_ms": norm_ms, "bytes_per_event": BYTES_PER_EVENT_NORM, "flop_per_event": FLOP_PER_EVENT}
+    fp64 = {"dfma_tflops_measured": B.probe_fp64(0, 4000) / 1e12, "dmma_tflops_measured": B.probe_fp64(1, 4000) / 1e12,
+            "nominal_tflops": FP64_PEAK_NOMINAL / 1e12}
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"configs[{args.cfg}]: full K*+Z model (R=11, K=27), {args.n_data} data / {args.n_norm} norm events per GPU, "
+                               f"P={P}, all lineshapes floating", "n_data": args.n_data, "n_norm": args.n_norm, "P": P,
+                   "l2": "inputs (2.1 GB kinematics cache) larger than L2; no flush needed", "parallelism": f"replicas x{world}"},
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+        "gpu_launches": int(launches),
+        "event_evals_per_s": value * (args.n_data + args.n_norm),
+        "phase_ms": {"lineshape": float(np.mean(t_line)), "data": float(np.mean(t_data)), "norm": norm_ms},
+        "roofline": roof, "fp64_probe": fp64, "clocks": clocks,
+        "setup": info, "nll_last": [float(v) for v in np.atleast_1d(nll_last)[:3]],
+    }
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(args)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def cpu_baseline(args, budget_events=1_500_000):
+    """The oracle, as it stands, timed on this box's host cores on a bounded sample of the same workload:
+    same model and call pattern, sample sizes scaled down by the same factor for data and norm events;
+    data events drawn by oracle-driven accept-reject (no oracle input comes from the CUDA path)."""
+    from oracle import oracle as O
+    cfg = args.cfg
+    P = 121 if cfg == 4 else 1
+    budget = max(budget_events // P, 6000)
+    n = max(int(budget * args.n_data / (args.n_data + args.n_norm)), 1000)
+    m = max(budget - n, 5000)
+    Mo = O.Model(W.DECAY, W.resonances(cfg))
+    c = W.couplings(cfg)
+    xn, wn = W.norm_events(cfg, m)
+    x, eff = W.data_events(cfg, lambda xx, ee: Mo.eval_events(c, xx, ee), n=n)
+    cs, mws = step_params(cfg, c, 0)
+    t0 = time.perf_counter()
+    nll, _ = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+    dt = time.perf_counter() - t0
+    full = dt * (args.n_data + args.n_norm) / (n + m)            # extrapolated time of one full-size call
+    return {"value": P / full, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "sample": f"{n} data + {m} norm events (same model, P={P}), {dt:.2f} s measured, scaled linearly to {args.n_data}+{args.n_norm}",
+            "event_evals_per_s": P * (n + m) / dt}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    cfg = args.cfg
+    P = 121 if cfg == 4 else 1
+    # bounded sample per step so that steps+warmup finish in a few minutes
+    per_step = max(1_200_000 // (P * max(args.steps + args.warmup, 1)), 4000)
+    n = max(int(per_step * args.n_data / (args.n_data + args.n_norm)), 500)
+    m = max(per_step - n, 2000)
+    Mo = O.Model(W.DECAY, W.resonances(cfg))
+    c = W.couplings(cfg)
+    xn, wn = W.norm_events(cfg, m)
+    x, eff = W.data_events(cfg, lambda xx, ee: Mo.eval_events(c, xx, ee), n=n)
+    times = []
+    for s in range(args.warmup + args.steps):
+        cs, mws = step_params(cfg, c, s)
+        t0 = time.perf_counter()
+        Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+        if s >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    dt = float(np.sum(times))
+    scale = (args.n_data + args.n_norm) / (n + m)
+    value = P * args.steps / (dt * scale)
+    sample = f"{n} data + {m} norm events per step (same model, P={P}), scaled linearly to {args.n_data}+{args.n_norm}"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * scale / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"configs[{cfg}]: full K*+Z model (R=11, K=27), {args.n_data} data / {args.n_norm} norm events, P={P}, "
+                                   "all lineshapes floating", "n_data": args.n_data, "n_norm": args.n_norm, "P": P},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="own", choices=["own", "reference"])
+    ap.add_argument("--cfg", type=int, default=3, choices=[3, 4], help="3: P=1 all lineshapes floating (headline); 4: P=121 fit-loop pattern")
+    ap.add_argument("--n-data", type=int, default=2_000_000)
+    ap.add_argument("--n-norm", type=int, default=10_000_000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "own" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_own(args)
+
+
+if __name__ == "__main__":
+    main()

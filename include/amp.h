@@ -138,6 +138,11 @@ amp_status amp_set_lineshape_mode(amp_model* m, int mode);
  * recomputed (data + norm), which normalisation path ran (1 direct, 2 matrix).                         */
 amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_recomputed, int* norm_path);
 
+/* Device time [ms] of the phases of the last amp_nll / amp_norm_integral call, from CUDA events recorded on
+ * the call's stream: ms4[0] lineshape columns, ms4[1] data-side combine + reduce, ms4[2] normalisation,
+ * ms4[3] final reductions and the copy of the result.                                                   */
+amp_status amp_last_call_timing(const amp_model* m, double* ms4);
+
 const char* amp_last_error(const amp_model* m);
 const char* amp_status_string(amp_status s);
 const char* amp_version(void);

@@ -20,7 +20,7 @@ SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
     "amp_load_norm", "amp_set_params", "amp_nll", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
     "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_set_norm_mode", "amp_set_lineshape_mode",
-    "amp_last_call_stats", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
+    "amp_last_call_stats", "amp_last_call_timing", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
 ]
 
 
@@ -70,6 +70,7 @@ def lib():
         "amp_set_norm_mode": (i, [vp, i]),
         "amp_set_lineshape_mode": (i, [vp, i]),
         "amp_last_call_stats": (i, [vp, pi, pi, pi]),
+        "amp_last_call_timing": (i, [vp, pd]),
         "amp_last_error": (C.c_char_p, [vp]),
         "amp_status_string": (C.c_char_p, [i]),
         "amp_version": (C.c_char_p, []),
@@ -220,6 +221,12 @@ class Model:
         a, b, c = C.c_int(), C.c_int(), C.c_int()
         self._check(lib().amp_last_call_stats(self._h, C.byref(a), C.byref(b), C.byref(c)), "amp_last_call_stats")
         return {"launches": a.value, "columns_recomputed": b.value, "norm_path": c.value}
+
+
+    def last_call_timing(self):
+        ms = (C.c_double * 4)()
+        self._check(lib().amp_last_call_timing(self._h, ms), "amp_last_call_timing")
+        return {"lineshape_ms": ms[0], "data_ms": ms[1], "norm_ms": ms[2], "final_ms": ms[3]}
 
 
 def probe_fp64(kind, iters=2000, stream=None):

@@ -42,6 +42,7 @@ struct amp_model {
     std::vector<double> mw;          // [P][R][2]
     std::vector<int> colidx;         // [P][R] pool slot, -1 for CONST, -2 for inline evaluation
     int miss_streak[AMP_MAX_RESONANCES]{};
+    bool was_inline[AMP_MAX_RESONANCES]{};   // evaluated in registers by the previous call
     long long call_id = 0;
 
     int norm_mode = 0, lineshape_mode = 0;
@@ -54,6 +55,8 @@ struct amp_model {
     double* h_pinned = nullptr;    // [2 * AMP_MAX_POINTS + 2]
 
     int stat_launches = 0, stat_columns = 0, stat_norm_path = 0;
+    cudaEvent_t ev[5]{};           // phase boundaries of the last evaluation (amp_last_call_timing)
+    bool ev_valid = false;
     std::string err;
 };
 
@@ -230,6 +233,7 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
     if (e == cudaSuccess) e = cudaMalloc(&m->d_result, sizeof(double) * 2 * AMP_MAX_POINTS);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_flag, sizeof(int));
     if (e == cudaSuccess) e = cudaMallocHost(&m->h_pinned, sizeof(double) * (2 * AMP_MAX_POINTS + 2));
+    for (int i = 0; i < 5 && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ev[i]);
     if (e != cudaSuccess) { amp_model_destroy(m); return e == cudaErrorMemoryAllocation ? AMP_ERR_NOMEM : AMP_ERR_CUDA; }
     *out = m;
     return AMP_OK;
@@ -244,6 +248,7 @@ amp_status amp_model_destroy(amp_model* m) {
     if (m->d_result) cudaFree(m->d_result);
     if (m->d_flag) cudaFree(m->d_flag);
     if (m->h_pinned) cudaFreeHost(m->h_pinned);
+    for (int i = 0; i < 5; ++i) if (m->ev[i]) cudaEventDestroy(m->ev[i]);
     delete m;
     return AMP_OK;
 }
@@ -279,6 +284,17 @@ amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_r
     if (launches) *launches = m->stat_launches;
     if (columns_recomputed) *columns_recomputed = m->stat_columns;
     if (norm_path) *norm_path = m->stat_norm_path;
+    return AMP_OK;
+}
+
+amp_status amp_last_call_timing(const amp_model* m, double* ms4) {
+    if (!m || !ms4) return AMP_ERR_INVALID;
+    if (!m->ev_valid) return AMP_ERR_STATE;
+    for (int i = 0; i < 4; ++i) {
+        float t = 0;
+        if (cudaEventElapsedTime(&t, m->ev[i], m->ev[i + 1]) != cudaSuccess) return AMP_ERR_CUDA;
+        ms4[i] = t;
+    }
     return AMP_OK;
 }
 
@@ -357,8 +373,14 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
             const PoolEntry& e = m->pool[sidx];
             if (e.r == keys[k].r && e.mass == keys[k].mass && e.width == keys[k].width) { keyslot[k] = sidx; break; }
         }
-    for (size_t k = 0; k < keys.size(); ++k)
-        if (keyslot[k] < 0) res_missed[keys[k].r] = true;
+    // a miss counts towards "floating" only if the pool already holds this resonance at other values
+    // (the first, cold fill of the pool says nothing about whether the parameter floats)
+    for (size_t k = 0; k < keys.size(); ++k) {
+        if (keyslot[k] >= 0) continue;
+        bool held = m->was_inline[keys[k].r];
+        for (const PoolEntry& e : m->pool) held |= (e.r == keys[k].r);
+        if (held) res_missed[keys[k].r] = true;
+    }
     for (int r = 0; r < R; ++r) m->miss_streak[r] = res_missed[r] ? m->miss_streak[r] + 1 : 0;
     std::vector<char> inline_key(keys.size(), 0);
     int need = 0;
@@ -391,10 +413,12 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
         }
     }
     m->colidx.assign((size_t)P * R, -1);
+    for (int r = 0; r < R; ++r) m->was_inline[r] = false;
     for (int p = 0; p < P; ++p)
         for (int r = 0; r < R; ++r) {
             const int k = keyidx[(size_t)p * R + r];
             if (k >= 0) m->colidx[(size_t)p * R + r] = inline_key[k] ? -2 : keyslot[k];
+            if (k >= 0 && inline_key[k]) m->was_inline[r] = true;
         }
     return AMP_OK;
 }
@@ -481,13 +505,16 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
     amp_status st = ensure_pool(m, 0);
     if (st != AMP_OK) return st;
     CK(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
+    m->ev_valid = false;
+    CK(cudaEventRecord(m->ev[0], s));
     if (want_nll) { st = refresh_columns(m, m->data, false, s); if (st != AMP_OK) return st; }
     st = refresh_columns(m, m->norm, true, s);
     if (st != AMP_OK) return st;
+    CK(cudaEventRecord(m->ev[1], s));
     const int gd = stream_grid(m->data.n), gn = stream_grid(m->norm.n);
     StreamArgs a;
-    for (int p = 0; p < P; ++p) {
-        if (want_nll) {
+    if (want_nll)
+        for (int p = 0; p < P; ++p) {
             if (m->data.n > 0) {
                 fill_stream_args(m, m->data, p, MODE_DATA, &a);
                 a.partial = m->d_partial + (size_t)p * PARTIAL_STRIDE;
@@ -497,11 +524,14 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
                 CK(cudaMemsetAsync(m->d_partial + (size_t)p * PARTIAL_STRIDE, 0, sizeof(double), s));
             }
         }
+    CK(cudaEventRecord(m->ev[2], s));
+    for (int p = 0; p < P; ++p) {
         fill_stream_args(m, m->norm, p, MODE_NORM, &a);
         a.partial = m->d_partial + (size_t)(P + p) * PARTIAL_STRIDE;
         CK(launch_stream(a, gn, s));
         m->stat_launches++;
     }
+    CK(cudaEventRecord(m->ev[3], s));
     if (want_nll) {
         CK(launch_finalize(m->d_partial, m->data.n > 0 ? gd : 1, PARTIAL_STRIDE, P, m->d_sums, s));
         m->stat_launches++;
@@ -513,7 +543,9 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
     m->stat_launches += 2;
     CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 2 * P, cudaMemcpyDeviceToHost, s));
     CK(cudaMemcpyAsync(m->h_pinned + 2 * P, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CK(cudaEventRecord(m->ev[4], s));
     CK(cudaStreamSynchronize(s));
+    m->ev_valid = true;
     int flag;
     std::memcpy(&flag, m->h_pinned + 2 * P, sizeof(int));
     bool bad = flag != 0;
