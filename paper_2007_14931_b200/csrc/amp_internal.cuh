@@ -73,6 +73,48 @@ __device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 c) {   // 
 __device__ __forceinline__ double2 cscale(double s, double2 a) { return make_double2(s * a.x, s * a.y); }
 __device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 
+// 1/d and 1/sqrt(d) for normal positive d: hardware seed (about 20 good bits) refined to the last bits
+// of FP64 (relative error of a few 1e-16; not correctly rounded — the parity bar is 1e-11).
+__device__ __forceinline__ double fast_rcp(double d) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    double e = fma(-d, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-d, r, 1.0);
+    return fma(r, e, r);
+}
+__device__ __forceinline__ double fast_rsqrt(double d) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+    double e = fma(-d * y, y, 1.0);                 // 1 - d y^2 ~ 1e-6
+    y = fma(y * fma(0.375, e, 0.5), e, y);          // third order: error ~ e^3
+    e = fma(-d * y, y, 1.0);
+    return fma(0.5 * y, e, y);
+}
+template <int L>
+__device__ __forceinline__ double bw_poly_c(double z) {
+    if (L == 0) return 1.0;
+    if (L == 1) return 1.0 + z;
+    if (L == 2) return fma(z + 3.0, z, 9.0);
+    if (L == 3) return fma(fma(z + 6.0, z, 45.0), z, 225.0);
+    return fma(fma(fma(z + 10.0, z, 135.0), z, 1575.0), z, 11025.0);
+}
+template <int N>
+__device__ __forceinline__ double powc(double x) {
+    if (N == 0) return 1.0;
+    if (N == 1) return x;
+    const double h = powc<N / 2>(x);
+    return (N & 1) ? h * h * x : h * h;
+}
+// Per-event factors of a barrier group with compile-time orbital momenta (see BarrierGroup).
+template <int LR, int LB>
+__device__ __forceinline__ void group_factors(double r2, double invm, double pR, double pB, double* F, double* G) {
+    const double DB = bw_poly_c<LB>(r2 * pB * pB);
+    const double DR = bw_poly_c<LR>(r2 * pR * pR);
+    const double rs = (LR == 0 && LB == 0) ? 1.0 : fast_rsqrt(DR * DB);
+    *F = rs * powc<LB>(pB) * powc<LR>(pR * invm);
+    *G = powc<2 * LR + 1>(pR) * invm * (rs * rs) * DB;
+}
 // Blatt-Weisskopf polynomial B_L(z), z = (r p)^2 (ref. [35]); L is warp-uniform.
 __device__ __forceinline__ double bw_poly(int L, double z) {
     switch (L) {
@@ -129,17 +171,25 @@ cudaError_t launch_lineshape(const Dataset& d, const LineshapeJob* jobs, int njo
 
 // Streaming combine + reduce for one parameter point (a3 + a5, P = 1)
 enum StreamMode { MODE_DATA = 0, MODE_NORM = 1, MODE_EVAL = 2 };
-struct SlotRef {
-    int column;      // lineshape column in the pool, or -1: evaluate inline from `lc` (not stored)
-    int lc;          // index into StreamArgs::lc for inline evaluation
-    int c0;          // first coupling slot of this resonance
+// One resonance as the streaming kernel sees it: the three per-(mass,width) constants of LineConst,
+// its first coupling slot, and either a pool column to read or -1 = evaluate in registers.
+struct ResEntry {
+    double kN, kG, M2;
+    int c0, column;
+};
+// Resonances that share (chain, L_R, L_B, radius) share the barrier factors and momentum powers:
+//   A^R = kN F / (M2 - m^2 - i kG G),  F = rs pB^LB (pR/m)^LR,  G = pR^(2LR+1) (1/m) rs^2 B_LB(zB)
+// F and G are computed once per event and group; entries [first, first+count) belong to the group.
+struct BarrierGroup {
+    double r2;
+    int first, count;
 };
 struct StreamArgs {
-    // resonances grouped by spin: order[jstart[J] .. jstart[J+1]) are the K*/CONST of spin J; zstart.. are Zs
-    SlotRef ref[AMP_MAX_RESONANCES];
-    int jstart[6];
-    int zend;                       // order[jstart[5] .. zend) are the Z resonances
-    LineConst lc[AMP_MAX_RESONANCES];
+    ResEntry ent[AMP_MAX_RESONANCES];
+    BarrierGroup grp[AMP_MAX_RESONANCES];
+    int gstart[7];                  // groups of K* spin J: grp[gstart[J] .. gstart[J+1]), J = 0..4; Z groups: gstart[5] .. gstart[6]
+    int nconst;                     // constant (lineshape == 1) terms
+    int const_c0[4];
     double2 c[AMP_MAX_COUPLINGS];   // couplings of this point
     const double* cache;
     const double* weight;

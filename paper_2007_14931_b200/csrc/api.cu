@@ -220,7 +220,9 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
         K += (a.kind == AMP_Z || (a.kind == AMP_KSTAR && a.J >= 1)) ? 3 : 1;
         if (a.kind == AMP_Z) m->has_z = true;
     }
-    if (K > AMP_MAX_COUPLINGS) { delete m; return AMP_ERR_INVALID; }
+    int nconst = 0;
+    for (int r = 0; r < n_res; ++r) nconst += res[r].kind == AMP_CONST;
+    if (K > AMP_MAX_COUPLINGS || nconst > 4) { delete m; return AMP_ERR_INVALID; }
     m->K = K;
     for (int r = 0; r < n_res; ++r) {
         LineConst lc;
@@ -385,8 +387,9 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
     std::vector<char> inline_key(keys.size(), 0);
     int need = 0;
     for (size_t k = 0; k < keys.size(); ++k) {
-        const bool want_inline = P == 1 && keyslot[k] < 0 &&
-                                 (m->lineshape_mode == 2 || (m->lineshape_mode == 0 && m->miss_streak[keys[k].r] >= 2));
+        // P == 1: evaluating a Breit-Wigner in registers is cheaper than reading its 16 B column on B200, so
+        // unless the caller forces the pool (mode 1) no column is stored or read at all
+        const bool want_inline = P == 1 && m->lineshape_mode != 1;
         inline_key[k] = want_inline;
         if (!want_inline) ++need;
     }
@@ -449,28 +452,38 @@ amp_status refresh_columns(amp_model* m, Dataset& d, bool is_norm, cudaStream_t 
     return AMP_OK;
 }
 
-// Arguments of the streaming kernel for point p on dataset d.
+// Arguments of the streaming kernel for point p on dataset d: resonances grouped by spin, then by
+// radius (a barrier group shares its Blatt-Weisskopf factors and momentum powers).
 void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, StreamArgs* a) {
     std::memset(a, 0, sizeof(*a));
-    int t = 0, nlc = 0;
-    auto add = [&](int r) {
-        SlotRef& ref = a->ref[t++];
-        ref.c0 = m->slot0[r];
-        const int sidx = m->colidx[(size_t)p * m->R + r];
-        if (sidx >= 0) { ref.column = sidx; ref.lc = 0; return; }
-        ref.column = -1;
-        ref.lc = nlc;
-        make_line_const(m, r, m->mw[((size_t)p * m->R + r) * 2], m->mw[((size_t)p * m->R + r) * 2 + 1], &a->lc[nlc++]);
+    int t = 0, g = 0;
+    auto add_groups = [&](int kind, int J) {
+        std::vector<char> done(m->R, 0);
+        for (int r = 0; r < m->R; ++r) {
+            if (done[r] || m->res[r].kind != kind || m->res[r].J != J) continue;
+            BarrierGroup& grp = a->grp[g++];
+            grp.r2 = m->res[r].radius * m->res[r].radius;
+            grp.first = t;
+            for (int r2 = r; r2 < m->R; ++r2) {
+                if (done[r2] || m->res[r2].kind != kind || m->res[r2].J != J || m->res[r2].radius != m->res[r].radius) continue;
+                done[r2] = 1;
+                LineConst lc;
+                make_line_const(m, r2, m->mw[((size_t)p * m->R + r2) * 2], m->mw[((size_t)p * m->R + r2) * 2 + 1], &lc);
+                ResEntry& e = a->ent[t++];
+                e.kN = lc.kN; e.kG = lc.kG; e.M2 = lc.M2;
+                e.c0 = m->slot0[r2];
+                const int sidx = m->colidx[(size_t)p * m->R + r2];
+                e.column = sidx >= 0 ? sidx : -1;
+            }
+            grp.count = t - grp.first;
+        }
     };
-    for (int J = 0; J < 5; ++J) {
-        a->jstart[J] = t;
-        for (int r = 0; r < m->R; ++r)
-            if (m->res[r].kind != AMP_Z && m->res[r].J == J) add(r);
-    }
-    a->jstart[5] = t;
+    for (int J = 0; J < 5; ++J) { a->gstart[J] = g; add_groups(AMP_KSTAR, J); }
+    a->gstart[5] = g;
+    add_groups(AMP_Z, 1);
+    a->gstart[6] = g;
     for (int r = 0; r < m->R; ++r)
-        if (m->res[r].kind == AMP_Z) add(r);
-    a->zend = t;
+        if (m->res[r].kind == AMP_CONST && a->nconst < 4) a->const_c0[a->nconst++] = m->slot0[r];
     for (int k = 0; k < m->K; ++k) a->c[k] = make_double2(m->couplings[((size_t)p * m->K + k) * 2], m->couplings[((size_t)p * m->K + k) * 2 + 1]);
     a->cache = d.cache;
     a->weight = d.weight;

@@ -1,34 +1,64 @@
-// stream.cu — steps a3 + a5 (and the direct-sum form of a4) for ONE parameter point: the streaming
-// amplitude combine fused with the -log L / normalisation reduction.
+// stream.cu — steps a2 + a3 + a5 (and the direct-sum form of a4) for ONE parameter point: lineshapes,
+// streaming amplitude combine and the -log L / normalisation reduction fused in one pass over the cache.
 //
-// Per event (Eqs. 4, 5, 10, 12), with c_k the couplings and BW_R the
-// lineshape of resonance R (read from its cached column, or evaluated in registers when the column is
-// transient — every lineshape floating, cfg 3):
+// Per event (Eqs. 2-5, 10, 12), with c_k the couplings and BW_R the lineshape
+// of resonance R:
 //   K* chain   V_l   = sum_J d^J_{l0}(theta_K*) sum_{R in J} c_{R,l} BW_R          l = -1, 0, +1
 //              A_xi  = sum_l e^{i l phi} d^1_{l xi}(theta_psi) V_l
 //   Z chain    T_l'  = d^1_{0 l'}(theta_Z) e^{i l' phi~} sum_Z c_{Z,l'} BW_Z
 //              A_xi += e^{i xi alpha} sum_l' d^1_{l' xi}(theta~) T_l'
 //   S = |A_+|^2 + |A_-|^2
-// The coherent sum is grouped by spin so that the d-functions multiply a partial sum once (the dense
+// The coherent sum is grouped by spin so the d-functions multiply a partial sum once (the dense
 // contraction events x basis x couplings with its angular factors pulled out).
 //
+// Lineshapes are evaluated in registers (no HBM round trip) unless an entry points at a pool column.
+// On B200 the FP64 pipe and HBM are balanced such that recomputing a Breit-Wigner (about 14 FP64
+// instructions once the barrier factors are shared, see BarrierGroup) is cheaper than reading its 16 B
+// column, so for P = 1 the in-register form is the default.  The spin loop
+// is unrolled at compile time: L_R = J and L_B are constants inside it, so barrier polynomials and
+// momentum powers are straight-line code.
+//
 // Reduction: per-thread running sum over a grid-stride loop -> fixed xor-shuffle tree -> fixed-order sum
-// of the 8 warp values -> one partial per block; a second kernel (k_finalize) adds the block partials
-// in a fixed order.  No floating-point atomics: bitwise reproducible for a given grid size.
+// of the 8 warp values -> one partial per block; k_finalize adds the block partials in a fixed order.
+// No floating-point atomics: bitwise reproducible.
 #include "amp_internal.cuh"
 
 namespace amp {
 
-__device__ __forceinline__ double2 fetch_bw(const StreamArgs& a, const SlotRef& r, long long i, double m2, double invm, double pR,
-                                            double pB) {
-    if (r.column >= 0) return a.cols[(size_t)r.column * a.npad + i];
-    return lineshape_eval(a.lc[r.lc], m2, invm, pR, pB);
+// A^R = kN F / (M2 - m2 - i kG G)
+__device__ __forceinline__ double2 bw_from_factors(const ResEntry& e, double m2, double F, double G) {
+    const double MG = e.kG * G, dre = e.M2 - m2;
+    const double s = e.kN * F * fast_rcp(fma(dre, dre, MG * MG));
+    return make_double2(s * dre, s * MG);
+}
+
+// Partial sums U_l = sum_{R in spin-J groups} c_{R,l} BW_R for one spin (compile-time J).
+template <int J>
+__device__ __forceinline__ void spin_sum(const StreamArgs& a, long long i, double m2, double invm, double q, double pB, double2& Um,
+                                         double2& U0, double2& Up) {
+    constexpr int LB = (J == 0) ? 1 : J - 1;   // lowest allowed L_B
+    for (int g = a.gstart[J]; g < a.gstart[J + 1]; ++g) {
+        const BarrierGroup grp = a.grp[g];
+        double F, G;
+        group_factors<J, LB>(grp.r2, invm, q, pB, &F, &G);
+        for (int t = grp.first; t < grp.first + grp.count; ++t) {
+            const ResEntry& e = a.ent[t];
+            const double2 bw = (e.column >= 0) ? a.cols[(size_t)e.column * a.npad + i] : bw_from_factors(e, m2, F, G);
+            if (J == 0) {
+                U0 = cfma(a.c[e.c0], bw, U0);
+            } else {
+                Um = cfma(a.c[e.c0], bw, Um);
+                U0 = cfma(a.c[e.c0 + 1], bw, U0);
+                Up = cfma(a.c[e.c0 + 2], bw, Up);
+            }
+        }
+    }
 }
 
 template <int MODE>
-__global__ void __launch_bounds__(256, 2) k_stream(const __grid_constant__ StreamArgs a) {
+__global__ void __launch_bounds__(256, 3) k_stream(const __grid_constant__ StreamArgs a) {
     const double RSQRT2 = 0.70710678118654752440;
-    const bool have_z = a.zend > a.jstart[5];
+    const bool have_z = a.gstart[6] > a.gstart[5];
     double acc = 0.0;
     bool bad = false;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < a.n; i += (long long)gridDim.x * blockDim.x) {
@@ -37,37 +67,42 @@ __global__ void __launch_bounds__(256, 2) k_stream(const __grid_constant__ Strea
         const double cK = col[C_CK * a.npad], sK = col[C_SK * a.npad];
         const double cpsi = col[C_CPSI * a.npad], spsi = col[C_SPSI * a.npad];
         const double cphi = col[C_CPHI * a.npad], sphi = col[C_SPHI * a.npad];
-
-        // d^J_{00} = P_J(cK), d^J_{+1,0} = -sK P_J'(cK) / sqrt(J(J+1)) (d^J_{-1,0} = -d^J_{+1,0})
         const double c2 = cK * cK;
-        double d0[5], d1[5];
-        d0[0] = 1.0;                                  d1[0] = 0.0;
-        d0[1] = cK;                                   d1[1] = -RSQRT2 * sK;
-        d0[2] = fma(1.5, c2, -0.5);                   d1[2] = -1.2247448713915890491 * sK * cK;            // sqrt(3/2)
-        d0[3] = cK * fma(2.5, c2, -1.5);              d1[3] = -0.43301270189221932338 * sK * fma(5.0, c2, -1.0);   // sqrt(3)/4
-        d0[4] = fma(fma(4.375, c2, -3.75), c2, 0.375); d1[4] = -0.55901699437494742410 * sK * cK * fma(7.0, c2, -3.0);  // sqrt(5)/4
 
         double2 V0 = make_double2(0, 0), Vp = V0, Vm = V0;
-#pragma unroll
-        for (int J = 0; J < 5; ++J) {
-            double2 U0 = make_double2(0, 0), Up = U0, Um = U0;
-            for (int t = a.jstart[J]; t < a.jstart[J + 1]; ++t) {
-                const SlotRef r = a.ref[t];
-                const double2 bw = fetch_bw(a, r, i, m2, invm, q, pB);
-                if (J == 0) {
-                    U0 = cfma(a.c[r.c0], bw, U0);
-                } else {
-                    Um = cfma(a.c[r.c0], bw, Um);
-                    U0 = cfma(a.c[r.c0 + 1], bw, U0);
-                    Up = cfma(a.c[r.c0 + 2], bw, Up);
-                }
-            }
-            V0 = cadd(V0, cscale(d0[J], U0));
-            if (J) { Vp = cadd(Vp, cscale(d1[J], Up)); Vm = cadd(Vm, cscale(-d1[J], Um)); }
+        for (int t = 0; t < a.nconst; ++t) V0 = cadd(V0, a.c[a.const_c0[t]]);   // constant term: lineshape 1, d^0_00 = 1
+        // d^J_{00} = P_J(cK), d^J_{+1,0} = -sK P_J'(cK) / sqrt(J(J+1)), d^J_{-1,0} = -d^J_{+1,0}
+        {
+            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
+            spin_sum<0>(a, i, m2, invm, q, pB, Um, U0, Up);
+            V0 = cadd(V0, U0);
+        }
+        {
+            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
+            spin_sum<1>(a, i, m2, invm, q, pB, Um, U0, Up);
+            const double d1 = -RSQRT2 * sK;
+            V0 = cadd(V0, cscale(cK, U0)); Vp = cadd(Vp, cscale(d1, Up)); Vm = cadd(Vm, cscale(-d1, Um));
+        }
+        {
+            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
+            spin_sum<2>(a, i, m2, invm, q, pB, Um, U0, Up);
+            const double d1 = -1.2247448713915890491 * sK * cK;                      // sqrt(3/2)
+            V0 = cadd(V0, cscale(fma(1.5, c2, -0.5), U0)); Vp = cadd(Vp, cscale(d1, Up)); Vm = cadd(Vm, cscale(-d1, Um));
+        }
+        {
+            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
+            spin_sum<3>(a, i, m2, invm, q, pB, Um, U0, Up);
+            const double d1 = -0.43301270189221932338 * sK * fma(5.0, c2, -1.0);     // sqrt(3)/4
+            V0 = cadd(V0, cscale(cK * fma(2.5, c2, -1.5), U0)); Vp = cadd(Vp, cscale(d1, Up)); Vm = cadd(Vm, cscale(-d1, Um));
+        }
+        {
+            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
+            spin_sum<4>(a, i, m2, invm, q, pB, Um, U0, Up);
+            const double d1 = -0.55901699437494742410 * sK * cK * fma(7.0, c2, -3.0);   // sqrt(5)/4
+            V0 = cadd(V0, cscale(fma(fma(4.375, c2, -3.75), c2, 0.375), U0)); Vp = cadd(Vp, cscale(d1, Up)); Vm = cadd(Vm, cscale(-d1, Um));
         }
         // A_xi = sum_l e^{i l phi} d^1_{l xi}(theta_psi) V_l ; d^1_{0,+-1} = +-s/sqrt2, d^1_{11} = d^1_{-1-1} = (1+c)/2, d^1_{1-1} = d^1_{-11} = (1-c)/2
-        const double2 eP = make_double2(cphi, sphi), eM = make_double2(cphi, -sphi);
-        const double2 Wp = cmul(eP, Vp), Wm = cmul(eM, Vm);
+        const double2 Wp = cmul(make_double2(cphi, sphi), Vp), Wm = cmul(make_double2(cphi, -sphi), Vm);
         const double hp = 0.5 * (1.0 + cpsi), hm = 0.5 * (1.0 - cpsi), h0 = RSQRT2 * spsi;
         double2 Ap = make_double2(h0 * V0.x + hp * Wp.x + hm * Wm.x, h0 * V0.y + hp * Wp.y + hm * Wm.y);
         double2 Am = make_double2(-h0 * V0.x + hm * Wp.x + hp * Wm.x, -h0 * V0.y + hm * Wp.y + hp * Wm.y);
@@ -77,12 +112,17 @@ __global__ void __launch_bounds__(256, 2) k_stream(const __grid_constant__ Strea
             const double cZ = col[C_CZ * a.npad], sZ = col[C_SZ * a.npad], ct = col[C_CT * a.npad], st = col[C_ST * a.npad];
             const double cpt = col[C_CPT * a.npad], spt = col[C_SPT * a.npad], ca = col[C_CA * a.npad], sa = col[C_SA * a.npad];
             double2 U0 = make_double2(0, 0), Up = U0, Um = U0;
-            for (int t = a.jstart[5]; t < a.zend; ++t) {
-                const SlotRef r = a.ref[t];
-                const double2 bw = fetch_bw(a, r, i, mZ2, invmZ, qZ, pBZ);
-                Um = cfma(a.c[r.c0], bw, Um);
-                U0 = cfma(a.c[r.c0 + 1], bw, U0);
-                Up = cfma(a.c[r.c0 + 2], bw, Up);
+            for (int g = a.gstart[5]; g < a.gstart[6]; ++g) {
+                const BarrierGroup grp = a.grp[g];
+                double F, G;
+                group_factors<0, 1>(grp.r2, invmZ, qZ, pBZ, &F, &G);   // 1+ Z: L_R = 0, L_B = 1
+                for (int t = grp.first; t < grp.first + grp.count; ++t) {
+                    const ResEntry& e = a.ent[t];
+                    const double2 bw = (e.column >= 0) ? a.cols[(size_t)e.column * a.npad + i] : bw_from_factors(e, mZ2, F, G);
+                    Um = cfma(a.c[e.c0], bw, Um);
+                    U0 = cfma(a.c[e.c0 + 1], bw, U0);
+                    Up = cfma(a.c[e.c0 + 2], bw, Up);
+                }
             }
             // T_l' = d^1_{0 l'}(theta_Z) e^{i l' phi~} U_l' ; d^1_{00} = cZ, d^1_{0,+-1} = +-sZ/sqrt2
             const double z1 = RSQRT2 * sZ;
@@ -122,7 +162,7 @@ __global__ void __launch_bounds__(256, 2) k_stream(const __grid_constant__ Strea
 
 int stream_grid(long long n) {
     long long blocks = (n + 255) / 256;
-    const long long cap = 148 * 2 * 4;   // a multiple of 148 SMs x 2 resident CTAs
+    const long long cap = 148 * 3 * 4;   // a multiple of 148 SMs x 3 resident CTAs
     return (int)(blocks < 1 ? 1 : (blocks > cap ? cap : blocks));
 }
 

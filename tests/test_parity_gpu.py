@@ -167,7 +167,20 @@ def test_nll_matches_oracle_full_config(cfg):
         nll2 = Mg.nll()[0]
         ref2 = Mo.nll(c, x, eff, xn, wn, mass_width=mw[None])[0][0]
         assert abs(nll2 - ref2) < RTOL_NLL * abs(ref2)
+        assert Mg.last_call_stats()["columns_recomputed"] == 0      # P = 1: lineshapes live in registers
+        # forced column pool: the first call fills all 11 columns for both samples, a Z-only change recomputes 2
+        Mg.set_lineshape_mode(1)
+        Mg.set_params(c)
+        nll3 = Mg.nll()[0]
+        assert Mg.last_call_stats()["columns_recomputed"] == 22
+        assert abs(nll3 - nll) < 1e-12 * abs(nll)
+        Mg.set_params(c, mw[None])
+        nll4 = Mg.nll()[0]
         assert Mg.last_call_stats()["columns_recomputed"] == 2      # the Z column, data + norm
+        assert abs(nll4 - ref2) < RTOL_NLL * abs(ref2)
+        Mg.set_params(c)
+        Mg.nll()
+        assert Mg.last_call_stats()["columns_recomputed"] == 0      # both Z variants are still held
 
 
 def test_nll_batched_points_small():
