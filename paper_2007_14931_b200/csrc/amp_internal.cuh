@@ -175,7 +175,8 @@ enum StreamMode { MODE_DATA = 0, MODE_NORM = 1, MODE_EVAL = 2 };
 // its first coupling slot, and either a pool column to read or -1 = evaluate in registers.
 struct ResEntry {
     double kN, kG, M2;
-    int c0, column;
+    double2 cm, c0, cp;   // couplings of lambda = -1, 0, +1 (J = 0: only c0)
+    int column;
 };
 // Resonances that share (chain, L_R, L_B, radius) share the barrier factors and momentum powers:
 //   A^R = kN F / (M2 - m^2 - i kG G),  F = rs pB^LB (pR/m)^LR,  G = pR^(2LR+1) (1/m) rs^2 B_LB(zB)
@@ -188,9 +189,10 @@ struct StreamArgs {
     ResEntry ent[AMP_MAX_RESONANCES];
     BarrierGroup grp[AMP_MAX_RESONANCES];
     int gstart[7];                  // groups of K* spin J: grp[gstart[J] .. gstart[J+1]), J = 0..4; Z groups: gstart[5] .. gstart[6]
-    int nconst;                     // constant (lineshape == 1) terms
-    int const_c0[4];
-    double2 c[AMP_MAX_COUPLINGS];   // couplings of this point
+    int shape[6];                   // resonances per K* spin 0..4 and Z's; entries are stored in that order
+    int shape_fixed;                // 1: one radius per spin, r2_spin valid: a shape-specialised kernel may run
+    double r2_spin[6];
+    double2 cconst;                 // sum of the couplings of the constant (lineshape == 1) terms
     const double* cache;
     const double* weight;
     const double2* cols;

@@ -471,20 +471,37 @@ void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, Str
                 make_line_const(m, r2, m->mw[((size_t)p * m->R + r2) * 2], m->mw[((size_t)p * m->R + r2) * 2 + 1], &lc);
                 ResEntry& e = a->ent[t++];
                 e.kN = lc.kN; e.kG = lc.kG; e.M2 = lc.M2;
-                e.c0 = m->slot0[r2];
+                const double* cp = &m->couplings[((size_t)p * m->K + m->slot0[r2]) * 2];
+                if (J == 0 && kind == AMP_KSTAR) {
+                    e.c0 = make_double2(cp[0], cp[1]);
+                    e.cm = e.cp = make_double2(0, 0);
+                } else {
+                    e.cm = make_double2(cp[0], cp[1]); e.c0 = make_double2(cp[2], cp[3]); e.cp = make_double2(cp[4], cp[5]);
+                }
                 const int sidx = m->colidx[(size_t)p * m->R + r2];
                 e.column = sidx >= 0 ? sidx : -1;
             }
             grp.count = t - grp.first;
         }
     };
+    a->shape_fixed = 1;
     for (int J = 0; J < 5; ++J) { a->gstart[J] = g; add_groups(AMP_KSTAR, J); }
     a->gstart[5] = g;
     add_groups(AMP_Z, 1);
     a->gstart[6] = g;
+    for (int sp = 0; sp < 6; ++sp) {
+        const int ng = a->gstart[sp + 1] - a->gstart[sp];
+        a->shape[sp] = 0;
+        for (int gg = a->gstart[sp]; gg < a->gstart[sp + 1]; ++gg) a->shape[sp] += a->grp[gg].count;
+        if (ng > 1) a->shape_fixed = 0;
+        a->r2_spin[sp] = ng >= 1 ? a->grp[a->gstart[sp]].r2 : 0.0;
+    }
+    a->cconst = make_double2(0, 0);
     for (int r = 0; r < m->R; ++r)
-        if (m->res[r].kind == AMP_CONST && a->nconst < 4) a->const_c0[a->nconst++] = m->slot0[r];
-    for (int k = 0; k < m->K; ++k) a->c[k] = make_double2(m->couplings[((size_t)p * m->K + k) * 2], m->couplings[((size_t)p * m->K + k) * 2 + 1]);
+        if (m->res[r].kind == AMP_CONST) {
+            const double* cp = &m->couplings[((size_t)p * m->K + m->slot0[r]) * 2];
+            a->cconst.x += cp[0]; a->cconst.y += cp[1];
+        }
     a->cache = d.cache;
     a->weight = d.weight;
     a->cols = d.cols;

@@ -32,118 +32,169 @@ __device__ __forceinline__ double2 bw_from_factors(const ResEntry& e, double m2,
     return make_double2(s * dre, s * MG);
 }
 
-// Partial sums U_l = sum_{R in spin-J groups} c_{R,l} BW_R for one spin (compile-time J).
+// E consecutive events per thread: each cache column is read with one 16-byte (E = 2) load per thread
+// (a warp covers 512 contiguous bytes), the group / resonance constants and couplings are fetched once
+// for E events, and the E independent dependency chains give the FP64 pipe instruction-level parallelism.
+#ifndef AMP_STREAM_E
+#define AMP_STREAM_E 2
+#endif
+#ifndef AMP_STREAM_MINB
+#define AMP_STREAM_MINB 2
+#endif
+constexpr int E = AMP_STREAM_E;
+
+struct Ev {   // per-thread event registers
+    double v[E];
+};
+__device__ __forceinline__ Ev load_col(const double* __restrict__ cache, int c, long long npad, long long i0) {
+    Ev r;
+    if (E == 2) {
+        const double2 t = *reinterpret_cast<const double2*>(cache + (size_t)c * npad + i0);
+        r.v[0] = t.x; r.v[E - 1] = t.y;
+    } else {
+#pragma unroll
+        for (int e = 0; e < E; ++e) r.v[e] = cache[(size_t)c * npad + i0 + e];
+    }
+    return r;
+}
+
+// One resonance: lineshape (from its pool column or in registers) times its couplings, added to U_l.
 template <int J>
-__device__ __forceinline__ void spin_sum(const StreamArgs& a, long long i, double m2, double invm, double q, double pB, double2& Um,
-                                         double2& U0, double2& Up) {
-    constexpr int LB = (J == 0) ? 1 : J - 1;   // lowest allowed L_B
-    for (int g = a.gstart[J]; g < a.gstart[J + 1]; ++g) {
-        const BarrierGroup grp = a.grp[g];
-        double F, G;
-        group_factors<J, LB>(grp.r2, invm, q, pB, &F, &G);
-        for (int t = grp.first; t < grp.first + grp.count; ++t) {
-            const ResEntry& e = a.ent[t];
-            const double2 bw = (e.column >= 0) ? a.cols[(size_t)e.column * a.npad + i] : bw_from_factors(e, m2, F, G);
-            if (J == 0) {
-                U0 = cfma(a.c[e.c0], bw, U0);
-            } else {
-                Um = cfma(a.c[e.c0], bw, Um);
-                U0 = cfma(a.c[e.c0 + 1], bw, U0);
-                Up = cfma(a.c[e.c0 + 2], bw, Up);
-            }
+__device__ __forceinline__ void add_resonance(const StreamArgs& a, const ResEntry& en, long long i0, const Ev& m2, const double (&F)[E],
+                                              const double (&G)[E], double2 (&Um)[E], double2 (&U0)[E], double2 (&Up)[E]) {
+    double2 bw[E];
+    if (en.column >= 0) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) bw[e] = a.cols[(size_t)en.column * a.npad + i0 + e];
+    } else {
+#pragma unroll
+        for (int e = 0; e < E; ++e) bw[e] = bw_from_factors(en, m2.v[e], F[e], G[e]);
+    }
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        U0[e] = cfma(en.c0, bw[e], U0[e]);
+        if (J) { Um[e] = cfma(en.cm, bw[e], Um[e]); Up[e] = cfma(en.cp, bw[e], Up[e]); }
+    }
+}
+
+// Partial sums U_l = sum_{R of spin J} c_{R,l} BW_R.  CNT >= 0: the model has exactly CNT resonances of this
+// spin, all with one radius, stored at ent[OFF..OFF+CNT): the loop unrolls and every constant becomes an
+// immediate constant-bank operand (no index arithmetic, no constant loads).  CNT < 0: generic model, runtime
+// loops over the barrier groups [g0, g1).
+template <int J, int LRv, int LBv, int CNT, int OFF, int SPIN>
+__device__ __forceinline__ void spin_sum(const StreamArgs& a, long long i0, const Ev& m2, const Ev& invm, const Ev& pR, const Ev& pB,
+                                         double2 (&Um)[E], double2 (&U0)[E], double2 (&Up)[E]) {
+    double F[E], G[E];
+    if (CNT >= 0) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) group_factors<LRv, LBv>(a.r2_spin[SPIN], invm.v[e], pR.v[e], pB.v[e], &F[e], &G[e]);
+#pragma unroll
+        for (int t = 0; t < CNT; ++t) add_resonance<J>(a, a.ent[OFF + t], i0, m2, F, G, Um, U0, Up);
+    } else {
+        for (int g = a.gstart[SPIN]; g < a.gstart[SPIN + 1]; ++g) {
+            const BarrierGroup grp = a.grp[g];
+#pragma unroll
+            for (int e = 0; e < E; ++e) group_factors<LRv, LBv>(grp.r2, invm.v[e], pR.v[e], pB.v[e], &F[e], &G[e]);
+            for (int t = grp.first; t < grp.first + grp.count; ++t) add_resonance<J>(a, a.ent[t], i0, m2, F, G, Um, U0, Up);
         }
     }
 }
 
-template <int MODE>
-__global__ void __launch_bounds__(256, 3) k_stream(const __grid_constant__ StreamArgs a) {
+// Model shape: number of resonances of K* spin 0..4 and of Z's; Generic = runtime loops.
+template <int A0, int A1, int A2, int A3, int A4, int AZ>
+struct Shape {
+    static constexpr int n0 = A0, n1 = A1, n2 = A2, n3 = A3, n4 = A4, nz = A4 < 0 ? -1 : AZ;
+    static constexpr int o1 = A0, o2 = A0 + A1, o3 = o2 + A2, o4 = o3 + A3, oz = o4 + A4;
+};
+using Generic = Shape<-1, -1, -1, -1, -1, -1>;
+
+template <int MODE, class SH>
+__global__ void __launch_bounds__(256, AMP_STREAM_MINB) k_stream(const __grid_constant__ StreamArgs a) {
     const double RSQRT2 = 0.70710678118654752440;
-    const bool have_z = a.gstart[6] > a.gstart[5];
+    const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[6] > a.gstart[5]);
     double acc = 0.0;
     bool bad = false;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < a.n; i += (long long)gridDim.x * blockDim.x) {
-        const double* col = a.cache + i;
-        const double m2 = col[C_M2 * a.npad], invm = col[C_INVM * a.npad], q = col[C_Q * a.npad], pB = col[C_PB * a.npad];
-        const double cK = col[C_CK * a.npad], sK = col[C_SK * a.npad];
-        const double cpsi = col[C_CPSI * a.npad], spsi = col[C_SPSI * a.npad];
-        const double cphi = col[C_CPHI * a.npad], sphi = col[C_SPHI * a.npad];
-        const double c2 = cK * cK;
+    // i0 = first of the E events of this thread; npad is a multiple of 32 so i0 + E <= npad
+    for (long long i0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) * E; i0 < a.n; i0 += (long long)gridDim.x * blockDim.x * E) {
+        const Ev m2 = load_col(a.cache, C_M2, a.npad, i0), invm = load_col(a.cache, C_INVM, a.npad, i0);
+        const Ev q = load_col(a.cache, C_Q, a.npad, i0), pB = load_col(a.cache, C_PB, a.npad, i0);
+        const Ev cK = load_col(a.cache, C_CK, a.npad, i0), sK = load_col(a.cache, C_SK, a.npad, i0);
+        const Ev cpsi = load_col(a.cache, C_CPSI, a.npad, i0), spsi = load_col(a.cache, C_SPSI, a.npad, i0);
+        const Ev cphi = load_col(a.cache, C_CPHI, a.npad, i0), sphi = load_col(a.cache, C_SPHI, a.npad, i0);
 
-        double2 V0 = make_double2(0, 0), Vp = V0, Vm = V0;
-        for (int t = 0; t < a.nconst; ++t) V0 = cadd(V0, a.c[a.const_c0[t]]);   // constant term: lineshape 1, d^0_00 = 1
+        double2 V0[E], Vp[E], Vm[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) { V0[e] = a.cconst; Vp[e] = make_double2(0, 0); Vm[e] = make_double2(0, 0); }   // constant terms: lineshape 1, d^0_00 = 1
         // d^J_{00} = P_J(cK), d^J_{+1,0} = -sK P_J'(cK) / sqrt(J(J+1)), d^J_{-1,0} = -d^J_{+1,0}
-        {
-            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
-            spin_sum<0>(a, i, m2, invm, q, pB, Um, U0, Up);
-            V0 = cadd(V0, U0);
+#define AMP_SPIN(J, LB, CNT, OFF, D0, D1)                                                              \
+        if (CNT != 0 && (CNT > 0 || a.gstart[J + 1] > a.gstart[J])) {                                  \
+            double2 Um[E], U0[E], Up[E];                                                               \
+            _Pragma("unroll") for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0);  \
+            spin_sum<J, J, LB, CNT, OFF, J>(a, i0, m2, invm, q, pB, Um, U0, Up);                       \
+            _Pragma("unroll") for (int e = 0; e < E; ++e) {                                            \
+                const double c = cK.v[e], s = sK.v[e], c2 = c * c;                                     \
+                (void)s; (void)c2;                                                                     \
+                const double d0 = (D0), d1 = (D1);                                                     \
+                V0[e] = cadd(V0[e], cscale(d0, U0[e]));                                                \
+                if (J) { Vp[e] = cadd(Vp[e], cscale(d1, Up[e])); Vm[e] = cadd(Vm[e], cscale(-d1, Um[e])); } \
+            }                                                                                          \
         }
-        {
-            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
-            spin_sum<1>(a, i, m2, invm, q, pB, Um, U0, Up);
-            const double d1 = -RSQRT2 * sK;
-            V0 = cadd(V0, cscale(cK, U0)); Vp = cadd(Vp, cscale(d1, Up)); Vm = cadd(Vm, cscale(-d1, Um));
-        }
-        {
-            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
-            spin_sum<2>(a, i, m2, invm, q, pB, Um, U0, Up);
-            const double d1 = -1.2247448713915890491 * sK * cK;                      // sqrt(3/2)
-            V0 = cadd(V0, cscale(fma(1.5, c2, -0.5), U0)); Vp = cadd(Vp, cscale(d1, Up)); Vm = cadd(Vm, cscale(-d1, Um));
-        }
-        {
-            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
-            spin_sum<3>(a, i, m2, invm, q, pB, Um, U0, Up);
-            const double d1 = -0.43301270189221932338 * sK * fma(5.0, c2, -1.0);     // sqrt(3)/4
-            V0 = cadd(V0, cscale(cK * fma(2.5, c2, -1.5), U0)); Vp = cadd(Vp, cscale(d1, Up)); Vm = cadd(Vm, cscale(-d1, Um));
-        }
-        {
-            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
-            spin_sum<4>(a, i, m2, invm, q, pB, Um, U0, Up);
-            const double d1 = -0.55901699437494742410 * sK * cK * fma(7.0, c2, -3.0);   // sqrt(5)/4
-            V0 = cadd(V0, cscale(fma(fma(4.375, c2, -3.75), c2, 0.375), U0)); Vp = cadd(Vp, cscale(d1, Up)); Vm = cadd(Vm, cscale(-d1, Um));
-        }
+        AMP_SPIN(0, 1, SH::n0, 0, 1.0, 0.0)
+        AMP_SPIN(1, 0, SH::n1, SH::o1, c, -RSQRT2 * s)
+        AMP_SPIN(2, 1, SH::n2, SH::o2, fma(1.5, c2, -0.5), -1.2247448713915890491 * s * c)                                  // sqrt(3/2)
+        AMP_SPIN(3, 2, SH::n3, SH::o3, c * fma(2.5, c2, -1.5), -0.43301270189221932338 * s * fma(5.0, c2, -1.0))            // sqrt(3)/4
+        AMP_SPIN(4, 3, SH::n4, SH::o4, fma(fma(4.375, c2, -3.75), c2, 0.375), -0.55901699437494742410 * s * c * fma(7.0, c2, -3.0))   // sqrt(5)/4
+#undef AMP_SPIN
         // A_xi = sum_l e^{i l phi} d^1_{l xi}(theta_psi) V_l ; d^1_{0,+-1} = +-s/sqrt2, d^1_{11} = d^1_{-1-1} = (1+c)/2, d^1_{1-1} = d^1_{-11} = (1-c)/2
-        const double2 Wp = cmul(make_double2(cphi, sphi), Vp), Wm = cmul(make_double2(cphi, -sphi), Vm);
-        const double hp = 0.5 * (1.0 + cpsi), hm = 0.5 * (1.0 - cpsi), h0 = RSQRT2 * spsi;
-        double2 Ap = make_double2(h0 * V0.x + hp * Wp.x + hm * Wm.x, h0 * V0.y + hp * Wp.y + hm * Wm.y);
-        double2 Am = make_double2(-h0 * V0.x + hm * Wp.x + hp * Wm.x, -h0 * V0.y + hm * Wp.y + hp * Wm.y);
-
-        if (have_z) {
-            const double mZ2 = col[C_MZ2 * a.npad], invmZ = col[C_INVMZ * a.npad], qZ = col[C_QZ * a.npad], pBZ = col[C_PBZ * a.npad];
-            const double cZ = col[C_CZ * a.npad], sZ = col[C_SZ * a.npad], ct = col[C_CT * a.npad], st = col[C_ST * a.npad];
-            const double cpt = col[C_CPT * a.npad], spt = col[C_SPT * a.npad], ca = col[C_CA * a.npad], sa = col[C_SA * a.npad];
-            double2 U0 = make_double2(0, 0), Up = U0, Um = U0;
-            for (int g = a.gstart[5]; g < a.gstart[6]; ++g) {
-                const BarrierGroup grp = a.grp[g];
-                double F, G;
-                group_factors<0, 1>(grp.r2, invmZ, qZ, pBZ, &F, &G);   // 1+ Z: L_R = 0, L_B = 1
-                for (int t = grp.first; t < grp.first + grp.count; ++t) {
-                    const ResEntry& e = a.ent[t];
-                    const double2 bw = (e.column >= 0) ? a.cols[(size_t)e.column * a.npad + i] : bw_from_factors(e, mZ2, F, G);
-                    Um = cfma(a.c[e.c0], bw, Um);
-                    U0 = cfma(a.c[e.c0 + 1], bw, U0);
-                    Up = cfma(a.c[e.c0 + 2], bw, Up);
-                }
-            }
-            // T_l' = d^1_{0 l'}(theta_Z) e^{i l' phi~} U_l' ; d^1_{00} = cZ, d^1_{0,+-1} = +-sZ/sqrt2
-            const double z1 = RSQRT2 * sZ;
-            const double2 T0 = cscale(cZ, U0);
-            const double2 Tp = cscale(z1, cmul(make_double2(cpt, spt), Up));
-            const double2 Tm = cscale(-z1, cmul(make_double2(cpt, -spt), Um));
-            const double gp = 0.5 * (1.0 + ct), gm = 0.5 * (1.0 - ct), g0 = RSQRT2 * st;
-            const double2 Zp = make_double2(g0 * T0.x + gp * Tp.x + gm * Tm.x, g0 * T0.y + gp * Tp.y + gm * Tm.y);
-            const double2 Zm = make_double2(-g0 * T0.x + gm * Tp.x + gp * Tm.x, -g0 * T0.y + gm * Tp.y + gp * Tm.y);
-            Ap = cfma(make_double2(ca, sa), Zp, Ap);    // e^{+i alpha}
-            Am = cfma(make_double2(ca, -sa), Zm, Am);   // e^{-i alpha}
+        double2 Ap[E], Am[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double2 Wp = cmul(make_double2(cphi.v[e], sphi.v[e]), Vp[e]), Wm = cmul(make_double2(cphi.v[e], -sphi.v[e]), Vm[e]);
+            const double hp = 0.5 * (1.0 + cpsi.v[e]), hm = 0.5 * (1.0 - cpsi.v[e]), h0 = RSQRT2 * spsi.v[e];
+            Ap[e] = make_double2(h0 * V0[e].x + hp * Wp.x + hm * Wm.x, h0 * V0[e].y + hp * Wp.y + hm * Wm.y);
+            Am[e] = make_double2(-h0 * V0[e].x + hm * Wp.x + hp * Wm.x, -h0 * V0[e].y + hm * Wp.y + hp * Wm.y);
         }
-        const double S = fma(Ap.x, Ap.x, fma(Ap.y, Ap.y, fma(Am.x, Am.x, Am.y * Am.y)));
-        if (MODE == MODE_DATA) {
-            bad |= !(S > 0.0) || !isfinite(S);
-            acc += log(S);
-        } else if (MODE == MODE_NORM) {
-            bad |= !isfinite(S);
-            acc = fma(a.weight[i], S, acc);
-        } else {
-            a.out[i] = a.weight[i] * S;
+        if (have_z) {
+            const Ev mZ2 = load_col(a.cache, C_MZ2, a.npad, i0), invmZ = load_col(a.cache, C_INVMZ, a.npad, i0);
+            const Ev qZ = load_col(a.cache, C_QZ, a.npad, i0), pBZ = load_col(a.cache, C_PBZ, a.npad, i0);
+            double2 Um[E], U0[E], Up[E];
+#pragma unroll
+            for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0);
+            spin_sum<1, 0, 1, SH::nz, SH::oz, 5>(a, i0, mZ2, invmZ, qZ, pBZ, Um, U0, Up);   // 1+ Z: L_R = 0, L_B = 1
+            const Ev cZ = load_col(a.cache, C_CZ, a.npad, i0), sZ = load_col(a.cache, C_SZ, a.npad, i0);
+            const Ev ct = load_col(a.cache, C_CT, a.npad, i0), st = load_col(a.cache, C_ST, a.npad, i0);
+            const Ev cpt = load_col(a.cache, C_CPT, a.npad, i0), spt = load_col(a.cache, C_SPT, a.npad, i0);
+            const Ev ca = load_col(a.cache, C_CA, a.npad, i0), sa = load_col(a.cache, C_SA, a.npad, i0);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                // T_l' = d^1_{0 l'}(theta_Z) e^{i l' phi~} U_l' ; d^1_{00} = cZ, d^1_{0,+-1} = +-sZ/sqrt2
+                const double z1 = RSQRT2 * sZ.v[e];
+                const double2 T0 = cscale(cZ.v[e], U0[e]);
+                const double2 Tp = cscale(z1, cmul(make_double2(cpt.v[e], spt.v[e]), Up[e]));
+                const double2 Tm = cscale(-z1, cmul(make_double2(cpt.v[e], -spt.v[e]), Um[e]));
+                const double gp = 0.5 * (1.0 + ct.v[e]), gm = 0.5 * (1.0 - ct.v[e]), g0 = RSQRT2 * st.v[e];
+                const double2 Zp = make_double2(g0 * T0.x + gp * Tp.x + gm * Tm.x, g0 * T0.y + gp * Tp.y + gm * Tm.y);
+                const double2 Zm = make_double2(-g0 * T0.x + gm * Tp.x + gp * Tm.x, -g0 * T0.y + gm * Tp.y + gp * Tm.y);
+                Ap[e] = cfma(make_double2(ca.v[e], sa.v[e]), Zp, Ap[e]);    // e^{+i alpha}
+                Am[e] = cfma(make_double2(ca.v[e], -sa.v[e]), Zm, Am[e]);   // e^{-i alpha}
+            }
+        }
+        Ev w;
+        if (MODE != MODE_DATA) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) w.v[e] = a.weight[i0 + e];
+        }
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double S = fma(Ap[e].x, Ap[e].x, fma(Ap[e].y, Ap[e].y, fma(Am[e].x, Am[e].x, Am[e].y * Am[e].y)));
+            const bool live = i0 + e < a.n;   // the last thread may hold padding events (weight 0)
+            if (MODE == MODE_DATA) {
+                if (live) { bad |= !(S > 0.0) || !isfinite(S); acc += log(S); }
+            } else if (MODE == MODE_NORM) {
+                if (live) { bad |= !isfinite(S); acc = fma(w.v[e], S, acc); }
+            } else {
+                if (live) a.out[i0 + e] = w.v[e] * S;
+            }
         }
     }
     if (MODE == MODE_EVAL) return;
@@ -161,17 +212,32 @@ __global__ void __launch_bounds__(256, 3) k_stream(const __grid_constant__ Strea
 }
 
 int stream_grid(long long n) {
-    long long blocks = (n + 255) / 256;
-    const long long cap = 148 * 3 * 4;   // a multiple of 148 SMs x 3 resident CTAs
+    long long blocks = (n + 256 * E - 1) / (256 * E);
+    const long long cap = 148 * AMP_STREAM_MINB * 4;   // a multiple of 148 SMs x resident CTAs
     return (int)(blocks < 1 ? 1 : (blocks > cap ? cap : blocks));
 }
 
-cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s) {
+template <class SH>
+static void launch_shape(const StreamArgs& a, int grid, cudaStream_t s) {
     switch (a.mode) {
-        case MODE_DATA: k_stream<MODE_DATA><<<grid, 256, 0, s>>>(a); break;
-        case MODE_NORM: k_stream<MODE_NORM><<<grid, 256, 0, s>>>(a); break;
-        default: k_stream<MODE_EVAL><<<grid, 256, 0, s>>>(a); break;
+        case MODE_DATA: k_stream<MODE_DATA, SH><<<grid, 256, 0, s>>>(a); break;
+        case MODE_NORM: k_stream<MODE_NORM, SH><<<grid, 256, 0, s>>>(a); break;
+        default: k_stream<MODE_EVAL, SH><<<grid, 256, 0, s>>>(a); break;
     }
+}
+
+// Shapes with a fully unrolled kernel: the paper's ten K* (three J = 0, three J = 1, two J = 2, one J = 3, one
+// J = 4) with and without one Z, and the single K*(892) of configs[0].  Any other resonance list
+// (or different radii within one spin) runs the generic kernel.
+cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s) {
+    const int* n = a.shape;
+    auto is = [&](int a0, int a1, int a2, int a3, int a4, int az) {
+        return a.shape_fixed && n[0] == a0 && n[1] == a1 && n[2] == a2 && n[3] == a3 && n[4] == a4 && n[5] == az;
+    };
+    if (is(3, 3, 2, 1, 1, 1)) launch_shape<Shape<3, 3, 2, 1, 1, 1>>(a, grid, s);
+    else if (is(3, 3, 2, 1, 1, 0)) launch_shape<Shape<3, 3, 2, 1, 1, 0>>(a, grid, s);
+    else if (is(0, 1, 0, 0, 0, 0)) launch_shape<Shape<0, 1, 0, 0, 0, 0>>(a, grid, s);
+    else launch_shape<Generic>(a, grid, s);
     return cudaGetLastError();
 }
 
