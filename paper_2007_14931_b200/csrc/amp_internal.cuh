@@ -2,7 +2,7 @@
 //
 // Data layout in HBM:
 //   kinematics cache  double[NCOL][npad]   structure-of-arrays, one column per cached quantity,
-//                                          npad = n rounded up to a multiple of 32 events
+//                                          npad = n rounded up to whole pipeline tiles (stream_pad)
 //   lineshape columns double2[ncol][npad]  complex A^R(m_i) (re, im) interleaved: one 128-bit load
 //                                          per (event, column)
 // One thread owns one event at a time; a warp reads 32 consecutive doubles (256 B) of a cache
@@ -203,7 +203,8 @@ struct StreamArgs {
     int mode;
 };
 cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s);
-int stream_grid(long long n);
+int stream_grid(long long n, bool have_z, int mode);
+long long stream_pad(long long n);   // events per column rounded up to whole pipeline tiles
 
 // fixed-order final reduction of per-block partials: out[j] = sum_b partial[j][b], j < nrows
 cudaError_t launch_finalize(const double* partial, int nblocks, int stride, int nrows, double* out, cudaStream_t s);

@@ -136,7 +136,7 @@ amp_status load_dataset(amp_model* m, Dataset& d, bool is_norm, const double* d_
     free_dataset(d);
     for (auto& e : m->pool) (is_norm ? e.valid_norm : e.valid_data) = false;
     d.n = n;
-    d.npad = pad32(n > 0 ? n : 1);
+    d.npad = stream_pad(n > 0 ? n : 1);
     d.ncache = m->has_z ? NCOL_ALL : NCOL_K;
     CK(cudaMalloc(&d.cache, sizeof(double) * d.ncache * d.npad));
     CK(cudaMalloc(&d.weight, sizeof(double) * d.npad));
@@ -541,7 +541,7 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
     st = refresh_columns(m, m->norm, true, s);
     if (st != AMP_OK) return st;
     CK(cudaEventRecord(m->ev[1], s));
-    const int gd = stream_grid(m->data.n), gn = stream_grid(m->norm.n);
+    const int gd = stream_grid(m->data.n, m->has_z, MODE_DATA), gn = stream_grid(m->norm.n, m->has_z, MODE_NORM);
     StreamArgs a;
     if (want_nll)
         for (int p = 0; p < P; ++p) {
@@ -618,7 +618,7 @@ amp_status amp_eval_events(amp_model* m, int p, double* d_out, void* stream) {
     StreamArgs a;
     fill_stream_args(m, m->data, p, MODE_EVAL, &a);
     a.out = d_out;
-    CK(launch_stream(a, stream_grid(m->data.n), s));
+    CK(launch_stream(a, stream_grid(m->data.n, m->has_z, MODE_EVAL), s));
     m->stat_launches++;
     CK(cudaStreamSynchronize(s));
     return AMP_OK;

@@ -43,19 +43,59 @@ __device__ __forceinline__ double2 bw_from_factors(const ResEntry& e, double m2,
 #endif
 constexpr int E = AMP_STREAM_E;
 
+constexpr int THREADS = 256;
+constexpr int TILE = THREADS * E;          // events per pipeline stage
+constexpr int NSTAGE = 2;
+
 struct Ev {   // per-thread event registers
     double v[E];
 };
-__device__ __forceinline__ Ev load_col(const double* __restrict__ cache, int c, long long npad, long long i0) {
+// The E events of this thread from column c of a staged tile (shared memory, [column][TILE] doubles):
+// consecutive threads read consecutive 16-byte words — conflict-free.
+__device__ __forceinline__ Ev load_col(const double* __restrict__ stage, int c) {
     Ev r;
+    const double* p = stage + c * TILE + threadIdx.x * E;
     if (E == 2) {
-        const double2 t = *reinterpret_cast<const double2*>(cache + (size_t)c * npad + i0);
+        const double2 t = *reinterpret_cast<const double2*>(p);
         r.v[0] = t.x; r.v[E - 1] = t.y;
     } else {
 #pragma unroll
-        for (int e = 0; e < E; ++e) r.v[e] = cache[(size_t)c * npad + i0 + e];
+        for (int e = 0; e < E; ++e) r.v[e] = p[e];
     }
     return r;
+}
+
+// ---- TMA bulk-copy pipeline (cp.async.bulk + mbarrier): one elected thread streams whole cache columns of the
+// next tile into shared memory while all warps compute on the current one, so no register holds data in flight.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
+                 "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+// columns of tile `tile` -> stage: ncache cache columns, then (if with_w) the weight column
+__device__ __forceinline__ void issue_tile(const StreamArgs& a, long long tile, double* stage, uint64_t* bar, int ncache, bool with_w) {
+    const uint32_t col_bytes = TILE * sizeof(double);
+    mbar_expect_tx(bar, col_bytes * (ncache + (with_w ? 1 : 0)));
+    for (int c = 0; c < ncache; ++c) bulk_g2s(stage + c * TILE, a.cache + (size_t)c * a.npad + tile * TILE, col_bytes, bar);
+    if (with_w) bulk_g2s(stage + ncache * TILE, a.weight + tile * TILE, col_bytes, bar);
 }
 
 // One resonance: lineshape (from its pool column or in registers) times its couplings, added to U_l.
@@ -109,18 +149,38 @@ struct Shape {
 using Generic = Shape<-1, -1, -1, -1, -1, -1>;
 
 template <int MODE, class SH>
-__global__ void __launch_bounds__(256, AMP_STREAM_MINB) k_stream(const __grid_constant__ StreamArgs a) {
+__global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __grid_constant__ StreamArgs a) {
     const double RSQRT2 = 0.70710678118654752440;
     const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[6] > a.gstart[5]);
     double acc = 0.0;
     bool bad = false;
-    // i0 = first of the E events of this thread; npad is a multiple of 32 so i0 + E <= npad
-    for (long long i0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) * E; i0 < a.n; i0 += (long long)gridDim.x * blockDim.x * E) {
-        const Ev m2 = load_col(a.cache, C_M2, a.npad, i0), invm = load_col(a.cache, C_INVM, a.npad, i0);
-        const Ev q = load_col(a.cache, C_Q, a.npad, i0), pB = load_col(a.cache, C_PB, a.npad, i0);
-        const Ev cK = load_col(a.cache, C_CK, a.npad, i0), sK = load_col(a.cache, C_SK, a.npad, i0);
-        const Ev cpsi = load_col(a.cache, C_CPSI, a.npad, i0), spsi = load_col(a.cache, C_SPSI, a.npad, i0);
-        const Ev cphi = load_col(a.cache, C_CPHI, a.npad, i0), sphi = load_col(a.cache, C_SPHI, a.npad, i0);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int ncache = have_z ? NCOL_ALL : NCOL_K;
+    const bool with_w = MODE != MODE_DATA;
+    const int stage_doubles = (ncache + (with_w ? 1 : 0)) * TILE;
+    double* stages = reinterpret_cast<double*>(smem_raw);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NSTAGE * stage_doubles * sizeof(double));
+    if (threadIdx.x == 0) {
+        for (int st = 0; st < NSTAGE; ++st) mbar_init(&full[st], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const long long ntiles = (a.n + TILE - 1) / TILE;   // npad is a multiple of TILE: every tile is fully backed by memory
+    if (threadIdx.x == 0 && (long long)blockIdx.x < ntiles) issue_tile(a, blockIdx.x, stages, &full[0], ncache, with_w);
+    int k = 0;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++k) {
+        const int st_cur = k % NSTAGE;
+        const double* stage = stages + (size_t)st_cur * stage_doubles;
+        // prefetch the next tile of this CTA into the other stage (freed by the __syncthreads that ended iteration k-1)
+        if (threadIdx.x == 0 && tile + gridDim.x < ntiles)
+            issue_tile(a, tile + gridDim.x, stages + (size_t)((k + 1) % NSTAGE) * stage_doubles, &full[(k + 1) % NSTAGE], ncache, with_w);
+        mbar_wait(&full[st_cur], (k / NSTAGE) & 1);
+        const long long i0 = tile * TILE + threadIdx.x * E;   // first of the E events of this thread
+        const Ev m2 = load_col(stage, C_M2), invm = load_col(stage, C_INVM);
+        const Ev q = load_col(stage, C_Q), pB = load_col(stage, C_PB);
+        const Ev cK = load_col(stage, C_CK), sK = load_col(stage, C_SK);
+        const Ev cpsi = load_col(stage, C_CPSI), spsi = load_col(stage, C_SPSI);
+        const Ev cphi = load_col(stage, C_CPHI), sphi = load_col(stage, C_SPHI);
 
         double2 V0[E], Vp[E], Vm[E];
 #pragma unroll
@@ -155,16 +215,16 @@ __global__ void __launch_bounds__(256, AMP_STREAM_MINB) k_stream(const __grid_co
             Am[e] = make_double2(-h0 * V0[e].x + hm * Wp.x + hp * Wm.x, -h0 * V0[e].y + hm * Wp.y + hp * Wm.y);
         }
         if (have_z) {
-            const Ev mZ2 = load_col(a.cache, C_MZ2, a.npad, i0), invmZ = load_col(a.cache, C_INVMZ, a.npad, i0);
-            const Ev qZ = load_col(a.cache, C_QZ, a.npad, i0), pBZ = load_col(a.cache, C_PBZ, a.npad, i0);
+            const Ev mZ2 = load_col(stage, C_MZ2), invmZ = load_col(stage, C_INVMZ);
+            const Ev qZ = load_col(stage, C_QZ), pBZ = load_col(stage, C_PBZ);
             double2 Um[E], U0[E], Up[E];
 #pragma unroll
             for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0);
             spin_sum<1, 0, 1, SH::nz, SH::oz, 5>(a, i0, mZ2, invmZ, qZ, pBZ, Um, U0, Up);   // 1+ Z: L_R = 0, L_B = 1
-            const Ev cZ = load_col(a.cache, C_CZ, a.npad, i0), sZ = load_col(a.cache, C_SZ, a.npad, i0);
-            const Ev ct = load_col(a.cache, C_CT, a.npad, i0), st = load_col(a.cache, C_ST, a.npad, i0);
-            const Ev cpt = load_col(a.cache, C_CPT, a.npad, i0), spt = load_col(a.cache, C_SPT, a.npad, i0);
-            const Ev ca = load_col(a.cache, C_CA, a.npad, i0), sa = load_col(a.cache, C_SA, a.npad, i0);
+            const Ev cZ = load_col(stage, C_CZ), sZ = load_col(stage, C_SZ);
+            const Ev ct = load_col(stage, C_CT), st = load_col(stage, C_ST);
+            const Ev cpt = load_col(stage, C_CPT), spt = load_col(stage, C_SPT);
+            const Ev ca = load_col(stage, C_CA), sa = load_col(stage, C_SA);
 #pragma unroll
             for (int e = 0; e < E; ++e) {
                 // T_l' = d^1_{0 l'}(theta_Z) e^{i l' phi~} U_l' ; d^1_{00} = cZ, d^1_{0,+-1} = +-sZ/sqrt2
@@ -180,10 +240,7 @@ __global__ void __launch_bounds__(256, AMP_STREAM_MINB) k_stream(const __grid_co
             }
         }
         Ev w;
-        if (MODE != MODE_DATA) {
-#pragma unroll
-            for (int e = 0; e < E; ++e) w.v[e] = a.weight[i0 + e];
-        }
+        if (MODE != MODE_DATA) w = load_col(stage, ncache);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const double S = fma(Ap[e].x, Ap[e].x, fma(Ap[e].y, Ap[e].y, fma(Am[e].x, Am[e].x, Am[e].y * Am[e].y)));
@@ -196,6 +253,7 @@ __global__ void __launch_bounds__(256, AMP_STREAM_MINB) k_stream(const __grid_co
                 if (live) a.out[i0 + e] = w.v[e] * S;
             }
         }
+        __syncthreads();   // every thread is done with this stage: it may be refilled in the next iteration
     }
     if (MODE == MODE_EVAL) return;
     if (bad) atomicOr(a.flag, 2);
@@ -211,19 +269,42 @@ __global__ void __launch_bounds__(256, AMP_STREAM_MINB) k_stream(const __grid_co
     }
 }
 
-int stream_grid(long long n) {
-    long long blocks = (n + 256 * E - 1) / (256 * E);
-    const long long cap = 148 * AMP_STREAM_MINB * 4;   // a multiple of 148 SMs x resident CTAs
-    return (int)(blocks < 1 ? 1 : (blocks > cap ? cap : blocks));
+static size_t stream_smem(bool have_z, int mode) {
+    const int ncols = (have_z ? NCOL_ALL : NCOL_K) + (mode != MODE_DATA ? 1 : 0);
+    return (size_t)NSTAGE * ncols * TILE * sizeof(double) + NSTAGE * sizeof(uint64_t);
 }
 
+// persistent grid: one CTA per resident slot (as many CTAs per SM as the staged tiles leave room for, at most
+// AMP_STREAM_MINB), never more than there are tiles
+int stream_grid(long long n, bool have_z, int mode) {
+    const long long ntiles = (n + TILE - 1) / TILE;
+    long long per_sm = (long long)((224 * 1024) / (stream_smem(have_z, mode) + 1024));
+    if (per_sm > AMP_STREAM_MINB) per_sm = AMP_STREAM_MINB;
+    if (per_sm < 1) per_sm = 1;
+    const long long cap = 148 * per_sm;
+    return (int)(ntiles < 1 ? 1 : (ntiles > cap ? cap : ntiles));
+}
+
+long long stream_pad(long long n) { return (n + TILE - 1) / TILE * TILE; }
+
 template <class SH>
-static void launch_shape(const StreamArgs& a, int grid, cudaStream_t s) {
-    switch (a.mode) {
-        case MODE_DATA: k_stream<MODE_DATA, SH><<<grid, 256, 0, s>>>(a); break;
-        case MODE_NORM: k_stream<MODE_NORM, SH><<<grid, 256, 0, s>>>(a); break;
-        default: k_stream<MODE_EVAL, SH><<<grid, 256, 0, s>>>(a); break;
+static cudaError_t launch_shape(const StreamArgs& a, int grid, cudaStream_t s) {
+    const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[6] > a.gstart[5]);
+    const size_t smem = stream_smem(have_z, a.mode);
+    cudaError_t e = cudaSuccess;
+#define AMP_LAUNCH(M)                                                                                              \
+    {                                                                                                              \
+        static bool attr_done = false;                                                                             \
+        if (!attr_done) { e = cudaFuncSetAttribute(k_stream<M, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; } \
+        if (e == cudaSuccess) k_stream<M, SH><<<grid, THREADS, smem, s>>>(a);                                      \
     }
+    switch (a.mode) {
+        case MODE_DATA: AMP_LAUNCH(MODE_DATA) break;
+        case MODE_NORM: AMP_LAUNCH(MODE_NORM) break;
+        default: AMP_LAUNCH(MODE_EVAL) break;
+    }
+#undef AMP_LAUNCH
+    return e;
 }
 
 // Shapes with a fully unrolled kernel: the paper's ten K* (three J = 0, three J = 1, two J = 2, one J = 3, one
@@ -234,11 +315,12 @@ cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s) {
     auto is = [&](int a0, int a1, int a2, int a3, int a4, int az) {
         return a.shape_fixed && n[0] == a0 && n[1] == a1 && n[2] == a2 && n[3] == a3 && n[4] == a4 && n[5] == az;
     };
-    if (is(3, 3, 2, 1, 1, 1)) launch_shape<Shape<3, 3, 2, 1, 1, 1>>(a, grid, s);
-    else if (is(3, 3, 2, 1, 1, 0)) launch_shape<Shape<3, 3, 2, 1, 1, 0>>(a, grid, s);
-    else if (is(0, 1, 0, 0, 0, 0)) launch_shape<Shape<0, 1, 0, 0, 0, 0>>(a, grid, s);
-    else launch_shape<Generic>(a, grid, s);
-    return cudaGetLastError();
+    cudaError_t e;
+    if (is(3, 3, 2, 1, 1, 1)) e = launch_shape<Shape<3, 3, 2, 1, 1, 1>>(a, grid, s);
+    else if (is(3, 3, 2, 1, 1, 0)) e = launch_shape<Shape<3, 3, 2, 1, 1, 0>>(a, grid, s);
+    else if (is(0, 1, 0, 0, 0, 0)) e = launch_shape<Shape<0, 1, 0, 0, 0, 0>>(a, grid, s);
+    else e = launch_shape<Generic>(a, grid, s);
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 }  // namespace amp
