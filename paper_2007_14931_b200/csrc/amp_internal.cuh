@@ -73,23 +73,20 @@ __device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 c) {   // 
 __device__ __forceinline__ double2 cscale(double s, double2 a) { return make_double2(s * a.x, s * a.y); }
 __device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 
-// 1/d and 1/sqrt(d) for normal positive d: hardware seed (about 20 good bits) refined to the last bits
-// of FP64 (relative error of a few 1e-16; not correctly rounded — the parity bar is 1e-11).
+// 1/d and 1/sqrt(d) for normal positive d: hardware seed (MUFU.RCP64H / RSQ64H, about 20 good bits) followed by
+// one third-order correction, error ~ seed_error^3 ~ 1e-18 before rounding: a few 1e-16 relative in the end
+// (not correctly rounded — the parity bar is 1e-11).
 __device__ __forceinline__ double fast_rcp(double d) {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
-    double e = fma(-d, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-d, r, 1.0);
-    return fma(r, e, r);
+    const double e = fma(-d, r, 1.0);               // 1 - d r ~ 1e-6
+    return fma(r, fma(e, e, e), r);                 // r (1 + e + e^2)
 }
 __device__ __forceinline__ double fast_rsqrt(double d) {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
-    double e = fma(-d * y, y, 1.0);                 // 1 - d y^2 ~ 1e-6
-    y = fma(y * fma(0.375, e, 0.5), e, y);          // third order: error ~ e^3
-    e = fma(-d * y, y, 1.0);
-    return fma(0.5 * y, e, y);
+    const double e = fma(-d * y, y, 1.0);           // 1 - d y^2 ~ 1e-6
+    return fma(y * fma(0.375, e, 0.5), e, y);       // y (1 + e/2 + 3 e^2 / 8)
 }
 template <int L>
 __device__ __forceinline__ double bw_poly_c(double z) {

@@ -45,7 +45,6 @@ constexpr int E = AMP_STREAM_E;
 
 constexpr int THREADS = 256;
 constexpr int TILE = THREADS * E;          // events per pipeline stage
-constexpr int NSTAGE = 2;
 
 struct Ev {   // per-thread event registers
     double v[E];
@@ -90,12 +89,14 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
-// columns of tile `tile` -> stage: ncache cache columns, then (if with_w) the weight column
-__device__ __forceinline__ void issue_tile(const StreamArgs& a, long long tile, double* stage, uint64_t* bar, int ncache, bool with_w) {
+// Columns [c0, c1) of the cache (and, if with_w, the weight column into slot wslot) of tile `tile` -> stage.
+__device__ __forceinline__ void issue_cols(const StreamArgs& a, long long tile, double* stage, uint64_t* bar, int c0, int c1, bool with_w,
+                                           int wslot) {
     const uint32_t col_bytes = TILE * sizeof(double);
-    mbar_expect_tx(bar, col_bytes * (ncache + (with_w ? 1 : 0)));
-    for (int c = 0; c < ncache; ++c) bulk_g2s(stage + c * TILE, a.cache + (size_t)c * a.npad + tile * TILE, col_bytes, bar);
-    if (with_w) bulk_g2s(stage + ncache * TILE, a.weight + tile * TILE, col_bytes, bar);
+    mbar_expect_tx(bar, col_bytes * (c1 - c0 + (with_w ? 1 : 0)));
+#pragma unroll 1
+    for (int c = c0; c < c1; ++c) bulk_g2s(stage + c * TILE, a.cache + (size_t)c * a.npad + tile * TILE, col_bytes, bar);
+    if (with_w) bulk_g2s(stage + wslot * TILE, a.weight + tile * TILE, col_bytes, bar);
 }
 
 // One resonance: lineshape (from its pool column or in registers) times its couplings, added to U_l.
@@ -154,33 +155,40 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[6] > a.gstart[5]);
     double acc = 0.0;
     bool bad = false;
+    // One staged tile per CTA, split in two regions with their own mbarrier: the K*-chain columns (+ weight) are
+    // copied to registers at the top of an iteration and their region is refilled at once with the next tile;
+    // the Z-chain region is refilled as soon as its values have been read, a little past the middle.  A region
+    // therefore has a whole iteration to arrive, and two CTAs (16 warps) fit on an SM.
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int ncache = have_z ? NCOL_ALL : NCOL_K;
     const bool with_w = MODE != MODE_DATA;
-    const int stage_doubles = (ncache + (with_w ? 1 : 0)) * TILE;
-    double* stages = reinterpret_cast<double*>(smem_raw);
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NSTAGE * stage_doubles * sizeof(double));
+    double* stage = reinterpret_cast<double*>(smem_raw);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)(ncache + 1) * TILE * sizeof(double));   // [0]: K* region, [1]: Z region
     if (threadIdx.x == 0) {
-        for (int st = 0; st < NSTAGE; ++st) mbar_init(&full[st], 1);
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     const long long ntiles = (a.n + TILE - 1) / TILE;   // npad is a multiple of TILE: every tile is fully backed by memory
-    if (threadIdx.x == 0 && (long long)blockIdx.x < ntiles) issue_tile(a, blockIdx.x, stages, &full[0], ncache, with_w);
-    int k = 0;
-    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++k) {
-        const int st_cur = k % NSTAGE;
-        const double* stage = stages + (size_t)st_cur * stage_doubles;
-        // prefetch the next tile of this CTA into the other stage (freed by the __syncthreads that ended iteration k-1)
-        if (threadIdx.x == 0 && tile + gridDim.x < ntiles)
-            issue_tile(a, tile + gridDim.x, stages + (size_t)((k + 1) % NSTAGE) * stage_doubles, &full[(k + 1) % NSTAGE], ncache, with_w);
-        mbar_wait(&full[st_cur], (k / NSTAGE) & 1);
+    if (threadIdx.x == 0 && (long long)blockIdx.x < ntiles) {
+        issue_cols(a, blockIdx.x, stage, &full[0], 0, NCOL_K, with_w, ncache);
+        if (have_z) issue_cols(a, blockIdx.x, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
+    }
+    uint32_t parity = 0;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, parity ^= 1) {
+        const bool has_next = tile + gridDim.x < ntiles;
         const long long i0 = tile * TILE + threadIdx.x * E;   // first of the E events of this thread
+        mbar_wait(&full[0], parity);
         const Ev m2 = load_col(stage, C_M2), invm = load_col(stage, C_INVM);
         const Ev q = load_col(stage, C_Q), pB = load_col(stage, C_PB);
         const Ev cK = load_col(stage, C_CK), sK = load_col(stage, C_SK);
         const Ev cpsi = load_col(stage, C_CPSI), spsi = load_col(stage, C_SPSI);
         const Ev cphi = load_col(stage, C_CPHI), sphi = load_col(stage, C_SPHI);
+        Ev w;
+        if (with_w) w = load_col(stage, ncache);
+        __syncthreads();   // K* region consumed by every thread: stream the next tile into it
+        if (threadIdx.x == 0 && has_next) issue_cols(a, tile + gridDim.x, stage, &full[0], 0, NCOL_K, with_w, ncache);
 
         double2 V0[E], Vp[E], Vm[E];
 #pragma unroll
@@ -215,16 +223,19 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
             Am[e] = make_double2(-h0 * V0[e].x + hm * Wp.x + hp * Wm.x, -h0 * V0[e].y + hm * Wp.y + hp * Wm.y);
         }
         if (have_z) {
+            mbar_wait(&full[1], parity);
             const Ev mZ2 = load_col(stage, C_MZ2), invmZ = load_col(stage, C_INVMZ);
             const Ev qZ = load_col(stage, C_QZ), pBZ = load_col(stage, C_PBZ);
-            double2 Um[E], U0[E], Up[E];
-#pragma unroll
-            for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0);
-            spin_sum<1, 0, 1, SH::nz, SH::oz, 5>(a, i0, mZ2, invmZ, qZ, pBZ, Um, U0, Up);   // 1+ Z: L_R = 0, L_B = 1
             const Ev cZ = load_col(stage, C_CZ), sZ = load_col(stage, C_SZ);
             const Ev ct = load_col(stage, C_CT), st = load_col(stage, C_ST);
             const Ev cpt = load_col(stage, C_CPT), spt = load_col(stage, C_SPT);
             const Ev ca = load_col(stage, C_CA), sa = load_col(stage, C_SA);
+            __syncthreads();   // Z region consumed: refill it with the next tile
+            if (threadIdx.x == 0 && has_next) issue_cols(a, tile + gridDim.x, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
+            double2 Um[E], U0[E], Up[E];
+#pragma unroll
+            for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0);
+            spin_sum<1, 0, 1, SH::nz, SH::oz, 5>(a, i0, mZ2, invmZ, qZ, pBZ, Um, U0, Up);   // 1+ Z: L_R = 0, L_B = 1
 #pragma unroll
             for (int e = 0; e < E; ++e) {
                 // T_l' = d^1_{0 l'}(theta_Z) e^{i l' phi~} U_l' ; d^1_{00} = cZ, d^1_{0,+-1} = +-sZ/sqrt2
@@ -239,8 +250,6 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
                 Am[e] = cfma(make_double2(ca.v[e], -sa.v[e]), Zm, Am[e]);   // e^{-i alpha}
             }
         }
-        Ev w;
-        if (MODE != MODE_DATA) w = load_col(stage, ncache);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const double S = fma(Ap[e].x, Ap[e].x, fma(Ap[e].y, Ap[e].y, fma(Am[e].x, Am[e].x, Am[e].y * Am[e].y)));
@@ -253,7 +262,6 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
                 if (live) a.out[i0 + e] = w.v[e] * S;
             }
         }
-        __syncthreads();   // every thread is done with this stage: it may be refilled in the next iteration
     }
     if (MODE == MODE_EVAL) return;
     if (bad) atomicOr(a.flag, 2);
@@ -270,8 +278,8 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
 }
 
 static size_t stream_smem(bool have_z, int mode) {
-    const int ncols = (have_z ? NCOL_ALL : NCOL_K) + (mode != MODE_DATA ? 1 : 0);
-    return (size_t)NSTAGE * ncols * TILE * sizeof(double) + NSTAGE * sizeof(uint64_t);
+    (void)mode;
+    return (size_t)((have_z ? NCOL_ALL : NCOL_K) + 1) * TILE * sizeof(double) + 2 * sizeof(uint64_t);
 }
 
 // persistent grid: one CTA per resident slot (as many CTAs per SM as the staged tiles leave room for, at most
