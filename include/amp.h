@@ -134,8 +134,12 @@ amp_status amp_set_norm_mode(amp_model* m, int mode);
  * on two successive calls is floating: evaluate it in registers inside the combine kernel, no HBM round
  * trip), 1 = always store columns in the pool, 2 = always evaluate missing columns in registers.        */
 amp_status amp_set_lineshape_mode(amp_model* m, int mode);
+/* How P > 1 points are evaluated: 0 = automatic (one batched DMMA launch per sample when P >= 24, the model has at
+ * most 28 couplings and the extended basis fits in shared memory, else as mode 1), 1 = a loop of single-point
+ * streaming launches over the stored lineshape columns.                                                  */
+amp_status amp_set_batch_mode(amp_model* m, int mode);
 /* Counters of the last amp_nll / amp_norm_integral call: kernels launched, lineshape columns
- * recomputed (data + norm), which normalisation path ran (1 direct, 2 matrix).                         */
+ * recomputed (data + norm), which normalisation path ran (1 direct streaming sum, 2 matrix, 3 batched DMMA sum).                         */
 amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_recomputed, int* norm_path);
 
 /* Device time [ms] of the phases of the last amp_nll / amp_norm_integral call, from CUDA events recorded on

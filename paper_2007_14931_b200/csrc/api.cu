@@ -54,7 +54,13 @@ struct amp_model {
     int* d_flag = nullptr;
     double* h_pinned = nullptr;    // [2 * AMP_MAX_POINTS + 2]
 
-    int stat_launches = 0, stat_columns = 0, stat_norm_path = 0;
+    // batched (P > 1) plan buffers: coefficient fragments, basis entries, sparse items
+    unsigned char* d_plan = nullptr;
+    unsigned char* h_plan = nullptr;   // pinned
+    size_t plan_cap = 0;
+    int batch_mode = 0;            // 0 auto (DMMA kernel when eligible), 1 never (loop of single-point kernels)
+
+    int stat_launches = 0, stat_columns = 0, stat_norm_path = 0, stat_batched = 0;
     cudaEvent_t ev[5]{};           // phase boundaries of the last evaluation (amp_last_call_timing)
     bool ev_valid = false;
     std::string err;
@@ -250,6 +256,8 @@ amp_status amp_model_destroy(amp_model* m) {
     if (m->d_result) cudaFree(m->d_result);
     if (m->d_flag) cudaFree(m->d_flag);
     if (m->h_pinned) cudaFreeHost(m->h_pinned);
+    if (m->d_plan) cudaFree(m->d_plan);
+    if (m->h_plan) cudaFreeHost(m->h_plan);
     for (int i = 0; i < 5; ++i) if (m->ev[i]) cudaEventDestroy(m->ev[i]);
     delete m;
     return AMP_OK;
@@ -272,6 +280,12 @@ amp_status amp_load_norm(amp_model* m, const double* d_x, const double* d_w, lon
 amp_status amp_set_norm_mode(amp_model* m, int mode) {
     if (!m || mode < 0 || mode > 2) return AMP_ERR_INVALID;
     m->norm_mode = mode;
+    return AMP_OK;
+}
+
+amp_status amp_set_batch_mode(amp_model* m, int mode) {
+    if (!m || mode < 0 || mode > 1) return AMP_ERR_INVALID;
+    m->batch_mode = mode;
     return AMP_OK;
 }
 
@@ -525,6 +539,124 @@ __global__ void k_nll_final(const double* __restrict__ sums, int P, double n_dat
     }
 }
 
+// ---- batched (P > 1) path: host-side plan of one launch over points [p0, p0 + Pc) --------------------------------
+struct BatchPlan {
+    std::vector<double> Adense;
+    std::vector<int2> entries, items;
+    std::vector<double> itemA;
+    int item_start[9];
+    int nent;
+};
+
+int slot_code(const amp_model* m, int r, int lam) { return (m->res[r].kind << 8) | (m->res[r].J << 4) | (lam + 1); }
+
+// false if the model or the points do not fit the DMMA kernel (too many couplings or extended entries)
+bool build_batch_plan(const amp_model* m, int p0, int Pc, BatchPlan* bp) {
+    const int R = m->R, K = m->K;
+    if (2 * K > BATCH_NKT * 4 || Pc > BATCH_POINTS) return false;
+    std::vector<int> slot_res(K), slot_lam(K);
+    for (int r = 0; r < R; ++r) {
+        const int ns = (m->res[r].kind == AMP_Z || (m->res[r].kind == AMP_KSTAR && m->res[r].J >= 1)) ? 3 : 1;
+        for (int j = 0; j < ns; ++j) { slot_res[m->slot0[r] + j] = r; slot_lam[m->slot0[r] + j] = ns == 3 ? j - 1 : 0; }
+    }
+    const int nbase = BATCH_NKT * 2;   // complex base entries incl. padding
+    bp->entries.assign(nbase, make_int2(-1, 0));
+    for (int k = 0; k < K; ++k) {
+        const int r = slot_res[k];
+        const int col = m->res[r].kind == AMP_CONST ? -2 : m->colidx[(size_t)p0 * R + r];
+        if (col == -1 || col < -2) return false;
+        bp->entries[k] = make_int2(col, slot_code(m, r, slot_lam[k]));
+    }
+    bp->Adense.assign((size_t)16 * 2 * BATCH_NKT * 32, 0.0);
+    struct Item { int row0, octet; double a[2][32]; };
+    std::vector<Item> items;
+    auto put = [](double (*a)[32], int row, int kk, double cre, double cim) {   // realified rows kk (b_re), kk+1 (b_im) of one k-tile
+        a[0][row * 4 + (kk & 3)] = cre;  a[0][row * 4 + (kk & 3) + 1] = -cim;   // Re A
+        a[1][row * 4 + (kk & 3)] = cim;  a[1][row * 4 + (kk & 3) + 1] = cre;    // Im A
+    };
+    for (int q = 0; q < Pc; ++q) {
+        const int p = p0 + q, o = q / 8, row = q % 8;
+        for (int k = 0; k < K; ++k) {
+            const int r = slot_res[k];
+            const double cre = m->couplings[((size_t)p * K + k) * 2], cim = m->couplings[((size_t)p * K + k) * 2 + 1];
+            const int col = m->res[r].kind == AMP_CONST ? -2 : m->colidx[(size_t)p * R + r];
+            if (col == -1 || col < -2) return false;
+            int e = k;
+            if (col != bp->entries[k].x) {   // this point uses another lineshape column for this slot: extended entry
+                e = -1;
+                for (int j = nbase; j < (int)bp->entries.size(); ++j)
+                    if (bp->entries[j].x == col && bp->entries[j].y == bp->entries[k].y) { e = j; break; }
+                if (e < 0) { bp->entries.push_back(make_int2(col, bp->entries[k].y)); e = (int)bp->entries.size() - 1; }
+            }
+            const int kk = 2 * e;   // realified row of b_re
+            if (e < nbase) {
+                double (*a)[32] = nullptr;
+                double tmp[2][32] = {};
+                a = tmp;
+                put(a, row, kk, cre, cim);
+                const int kt = kk / 4;
+                for (int ri = 0; ri < 2; ++ri)
+                    for (int c = 0; c < 2; ++c) {
+                        const int lane = row * 4 + (kk & 3) + c;
+                        bp->Adense[((((size_t)o * 2 + ri) * BATCH_NKT) + kt) * 32 + lane] = tmp[ri][lane];
+                    }
+            } else {
+                const int row0 = kk / 4 * 4;
+                Item* itp = nullptr;
+                for (auto& it : items)
+                    if (it.row0 == row0 && it.octet == o) { itp = &it; break; }
+                if (!itp) { items.push_back(Item{row0, o, {}}); itp = &items.back(); }
+                put(itp->a, row, kk, cre, cim);
+            }
+        }
+    }
+    if (bp->entries.size() & 1) bp->entries.push_back(make_int2(-1, 0));
+    bp->nent = (int)bp->entries.size();
+    if (bp->nent > batch_max_entries()) return false;
+    // items grouped by owning warp (octet / 2)
+    bp->items.clear();
+    bp->itemA.clear();
+    for (int w = 0; w < 8; ++w) {
+        bp->item_start[w] = (int)bp->items.size();
+        for (auto& it : items)
+            if (it.octet / 2 == w) {
+                bp->items.push_back(make_int2(it.row0, it.octet & 1));
+                for (int ri = 0; ri < 2; ++ri) bp->itemA.insert(bp->itemA.end(), it.a[ri], it.a[ri] + 32);
+            }
+    }
+    bp->item_start[8] = (int)bp->items.size();
+    return true;
+}
+
+// upload a plan and launch the DMMA kernel on dataset d; partial rows [row0, row0 + Pc)
+amp_status run_batch(amp_model* m, const Dataset& d, const BatchPlan& bp, int Pc, int mode, size_t plan_off, double* partial, cudaStream_t s,
+                     int* grid_out) {
+    const size_t bA = bp.Adense.size() * sizeof(double), bE = bp.entries.size() * sizeof(int2), bI = bp.items.size() * sizeof(int2),
+                 bIA = bp.itemA.size() * sizeof(double);
+    auto al = [](size_t x) { return (x + 255) / 256 * 256; };
+    const size_t oA = plan_off, oE = oA + al(bA), oI = oE + al(bE), oIA = oI + al(bI), end = oIA + al(bIA);
+    if (end > m->plan_cap) return fail(m, AMP_ERR_NOMEM, "batch plan buffer too small");
+    std::memcpy(m->h_plan + oA, bp.Adense.data(), bA);
+    std::memcpy(m->h_plan + oE, bp.entries.data(), bE);
+    if (bI) std::memcpy(m->h_plan + oI, bp.items.data(), bI);
+    if (bIA) std::memcpy(m->h_plan + oIA, bp.itemA.data(), bIA);
+    CK(cudaMemcpyAsync(m->d_plan + plan_off, m->h_plan + plan_off, end - plan_off, cudaMemcpyHostToDevice, s));
+    BatchArgs a{};
+    a.cache = d.cache; a.weight = d.weight; a.cols = d.cols; a.n = d.n; a.npad = d.npad;
+    a.Adense = reinterpret_cast<const double*>(m->d_plan + oA);
+    a.entries = reinterpret_cast<const int2*>(m->d_plan + oE);
+    a.items = reinterpret_cast<const int2*>(m->d_plan + oI);
+    a.itemA = reinterpret_cast<const double*>(m->d_plan + oIA);
+    for (int w = 0; w < 9; ++w) a.item_start[w] = bp.item_start[w];
+    a.nent = bp.nent; a.nkt = BATCH_NKT; a.P = Pc; a.have_z = m->has_z ? 1 : 0; a.mode = mode;
+    a.partial = partial; a.partial_stride = PARTIAL_STRIDE; a.flag = m->d_flag;
+    const int grid = batch_grid(d.n);
+    CK(launch_batch(a, grid, s));
+    m->stat_launches++;
+    *grid_out = grid;
+    return AMP_OK;
+}
+
 amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cudaStream_t s) {
     if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
     if (want_nll && !m->data.loaded) return fail(m, AMP_ERR_STATE, "no data events loaded (amp_load_events)");
@@ -541,7 +673,50 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
     st = refresh_columns(m, m->norm, true, s);
     if (st != AMP_OK) return st;
     CK(cudaEventRecord(m->ev[1], s));
-    const int gd = stream_grid(m->data.n, m->has_z, MODE_DATA), gn = stream_grid(m->norm.n, m->has_z, MODE_NORM);
+    int gd = stream_grid(m->data.n, m->has_z, MODE_DATA), gn = stream_grid(m->norm.n, m->has_z, MODE_NORM);
+    // P > 1: one DMMA launch per dataset and chunk of <= 128 points, if the model and the points fit its plan
+    std::vector<BatchPlan> plans;
+    // (below ~24 points the streaming kernel, which shares the angular structure, is cheaper per point)
+    bool batched = P >= 24 && m->batch_mode == 0;
+    if (batched) {
+        for (int p0 = 0; p0 < P && batched; p0 += BATCH_POINTS) {
+            plans.emplace_back();
+            batched = build_batch_plan(m, p0, std::min((int)BATCH_POINTS, P - p0), &plans.back());
+        }
+    }
+    m->stat_batched = batched ? 1 : 0;
+    if (batched) m->stat_norm_path = 3;
+    if (batched) {
+        const size_t per_plan = (size_t)1 << 20, need = per_plan * plans.size() * 2;
+        if (need > m->plan_cap) {
+            if (m->d_plan) cudaFree(m->d_plan);
+            if (m->h_plan) cudaFreeHost(m->h_plan);
+            m->d_plan = m->h_plan = nullptr;
+            m->plan_cap = 0;
+            CK(cudaMalloc(&m->d_plan, need));
+            CK(cudaMallocHost(&m->h_plan, need));
+            m->plan_cap = need;
+        }
+        size_t slot = 0;
+        if (want_nll) {
+            for (size_t c = 0; c < plans.size(); ++c) {
+                const int p0 = (int)c * BATCH_POINTS, Pc = std::min((int)BATCH_POINTS, P - p0);
+                if (m->data.n > 0) {
+                    st = run_batch(m, m->data, plans[c], Pc, MODE_DATA, per_plan * slot++, m->d_partial + (size_t)p0 * PARTIAL_STRIDE, s, &gd);
+                    if (st != AMP_OK) return st;
+                } else {
+                    for (int p = p0; p < p0 + Pc; ++p) CK(cudaMemsetAsync(m->d_partial + (size_t)p * PARTIAL_STRIDE, 0, sizeof(double), s));
+                }
+            }
+        }
+        CK(cudaEventRecord(m->ev[2], s));
+        for (size_t c = 0; c < plans.size(); ++c) {
+            const int p0 = (int)c * BATCH_POINTS, Pc = std::min((int)BATCH_POINTS, P - p0);
+            st = run_batch(m, m->norm, plans[c], Pc, MODE_NORM, per_plan * slot++, m->d_partial + (size_t)(P + p0) * PARTIAL_STRIDE, s, &gn);
+            if (st != AMP_OK) return st;
+        }
+        CK(cudaEventRecord(m->ev[3], s));
+    } else {
     StreamArgs a;
     if (want_nll)
         for (int p = 0; p < P; ++p) {
@@ -562,6 +737,7 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         m->stat_launches++;
     }
     CK(cudaEventRecord(m->ev[3], s));
+    }
     if (want_nll) {
         CK(launch_finalize(m->d_partial, m->data.n > 0 ? gd : 1, PARTIAL_STRIDE, P, m->d_sums, s));
         m->stat_launches++;

@@ -195,7 +195,14 @@ def test_nll_batched_points_small():
     nll = Mg.nll()
     ref, refI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
     assert nll.shape == (121,)
+    assert Mg.last_call_stats()["norm_path"] == 3            # the batched DMMA kernel ran
     assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
+    # the loop of single-point streaming launches gives the same numbers
+    Mg.set_batch_mode(1)
+    nll_seq = Mg.nll()
+    assert Mg.last_call_stats()["norm_path"] == 1
+    assert np.max(np.abs(nll_seq - nll) / np.abs(nll)) < 1e-12
+    Mg.set_batch_mode(0)
     I = Mg.norm_integral()
     assert np.max(np.abs(I - refI) / refI) < 1e-12
     # the finite differences themselves (what MINUIT uses) agree: compare NLL(p) - NLL(0)
