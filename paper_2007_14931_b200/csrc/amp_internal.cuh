@@ -204,14 +204,16 @@ int stream_grid(long long n, bool have_z, int mode);
 long long stream_pad(long long n);   // events per column rounded up to whole pipeline tiles
 
 // Batched combine (P > 1) on the FP64 tensor cores, see batch.cu
-enum { BATCH_NKT = 14, BATCH_POINTS = 128 };   // dense k-tiles (2K <= 56 realified rows) and points per launch
+enum { BATCH_NKT = 14, BATCH_POINTS = 128, BATCH_MAX_COLS = 48 };   // dense k-tiles (2K <= 56 realified rows) and points per launch
 struct BatchArgs {
     const double* cache;
     const double* weight;
     const double2* cols;
     long long n, npad;
     const double* Adense;   // [16 octets][re/im][BATCH_NKT][32 lanes]: coefficient fragments of the K base entries
-    const int2* entries;    // [nent] (lineshape column | -1 empty | -2 lineshape == 1, angular code) per complex basis entry
+    const int2* entries;    // [nent] (index into colu | -1 empty | -2 lineshape == 1, angular code) per complex basis entry
+    int colu[BATCH_MAX_COLS];   // distinct pool columns the entries use (staged per tile)
+    int ncolu;
     const int2* items;      // [nitems] (first realified row of an extended k-tile, octet 0/1 within the warp)
     const double* itemA;    // [nitems][re/im][32 lanes]
     int item_start[9];      // items of warp w: [item_start[w], item_start[w+1])
@@ -226,7 +228,7 @@ struct BatchArgs {
 };
 cudaError_t launch_batch(const BatchArgs& a, int grid, cudaStream_t s);
 int batch_grid(long long n);
-int batch_max_entries();
+bool batch_fits(int nent, int ncolu);
 
 // fixed-order final reduction of per-block partials: out[j] = sum_b partial[j][b], j < nrows
 cudaError_t launch_finalize(const double* partial, int nblocks, int stride, int nrows, double* out, cudaStream_t s);

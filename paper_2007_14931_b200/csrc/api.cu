@@ -546,6 +546,7 @@ struct BatchPlan {
     std::vector<double> itemA;
     int item_start[9];
     int nent;
+    std::vector<int> colu;   // distinct pool columns; entries[].x indexes this list
 };
 
 int slot_code(const amp_model* m, int r, int lam) { return (m->res[r].kind << 8) | (m->res[r].J << 4) | (lam + 1); }
@@ -612,7 +613,17 @@ bool build_batch_plan(const amp_model* m, int p0, int Pc, BatchPlan* bp) {
     }
     if (bp->entries.size() & 1) bp->entries.push_back(make_int2(-1, 0));
     bp->nent = (int)bp->entries.size();
-    if (bp->nent > batch_max_entries()) return false;
+    // pool columns -> indices into the list of distinct columns the kernel stages per tile
+    bp->colu.clear();
+    for (auto& en : bp->entries) {
+        if (en.x < 0) continue;
+        int j = 0;
+        for (; j < (int)bp->colu.size(); ++j)
+            if (bp->colu[j] == en.x) break;
+        if (j == (int)bp->colu.size()) bp->colu.push_back(en.x);
+        en.x = j;
+    }
+    if (!batch_fits(bp->nent, (int)bp->colu.size())) return false;
     // items grouped by owning warp (octet / 2)
     bp->items.clear();
     bp->itemA.clear();
@@ -648,6 +659,8 @@ amp_status run_batch(amp_model* m, const Dataset& d, const BatchPlan& bp, int Pc
     a.items = reinterpret_cast<const int2*>(m->d_plan + oI);
     a.itemA = reinterpret_cast<const double*>(m->d_plan + oIA);
     for (int w = 0; w < 9; ++w) a.item_start[w] = bp.item_start[w];
+    a.ncolu = (int)bp.colu.size();
+    for (int j = 0; j < a.ncolu; ++j) a.colu[j] = bp.colu[j];
     a.nent = bp.nent; a.nkt = BATCH_NKT; a.P = Pc; a.have_z = m->has_z ? 1 : 0; a.mode = mode;
     a.partial = partial; a.partial_stride = PARTIAL_STRIDE; a.flag = m->d_flag;
     const int grid = batch_grid(d.n);

@@ -27,6 +27,47 @@ __device__ __forceinline__ void dmma884(double (&d)[2], double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
 }
 
+// TMA bulk copy + mbarrier helpers (same PTX as in stream.cu)
+__device__ __forceinline__ uint32_t bsmem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void bmbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bsmem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void bmbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bsmem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bmbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "BWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra BDONE_%=;\n"
+        "bra BWAIT_%=;\n"
+        "BDONE_%=:\n"
+        "}\n" ::"r"(bsmem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bbulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(bsmem_u32(dst)), "l"(src),
+                 "r"(bytes), "r"(bsmem_u32(bar))
+                 : "memory");
+}
+
+constexpr int BT_NANG = 14;   // staged cache columns: the angular ones (C_CK .. C_SPHI, C_CZ .. C_SA)
+__device__ __forceinline__ int ang_col(int j) { return j < 6 ? C_CK + j : C_CZ + (j - 6); }
+
+// raw inputs of one tile -> staging area: the distinct lineshape columns (64 x 16 B each), the angular cache
+// columns and the weights (64 x 8 B each); issued by one thread, lands while the previous tile is multiplied
+__device__ __forceinline__ void issue_stage(const BatchArgs& a, long long tile, double2* scol, double* sang, double* sw, uint64_t* bar, int nang,
+                                            bool with_w) {
+    const long long i0 = tile * BT_EVENTS;
+    bmbar_expect_tx(bar, (uint32_t)(a.ncolu * BT_EVENTS * 16 + (nang + (with_w ? 1 : 0)) * BT_EVENTS * 8));
+#pragma unroll 1
+    for (int c = 0; c < a.ncolu; ++c) bbulk_g2s(scol + (size_t)c * BT_EVENTS, a.cols + (size_t)a.colu[c] * a.npad + i0, BT_EVENTS * 16, bar);
+#pragma unroll 1
+    for (int j = 0; j < nang; ++j) bbulk_g2s(sang + (size_t)j * BT_EVENTS, a.cache + (size_t)ang_col(j) * a.npad + i0, BT_EVENTS * 8, bar);
+    if (with_w) bbulk_g2s(sw, a.weight + i0, BT_EVENTS * 8, bar);
+}
+
 // angular factor g_xi (xi = +1, -1) of one basis entry at one event; `code` is warp-uniform
 struct Angles {
     double cK, sK, cpsi, spsi, cphi, sphi;
@@ -79,7 +120,13 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_batch(const __grid_constant__
     extern __shared__ __align__(16) double smem[];
     const int KP = a.nent * 2;                                 // realified rows (multiple of 4)
     double* Bs = smem;                                         // [2][KP][BT_STRIDE]
-    double* ws = smem + (size_t)2 * KP * BT_STRIDE;            // [BT_EVENTS]
+    double* ws = smem + (size_t)2 * KP * BT_STRIDE;            // [BT_EVENTS] weights of the tile being multiplied
+    double* sw = ws + BT_EVENTS;                               // staging: weights, angular columns, lineshape columns
+    double* sang = sw + BT_EVENTS;                             // [BT_NANG][BT_EVENTS]
+    double2* scol = reinterpret_cast<double2*>(sang + BT_NANG * BT_EVENTS);   // [ncolu][BT_EVENTS]
+    uint64_t* full = reinterpret_cast<uint64_t*>(scol + (size_t)a.ncolu * BT_EVENTS);
+    const int nang = a.have_z ? BT_NANG : 6;
+    const bool with_w = MODE == MODE_NORM;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     // coefficient fragments of this warp's 16 points: [octet][re/im][k-tile]
@@ -98,24 +145,31 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_batch(const __grid_constant__
     double sum[2] = {0.0, 0.0}, prod[2] = {1.0, 1.0};
     bool bad = false;
     const long long ntiles = (a.n + BT_EVENTS - 1) / BT_EVENTS;
-    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        // ---- basis tile: thread (part, ev) fills entries part, part+4, ... of event ev for both helicities
+    if (tid == 0) {
+        bmbar_init(full, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0 && (long long)blockIdx.x < ntiles) issue_stage(a, blockIdx.x, scol, sang, sw, full, nang, with_w);
+    uint32_t parity = 0;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, parity ^= 1) {
+        // ---- basis tile from the staged inputs: thread (part, ev) fills entries part, part+4, ... of event ev, both helicities
+        bmbar_wait(full, parity);
         {
             const int ev = tid & (BT_EVENTS - 1), part = tid / BT_EVENTS;
             const long long i = tile * BT_EVENTS + ev;          // < npad (npad is a multiple of 512)
-            const double* col = a.cache + i;
             Angles g;
-            g.cK = col[C_CK * a.npad]; g.sK = col[C_SK * a.npad]; g.cpsi = col[C_CPSI * a.npad]; g.spsi = col[C_SPSI * a.npad];
-            g.cphi = col[C_CPHI * a.npad]; g.sphi = col[C_SPHI * a.npad];
+            g.cK = sang[0 * BT_EVENTS + ev]; g.sK = sang[1 * BT_EVENTS + ev]; g.cpsi = sang[2 * BT_EVENTS + ev]; g.spsi = sang[3 * BT_EVENTS + ev];
+            g.cphi = sang[4 * BT_EVENTS + ev]; g.sphi = sang[5 * BT_EVENTS + ev];
             if (a.have_z) {
-                g.cZ = col[C_CZ * a.npad]; g.sZ = col[C_SZ * a.npad]; g.ct = col[C_CT * a.npad]; g.st = col[C_ST * a.npad];
-                g.cpt = col[C_CPT * a.npad]; g.spt = col[C_SPT * a.npad]; g.ca = col[C_CA * a.npad]; g.sa = col[C_SA * a.npad];
+                g.cZ = sang[6 * BT_EVENTS + ev]; g.sZ = sang[7 * BT_EVENTS + ev]; g.ct = sang[8 * BT_EVENTS + ev]; g.st = sang[9 * BT_EVENTS + ev];
+                g.cpt = sang[10 * BT_EVENTS + ev]; g.spt = sang[11 * BT_EVENTS + ev]; g.ca = sang[12 * BT_EVENTS + ev]; g.sa = sang[13 * BT_EVENTS + ev];
             }
             for (int e = part; e < a.nent; e += BT_THREADS / BT_EVENTS) {
-                const int2 en = a.entries[e];                   // (column, code); column -1: empty entry, -2: lineshape == 1
+                const int2 en = a.entries[e];                   // (staged column, code); column -1: empty entry, -2: lineshape == 1
                 double2 bp = make_double2(0, 0), bm = bp;
                 if (en.x != -1) {
-                    const double2 bw = en.x >= 0 ? a.cols[(size_t)en.x * a.npad + i] : make_double2(1.0, 0.0);
+                    const double2 bw = en.x >= 0 ? scol[(size_t)en.x * BT_EVENTS + ev] : make_double2(1.0, 0.0);
                     double2 gp, gm;
                     angular_factor(g, en.y, &gp, &gm);
                     bp = cmul(bw, gp);
@@ -125,9 +179,10 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_batch(const __grid_constant__
                 r0[0] = bp.x; r0[BT_STRIDE] = bp.y;
                 r0[(size_t)KP * BT_STRIDE] = bm.x; r0[(size_t)KP * BT_STRIDE + BT_STRIDE] = bm.y;
             }
-            if (part == 0) ws[ev] = (i < a.n) ? (MODE == MODE_NORM ? a.weight[i] : 1.0) : 0.0;
+            if (part == 0) ws[ev] = (i < a.n) ? (with_w ? sw[ev] : 1.0) : 0.0;
         }
-        __syncthreads();
+        __syncthreads();   // basis tile complete, staging area consumed: stream the next tile into it during the DMMA phase
+        if (tid == 0 && tile + gridDim.x < ntiles) issue_stage(a, tile + gridDim.x, scol, sang, sw, full, nang, with_w);
         // ---- DMMA: this warp's 16 points x 64 events x both helicities
 #pragma unroll 1
         for (int nt = 0; nt < BT_EVENTS / 8; ++nt) {
@@ -191,8 +246,10 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_batch(const __grid_constant__
     }
 }
 
-size_t batch_smem(int nent) { return ((size_t)2 * nent * 2 * BT_STRIDE + BT_EVENTS) * sizeof(double); }
-int batch_max_entries() { return (int)(((224 * 1024) / sizeof(double) - BT_EVENTS) / (4 * BT_STRIDE)) & ~1; }
+size_t batch_smem(int nent, int ncolu) {
+    return ((size_t)2 * nent * 2 * BT_STRIDE + 2 * BT_EVENTS + BT_NANG * BT_EVENTS + (size_t)ncolu * BT_EVENTS * 2) * sizeof(double) + 16;
+}
+bool batch_fits(int nent, int ncolu) { return ncolu <= BATCH_MAX_COLS && batch_smem(nent, ncolu) <= (size_t)224 * 1024; }
 
 int batch_grid(long long n) {
     const long long ntiles = (n + BT_EVENTS - 1) / BT_EVENTS;
@@ -200,7 +257,7 @@ int batch_grid(long long n) {
 }
 
 cudaError_t launch_batch(const BatchArgs& a, int grid, cudaStream_t s) {
-    const size_t smem = batch_smem(a.nent);
+    const size_t smem = batch_smem(a.nent, a.ncolu);
     cudaError_t e = cudaSuccess;
 #define AMP_LAUNCH(NKT, M)                                                                                           \
     {                                                                                                                \
