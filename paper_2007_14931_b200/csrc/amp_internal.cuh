@@ -217,6 +217,7 @@ struct BatchArgs {
     const int2* items;      // [nitems] (first realified row of an extended k-tile, octet 0/1 within the warp)
     const double* itemA;    // [nitems][re/im][32 lanes]
     int item_start[9];      // items of warp w: [item_start[w], item_start[w+1])
+    short point_of_row[BATCH_POINTS];   // GEMM row (16 per warp) -> point of this launch, -1: unused row
     int nent;               // complex basis entries (base, padded to BATCH_NKT * 2, then extended), even
     int nkt;
     int P;                  // points in this launch (<= BATCH_POINTS)

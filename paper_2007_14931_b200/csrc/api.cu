@@ -547,6 +547,7 @@ struct BatchPlan {
     int item_start[9];
     int nent;
     std::vector<int> colu;   // distinct pool columns; entries[].x indexes this list
+    int point_of_row[BATCH_POINTS];
 };
 
 int slot_code(const amp_model* m, int r, int lam) { return (m->res[r].kind << 8) | (m->res[r].J << 4) | (lam + 1); }
@@ -575,8 +576,30 @@ bool build_batch_plan(const amp_model* m, int p0, int Pc, BatchPlan* bp) {
         a[0][row * 4 + (kk & 3)] = cre;  a[0][row * 4 + (kk & 3) + 1] = -cim;   // Re A
         a[1][row * 4 + (kk & 3)] = cim;  a[1][row * 4 + (kk & 3) + 1] = cre;    // Im A
     };
+    // Rows of the GEMM: points that use a lineshape column other than the base one own extra (sparse) blocks; deal
+    // them round-robin over the eight warps so every warp multiplies about the same number of blocks.
+    std::vector<int> row_of(Pc, -1);
+    {
+        int next_row[8], nvar = 0;
+        for (int w = 0; w < 8; ++w) next_row[w] = 16 * w;
+        std::vector<char> is_var(Pc, 0);
+        for (int q = 0; q < Pc; ++q)
+            for (int r = 0; r < R; ++r)
+                if (m->res[r].kind != AMP_CONST && m->colidx[(size_t)(p0 + q) * R + r] != m->colidx[(size_t)p0 * R + r]) is_var[q] = 1;
+        for (int q = 0; q < Pc; ++q)
+            if (is_var[q]) { const int w = nvar++ % 8; row_of[q] = next_row[w]++; }
+        int w = 0;
+        for (int q = 0; q < Pc; ++q) {
+            if (is_var[q]) continue;
+            while (next_row[w] >= 16 * (w + 1)) w = (w + 1) % 8;
+            row_of[q] = next_row[w]++;
+            w = (w + 1) % 8;
+        }
+        for (int i = 0; i < BATCH_POINTS; ++i) bp->point_of_row[i] = -1;
+        for (int q = 0; q < Pc; ++q) bp->point_of_row[row_of[q]] = q;
+    }
     for (int q = 0; q < Pc; ++q) {
-        const int p = p0 + q, o = q / 8, row = q % 8;
+        const int p = p0 + q, o = row_of[q] / 8, row = row_of[q] % 8;
         for (int k = 0; k < K; ++k) {
             const int r = slot_res[k];
             const double cre = m->couplings[((size_t)p * K + k) * 2], cim = m->couplings[((size_t)p * K + k) * 2 + 1];
@@ -659,6 +682,7 @@ amp_status run_batch(amp_model* m, const Dataset& d, const BatchPlan& bp, int Pc
     a.items = reinterpret_cast<const int2*>(m->d_plan + oI);
     a.itemA = reinterpret_cast<const double*>(m->d_plan + oIA);
     for (int w = 0; w < 9; ++w) a.item_start[w] = bp.item_start[w];
+    for (int i = 0; i < BATCH_POINTS; ++i) a.point_of_row[i] = (short)bp.point_of_row[i];
     a.ncolu = (int)bp.colu.size();
     for (int j = 0; j < a.ncolu; ++j) a.colu[j] = bp.colu[j];
     a.nent = bp.nent; a.nkt = BATCH_NKT; a.P = Pc; a.have_z = m->has_z ? 1 : 0; a.mode = mode;

@@ -139,8 +139,10 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_batch(const __grid_constant__
             for (int kt = 0; kt < NKT; ++kt) Afr[o][ri][kt] = a.Adense[((((size_t)(2 * warp + o) * 2 + ri) * NKT) + kt) * 32 + lane];
     const int it0 = a.item_start[warp], it1 = a.item_start[warp + 1];
     const int prow = lane >> 2;                                // point row within an octet
-    const bool live0 = 16 * warp + prow < a.P, live1 = 16 * warp + 8 + prow < a.P;
-    const bool oct0 = 16 * warp < a.P, oct1 = 16 * warp + 8 < a.P;   // octets without any point are skipped (warp-uniform)
+    // row -> parameter point (the host spreads the points that own extended-basis blocks evenly over the warps)
+    const int pt0 = a.point_of_row[16 * warp + prow], pt1 = a.point_of_row[16 * warp + 8 + prow];
+    const bool live0 = pt0 >= 0, live1 = pt1 >= 0;
+    const bool warp_live = __any_sync(0xffffffffu, live0 || live1);
 
     double sum[2] = {0.0, 0.0}, prod[2] = {1.0, 1.0};
     bool bad = false;
@@ -185,34 +187,48 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_batch(const __grid_constant__
         if (tid == 0 && tile + gridDim.x < ntiles) issue_stage(a, tile + gridDim.x, scol, sang, sw, full, nang, with_w);
         // ---- DMMA: this warp's 16 points x 64 events x both helicities
 #pragma unroll 1
-        for (int nt = 0; nt < BT_EVENTS / 8; ++nt) {
-            double S[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+        for (int nt = 0; nt < (warp_live ? BT_EVENTS / 8 : 0); ++nt) {
+            // both helicities side by side: eight independent accumulator chains per warp keep the DMMA pipe fed
+            double acc[2][2][2][2];   // [xi][octet][re/im][event pair]
 #pragma unroll
-            for (int xi = 0; xi < 2; ++xi) {
-                double acc[2][2][2];
-#pragma unroll
-                for (int o = 0; o < 2; ++o)
-#pragma unroll
-                    for (int ri = 0; ri < 2; ++ri) acc[o][ri][0] = acc[o][ri][1] = 0.0;
-                const double* bbase = Bs + (size_t)xi * KP * BT_STRIDE + (size_t)(lane & 3) * BT_STRIDE + 8 * nt + (lane >> 2);
-#pragma unroll
-                for (int kt = 0; kt < NKT; ++kt) {
-                    const double b = bbase[(size_t)4 * kt * BT_STRIDE];
-                    if (oct0) { dmma884(acc[0][0], Afr[0][0][kt], b); dmma884(acc[0][1], Afr[0][1][kt], b); }
-                    if (oct1) { dmma884(acc[1][0], Afr[1][0][kt], b); dmma884(acc[1][1], Afr[1][1][kt], b); }
-                }
-                for (int it = it0; it < it1; ++it) {           // non-zero blocks of the extended (variant) basis
-                    const int2 item = a.items[it];               // (first realified row of the k-tile, octet 0/1 of this warp)
-                    const double b = bbase[(size_t)item.x * BT_STRIDE];
-                    const double are = a.itemA[((size_t)it * 2) * 32 + lane], aim = a.itemA[((size_t)it * 2 + 1) * 32 + lane];
-                    if (item.y == 0) { dmma884(acc[0][0], are, b); dmma884(acc[0][1], aim, b); }
-                    else { dmma884(acc[1][0], are, b); dmma884(acc[1][1], aim, b); }
-                }
+            for (int xi = 0; xi < 2; ++xi)
 #pragma unroll
                 for (int o = 0; o < 2; ++o)
 #pragma unroll
-                    for (int j = 0; j < 2; ++j) S[o][j] = fma(acc[o][0][j], acc[o][0][j], fma(acc[o][1][j], acc[o][1][j], S[o][j]));
+                    for (int ri = 0; ri < 2; ++ri) acc[xi][o][ri][0] = acc[xi][o][ri][1] = 0.0;
+            const double* bbase = Bs + (size_t)(lane & 3) * BT_STRIDE + 8 * nt + (lane >> 2);
+            const size_t xoff = (size_t)KP * BT_STRIDE;
+#pragma unroll
+            for (int kt = 0; kt < NKT; ++kt) {
+                const double bP = bbase[(size_t)4 * kt * BT_STRIDE], bM = bbase[xoff + (size_t)4 * kt * BT_STRIDE];
+                dmma884(acc[0][0][0], Afr[0][0][kt], bP);
+                dmma884(acc[1][0][0], Afr[0][0][kt], bM);
+                dmma884(acc[0][0][1], Afr[0][1][kt], bP);
+                dmma884(acc[1][0][1], Afr[0][1][kt], bM);
+                dmma884(acc[0][1][0], Afr[1][0][kt], bP);
+                dmma884(acc[1][1][0], Afr[1][0][kt], bM);
+                dmma884(acc[0][1][1], Afr[1][1][kt], bP);
+                dmma884(acc[1][1][1], Afr[1][1][kt], bM);
             }
+            for (int it = it0; it < it1; ++it) {           // non-zero blocks of the extended (variant) basis
+                const int2 item = a.items[it];               // (first realified row of the k-tile, octet 0/1 of this warp)
+                const double bP = bbase[(size_t)item.x * BT_STRIDE], bM = bbase[xoff + (size_t)item.x * BT_STRIDE];
+                const double are = a.itemA[((size_t)it * 2) * 32 + lane], aim = a.itemA[((size_t)it * 2 + 1) * 32 + lane];
+                if (item.y == 0) {
+                    dmma884(acc[0][0][0], are, bP); dmma884(acc[1][0][0], are, bM);
+                    dmma884(acc[0][0][1], aim, bP); dmma884(acc[1][0][1], aim, bM);
+                } else {
+                    dmma884(acc[0][1][0], are, bP); dmma884(acc[1][1][0], are, bM);
+                    dmma884(acc[0][1][1], aim, bP); dmma884(acc[1][1][1], aim, bM);
+                }
+            }
+            double S[2][2];
+#pragma unroll
+            for (int o = 0; o < 2; ++o)
+#pragma unroll
+                for (int j = 0; j < 2; ++j)
+                    S[o][j] = fma(acc[0][o][0][j], acc[0][o][0][j], fma(acc[0][o][1][j], acc[0][o][1][j],
+                              fma(acc[1][o][0][j], acc[1][o][0][j], acc[1][o][1][j] * acc[1][o][1][j])));
             const double w0 = ws[8 * nt + 2 * (lane & 3)], w1 = ws[8 * nt + 2 * (lane & 3) + 1];
             if (MODE == MODE_NORM) {
 #pragma unroll
@@ -241,8 +257,8 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_batch(const __grid_constant__
         double v = sum[o];
         v += __shfl_xor_sync(0xffffffffu, v, 1);
         v += __shfl_xor_sync(0xffffffffu, v, 2);
-        const int p = 16 * warp + 8 * o + prow;
-        if ((lane & 3) == 0 && p < a.P) a.partial[(size_t)p * a.partial_stride + blockIdx.x] = v;
+        const int p = o ? pt1 : pt0;
+        if ((lane & 3) == 0 && p >= 0) a.partial[(size_t)p * a.partial_stride + blockIdx.x] = v;
     }
 }
 
