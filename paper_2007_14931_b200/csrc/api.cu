@@ -60,7 +60,24 @@ struct amp_model {
     size_t plan_cap = 0;
     int batch_mode = 0;            // 0 auto (DMMA kernel when eligible), 1 never (loop of single-point kernels)
 
-    int stat_launches = 0, stat_columns = 0, stat_norm_path = 0, stat_batched = 0;
+    // normalisation matrix (a4): Gram matrix of the last lineshape state, its signature, and work buffers
+    struct GramKey { int r; double mass, width; int code; };
+    std::vector<GramKey> gram_sig;
+    std::vector<int2> gram_tiles;
+    bool gram_valid = false;
+    int gram_KP = 0;
+    double* d_G = nullptr;         // [KP][KP] dense symmetric realified Gram matrix (sum_j w_j b' b'^T)
+    double* d_gt = nullptr;        // [ntile][64]
+    double* d_gpartial = nullptr;  // [148][ntile][64]
+    size_t gram_cap_KP = 0, gram_cap_tiles = 0;
+    unsigned char* d_hk = nullptr; // herk plan: entries, tiles, coefficients
+    unsigned char* h_hk = nullptr; // pinned
+    size_t hk_cap = 0;
+    bool stream_inline = true;     // P == 1: streaming launches evaluate lineshapes in registers even if columns exist
+    bool want_matrix = false;      // set_params decided that the normalisation should go through the matrix
+    std::vector<double> prev_mw;   // masses and widths of the previous single-point call (static-lineshape detection)
+
+    int stat_launches = 0, stat_columns = 0, stat_norm_path = 0, stat_batched = 0, stat_gram_built = 0;
     cudaEvent_t ev[5]{};           // phase boundaries of the last evaluation (amp_last_call_timing)
     bool ev_valid = false;
     std::string err;
@@ -141,6 +158,7 @@ amp_status load_dataset(amp_model* m, Dataset& d, bool is_norm, const double* d_
     if (n < 0 || (n > 0 && !d_x)) return fail(m, AMP_ERR_INVALID, "load: null events or negative count");
     free_dataset(d);
     for (auto& e : m->pool) (is_norm ? e.valid_norm : e.valid_data) = false;
+    if (is_norm) m->gram_valid = false;
     d.n = n;
     d.npad = stream_pad(n > 0 ? n : 1);
     d.ncache = m->has_z ? NCOL_ALL : NCOL_K;
@@ -258,6 +276,11 @@ amp_status amp_model_destroy(amp_model* m) {
     if (m->h_pinned) cudaFreeHost(m->h_pinned);
     if (m->d_plan) cudaFree(m->d_plan);
     if (m->h_plan) cudaFreeHost(m->h_plan);
+    if (m->d_G) cudaFree(m->d_G);
+    if (m->d_gt) cudaFree(m->d_gt);
+    if (m->d_gpartial) cudaFree(m->d_gpartial);
+    if (m->d_hk) cudaFree(m->d_hk);
+    if (m->h_hk) cudaFreeHost(m->h_hk);
     for (int i = 0; i < 5; ++i) if (m->ev[i]) cudaEventDestroy(m->ev[i]);
     delete m;
     return AMP_OK;
@@ -365,6 +388,13 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
     m->couplings.assign(h_couplings, h_couplings + (size_t)P * K * 2);
     m->mw.swap(mw);
     m->call_id++;
+    // Normalisation path.  The matrix M pays when it can be reused or shared: a single point whose masses and widths
+    // equal those of the previous call (lineshapes are not moving: M is built once, every later call is O(K^2)), or a
+    // large batch of points (one Gram pass instead of one pass per point).  Otherwise the direct sum is cheaper.
+    const bool mw_same = P == 1 && m->prev_mw.size() == m->mw.size() && std::equal(m->mw.begin(), m->mw.end(), m->prev_mw.begin());
+    m->want_matrix = m->norm_mode == 2 || (m->norm_mode == 0 && (P == 1 ? mw_same : (P >= 24 && m->batch_mode == 0)));
+    if (P == 1) m->prev_mw = m->mw; else m->prev_mw.clear();
+    m->stream_inline = P == 1 && m->lineshape_mode != 1;
 
     // distinct (resonance, mass, width) keys of this call
     struct Key { int r; double mass, width; };
@@ -403,7 +433,7 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
     for (size_t k = 0; k < keys.size(); ++k) {
         // P == 1: evaluating a Breit-Wigner in registers is cheaper than reading its 16 B column on B200, so
         // unless the caller forces the pool (mode 1) no column is stored or read at all
-        const bool want_inline = P == 1 && m->lineshape_mode != 1;
+        const bool want_inline = m->stream_inline && !m->want_matrix;
         inline_key[k] = want_inline;
         if (!want_inline) ++need;
     }
@@ -493,7 +523,7 @@ void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, Str
                     e.cm = make_double2(cp[0], cp[1]); e.c0 = make_double2(cp[2], cp[3]); e.cp = make_double2(cp[4], cp[5]);
                 }
                 const int sidx = m->colidx[(size_t)p * m->R + r2];
-                e.column = sidx >= 0 ? sidx : -1;
+                e.column = (sidx >= 0 && !m->stream_inline) ? sidx : -1;
             }
             grp.count = t - grp.first;
         }
@@ -694,6 +724,164 @@ amp_status run_batch(amp_model* m, const Dataset& d, const BatchPlan& bp, int Pc
     return AMP_OK;
 }
 
+// ---- normalisation through the matrix M (a4) -------------------------------------------------------------------
+struct HerkPlan {
+    std::vector<int2> entries;          // (index into colu | -1 | -2, angular code), nent a multiple of 4
+    std::vector<int> colu;
+    std::vector<double2> C;             // [P][nent] coefficient of every entry at every point
+    std::vector<int2> tiles;            // needed (I <= J) tiles, grouped by owning warp
+    int tile_start[9];
+    std::vector<amp_model::GramKey> sig;
+    int nent;
+};
+
+// Extended basis over ALL P points (base = the columns of point 0) and the Gram tiles some point needs.
+bool build_herk_plan(const amp_model* m, HerkPlan* hp, int pbase = 0, int npts = -1) {
+    const int R = m->R, K = m->K, P = npts < 0 ? m->P : npts;
+    std::vector<int> slot_res(K), slot_lam(K);
+    for (int r = 0; r < R; ++r) {
+        const int ns = (m->res[r].kind == AMP_Z || (m->res[r].kind == AMP_KSTAR && m->res[r].J >= 1)) ? 3 : 1;
+        for (int j = 0; j < ns; ++j) { slot_res[m->slot0[r] + j] = r; slot_lam[m->slot0[r] + j] = ns == 3 ? j - 1 : 0; }
+    }
+    std::vector<int2> ent(K);           // pool column (or -2) and code, base entries
+    for (int k = 0; k < K; ++k) {
+        const int r = slot_res[k];
+        const int col = m->res[r].kind == AMP_CONST ? -2 : m->colidx[(size_t)pbase * R + r];
+        if (col == -1 || col < -2) return false;
+        ent[k] = make_int2(col, slot_code(m, r, slot_lam[k]));
+    }
+    std::vector<std::vector<std::pair<int, double2>>> coef(P);
+    for (int q = 0; q < P; ++q)
+        for (int k = 0; k < K; ++k) {
+            const int p = pbase + q;
+            const int r = slot_res[k];
+            const int col = m->res[r].kind == AMP_CONST ? -2 : m->colidx[(size_t)p * R + r];
+            if (col == -1 || col < -2) return false;
+            int e = k;
+            if (col != ent[k].x) {
+                e = -1;
+                for (int j = K; j < (int)ent.size(); ++j)
+                    if (ent[j].x == col && ent[j].y == ent[k].y) { e = j; break; }
+                if (e < 0) { ent.push_back(make_int2(col, ent[k].y)); e = (int)ent.size() - 1; }
+            }
+            coef[q].push_back({e, make_double2(m->couplings[((size_t)p * K + k) * 2], m->couplings[((size_t)p * K + k) * 2 + 1])});
+        }
+    while (ent.size() % 4) ent.push_back(make_int2(-1, 0));
+    hp->nent = (int)ent.size();
+    // signature: what each entry is, independent of pool slot numbers
+    hp->sig.clear();
+    for (auto& en : ent) {
+        amp_model::GramKey g{-1, 0, 0, en.y};
+        if (en.x >= 0) { g.r = m->pool[en.x].r; g.mass = m->pool[en.x].mass; g.width = m->pool[en.x].width; }
+        else g.r = en.x;
+        hp->sig.push_back(g);
+    }
+    hp->colu.clear();
+    hp->entries = ent;
+    for (auto& en : hp->entries) {
+        if (en.x < 0) continue;
+        int j = 0;
+        for (; j < (int)hp->colu.size(); ++j)
+            if (hp->colu[j] == en.x) break;
+        if (j == (int)hp->colu.size()) hp->colu.push_back(en.x);
+        en.x = j;
+    }
+    if (!batch_fits(hp->nent, (int)hp->colu.size())) return false;
+    hp->C.assign((size_t)P * hp->nent, make_double2(0, 0));
+    const int NT = hp->nent / 4;        // row tiles (8 realified rows = 4 complex entries)
+    std::vector<char> need((size_t)NT * NT, 0);
+    for (int p = 0; p < P; ++p) {
+        std::vector<char> used(NT, 0);
+        for (auto& ce : coef[p]) {
+            hp->C[(size_t)p * hp->nent + ce.first] = ce.second;
+            used[ce.first / 4] = 1;   // structural: every entry the point references, whatever its coupling's value
+        }
+        for (int I = 0; I < NT; ++I)
+            if (used[I])
+                for (int J = I; J < NT; ++J)
+                    if (used[J]) need[(size_t)I * NT + J] = 1;
+    }
+    std::vector<int2> all;
+    for (int I = 0; I < NT; ++I)
+        for (int J = I; J < NT; ++J)
+            if (need[(size_t)I * NT + J]) all.push_back(make_int2(I, J));
+    if ((int)all.size() > herk_max_tiles()) return false;
+    // contiguous, equally sized chunks of the row-sorted list: a warp reloads its A fragment only when I changes
+    hp->tiles = all;
+    const int n = (int)all.size();
+    for (int w = 0; w <= 8; ++w) hp->tile_start[w] = (int)((long long)n * w / 8);
+    return true;
+}
+
+bool gram_hit(const amp_model* m, const HerkPlan& hp) {
+    if (!m->gram_valid || m->gram_KP != hp.nent * 2 || m->gram_sig.size() != hp.sig.size() || m->gram_tiles.size() != hp.tiles.size()) return false;
+    for (size_t i = 0; i < hp.sig.size(); ++i) {
+        const auto &a = m->gram_sig[i], &b = hp.sig[i];
+        if (a.r != b.r || a.mass != b.mass || a.width != b.width || a.code != b.code) return false;
+    }
+    for (size_t i = 0; i < hp.tiles.size(); ++i)
+        if (m->gram_tiles[i].x != hp.tiles[i].x || m->gram_tiles[i].y != hp.tiles[i].y) return false;
+    return true;
+}
+
+// G' (re)built if the signature changed; then out[p] = c(p)^H M c(p) (unnormalised: sum_j w_j S_j) for all points
+amp_status norm_via_matrix(amp_model* m, const HerkPlan& hp, double* d_out, cudaStream_t s) {
+    const int KP = hp.nent * 2, ntile = (int)hp.tiles.size(), P = (int)(hp.C.size() / hp.nent);
+    bool hit = gram_hit(m, hp);
+    auto al = [](size_t x) { return (x + 255) / 256 * 256; };
+    const size_t bE = hp.entries.size() * sizeof(int2), bT = hp.tiles.size() * sizeof(int2), bC = hp.C.size() * sizeof(double2);
+    const size_t oE = 0, oT = al(bE), oC = oT + al(bT), end = oC + al(bC);
+    if (end > m->hk_cap) {
+        if (m->d_hk) cudaFree(m->d_hk);
+        if (m->h_hk) cudaFreeHost(m->h_hk);
+        m->d_hk = m->h_hk = nullptr;
+        m->hk_cap = 0;
+        CK(cudaMalloc(&m->d_hk, end * 2));
+        CK(cudaMallocHost(&m->h_hk, end * 2));
+        m->hk_cap = end * 2;
+    }
+    if ((size_t)KP > m->gram_cap_KP || (size_t)ntile > m->gram_cap_tiles) {
+        for (double** b : {&m->d_G, &m->d_gt, &m->d_gpartial}) { if (*b) cudaFree(*b); *b = nullptr; }
+        m->gram_valid = false;
+        hit = false;
+        m->gram_cap_KP = KP;
+        m->gram_cap_tiles = ntile;
+        CK(cudaMalloc(&m->d_G, sizeof(double) * (size_t)KP * KP));
+        CK(cudaMalloc(&m->d_gt, sizeof(double) * (size_t)ntile * 64));
+        CK(cudaMalloc(&m->d_gpartial, sizeof(double) * (size_t)148 * ntile * 64));
+    }
+    std::memcpy(m->h_hk + oE, hp.entries.data(), bE);
+    std::memcpy(m->h_hk + oT, hp.tiles.data(), bT);
+    std::memcpy(m->h_hk + oC, hp.C.data(), bC);
+    CK(cudaMemcpyAsync(m->d_hk, m->h_hk, end, cudaMemcpyHostToDevice, s));
+    if (!hit) {
+        HerkArgs h{};
+        const Dataset& d = m->norm;
+        h.b.cache = d.cache; h.b.weight = d.weight; h.b.cols = d.cols; h.b.n = d.n; h.b.npad = d.npad;
+        h.b.entries = reinterpret_cast<const int2*>(m->d_hk + oE);
+        h.b.nent = hp.nent;
+        h.b.ncolu = (int)hp.colu.size();
+        for (int j = 0; j < h.b.ncolu; ++j) h.b.colu[j] = hp.colu[j];
+        h.b.have_z = m->has_z ? 1 : 0;
+        h.tiles = reinterpret_cast<const int2*>(m->d_hk + oT);
+        for (int w = 0; w < 9; ++w) h.tile_start[w] = hp.tile_start[w];
+        h.ntile = ntile;
+        h.partial = m->d_gpartial;
+        const int grid = batch_grid(d.n);
+        CK(launch_herk(h, grid, s));
+        CK(launch_herk_finish(m->d_gpartial, grid, ntile, h.tiles, KP, m->d_gt, m->d_G, s));
+        m->stat_launches += 3;
+        m->gram_sig = hp.sig;
+        m->gram_tiles = hp.tiles;
+        m->gram_KP = KP;
+        m->gram_valid = true;
+        m->stat_gram_built = 1;
+    }
+    CK(launch_quadform(m->d_G, KP, reinterpret_cast<const double2*>(m->d_hk + oC), hp.nent, P, d_out, s));
+    m->stat_launches++;
+    return AMP_OK;
+}
+
 amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cudaStream_t s) {
     if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
     if (want_nll && !m->data.loaded) return fail(m, AMP_ERR_STATE, "no data events loaded (amp_load_events)");
@@ -706,9 +894,15 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
     CK(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
     m->ev_valid = false;
     CK(cudaEventRecord(m->ev[0], s));
-    if (want_nll) { st = refresh_columns(m, m->data, false, s); if (st != AMP_OK) return st; }
-    st = refresh_columns(m, m->norm, true, s);
-    if (st != AMP_OK) return st;
+    m->stat_gram_built = 0;
+    HerkPlan hp;
+    bool use_matrix = m->want_matrix && build_herk_plan(m, &hp);
+    if (use_matrix) {   // the cached matrix may already cover this lineshape state: then no norm column is needed at all
+        const bool hit = gram_hit(m, hp);
+        if (!hit) { st = refresh_columns(m, m->norm, true, s); if (st != AMP_OK) return st; }
+    }
+    if (want_nll && !m->stream_inline) { st = refresh_columns(m, m->data, false, s); if (st != AMP_OK) return st; }
+    if (!use_matrix && !m->stream_inline) { st = refresh_columns(m, m->norm, true, s); if (st != AMP_OK) return st; }
     CK(cudaEventRecord(m->ev[1], s));
     int gd = stream_grid(m->data.n, m->has_z, MODE_DATA), gn = stream_grid(m->norm.n, m->has_z, MODE_NORM);
     // P > 1: one DMMA launch per dataset and chunk of <= 128 points, if the model and the points fit its plan
@@ -747,12 +941,11 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
             }
         }
         CK(cudaEventRecord(m->ev[2], s));
-        for (size_t c = 0; c < plans.size(); ++c) {
+        for (size_t c = 0; c < plans.size() && !use_matrix; ++c) {
             const int p0 = (int)c * BATCH_POINTS, Pc = std::min((int)BATCH_POINTS, P - p0);
             st = run_batch(m, m->norm, plans[c], Pc, MODE_NORM, per_plan * slot++, m->d_partial + (size_t)(P + p0) * PARTIAL_STRIDE, s, &gn);
             if (st != AMP_OK) return st;
         }
-        CK(cudaEventRecord(m->ev[3], s));
     } else {
     StreamArgs a;
     if (want_nll)
@@ -767,19 +960,24 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
             }
         }
     CK(cudaEventRecord(m->ev[2], s));
-    for (int p = 0; p < P; ++p) {
+    for (int p = 0; p < P && !use_matrix; ++p) {
         fill_stream_args(m, m->norm, p, MODE_NORM, &a);
         a.partial = m->d_partial + (size_t)(P + p) * PARTIAL_STRIDE;
         CK(launch_stream(a, gn, s));
         m->stat_launches++;
     }
-    CK(cudaEventRecord(m->ev[3], s));
     }
+    if (use_matrix) {
+        st = norm_via_matrix(m, hp, m->d_sums + P, s);
+        if (st != AMP_OK) return st;
+        m->stat_norm_path = 2;
+    }
+    CK(cudaEventRecord(m->ev[3], s));
     if (want_nll) {
         CK(launch_finalize(m->d_partial, m->data.n > 0 ? gd : 1, PARTIAL_STRIDE, P, m->d_sums, s));
         m->stat_launches++;
     }
-    CK(launch_finalize(m->d_partial + (size_t)P * PARTIAL_STRIDE, gn, PARTIAL_STRIDE, P, m->d_sums + P, s));
+    if (!use_matrix) CK(launch_finalize(m->d_partial + (size_t)P * PARTIAL_STRIDE, gn, PARTIAL_STRIDE, P, m->d_sums + P, s));
     k_nll_final<<<(P + 127) / 128, 128, 0, s>>>(m->d_sums, P, (double)m->data.n, m->data.loaded ? m->data.wsum : 0.0, m->norm.wsum, want_nll ? 1 : 0,
                                                 m->d_result);
     CK(cudaGetLastError());
@@ -826,8 +1024,10 @@ amp_status amp_eval_events(amp_model* m, int p, double* d_out, void* stream) {
     m->stat_launches = m->stat_columns = 0;
     amp_status st = ensure_pool(m, 0);
     if (st != AMP_OK) return st;
-    st = refresh_columns(m, m->data, false, s);
-    if (st != AMP_OK) return st;
+    if (!m->stream_inline) {
+        st = refresh_columns(m, m->data, false, s);
+        if (st != AMP_OK) return st;
+    }
     StreamArgs a;
     fill_stream_args(m, m->data, p, MODE_EVAL, &a);
     a.out = d_out;
@@ -873,8 +1073,36 @@ amp_status amp_eval_lineshape(amp_model* m, int which, int r, double mass, doubl
 }
 
 amp_status amp_norm_matrix(amp_model* m, int p, double* h_M, void* stream) {
-    (void)p; (void)h_M; (void)stream;
-    return fail(m, AMP_ERR_STATE, "amp_norm_matrix: not built yet");
+    if (!m) return AMP_ERR_INVALID;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
+    if (m->P < 1) return fail(m, AMP_ERR_STATE, "no parameters set (amp_set_params)");
+    if (p < 0 || p >= m->P || !h_M) return fail(m, AMP_ERR_INVALID, "amp_norm_matrix: bad point index or null output");
+    HerkPlan hp;
+    if (!build_herk_plan(m, &hp, p, 1))
+        return fail(m, AMP_ERR_STATE, "amp_norm_matrix: the lineshape columns of this point are not held; call amp_set_norm_mode(m, 2) before amp_set_params");
+    m->stat_launches = m->stat_columns = 0;
+    amp_status st = ensure_pool(m, 0);
+    if (st != AMP_OK) return st;
+    st = refresh_columns(m, m->norm, true, s);
+    if (st != AMP_OK) return st;
+    const int KP = hp.nent * 2, K = m->K;
+    double* d_tmp = nullptr;
+    CK(cudaMalloc(&d_tmp, sizeof(double)));
+    st = norm_via_matrix(m, hp, d_tmp, s);
+    std::vector<double> G((size_t)KP * KP);
+    cudaError_t e = st == AMP_OK ? cudaMemcpyAsync(G.data(), m->d_G, sizeof(double) * G.size(), cudaMemcpyDeviceToHost, s) : cudaSuccess;
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(d_tmp);
+    if (st != AMP_OK) return st;
+    if (e != cudaSuccess) return cuda_fail(m, e, "amp_norm_matrix");
+    for (int k = 0; k < K; ++k)
+        for (int l = 0; l < K; ++l) {
+            const double* g = &G[(size_t)(2 * k) * KP + 2 * l];
+            h_M[((size_t)k * K + l) * 2] = (g[0] + g[KP + 1]) / m->norm.wsum;
+            h_M[((size_t)k * K + l) * 2 + 1] = (g[1] - g[KP]) / m->norm.wsum;
+        }
+    return AMP_OK;
 }
 
 }  // extern "C"

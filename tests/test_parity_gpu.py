@@ -195,10 +195,21 @@ def test_nll_batched_points_small():
     nll = Mg.nll()
     ref, refI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
     assert nll.shape == (121,)
-    assert Mg.last_call_stats()["norm_path"] == 3            # the batched DMMA kernel ran
+    assert Mg.last_call_stats()["norm_path"] == 2            # batched DMMA combine on the data, matrix M for the integrals
     assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
+    # the same batch with the normalisation as a direct DMMA sum over the norm events
+    Mg.set_norm_mode(1)
+    Mg.set_params(cs, mws)
+    nll_direct = Mg.nll()
+    assert Mg.last_call_stats()["norm_path"] == 3
+    assert np.max(np.abs(nll_direct - ref) / np.abs(ref)) < RTOL_NLL
+    assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12
+    Mg.set_norm_mode(0)
+    Mg.set_params(cs, mws)
+    assert np.max(np.abs(Mg.nll() - nll) / np.abs(nll)) < 1e-13
     # the loop of single-point streaming launches gives the same numbers
     Mg.set_batch_mode(1)
+    Mg.set_params(cs, mws)
     nll_seq = Mg.nll()
     assert Mg.last_call_stats()["norm_path"] == 1
     assert np.max(np.abs(nll_seq - nll) / np.abs(nll)) < 1e-12
@@ -208,6 +219,60 @@ def test_nll_batched_points_small():
     # the finite differences themselves (what MINUIT uses) agree: compare NLL(p) - NLL(0)
     d, dref = nll[1:] - nll[0], ref[1:] - ref[0]
     assert np.max(np.abs(d - dref)) < 1e-9 * abs(ref[0])
+
+
+def test_norm_matrix_matches_oracle_and_direct_sum():
+    """a4: the Hermitian matrix M from the HERK kernel against the oracle's plain double loop, and c^H M c against
+    the direct sum (pin P10 on the GPU side)."""
+    cfg = 2
+    Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+    c = W.couplings(cfg)
+    xn, wn = W.norm_events(cfg, 7001)
+    Mg.load_norm(dev(xn), dev(wn))
+    Mg.set_norm_mode(2)
+    Mg.set_params(c)
+    M = Mg.norm_matrix(0)
+    ref = Mo.norm_matrix(xn, wn)
+    assert np.abs(M - ref).max() < 1e-12 * np.abs(ref).max()
+    assert np.abs(M - M.conj().T).max() < 1e-15 * np.abs(M).max()
+    I_mat = Mg.norm_integral()[0]
+    assert Mg.last_call_stats()["norm_path"] == 2
+    assert abs(I_mat - (c.conj() @ ref @ c).real) < 1e-12 * I_mat
+    Mg.set_norm_mode(1)
+    Mg.set_params(c)
+    I_dir = Mg.norm_integral()[0]
+    assert Mg.last_call_stats()["norm_path"] == 1
+    assert abs(I_mat - I_dir) < 1e-12 * I_dir
+    assert abs(I_dir - Mo.norm_integral(c, xn, wn)[0]) < 1e-12 * I_dir
+
+
+def test_static_lineshapes_switch_to_the_matrix():
+    """cfg 1 call pattern (masses and widths fixed, couplings move): the second call with unchanged lineshapes builds
+    M once, later calls only evaluate c^H M c; a moved mass goes back to the direct sum."""
+    cfg = 1
+    Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+    c = W.couplings(cfg)
+    x, eff, xn, wn = make_inputs(cfg, 20011, 60013)
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    rng = np.random.default_rng(11)
+    paths, launches = [], []
+    for it in range(4):
+        ci = c * (1 + 0.05 * rng.uniform(-1, 1, c.size))
+        Mg.set_params(ci)
+        nll = Mg.nll()[0]
+        ref = Mo.nll(ci, x, eff, xn, wn)[0][0]
+        assert abs(nll - ref) < RTOL_NLL * abs(ref)
+        st = Mg.last_call_stats()
+        paths.append(st["norm_path"]); launches.append(st["launches"])
+    assert paths == [1, 2, 2, 2]
+    assert launches[3] < launches[1]          # no lineshape / HERK launches once M is held
+    mw = W.step_mass_width(3, 5)[:10]
+    Mg.set_params(c, mw[None])
+    nll = Mg.nll()[0]
+    assert Mg.last_call_stats()["norm_path"] == 1
+    ref = Mo.nll(c, x, eff, xn, wn, mass_width=mw[None])[0][0]
+    assert abs(nll - ref) < RTOL_NLL * abs(ref)
 
 
 def test_edge_cases():
