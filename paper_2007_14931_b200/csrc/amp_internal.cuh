@@ -231,15 +231,16 @@ struct BatchArgs {
 // cols, n, npad, entries, nent (a multiple of 4), colu, ncolu, have_z); its GEMM fields are unused.
 struct HerkArgs {
     BatchArgs b;
-    const int2* tiles;      // [ntile] (row tile I, column tile J), I <= J, 8 realified rows per tile; sorted by I within a warp
-    int tile_start[9];      // tiles of warp w: [tile_start[w], tile_start[w+1])
+    const int4* runs;       // [8 warps][nrun] (row tile I, column tiles J0, J1, unused); 8 realified rows per tile
+    const int2* runs_out;   // [8 warps][nrun] index of (I,J0), (I,J1) in the tile list, -1: padding (result dropped)
+    int nrun;               // runs per warp (padded to the kernel's unroll count by launch_herk's choice: even numbers up to 12)
     int ntile;
     double* partial;        // [grid][ntile][64]
 };
 cudaError_t launch_herk(const HerkArgs& h, int grid, cudaStream_t s);
 cudaError_t launch_herk_finish(const double* partial, int ncta, int ntile, const int2* tiles, int KP, double* gt, double* G, cudaStream_t s);
 cudaError_t launch_quadform(const double* G, int KP, const double2* C, int nent, int P, double* out, cudaStream_t s);
-int herk_max_tiles();
+int herk_max_runs();
 cudaError_t launch_batch(const BatchArgs& a, int grid, cudaStream_t s);
 int batch_grid(long long n);
 bool batch_fits(int nent, int ncolu);

@@ -730,7 +730,9 @@ struct HerkPlan {
     std::vector<int> colu;
     std::vector<double2> C;             // [P][nent] coefficient of every entry at every point
     std::vector<int2> tiles;            // needed (I <= J) tiles, grouped by owning warp
-    int tile_start[9];
+    std::vector<int4> runs;             // [8][nrun] (I, J0, J1, 0)
+    std::vector<int2> runs_out;         // [8][nrun] tile indices of the two products, -1: padding
+    int nrun;
     std::vector<amp_model::GramKey> sig;
     int nent;
 };
@@ -805,11 +807,35 @@ bool build_herk_plan(const amp_model* m, HerkPlan* hp, int pbase = 0, int npts =
     for (int I = 0; I < NT; ++I)
         for (int J = I; J < NT; ++J)
             if (need[(size_t)I * NT + J]) all.push_back(make_int2(I, J));
-    if ((int)all.size() > herk_max_tiles()) return false;
-    // contiguous, equally sized chunks of the row-sorted list: a warp reloads its A fragment only when I changes
     hp->tiles = all;
-    const int n = (int)all.size();
-    for (int w = 0; w <= 8; ++w) hp->tile_start[w] = (int)((long long)n * w / 8);
+    // runs: one row tile with two of its column tiles (three fragment loads feed two DMMAs); dealt to the warps in
+    // contiguous, equally long chunks, padded with dummy runs whose results are dropped
+    std::vector<int4> runs;
+    std::vector<int2> outs;
+    for (size_t i = 0; i < all.size();) {
+        if (i + 1 < all.size() && all[i + 1].x == all[i].x) {
+            runs.push_back(make_int4(all[i].x, all[i].y, all[i + 1].y, 0));
+            outs.push_back(make_int2((int)i, (int)i + 1));
+            i += 2;
+        } else {
+            runs.push_back(make_int4(all[i].x, all[i].y, all[i].y, 0));
+            outs.push_back(make_int2((int)i, -1));
+            i += 1;
+        }
+    }
+    int nrun = ((int)runs.size() + 7) / 8;
+    nrun = (nrun + 1) / 2 * 2;
+    if (nrun < 2) nrun = 2;
+    if (nrun > herk_max_runs()) return false;
+    hp->nrun = nrun;
+    hp->runs.assign((size_t)8 * nrun, make_int4(0, 0, 0, 0));
+    hp->runs_out.assign((size_t)8 * nrun, make_int2(-1, -1));
+    const int per = ((int)runs.size() + 7) / 8;
+    for (size_t i = 0; i < runs.size(); ++i) {
+        const int w = (int)i / per, r = (int)i % per;
+        hp->runs[(size_t)w * nrun + r] = runs[i];
+        hp->runs_out[(size_t)w * nrun + r] = outs[i];
+    }
     return true;
 }
 
@@ -830,7 +856,8 @@ amp_status norm_via_matrix(amp_model* m, const HerkPlan& hp, double* d_out, cuda
     bool hit = gram_hit(m, hp);
     auto al = [](size_t x) { return (x + 255) / 256 * 256; };
     const size_t bE = hp.entries.size() * sizeof(int2), bT = hp.tiles.size() * sizeof(int2), bC = hp.C.size() * sizeof(double2);
-    const size_t oE = 0, oT = al(bE), oC = oT + al(bT), end = oC + al(bC);
+    const size_t bR = hp.runs.size() * sizeof(int4), bRO = hp.runs_out.size() * sizeof(int2);
+    const size_t oE = 0, oT = al(bE), oC = oT + al(bT), oR = oC + al(bC), oRO = oR + al(bR), end = oRO + al(bRO);
     if (end > m->hk_cap) {
         if (m->d_hk) cudaFree(m->d_hk);
         if (m->h_hk) cudaFreeHost(m->h_hk);
@@ -853,6 +880,8 @@ amp_status norm_via_matrix(amp_model* m, const HerkPlan& hp, double* d_out, cuda
     std::memcpy(m->h_hk + oE, hp.entries.data(), bE);
     std::memcpy(m->h_hk + oT, hp.tiles.data(), bT);
     std::memcpy(m->h_hk + oC, hp.C.data(), bC);
+    std::memcpy(m->h_hk + oR, hp.runs.data(), bR);
+    std::memcpy(m->h_hk + oRO, hp.runs_out.data(), bRO);
     CK(cudaMemcpyAsync(m->d_hk, m->h_hk, end, cudaMemcpyHostToDevice, s));
     if (!hit) {
         HerkArgs h{};
@@ -863,13 +892,14 @@ amp_status norm_via_matrix(amp_model* m, const HerkPlan& hp, double* d_out, cuda
         h.b.ncolu = (int)hp.colu.size();
         for (int j = 0; j < h.b.ncolu; ++j) h.b.colu[j] = hp.colu[j];
         h.b.have_z = m->has_z ? 1 : 0;
-        h.tiles = reinterpret_cast<const int2*>(m->d_hk + oT);
-        for (int w = 0; w < 9; ++w) h.tile_start[w] = hp.tile_start[w];
+        h.runs = reinterpret_cast<const int4*>(m->d_hk + oR);
+        h.runs_out = reinterpret_cast<const int2*>(m->d_hk + oRO);
+        h.nrun = hp.nrun;
         h.ntile = ntile;
         h.partial = m->d_gpartial;
         const int grid = batch_grid(d.n);
         CK(launch_herk(h, grid, s));
-        CK(launch_herk_finish(m->d_gpartial, grid, ntile, h.tiles, KP, m->d_gt, m->d_G, s));
+        CK(launch_herk_finish(m->d_gpartial, grid, ntile, reinterpret_cast<const int2*>(m->d_hk + oT), KP, m->d_gt, m->d_G, s));
         m->stat_launches += 3;
         m->gram_sig = hp.sig;
         m->gram_tiles = hp.tiles;

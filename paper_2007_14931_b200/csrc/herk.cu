@@ -13,8 +13,17 @@
 
 namespace amp {
 
-constexpr int HERK_MAXT = 24;   // tiles per warp (8 warps -> up to 192 tiles)
+constexpr int HERK_MAXRUN = 12;   // runs per warp; a run = one row tile I with two column tiles J0, J1 (3 fragment loads, 2 DMMA)
 
+__device__ __forceinline__ double lds_f64(uint32_t addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+
+// The basis tile is built with every event scaled by sqrt(w_j), so G' = sum_j (sqrt(w) b')(sqrt(w) b')^T needs no
+// per-fragment weight and both MMA operands are plain fragment loads of the same tile.
+template <int NRUN>
 __global__ void __launch_bounds__(BT_THREADS, 1) k_herk(const __grid_constant__ HerkArgs h) {
     extern __shared__ __align__(16) double smem[];
     const BatchArgs& a = h.b;
@@ -22,11 +31,20 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_herk(const __grid_constant__ 
     const TileSmem t = carve_tile_smem(smem, KP, a.ncolu);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nang = a.have_z ? BT_NANG : 6;
-    const int t0 = h.tile_start[warp], nt = h.tile_start[warp + 1] - t0;
 
-    double acc[HERK_MAXT][2];
+    double acc[NRUN][2][2];
+    uint32_t offA[NRUN], offB[NRUN][2];   // byte offsets of the fragments' row tiles inside one helicity plane
+    int outidx[NRUN][2];                  // tile index in the partial buffer, -1: padding
 #pragma unroll
-    for (int i = 0; i < HERK_MAXT; ++i) acc[i][0] = acc[i][1] = 0.0;
+    for (int r = 0; r < NRUN; ++r) {
+        const int4 run = h.runs[warp * NRUN + r];   // (I, J0, J1, flags: bit0 J0 real, bit1 J1 real) ; outs in runs_out
+        const int2 ro = h.runs_out[warp * NRUN + r];
+        offA[r] = (uint32_t)(8 * run.x * BT_STRIDE * sizeof(double));
+        offB[r][0] = (uint32_t)(8 * run.y * BT_STRIDE * sizeof(double));
+        offB[r][1] = (uint32_t)(8 * run.z * BT_STRIDE * sizeof(double));
+        outidx[r][0] = ro.x; outidx[r][1] = ro.y;
+        acc[r][0][0] = acc[r][0][1] = acc[r][1][0] = acc[r][1][1] = 0.0;
+    }
 
     const long long ntiles = (a.n + BT_EVENTS - 1) / BT_EVENTS;
     if (tid == 0) {
@@ -36,9 +54,10 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_herk(const __grid_constant__ 
     __syncthreads();
     if (tid == 0 && (long long)blockIdx.x < ntiles) issue_stage(a, blockIdx.x, t.scol, t.sang, t.sw, t.full, nang, true);
     uint32_t parity = 0;
+    const uint32_t bs32 = bsmem_u32(t.Bs) + (uint32_t)(((lane >> 2) * BT_STRIDE + (lane & 3)) * sizeof(double));
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, parity ^= 1) {
         bmbar_wait(t.full, parity);
-        build_basis_tile(a, t, tile, KP, true);
+        build_basis_tile(a, t, tile, KP, true, true);
         __syncthreads();   // basis tile complete, staging consumed: stream the next tile in during the DMMA phase
         if (tid == 0 && tile + gridDim.x < ntiles) issue_stage(a, tile + gridDim.x, t.scol, t.sang, t.sw, t.full, nang, true);
 #pragma unroll 1
@@ -46,30 +65,27 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_herk(const __grid_constant__ 
 #pragma unroll 1
             for (int ks = 0; ks < BT_EVENTS / 4; ++ks) {
                 // fragment element of this lane: basis row (tile row lane/4), event 4 ks + lane%4
-                const double* fb = t.Bs + (size_t)xi * KP * BT_STRIDE + (size_t)(lane >> 2) * BT_STRIDE + 4 * ks + (lane & 3);
-                const double wv = t.ws[4 * ks + (lane & 3)];
-                int lastI = -1;
-                double afr = 0.0;
+                const uint32_t fb = bs32 + (uint32_t)((xi * KP * BT_STRIDE + 4 * ks) * sizeof(double));
 #pragma unroll
-                for (int i = 0; i < HERK_MAXT; ++i) {
-                    if (i < nt) {
-                        const int2 c = h.tiles[t0 + i];   // (row tile I, column tile J), sorted by I within a warp
-                        if (c.x != lastI) { afr = fb[(size_t)8 * c.x * BT_STRIDE] * wv; lastI = c.x; }
-                        const double bfr = fb[(size_t)8 * c.y * BT_STRIDE];
-                        dmma884(acc[i], afr, bfr);
-                    }
+                for (int r = 0; r < NRUN; ++r) {
+                    const double af = lds_f64(fb + offA[r]);
+                    const double b0 = lds_f64(fb + offB[r][0]), b1 = lds_f64(fb + offB[r][1]);
+                    dmma884(acc[r][0], af, b0);
+                    dmma884(acc[r][1], af, b1);
                 }
             }
         }
         __syncthreads();
     }
 #pragma unroll
-    for (int i = 0; i < HERK_MAXT; ++i)
-        if (i < nt) {
-            double* o = h.partial + ((size_t)blockIdx.x * h.ntile + t0 + i) * 64 + 2 * lane;   // C fragment: row lane/4, columns 2 (lane%4) + {0,1}
-            o[0] = acc[i][0];
-            o[1] = acc[i][1];
-        }
+    for (int r = 0; r < NRUN; ++r)
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+            if (outidx[r][c] >= 0) {
+                double* o = h.partial + ((size_t)blockIdx.x * h.ntile + outidx[r][c]) * 64 + 2 * lane;   // C fragment: row lane/4, columns 2 (lane%4) + {0,1}
+                o[0] = acc[r][c][0];
+                o[1] = acc[r][c][1];
+            }
 }
 
 // G'[tile][64] = sum over CTAs of partial[cta][tile][64], CTA order fixed
@@ -117,15 +133,29 @@ __global__ void __launch_bounds__(256) k_quadform(const double* __restrict__ G, 
     }
 }
 
-int herk_max_tiles() { return HERK_MAXT * 8; }
+int herk_max_runs() { return HERK_MAXRUN; }
 
-cudaError_t launch_herk(const HerkArgs& h, int grid, cudaStream_t s) {
+template <int NRUN>
+static cudaError_t launch_herk_n(const HerkArgs& h, int grid, cudaStream_t s) {
     static bool attr_done = false;
     cudaError_t e = cudaSuccess;
-    if (!attr_done) { e = cudaFuncSetAttribute(k_herk, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
+    if (!attr_done) { e = cudaFuncSetAttribute(k_herk<NRUN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
     if (e != cudaSuccess) return e;
-    k_herk<<<grid, BT_THREADS, tile_smem_bytes(h.b.nent, h.b.ncolu), s>>>(h);
+    k_herk<NRUN><<<grid, BT_THREADS, tile_smem_bytes(h.b.nent, h.b.ncolu), s>>>(h);
     return cudaGetLastError();
+}
+
+// h.nrun = runs per warp (the host pads every warp's list to this length)
+cudaError_t launch_herk(const HerkArgs& h, int grid, cudaStream_t s) {
+    switch (h.nrun) {
+        case 1: case 2: return launch_herk_n<2>(h, grid, s);
+        case 3: case 4: return launch_herk_n<4>(h, grid, s);
+        case 5: case 6: return launch_herk_n<6>(h, grid, s);
+        case 7: case 8: return launch_herk_n<8>(h, grid, s);
+        case 9: case 10: return launch_herk_n<10>(h, grid, s);
+        case 11: case 12: return launch_herk_n<12>(h, grid, s);
+    }
+    return cudaErrorInvalidValue;
 }
 
 cudaError_t launch_herk_finish(const double* partial, int ncta, int ntile, const int2* tiles, int KP, double* gt, double* G, cudaStream_t s) {

@@ -128,7 +128,9 @@ static inline size_t tile_smem_bytes(int nent, int ncolu) {
 
 // Basis tile from the staged inputs: thread (part, ev) fills entries part, part+4, ... of event ev for both helicities.
 // Call with all BT_THREADS threads after the staging barrier completed; follow with __syncthreads().
-__device__ __forceinline__ void build_basis_tile(const BatchArgs& a, const TileSmem& t, long long tile, int KP, bool with_w) {
+// scale_sqrt_w: multiply the event's basis by sqrt(w) (Gram kernel) — then ws holds 1 for live events.
+__device__ __forceinline__ void build_basis_tile(const BatchArgs& a, const TileSmem& t, long long tile, int KP, bool with_w,
+                                                 bool scale_sqrt_w = false) {
     const int tid = threadIdx.x;
     const int ev = tid & (BT_EVENTS - 1), part = tid / BT_EVENTS;
     const long long i = tile * BT_EVENTS + ev;          // < npad (npad is a multiple of 512)
@@ -140,6 +142,7 @@ __device__ __forceinline__ void build_basis_tile(const BatchArgs& a, const TileS
         g.cZ = sang[6 * BT_EVENTS + ev]; g.sZ = sang[7 * BT_EVENTS + ev]; g.ct = sang[8 * BT_EVENTS + ev]; g.st = sang[9 * BT_EVENTS + ev];
         g.cpt = sang[10 * BT_EVENTS + ev]; g.spt = sang[11 * BT_EVENTS + ev]; g.ca = sang[12 * BT_EVENTS + ev]; g.sa = sang[13 * BT_EVENTS + ev];
     }
+    const double sc = scale_sqrt_w ? ((i < a.n) ? sqrt(t.sw[ev]) : 0.0) : 1.0;
     for (int e = part; e < a.nent; e += BT_THREADS / BT_EVENTS) {
         const int2 en = a.entries[e];                   // (staged column, code); column -1: empty entry, -2: lineshape == 1
         double2 bp = make_double2(0, 0), bm = bp;
@@ -149,6 +152,7 @@ __device__ __forceinline__ void build_basis_tile(const BatchArgs& a, const TileS
             angular_factor(g, en.y, &gp, &gm);
             bp = cmul(bw, gp);
             bm = cmul(bw, gm);
+            if (scale_sqrt_w) { bp = cscale(sc, bp); bm = cscale(sc, bm); }
         }
         double* r0 = t.Bs + (size_t)(2 * e) * BT_STRIDE + ev;
         r0[0] = bp.x; r0[BT_STRIDE] = bp.y;
