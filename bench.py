@@ -36,6 +36,9 @@ BYTES_PER_EVENT_DATA = 22 * 8
 BYTES_PER_EVENT_NORM = 23 * 8
 FLOP_PER_EVENT = 730.0
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # 148 SMs x 64 DFMA/clk x 2 flop x 1965 MHz
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed `ncu --set full` capture
+# (profiles/): per launch, at the default sizes; None until a capture of the current kernel exists
+TRAFFIC_NCU_BYTES = None
 
 
 def measured_peaks():
@@ -173,13 +176,15 @@ def run_own(args):
         sampler.start()
         time.sleep(0.02)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    launches, t_norm, t_data, t_line = 0, [], [], []
+    launches, t_norm, t_data, t_line, paths = 0, [], [], [], set()
     nll_last = None
     t_wall0 = time.perf_counter()
     ev0.record()
     for s in range(args.warmup, args.warmup + args.steps):
         nll_last = one_step(s)
-        launches += model.last_call_stats()["launches"]
+        st = model.last_call_stats()
+        launches += st["launches"]
+        paths.add(st["norm_path"])
         tm = model.last_call_timing()
         t_norm.append(tm["norm_ms"]); t_data.append(tm["data_ms"]); t_line.append(tm["lineshape_ms"])
     ev1.record()
@@ -204,6 +209,17 @@ def run_own(args):
     norm_ms = float(np.mean(t_norm))
     if args.cfg == 4:
         roof = None
+    elif paths == {4}:
+        # one fused launch per step: lineshapes + combine + both reductions over the data tiles then the norm tiles
+        k_ms = float(np.mean(t_data))
+        nbytes = BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm
+        ach = nbytes / (k_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "k_stream<MODE_FUSED> (the whole step: lineshapes + combine + -log L / normalisation reductions, data then norm tiles)",
+                "achieved": ach, "peak": hbm_peak, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})", "unit": "GB/s",
+                "frac": ach / hbm_peak, "traffic": TRAFFIC_NCU_BYTES,
+                "alu_frac_nominal": FLOP_PER_EVENT * (args.n_data + args.n_norm) / (k_ms * 1e-3) / FP64_PEAK_NOMINAL,
+                "kernel_ms": k_ms, "bytes_per_launch": nbytes, "bytes_per_event": [BYTES_PER_EVENT_DATA, BYTES_PER_EVENT_NORM],
+                "flop_per_event": FLOP_PER_EVENT}
     else:
         ach = BYTES_PER_EVENT_NORM * args.n_norm / (norm_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": "k_stream<MODE_NORM> (fused lineshape + combine + reduce over the norm sample)",

@@ -134,17 +134,26 @@ amp_status amp_set_norm_mode(amp_model* m, int mode);
  * on two successive calls is floating: evaluate it in registers inside the combine kernel, no HBM round
  * trip), 1 = always store columns in the pool, 2 = always evaluate missing columns in registers.        */
 amp_status amp_set_lineshape_mode(amp_model* m, int mode);
-/* How P > 1 points are evaluated: 0 = automatic (one batched DMMA launch per sample when P >= 24, the model has at
- * most 28 couplings and the extended basis fits in shared memory, else as mode 1), 1 = a loop of single-point
- * streaming launches over the stored lineshape columns.                                                  */
+/* How P > 1 points are evaluated: 0 = automatic: a batch whose points 1..P-1 differ from point 0 in few resonances (a
+ * MINUIT-style gradient step: on average <= 3 changed resonances per point) runs the gradient-batch kernel, one fused
+ * launch over data and normalisation events with no lineshape column and no matrix; any other batch with P >= 24, at
+ * most 28 couplings and an extended basis that fits in shared memory runs one dense DMMA launch per sample; else as
+ * mode 1.  1 = a loop of single-point streaming launches over the stored lineshape columns.  2 = as 0 without the
+ * gradient-batch kernel (dense DMMA contraction even for sparse batches).                                        */
 amp_status amp_set_batch_mode(amp_model* m, int mode);
+/* How a P == 1 step with lineshapes in registers and a direct-sum normalisation is launched: 0 = automatic (ONE fused
+ * launch: data tiles, then normalisation tiles, the last thread block forms the NLL), 1 = separate data / normalisation /
+ * reduction launches (per-phase timing, parity tests of the two forms against each other).                       */
+amp_status amp_set_fused_mode(amp_model* m, int mode);
 /* Counters of the last amp_nll / amp_norm_integral call: kernels launched, lineshape columns
- * recomputed (data + norm), which normalisation path ran (1 direct streaming sum, 2 matrix, 3 batched DMMA sum).                         */
+ * recomputed (data + norm), which normalisation path ran (1 direct streaming sum, 2 matrix, 3 batched DMMA sum,
+ * 4 fused single launch, 5 gradient-batch delta kernel).                         */
 amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_recomputed, int* norm_path);
 
 /* Device time [ms] of the phases of the last amp_nll / amp_norm_integral call, from CUDA events recorded on
  * the call's stream: ms4[0] lineshape columns, ms4[1] data-side combine + reduce, ms4[2] normalisation,
- * ms4[3] final reductions and the copy of the result.                                                   */
+ * ms4[3] final reductions and the copy of the result.  After a fused single launch (path 4): ms4[1] = that launch,
+ * the others 0.                                                                                          */
 amp_status amp_last_call_timing(const amp_model* m, double* ms4);
 
 const char* amp_last_error(const amp_model* m);

@@ -167,7 +167,7 @@ enum { MAX_LINE_JOBS = 64 };
 cudaError_t launch_lineshape(const Dataset& d, const LineshapeJob* jobs, int njobs, cudaStream_t s);
 
 // Streaming combine + reduce for one parameter point (a3 + a5, P = 1)
-enum StreamMode { MODE_DATA = 0, MODE_NORM = 1, MODE_EVAL = 2 };
+enum StreamMode { MODE_DATA = 0, MODE_NORM = 1, MODE_EVAL = 2, MODE_FUSED = 3 };   // FUSED: data (sum log S) then norm (sum w S) in one launch + final NLL
 // One resonance as the streaming kernel sees it: the three per-(mass,width) constants of LineConst,
 // its first coupling slot, and either a pool column to read or -1 = evaluate in registers.
 struct ResEntry {
@@ -182,6 +182,15 @@ struct BarrierGroup {
     double r2;
     int first, count;
 };
+// A^R = kN F / (M2 - m2 - i kG G)
+__device__ __forceinline__ double2 bw_from_consts(double kN, double kG, double M2, double m2, double F, double G) {
+    const double MG = kG * G, dre = M2 - m2;
+    const double s = kN * F * fast_rcp(fma(dre, dre, MG * MG));
+    return make_double2(s * dre, s * MG);
+}
+__device__ __forceinline__ double2 bw_from_factors(const ResEntry& e, double m2, double F, double G) {
+    return bw_from_consts(e.kN, e.kG, e.M2, m2, F, G);
+}
 struct StreamArgs {
     ResEntry ent[AMP_MAX_RESONANCES];
     BarrierGroup grp[AMP_MAX_RESONANCES];
@@ -198,10 +207,46 @@ struct StreamArgs {
     double* out;                    // MODE_EVAL: [n] eps_i S_i
     int* flag;
     int mode;
+    // MODE_FUSED: the normalisation sample (second dataset), its partials, and what the last CTA needs to finish the NLL
+    const double* cache2;
+    const double* weight2;
+    long long n2, npad2;
+    double* partial2;               // [grid] sum w S
+    unsigned int* ticket;           // device counter, 0 between launches
+    double* result;                 // [3]: NLL, I, domain flag
+    double sum_log_eff, wsum;
 };
 cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s);
 int stream_grid(long long n, bool have_z, int mode);
+int stream_grid_fused(long long n_data, long long n_norm, bool have_z);
 long long stream_pad(long long n);   // events per column rounded up to whole pipeline tiles
+
+// Gradient batches (P > 1 points that differ from point 0 in a few resonances), see delta.cu.
+// One item = one (point, resonance) change; the items of a point are consecutive, the last one is flagged.
+struct DeltaItem {
+    double2 g[3];       // lineshape unchanged: c(p) - c(0) per helicity (-1, 0, +1); changed: c(p)
+    double2 c0[3];      // couplings of point 0 (used when the lineshape changed)
+    double kN, kG, M2;  // lineshape constants of this point's (mass, width) (used when the lineshape changed)
+    int ent;            // index into StreamArgs::ent: whose BW(0) this item modifies
+    int grp;            // its barrier group (F, G of the event)
+    int J;              // spin of a K*; 256 for a Z
+    int flags;          // bit 0: lineshape changed; bits 1-3: helicities -1, 0, +1 that change; bit 4: last item of its point
+};
+enum { DELTA_MAX_SORTED = 128, DELTA_TILE = 256 };   // points per launch besides point 0 (four 32-point blocks); events per tile
+struct DeltaArgs {
+    StreamArgs a;                   // point 0 as the streaming kernel sees it (cache/weight/n/npad: data; cache2/...: norm)
+    const DeltaItem* items;
+    int nsorted;                    // points in `items` order, padded to a multiple of 32 with empty points
+    const int* point_of_sorted;     // [nsorted] -> point index 1..P-1 of this call, -1: padding
+    int P;
+    double* partial;                // [2][1 + nsorted][stride] per-CTA partials: sum log S (data) and sum w S (norm); row 0 = point 0
+    int stride;
+    double* result;                 // [2 P + 1]: NLL[P], I[P], domain flag
+    int want_nll;
+};
+cudaError_t launch_delta(const DeltaArgs& d, int grid, cudaStream_t s);
+int delta_grid(long long n_data, long long n_norm);
+bool delta_fits(int nent, int ngrp);
 
 // Batched combine (P > 1) on the FP64 tensor cores, see batch.cu
 enum { BATCH_NKT = 14, BATCH_POINTS = 128, BATCH_MAX_COLS = 48 };   // dense k-tiles (2K <= 56 realified rows) and points per launch

@@ -52,6 +52,7 @@ struct amp_model {
     double* d_sums = nullptr;      // [2 * AMP_MAX_POINTS]
     double* d_result = nullptr;    // [2 * AMP_MAX_POINTS]
     int* d_flag = nullptr;
+    unsigned int* d_ticket = nullptr;   // last-CTA ticket of the fused single-launch step (0 between launches)
     double* h_pinned = nullptr;    // [2 * AMP_MAX_POINTS + 2]
 
     // batched (P > 1) plan buffers: coefficient fragments, basis entries, sparse items
@@ -80,6 +81,11 @@ struct amp_model {
     int stat_launches = 0, stat_columns = 0, stat_norm_path = 0, stat_batched = 0, stat_gram_built = 0;
     cudaEvent_t ev[5]{};           // phase boundaries of the last evaluation (amp_last_call_timing)
     bool ev_valid = false;
+    bool fused_valid = false;      // the last evaluation was the fused single launch: ev[0], ev[1] bracket it
+    bool use_delta = false;        // P > 1 and the points are sparse changes of point 0: gradient-batch kernel (delta.cu)
+    std::vector<DeltaItem> delta_items;       // items of points 1..P-1, point after point
+    std::vector<int> delta_first;             // [P]: first item of point p (p >= 1), delta_first[P] = total
+    int fused_mode = 0;            // 0: P == 1 steps with floating lineshapes run as one fused launch; 1: separate launches
     std::string err;
 };
 
@@ -256,8 +262,11 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { delete m; return AMP_ERR_CUDA; }
     cudaError_t e = cudaMalloc(&m->d_partial, sizeof(double) * 2 * AMP_MAX_POINTS * PARTIAL_STRIDE);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_sums, sizeof(double) * 2 * AMP_MAX_POINTS);
-    if (e == cudaSuccess) e = cudaMalloc(&m->d_result, sizeof(double) * 2 * AMP_MAX_POINTS);
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_result, sizeof(double) * (2 * AMP_MAX_POINTS + 2));
     if (e == cudaSuccess) e = cudaMalloc(&m->d_flag, sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_ticket, sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(m->d_ticket, 0, sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(m->d_flag, 0, sizeof(int));
     if (e == cudaSuccess) e = cudaMallocHost(&m->h_pinned, sizeof(double) * (2 * AMP_MAX_POINTS + 2));
     for (int i = 0; i < 5 && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ev[i]);
     if (e != cudaSuccess) { amp_model_destroy(m); return e == cudaErrorMemoryAllocation ? AMP_ERR_NOMEM : AMP_ERR_CUDA; }
@@ -273,6 +282,7 @@ amp_status amp_model_destroy(amp_model* m) {
     if (m->d_sums) cudaFree(m->d_sums);
     if (m->d_result) cudaFree(m->d_result);
     if (m->d_flag) cudaFree(m->d_flag);
+    if (m->d_ticket) cudaFree(m->d_ticket);
     if (m->h_pinned) cudaFreeHost(m->h_pinned);
     if (m->d_plan) cudaFree(m->d_plan);
     if (m->h_plan) cudaFreeHost(m->h_plan);
@@ -307,8 +317,14 @@ amp_status amp_set_norm_mode(amp_model* m, int mode) {
 }
 
 amp_status amp_set_batch_mode(amp_model* m, int mode) {
-    if (!m || mode < 0 || mode > 1) return AMP_ERR_INVALID;
+    if (!m || mode < 0 || mode > 2) return AMP_ERR_INVALID;
     m->batch_mode = mode;
+    return AMP_OK;
+}
+
+amp_status amp_set_fused_mode(amp_model* m, int mode) {
+    if (!m || mode < 0 || mode > 1) return AMP_ERR_INVALID;
+    m->fused_mode = mode;
     return AMP_OK;
 }
 
@@ -328,6 +344,12 @@ amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_r
 
 amp_status amp_last_call_timing(const amp_model* m, double* ms4) {
     if (!m || !ms4) return AMP_ERR_INVALID;
+    if (m->fused_valid) {   // one launch: everything is reported as the combine phase of both samples
+        float t = 0;
+        if (cudaEventElapsedTime(&t, m->ev[0], m->ev[1]) != cudaSuccess) return AMP_ERR_CUDA;
+        ms4[0] = 0; ms4[1] = t; ms4[2] = 0; ms4[3] = 0;
+        return AMP_OK;
+    }
     if (!m->ev_valid) return AMP_ERR_STATE;
     for (int i = 0; i < 4; ++i) {
         float t = 0;
@@ -365,6 +387,69 @@ amp_status ensure_pool(amp_model* m, int need) {
     return AMP_OK;
 }
 
+// Gradient-batch structure: for every point p >= 1 the resonances whose couplings or (mass, width) differ from point 0.
+// False if the batch is not a sparse change of point 0 (too many items) or touches what the kernel does not carry
+// (a constant term's coupling, more points than its blocks hold is handled by chunking in evaluate()).
+bool build_delta_items(amp_model* m) {
+    const int P = m->P, R = m->R, K = m->K;
+    m->delta_items.clear();
+    m->delta_first.assign(P + 1, 0);
+    if (P < 2) return false;
+    int nent = 0, ngrp = 0;
+    {
+        std::vector<std::pair<int, double>> seen;   // (kind * 8 + J, radius) = one barrier group
+        for (int r = 0; r < R; ++r) {
+            if (m->res[r].kind == AMP_CONST) continue;
+            ++nent;
+            const std::pair<int, double> key(m->res[r].kind * 8 + m->res[r].J, m->res[r].radius);
+            if (std::find(seen.begin(), seen.end(), key) == seen.end()) seen.push_back(key);
+        }
+        ngrp = (int)seen.size();
+    }
+    if (!delta_fits(nent, ngrp)) return false;
+    const size_t cap = (size_t)3 * (P - 1) + 8;   // beyond ~3 changed resonances per point the dense contraction is the better form
+    for (int p = 1; p < P; ++p) {
+        m->delta_first[p] = (int)m->delta_items.size();
+        const size_t first = m->delta_items.size();
+        for (int r = 0; r < R; ++r) {
+            const amp_resonance& rs = m->res[r];
+            const int ns = (rs.kind == AMP_Z || (rs.kind == AMP_KSTAR && rs.J >= 1)) ? 3 : 1;
+            const double* c0 = &m->couplings[((size_t)0 * K + m->slot0[r]) * 2];
+            const double* cp = &m->couplings[((size_t)p * K + m->slot0[r]) * 2];
+            bool dc[3] = {false, false, false}, anyc = false;
+            for (int j = 0; j < ns; ++j) { dc[j] = cp[2 * j] != c0[2 * j] || cp[2 * j + 1] != c0[2 * j + 1]; anyc |= dc[j]; }
+            if (rs.kind == AMP_CONST) { if (anyc) return false; continue; }
+            const double* mw0 = &m->mw[((size_t)0 * R + r) * 2];
+            const double* mwp = &m->mw[((size_t)p * R + r) * 2];
+            const bool ls = mwp[0] != mw0[0] || mwp[1] != mw0[1];
+            if (!anyc && !ls) continue;
+            DeltaItem it{};
+            it.ent = r;   // resonance index for now; evaluate() maps it to the kernel's entry / group numbering
+            it.grp = 0;
+            it.J = rs.kind == AMP_Z ? 256 : rs.J;
+            it.flags = ls ? 1 : 0;
+            for (int j = 0; j < ns; ++j) {
+                const int l = ns == 3 ? j : 1;   // helicity index -1, 0, +1 -> 0, 1, 2
+                const bool nz = cp[2 * j] != 0.0 || cp[2 * j + 1] != 0.0 || c0[2 * j] != 0.0 || c0[2 * j + 1] != 0.0;
+                if (ls ? nz : dc[j]) it.flags |= 2 << l;
+                it.c0[l] = make_double2(c0[2 * j], c0[2 * j + 1]);
+                it.g[l] = ls ? make_double2(cp[2 * j], cp[2 * j + 1]) : make_double2(cp[2 * j] - c0[2 * j], cp[2 * j + 1] - c0[2 * j + 1]);
+            }
+            if (ls) {
+                LineConst lc;
+                make_line_const(m, r, mwp[0], mwp[1], &lc);
+                it.kN = lc.kN; it.kG = lc.kG; it.M2 = lc.M2;
+            }
+            m->delta_items.push_back(it);
+            if (m->delta_items.size() > cap) return false;
+        }
+        if (m->delta_items.size() == first) m->delta_items.push_back(DeltaItem{});   // identical to point 0: an empty item
+        m->delta_items.back().flags |= 16;
+    }
+    m->delta_first[P] = (int)m->delta_items.size();
+    return true;
+}
+
 }  // namespace
 
 extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_couplings, const double* h_mass_width) {
@@ -392,9 +477,12 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
     // equal those of the previous call (lineshapes are not moving: M is built once, every later call is O(K^2)), or a
     // large batch of points (one Gram pass instead of one pass per point).  Otherwise the direct sum is cheaper.
     const bool mw_same = P == 1 && m->prev_mw.size() == m->mw.size() && std::equal(m->mw.begin(), m->mw.end(), m->prev_mw.begin());
-    m->want_matrix = m->norm_mode == 2 || (m->norm_mode == 0 && (P == 1 ? mw_same : (P >= 24 && m->batch_mode == 0)));
+    m->want_matrix = m->norm_mode == 2 || (m->norm_mode == 0 && (P == 1 ? mw_same : (P >= 24 && m->batch_mode != 1)));
     if (P == 1) m->prev_mw = m->mw; else m->prev_mw.clear();
-    m->stream_inline = P == 1 && m->lineshape_mode != 1;
+    // P > 1: a batch whose points are sparse changes of point 0 (a gradient step) runs the delta kernel: no column, no matrix
+    m->use_delta = P > 1 && m->batch_mode == 0 && m->lineshape_mode != 1 && m->norm_mode != 2 && build_delta_items(m);
+    if (m->use_delta) m->want_matrix = false;
+    m->stream_inline = (P == 1 || m->use_delta) && m->lineshape_mode != 1;
 
     // distinct (resonance, mass, width) keys of this call
     struct Key { int r; double mass, width; };
@@ -498,7 +586,7 @@ amp_status refresh_columns(amp_model* m, Dataset& d, bool is_norm, cudaStream_t 
 
 // Arguments of the streaming kernel for point p on dataset d: resonances grouped by spin, then by
 // radius (a barrier group shares its Blatt-Weisskopf factors and momentum powers).
-void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, StreamArgs* a) {
+void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, StreamArgs* a, int* ent_of_res = nullptr, int* grp_of_res = nullptr) {
     std::memset(a, 0, sizeof(*a));
     int t = 0, g = 0;
     auto add_groups = [&](int kind, int J) {
@@ -513,6 +601,7 @@ void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, Str
                 done[r2] = 1;
                 LineConst lc;
                 make_line_const(m, r2, m->mw[((size_t)p * m->R + r2) * 2], m->mw[((size_t)p * m->R + r2) * 2 + 1], &lc);
+                if (ent_of_res) { ent_of_res[r2] = t; grp_of_res[r2] = g - 1; }
                 ResEntry& e = a->ent[t++];
                 e.kN = lc.kN; e.kG = lc.kG; e.M2 = lc.M2;
                 const double* cp = &m->couplings[((size_t)p * m->K + m->slot0[r2]) * 2];
@@ -921,8 +1010,97 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
     m->stat_norm_path = 1;
     amp_status st = ensure_pool(m, 0);
     if (st != AMP_OK) return st;
-    CK(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
     m->ev_valid = false;
+    if (m->use_delta) {
+        // Gradient batch: one fused launch per chunk of <= 128 points besides point 0 (delta.cu)
+        int ent_of_res[AMP_MAX_RESONANCES], grp_of_res[AMP_MAX_RESONANCES];
+        DeltaArgs d{};
+        fill_stream_args(m, m->data, 0, MODE_FUSED, &d.a, ent_of_res, grp_of_res);
+        d.a.cache2 = m->norm.cache; d.a.weight2 = m->norm.weight; d.a.n2 = m->norm.n; d.a.npad2 = m->norm.npad;
+        d.a.ticket = m->d_ticket;
+        d.a.sum_log_eff = m->data.loaded ? m->data.wsum : 0.0;
+        d.a.wsum = m->norm.wsum;
+        if (!want_nll) { d.a.n = 0; }
+        d.P = P;
+        d.partial = m->d_partial;
+        d.stride = PARTIAL_STRIDE;
+        d.result = m->d_result;
+        d.want_nll = want_nll ? 1 : 0;
+        const size_t need = m->delta_items.size() * sizeof(DeltaItem) + (size_t)(P + 32) * (sizeof(DeltaItem) + sizeof(int)) + 4096;
+        if (need > m->plan_cap) {
+            if (m->d_plan) cudaFree(m->d_plan);
+            if (m->h_plan) cudaFreeHost(m->h_plan);
+            m->d_plan = m->h_plan = nullptr;
+            m->plan_cap = 0;
+            CK(cudaMalloc(&m->d_plan, need * 2));
+            CK(cudaMallocHost(&m->h_plan, need * 2));
+            m->plan_cap = need * 2;
+        }
+        CK(cudaEventRecord(m->ev[0], s));
+        size_t off = 0;
+        for (int p0 = 1; p0 < P; p0 += DELTA_MAX_SORTED) {
+            const int np = std::min((int)DELTA_MAX_SORTED, P - p0), nsorted = (np + 31) / 32 * 32;
+            DeltaItem* hi = reinterpret_cast<DeltaItem*>(m->h_plan + off);
+            const int i0 = m->delta_first[p0], i1 = m->delta_first[p0 + np];
+            int ni = 0;
+            for (int i = i0; i < i1; ++i) {
+                hi[ni] = m->delta_items[i];
+                if (hi[ni].flags & 0xe) { const int r = hi[ni].ent; hi[ni].ent = ent_of_res[r]; hi[ni].grp = grp_of_res[r]; }
+                ++ni;
+            }
+            for (int q = np; q < nsorted; ++q) { hi[ni] = DeltaItem{}; hi[ni].flags = 16; ++ni; }   // padding points
+            const size_t bI = ((size_t)ni * sizeof(DeltaItem) + 255) / 256 * 256;
+            int* hp = reinterpret_cast<int*>(m->h_plan + off + bI);
+            for (int q = 0; q < nsorted; ++q) hp[q] = q < np ? p0 + q : -1;
+            const size_t bP = ((size_t)nsorted * sizeof(int) + 255) / 256 * 256;
+            CK(cudaMemcpyAsync(m->d_plan + off, m->h_plan + off, bI + bP, cudaMemcpyHostToDevice, s));
+            d.items = reinterpret_cast<const DeltaItem*>(m->d_plan + off);
+            d.point_of_sorted = reinterpret_cast<const int*>(m->d_plan + off + bI);
+            d.nsorted = nsorted;
+            CK(launch_delta(d, delta_grid(d.a.n, d.a.n2), s));
+            m->stat_launches++;
+            off += bI + bP;
+        }
+        CK(cudaEventRecord(m->ev[1], s));
+        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (2 * P + 1), cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));
+        m->stat_norm_path = 5;
+        m->fused_valid = true;
+        bool bad = m->h_pinned[2 * P] != 0.0;
+        for (int p = 0; p < P; ++p) {
+            if (h_nll) { h_nll[p] = m->h_pinned[p]; bad |= !std::isfinite(h_nll[p]); }
+            if (h_I) { h_I[p] = m->h_pinned[P + p]; bad |= !(h_I[p] > 0) || !std::isfinite(h_I[p]); }
+        }
+        if (bad) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
+        return AMP_OK;
+    }
+    if (want_nll && P == 1 && m->stream_inline && !m->want_matrix && m->fused_mode == 0) {
+        // The whole step in ONE launch: lineshapes in registers, combine and both reductions over the data tiles and
+        // then the normalisation tiles of one persistent grid; the last CTA forms the NLL (stream.cu, MODE_FUSED).
+        StreamArgs a;
+        fill_stream_args(m, m->data, 0, MODE_FUSED, &a);
+        a.partial = m->d_partial;
+        a.partial2 = m->d_partial + PARTIAL_STRIDE;
+        a.cache2 = m->norm.cache; a.weight2 = m->norm.weight; a.n2 = m->norm.n; a.npad2 = m->norm.npad;
+        a.ticket = m->d_ticket;
+        a.result = m->d_result;
+        a.sum_log_eff = m->data.wsum;
+        a.wsum = m->norm.wsum;
+        CK(cudaEventRecord(m->ev[0], s));
+        CK(launch_stream(a, stream_grid_fused(m->data.n, m->norm.n, m->has_z), s));
+        CK(cudaEventRecord(m->ev[1], s));
+        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 3, cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));
+        m->stat_launches = 1;
+        m->stat_norm_path = 4;
+        m->fused_valid = true;
+        h_nll[0] = m->h_pinned[0];
+        if (h_I) h_I[0] = m->h_pinned[1];
+        if (m->h_pinned[2] != 0.0 || !std::isfinite(h_nll[0])) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
+        return AMP_OK;
+    }
+    m->fused_valid = false;
+    CK(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
     CK(cudaEventRecord(m->ev[0], s));
     m->stat_gram_built = 0;
     HerkPlan hp;
@@ -938,7 +1116,7 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
     // P > 1: one DMMA launch per dataset and chunk of <= 128 points, if the model and the points fit its plan
     std::vector<BatchPlan> plans;
     // (below ~24 points the streaming kernel, which shares the angular structure, is cheaper per point)
-    bool batched = P >= 24 && m->batch_mode == 0;
+    bool batched = P >= 24 && m->batch_mode != 1;
     if (batched) {
         for (int p0 = 0; p0 < P && batched; p0 += BATCH_POINTS) {
             plans.emplace_back();

@@ -25,12 +25,6 @@
 
 namespace amp {
 
-// A^R = kN F / (M2 - m2 - i kG G)
-__device__ __forceinline__ double2 bw_from_factors(const ResEntry& e, double m2, double F, double G) {
-    const double MG = e.kG * G, dre = e.M2 - m2;
-    const double s = e.kN * F * fast_rcp(fma(dre, dre, MG * MG));
-    return make_double2(s * dre, s * MG);
-}
 
 // E consecutive events per thread: each cache column is read with one 16-byte (E = 2) load per thread
 // (a warp covers 512 contiguous bytes), the group / resonance constants and couplings are fetched once
@@ -90,13 +84,41 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  : "memory");
 }
 // Columns [c0, c1) of the cache (and, if with_w, the weight column into slot wslot) of tile `tile` -> stage.
-__device__ __forceinline__ void issue_cols(const StreamArgs& a, long long tile, double* stage, uint64_t* bar, int c0, int c1, bool with_w,
-                                           int wslot) {
+__device__ __forceinline__ void issue_cols(const double* cache, const double* weight, long long npad, long long tile, double* stage,
+                                           uint64_t* bar, int c0, int c1, bool with_w, int wslot) {
     const uint32_t col_bytes = TILE * sizeof(double);
     mbar_expect_tx(bar, col_bytes * (c1 - c0 + (with_w ? 1 : 0)));
 #pragma unroll 1
-    for (int c = c0; c < c1; ++c) bulk_g2s(stage + c * TILE, a.cache + (size_t)c * a.npad + tile * TILE, col_bytes, bar);
-    if (with_w) bulk_g2s(stage + wslot * TILE, a.weight + tile * TILE, col_bytes, bar);
+    for (int c = c0; c < c1; ++c) bulk_g2s(stage + c * TILE, cache + (size_t)c * npad + tile * TILE, col_bytes, bar);
+    if (with_w) bulk_g2s(stage + wslot * TILE, weight + tile * TILE, col_bytes, bar);
+}
+// MODE_FUSED walks one tile space: the data tiles first, then the normalisation tiles (second dataset of StreamArgs).
+template <int MODE>
+__device__ __forceinline__ void issue_tile(const StreamArgs& a, long long ntd, long long tile, double* stage, uint64_t* bar, int c0, int c1,
+                                           bool region_has_w, int wslot) {
+    if (MODE == MODE_FUSED && tile >= ntd)
+        issue_cols(a.cache2, a.weight2, a.npad2, tile - ntd, stage, bar, c0, c1, region_has_w, wslot);
+    else
+        issue_cols(a.cache, a.weight, a.npad, tile, stage, bar, c0, c1, region_has_w && MODE != MODE_DATA && MODE != MODE_FUSED, wslot);
+}
+
+// fixed-order block sum: xor-shuffle tree, then the 8 warp values in warp order; result valid in thread 0
+__device__ __forceinline__ double block_sum(double v, double* sm) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();   // sm may still be read from a previous use
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int wv = 0; wv < 8; ++wv) t += sm[wv];
+    return t;
+}
+// sum of the per-CTA partials in the order k_finalize uses (thread t adds b = t, t + 256, ...; fixed tree): every thread calls it
+__device__ __forceinline__ double partial_sum(const double* p, int n, double* sm) {
+    double v = 0.0;
+    for (int b = threadIdx.x; b < n; b += THREADS) v += __ldcg(p + b);
+    return block_sum(v, sm);
 }
 
 // One resonance: lineshape (from its pool column or in registers) times its couplings, added to U_l.
@@ -161,7 +183,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     // therefore has a whole iteration to arrive, and two CTAs (16 warps) fit on an SM.
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int ncache = have_z ? NCOL_ALL : NCOL_K;
-    const bool with_w = MODE != MODE_DATA;
+    const bool with_w = MODE != MODE_DATA;   // the K* region carries the weight column (MODE_FUSED: only for normalisation tiles)
     double* stage = reinterpret_cast<double*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)(ncache + 1) * TILE * sizeof(double));   // [0]: K* region, [1]: Z region
     if (threadIdx.x == 0) {
@@ -170,15 +192,28 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    const long long ntiles = (a.n + TILE - 1) / TILE;   // npad is a multiple of TILE: every tile is fully backed by memory
+    // npad is a multiple of TILE: every tile is fully backed by memory
+    const long long ntd = (a.n + TILE - 1) / TILE;                                              // tiles of the first dataset
+    const long long ntiles = MODE == MODE_FUSED ? ntd + (a.n2 + TILE - 1) / TILE : ntd;
     if (threadIdx.x == 0 && (long long)blockIdx.x < ntiles) {
-        issue_cols(a, blockIdx.x, stage, &full[0], 0, NCOL_K, with_w, ncache);
-        if (have_z) issue_cols(a, blockIdx.x, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
+        issue_tile<MODE>(a, ntd, blockIdx.x, stage, &full[0], 0, NCOL_K, true, ncache);
+        if (have_z) issue_tile<MODE>(a, ntd, blockIdx.x, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
     }
+    __shared__ double sm[8];
     uint32_t parity = 0;
+    bool in_norm = false;   // MODE_FUSED: this CTA has passed from the data tiles to the normalisation tiles
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, parity ^= 1) {
         const bool has_next = tile + gridDim.x < ntiles;
-        const long long i0 = tile * TILE + threadIdx.x * E;   // first of the E events of this thread
+        const bool is_norm = MODE == MODE_FUSED ? tile >= ntd : MODE == MODE_NORM;
+        if (MODE == MODE_FUSED && is_norm && !in_norm) {   // sum log S of this CTA's data tiles is complete
+            const double t = block_sum(acc, sm);
+            if (threadIdx.x == 0) a.partial[blockIdx.x] = t;
+            acc = 0.0;
+            in_norm = true;
+        }
+        const long long lt = (MODE == MODE_FUSED && is_norm) ? tile - ntd : tile;
+        const long long nlive = (MODE == MODE_FUSED && is_norm) ? a.n2 : a.n;
+        const long long i0 = lt * TILE + threadIdx.x * E;     // first of the E events of this thread
         mbar_wait(&full[0], parity);
         const Ev m2 = load_col(stage, C_M2), invm = load_col(stage, C_INVM);
         const Ev q = load_col(stage, C_Q), pB = load_col(stage, C_PB);
@@ -186,9 +221,9 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         const Ev cpsi = load_col(stage, C_CPSI), spsi = load_col(stage, C_SPSI);
         const Ev cphi = load_col(stage, C_CPHI), sphi = load_col(stage, C_SPHI);
         Ev w;
-        if (with_w) w = load_col(stage, ncache);
+        if (MODE == MODE_FUSED ? is_norm : with_w) w = load_col(stage, ncache);
         __syncthreads();   // K* region consumed by every thread: stream the next tile into it
-        if (threadIdx.x == 0 && has_next) issue_cols(a, tile + gridDim.x, stage, &full[0], 0, NCOL_K, with_w, ncache);
+        if (threadIdx.x == 0 && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[0], 0, NCOL_K, true, ncache);
 
         double2 V0[E], Vp[E], Vm[E];
 #pragma unroll
@@ -231,7 +266,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
             const Ev cpt = load_col(stage, C_CPT), spt = load_col(stage, C_SPT);
             const Ev ca = load_col(stage, C_CA), sa = load_col(stage, C_SA);
             __syncthreads();   // Z region consumed: refill it with the next tile
-            if (threadIdx.x == 0 && has_next) issue_cols(a, tile + gridDim.x, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
+            if (threadIdx.x == 0 && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
             double2 Um[E], U0[E], Up[E];
 #pragma unroll
             for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0);
@@ -253,10 +288,10 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const double S = fma(Ap[e].x, Ap[e].x, fma(Ap[e].y, Ap[e].y, fma(Am[e].x, Am[e].x, Am[e].y * Am[e].y)));
-            const bool live = i0 + e < a.n;   // the last thread may hold padding events (weight 0)
-            if (MODE == MODE_DATA) {
+            const bool live = i0 + e < nlive;   // the last thread may hold padding events (weight 0)
+            if (MODE == MODE_DATA || (MODE == MODE_FUSED && !is_norm)) {
                 if (live) { bad |= !(S > 0.0) || !isfinite(S); acc += log(S); }
-            } else if (MODE == MODE_NORM) {
+            } else if (MODE == MODE_NORM || MODE == MODE_FUSED) {
                 if (live) { bad |= !isfinite(S); acc = fma(w.v[e], S, acc); }
             } else {
                 if (live) a.out[i0 + e] = w.v[e] * S;
@@ -265,15 +300,34 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     }
     if (MODE == MODE_EVAL) return;
     if (bad) atomicOr(a.flag, 2);
-    __shared__ double sm[8];
-#pragma unroll
-    for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = acc;
-    __syncthreads();
+    {
+        const double t = block_sum(acc, sm);
+        if (threadIdx.x == 0) {
+            if (MODE == MODE_FUSED && !in_norm) { a.partial[blockIdx.x] = t; a.partial2[blockIdx.x] = 0.0; }   // this CTA saw data tiles only
+            else (MODE == MODE_FUSED ? a.partial2 : a.partial)[blockIdx.x] = t;
+        }
+    }
+    if (MODE != MODE_FUSED) return;
+    // The last CTA to finish (integer ticket) adds the per-CTA partials in a fixed order and forms the NLL: the result
+    // does not depend on which CTA that is, so it stays bit-reproducible; no second launch, no host round trip.
+    __shared__ bool s_last;
     if (threadIdx.x == 0) {
-        double t = 0.0;
-        for (int wv = 0; wv < 8; ++wv) t += sm[wv];
-        a.partial[blockIdx.x] = t;
+        __threadfence();
+        s_last = atomicAdd(a.ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    const double slog = partial_sum(a.partial, gridDim.x, sm);
+    const double swS = partial_sum(a.partial2, gridDim.x, sm);
+    if (threadIdx.x == 0) {
+        const double I = swS / a.wsum;
+        double v = -(slog + a.sum_log_eff) + (double)a.n * log(I);
+        if (!isfinite(v) || !(I > 0.0)) v = INFINITY;
+        a.result[0] = v;
+        a.result[1] = I;
+        a.result[2] = (double)atomicExch(a.flag, 0);   // domain flag of this call, cleared for the next one
+        *a.ticket = 0u;
     }
 }
 
@@ -293,6 +347,11 @@ int stream_grid(long long n, bool have_z, int mode) {
     return (int)(ntiles < 1 ? 1 : (ntiles > cap ? cap : ntiles));
 }
 
+int stream_grid_fused(long long n1, long long n2, bool have_z) {
+    const long long t1 = (n1 + TILE - 1) / TILE, t2 = (n2 + TILE - 1) / TILE;
+    return stream_grid((t1 + t2) * TILE, have_z, MODE_FUSED);
+}
+
 long long stream_pad(long long n) { return (n + TILE - 1) / TILE * TILE; }
 
 template <class SH>
@@ -309,6 +368,7 @@ static cudaError_t launch_shape(const StreamArgs& a, int grid, cudaStream_t s) {
     switch (a.mode) {
         case MODE_DATA: AMP_LAUNCH(MODE_DATA) break;
         case MODE_NORM: AMP_LAUNCH(MODE_NORM) break;
+        case MODE_FUSED: AMP_LAUNCH(MODE_FUSED) break;
         default: AMP_LAUNCH(MODE_EVAL) break;
     }
 #undef AMP_LAUNCH

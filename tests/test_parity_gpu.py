@@ -161,6 +161,16 @@ def test_nll_matches_oracle_full_config(cfg):
     assert abs(nll - ref_nll[0]) < RTOL_NLL * abs(ref_nll[0]), (nll, ref_nll[0])
     # bitwise reproducible
     assert Mg.nll()[0] == nll
+    # the default P = 1 step is ONE fused launch (data tiles, norm tiles, last-block NLL); the separate-launch form agrees
+    st = Mg.last_call_stats()
+    assert st["norm_path"] == 4 and st["launches"] == 1
+    Mg.set_fused_mode(1)
+    nll_sep = Mg.nll()[0]
+    st = Mg.last_call_stats()
+    assert st["norm_path"] == 1 and st["launches"] > 1
+    assert abs(nll_sep - nll) < 1e-13 * abs(nll)
+    assert abs(nll_sep - ref_nll[0]) < RTOL_NLL * abs(ref_nll[0])
+    Mg.set_fused_mode(0)
     if cfg == 2:   # Z mass and width float (configs[2])
         mw = W.step_mass_width(2, 1)
         Mg.set_params(c, mw[None])
@@ -195,9 +205,31 @@ def test_nll_batched_points_small():
     nll = Mg.nll()
     ref, refI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
     assert nll.shape == (121,)
-    assert Mg.last_call_stats()["norm_path"] == 2            # batched DMMA combine on the data, matrix M for the integrals
+    st = Mg.last_call_stats()
+    assert st["norm_path"] == 5 and st["launches"] == 1     # gradient-batch kernel: one fused launch, no columns, no matrix
+    assert st["columns_recomputed"] == 0
     assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
-    # the same batch with the normalisation as a direct DMMA sum over the norm events
+    assert np.array_equal(Mg.nll(), nll)                     # bit-reproducible
+    I = Mg.norm_integral()
+    assert Mg.last_call_stats()["norm_path"] == 5
+    assert np.max(np.abs(I - refI) / refI) < 1e-12
+    # the finite differences themselves (what MINUIT uses) agree: compare NLL(p) - NLL(0)
+    d, dref = nll[1:] - nll[0], ref[1:] - ref[0]
+    assert np.max(np.abs(d - dref)) < 1e-9 * abs(ref[0])
+    # per-event density of a perturbed point (lineshapes in registers)
+    for p in (0, 5, 97, 120):
+        v = Mg.eval_events(p).cpu().numpy()
+        res2 = [(r[0], r[1], mws[p, i, 0], mws[p, i, 1], r[4]) for i, r in enumerate(W.resonances(cfg))]
+        vref = O.Model(W.DECAY, res2).eval_events(cs[p], x, eff)
+        assert np.max(np.abs(v - vref) / vref) < RTOL_EVENT
+    # the same batch as the dense DMMA contraction on the data and the matrix M for the integrals
+    Mg.set_batch_mode(2)
+    Mg.set_params(cs, mws)
+    nll_dense = Mg.nll()
+    assert Mg.last_call_stats()["norm_path"] == 2
+    assert np.max(np.abs(nll_dense - ref) / np.abs(ref)) < RTOL_NLL
+    assert np.max(np.abs(nll_dense - nll) / np.abs(nll)) < 1e-12
+    # ... with the normalisation as a direct DMMA sum over the norm events
     Mg.set_norm_mode(1)
     Mg.set_params(cs, mws)
     nll_direct = Mg.nll()
@@ -205,8 +237,6 @@ def test_nll_batched_points_small():
     assert np.max(np.abs(nll_direct - ref) / np.abs(ref)) < RTOL_NLL
     assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12
     Mg.set_norm_mode(0)
-    Mg.set_params(cs, mws)
-    assert np.max(np.abs(Mg.nll() - nll) / np.abs(nll)) < 1e-13
     # the loop of single-point streaming launches gives the same numbers
     Mg.set_batch_mode(1)
     Mg.set_params(cs, mws)
@@ -214,11 +244,51 @@ def test_nll_batched_points_small():
     assert Mg.last_call_stats()["norm_path"] == 1
     assert np.max(np.abs(nll_seq - nll) / np.abs(nll)) < 1e-12
     Mg.set_batch_mode(0)
-    I = Mg.norm_integral()
-    assert np.max(np.abs(I - refI) / refI) < 1e-12
-    # the finite differences themselves (what MINUIT uses) agree: compare NLL(p) - NLL(0)
-    d, dref = nll[1:] - nll[0], ref[1:] - ref[0]
-    assert np.max(np.abs(d - dref)) < 1e-9 * abs(ref[0])
+
+
+def test_delta_batches_general():
+    """gradient-batch kernel beyond the cfg 4 pattern: ragged point counts (1, 31, 32, 33, 129, 200 points besides point 0,
+    i.e. partial blocks and two launches), points equal to point 0, points that change two resonances at once, a K*-only
+    model, and a dense random batch that must fall back to the DMMA contraction."""
+    rng = np.random.default_rng(5)
+    for cfg in (2, 1):
+        Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+        x, eff, xn, wn = make_inputs(cfg, 3001, 7013)
+        Mg.load_events(dev(x), dev(eff))
+        Mg.load_norm(dev(xn), dev(wn))
+        c0 = W.couplings(cfg)
+        mw0 = np.array([[r[2], r[3]] for r in W.resonances(cfg)])
+        K, R = len(c0), len(mw0)
+        slots = W.slot_table(W.resonances(cfg))
+        for P in (2, 32, 33, 34, 130, 201):
+            cs, mws = np.tile(c0, (P, 1)), np.tile(mw0, (P, 1, 1))
+            for p in range(1, P):
+                kind = p % 5
+                if kind == 0:
+                    continue                                   # identical to point 0
+                k = rng.integers(K)
+                cs[p, k] *= 1 + 0.3 * rng.uniform(-1, 1) + 0.2j * rng.uniform(-1, 1)
+                if kind >= 3:                                  # a second resonance: its mass and width
+                    r = rng.integers(R)
+                    mws[p, r] *= 1 + 0.01 * rng.uniform(-1, 1, 2)
+                if kind == 4:                                  # ... and a coupling of that same resonance
+                    ks = [i for i, (rr, _l) in enumerate(slots) if rr == r]
+                    cs[p, ks[0]] += 0.1
+            Mg.set_params(cs, mws)
+            nll = Mg.nll()
+            st = Mg.last_call_stats()
+            assert st["norm_path"] == 5 and st["launches"] == (P - 1 + 127) // 128
+            ref, refI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+            assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL, (cfg, P)
+            assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12, (cfg, P)
+        # dense random batch: every coupling differs -> not a gradient batch
+        P = 40
+        cs = c0[None] * (1 + 0.1 * rng.uniform(-1, 1, (P, K)))
+        Mg.set_params(cs)
+        nll = Mg.nll()
+        assert Mg.last_call_stats()["norm_path"] in (2, 3)
+        ref, _ = Mo.nll(cs, x, eff, xn, wn)
+        assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
 
 
 def test_norm_matrix_matches_oracle_and_direct_sum():
@@ -265,12 +335,12 @@ def test_static_lineshapes_switch_to_the_matrix():
         assert abs(nll - ref) < RTOL_NLL * abs(ref)
         st = Mg.last_call_stats()
         paths.append(st["norm_path"]); launches.append(st["launches"])
-    assert paths == [1, 2, 2, 2]
+    assert paths == [4, 2, 2, 2]      # first call: fused single launch with a direct-sum normalisation; then the matrix
     assert launches[3] < launches[1]          # no lineshape / HERK launches once M is held
     mw = W.step_mass_width(3, 5)[:10]
     Mg.set_params(c, mw[None])
     nll = Mg.nll()[0]
-    assert Mg.last_call_stats()["norm_path"] == 1
+    assert Mg.last_call_stats()["norm_path"] == 4
     ref = Mo.nll(c, x, eff, xn, wn, mass_width=mw[None])[0][0]
     assert abs(nll - ref) < RTOL_NLL * abs(ref)
 
