@@ -222,31 +222,41 @@ int stream_grid_fused(long long n_data, long long n_norm, bool have_z);
 long long stream_pad(long long n);   // events per column rounded up to whole pipeline tiles
 
 // Gradient batches (P > 1 points that differ from point 0 in a few resonances), see delta.cu.
-// One item = one (point, resonance) change; the items of a point are consecutive, the last one is flagged.
-struct DeltaItem {
-    double2 g[3];       // lineshape unchanged: c(p) - c(0) per helicity (-1, 0, +1); changed: c(p)
-    double2 c0[3];      // couplings of point 0 (used when the lineshape changed)
-    double kN, kG, M2;  // lineshape constants of this point's (mass, width) (used when the lineshape changed)
-    int ent;            // index into StreamArgs::ent: whose BW(0) this item modifies
-    int grp;            // its barrier group (F, G of the event)
-    int J;              // spin of a K*; 256 for a Z
-    int flags;          // bit 0: lineshape changed; bits 1-3: helicities -1, 0, +1 that change; bit 4: last item of its point
+// The host compiles a batch into a small program the kernel keeps in shared memory:
+//   A_xi(p) = A_xi(0) + sum over the point's contributions of  coef * SLOT_xi
+// SLOT = a complex pair (xi = +1, -1) per event, a sum of terms  weight * [BW_ent(0)] * g_{J,lambda,xi}  (the angular
+// factors of Eq. 4 or Eq. 10); consecutive contributions that use the same slot reuse it from registers.
+//   coupling change of slot k:              coef = c_k(p) - c_k(0),      SLOT = BW_R(0) g_k          (1 term, unit weight)
+//   mass/width change of resonance R:       coef = BW_R(p) - BW_R(0),    SLOT = sum_l c_{R,l}(0) g_{R,l}
+//   both at once:                           coef = BW_R(p), SLOT = sum_l c_{R,l}(p) g_{R,l}   and   coef = -1, SLOT = sum_l c_{R,l}(0) BW_R(0) g_{R,l}
+struct DeltaContrib {   // 32 bytes
+    int hdr;            // bits 0-1: coef kind (0 explicit (a, b); 1 BW(kN=a, kG=b, M2=c) - BW_ent(0) of the slot; 2 BW(a, b, c));
+                        // bit 2: last contribution of its point; bit 3: slot differs from the previous contribution's;
+                        // bit 4: empty (point equal to point 0 / padding); bit 5: the BW runs on the Z chain; bits 8-11: barrier group
+    int slot;           // offset of the slot record in the slot area, in 8-byte words
+    double a, b, c;
 };
-enum { DELTA_MAX_SORTED = 128, DELTA_TILE = 256 };   // points per launch besides point 0 (four 32-point blocks); events per tile
+// slot record: int2 {nterms, bw0 spec (ent | grp << 8 | isZ << 12, or -1: no BW(0) needed by kind-1 contributions)}, then
+// per term: int2 {hdr, 0}, double w_re, double w_im;  term hdr: bits 0-7 ent (255: no BW factor), 8-11 grp, 12-14 J,
+// 15-16 lambda + 1, 17 Z-chain term, 18 unit weight
+enum { DELTA_MAX_SORTED = 128, DELTA_MAX_CONTRIB = 320, DELTA_MAX_SLOTWORDS = 1536 };   // per launch: points besides point 0; program sizes
 struct DeltaArgs {
     StreamArgs a;                   // point 0 as the streaming kernel sees it (cache/weight/n/npad: data; cache2/...: norm)
-    const DeltaItem* items;
-    int nsorted;                    // points in `items` order, padded to a multiple of 32 with empty points
+    const DeltaContrib* contrib;    // [ncontrib] device
+    const double* slots;            // [nslotwords] device
+    int ncontrib, nslotwords;
+    int nsorted;                    // points of this launch, padded to a multiple of 32 with empty points
     const int* point_of_sorted;     // [nsorted] -> point index 1..P-1 of this call, -1: padding
     int P;
     double* partial;                // [2][1 + nsorted][stride] per-CTA partials: sum log S (data) and sum w S (norm); row 0 = point 0
     int stride;
     double* result;                 // [2 P + 1]: NLL[P], I[P], domain flag
     int want_nll;
+    int first_chunk;                // 0: a later launch of the same call: the domain flag adds to the earlier launches'
 };
 cudaError_t launch_delta(const DeltaArgs& d, int grid, cudaStream_t s);
 int delta_grid(long long n_data, long long n_norm);
-bool delta_fits(int nent, int ngrp);
+bool delta_fits(int ngrp);
 
 // Batched combine (P > 1) on the FP64 tensor cores, see batch.cu
 enum { BATCH_NKT = 14, BATCH_POINTS = 128, BATCH_MAX_COLS = 48 };   // dense k-tiles (2K <= 56 realified rows) and points per launch

@@ -83,8 +83,8 @@ struct amp_model {
     bool ev_valid = false;
     bool fused_valid = false;      // the last evaluation was the fused single launch: ev[0], ev[1] bracket it
     bool use_delta = false;        // P > 1 and the points are sparse changes of point 0: gradient-batch kernel (delta.cu)
-    std::vector<DeltaItem> delta_items;       // items of points 1..P-1, point after point
-    std::vector<int> delta_first;             // [P]: first item of point p (p >= 1), delta_first[P] = total
+    struct DeltaChunk { int p0, np, nsorted; std::vector<DeltaContrib> contrib; std::vector<double> slots; };
+    std::vector<DeltaChunk> delta_chunks;     // compiled program of the last amp_set_params (points p0 .. p0 + np - 1 per launch)
     int fused_mode = 0;            // 0: P == 1 steps with floating lineshapes run as one fused launch; 1: separate launches
     std::string err;
 };
@@ -387,66 +387,125 @@ amp_status ensure_pool(amp_model* m, int need) {
     return AMP_OK;
 }
 
-// Gradient-batch structure: for every point p >= 1 the resonances whose couplings or (mass, width) differ from point 0.
-// False if the batch is not a sparse change of point 0 (too many items) or touches what the kernel does not carry
-// (a constant term's coupling, more points than its blocks hold is handled by chunking in evaluate()).
-bool build_delta_items(amp_model* m) {
+void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, StreamArgs* a, int* ent_of_res = nullptr, int* grp_of_res = nullptr);
+
+// Compile a batch whose points 1..P-1 are sparse changes of point 0 into the gradient-batch kernel's program
+// (amp_internal.cuh, DeltaContrib): per chunk of <= 128 points a contribution list and the slot records it refers to.
+// False if the batch is not sparse (more than ~3 changed resonances per point on average), touches a constant term's
+// coupling, or does not fit the kernel's shared memory: the caller then takes the dense path.
+bool build_delta_plan(amp_model* m) {
     const int P = m->P, R = m->R, K = m->K;
-    m->delta_items.clear();
-    m->delta_first.assign(P + 1, 0);
+    m->delta_chunks.clear();
     if (P < 2) return false;
-    int nent = 0, ngrp = 0;
+    int ent_of_res[AMP_MAX_RESONANCES], grp_of_res[AMP_MAX_RESONANCES];
     {
-        std::vector<std::pair<int, double>> seen;   // (kind * 8 + J, radius) = one barrier group
-        for (int r = 0; r < R; ++r) {
-            if (m->res[r].kind == AMP_CONST) continue;
-            ++nent;
-            const std::pair<int, double> key(m->res[r].kind * 8 + m->res[r].J, m->res[r].radius);
-            if (std::find(seen.begin(), seen.end(), key) == seen.end()) seen.push_back(key);
-        }
-        ngrp = (int)seen.size();
+        StreamArgs tmp;
+        fill_stream_args(m, m->norm, 0, MODE_FUSED, &tmp, ent_of_res, grp_of_res);
+        if (!delta_fits(tmp.gstart[6])) return false;
     }
-    if (!delta_fits(nent, ngrp)) return false;
-    const size_t cap = (size_t)3 * (P - 1) + 8;   // beyond ~3 changed resonances per point the dense contraction is the better form
-    for (int p = 1; p < P; ++p) {
-        m->delta_first[p] = (int)m->delta_items.size();
-        const size_t first = m->delta_items.size();
-        for (int r = 0; r < R; ++r) {
-            const amp_resonance& rs = m->res[r];
-            const int ns = (rs.kind == AMP_Z || (rs.kind == AMP_KSTAR && rs.J >= 1)) ? 3 : 1;
-            const double* c0 = &m->couplings[((size_t)0 * K + m->slot0[r]) * 2];
-            const double* cp = &m->couplings[((size_t)p * K + m->slot0[r]) * 2];
-            bool dc[3] = {false, false, false}, anyc = false;
-            for (int j = 0; j < ns; ++j) { dc[j] = cp[2 * j] != c0[2 * j] || cp[2 * j + 1] != c0[2 * j + 1]; anyc |= dc[j]; }
-            if (rs.kind == AMP_CONST) { if (anyc) return false; continue; }
-            const double* mw0 = &m->mw[((size_t)0 * R + r) * 2];
-            const double* mwp = &m->mw[((size_t)p * R + r) * 2];
-            const bool ls = mwp[0] != mw0[0] || mwp[1] != mw0[1];
-            if (!anyc && !ls) continue;
-            DeltaItem it{};
-            it.ent = r;   // resonance index for now; evaluate() maps it to the kernel's entry / group numbering
-            it.grp = 0;
-            it.J = rs.kind == AMP_Z ? 256 : rs.J;
-            it.flags = ls ? 1 : 0;
-            for (int j = 0; j < ns; ++j) {
-                const int l = ns == 3 ? j : 1;   // helicity index -1, 0, +1 -> 0, 1, 2
-                const bool nz = cp[2 * j] != 0.0 || cp[2 * j + 1] != 0.0 || c0[2 * j] != 0.0 || c0[2 * j + 1] != 0.0;
-                if (ls ? nz : dc[j]) it.flags |= 2 << l;
-                it.c0[l] = make_double2(c0[2 * j], c0[2 * j + 1]);
-                it.g[l] = ls ? make_double2(cp[2 * j], cp[2 * j + 1]) : make_double2(cp[2 * j] - c0[2 * j], cp[2 * j + 1] - c0[2 * j + 1]);
+    size_t total = 0;
+    const size_t cap = (size_t)3 * (P - 1) + 8;
+    for (int p0 = 1; p0 < P; p0 += DELTA_MAX_SORTED) {
+        amp_model::DeltaChunk ch;
+        ch.p0 = p0;
+        ch.np = std::min((int)DELTA_MAX_SORTED, P - p0);
+        ch.nsorted = (ch.np + 31) / 32 * 32;
+        std::vector<std::pair<std::vector<double>, int>> known;   // slot record -> offset
+        auto add_slot = [&](const std::vector<double>& rec) {
+            for (auto& kv : known)
+                if (kv.first.size() == rec.size() && std::memcmp(kv.first.data(), rec.data(), rec.size() * sizeof(double)) == 0) return kv.second;
+            const int off = (int)ch.slots.size();
+            ch.slots.insert(ch.slots.end(), rec.begin(), rec.end());
+            known.emplace_back(rec, off);
+            return off;
+        };
+        auto word = [](int lo, int hi) { double d; const int v[2] = {lo, hi}; std::memcpy(&d, v, 8); return d; };
+        int prev_slot = -1;
+        auto push = [&](int kind, int slot, int r, double a, double b, double c) {
+            DeltaContrib dc{};
+            const bool isz = r >= 0 && m->res[r].kind == AMP_Z;
+            dc.hdr = kind | (slot != prev_slot ? 8 : 0) | (isz ? 32 : 0) | ((r >= 0 ? grp_of_res[r] : 0) << 8);
+            dc.slot = slot;
+            dc.a = a; dc.b = b; dc.c = c;
+            prev_slot = slot;
+            ch.contrib.push_back(dc);
+        };
+        for (int q = 0; q < ch.nsorted; ++q) {
+            const size_t first = ch.contrib.size();
+            const int p = p0 + q;
+            for (int r = 0; q < ch.np && r < R; ++r) {
+                const amp_resonance& rs = m->res[r];
+                const int ns = (rs.kind == AMP_Z || (rs.kind == AMP_KSTAR && rs.J >= 1)) ? 3 : 1;
+                const double* c0 = &m->couplings[((size_t)0 * K + m->slot0[r]) * 2];
+                const double* cp = &m->couplings[((size_t)p * K + m->slot0[r]) * 2];
+                bool dcf[3] = {false, false, false}, anyc = false;
+                for (int j = 0; j < ns; ++j) { dcf[j] = cp[2 * j] != c0[2 * j] || cp[2 * j + 1] != c0[2 * j + 1]; anyc |= dcf[j]; }
+                if (rs.kind == AMP_CONST) { if (anyc) return false; continue; }
+                const double* mw0 = &m->mw[((size_t)0 * R + r) * 2];
+                const double* mwp = &m->mw[((size_t)p * R + r) * 2];
+                const bool ls = mwp[0] != mw0[0] || mwp[1] != mw0[1];
+                if (!anyc && !ls) continue;
+                const bool isz = rs.kind == AMP_Z;
+                const int Jf = isz ? 1 : rs.J;
+                auto term_hdr = [&](int j, bool with_bw, bool unit) {
+                    const int l = ns == 3 ? j : 1;   // helicity -1, 0, +1 -> 0, 1, 2
+                    return (with_bw ? ent_of_res[r] : 255) | (grp_of_res[r] << 8) | (Jf << 12) | (l << 15) | ((isz ? 1 : 0) << 17) | ((unit ? 1 : 0) << 18);
+                };
+                // slot = sum_j weight_j [BW_R(0)] g_{R,j}; bw0spec: the slot also carries BW_R(0) for kind-1 contributions
+                auto weighted_slot = [&](const double* cc, bool with_bw, int bw0spec) {
+                    std::vector<double> rec(1, 0.0);
+                    int nt = 0;
+                    for (int j = 0; j < ns; ++j) {
+                        if (cc[2 * j] == 0.0 && cc[2 * j + 1] == 0.0) continue;
+                        rec.push_back(word(term_hdr(j, with_bw, false), 0));
+                        rec.push_back(cc[2 * j]);
+                        rec.push_back(cc[2 * j + 1]);
+                        ++nt;
+                    }
+                    rec[0] = word(nt, bw0spec);
+                    return nt ? add_slot(rec) : -1;
+                };
+                if (!ls) {
+                    // coupling changes only: helicities that move by the same amount share one slot (Eq. 11 ties H_+1 = H_-1 of a 1+ Z)
+                    bool done[3] = {false, false, false};
+                    for (int j = 0; j < ns; ++j) {
+                        if (!dcf[j] || done[j]) continue;
+                        const double dre = cp[2 * j] - c0[2 * j], dim = cp[2 * j + 1] - c0[2 * j + 1];
+                        std::vector<double> rec(1, 0.0);
+                        int nt = 0;
+                        for (int j2 = j; j2 < ns; ++j2)
+                            if (dcf[j2] && !done[j2] && cp[2 * j2] - c0[2 * j2] == dre && cp[2 * j2 + 1] - c0[2 * j2 + 1] == dim) {
+                                done[j2] = true;
+                                rec.push_back(word(term_hdr(j2, true, true), 0));
+                                rec.push_back(1.0);
+                                rec.push_back(0.0);
+                                ++nt;
+                            }
+                        rec[0] = word(nt, -1);
+                        push(0, add_slot(rec), r, dre, dim, 0.0);
+                    }
+                } else {
+                    LineConst lc;
+                    make_line_const(m, r, mwp[0], mwp[1], &lc);
+                    const int spec = ent_of_res[r] | (grp_of_res[r] << 8) | ((isz ? 1 : 0) << 12);
+                    if (!anyc) {
+                        const int sl = weighted_slot(c0, false, spec);        // (BW(p) - BW(0)) sum_j c_j(0) g_j
+                        if (sl >= 0) push(1, sl, r, lc.kN, lc.kG, lc.M2);
+                    } else {
+                        const int s1 = weighted_slot(cp, false, -1);          // BW(p) sum_j c_j(p) g_j
+                        if (s1 >= 0) push(2, s1, r, lc.kN, lc.kG, lc.M2);
+                        const int s0 = weighted_slot(c0, true, -1);           // - sum_j c_j(0) BW(0) g_j
+                        if (s0 >= 0) push(0, s0, r, -1.0, 0.0, 0.0);
+                    }
+                }
             }
-            if (ls) {
-                LineConst lc;
-                make_line_const(m, r, mwp[0], mwp[1], &lc);
-                it.kN = lc.kN; it.kG = lc.kG; it.M2 = lc.M2;
-            }
-            m->delta_items.push_back(it);
-            if (m->delta_items.size() > cap) return false;
+            if (ch.contrib.size() == first) { DeltaContrib e{}; e.hdr = 16; e.slot = -1; ch.contrib.push_back(e); }   // equal to point 0, or padding
+            ch.contrib.back().hdr |= 4;
+            if (q < ch.np) total += ch.contrib.size() - first;
+            if (total > cap || ch.contrib.size() > DELTA_MAX_CONTRIB || ch.slots.size() > DELTA_MAX_SLOTWORDS) return false;
         }
-        if (m->delta_items.size() == first) m->delta_items.push_back(DeltaItem{});   // identical to point 0: an empty item
-        m->delta_items.back().flags |= 16;
+        m->delta_chunks.push_back(std::move(ch));
     }
-    m->delta_first[P] = (int)m->delta_items.size();
     return true;
 }
 
@@ -480,7 +539,7 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
     m->want_matrix = m->norm_mode == 2 || (m->norm_mode == 0 && (P == 1 ? mw_same : (P >= 24 && m->batch_mode != 1)));
     if (P == 1) m->prev_mw = m->mw; else m->prev_mw.clear();
     // P > 1: a batch whose points are sparse changes of point 0 (a gradient step) runs the delta kernel: no column, no matrix
-    m->use_delta = P > 1 && m->batch_mode == 0 && m->lineshape_mode != 1 && m->norm_mode != 2 && build_delta_items(m);
+    m->use_delta = P > 1 && m->batch_mode == 0 && m->lineshape_mode != 1 && m->norm_mode != 2 && build_delta_plan(m);
     if (m->use_delta) m->want_matrix = false;
     m->stream_inline = (P == 1 || m->use_delta) && m->lineshape_mode != 1;
 
@@ -586,7 +645,7 @@ amp_status refresh_columns(amp_model* m, Dataset& d, bool is_norm, cudaStream_t 
 
 // Arguments of the streaming kernel for point p on dataset d: resonances grouped by spin, then by
 // radius (a barrier group shares its Blatt-Weisskopf factors and momentum powers).
-void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, StreamArgs* a, int* ent_of_res = nullptr, int* grp_of_res = nullptr) {
+void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, StreamArgs* a, int* ent_of_res, int* grp_of_res) {
     std::memset(a, 0, sizeof(*a));
     int t = 0, g = 0;
     auto add_groups = [&](int kind, int J) {
@@ -611,7 +670,8 @@ void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, Str
                 } else {
                     e.cm = make_double2(cp[0], cp[1]); e.c0 = make_double2(cp[2], cp[3]); e.cp = make_double2(cp[4], cp[5]);
                 }
-                const int sidx = m->colidx[(size_t)p * m->R + r2];
+                const size_t ci = (size_t)p * m->R + r2;
+                const int sidx = ci < m->colidx.size() ? m->colidx[ci] : -1;
                 e.column = (sidx >= 0 && !m->stream_inline) ? sidx : -1;
             }
             grp.count = t - grp.first;
@@ -1026,7 +1086,8 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         d.stride = PARTIAL_STRIDE;
         d.result = m->d_result;
         d.want_nll = want_nll ? 1 : 0;
-        const size_t need = m->delta_items.size() * sizeof(DeltaItem) + (size_t)(P + 32) * (sizeof(DeltaItem) + sizeof(int)) + 4096;
+        size_t need = 4096;
+        for (auto& ch : m->delta_chunks) need += ch.contrib.size() * sizeof(DeltaContrib) + ch.slots.size() * sizeof(double) + ch.nsorted * sizeof(int) + 1024;
         if (need > m->plan_cap) {
             if (m->d_plan) cudaFree(m->d_plan);
             if (m->h_plan) cudaFreeHost(m->h_plan);
@@ -1036,30 +1097,33 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
             CK(cudaMallocHost(&m->h_plan, need * 2));
             m->plan_cap = need * 2;
         }
-        CK(cudaEventRecord(m->ev[0], s));
+        // one upload for all chunks, then one launch per chunk
+        auto al = [](size_t x) { return (x + 255) / 256 * 256; };
         size_t off = 0;
-        for (int p0 = 1; p0 < P; p0 += DELTA_MAX_SORTED) {
-            const int np = std::min((int)DELTA_MAX_SORTED, P - p0), nsorted = (np + 31) / 32 * 32;
-            DeltaItem* hi = reinterpret_cast<DeltaItem*>(m->h_plan + off);
-            const int i0 = m->delta_first[p0], i1 = m->delta_first[p0 + np];
-            int ni = 0;
-            for (int i = i0; i < i1; ++i) {
-                hi[ni] = m->delta_items[i];
-                if (hi[ni].flags & 0xe) { const int r = hi[ni].ent; hi[ni].ent = ent_of_res[r]; hi[ni].grp = grp_of_res[r]; }
-                ++ni;
-            }
-            for (int q = np; q < nsorted; ++q) { hi[ni] = DeltaItem{}; hi[ni].flags = 16; ++ni; }   // padding points
-            const size_t bI = ((size_t)ni * sizeof(DeltaItem) + 255) / 256 * 256;
-            int* hp = reinterpret_cast<int*>(m->h_plan + off + bI);
-            for (int q = 0; q < nsorted; ++q) hp[q] = q < np ? p0 + q : -1;
-            const size_t bP = ((size_t)nsorted * sizeof(int) + 255) / 256 * 256;
-            CK(cudaMemcpyAsync(m->d_plan + off, m->h_plan + off, bI + bP, cudaMemcpyHostToDevice, s));
-            d.items = reinterpret_cast<const DeltaItem*>(m->d_plan + off);
-            d.point_of_sorted = reinterpret_cast<const int*>(m->d_plan + off + bI);
-            d.nsorted = nsorted;
+        std::vector<size_t> offs;
+        for (auto& ch : m->delta_chunks) {
+            offs.push_back(off);
+            const size_t bC = al(ch.contrib.size() * sizeof(DeltaContrib)), bS = al(ch.slots.size() * sizeof(double) + 8);
+            std::memcpy(m->h_plan + off, ch.contrib.data(), ch.contrib.size() * sizeof(DeltaContrib));
+            if (!ch.slots.empty()) std::memcpy(m->h_plan + off + bC, ch.slots.data(), ch.slots.size() * sizeof(double));
+            int* hp = reinterpret_cast<int*>(m->h_plan + off + bC + bS);
+            for (int q = 0; q < ch.nsorted; ++q) hp[q] = q < ch.np ? ch.p0 + q : -1;
+            off += bC + bS + al(ch.nsorted * sizeof(int));
+        }
+        CK(cudaEventRecord(m->ev[0], s));
+        CK(cudaMemcpyAsync(m->d_plan, m->h_plan, off, cudaMemcpyHostToDevice, s));
+        for (size_t c = 0; c < m->delta_chunks.size(); ++c) {
+            const auto& ch = m->delta_chunks[c];
+            const size_t bC = al(ch.contrib.size() * sizeof(DeltaContrib)), bS = al(ch.slots.size() * sizeof(double) + 8);
+            d.contrib = reinterpret_cast<const DeltaContrib*>(m->d_plan + offs[c]);
+            d.slots = reinterpret_cast<const double*>(m->d_plan + offs[c] + bC);
+            d.point_of_sorted = reinterpret_cast<const int*>(m->d_plan + offs[c] + bC + bS);
+            d.ncontrib = (int)ch.contrib.size();
+            d.nslotwords = (int)ch.slots.size();
+            d.nsorted = ch.nsorted;
+            d.first_chunk = c == 0 ? 1 : 0;
             CK(launch_delta(d, delta_grid(d.a.n, d.a.n2), s));
             m->stat_launches++;
-            off += bI + bP;
         }
         CK(cudaEventRecord(m->ev[1], s));
         CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (2 * P + 1), cudaMemcpyDeviceToHost, s));

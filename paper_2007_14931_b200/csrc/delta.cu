@@ -2,80 +2,38 @@
 // point 0 in a few resonances only (MINUIT's finite-difference pattern, BASELINE.json configs[4]: the central value
 // plus theta_k +- h_k for ~60 parameters; "> 60 free parameters").
 //
-// With B_k,xi the basis terms of Eqs. 4 and 10, a point that changes resonance R only gives
-//   A_xi(p) = A_xi(0) + sum_{l in R} [ c_{R,l}(p) BW_R(p) - c_{R,l}(0) BW_R(0) ] g_{R,l,xi}          (Eq. 12 is linear in c BW)
-// i.e. one to three complex multiply-adds per muon helicity instead of the 27 of the dense contraction, and the
-// perturbed Breit-Wigner (Eqs. 2-3) costs ~12 FP64 instructions because the barrier factors of its spin group are
-// those of point 0.  One fused persistent launch walks the data tiles (sum_i log S_i(p)) and then the normalisation
-// tiles (sum_j w_j S_j(p)) for ALL points; no lineshape column, no normalisation matrix, no second pass.
+// Eq. 12 is linear in (coupling x lineshape), so with g_k,xi the angular factors of Eqs. 4 and 10
+// a point that changes resonance R only gives
+//   A_xi(p) = A_xi(0) + sum_{l in R} [ c_{R,l}(p) BW_R(p) - c_{R,l}(0) BW_R(0) ] g_{R,l,xi}
+// — one complex multiply-add per muon helicity instead of the 27 of the dense contraction, and a perturbed
+// Breit-Wigner (Eqs. 2-3) costs ~12 FP64 instructions because the barrier factors (F, G) of its spin group are those
+// of point 0.  The host compiles the batch into contributions `coef * SLOT` (amp_internal.cuh, DeltaContrib); the
+// kernel is the streaming kernel (stream.cu: TMA-fed 512-event tiles, two events per thread, point 0 with lineshapes
+// in registers) followed, per tile, by the point loop.  One fused persistent launch walks the data tiles
+// (sum_i log S_i(p)) and then the normalisation tiles (sum_j w_j S_j(p)) for ALL points: no lineshape column, no
+// normalisation matrix, no second pass.
 //
-// Thread = one event.  Per tile: (1) point 0 exactly as the streaming kernel does it, but the Breit-Wigners and the
-// group factors (F, G) of the event are kept in a thread-private shared-memory record; (2) the points, 32 at a time:
-// every lane evaluates S(p) of its own event for the 32 points of a block in order, and a recursive-halving
-// exchange (one shuffle + one add/multiply per point and lane) leaves lane l with the total of point 32 b + l over
-// the warp's 32 events.  Data side: S = f 2^e is split with integer ops, mantissas are multiplied and exponents
-// added, so the sum of logs needs ONE log per (point, warp) at the very end instead of one per (point, event).
+// Point loop: every lane evaluates S(p) of its two events for the 32 points of a block in order; a recursive-halving
+// exchange (one shuffle + one add or multiply per point and lane) leaves lane l with the total of point 32 b + l over
+// the warp's 64 events.  Data side: S = f 2^e is split with integer ops, mantissas are multiplied and exponents
+// added, so the sum of logs takes ONE log per (point, warp) at the very end instead of one per (point, event).
 // Everything is fixed-order: bit-reproducible.  Bound: plain FP64 ALUs.
-#include "amp_internal.cuh"
+#include "stream_core.cuh"
 
 namespace amp {
 
 namespace {
 
-constexpr int DT = DELTA_TILE;       // events per tile = threads per CTA
-constexpr int DNCOL = NCOL_ALL + 1;  // staged columns per tile: the cache + the weight
 constexpr int DBLK = DELTA_MAX_SORTED / 32;
 
-__device__ __forceinline__ uint32_t d_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void d_mbar_init(uint64_t* bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(d_smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void d_mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(d_smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void d_mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "DWAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DDONE_%=;\n"
-        "bra DWAIT_%=;\n"
-        "DDONE_%=:\n"
-        "}\n" ::"r"(d_smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void d_bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(d_smem_u32(dst)), "l"(src),
-                 "r"(bytes), "r"(d_smem_u32(bar))
-                 : "memory");
-}
-
-// all columns of one 256-event tile (unified tile space: data tiles first, then normalisation tiles) -> stage
-__device__ __forceinline__ void issue_tile(const StreamArgs& a, long long ntd, long long tile, int ncache, double* stage, uint64_t* bar) {
-    const bool is_norm = tile >= ntd;
-    const double* cache = is_norm ? a.cache2 : a.cache;
-    const long long npad = is_norm ? a.npad2 : a.npad, lt = is_norm ? tile - ntd : tile;
-    const uint32_t col_bytes = DT * sizeof(double);
-    d_mbar_expect_tx(bar, col_bytes * (ncache + (is_norm ? 1 : 0)));
-#pragma unroll 1
-    for (int c = 0; c < ncache; ++c) d_bulk_g2s(stage + c * DT, cache + (size_t)c * npad + lt * DT, col_bytes, bar);
-    if (is_norm) d_bulk_g2s(stage + NCOL_ALL * DT, a.weight2 + lt * DT, col_bytes, bar);
-}
-
-// S = f 2^e with f in [0.5, 1) for normal positive S (integer ops on the exponent field)
+// S = f 2^e with f in [0.5, 1) for positive finite S (integer ops on the exponent field)
 __device__ __forceinline__ void split_exp(double S, double* f, int* e) {
-    if (S < 1e-290) { S *= 1.3407807929942597e154; *e = -512; } else *e = 0;   // 2^512: keeps subnormals out of the bit trick
+    int e0 = 0;
+    if (S < 1e-290) { S *= 1.3407807929942597e154; e0 = -512; }   // 2^512: keeps subnormals out of the bit trick
     const int hi = __double2hiint(S), lo = __double2loint(S);
-    *e += ((hi >> 20) & 0x7ff) - 1022;
+    *e = e0 + ((hi >> 20) & 0x7ff) - 1022;
     *f = __hiloint2double((hi & 0x800fffff) | 0x3fe00000, lo);
 }
-
-struct EvK {   // what the point loop needs of one event (registers)
-    double2 Ap, Am;                 // A_xi(0)
-    double m2, mZ2;
-    double cK, sK;
-    double h0, a1, a2, a3, a4;      // d^1_{0,+}(theta_psi); hp cos phi, hp sin phi, hm cos phi, hm sin phi
-};
 
 // d^J_{00}, d^J_{+1,0} (Eq. 4), J warp-uniform
 __device__ __forceinline__ void dJ(int J, double c, double s, double* d0, double* d1) {
@@ -89,99 +47,140 @@ __device__ __forceinline__ void dJ(int J, double c, double s, double* d0, double
     }
 }
 
-// Point 0 of one event: Eqs. 2-5, 10, 12 with the resonances grouped by spin (as stream.cu), E = 1, runtime group loops.
-// Stores BW_R(0) of every entry and (F, G) of every barrier group in the thread's shared-memory record.
-template <int J, int LR, int LB>
-__device__ __forceinline__ void spin_group(const StreamArgs& a, int sp, double m2, double invm, double pR, double pB, double2* bw_rec, double2* fg_rec,
-                                           double2& Um, double2& U0, double2& Up) {
-    for (int g = a.gstart[sp]; g < a.gstart[sp + 1]; ++g) {
-        double F, G;
-        group_factors<LR, LB>(a.grp[g].r2, invm, pR, pB, &F, &G);
-        fg_rec[g * DT] = make_double2(F, G);
-        for (int t = a.grp[g].first; t < a.grp[g].first + a.grp[g].count; ++t) {
-            const double2 bw = bw_from_factors(a.ent[t], m2, F, G);
-            bw_rec[t * DT] = bw;
-            U0 = cfma(a.ent[t].c0, bw, U0);
-            if (J) { Um = cfma(a.ent[t].cm, bw, Um); Up = cfma(a.ent[t].cp, bw, Up); }
+struct EvK {   // what the point loop keeps of one event in registers
+    double2 Ap, Am;                 // A_xi(0)
+    double m2, mZ2;
+    double cK, sK;
+    double h0, a1, a2, a3, a4;      // d^1_{0,+}(theta_psi); hp cos phi, hp sin phi, hm cos phi, hm sin phi
+};
+struct SlotVal {   // the current slot of one event
+    double2 Sp, Sm;                 // xi = +1, -1
+    double2 bw0;                    // BW(0) of the slot's resonance (kind-1 contributions subtract it)
+};
+
+// BW of entry `ent` at point 0 for one event, from the saved group factors
+__device__ __forceinline__ double2 bw_point0(const StreamArgs& a, int ent, int grp, bool isz, const EvK& k, const double2* fg) {
+    const double2 f = fg[grp * TILE];
+    return bw_from_consts(a.ent[ent].kN, a.ent[ent].kG, a.ent[ent].M2, isz ? k.mZ2 : k.m2, f.x, f.y);
+}
+
+// Angular factor g_{J,lambda,xi} of one term for one event (Eq. 4 for a K*, Eq. 10 for the Z).
+// zst: this event's element of the staged tile (the Z-chain angles stay there during the point loop).
+__device__ __forceinline__ void term_angular(int J, int lam, bool isz, const EvK& k, const double* zst, double2* gp, double2* gm) {
+    const double RSQRT2 = 0.70710678118654752440;
+    if (!isz) {
+        double d0, d1;
+        dJ(J, k.cK, k.sK, &d0, &d1);
+        if (lam == 0) {
+            const double t = d0 * k.h0;
+            *gp = make_double2(t, 0.0);
+            *gm = make_double2(-t, 0.0);
+        } else if (lam > 0) {                     // e^{+i phi} (hp, hm)
+            *gp = make_double2(d1 * k.a1, d1 * k.a2);
+            *gm = make_double2(d1 * k.a3, d1 * k.a4);
+        } else {                                  // e^{-i phi} (hm, hp); d^J_{-1,0} = -d^J_{+1,0}
+            *gp = make_double2(-d1 * k.a3, d1 * k.a4);
+            *gm = make_double2(-d1 * k.a1, d1 * k.a2);
         }
+        return;
+    }
+    // d^1_{0 l'}(theta_Z) e^{i l' phi~} d^1_{l' xi}(theta~) e^{i xi alpha}
+    const double cZ = zst[C_CZ * TILE], sZ = zst[C_SZ * TILE], ct = zst[C_CT * TILE], st = zst[C_ST * TILE];
+    const double cpt = zst[C_CPT * TILE], spt = zst[C_SPT * TILE], ca = zst[C_CA * TILE], sa = zst[C_SA * TILE];
+    const double zf = lam == 0 ? cZ : (lam > 0 ? RSQRT2 * sZ : -RSQRT2 * sZ);
+    const double dp = lam == 0 ? RSQRT2 * st : (lam > 0 ? 0.5 * (1.0 + ct) : 0.5 * (1.0 - ct));
+    const double dm = lam == 0 ? -RSQRT2 * st : (lam > 0 ? 0.5 * (1.0 - ct) : 0.5 * (1.0 + ct));
+    const double2 eph = lam == 0 ? make_double2(1.0, 0.0) : make_double2(cpt, lam > 0 ? spt : -spt);
+    *gp = cscale(zf * dp, cmul(eph, make_double2(ca, sa)));
+    *gm = cscale(zf * dm, cmul(eph, make_double2(ca, -sa)));
+}
+
+// Evaluate the slot record at `rec` (shared memory) for the thread's E events.
+__device__ __forceinline__ void eval_slot(const StreamArgs& a, const double* rec, const EvK (&k)[E], const double2* fg, const double* zst,
+                                          SlotVal (&sv)[E]) {
+    const int2 h = *reinterpret_cast<const int2*>(rec);
+#pragma unroll
+    for (int e = 0; e < E; ++e) sv[e].Sp = sv[e].Sm = make_double2(0.0, 0.0);
+    for (int t = 0; t < h.x; ++t) {
+        const int th = *reinterpret_cast<const int*>(rec + 1 + 3 * t);
+        const int ent = th & 255, grp = (th >> 8) & 15, J = (th >> 12) & 7, lam = ((th >> 15) & 3) - 1;
+        const bool isz = (th >> 17) & 1, unit = (th >> 18) & 1;
+        const double2 wgt = make_double2(rec[2 + 3 * t], rec[3 + 3 * t]);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            double2 gp, gm;
+            term_angular(J, lam, isz, k[e], zst + e, &gp, &gm);
+            if (ent != 255) {
+                const double2 bw = bw_point0(a, ent, grp, isz, k[e], fg + e);
+                gp = cmul(bw, gp);
+                gm = cmul(bw, gm);
+            }
+            if (!unit) { gp = cmul(wgt, gp); gm = cmul(wgt, gm); }
+            sv[e].Sp = cadd(sv[e].Sp, gp);
+            sv[e].Sm = cadd(sv[e].Sm, gm);
+        }
+    }
+    if (h.y >= 0) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) sv[e].bw0 = bw_point0(a, h.y & 255, (h.y >> 8) & 15, (h.y >> 12) & 1, k[e], fg + e);
     }
 }
 
-// fixed-order block sum (xor-shuffle tree, then the 8 warp values in warp order); valid in thread 0
-__device__ __forceinline__ double block_sum(double v, double* sm) {
-#pragma unroll
-    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
-    __syncthreads();
-    double t = 0.0;
-    if (threadIdx.x == 0)
-        for (int wv = 0; wv < 8; ++wv) t += sm[wv];
-    return t;
-}
 
-// S(p) of this thread's event for the point whose items start at items[it]; advances it past the point.
-__device__ __forceinline__ double point_density(const DeltaItem* __restrict__ items, int& it, const EvK& k, const double2* bw_rec,
-                                                const double2* fg_rec, const double* zst /* this event's slot in the staged tile */) {
-    const double RSQRT2 = 0.70710678118654752440;
-    double2 Ap = k.Ap, Am = k.Am;
-    int flags;
+// One point for the thread's E events as a leaf of the reduction tree.  NORM: *v = sum_e w_e S_e; DATA: *v = product of
+// the mantissas of S_e, *ex = sum of their exponents.  `it` walks the contribution list; `sv` caches the current slot.
+template <bool NORM>
+__device__ __forceinline__ void leaf(const StreamArgs& a, const DeltaContrib* prog, const double* slots, int& it, const EvK (&k)[E],
+                                     const double2* fg, const double* zst, SlotVal (&sv)[E], const double (&w)[E], const bool (&live)[E],
+                                     bool& bad, double* v, int* ex) {
+    double2 Ap[E], Am[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) { Ap[e] = k[e].Ap; Am[e] = k[e].Am; }
+    int hdr;
     do {
-        const DeltaItem* d = items + it++;
-        flags = d->flags;
-        if ((flags & 0xe) == 0) continue;                      // empty point (padding, or identical to point 0)
-        const bool isz = d->J == 256;
-        const double2 bw0 = bw_rec[d->ent * DT];
-        double2 gam[3];                                        // c(p) BW(p) - c(0) BW(0) per helicity
-        if (flags & 1) {
-            const double2 fg = fg_rec[d->grp * DT];
-            const double2 bw1 = bw_from_consts(d->kN, d->kG, d->M2, isz ? k.mZ2 : k.m2, fg.x, fg.y);
+        const int4 h4 = *reinterpret_cast<const int4*>(prog + it);            // hdr, slot, a (two words)
+        const double2 bc = *reinterpret_cast<const double2*>(&prog[it].b);    // b, c
+        ++it;
+        hdr = h4.x;
+        if (hdr & 16) continue;                                                 // empty point
+        if (hdr & 8) eval_slot(a, slots + h4.y, k, fg, zst, sv);
+        const double ca = __hiloint2double(h4.w, h4.z);
+        const int kind = hdr & 3;
 #pragma unroll
-            for (int l = 0; l < 3; ++l)
-                if (flags & (2 << l)) {
-                    const double2 t = cmul(d->c0[l], bw0);
-                    gam[l] = cfma(d->g[l], bw1, make_double2(-t.x, -t.y));
-                }
-        } else {
+        for (int e = 0; e < E; ++e) {
+            double2 coef = make_double2(ca, bc.x);
+            if (kind) {
+                const double2 f = fg[((hdr >> 8) & 15) * TILE + e];
+                coef = bw_from_consts(ca, bc.x, bc.y, (hdr & 32) ? k[e].mZ2 : k[e].m2, f.x, f.y);
+                if (kind == 1) { coef.x -= sv[e].bw0.x; coef.y -= sv[e].bw0.y; }
+            }
+            Ap[e] = cfma(coef, sv[e].Sp, Ap[e]);
+            Am[e] = cfma(coef, sv[e].Sm, Am[e]);
+        }
+    } while (!(hdr & 4));
+    double S[E];
 #pragma unroll
-            for (int l = 0; l < 3; ++l)
-                if (flags & (2 << l)) gam[l] = cmul(d->g[l], bw0);
+    for (int e = 0; e < E; ++e) S[e] = fma(Ap[e].x, Ap[e].x, fma(Ap[e].y, Ap[e].y, fma(Am[e].x, Am[e].x, Am[e].y * Am[e].y)));
+    if (NORM) {
+        double t = 0.0;
+#pragma unroll
+        for (int e = 0; e < E; ++e) { bad |= live[e] && !isfinite(S[e]); t = fma(w[e], S[e], t); }   // padding events carry w = 0
+        *v = t;
+        *ex = 0;
+    } else {
+        double f = 1.0;
+        int x = 0;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const bool ok = S[e] > 0.0 && isfinite(S[e]);
+            bad |= live[e] && !ok;
+            double fe; int xe;
+            split_exp((live[e] && ok) ? S[e] : 1.0, &fe, &xe);
+            f *= fe; x += xe;
         }
-        if (!isz) {
-            // Eq. 4: d^J_{l0}(theta_K*) e^{i l phi} d^1_{l xi}(theta_psi); d^J_{-1,0} = -d^J_{+1,0}
-            double d0, d1;
-            dJ(d->J, k.cK, k.sK, &d0, &d1);
-            if (flags & 4) { const double t = d0 * k.h0; Ap.x = fma(t, gam[1].x, Ap.x); Ap.y = fma(t, gam[1].y, Ap.y); Am.x = fma(-t, gam[1].x, Am.x); Am.y = fma(-t, gam[1].y, Am.y); }
-            if (flags & 8) {   // lambda = +1: e^{+i phi} (hp, hm)
-                const double2 t = cscale(d1, gam[2]);
-                Ap = cfma(t, make_double2(k.a1, k.a2), Ap);
-                Am = cfma(t, make_double2(k.a3, k.a4), Am);
-            }
-            if (flags & 2) {   // lambda = -1: e^{-i phi} (hm, hp), sign of d^J_{-1,0}
-                const double2 t = cscale(-d1, gam[0]);
-                Ap = cfma(t, make_double2(k.a3, -k.a4), Ap);
-                Am = cfma(t, make_double2(k.a1, -k.a2), Am);
-            }
-        } else {
-            // Eq. 10: d^1_{0 l'}(theta_Z) e^{i l' phi~} d^1_{l' xi}(theta~) e^{i xi alpha}; angles from the staged tile
-            const double cZ = zst[C_CZ * DT], sZ = zst[C_SZ * DT], ct = zst[C_CT * DT], st = zst[C_ST * DT];
-            const double cpt = zst[C_CPT * DT], spt = zst[C_SPT * DT], ca = zst[C_CA * DT], sa = zst[C_SA * DT];
-            const double z1 = RSQRT2 * sZ, gp = 0.5 * (1.0 + ct), gm = 0.5 * (1.0 - ct), g0 = RSQRT2 * st;
-            double2 Zp = make_double2(0, 0), Zm = Zp;
-            if (flags & 4) { const double2 T0 = cscale(cZ, gam[1]); Zp = cscale(g0, T0); Zm = cscale(-g0, T0); }
-            if (flags & 8) {
-                const double2 Tp = cscale(z1, cmul(make_double2(cpt, spt), gam[2]));
-                Zp.x = fma(gp, Tp.x, Zp.x); Zp.y = fma(gp, Tp.y, Zp.y); Zm.x = fma(gm, Tp.x, Zm.x); Zm.y = fma(gm, Tp.y, Zm.y);
-            }
-            if (flags & 2) {
-                const double2 Tm = cscale(-z1, cmul(make_double2(cpt, -spt), gam[0]));
-                Zp.x = fma(gm, Tm.x, Zp.x); Zp.y = fma(gm, Tm.y, Zp.y); Zm.x = fma(gp, Tm.x, Zm.x); Zm.y = fma(gp, Tm.y, Zm.y);
-            }
-            Ap = cfma(make_double2(ca, sa), Zp, Ap);
-            Am = cfma(make_double2(ca, -sa), Zm, Am);
-        }
-    } while (!(flags & 16));
-    return fma(Ap.x, Ap.x, fma(Ap.y, Ap.y, fma(Am.x, Am.x, Am.y * Am.y)));
+        *v = f;
+        *ex = x;
+    }
 }
 
 // Recursive halving over the 32 lanes: `a` belongs to the earlier half of the points, `b` to the later half; lanes with
@@ -200,190 +199,211 @@ __device__ __forceinline__ void halve(int level, int lane, double a, int ea, dou
     }
 }
 
-// one point of this thread's event as a tree leaf: NORM: w S; DATA: (mantissa, exponent) of S
+// The 32 points of one block; on return lane l holds the warp total of point 32 blk + l (NORM: sum of w S; DATA:
+// product of mantissas in *v — at least 2^-64 — and sum of exponents in *ex).  Binary-counter carries: q is uniform.
 template <bool NORM>
-__device__ __forceinline__ void leaf(const DeltaItem* __restrict__ items, int& it, const EvK& k, const double2* bw_rec, const double2* fg_rec,
-                                     const double* zst, double w, bool live, bool& bad, double* v, int* e) {
-    const double S = point_density(items, it, k, bw_rec, fg_rec, zst);
-    if (NORM) {
-        bad |= live && !isfinite(S);
-        *v = w * S;
-        *e = 0;
-    } else {
-        const bool ok = S > 0.0 && isfinite(S);
-        bad |= live && !ok;
-        split_exp((live && ok) ? S : 1.0, v, e);
-    }
-}
-
-// The 32 points of one block for this thread's event; on return lane l holds the warp total of point 32 blk + l
-// (NORM: sum of w S; DATA: product of mantissas in *v, sum of exponents in *e).
-template <bool NORM>
-__device__ __forceinline__ void eval_block(const DeltaItem* __restrict__ items, int& it, const EvK& k, const double2* bw_rec, const double2* fg_rec,
-                                           const double* zst, double w, bool live, bool& bad, int lane, double* v, int* e) {
-    double s2 = 0, s3 = 0, s4 = 0;
-    int e2 = 0, e3 = 0, e4 = 0;
+__device__ __forceinline__ void eval_block(const StreamArgs& a, const DeltaContrib* prog, const double* slots, int& it, const EvK (&k)[E],
+                                           const double2* fg, const double* zst, SlotVal (&sv)[E], const double (&w)[E],
+                                           const bool (&live)[E], bool& bad, int lane, double* v, int* ex) {
+    double s0 = 0, s1 = 0, s2 = 0, s3 = 0, s4 = 0;
+    int e0 = 0, e1 = 0, e2 = 0, e3 = 0, e4 = 0;
 #pragma unroll 1
-    for (int g = 0; g < 8; ++g) {
-        double v0, v1, u0, u1, x;
-        int f0, f1, q0, q1, ex;
-        leaf<NORM>(items, it, k, bw_rec, fg_rec, zst, w, live, bad, &v0, &f0);
-        leaf<NORM>(items, it, k, bw_rec, fg_rec, zst, w, live, bad, &v1, &f1);
-        halve<NORM>(0, lane, v0, f0, v1, f1, &u0, &q0);
-        leaf<NORM>(items, it, k, bw_rec, fg_rec, zst, w, live, bad, &v0, &f0);
-        leaf<NORM>(items, it, k, bw_rec, fg_rec, zst, w, live, bad, &v1, &f1);
-        halve<NORM>(0, lane, v0, f0, v1, f1, &u1, &q1);
-        halve<NORM>(1, lane, u0, q0, u1, q1, &x, &ex);
-        // binary-counter carries through levels 2, 3, 4 (g is uniform)
-        if ((g & 1) == 0) { s2 = x; e2 = ex; continue; }
-        halve<NORM>(2, lane, s2, e2, x, ex, &x, &ex);
-        if ((g & 2) == 0) { s3 = x; e3 = ex; continue; }
-        halve<NORM>(3, lane, s3, e3, x, ex, &x, &ex);
-        if ((g & 4) == 0) { s4 = x; e4 = ex; continue; }
-        halve<NORM>(4, lane, s4, e4, x, ex, v, e);
+    for (int q = 0; q < 32; ++q) {
+        double x; int xe;
+        leaf<NORM>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, &x, &xe);
+        if (!(q & 1)) { s0 = x; e0 = xe; continue; }
+        halve<NORM>(0, lane, s0, e0, x, xe, &x, &xe);
+        if (!(q & 2)) { s1 = x; e1 = xe; continue; }
+        halve<NORM>(1, lane, s1, e1, x, xe, &x, &xe);
+        if (!(q & 4)) { s2 = x; e2 = xe; continue; }
+        halve<NORM>(2, lane, s2, e2, x, xe, &x, &xe);
+        if (!(q & 8)) { s3 = x; e3 = xe; continue; }
+        halve<NORM>(3, lane, s3, e3, x, xe, &x, &xe);
+        if (!(q & 16)) { s4 = x; e4 = xe; continue; }
+        halve<NORM>(4, lane, s4, e4, x, xe, v, ex);
     }
 }
 
 }  // namespace
 
-__global__ void __launch_bounds__(DT, 1) k_delta(const __grid_constant__ DeltaArgs d) {
+template <class SH>
+__global__ void __launch_bounds__(THREADS, 1) k_delta(const __grid_constant__ DeltaArgs d) {
     const StreamArgs& a = d.a;
     const double RSQRT2 = 0.70710678118654752440;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const bool have_z = a.gstart[6] > a.gstart[5];
+    const int tid = threadIdx.x, lane = tid & 31;
+    const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[6] > a.gstart[5]);
     const int ncache = have_z ? NCOL_ALL : NCOL_K;
-    int nent = 0;
-    for (int sp = 0; sp < 6; ++sp) nent += a.shape[sp];
     const int ngrp = a.gstart[6];
     const int nblk = d.nsorted / 32;
 
+    // shared memory: staged tile (two regions, as k_stream) | group factors | per-lane point accumulators | the program
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double* stage = reinterpret_cast<double*>(smem_raw);                       // [2][DNCOL][DT]
-    double2* bw_base = reinterpret_cast<double2*>(stage + 2 * DNCOL * DT);      // [nent][DT]
-    double2* fg_base = bw_base + (size_t)nent * DT;                             // [ngrp][DT]
-    double* accN = reinterpret_cast<double*>(fg_base + (size_t)ngrp * DT);      // [DBLK][8 warps][32] sum w S
-    double* accF = accN + DBLK * DT;                                            // [DBLK][8][32] mantissa products (data)
-    int* accE = reinterpret_cast<int*>(accF + DBLK * DT);                       // [DBLK][8][32] exponent sums (data)
-    uint64_t* full = reinterpret_cast<uint64_t*>(accE + DBLK * DT);             // [2]
+    double* stage = reinterpret_cast<double*>(smem_raw);                          // [ncache + 1][TILE]
+    double2* fg_base = reinterpret_cast<double2*>(stage + (size_t)(ncache + 1) * TILE);   // [ngrp][TILE]
+    double* accN = reinterpret_cast<double*>(fg_base + (size_t)ngrp * TILE);      // [DBLK][THREADS] sum w S
+    double* accF = accN + DBLK * THREADS;                                         // [DBLK][THREADS] mantissa products (data)
+    int* accE = reinterpret_cast<int*>(accF + DBLK * THREADS);                    // [DBLK][THREADS] exponent sums (data)
+    DeltaContrib* prog = reinterpret_cast<DeltaContrib*>(accE + DBLK * THREADS);  // [DELTA_MAX_CONTRIB]
+    double* slots = reinterpret_cast<double*>(prog + DELTA_MAX_CONTRIB);          // [DELTA_MAX_SLOTWORDS]
+    uint64_t* full = reinterpret_cast<uint64_t*>(slots + DELTA_MAX_SLOTWORDS);    // [2]
     __shared__ double sm[8];
     __shared__ bool s_last;
-    for (int b = 0; b < DBLK; ++b) { accN[b * DT + tid] = 0.0; accF[b * DT + tid] = 1.0; accE[b * DT + tid] = 0; }
+    for (int b = 0; b < DBLK; ++b) { accN[b * THREADS + tid] = 0.0; accF[b * THREADS + tid] = 1.0; accE[b * THREADS + tid] = 0; }
+    for (int i = tid; i < d.ncontrib * 4; i += THREADS) reinterpret_cast<double*>(prog)[i] = reinterpret_cast<const double*>(d.contrib)[i];
+    for (int i = tid; i < d.nslotwords; i += THREADS) slots[i] = d.slots[i];
     if (tid == 0) {
-        d_mbar_init(&full[0], 1);
-        d_mbar_init(&full[1], 1);
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    const long long ntd = d.want_nll ? (a.n + DT - 1) / DT : 0;
-    const long long ntiles = ntd + (a.n2 + DT - 1) / DT;
-    if (tid == 0 && (long long)blockIdx.x < ntiles) issue_tile(a, ntd, blockIdx.x, ncache, stage, &full[0]);
-
-    double2* bw_rec = bw_base + tid;
-    double2* fg_rec = fg_base + tid;
+    const long long ntd = d.want_nll ? (a.n + TILE - 1) / TILE : 0;              // data tiles first, then normalisation tiles
+    const long long ntiles = ntd + (a.n2 + TILE - 1) / TILE;
+    auto issue = [&](long long tile, int region) {
+        const bool nrm = tile >= ntd;
+        const double* cache = nrm ? a.cache2 : a.cache;
+        const long long npad = nrm ? a.npad2 : a.npad, lt = nrm ? tile - ntd : tile;
+        if (region == 0) issue_cols(cache, a.weight2, npad, lt, stage, &full[0], 0, NCOL_K, nrm, ncache);
+        else issue_cols(cache, nullptr, npad, lt, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
+    };
+    if (tid == 0 && (long long)blockIdx.x < ntiles) {
+        issue(blockIdx.x, 0);
+        if (have_z) issue(blockIdx.x, 1);
+    }
+    double2* fg = fg_base + tid * E;
+    const double* zst = stage + tid * E;
     double acc0N = 0.0, acc0F = 1.0;   // point 0: sum w S ; mantissa product and exponent sum of S
     int acc0E = 0;
     bool bad = false;
-    uint32_t par0 = 0, par1 = 0;
-    int buf = 0;
-    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, buf ^= 1) {
-        // the other buffer was last read before the __syncthreads that closed the previous iteration: refill it now
-        if (tid == 0 && tile + gridDim.x < ntiles) issue_tile(a, ntd, tile + gridDim.x, ncache, stage + (buf ^ 1) * DNCOL * DT, &full[buf ^ 1]);
+    uint32_t parity = 0;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, parity ^= 1) {
+        const bool has_next = tile + gridDim.x < ntiles;
         const bool is_norm = tile >= ntd;
         const long long lt = is_norm ? tile - ntd : tile;
-        const bool live = lt * DT + tid < (is_norm ? a.n2 : a.n);
-        if (buf == 0) { d_mbar_wait(&full[0], par0); par0 ^= 1; } else { d_mbar_wait(&full[1], par1); par1 ^= 1; }
-        const double* st = stage + buf * DNCOL * DT + tid;
+        const long long i0 = lt * TILE + tid * E;
+        const long long nlive = is_norm ? a.n2 : a.n;
+        // ---- point 0: the K* chain (as k_stream)
+        mbar_wait(&full[0], parity);
+        const Ev m2 = load_col(stage, C_M2), invm = load_col(stage, C_INVM);
+        const Ev q = load_col(stage, C_Q), pB = load_col(stage, C_PB);
+        const Ev cK = load_col(stage, C_CK), sK = load_col(stage, C_SK);
+        const Ev cpsi = load_col(stage, C_CPSI), spsi = load_col(stage, C_SPSI);
+        const Ev cphi = load_col(stage, C_CPHI), sphi = load_col(stage, C_SPHI);
+        Ev wv;
+        if (is_norm) wv = load_col(stage, ncache);
+        __syncthreads();   // K* region consumed by every thread: stream the next tile into it during the point loop
+        if (tid == 0 && has_next) issue(tile + gridDim.x, 0);
 
-        // ---- point 0 (as stream.cu, one event per thread)
-        EvK k;
-        k.m2 = st[C_M2 * DT];
-        k.cK = st[C_CK * DT]; k.sK = st[C_SK * DT];
-        double2 V0 = a.cconst, Vp = make_double2(0, 0), Vm = Vp;
-        {
-            const double invm = st[C_INVM * DT], q = st[C_Q * DT], pB = st[C_PB * DT];
-            const double c = k.cK, s = k.sK;
-#define AMP_DSPIN(J, LB)                                                                         \
-            if (a.gstart[J + 1] > a.gstart[J]) {                                                   \
-                double2 Um = make_double2(0, 0), U0 = Um, Up = Um;                                 \
-                spin_group<J, J, LB>(a, J, k.m2, invm, q, pB, bw_rec, fg_rec, Um, U0, Up);         \
-                double d0, d1;                                                                     \
-                dJ(J, c, s, &d0, &d1);                                                             \
-                V0 = cadd(V0, cscale(d0, U0));                                                     \
-                if (J) { Vp = cadd(Vp, cscale(d1, Up)); Vm = cadd(Vm, cscale(-d1, Um)); }          \
-            }
-            AMP_DSPIN(0, 1)
-            AMP_DSPIN(1, 0)
-            AMP_DSPIN(2, 1)
-            AMP_DSPIN(3, 2)
-            AMP_DSPIN(4, 3)
-#undef AMP_DSPIN
+        double2 V0[E], Vp[E], Vm[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) { V0[e] = a.cconst; Vp[e] = make_double2(0, 0); Vm[e] = make_double2(0, 0); }
+#define AMP_SPIN(J, LB, CNT, OFF, D0, D1)                                                              \
+        if (CNT != 0 && (CNT > 0 || a.gstart[J + 1] > a.gstart[J])) {                                  \
+            double2 Um[E], U0[E], Up[E];                                                               \
+            _Pragma("unroll") for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0);  \
+            spin_sum<J, J, LB, CNT, OFF, J, true>(a, i0, m2, invm, q, pB, Um, U0, Up, fg);             \
+            _Pragma("unroll") for (int e = 0; e < E; ++e) {                                            \
+                const double c = cK.v[e], s = sK.v[e], c2 = c * c;                                     \
+                (void)s; (void)c2;                                                                     \
+                const double d0 = (D0), d1 = (D1);                                                     \
+                V0[e] = cadd(V0[e], cscale(d0, U0[e]));                                                \
+                if (J) { Vp[e] = cadd(Vp[e], cscale(d1, Up[e])); Vm[e] = cadd(Vm[e], cscale(-d1, Um[e])); } \
+            }                                                                                          \
         }
-        {
-            const double cpsi = st[C_CPSI * DT], spsi = st[C_SPSI * DT], cphi = st[C_CPHI * DT], sphi = st[C_SPHI * DT];
-            const double hp = 0.5 * (1.0 + cpsi), hm = 0.5 * (1.0 - cpsi);
-            k.h0 = RSQRT2 * spsi;
-            k.a1 = hp * cphi; k.a2 = hp * sphi; k.a3 = hm * cphi; k.a4 = hm * sphi;
+        AMP_SPIN(0, 1, SH::n0, 0, 1.0, 0.0)
+        AMP_SPIN(1, 0, SH::n1, SH::o1, c, -RSQRT2 * s)
+        AMP_SPIN(2, 1, SH::n2, SH::o2, fma(1.5, c2, -0.5), -1.2247448713915890491 * s * c)
+        AMP_SPIN(3, 2, SH::n3, SH::o3, c * fma(2.5, c2, -1.5), -0.43301270189221932338 * s * fma(5.0, c2, -1.0))
+        AMP_SPIN(4, 3, SH::n4, SH::o4, fma(fma(4.375, c2, -3.75), c2, 0.375), -0.55901699437494742410 * s * c * fma(7.0, c2, -3.0))
+#undef AMP_SPIN
+        EvK k[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double hp = 0.5 * (1.0 + cpsi.v[e]), hm = 0.5 * (1.0 - cpsi.v[e]);
+            k[e].m2 = m2.v[e]; k[e].mZ2 = 0.0;
+            k[e].cK = cK.v[e]; k[e].sK = sK.v[e];
+            k[e].h0 = RSQRT2 * spsi.v[e];
+            k[e].a1 = hp * cphi.v[e]; k[e].a2 = hp * sphi.v[e]; k[e].a3 = hm * cphi.v[e]; k[e].a4 = hm * sphi.v[e];
             // A_xi = sum_l e^{i l phi} d^1_{l xi}(theta_psi) V_l
-            k.Ap = make_double2(k.h0 * V0.x, k.h0 * V0.y);
-            k.Am = make_double2(-k.Ap.x, -k.Ap.y);
-            k.Ap = cfma(Vp, make_double2(k.a1, k.a2), k.Ap);
-            k.Am = cfma(Vp, make_double2(k.a3, k.a4), k.Am);
-            k.Ap = cfma(Vm, make_double2(k.a3, -k.a4), k.Ap);
-            k.Am = cfma(Vm, make_double2(k.a1, -k.a2), k.Am);
+            k[e].Ap = make_double2(k[e].h0 * V0[e].x, k[e].h0 * V0[e].y);
+            k[e].Am = make_double2(-k[e].Ap.x, -k[e].Ap.y);
+            k[e].Ap = cfma(Vp[e], make_double2(k[e].a1, k[e].a2), k[e].Ap);
+            k[e].Am = cfma(Vp[e], make_double2(k[e].a3, k[e].a4), k[e].Am);
+            k[e].Ap = cfma(Vm[e], make_double2(k[e].a3, -k[e].a4), k[e].Ap);
+            k[e].Am = cfma(Vm[e], make_double2(k[e].a1, -k[e].a2), k[e].Am);
         }
-        k.mZ2 = 0.0;
+        // ---- point 0: the Z chain; its staged columns stay in place for the point loop (Z slots read the angles)
         if (have_z) {
-            k.mZ2 = st[C_MZ2 * DT];
-            const double invmZ = st[C_INVMZ * DT], qZ = st[C_QZ * DT], pBZ = st[C_PBZ * DT];
-            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
-            spin_group<1, 0, 1>(a, 5, k.mZ2, invmZ, qZ, pBZ, bw_rec, fg_rec, Um, U0, Up);   // 1+ Z: L_R = 0, L_B = 1
-            const double cZ = st[C_CZ * DT], sZ = st[C_SZ * DT], ct = st[C_CT * DT], stt = st[C_ST * DT];
-            const double cpt = st[C_CPT * DT], spt = st[C_SPT * DT], ca = st[C_CA * DT], sa = st[C_SA * DT];
-            const double z1 = RSQRT2 * sZ;
-            const double2 T0 = cscale(cZ, U0);
-            const double2 Tp = cscale(z1, cmul(make_double2(cpt, spt), Up));
-            const double2 Tm = cscale(-z1, cmul(make_double2(cpt, -spt), Um));
-            const double gp = 0.5 * (1.0 + ct), gm = 0.5 * (1.0 - ct), g0 = RSQRT2 * stt;
-            const double2 Zp = make_double2(g0 * T0.x + gp * Tp.x + gm * Tm.x, g0 * T0.y + gp * Tp.y + gm * Tm.y);
-            const double2 Zm = make_double2(-g0 * T0.x + gm * Tp.x + gp * Tm.x, -g0 * T0.y + gm * Tp.y + gp * Tm.y);
-            k.Ap = cfma(make_double2(ca, sa), Zp, k.Ap);
-            k.Am = cfma(make_double2(ca, -sa), Zm, k.Am);
+            mbar_wait(&full[1], parity);
+            const Ev mZ2 = load_col(stage, C_MZ2), invmZ = load_col(stage, C_INVMZ);
+            const Ev qZ = load_col(stage, C_QZ), pBZ = load_col(stage, C_PBZ);
+            const Ev cZ = load_col(stage, C_CZ), sZ = load_col(stage, C_SZ);
+            const Ev ct = load_col(stage, C_CT), st = load_col(stage, C_ST);
+            const Ev cpt = load_col(stage, C_CPT), spt = load_col(stage, C_SPT);
+            const Ev ca = load_col(stage, C_CA), sa = load_col(stage, C_SA);
+            double2 Um[E], U0[E], Up[E];
+#pragma unroll
+            for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0);
+            spin_sum<1, 0, 1, SH::nz, SH::oz, 5, true>(a, i0, mZ2, invmZ, qZ, pBZ, Um, U0, Up, fg);   // 1+ Z: L_R = 0, L_B = 1
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const double z1 = RSQRT2 * sZ.v[e];
+                const double2 T0 = cscale(cZ.v[e], U0[e]);
+                const double2 Tp = cscale(z1, cmul(make_double2(cpt.v[e], spt.v[e]), Up[e]));
+                const double2 Tm = cscale(-z1, cmul(make_double2(cpt.v[e], -spt.v[e]), Um[e]));
+                const double gp = 0.5 * (1.0 + ct.v[e]), gm = 0.5 * (1.0 - ct.v[e]), g0 = RSQRT2 * st.v[e];
+                const double2 Zp = make_double2(g0 * T0.x + gp * Tp.x + gm * Tm.x, g0 * T0.y + gp * Tp.y + gm * Tm.y);
+                const double2 Zm = make_double2(-g0 * T0.x + gm * Tp.x + gp * Tm.x, -g0 * T0.y + gm * Tp.y + gp * Tm.y);
+                k[e].Ap = cfma(make_double2(ca.v[e], sa.v[e]), Zp, k[e].Ap);
+                k[e].Am = cfma(make_double2(ca.v[e], -sa.v[e]), Zm, k[e].Am);
+                k[e].mZ2 = mZ2.v[e];
+            }
         }
-        const double S0 = fma(k.Ap.x, k.Ap.x, fma(k.Ap.y, k.Ap.y, fma(k.Am.x, k.Am.x, k.Am.y * k.Am.y)));
-        const double w = is_norm ? st[NCOL_ALL * DT] : 0.0;
-        if (is_norm) {
-            bad |= live && !isfinite(S0);
-            acc0N = fma(w, S0, acc0N);      // padding events carry w = 0
-        } else {
-            const bool ok = S0 > 0.0 && isfinite(S0);
-            bad |= live && !ok;
-            double f; int e1, e2;
-            split_exp((live && ok) ? S0 : 1.0, &f, &e1);
-            split_exp(acc0F * f, &acc0F, &e2);   // running product of mantissas, renormalised to [0.5, 1)
-            acc0E += e1 + e2;
+        double w[E];
+        bool live[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            live[e] = i0 + e < nlive;
+            w[e] = is_norm ? wv.v[e] : 0.0;
+            const double S0 = fma(k[e].Ap.x, k[e].Ap.x, fma(k[e].Ap.y, k[e].Ap.y, fma(k[e].Am.x, k[e].Am.x, k[e].Am.y * k[e].Am.y)));
+            if (is_norm) {
+                bad |= live[e] && !isfinite(S0);
+                acc0N = fma(w[e], S0, acc0N);
+            } else {
+                const bool ok = S0 > 0.0 && isfinite(S0);
+                bad |= live[e] && !ok;
+                double f; int x1, x2;
+                split_exp((live[e] && ok) ? S0 : 1.0, &f, &x1);
+                split_exp(acc0F * f, &acc0F, &x2);   // running product of mantissas, renormalised to [0.5, 1)
+                acc0E += x1 + x2;
+            }
         }
-        // ---- the points, 32 per block; the warp totals go to the per-warp accumulators
+        // ---- the points, 32 per block; lane totals go to the per-lane accumulators
+        SlotVal sv[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) sv[e].Sp = sv[e].Sm = sv[e].bw0 = make_double2(0.0, 0.0);
         int it = 0;
         for (int b = 0; b < nblk; ++b) {
-            double v; int e;
-            const int slot = b * DT + warp * 32 + lane;
+            double v; int x;
+            const int slot = b * THREADS + tid;
             if (is_norm) {
-                eval_block<true>(d.items, it, k, bw_rec, fg_rec, st, w, live, bad, lane, &v, &e);
+                eval_block<true>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, lane, &v, &x);
                 accN[slot] += v;
             } else {
-                eval_block<false>(d.items, it, k, bw_rec, fg_rec, st, w, live, bad, lane, &v, &e);
-                double f; int e2;
-                split_exp(accF[slot] * v, &f, &e2);
+                eval_block<false>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, lane, &v, &x);
+                double f; int x2;
+                split_exp(accF[slot] * v, &f, &x2);
                 accF[slot] = f;
-                accE[slot] += e + e2;
+                accE[slot] += x + x2;
             }
         }
-        __syncthreads();   // every thread is done with this buffer
+        __syncthreads();   // Z region (and the group factors) no longer needed: stream the next tile's Z columns
+        if (have_z && tid == 0 && has_next) issue(tile + gridDim.x, 1);
     }
     if (bad) atomicOr(a.flag, 2);
 
     // ---- per-CTA partials: partial[(seg * rows + row) * stride + cta], seg 0 = sum log S (data), 1 = sum w S (norm);
-    //      row 0 = point 0, row 1 + s = sorted point s
+    //      row 0 = point 0, row 1 + s = point s of this launch
     const double LN2 = 0.69314718055994530942;
     const int rows = 1 + d.nsorted;
     {
@@ -391,11 +411,12 @@ __global__ void __launch_bounds__(DT, 1) k_delta(const __grid_constant__ DeltaAr
         const double t1 = block_sum(acc0N, sm);
         if (tid == 0) { d.partial[(size_t)0 * d.stride + blockIdx.x] = t0; d.partial[(size_t)rows * d.stride + blockIdx.x] = t1; }
     }
-    for (int idx = tid; idx < d.nsorted; idx += DT) {
+    __syncthreads();
+    for (int idx = tid; idx < d.nsorted; idx += THREADS) {
         const int b = idx >> 5, l = idx & 31;
         double sN = 0.0, sL = 0.0;
-        for (int wv = 0; wv < 8; ++wv) {   // the 8 warp totals in warp order
-            const int slot = b * DT + wv * 32 + l;
+        for (int wv = 0; wv < THREADS / 32; ++wv) {   // the warp totals in warp order
+            const int slot = b * THREADS + wv * 32 + l;
             sN += accN[slot];
             sL += log(accF[slot]) + (double)accE[slot] * LN2;
         }
@@ -409,15 +430,15 @@ __global__ void __launch_bounds__(DT, 1) k_delta(const __grid_constant__ DeltaAr
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    double* tot = accN;   // [2 rows] (accN/accF are dead; 2 * 129 doubles fit)
-    for (int r = tid; r < 2 * rows; r += DT) {
+    double* tot = accN;   // [2 rows]: the accumulators are dead (2 * 129 doubles fit)
+    for (int r = tid; r < 2 * rows; r += THREADS) {
         const double* p = d.partial + (size_t)r * d.stride;
         double s = 0.0;
         for (unsigned c = 0; c < gridDim.x; ++c) s += __ldcg(p + c);
         tot[r] = s;
     }
     __syncthreads();
-    for (int r = tid; r < rows; r += DT) {
+    for (int r = tid; r < rows; r += THREADS) {
         const int p = r == 0 ? 0 : d.point_of_sorted[r - 1];
         if (p < 0) continue;
         const double I = tot[rows + r] / a.wsum;
@@ -427,36 +448,46 @@ __global__ void __launch_bounds__(DT, 1) k_delta(const __grid_constant__ DeltaAr
         d.result[p] = d.want_nll ? v : 0.0;
     }
     if (tid == 0) {
-        d.result[2 * d.P] = (double)atomicExch(a.flag, 0);
+        const double fl = (double)atomicExch(a.flag, 0);   // domain flag of this launch, cleared for the next one
+        d.result[2 * d.P] = d.first_chunk ? fl : d.result[2 * d.P] + fl;
         *a.ticket = 0u;
     }
 }
 
 namespace {
 
-size_t delta_smem(int nent, int ngrp) {
-    return (size_t)2 * DNCOL * DT * sizeof(double) + (size_t)(nent + ngrp) * DT * sizeof(double2) + (size_t)DBLK * DT * (2 * sizeof(double) + sizeof(int)) +
-           2 * sizeof(uint64_t);
+size_t delta_smem(bool have_z, int ngrp) {
+    return (size_t)((have_z ? NCOL_ALL : NCOL_K) + 1) * TILE * sizeof(double) + (size_t)ngrp * TILE * sizeof(double2) +
+           (size_t)DBLK * THREADS * (2 * sizeof(double) + sizeof(int)) + (size_t)DELTA_MAX_CONTRIB * sizeof(DeltaContrib) +
+           (size_t)DELTA_MAX_SLOTWORDS * sizeof(double) + 2 * sizeof(uint64_t);
+}
+
+template <class SH>
+cudaError_t launch_delta_shape(const DeltaArgs& d, int grid, cudaStream_t s) {
+    static bool attr_done = false;
+    cudaError_t e = cudaSuccess;
+    if (!attr_done) { e = cudaFuncSetAttribute(k_delta<SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
+    if (e != cudaSuccess) return e;
+    const bool have_z = d.a.gstart[6] > d.a.gstart[5];
+    k_delta<SH><<<grid, THREADS, delta_smem(have_z, d.a.gstart[6]), s>>>(d);
+    return cudaGetLastError();
 }
 
 }  // namespace
 
-bool delta_fits(int nent, int ngrp) { return delta_smem(nent, ngrp) <= (size_t)224 * 1024; }
+bool delta_fits(int ngrp) { return delta_smem(true, ngrp) <= (size_t)224 * 1024; }
 
 int delta_grid(long long n_data, long long n_norm) {
-    const long long ntiles = (n_data + DT - 1) / DT + (n_norm + DT - 1) / DT;
+    const long long ntiles = (n_data + TILE - 1) / TILE + (n_norm + TILE - 1) / TILE;
     return (int)(ntiles < 1 ? 1 : (ntiles > 148 ? 148 : ntiles));   // persistent: one CTA per SM
 }
 
+// the paper's model (ten K* + one Z, one radius per spin) runs the unrolled shape; anything else the generic loops
 cudaError_t launch_delta(const DeltaArgs& d, int grid, cudaStream_t s) {
-    static bool attr_done = false;
-    cudaError_t e = cudaSuccess;
-    if (!attr_done) { e = cudaFuncSetAttribute(k_delta, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
-    if (e != cudaSuccess) return e;
-    int nent = 0;
-    for (int sp = 0; sp < 6; ++sp) nent += d.a.shape[sp];
-    k_delta<<<grid, DT, delta_smem(nent, d.a.gstart[6]), s>>>(d);
-    return cudaGetLastError();
+    const int* n = d.a.shape;
+    if (d.a.shape_fixed && n[0] == 3 && n[1] == 3 && n[2] == 2 && n[3] == 1 && n[4] == 1 && n[5] == 1)
+        return launch_delta_shape<Shape<3, 3, 2, 1, 1, 1>>(d, grid, s);
+    return launch_delta_shape<Generic>(d, grid, s);
 }
 
 }  // namespace amp

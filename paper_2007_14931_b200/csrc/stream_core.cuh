@@ -124,13 +124,19 @@ __device__ __forceinline__ void add_resonance(const StreamArgs& a, const ResEntr
 // spin, all with one radius, stored at ent[OFF..OFF+CNT): the loop unrolls and every constant becomes an
 // immediate constant-bank operand (no index arithmetic, no constant loads).  CNT < 0: generic model, runtime
 // loops over the barrier groups [g0, g1).
-template <int J, int LRv, int LBv, int CNT, int OFF, int SPIN>
+// SAVE: also store the group factors (F, G) of the thread's E events at fg[g * TILE + e] (delta.cu re-evaluates
+// Breit-Wigners of perturbed points from them).
+template <int J, int LRv, int LBv, int CNT, int OFF, int SPIN, bool SAVE = false>
 __device__ __forceinline__ void spin_sum(const StreamArgs& a, long long i0, const Ev& m2, const Ev& invm, const Ev& pR, const Ev& pB,
-                                         double2 (&Um)[E], double2 (&U0)[E], double2 (&Up)[E]) {
+                                         double2 (&Um)[E], double2 (&U0)[E], double2 (&Up)[E], double2* fg = nullptr) {
     double F[E], G[E];
     if (CNT >= 0) {
 #pragma unroll
         for (int e = 0; e < E; ++e) group_factors<LRv, LBv>(a.r2_spin[SPIN], invm.v[e], pR.v[e], pB.v[e], &F[e], &G[e]);
+        if (SAVE) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) fg[a.gstart[SPIN] * TILE + e] = make_double2(F[e], G[e]);
+        }
 #pragma unroll
         for (int t = 0; t < CNT; ++t) add_resonance<J>(a, a.ent[OFF + t], i0, m2, F, G, Um, U0, Up);
     } else {
@@ -138,6 +144,10 @@ __device__ __forceinline__ void spin_sum(const StreamArgs& a, long long i0, cons
             const BarrierGroup grp = a.grp[g];
 #pragma unroll
             for (int e = 0; e < E; ++e) group_factors<LRv, LBv>(grp.r2, invm.v[e], pR.v[e], pB.v[e], &F[e], &G[e]);
+            if (SAVE) {
+#pragma unroll
+                for (int e = 0; e < E; ++e) fg[g * TILE + e] = make_double2(F[e], G[e]);
+            }
             for (int t = grp.first; t < grp.first + grp.count; ++t) add_resonance<J>(a, a.ent[t], i0, m2, F, G, Um, U0, Up);
         }
     }
