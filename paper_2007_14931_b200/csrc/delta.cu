@@ -127,44 +127,13 @@ __device__ __forceinline__ void eval_slot(const StreamArgs& a, const double* rec
 }
 
 
-// One point for the thread's E events as a leaf of the reduction tree.  NORM: *v = sum_e w_e S_e; DATA: *v = product of
-// the mantissas of S_e, *ex = sum of their exponents.  `it` walks the contribution list; `sv` caches the current slot.
+// NORM: sum_e w_e S_e; DATA: mantissa product / exponent sum of the S_e (the tail of a leaf)
 template <bool NORM>
-__device__ __forceinline__ void leaf(const StreamArgs& a, const DeltaContrib* prog, const double* slots, int& it, const EvK (&k)[E],
-                                     const double2* fg, const double* zst, SlotVal (&sv)[E], const double (&w)[E], const bool (&live)[E],
-                                     bool& bad, double* v, int* ex) {
-    double2 Ap[E], Am[E];
-#pragma unroll
-    for (int e = 0; e < E; ++e) { Ap[e] = k[e].Ap; Am[e] = k[e].Am; }
-    int hdr;
-    do {
-        const int4 h4 = *reinterpret_cast<const int4*>(prog + it);            // hdr, slot, a (two words)
-        const double2 bc = *reinterpret_cast<const double2*>(&prog[it].b);    // b, c
-        ++it;
-        hdr = h4.x;
-        if (hdr & 16) continue;                                                 // empty point
-        if (hdr & 8) eval_slot(a, slots + h4.y, k, fg, zst, sv);
-        const double ca = __hiloint2double(h4.w, h4.z);
-        const int kind = hdr & 3;
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            double2 coef = make_double2(ca, bc.x);
-            if (kind) {
-                const double2 f = fg[((hdr >> 8) & 15) * TILE + e];
-                coef = bw_from_consts(ca, bc.x, bc.y, (hdr & 32) ? k[e].mZ2 : k[e].m2, f.x, f.y);
-                if (kind == 1) { coef.x -= sv[e].bw0.x; coef.y -= sv[e].bw0.y; }
-            }
-            Ap[e] = cfma(coef, sv[e].Sp, Ap[e]);
-            Am[e] = cfma(coef, sv[e].Sm, Am[e]);
-        }
-    } while (!(hdr & 4));
-    double S[E];
-#pragma unroll
-    for (int e = 0; e < E; ++e) S[e] = fma(Ap[e].x, Ap[e].x, fma(Ap[e].y, Ap[e].y, fma(Am[e].x, Am[e].x, Am[e].y * Am[e].y)));
+__device__ __forceinline__ void leaf_value(const double (&S)[E], const double (&w)[E], const bool (&live)[E], bool& bad, double* v, int* ex) {
     if (NORM) {
         double t = 0.0;
 #pragma unroll
-        for (int e = 0; e < E; ++e) { bad |= live[e] && !isfinite(S[e]); t = fma(w[e], S[e], t); }   // padding events carry w = 0
+        for (int e = 0; e < E; ++e) t = fma(w[e], S[e], t);
         *v = t;
         *ex = 0;
     } else {
@@ -181,6 +150,93 @@ __device__ __forceinline__ void leaf(const StreamArgs& a, const DeltaContrib* pr
         *v = f;
         *ex = x;
     }
+}
+
+// coef * SLOT of one contribution added to (Bp, Bm) -> (Ap, Am), for the thread's E events
+__device__ __forceinline__ void apply_contrib(int hdr, double ca, double2 bc, const EvK (&k)[E], const double2* fg, const SlotVal (&sv)[E],
+                                              const double2 (&Bp)[E], const double2 (&Bm)[E], double2 (&Ap)[E], double2 (&Am)[E]) {
+    const int kind = hdr & 3;
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        double2 coef = make_double2(ca, bc.x);
+        if (kind) {
+            const double2 f = fg[((hdr >> 8) & 15) * TILE + e];
+            coef = bw_from_consts(ca, bc.x, bc.y, (hdr & 32) ? k[e].mZ2 : k[e].m2, f.x, f.y);
+            if (kind == 1) { coef.x -= sv[e].bw0.x; coef.y -= sv[e].bw0.y; }
+        }
+        Ap[e] = cfma(coef, sv[e].Sp, Bp[e]);
+        Am[e] = cfma(coef, sv[e].Sm, Bm[e]);
+    }
+}
+
+// One point for the thread's E events as a leaf of the reduction tree.  NORM: *v = sum_e w_e S_e; DATA: *v = product of
+// the mantissas of S_e, *ex = sum of their exponents.  `it` walks the contribution list; `sv` caches the current slot.
+// The first contribution is applied straight onto A(0) (no copy of the four complex amplitudes per point).
+template <bool NORM>
+__device__ __forceinline__ void leaf(const StreamArgs& a, const DeltaContrib* prog, const double* slots, int& it, const EvK (&k)[E],
+                                     const double2* fg, const double* zst, SlotVal (&sv)[E], const double (&w)[E], const bool (&live)[E],
+                                     bool& bad, double* v, int* ex) {
+    double2 A0p[E], A0m[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) { A0p[e] = k[e].Ap; A0m[e] = k[e].Am; }
+    int4 h4 = *reinterpret_cast<const int4*>(prog + it);                      // hdr, slot, a (two words)
+    double2 bc = *reinterpret_cast<const double2*>(&prog[it].b);              // b, c
+    ++it;
+    int hdr = h4.x;
+    double S[E];
+    if ((hdr & 20) == 4) {
+        // the common gradient point: ONE contribution.  Its own copy of the tail keeps the amplitudes of the general
+        // path out of the merge (no register moves per point).
+        if (hdr & 8) eval_slot(a, slots + h4.y, k, fg, zst, sv);
+        double2 Ap[E], Am[E];
+        apply_contrib(hdr, __hiloint2double(h4.w, h4.z), bc, k, fg, sv, A0p, A0m, Ap, Am);
+#pragma unroll
+        for (int e = 0; e < E; ++e) S[e] = fma(Ap[e].x, Ap[e].x, fma(Ap[e].y, Ap[e].y, fma(Am[e].x, Am[e].x, Am[e].y * Am[e].y)));
+    } else {
+        double2 Ap[E], Am[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) { Ap[e] = A0p[e]; Am[e] = A0m[e]; }
+        if (!(hdr & 16)) {                                                    // (an empty point has S(p) = S(0))
+            for (;;) {
+                if (hdr & 8) eval_slot(a, slots + h4.y, k, fg, zst, sv);
+                apply_contrib(hdr, __hiloint2double(h4.w, h4.z), bc, k, fg, sv, Ap, Am, Ap, Am);
+                if (hdr & 4) break;
+                h4 = *reinterpret_cast<const int4*>(prog + it);
+                bc = *reinterpret_cast<const double2*>(&prog[it].b);
+                ++it;
+                hdr = h4.x;
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < E; ++e) S[e] = fma(Ap[e].x, Ap[e].x, fma(Ap[e].y, Ap[e].y, fma(Am[e].x, Am[e].x, Am[e].y * Am[e].y)));
+    }
+    leaf_value<NORM>(S, w, live, bad, v, ex);   // (NORM: a non-finite S makes the point's total non-finite: flagged at the end)
+}
+
+// Two consecutive single-contribution points of the same kind on the same slot (theta_k + h and theta_k - h of a
+// gradient step) as ONE straight-line block: 2 points x E events = four independent dependency chains, which is what
+// keeps the FP64 pipe busy with two warps per scheduler.
+template <bool NORM, int KIND>
+__device__ __forceinline__ void leaf_pair(const int4 (&h4)[2], const double2 (&bc)[2], const EvK (&k)[E], const double2* fg, const SlotVal (&sv)[E],
+                                          const double (&w)[E], const bool (&live)[E], bool& bad, double (&v)[2], int (&ex)[2]) {
+    double S[2][E];
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+        const double ca = __hiloint2double(h4[j].w, h4[j].z);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            double2 coef = make_double2(ca, bc[j].x);
+            if (KIND) {
+                const double2 f = fg[((h4[j].x >> 8) & 15) * TILE + e];
+                coef = bw_from_consts(ca, bc[j].x, bc[j].y, (h4[j].x & 32) ? k[e].mZ2 : k[e].m2, f.x, f.y);
+                if (KIND == 1) { coef.x -= sv[e].bw0.x; coef.y -= sv[e].bw0.y; }
+            }
+            const double2 Ap = cfma(coef, sv[e].Sp, k[e].Ap), Am = cfma(coef, sv[e].Sm, k[e].Am);
+            S[j][e] = fma(Ap.x, Ap.x, Ap.y * Ap.y) + fma(Am.x, Am.x, Am.y * Am.y);
+        }
+    }
+    leaf_value<NORM>(S[0], w, live, bad, &v[0], &ex[0]);
+    leaf_value<NORM>(S[1], w, live, bad, &v[1], &ex[1]);
 }
 
 // Recursive halving over the 32 lanes: `a` belongs to the earlier half of the points, `b` to the later half; lanes with
@@ -205,14 +261,35 @@ template <bool NORM>
 __device__ __forceinline__ void eval_block(const StreamArgs& a, const DeltaContrib* prog, const double* slots, int& it, const EvK (&k)[E],
                                            const double2* fg, const double* zst, SlotVal (&sv)[E], const double (&w)[E],
                                            const bool (&live)[E], bool& bad, int lane, double* v, int* ex) {
-    double s0 = 0, s1 = 0, s2 = 0, s3 = 0, s4 = 0;
-    int e0 = 0, e1 = 0, e2 = 0, e3 = 0, e4 = 0;
+    double s1 = 0, s2 = 0, s3 = 0, s4 = 0;
+    int e1 = 0, e2 = 0, e3 = 0, e4 = 0;
 #pragma unroll 1
-    for (int q = 0; q < 32; ++q) {
-        double x; int xe;
-        leaf<NORM>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, &x, &xe);
-        if (!(q & 1)) { s0 = x; e0 = xe; continue; }
-        halve<NORM>(0, lane, s0, e0, x, xe, &x, &xe);
+    for (int q = 0; q < 32; q += 2) {
+        double x0, x; int xe0, xe;
+        {
+            int4 h4[2];
+            double2 bc[2];
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                h4[j] = *reinterpret_cast<const int4*>(prog + it + j);
+                bc[j] = *reinterpret_cast<const double2*>(&prog[it + j].b);
+            }
+            // both single-contribution and non-empty, same coefficient kind, the second on the first one's slot
+            if ((h4[0].x & 20) == 4 && (h4[1].x & 28) == 4 && ((h4[0].x ^ h4[1].x) & 3) == 0) {
+                it += 2;
+                if (h4[0].x & 8) eval_slot(a, slots + h4[0].y, k, fg, zst, sv);
+                double v2[2]; int e2[2];
+                const int kind = h4[0].x & 3;
+                if (kind == 0) leaf_pair<NORM, 0>(h4, bc, k, fg, sv, w, live, bad, v2, e2);
+                else if (kind == 1) leaf_pair<NORM, 1>(h4, bc, k, fg, sv, w, live, bad, v2, e2);
+                else leaf_pair<NORM, 2>(h4, bc, k, fg, sv, w, live, bad, v2, e2);
+                x0 = v2[0]; xe0 = e2[0]; x = v2[1]; xe = e2[1];
+            } else {
+                leaf<NORM>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, &x0, &xe0);
+                leaf<NORM>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, &x, &xe);
+            }
+        }
+        halve<NORM>(0, lane, x0, xe0, x, xe, &x, &xe);
         if (!(q & 2)) { s1 = x; e1 = xe; continue; }
         halve<NORM>(1, lane, s1, e1, x, xe, &x, &xe);
         if (!(q & 4)) { s2 = x; e2 = xe; continue; }
@@ -400,6 +477,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_delta(const __grid_constant__ De
         __syncthreads();   // Z region (and the group factors) no longer needed: stream the next tile's Z columns
         if (have_z && tid == 0 && has_next) issue(tile + gridDim.x, 1);
     }
+    for (int b = 0; b < nblk; ++b) bad |= !isfinite(accN[b * THREADS + tid]);   // a non-finite S on the normalisation side
     if (bad) atomicOr(a.flag, 2);
 
     // ---- per-CTA partials: partial[(seg * rows + row) * stride + cta], seg 0 = sum log S (data), 1 = sum w S (norm);
