@@ -39,6 +39,11 @@ FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # 148 SMs x 64 DFMA/clk x 2 flop x 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed `ncu --set full` capture
 # (profiles/): per launch, at the default sizes; None until a capture of the current kernel exists
 TRAFFIC_NCU_BYTES = None
+TRAFFIC_NCU_BYTES_CFG4 = None
+# Algorithmic flop per event of the gradient batch of configs[4] in its sparse form: point 0 (730) + 31 slots
+# (Breit-Wigner of point 0 from the saved barrier factors ~20, angular factor ~8, two complex products 12) + 100 coupling
+# points (two complex multiply-adds 16, |A|^2 7, accumulate 2) + 20 mass/width points (perturbed Breit-Wigner ~22, the same 25)
+DELTA_FLOP_PER_EVENT = 730.0 + 31 * 40.0 + 100 * 25.0 + 20 * 47.0
 
 
 def measured_peaks():
@@ -207,7 +212,18 @@ def run_own(args):
     e2e = evals / t_wall
     hbm_peak, peak_kind = measured_peaks()
     norm_ms = float(np.mean(t_norm))
-    if args.cfg == 4:
+    if args.cfg == 4 and paths == {5}:
+        # gradient batch: one fused k_delta launch per step, bound by the plain FP64 ALUs (DESIGN.md 5.6 / 6)
+        k_ms = float(np.mean(t_data))
+        flop = DELTA_FLOP_PER_EVENT * (args.n_data + args.n_norm)
+        ach = flop / (k_ms * 1e-3) / 1e12
+        roof = {"bound": "alu", "kernel": "k_delta (gradient batch: point 0 + 120 sparse points, data then norm tiles, one launch)",
+                "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12,
+                "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md 6; the DFMA probe below measures it)", "unit": "TFLOP/s",
+                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": TRAFFIC_NCU_BYTES_CFG4, "kernel_ms": k_ms,
+                "flop_per_event": DELTA_FLOP_PER_EVENT, "flop_per_launch": flop,
+                "hbm_frac": (BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}
+    elif args.cfg == 4:
         roof = None
     elif paths == {4}:
         # one fused launch per step: lineshapes + combine + both reductions over the data tiles then the norm tiles
@@ -250,28 +266,36 @@ def run_own(args):
         dist.destroy_process_group()
 
 
-def cpu_baseline(args, budget_events=1_500_000):
-    """The oracle, as it stands, timed on this box's host cores on a bounded sample of the same workload:
-    same model and call pattern, sample sizes scaled down by the same factor for data and norm events;
-    data events drawn by oracle-driven accept-reject (no oracle input comes from the CUDA path)."""
+def cpu_baseline(args, target_evals=None):
+    """The oracle, as it stands, timed on this box's host cores on a bounded sample of the same workload (about 10-30 s
+    of CPU work): same model and call pattern, data and norm sizes scaled down by one factor (1 = the full workload) and
+    the evaluation repeated so that about `target_evals` event-evaluations are timed; data events drawn by
+    oracle-driven accept-reject (no oracle input comes from the CUDA path)."""
     from oracle import oracle as O
     cfg = args.cfg
     P = 121 if cfg == 4 else 1
-    budget = max(budget_events // P, 6000)
-    n = max(int(budget * args.n_data / (args.n_data + args.n_norm)), 1000)
-    m = max(budget - n, 5000)
+    if target_evals is None:   # ~10-20 s on 16 cores: the oracle shares an event's angles between the points of a batch
+        target_evals = 180_000_000 if P > 1 else 36_000_000
+    total = args.n_data + args.n_norm
+    frac = min(1.0, target_evals / (P * total))
+    n = max(int(args.n_data * frac), 1000)
+    m = max(int(args.n_norm * frac), 5000)
+    reps = max(1, int(round(target_evals / (P * (n + m)))))
     Mo = O.Model(W.DECAY, W.resonances(cfg))
     c = W.couplings(cfg)
     xn, wn = W.norm_events(cfg, m)
     x, eff = W.data_events(cfg, lambda xx, ee: Mo.eval_events(c, xx, ee), n=n)
-    cs, mws = step_params(cfg, c, 0)
-    t0 = time.perf_counter()
-    nll, _ = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
-    dt = time.perf_counter() - t0
-    full = dt * (args.n_data + args.n_norm) / (n + m)            # extrapolated time of one full-size call
+    dt = 0.0
+    for r in range(reps):
+        cs, mws = step_params(cfg, c, r)
+        t0 = time.perf_counter()
+        Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+        dt += time.perf_counter() - t0
+    full = dt / reps * total / (n + m)            # time of one full-size call (scaled linearly if the sample is smaller)
     return {"value": P / full, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
-            "sample": f"{n} data + {m} norm events (same model, P={P}), {dt:.2f} s measured, scaled linearly to {args.n_data}+{args.n_norm}",
-            "event_evals_per_s": P * (n + m) / dt}
+            "sample": f"{reps} x ({n} data + {m} norm events, same model, P={P}), {dt:.2f} s measured"
+                      + ("" if n + m == total else f", scaled linearly to {args.n_data}+{args.n_norm}"),
+            "event_evals_per_s": P * (n + m) * reps / dt}
 
 
 def run_reference(args):

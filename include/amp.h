@@ -111,6 +111,16 @@ amp_status amp_set_params(amp_model* m, int P, const double* h_couplings, const 
  * finite and positive: h_nll[p] = +inf for those points, the others are valid.                         */
 amp_status amp_nll(amp_model* m, double* h_nll, void* stream);
 
+/* The two sums behind amp_nll, for callers that shard the events over several devices or processes:
+ *   h_sum_log[p] = sum_i log S_i(p) over the loaded data events (without the efficiency), h_sum_wS[p] = sum_j w_j S_j(p)
+ * over the loaded normalisation events, host [P] each.  With the constants of amp_dataset_sums summed over the shards,
+ *   NLL(p) = -( sum_shards sum_log[p] + sum_shards sum_log_eff ) + N_total log( sum_shards sum_wS[p] / sum_shards sum_w ).
+ * Same launches, states and errors as amp_nll.                                                                       */
+amp_status amp_nll_terms(amp_model* m, double* h_sum_log, double* h_sum_wS, void* stream);
+/* Per-dataset constants fixed at load time: number of data events, sum_i log eps_i, number of normalisation events,
+ * sum_j w_j (0 for a sample that is not loaded).  Any output pointer may be NULL.                                     */
+amp_status amp_dataset_sums(const amp_model* m, long long* n_data, double* sum_log_eff, long long* n_norm, double* sum_w);
+
 /* Diagnostics / parity. */
 /* d_out device [n]: eps_i * S_i(p) of the loaded data events for point p of the last amp_set_params.   */
 amp_status amp_eval_events(amp_model* m, int p, double* d_out, void* stream);

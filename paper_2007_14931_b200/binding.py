@@ -18,7 +18,7 @@ AMP_MAX_RESONANCES, AMP_MAX_COUPLINGS, AMP_MAX_POINTS = 16, 48, 256
 # every symbol include/amp.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
-    "amp_load_norm", "amp_set_params", "amp_nll", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
+    "amp_load_norm", "amp_set_params", "amp_nll", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
     "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode",
     "amp_last_call_stats", "amp_last_call_timing", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
 ]
@@ -61,6 +61,8 @@ def lib():
         "amp_load_norm": (i, [vp, vp, vp, ll, vp]),
         "amp_set_params": (i, [vp, i, vp, vp]),
         "amp_nll": (i, [vp, vp, vp]),
+        "amp_nll_terms": (i, [vp, vp, vp, vp]),
+        "amp_dataset_sums": (i, [vp, C.POINTER(ll), pd, C.POINTER(ll), pd]),
         "amp_eval_events": (i, [vp, i, vp, vp]),
         "amp_norm_integral": (i, [vp, vp, vp]),
         "amp_dump_cache": (i, [vp, i, vp, pi, vp]),
@@ -177,6 +179,18 @@ class Model:
         if not (allow_domain_error and st == AMP_ERR_DOMAIN):
             self._check(st, "amp_nll")
         return out[:self.P]
+
+    def nll_terms(self, stream=None):
+        """(sum_i log S_i(p), sum_j w_j S_j(p)) of this model's own events, [P] each: the per-shard sums behind nll()"""
+        a, b = np.empty(max(self.P, 1)), np.empty(max(self.P, 1))
+        self._check(lib().amp_nll_terms(self._h, a.ctypes.data_as(C.c_void_p), b.ctypes.data_as(C.c_void_p), _stream_ptr(stream)), "amp_nll_terms")
+        return a[:self.P], b[:self.P]
+
+    def dataset_sums(self):
+        """(n_data, sum_i log eps_i, n_norm, sum_j w_j)"""
+        n, m, sl, sw = C.c_longlong(), C.c_longlong(), C.c_double(), C.c_double()
+        self._check(lib().amp_dataset_sums(self._h, C.byref(n), C.byref(sl), C.byref(m), C.byref(sw)), "amp_dataset_sums")
+        return n.value, sl.value, m.value, sw.value
 
     def norm_integral(self, stream=None):
         out = np.empty(max(self.P, 1), dtype=np.float64)

@@ -213,7 +213,7 @@ struct StreamArgs {
     long long n2, npad2;
     double* partial2;               // [grid] sum w S
     unsigned int* ticket;           // device counter, 0 between launches
-    double* result;                 // [3]: NLL, I, domain flag
+    double* result;                 // [5]: NLL, I, domain flag, sum log S, sum w S
     double sum_log_eff, wsum;
 };
 cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s);
@@ -250,7 +250,7 @@ struct DeltaArgs {
     int P;
     double* partial;                // [2][1 + nsorted][stride] per-CTA partials: sum log S (data) and sum w S (norm); row 0 = point 0
     int stride;
-    double* result;                 // [2 P + 1]: NLL[P], I[P], domain flag
+    double* result;                 // [4 P + 1]: NLL[P], I[P], domain flag, sum log S [P], sum w S [P]
     int want_nll;
     int first_chunk;                // 0: a later launch of the same call: the domain flag adds to the earlier launches'
 };

@@ -50,10 +50,11 @@ struct amp_model {
     // scratch
     double* d_partial = nullptr;   // [2 * AMP_MAX_POINTS][PARTIAL_STRIDE]
     double* d_sums = nullptr;      // [2 * AMP_MAX_POINTS]
-    double* d_result = nullptr;    // [2 * AMP_MAX_POINTS]
+    double* d_result = nullptr;    // [4 * AMP_MAX_POINTS + 4]: NLL[P], I[P], domain flag, sum log S [P], sum w S [P]
     int* d_flag = nullptr;
     unsigned int* d_ticket = nullptr;   // last-CTA ticket of the fused single-launch step (0 between launches)
-    double* h_pinned = nullptr;    // [2 * AMP_MAX_POINTS + 2]
+    double* h_pinned = nullptr;    // same layout
+    std::vector<double> last_slog, last_swS;   // the two sums of the last amp_nll, per point (amp_nll_terms)
 
     // batched (P > 1) plan buffers: coefficient fragments, basis entries, sparse items
     unsigned char* d_plan = nullptr;
@@ -262,12 +263,12 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { delete m; return AMP_ERR_CUDA; }
     cudaError_t e = cudaMalloc(&m->d_partial, sizeof(double) * 2 * AMP_MAX_POINTS * PARTIAL_STRIDE);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_sums, sizeof(double) * 2 * AMP_MAX_POINTS);
-    if (e == cudaSuccess) e = cudaMalloc(&m->d_result, sizeof(double) * (2 * AMP_MAX_POINTS + 2));
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_result, sizeof(double) * (4 * AMP_MAX_POINTS + 4));
     if (e == cudaSuccess) e = cudaMalloc(&m->d_flag, sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&m->d_ticket, sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(m->d_ticket, 0, sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(m->d_flag, 0, sizeof(int));
-    if (e == cudaSuccess) e = cudaMallocHost(&m->h_pinned, sizeof(double) * (2 * AMP_MAX_POINTS + 2));
+    if (e == cudaSuccess) e = cudaMallocHost(&m->h_pinned, sizeof(double) * (4 * AMP_MAX_POINTS + 4));
     for (int i = 0; i < 5 && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ev[i]);
     if (e != cudaSuccess) { amp_model_destroy(m); return e == cudaErrorMemoryAllocation ? AMP_ERR_NOMEM : AMP_ERR_CUDA; }
     *out = m;
@@ -1126,8 +1127,10 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
             m->stat_launches++;
         }
         CK(cudaEventRecord(m->ev[1], s));
-        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (2 * P + 1), cudaMemcpyDeviceToHost, s));
+        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (4 * P + 1), cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));
+        m->last_slog.assign(m->h_pinned + 2 * P + 1, m->h_pinned + 3 * P + 1);
+        m->last_swS.assign(m->h_pinned + 3 * P + 1, m->h_pinned + 4 * P + 1);
         m->stat_norm_path = 5;
         m->fused_valid = true;
         bool bad = m->h_pinned[2 * P] != 0.0;
@@ -1153,8 +1156,10 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         CK(cudaEventRecord(m->ev[0], s));
         CK(launch_stream(a, stream_grid_fused(m->data.n, m->norm.n, m->has_z), s));
         CK(cudaEventRecord(m->ev[1], s));
-        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 3, cudaMemcpyDeviceToHost, s));
+        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 5, cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));
+        m->last_slog.assign(1, m->h_pinned[3]);
+        m->last_swS.assign(1, m->h_pinned[4]);
         m->stat_launches = 1;
         m->stat_norm_path = 4;
         m->fused_valid = true;
@@ -1256,9 +1261,12 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
     m->stat_launches += 2;
     CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 2 * P, cudaMemcpyDeviceToHost, s));
     CK(cudaMemcpyAsync(m->h_pinned + 2 * P, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(m->h_pinned + 2 * P + 1, m->d_sums, sizeof(double) * 2 * P, cudaMemcpyDeviceToHost, s));
     CK(cudaEventRecord(m->ev[4], s));
     CK(cudaStreamSynchronize(s));
     m->ev_valid = true;
+    m->last_slog.assign(m->h_pinned + 2 * P + 1, m->h_pinned + 3 * P + 1);
+    m->last_swS.assign(m->h_pinned + 3 * P + 1, m->h_pinned + 4 * P + 1);
     int flag;
     std::memcpy(&flag, m->h_pinned + 2 * P, sizeof(int));
     bool bad = flag != 0;
@@ -1278,6 +1286,25 @@ amp_status amp_nll(amp_model* m, double* h_nll, void* stream) {
     if (!m) return AMP_ERR_INVALID;
     if (!h_nll) return fail(m, AMP_ERR_INVALID, "amp_nll: null output");
     return evaluate(m, true, h_nll, nullptr, (cudaStream_t)stream);
+}
+
+amp_status amp_nll_terms(amp_model* m, double* h_sum_log, double* h_sum_wS, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    if (!h_sum_log || !h_sum_wS) return fail(m, AMP_ERR_INVALID, "amp_nll_terms: null output");
+    std::vector<double> nll((size_t)std::max(m->P, 1));
+    const amp_status st = evaluate(m, true, nll.data(), nullptr, (cudaStream_t)stream);
+    if (st != AMP_OK && st != AMP_ERR_DOMAIN) return st;
+    for (int p = 0; p < m->P; ++p) { h_sum_log[p] = m->last_slog[p]; h_sum_wS[p] = m->last_swS[p]; }
+    return st;
+}
+
+amp_status amp_dataset_sums(const amp_model* m, long long* n_data, double* sum_log_eff, long long* n_norm, double* sum_w) {
+    if (!m) return AMP_ERR_INVALID;
+    if (n_data) *n_data = m->data.loaded ? m->data.n : 0;
+    if (sum_log_eff) *sum_log_eff = m->data.loaded ? m->data.wsum : 0.0;
+    if (n_norm) *n_norm = m->norm.loaded ? m->norm.n : 0;
+    if (sum_w) *sum_w = m->norm.loaded ? m->norm.wsum : 0.0;
+    return AMP_OK;
 }
 
 amp_status amp_norm_integral(amp_model* m, double* h_I, void* stream) {

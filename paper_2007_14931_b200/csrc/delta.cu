@@ -521,6 +521,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_delta(const __grid_constant__ De
         if (p < 0) continue;
         const double I = tot[rows + r] / a.wsum;
         d.result[d.P + p] = I;
+        d.result[2 * d.P + 1 + p] = tot[r];
+        d.result[3 * d.P + 1 + p] = tot[rows + r];
         double v = -(tot[r] + a.sum_log_eff) + (double)a.n * log(I);
         if (!isfinite(v) || !(I > 0.0)) v = INFINITY;
         d.result[p] = d.want_nll ? v : 0.0;

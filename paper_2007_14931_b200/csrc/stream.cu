@@ -182,6 +182,8 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         if (!isfinite(v) || !(I > 0.0)) v = INFINITY;
         a.result[0] = v;
         a.result[1] = I;
+        a.result[3] = slog;
+        a.result[4] = swS;
         a.result[2] = (double)atomicExch(a.flag, 0);   // domain flag of this call, cleared for the next one
         *a.ticket = 0u;
     }

@@ -418,3 +418,45 @@ def test_mass_width_override_equals_new_model():
     a = M.nll(c, xn[:, :100], wn[:100], xn, wn, mass_width=mw[None])[0][0]
     b = O.Model(DEC, res2).nll(c, xn[:, :100], wn[:100], xn, wn)[0][0]
     assert a == b
+
+
+# ------------------------------------------------------------------ golden fixtures (tests/golden/)
+GOLDEN = __import__("os").path.join(__import__("os").path.dirname(__import__("os").path.abspath(__file__)), "golden")
+
+
+def test_golden_wigner_d_exact_values():
+    """tests/golden/wigner_d_exact.txt: exact surd values of the PDG d-function table at pi/3 and pi/2 (hand-written
+    expressions, evaluated here with math.sqrt) against the oracle's factorial sum."""
+    n = 0
+    for line in open(__import__("os").path.join(GOLDEN, "wigner_d_exact.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        j, mp, m, b, expr = line.split(None, 4)
+        beta = eval(b, {"pi": math.pi})
+        val = eval(expr, {"sqrt": math.sqrt})
+        assert abs(O.wigner_d(int(j), int(mp), int(m), beta) - val) < 3e-16 + 1e-15 * abs(val), line
+        n += 1
+    assert n >= 20
+
+
+def test_golden_oracle_regression():
+    """tests/golden/oracle_regression.json (written by make_golden.py from oracle/ only): the oracle still gives the stored
+    values — guards against silent drift of its arithmetic; correctness is pinned by P1-P12 above."""
+    import json
+    g = json.load(open(__import__("os").path.join(GOLDEN, "oracle_regression.json")))
+    for cfg in (0, 1, 2):
+        e = g["configs"][str(cfg)]
+        Mo = model(cfg)
+        c = W.couplings(cfg)
+        xn, wn = W.norm_events(cfg, e["n_norm"])
+        x, eff = W.data_events(cfg, lambda xx, ee: Mo.eval_events(c, xx, ee), n=e["n_data"])
+        assert [float(t).hex() for t in x[:, 0]] == e["x0"]            # the seeded generators are unchanged
+        v = Mo.eval_events(c, x, eff)
+        ref = np.array([float.fromhex(t) for t in e["eps_S"]])
+        assert np.max(np.abs(v[:12] - ref) / ref) < 1e-13
+        B = Mo.basis_terms(x[:, 0]).ravel()
+        Bref = np.array([complex(float.fromhex(a), float.fromhex(b)) for a, b in e["basis_terms_event0"]])
+        assert np.max(np.abs(B - Bref)) < 1e-13 * np.max(np.abs(Bref))
+        nll, integral = Mo.nll(c, x, eff, xn, wn)
+        assert abs(nll[0] - float.fromhex(e["nll"])) < 1e-12 * abs(nll[0])
+        assert abs(integral[0] - float.fromhex(e["integral"])) < 1e-13 * integral[0]

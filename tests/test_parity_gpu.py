@@ -291,6 +291,41 @@ def test_delta_batches_general():
         assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
 
 
+def test_nll_terms_of_two_shards_add_up():
+    """amp_nll_terms / amp_dataset_sums: the per-shard sums of two models that each hold half of the events combine
+    (sharded.py's formula, here without a process group) to the oracle's NLL of the whole sample — for the fused
+    P = 1 launch, the gradient-batch kernel and the separate-launch path."""
+    from paper_2007_14931_b200 import sharded as S
+    cfg = 2
+    Mo = oracle_model(cfg)
+    x, eff, xn, wn = make_inputs(cfg, 4001, 9001)
+    shards = []
+    for r in range(2):
+        lo, hi = S.shard_bounds(x.shape[1], r, 2)
+        ln, hn = S.shard_bounds(xn.shape[1], r, 2)
+        Mg = gpu_model(cfg)
+        Mg.load_events(dev(x[:, lo:hi]), dev(eff[lo:hi]))
+        Mg.load_norm(dev(xn[:, ln:hn]), dev(wn[ln:hn]))
+        shards.append(Mg)
+    c = W.couplings(cfg)
+    cs4, mws4 = W.fit_points(4)
+    for cs, mws, fused_mode, path in ((c[None], None, 0, 4), (c[None], None, 1, 1), (cs4[:40], mws4[:40], 0, 5)):
+        tot = np.zeros(4)
+        sl, sw = 0.0, 0.0
+        for Mg in shards:
+            Mg.set_fused_mode(fused_mode)
+            Mg.set_params(cs, mws)
+            a, b = Mg.nll_terms()
+            assert Mg.last_call_stats()["norm_path"] == path
+            sl, sw = sl + a, sw + b
+            tot += np.array(Mg.dataset_sums())
+        assert tot[0] == x.shape[1] and tot[2] == xn.shape[1]
+        assert abs(tot[1] - np.sum(np.log(eff))) < 1e-9 and abs(tot[3] - np.sum(wn)) < 1e-9 * tot[3]
+        nll = -(sl + tot[1]) + tot[0] * np.log(sw / tot[3])
+        ref, _ = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+        assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
+
+
 def test_norm_matrix_matches_oracle_and_direct_sum():
     """a4: the Hermitian matrix M from the HERK kernel against the oracle's plain double loop, and c^H M c against
     the direct sum (pin P10 on the GPU side)."""
