@@ -166,6 +166,12 @@ amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_r
  * the others 0.                                                                                          */
 amp_status amp_last_call_timing(const amp_model* m, double* ms4);
 
+/* Device time [ms] of the launches of the most recent single-launch evaluations (paths 4 and 5), from CUDA event pairs
+ * recorded around them on the call's stream and kept in a ring of 256: h_ms[0 .. *n_out) = the last min(max_calls, 256,
+ * calls so far) such evaluations, oldest first.  Reading costs nothing in the timed calls themselves (bench.py's
+ * roofline).  The evaluations must have completed (amp_nll is synchronous).                                        */
+amp_status amp_recent_launch_ms(const amp_model* m, int max_calls, double* h_ms, int* n_out);
+
 const char* amp_last_error(const amp_model* m);
 const char* amp_status_string(amp_status s);
 const char* amp_version(void);

@@ -20,7 +20,7 @@ SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
     "amp_load_norm", "amp_set_params", "amp_nll", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
     "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode",
-    "amp_last_call_stats", "amp_last_call_timing", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
+    "amp_last_call_stats", "amp_last_call_timing", "amp_recent_launch_ms", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
 ]
 
 
@@ -75,6 +75,7 @@ def lib():
         "amp_set_fused_mode": (i, [vp, i]),
         "amp_last_call_stats": (i, [vp, pi, pi, pi]),
         "amp_last_call_timing": (i, [vp, pd]),
+        "amp_recent_launch_ms": (i, [vp, i, pd, pi]),
         "amp_last_error": (C.c_char_p, [vp]),
         "amp_status_string": (C.c_char_p, [i]),
         "amp_version": (C.c_char_p, []),
@@ -249,6 +250,17 @@ class Model:
         ms = (C.c_double * 4)()
         self._check(lib().amp_last_call_timing(self._h, ms), "amp_last_call_timing")
         return {"lineshape_ms": ms[0], "data_ms": ms[1], "norm_ms": ms[2], "final_ms": ms[3]}
+
+
+def _recent_launch_ms(self, max_calls=256):
+    """device ms of the launches of the most recent fused / gradient-batch evaluations, oldest first"""
+    buf = (C.c_double * max(max_calls, 1))()
+    n = C.c_int(0)
+    self._check(lib().amp_recent_launch_ms(self._h, int(max_calls), buf, C.byref(n)), "amp_recent_launch_ms")
+    return np.array(buf[:n.value])
+
+
+Model.recent_launch_ms = _recent_launch_ms
 
 
 def probe_fp64(kind, iters=2000, stream=None):

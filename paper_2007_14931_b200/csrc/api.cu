@@ -82,7 +82,11 @@ struct amp_model {
     int stat_launches = 0, stat_columns = 0, stat_norm_path = 0, stat_batched = 0, stat_gram_built = 0;
     cudaEvent_t ev[5]{};           // phase boundaries of the last evaluation (amp_last_call_timing)
     bool ev_valid = false;
-    bool fused_valid = false;      // the last evaluation was the fused single launch: ev[0], ev[1] bracket it
+    bool fused_valid = false;      // the last evaluation was one fused launch (or the gradient-batch launches): ring[ring_last] brackets it
+    enum { RING = 256 };
+    cudaEvent_t ring[2 * RING]{};  // event pairs around the launches of the fused / gradient-batch evaluations, newest at ring_last
+    int ring_last = -1;
+    long long ring_calls = 0;      // such evaluations since amp_model_create (amp_recent_launch_ms)
     bool use_delta = false;        // P > 1 and the points are sparse changes of point 0: gradient-batch kernel (delta.cu)
     struct DeltaChunk { int p0, np, nsorted; std::vector<DeltaContrib> contrib; std::vector<double> slots; };
     std::vector<DeltaChunk> delta_chunks;     // compiled program of the last amp_set_params (points p0 .. p0 + np - 1 per launch)
@@ -270,6 +274,7 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
     if (e == cudaSuccess) e = cudaMemset(m->d_flag, 0, sizeof(int));
     if (e == cudaSuccess) e = cudaMallocHost(&m->h_pinned, sizeof(double) * (4 * AMP_MAX_POINTS + 4));
     for (int i = 0; i < 5 && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ev[i]);
+    for (int i = 0; i < 2 * amp_model::RING && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ring[i]);
     if (e != cudaSuccess) { amp_model_destroy(m); return e == cudaErrorMemoryAllocation ? AMP_ERR_NOMEM : AMP_ERR_CUDA; }
     *out = m;
     return AMP_OK;
@@ -293,6 +298,7 @@ amp_status amp_model_destroy(amp_model* m) {
     if (m->d_hk) cudaFree(m->d_hk);
     if (m->h_hk) cudaFreeHost(m->h_hk);
     for (int i = 0; i < 5; ++i) if (m->ev[i]) cudaEventDestroy(m->ev[i]);
+    for (int i = 0; i < 2 * amp_model::RING; ++i) if (m->ring[i]) cudaEventDestroy(m->ring[i]);
     delete m;
     return AMP_OK;
 }
@@ -347,7 +353,7 @@ amp_status amp_last_call_timing(const amp_model* m, double* ms4) {
     if (!m || !ms4) return AMP_ERR_INVALID;
     if (m->fused_valid) {   // one launch: everything is reported as the combine phase of both samples
         float t = 0;
-        if (cudaEventElapsedTime(&t, m->ev[0], m->ev[1]) != cudaSuccess) return AMP_ERR_CUDA;
+        if (cudaEventElapsedTime(&t, m->ring[2 * m->ring_last], m->ring[2 * m->ring_last + 1]) != cudaSuccess) return AMP_ERR_CUDA;
         ms4[0] = 0; ms4[1] = t; ms4[2] = 0; ms4[3] = 0;
         return AMP_OK;
     }
@@ -357,6 +363,20 @@ amp_status amp_last_call_timing(const amp_model* m, double* ms4) {
         if (cudaEventElapsedTime(&t, m->ev[i], m->ev[i + 1]) != cudaSuccess) return AMP_ERR_CUDA;
         ms4[i] = t;
     }
+    return AMP_OK;
+}
+
+amp_status amp_recent_launch_ms(const amp_model* m, int max_calls, double* h_ms, int* n_out) {
+    if (!m || !h_ms || !n_out || max_calls < 0) return AMP_ERR_INVALID;
+    const long long have = std::min<long long>(m->ring_calls, amp_model::RING);
+    const int n = (int)std::min<long long>(have, max_calls);
+    for (int i = 0; i < n; ++i) {   // oldest of the n first
+        const int slot = ((m->ring_last - (n - 1 - i)) % amp_model::RING + amp_model::RING) % amp_model::RING;
+        float t = 0;
+        if (cudaEventElapsedTime(&t, m->ring[2 * slot], m->ring[2 * slot + 1]) != cudaSuccess) return AMP_ERR_CUDA;
+        h_ms[i] = t;
+    }
+    *n_out = n;
     return AMP_OK;
 }
 
@@ -1111,7 +1131,9 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
             for (int q = 0; q < ch.nsorted; ++q) hp[q] = q < ch.np ? ch.p0 + q : -1;
             off += bC + bS + al(ch.nsorted * sizeof(int));
         }
-        CK(cudaEventRecord(m->ev[0], s));
+        m->ring_last = (m->ring_last + 1) % amp_model::RING;
+        m->ring_calls++;
+        CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
         CK(cudaMemcpyAsync(m->d_plan, m->h_plan, off, cudaMemcpyHostToDevice, s));
         for (size_t c = 0; c < m->delta_chunks.size(); ++c) {
             const auto& ch = m->delta_chunks[c];
@@ -1126,7 +1148,7 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
             CK(launch_delta(d, delta_grid(d.a.n, d.a.n2), s));
             m->stat_launches++;
         }
-        CK(cudaEventRecord(m->ev[1], s));
+        CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
         CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (4 * P + 1), cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));
         m->last_slog.assign(m->h_pinned + 2 * P + 1, m->h_pinned + 3 * P + 1);
@@ -1153,9 +1175,11 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         a.result = m->d_result;
         a.sum_log_eff = m->data.wsum;
         a.wsum = m->norm.wsum;
-        CK(cudaEventRecord(m->ev[0], s));
+        m->ring_last = (m->ring_last + 1) % amp_model::RING;
+        m->ring_calls++;
+        CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
         CK(launch_stream(a, stream_grid_fused(m->data.n, m->norm.n, m->has_z), s));
-        CK(cudaEventRecord(m->ev[1], s));
+        CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
         CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 5, cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));
         m->last_slog.assign(1, m->h_pinned[3]);

@@ -18,6 +18,16 @@
 // the warp's 64 events.  Data side: S = f 2^e is split with integer ops, mantissas are multiplied and exponents
 // added, so the sum of logs takes ONE log per (point, warp) at the very end instead of one per (point, event).
 // Everything is fixed-order: bit-reproducible.  Bound: plain FP64 ALUs.
+// Two events per thread x 256 threads (as k_stream).  Measured alternative: one event per thread x 512 threads (16 warps,
+// 128 registers) hides latency better but pays the warp-uniform per-point overhead twice: 6.20 ms vs 6.12 ms on configs[4].
+#ifndef AMP_DELTA_E
+#define AMP_DELTA_E 2
+#endif
+#ifndef AMP_DELTA_THREADS
+#define AMP_DELTA_THREADS 256
+#endif
+#define AMP_STREAM_E AMP_DELTA_E
+#define AMP_STREAM_THREADS AMP_DELTA_THREADS
 #include "stream_core.cuh"
 
 namespace amp {
@@ -323,7 +333,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_delta(const __grid_constant__ De
     DeltaContrib* prog = reinterpret_cast<DeltaContrib*>(accE + DBLK * THREADS);  // [DELTA_MAX_CONTRIB]
     double* slots = reinterpret_cast<double*>(prog + DELTA_MAX_CONTRIB);          // [DELTA_MAX_SLOTWORDS]
     uint64_t* full = reinterpret_cast<uint64_t*>(slots + DELTA_MAX_SLOTWORDS);    // [2]
-    __shared__ double sm[8];
+    __shared__ double sm[NWARPS];
     __shared__ bool s_last;
     for (int b = 0; b < DBLK; ++b) { accN[b * THREADS + tid] = 0.0; accF[b * THREADS + tid] = 1.0; accE[b * THREADS + tid] = 0; }
     for (int i = tid; i < d.ncontrib * 4; i += THREADS) reinterpret_cast<double*>(prog)[i] = reinterpret_cast<const double*>(d.contrib)[i];

@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         issue_tile<MODE>(a, ntd, blockIdx.x, stage, &full[0], 0, NCOL_K, true, ncache);
         if (have_z) issue_tile<MODE>(a, ntd, blockIdx.x, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
     }
-    __shared__ double sm[8];
+    __shared__ double sm[NWARPS];
     uint32_t parity = 0;
     bool in_norm = false;   // MODE_FUSED: this CTA has passed from the data tiles to the normalisation tiles
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, parity ^= 1) {

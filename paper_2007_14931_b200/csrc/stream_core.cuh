@@ -17,7 +17,11 @@ namespace amp {
 #endif
 constexpr int E = AMP_STREAM_E;
 
-constexpr int THREADS = 256;
+#ifndef AMP_STREAM_THREADS
+#define AMP_STREAM_THREADS 256
+#endif
+constexpr int THREADS = AMP_STREAM_THREADS;
+constexpr int NWARPS = THREADS / 32;
 constexpr int TILE = THREADS * E;          // events per pipeline stage
 
 struct Ev {   // per-thread event registers
@@ -91,7 +95,7 @@ __device__ __forceinline__ double block_sum(double v, double* sm) {
     __syncthreads();
     double t = 0.0;
     if (threadIdx.x == 0)
-        for (int wv = 0; wv < 8; ++wv) t += sm[wv];
+        for (int wv = 0; wv < NWARPS; ++wv) t += sm[wv];
     return t;
 }
 // sum of the per-CTA partials in the order k_finalize uses (thread t adds b = t, t + 256, ...; fixed tree): every thread calls it

@@ -309,7 +309,7 @@ def test_nll_terms_of_two_shards_add_up():
         shards.append(Mg)
     c = W.couplings(cfg)
     cs4, mws4 = W.fit_points(4)
-    for cs, mws, fused_mode, path in ((c[None], None, 0, 4), (c[None], None, 1, 1), (cs4[:40], mws4[:40], 0, 5)):
+    for cs, mws, fused_mode, path in ((c[None], None, 0, 4), (c[None], None, 1, 2), (cs4[:40], mws4[:40], 0, 5)):   # (2: same masses twice -> matrix M)
         tot = np.zeros(4)
         sl, sw = 0.0, 0.0
         for Mg in shards:
