@@ -1,8 +1,11 @@
 // amp_internal.cuh — shared declarations of the CUDA path (product code; shares nothing with oracle/).
 //
 // Data layout in HBM:
-//   kinematics cache  double[NCOL][npad]   structure-of-arrays, one column per cached quantity,
-//                                          npad = n rounded up to whole pipeline tiles (stream_pad)
+//   kinematics cache  double[npad/512][NCOL + 1][512]   tiled structure-of-arrays: blocks of 512 events, inside a block
+//                                          one 4 KB column per cached quantity and the event weights as the last
+//                                          column.  A streaming tile is ONE contiguous block (94 KB with the Z
+//                                          chain): a CTA reads it with three bulk copies and HBM sees long sequential
+//                                          bursts instead of 23 scattered 4 KB pieces.  npad = n rounded up to 512.
 //   lineshape columns double2[ncol][npad]  complex A^R(m_i) (re, im) interleaved: one 128-bit load
 //                                          per (event, column)
 // One thread owns one event at a time; a warp reads 32 consecutive doubles (256 B) of a cache
@@ -55,8 +58,7 @@ struct LineConst {
 
 struct Dataset {
     long long n = 0, npad = 0;
-    double* cache = nullptr;   // [NCOL][npad]
-    double* weight = nullptr;  // [npad] eps_i (data) or w_j (norm); 1 if the caller gave none
+    double* cache = nullptr;   // [npad / 512][ncache + 1][512]; last column: eps_i (data) or w_j (norm), 1 if the caller gave none
     double2* cols = nullptr;   // lineshape column pool [capacity][npad]
     int ncache = 0;            // columns present (NCOL_K or NCOL_ALL)
     double wsum = 0;           // sum_j w_j (norm) ; sum_i log eps_i (data)
@@ -64,6 +66,13 @@ struct Dataset {
 };
 
 static inline long long pad32(long long n) { return (n + 31) / 32 * 32; }
+
+// ---- tiled cache addressing --------------------------------------------------------------------------
+constexpr int CACHE_TILE = 512;
+// element (col, i) of a cache with ncolw = ncache + 1 columns per block (the weight is column ncache)
+__host__ __device__ __forceinline__ size_t cache_idx(int ncolw, int col, long long i) {
+    return ((size_t)(i / CACHE_TILE) * ncolw + col) * CACHE_TILE + (size_t)(i % CACHE_TILE);
+}
 
 // ---- device helpers ------------------------------------------------------------------------------
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
@@ -148,8 +157,8 @@ struct KinArgs {
     DecayConst dk;
     const double* x;      // [4][n] input events (borrowed)
     const double* w;      // [n] or null
-    double* cache;        // [ncache][npad]
-    double* weight;       // [npad]
+    double* cache;        // tiled, ncolw columns per block (the last one receives the weight)
+    int ncolw;
     long long n, npad;
     int with_z;           // also fill the Z-chain columns
     int weight_positive;  // 1: weights must be > 0 (eps), 0: >= 0 (norm weights)
@@ -199,8 +208,8 @@ struct StreamArgs {
     int shape_fixed;                // 1: one radius per spin, r2_spin valid: a shape-specialised kernel may run
     double r2_spin[6];
     double2 cconst;                 // sum of the couplings of the constant (lineshape == 1) terms
-    const double* cache;
-    const double* weight;
+    const double* cache;            // tiled cache of the (first) sample, ncolw columns per 512-event block
+    int ncolw;
     const double2* cols;
     long long n, npad;
     double* partial;                // [grid] (MODE_DATA: sum log S; MODE_NORM: sum w S)
@@ -209,7 +218,6 @@ struct StreamArgs {
     int mode;
     // MODE_FUSED: the normalisation sample (second dataset), its partials, and what the last CTA needs to finish the NLL
     const double* cache2;
-    const double* weight2;
     long long n2, npad2;
     double* partial2;               // [grid] sum w S
     unsigned int* ticket;           // device counter, 0 between launches
@@ -261,8 +269,8 @@ bool delta_fits(int ngrp);
 // Batched combine (P > 1) on the FP64 tensor cores, see batch.cu
 enum { BATCH_NKT = 14, BATCH_POINTS = 128, BATCH_MAX_COLS = 48 };   // dense k-tiles (2K <= 56 realified rows) and points per launch
 struct BatchArgs {
-    const double* cache;
-    const double* weight;
+    const double* cache;    // tiled cache, ncolw columns per block (weight last)
+    int ncolw;
     const double2* cols;
     long long n, npad;
     const double* Adense;   // [16 octets][re/im][BATCH_NKT][32 lanes]: coefficient fragments of the K base entries

@@ -159,7 +159,6 @@ bool make_line_const(const amp_model* m, int r, double mass, double width, LineC
 
 void free_dataset(Dataset& d) {
     if (d.cache) cudaFree(d.cache);
-    if (d.weight) cudaFree(d.weight);
     if (d.cols) cudaFree(d.cols);
     d = Dataset{};
 }
@@ -173,8 +172,7 @@ amp_status load_dataset(amp_model* m, Dataset& d, bool is_norm, const double* d_
     d.n = n;
     d.npad = stream_pad(n > 0 ? n : 1);
     d.ncache = m->has_z ? NCOL_ALL : NCOL_K;
-    CK(cudaMalloc(&d.cache, sizeof(double) * d.ncache * d.npad));
-    CK(cudaMalloc(&d.weight, sizeof(double) * d.npad));
+    CK(cudaMalloc(&d.cache, sizeof(double) * (d.ncache + 1) * d.npad));   // tiled: [npad / 512][ncache + 1][512], weight last
     CK(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
     const int grid = kinematics_grid(d.npad);
     KinArgs a{};
@@ -182,7 +180,7 @@ amp_status load_dataset(amp_model* m, Dataset& d, bool is_norm, const double* d_
     a.x = d_x;
     a.w = d_w;
     a.cache = d.cache;
-    a.weight = d.weight;
+    a.ncolw = d.ncache + 1;
     a.n = n;
     a.npad = d.npad;
     a.with_z = m->has_z ? 1 : 0;
@@ -717,12 +715,21 @@ void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, Str
             a->cconst.x += cp[0]; a->cconst.y += cp[1];
         }
     a->cache = d.cache;
-    a->weight = d.weight;
+    a->ncolw = (m->has_z ? NCOL_ALL : NCOL_K) + 1;
     a->cols = d.cols;
     a->n = d.n;
     a->npad = d.npad;
     a->flag = m->d_flag;
     a->mode = mode;
+}
+
+// plain [column][n] copy of the tiled cache (amp_dump_cache)
+__global__ void k_dump_cache(const double* __restrict__ cache, int ncolw, int ncols, long long n, double* __restrict__ out) {
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n * ncols; idx += (long long)gridDim.x * blockDim.x) {
+        const int c = (int)(idx / n);
+        const long long i = idx % n;
+        out[idx] = cache[cache_idx(ncolw, c, i)];
+    }
 }
 
 // nll[p] = -(sum_i log S_i + sum_i log eps_i) + N log I(p), I(p) = sum_j w_j S_j / sum_j w_j
@@ -876,7 +883,7 @@ amp_status run_batch(amp_model* m, const Dataset& d, const BatchPlan& bp, int Pc
     if (bIA) std::memcpy(m->h_plan + oIA, bp.itemA.data(), bIA);
     CK(cudaMemcpyAsync(m->d_plan + plan_off, m->h_plan + plan_off, end - plan_off, cudaMemcpyHostToDevice, s));
     BatchArgs a{};
-    a.cache = d.cache; a.weight = d.weight; a.cols = d.cols; a.n = d.n; a.npad = d.npad;
+    a.cache = d.cache; a.ncolw = d.ncache + 1; a.cols = d.cols; a.n = d.n; a.npad = d.npad;
     a.Adense = reinterpret_cast<const double*>(m->d_plan + oA);
     a.entries = reinterpret_cast<const int2*>(m->d_plan + oE);
     a.items = reinterpret_cast<const int2*>(m->d_plan + oI);
@@ -1056,7 +1063,7 @@ amp_status norm_via_matrix(amp_model* m, const HerkPlan& hp, double* d_out, cuda
     if (!hit) {
         HerkArgs h{};
         const Dataset& d = m->norm;
-        h.b.cache = d.cache; h.b.weight = d.weight; h.b.cols = d.cols; h.b.n = d.n; h.b.npad = d.npad;
+        h.b.cache = d.cache; h.b.ncolw = d.ncache + 1; h.b.cols = d.cols; h.b.n = d.n; h.b.npad = d.npad;
         h.b.entries = reinterpret_cast<const int2*>(m->d_hk + oE);
         h.b.nent = hp.nent;
         h.b.ncolu = (int)hp.colu.size();
@@ -1097,7 +1104,7 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         int ent_of_res[AMP_MAX_RESONANCES], grp_of_res[AMP_MAX_RESONANCES];
         DeltaArgs d{};
         fill_stream_args(m, m->data, 0, MODE_FUSED, &d.a, ent_of_res, grp_of_res);
-        d.a.cache2 = m->norm.cache; d.a.weight2 = m->norm.weight; d.a.n2 = m->norm.n; d.a.npad2 = m->norm.npad;
+        d.a.cache2 = m->norm.cache; d.a.n2 = m->norm.n; d.a.npad2 = m->norm.npad;
         d.a.ticket = m->d_ticket;
         d.a.sum_log_eff = m->data.loaded ? m->data.wsum : 0.0;
         d.a.wsum = m->norm.wsum;
@@ -1170,7 +1177,7 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         fill_stream_args(m, m->data, 0, MODE_FUSED, &a);
         a.partial = m->d_partial;
         a.partial2 = m->d_partial + PARTIAL_STRIDE;
-        a.cache2 = m->norm.cache; a.weight2 = m->norm.weight; a.n2 = m->norm.n; a.npad2 = m->norm.npad;
+        a.cache2 = m->norm.cache; a.n2 = m->norm.n; a.npad2 = m->norm.npad;
         a.ticket = m->d_ticket;
         a.result = m->d_result;
         a.sum_log_eff = m->data.wsum;
@@ -1371,7 +1378,8 @@ amp_status amp_dump_cache(amp_model* m, int which, double* d_out, int* ncols, vo
     if (ncols) *ncols = d.ncache;
     if (!d_out || d.n == 0) return AMP_OK;
     cudaStream_t s = (cudaStream_t)stream;
-    CK(cudaMemcpy2DAsync(d_out, sizeof(double) * d.n, d.cache, sizeof(double) * d.npad, sizeof(double) * d.n, d.ncache, cudaMemcpyDeviceToDevice, s));
+    k_dump_cache<<<148 * 4, 256, 0, s>>>(d.cache, d.ncache + 1, d.ncache, d.n, d_out);
+    CK(cudaGetLastError());
     CK(cudaStreamSynchronize(s));
     return AMP_OK;
 }

@@ -349,9 +349,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_delta(const __grid_constant__ De
     auto issue = [&](long long tile, int region) {
         const bool nrm = tile >= ntd;
         const double* cache = nrm ? a.cache2 : a.cache;
-        const long long npad = nrm ? a.npad2 : a.npad, lt = nrm ? tile - ntd : tile;
-        if (region == 0) issue_cols(cache, a.weight2, npad, lt, stage, &full[0], 0, NCOL_K, nrm, ncache);
-        else issue_cols(cache, nullptr, npad, lt, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
+        const long long lt = nrm ? tile - ntd : tile;
+        if (region == 0) issue_cols(cache, a.ncolw, lt, stage, &full[0], 0, NCOL_K, nrm);
+        else issue_cols(cache, a.ncolw, lt, stage, &full[1], NCOL_K, NCOL_ALL, false);
     };
     if (tid == 0 && (long long)blockIdx.x < ntiles) {
         issue(blockIdx.x, 0);

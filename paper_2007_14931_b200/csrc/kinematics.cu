@@ -10,7 +10,8 @@
 // direction, K on the +x side), so only z components change under the boost along z and the two
 // dihedral angles reduce to ratios of components of the mu+ direction.
 //
-// HBM-bound: reads 32-40 B, writes 88-184 B per event; one thread per event, fully coalesced.
+// HBM-bound: reads 32-40 B, writes 88-184 B per event; one thread per event, fully coalesced.  The cache is written in
+// the tiled layout of amp_internal.cuh (blocks of 512 events, one 4 KB column per quantity, the weight last).
 #include "amp_internal.cuh"
 
 namespace amp {
@@ -25,10 +26,10 @@ __global__ void __launch_bounds__(256) k_kinematics(const KinArgs a) {
     double acc = 0.0;
     bool bad = false;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < a.npad; i += (long long)gridDim.x * blockDim.x) {
-        double* col = a.cache + i;
+        double* col = a.cache + cache_idx(a.ncolw, 0, i);   // this event's element of column 0; column c is CACHE_TILE * c further
         if (i >= a.n) {   // padding: benign values, weight 0
-            for (int c = 0; c < (a.with_z ? NCOL_ALL : NCOL_K); ++c) col[c * a.npad] = 1.0;
-            a.weight[i] = 0.0;
+            for (int c = 0; c < a.ncolw - 1; ++c) col[c * CACHE_TILE] = 1.0;
+            col[(a.ncolw - 1) * CACHE_TILE] = 0.0;
             continue;
         }
         const double m = a.x[i], cK = a.x[a.n + i], cpsi = a.x[2 * a.n + i], phi = a.x[3 * a.n + i];
@@ -37,7 +38,7 @@ __global__ void __launch_bounds__(256) k_kinematics(const KinArgs a) {
         const bool ok = (m > mK + mpi) && (m < MB - mpsi) && (fabs(cK) <= 1.0) && (fabs(cpsi) <= 1.0) && isfinite(phi) &&
                         isfinite(w) && (a.weight_positive ? (w > 0.0) : (w >= 0.0));
         if (!ok) { bad = true; continue; }
-        a.weight[i] = w;
+        col[(a.ncolw - 1) * CACHE_TILE] = w;
         acc += a.weight_positive ? log(w) : w;
 
         const double m2 = m * m, invm = 1.0 / m;
@@ -46,16 +47,16 @@ __global__ void __launch_bounds__(256) k_kinematics(const KinArgs a) {
         const double sK = sqrt((1.0 - cK) * (1.0 + cK)), spsi = sqrt((1.0 - cpsi) * (1.0 + cpsi));
         double sphi, cphi;
         sincos(phi, &sphi, &cphi);
-        col[C_M2 * a.npad] = m2;
-        col[C_INVM * a.npad] = invm;
-        col[C_Q * a.npad] = q;
-        col[C_PB * a.npad] = pB;
-        col[C_CK * a.npad] = cK;
-        col[C_SK * a.npad] = sK;
-        col[C_CPSI * a.npad] = cpsi;
-        col[C_SPSI * a.npad] = spsi;
-        col[C_CPHI * a.npad] = cphi;
-        col[C_SPHI * a.npad] = sphi;
+        col[C_M2 * CACHE_TILE] = m2;
+        col[C_INVM * CACHE_TILE] = invm;
+        col[C_Q * CACHE_TILE] = q;
+        col[C_PB * CACHE_TILE] = pB;
+        col[C_CK * CACHE_TILE] = cK;
+        col[C_SK * CACHE_TILE] = sK;
+        col[C_CPSI * CACHE_TILE] = cpsi;
+        col[C_SPSI * CACHE_TILE] = spsi;
+        col[C_CPHI * CACHE_TILE] = cphi;
+        col[C_SPHI * CACHE_TILE] = sphi;
         if (!a.with_z) continue;
 
         // B frame, z along the K pi system.  Energies in the K pi frame, then boosted with gamma = E_Kpi/m.
@@ -88,18 +89,18 @@ __global__ void __launch_bounds__(256) k_kinematics(const KinArgs a) {
         const double iden = 1.0 / (pKZ * qZ);
         const double cZ = (EKZ * EpiZ - 0.5 * (m2 - mK * mK - mpi * mpi)) * iden;
         const double sZ = MB * q * pB * sK * invmZ * iden;
-        col[C_MZ2 * a.npad] = mZ2;
-        col[C_INVMZ * a.npad] = invmZ;
-        col[C_QZ * a.npad] = qZ;
-        col[C_PBZ * a.npad] = pBZ;
-        col[C_CZ * a.npad] = cZ;
-        col[C_SZ * a.npad] = sZ;
-        col[C_CT * a.npad] = ct;
-        col[C_ST * a.npad] = st;
-        col[C_CPT * a.npad] = cpt;
-        col[C_SPT * a.npad] = spt;
-        col[C_CA * a.npad] = ca;
-        col[C_SA * a.npad] = sa;
+        col[C_MZ2 * CACHE_TILE] = mZ2;
+        col[C_INVMZ * CACHE_TILE] = invmZ;
+        col[C_QZ * CACHE_TILE] = qZ;
+        col[C_PBZ * CACHE_TILE] = pBZ;
+        col[C_CZ * CACHE_TILE] = cZ;
+        col[C_SZ * CACHE_TILE] = sZ;
+        col[C_CT * CACHE_TILE] = ct;
+        col[C_ST * CACHE_TILE] = st;
+        col[C_CPT * CACHE_TILE] = cpt;
+        col[C_SPT * CACHE_TILE] = spt;
+        col[C_CA * CACHE_TILE] = ca;
+        col[C_SA * CACHE_TILE] = sa;
     }
     if (bad) atomicOr(a.flag, 1);
     // deterministic block reduction of acc (fixed shuffle tree, fixed warp order)

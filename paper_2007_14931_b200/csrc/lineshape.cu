@@ -13,16 +13,17 @@ struct LineshapeArgs {
     int njobs;
     int any_k, any_z;
     const double* cache;
+    int ncolw;
     double2* cols;
     long long n, npad;
 };
 
 __global__ void __launch_bounds__(256) k_lineshape(const __grid_constant__ LineshapeArgs a) {
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < a.n; i += (long long)gridDim.x * blockDim.x) {
-        const double* col = a.cache + i;
+        const double* col = a.cache + cache_idx(a.ncolw, 0, i);
         double m2 = 0, invm = 0, q = 0, pB = 0, mZ2 = 0, invmZ = 0, qZ = 0, pBZ = 0;
-        if (a.any_k) { m2 = col[C_M2 * a.npad]; invm = col[C_INVM * a.npad]; q = col[C_Q * a.npad]; pB = col[C_PB * a.npad]; }
-        if (a.any_z) { mZ2 = col[C_MZ2 * a.npad]; invmZ = col[C_INVMZ * a.npad]; qZ = col[C_QZ * a.npad]; pBZ = col[C_PBZ * a.npad]; }
+        if (a.any_k) { m2 = col[C_M2 * CACHE_TILE]; invm = col[C_INVM * CACHE_TILE]; q = col[C_Q * CACHE_TILE]; pB = col[C_PB * CACHE_TILE]; }
+        if (a.any_z) { mZ2 = col[C_MZ2 * CACHE_TILE]; invmZ = col[C_INVMZ * CACHE_TILE]; qZ = col[C_QZ * CACHE_TILE]; pBZ = col[C_PBZ * CACHE_TILE]; }
         for (int j = 0; j < a.njobs; ++j) {
             const LineConst& lc = a.job[j].lc;
             const double2 A = (lc.chain == 1) ? lineshape_eval(lc, mZ2, invmZ, qZ, pBZ) : lineshape_eval(lc, m2, invm, q, pB);
@@ -42,6 +43,7 @@ cudaError_t launch_lineshape(const Dataset& d, const LineshapeJob* jobs, int njo
             if (a.job[j].lc.chain == 1) a.any_z = 1;
         }
         a.cache = d.cache;
+        a.ncolw = d.ncache + 1;
         a.cols = d.cols;
         a.n = d.n;
         a.npad = d.npad;

@@ -52,8 +52,8 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     const long long ntd = (a.n + TILE - 1) / TILE;                                              // tiles of the first dataset
     const long long ntiles = MODE == MODE_FUSED ? ntd + (a.n2 + TILE - 1) / TILE : ntd;
     if (threadIdx.x == 0 && (long long)blockIdx.x < ntiles) {
-        issue_tile<MODE>(a, ntd, blockIdx.x, stage, &full[0], 0, NCOL_K, true, ncache);
-        if (have_z) issue_tile<MODE>(a, ntd, blockIdx.x, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
+        issue_tile<MODE>(a, ntd, blockIdx.x, stage, &full[0], 0, NCOL_K, true);
+        if (have_z) issue_tile<MODE>(a, ntd, blockIdx.x, stage, &full[1], NCOL_K, NCOL_ALL, false);
     }
     __shared__ double sm[NWARPS];
     uint32_t parity = 0;
@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         Ev w;
         if (MODE == MODE_FUSED ? is_norm : with_w) w = load_col(stage, ncache);
         __syncthreads();   // K* region consumed by every thread: stream the next tile into it
-        if (threadIdx.x == 0 && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[0], 0, NCOL_K, true, ncache);
+        if (threadIdx.x == 0 && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[0], 0, NCOL_K, true);
 
         double2 V0[E], Vp[E], Vm[E];
 #pragma unroll
@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
             const Ev cpt = load_col(stage, C_CPT), spt = load_col(stage, C_SPT);
             const Ev ca = load_col(stage, C_CA), sa = load_col(stage, C_SA);
             __syncthreads();   // Z region consumed: refill it with the next tile
-            if (threadIdx.x == 0 && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[1], NCOL_K, NCOL_ALL, false, 0);
+            if (threadIdx.x == 0 && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[1], NCOL_K, NCOL_ALL, false);
             double2 Um[E], U0[E], Up[E];
 #pragma unroll
             for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0);
@@ -210,7 +210,7 @@ int stream_grid_fused(long long n1, long long n2, bool have_z) {
     return stream_grid((t1 + t2) * TILE, have_z, MODE_FUSED);
 }
 
-long long stream_pad(long long n) { return (n + TILE - 1) / TILE * TILE; }
+long long stream_pad(long long n) { return (n + 511) / 512 * 512; }   // whole tiles of every streaming kernel (k_stream, k_delta: 512 events)
 
 template <class SH>
 static cudaError_t launch_shape(const StreamArgs& a, int grid, cudaStream_t s) {

@@ -67,23 +67,24 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
-// Columns [c0, c1) of the cache (and, if with_w, the weight column into slot wslot) of tile `tile` -> stage.
-__device__ __forceinline__ void issue_cols(const double* cache, const double* weight, long long npad, long long tile, double* stage,
-                                           uint64_t* bar, int c0, int c1, bool with_w, int wslot) {
-    const uint32_t col_bytes = TILE * sizeof(double);
-    mbar_expect_tx(bar, col_bytes * (c1 - c0 + (with_w ? 1 : 0)));
-#pragma unroll 1
-    for (int c = c0; c < c1; ++c) bulk_g2s(stage + c * TILE, cache + (size_t)c * npad + tile * TILE, col_bytes, bar);
-    if (with_w) bulk_g2s(stage + wslot * TILE, weight + tile * TILE, col_bytes, bar);
+// Columns [c0, c1) of block `tile` of a tiled cache (and, if with_w, its weight column) -> the same places of the stage.
+// The columns of a block are contiguous, so a region is ONE bulk copy (40 KB for the K* chain, 48 KB for the Z chain).
+static_assert(TILE == CACHE_TILE, "a streaming tile is one cache block");
+__device__ __forceinline__ void issue_cols(const double* cache, int ncolw, long long tile, double* stage, uint64_t* bar, int c0, int c1, bool with_w) {
+    const double* blk = cache + (size_t)tile * ncolw * TILE;
+    const uint32_t bytes = (uint32_t)(c1 - c0) * TILE * sizeof(double), wbytes = TILE * sizeof(double);
+    mbar_expect_tx(bar, bytes + (with_w ? wbytes : 0));
+    bulk_g2s(stage + c0 * TILE, blk + c0 * TILE, bytes, bar);
+    if (with_w) bulk_g2s(stage + (ncolw - 1) * TILE, blk + (ncolw - 1) * TILE, wbytes, bar);
 }
 // MODE_FUSED walks one tile space: the data tiles first, then the normalisation tiles (second dataset of StreamArgs).
 template <int MODE>
 __device__ __forceinline__ void issue_tile(const StreamArgs& a, long long ntd, long long tile, double* stage, uint64_t* bar, int c0, int c1,
-                                           bool region_has_w, int wslot) {
+                                           bool region_has_w) {
     if (MODE == MODE_FUSED && tile >= ntd)
-        issue_cols(a.cache2, a.weight2, a.npad2, tile - ntd, stage, bar, c0, c1, region_has_w, wslot);
+        issue_cols(a.cache2, a.ncolw, tile - ntd, stage, bar, c0, c1, region_has_w);
     else
-        issue_cols(a.cache, a.weight, a.npad, tile, stage, bar, c0, c1, region_has_w && MODE != MODE_DATA && MODE != MODE_FUSED, wslot);
+        issue_cols(a.cache, a.ncolw, tile, stage, bar, c0, c1, region_has_w && MODE != MODE_DATA && MODE != MODE_FUSED);
 }
 
 // fixed-order block sum: xor-shuffle tree, then the 8 warp values in warp order; result valid in thread 0

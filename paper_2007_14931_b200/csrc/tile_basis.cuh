@@ -51,8 +51,8 @@ __device__ __forceinline__ void issue_stage(const BatchArgs& a, long long tile, 
 #pragma unroll 1
     for (int c = 0; c < a.ncolu; ++c) bbulk_g2s(scol + (size_t)c * BT_EVENTS, a.cols + (size_t)a.colu[c] * a.npad + i0, BT_EVENTS * 16, bar);
 #pragma unroll 1
-    for (int j = 0; j < nang; ++j) bbulk_g2s(sang + (size_t)j * BT_EVENTS, a.cache + (size_t)ang_col(j) * a.npad + i0, BT_EVENTS * 8, bar);
-    if (with_w) bbulk_g2s(sw, a.weight + i0, BT_EVENTS * 8, bar);
+    for (int j = 0; j < nang; ++j) bbulk_g2s(sang + (size_t)j * BT_EVENTS, a.cache + cache_idx(a.ncolw, ang_col(j), i0), BT_EVENTS * 8, bar);
+    if (with_w) bbulk_g2s(sw, a.cache + cache_idx(a.ncolw, a.ncolw - 1, i0), BT_EVENTS * 8, bar);   // (64 divides the 512-event cache block)
 }
 
 // angular factor g_xi (xi = +1, -1) of one basis entry at one event; `code` is warp-uniform
