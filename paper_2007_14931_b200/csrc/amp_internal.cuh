@@ -97,6 +97,15 @@ __device__ __forceinline__ double fast_rsqrt(double d) {
     const double e = fma(-d * y, y, 1.0);           // 1 - d y^2 ~ 1e-6
     return fma(y * fma(0.375, e, 0.5), e, y);       // y (1 + e/2 + 3 e^2 / 8)
 }
+// Sums of logs without a log per event: S = f 2^e with f in [0.5, 1) for positive finite S (integer ops on the exponent field)
+__device__ __forceinline__ void split_exp(double S, double* f, int* e) {
+    int e0 = 0;
+    if (S < 1e-290) { S *= 1.3407807929942597e154; e0 = -512; }   // 2^512: keeps subnormals out of the bit trick
+    const int hi = __double2hiint(S), lo = __double2loint(S);
+    *e = e0 + ((hi >> 20) & 0x7ff) - 1022;
+    *f = __hiloint2double((hi & 0x800fffff) | 0x3fe00000, lo);
+}
+
 template <int L>
 __device__ __forceinline__ double bw_poly_c(double z) {
     if (L == 0) return 1.0;
@@ -115,8 +124,8 @@ __device__ __forceinline__ double powc(double x) {
 // Per-event factors of a barrier group with compile-time orbital momenta (see BarrierGroup).
 template <int LR, int LB>
 __device__ __forceinline__ void group_factors(double r2, double invm, double pR, double pB, double* F, double* G) {
-    const double DB = bw_poly_c<LB>(r2 * pB * pB);
-    const double DR = bw_poly_c<LR>(r2 * pR * pR);
+    const double DB = bw_poly_c<LB>(r2 * (pB * pB));   // (pB pB), (pR pR): shared by every spin group of the event
+    const double DR = bw_poly_c<LR>(r2 * (pR * pR));
     const double rs = (LR == 0 && LB == 0) ? 1.0 : fast_rsqrt(DR * DB);
     *F = rs * powc<LB>(pB) * powc<LR>(pR * invm);
     *G = powc<2 * LR + 1>(pR) * invm * (rs * rs) * DB;
@@ -181,7 +190,8 @@ enum StreamMode { MODE_DATA = 0, MODE_NORM = 1, MODE_EVAL = 2, MODE_FUSED = 3 };
 // its first coupling slot, and either a pool column to read or -1 = evaluate in registers.
 struct ResEntry {
     double kN, kG, M2;
-    double2 cm, c0, cp;   // couplings of lambda = -1, 0, +1 (J = 0: only c0)
+    double2 cm, c0, cp;   // couplings of lambda = -1, 0, +1 (J = 0: only c0); times kN when the lineshape is evaluated in
+                          // registers (column < 0): the kernels then form A^R / kN (bw_unscaled)
     int column;
 };
 // Resonances that share (chain, L_R, L_B, radius) share the barrier factors and momentum powers:
@@ -199,6 +209,12 @@ __device__ __forceinline__ double2 bw_from_consts(double kN, double kG, double M
 }
 __device__ __forceinline__ double2 bw_from_factors(const ResEntry& e, double m2, double F, double G) {
     return bw_from_consts(e.kN, e.kG, e.M2, m2, F, G);
+}
+// A^R / kN: the streaming kernels multiply it with couplings that the host has scaled by kN (one multiply less per resonance)
+__device__ __forceinline__ double2 bw_unscaled(const ResEntry& e, double m2, double F, double G) {
+    const double MG = e.kG * G, dre = e.M2 - m2;
+    const double s = F * fast_rcp(fma(dre, dre, MG * MG));
+    return make_double2(s * dre, s * MG);
 }
 struct StreamArgs {
     ResEntry ent[AMP_MAX_RESONANCES];

@@ -692,6 +692,9 @@ void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, Str
                 const size_t ci = (size_t)p * m->R + r2;
                 const int sidx = ci < m->colidx.size() ? m->colidx[ci] : -1;
                 e.column = (sidx >= 0 && !m->stream_inline) ? sidx : -1;
+                if (e.column < 0) {   // lineshape in registers: fold its constant kN into the couplings
+                    e.cm.x *= lc.kN; e.cm.y *= lc.kN; e.c0.x *= lc.kN; e.c0.y *= lc.kN; e.cp.x *= lc.kN; e.cp.y *= lc.kN;
+                }
             }
             grp.count = t - grp.first;
         }

@@ -36,15 +36,6 @@ namespace {
 
 constexpr int DBLK = DELTA_MAX_SORTED / 32;
 
-// S = f 2^e with f in [0.5, 1) for positive finite S (integer ops on the exponent field)
-__device__ __forceinline__ void split_exp(double S, double* f, int* e) {
-    int e0 = 0;
-    if (S < 1e-290) { S *= 1.3407807929942597e154; e0 = -512; }   // 2^512: keeps subnormals out of the bit trick
-    const int hi = __double2hiint(S), lo = __double2loint(S);
-    *e = e0 + ((hi >> 20) & 0x7ff) - 1022;
-    *f = __hiloint2double((hi & 0x800fffff) | 0x3fe00000, lo);
-}
-
 // d^J_{00}, d^J_{+1,0} (Eq. 4), J warp-uniform
 __device__ __forceinline__ void dJ(int J, double c, double s, double* d0, double* d1) {
     const double c2 = c * c;

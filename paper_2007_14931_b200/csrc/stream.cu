@@ -31,7 +31,11 @@ template <int MODE, class SH>
 __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __grid_constant__ StreamArgs a) {
     const double RSQRT2 = 0.70710678118654752440;
     const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[6] > a.gstart[5]);
-    double acc = 0.0;
+    // sum w S (normalisation tiles) lives in `acc`; sum log S (data tiles) as a running product of mantissas in `acc` and a
+    // sum of exponents in `accE` (split_exp: integer ops + one multiply per event instead of a ~35-instruction FP64 log)
+    const double LN2 = 0.69314718055994530942;
+    double acc = (MODE == MODE_DATA || MODE == MODE_FUSED) ? 1.0 : 0.0;
+    int accE = 0;
     bool bad = false;
     // One staged tile per CTA, split in two regions with their own mbarrier: the K*-chain columns (+ weight) are
     // copied to registers at the top of an iteration and their region is refilled at once with the next tile;
@@ -62,7 +66,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         const bool has_next = tile + gridDim.x < ntiles;
         const bool is_norm = MODE == MODE_FUSED ? tile >= ntd : MODE == MODE_NORM;
         if (MODE == MODE_FUSED && is_norm && !in_norm) {   // sum log S of this CTA's data tiles is complete
-            const double t = block_sum(acc, sm);
+            const double t = block_sum(log(acc) + (double)accE * LN2, sm);
             if (threadIdx.x == 0) a.partial[blockIdx.x] = t;
             acc = 0.0;
             in_norm = true;
@@ -146,18 +150,29 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
             const double S = fma(Ap[e].x, Ap[e].x, fma(Ap[e].y, Ap[e].y, fma(Am[e].x, Am[e].x, Am[e].y * Am[e].y)));
             const bool live = i0 + e < nlive;   // the last thread may hold padding events (weight 0)
             if (MODE == MODE_DATA || (MODE == MODE_FUSED && !is_norm)) {
-                if (live) { bad |= !(S > 0.0) || !isfinite(S); acc += log(S); }
+                const bool ok = S > 0.0 && isfinite(S);
+                bad |= live && !ok;
+                double f; int x;
+                split_exp((live && ok) ? S : 1.0, &f, &x);
+                acc *= f;
+                accE += x;
             } else if (MODE == MODE_NORM || MODE == MODE_FUSED) {
                 if (live) { bad |= !isfinite(S); acc = fma(w.v[e], S, acc); }
             } else {
                 if (live) a.out[i0 + e] = w.v[e] * S;
             }
         }
+        if (MODE == MODE_DATA || (MODE == MODE_FUSED && !is_norm)) {   // running product back to [0.5, 1) once per tile
+            int x;
+            split_exp(acc, &acc, &x);
+            accE += x;
+        }
     }
     if (MODE == MODE_EVAL) return;
     if (bad) atomicOr(a.flag, 2);
     {
-        const double t = block_sum(acc, sm);
+        const bool logs = MODE == MODE_DATA || (MODE == MODE_FUSED && !in_norm);
+        const double t = block_sum(logs ? log(acc) + (double)accE * LN2 : acc, sm);
         if (threadIdx.x == 0) {
             if (MODE == MODE_FUSED && !in_norm) { a.partial[blockIdx.x] = t; a.partial2[blockIdx.x] = 0.0; }   // this CTA saw data tiles only
             else (MODE == MODE_FUSED ? a.partial2 : a.partial)[blockIdx.x] = t;

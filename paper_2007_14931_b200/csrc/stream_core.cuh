@@ -116,7 +116,7 @@ __device__ __forceinline__ void add_resonance(const StreamArgs& a, const ResEntr
         for (int e = 0; e < E; ++e) bw[e] = a.cols[(size_t)en.column * a.npad + i0 + e];
     } else {
 #pragma unroll
-        for (int e = 0; e < E; ++e) bw[e] = bw_from_factors(en, m2.v[e], F[e], G[e]);
+        for (int e = 0; e < E; ++e) bw[e] = bw_unscaled(en, m2.v[e], F[e], G[e]);   // couplings carry kN
     }
 #pragma unroll
     for (int e = 0; e < E; ++e) {
