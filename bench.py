@@ -38,8 +38,8 @@ FLOP_PER_EVENT = 730.0
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # 148 SMs x 64 DFMA/clk x 2 flop x 1965 MHz
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed `ncu --set full` capture
 # (profiles/): per launch, at the default sizes; None until a capture of the current kernel exists
-TRAFFIC_NCU_BYTES = None
-TRAFFIC_NCU_BYTES_CFG4 = None
+TRAFFIC_NCU_BYTES = 2.192192e9 + 3.88e6       # profiles/r01c_ncu_full_stream_fused_cfg3.csv (2M + 10M events)
+TRAFFIC_NCU_BYTES_CFG4 = 2.192431e9 + 4.04e6  # profiles/r01c_ncu_full_delta_cfg4.csv
 # Algorithmic flop per event of the gradient batch of configs[4] in its sparse form: point 0 (730) + 31 slots
 # (Breit-Wigner of point 0 from the saved barrier factors ~20, angular factor ~8, two complex products 12) + 100 coupling
 # points (two complex multiply-adds 16, |A|^2 7, accumulate 2) + 20 mass/width points (perturbed Breit-Wigner ~22, the same 25)
@@ -224,7 +224,7 @@ def run_own(args):
         roof = {"bound": "alu", "kernel": "k_delta (gradient batch: point 0 + 120 sparse points, data then norm tiles, one launch)",
                 "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12,
                 "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md 6; the DFMA probe below measures it)", "unit": "TFLOP/s",
-                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": TRAFFIC_NCU_BYTES_CFG4, "kernel_ms": k_ms,
+                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": TRAFFIC_NCU_BYTES_CFG4 if (args.n_data, args.n_norm) == (2_000_000, 10_000_000) else None, "kernel_ms": k_ms,
                 "flop_per_event": DELTA_FLOP_PER_EVENT, "flop_per_launch": flop,
                 "hbm_frac": (BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}
     elif args.cfg == 4:
@@ -236,7 +236,7 @@ def run_own(args):
         ach = nbytes / (k_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": "k_stream<MODE_FUSED> (the whole step: lineshapes + combine + -log L / normalisation reductions, data then norm tiles)",
                 "achieved": ach, "peak": hbm_peak, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})", "unit": "GB/s",
-                "frac": ach / hbm_peak, "traffic": TRAFFIC_NCU_BYTES,
+                "frac": ach / hbm_peak, "traffic": TRAFFIC_NCU_BYTES if (args.n_data, args.n_norm) == (2_000_000, 10_000_000) else None,
                 "alu_frac_nominal": FLOP_PER_EVENT * (args.n_data + args.n_norm) / (k_ms * 1e-3) / FP64_PEAK_NOMINAL,
                 "kernel_ms": k_ms, "bytes_per_launch": nbytes, "bytes_per_event": [BYTES_PER_EVENT_DATA, BYTES_PER_EVENT_NORM],
                 "flop_per_event": FLOP_PER_EVENT}

@@ -128,7 +128,8 @@ __device__ __forceinline__ void group_factors(double r2, double invm, double pR,
     const double DR = bw_poly_c<LR>(r2 * (pR * pR));
     const double rs = (LR == 0 && LB == 0) ? 1.0 : fast_rsqrt(DR * DB);
     *F = rs * powc<LB>(pB) * powc<LR>(pR * invm);
-    *G = powc<2 * LR + 1>(pR) * invm * (rs * rs) * DB;
+    // G = pR^(2LR+1) (1/m) / B_LR(zR); rs^2 B_LB(zB) = 1 / B_LR(zR), which is 1 for L_R = 0
+    *G = (LR == 0) ? pR * invm : powc<2 * LR + 1>(pR) * invm * (rs * rs) * DB;
 }
 // Blatt-Weisskopf polynomial B_L(z), z = (r p)^2 (ref. [35]); L is warp-uniform.
 __device__ __forceinline__ double bw_poly(int L, double z) {
