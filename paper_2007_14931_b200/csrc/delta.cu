@@ -214,15 +214,16 @@ __device__ __forceinline__ void leaf(const StreamArgs& a, const DeltaContrib* pr
     leaf_value<NORM>(S, w, live, bad, v, ex);   // (NORM: a non-finite S makes the point's total non-finite: flagged at the end)
 }
 
-// Two consecutive single-contribution points of the same kind on the same slot (theta_k + h and theta_k - h of a
-// gradient step) as ONE straight-line block: 2 points x E events = four independent dependency chains, which is what
-// keeps the FP64 pipe busy with two warps per scheduler.
-template <bool NORM, int KIND>
-__device__ __forceinline__ void leaf_pair(const int4 (&h4)[2], const double2 (&bc)[2], const EvK (&k)[E], const double2* fg, const SlotVal (&sv)[E],
-                                          const double (&w)[E], const bool (&live)[E], bool& bad, double (&v)[2], int (&ex)[2]) {
-    double S[2][E];
+// NP = 2 or 4 consecutive single-contribution points of the same kind on the same slot (theta_k +- h; modulus and phase of
+// one coupling; mass and width of one resonance) as ONE straight-line block: NP points x E events independent dependency
+// chains, which is what keeps the FP64 pipe busy with two warps per scheduler.
+template <bool NORM, int KIND, int NP>
+__device__ __forceinline__ void leaf_multi(const int4 (&h4)[NP], const double2 (&bc)[NP], const EvK (&k)[E], const double2* fg,
+                                           const SlotVal (&sv)[E], const double (&w)[E], const bool (&live)[E], bool& bad, double (&v)[NP],
+                                           int (&ex)[NP]) {
+    double S[NP][E];
 #pragma unroll
-    for (int j = 0; j < 2; ++j) {
+    for (int j = 0; j < NP; ++j) {
         const double ca = __hiloint2double(h4[j].w, h4[j].z);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
@@ -236,8 +237,8 @@ __device__ __forceinline__ void leaf_pair(const int4 (&h4)[2], const double2 (&b
             S[j][e] = fma(Ap.x, Ap.x, Ap.y * Ap.y) + fma(Am.x, Am.x, Am.y * Am.y);
         }
     }
-    leaf_value<NORM>(S[0], w, live, bad, &v[0], &ex[0]);
-    leaf_value<NORM>(S[1], w, live, bad, &v[1], &ex[1]);
+#pragma unroll
+    for (int j = 0; j < NP; ++j) leaf_value<NORM>(S[j], w, live, bad, &v[j], &ex[j]);
 }
 
 // Recursive halving over the 32 lanes: `a` belongs to the earlier half of the points, `b` to the later half; lanes with
@@ -262,37 +263,61 @@ template <bool NORM>
 __device__ __forceinline__ void eval_block(const StreamArgs& a, const DeltaContrib* prog, const double* slots, int& it, const EvK (&k)[E],
                                            const double2* fg, const double* zst, SlotVal (&sv)[E], const double (&w)[E],
                                            const bool (&live)[E], bool& bad, int lane, double* v, int* ex) {
-    double s1 = 0, s2 = 0, s3 = 0, s4 = 0;
-    int e1 = 0, e2 = 0, e3 = 0, e4 = 0;
-#pragma unroll 1
-    for (int q = 0; q < 32; q += 2) {
-        double x0, x; int xe0, xe;
-        {
-            int4 h4[2];
-            double2 bc[2];
+    double s2 = 0, s3 = 0, s4 = 0;
+    int e2 = 0, e3 = 0, e4 = 0;
+    // two points: as one block if both are single-contribution, non-empty, of one kind and on one slot, else one by one
+    auto two_points = [&](double* y, int* ye) {
+        int4 h4[2];
+        double2 bc[2];
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
+        for (int j = 0; j < 2; ++j) {
+            h4[j] = *reinterpret_cast<const int4*>(prog + it + j);
+            bc[j] = *reinterpret_cast<const double2*>(&prog[it + j].b);
+        }
+        if ((h4[0].x & 20) == 4 && (h4[1].x & 28) == 4 && ((h4[0].x ^ h4[1].x) & 3) == 0) {
+            it += 2;
+            if (h4[0].x & 8) eval_slot(a, slots + h4[0].y, k, fg, zst, sv);
+            double v2[2]; int x2[2];
+            const int kind = h4[0].x & 3;
+            if (kind == 0) leaf_multi<NORM, 0, 2>(h4, bc, k, fg, sv, w, live, bad, v2, x2);
+            else if (kind == 1) leaf_multi<NORM, 1, 2>(h4, bc, k, fg, sv, w, live, bad, v2, x2);
+            else leaf_multi<NORM, 2, 2>(h4, bc, k, fg, sv, w, live, bad, v2, x2);
+            y[0] = v2[0]; ye[0] = x2[0]; y[1] = v2[1]; ye[1] = x2[1];
+        } else {
+            leaf<NORM>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, &y[0], &ye[0]);
+            leaf<NORM>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, &y[1], &ye[1]);
+        }
+    };
+#pragma unroll 1
+    for (int q = 0; q < 32; q += 4) {
+        double y[4]; int ye[4];
+        {
+            int4 h4[4];
+            double2 bc[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
                 h4[j] = *reinterpret_cast<const int4*>(prog + it + j);
                 bc[j] = *reinterpret_cast<const double2*>(&prog[it + j].b);
             }
-            // both single-contribution and non-empty, same coefficient kind, the second on the first one's slot
-            if ((h4[0].x & 20) == 4 && (h4[1].x & 28) == 4 && ((h4[0].x ^ h4[1].x) & 3) == 0) {
-                it += 2;
+            // four single-contribution points of kind 0 or 1 on one slot (the gradient pattern): one straight-line block
+            const int kind = h4[0].x & 3;
+            bool quad = (h4[0].x & 20) == 4 && kind < 2;
+#pragma unroll
+            for (int j = 1; j < 4; ++j) quad = quad && (h4[j].x & 28) == 4 && ((h4[0].x ^ h4[j].x) & 3) == 0;
+            if (quad) {
+                it += 4;
                 if (h4[0].x & 8) eval_slot(a, slots + h4[0].y, k, fg, zst, sv);
-                double v2[2]; int e2[2];
-                const int kind = h4[0].x & 3;
-                if (kind == 0) leaf_pair<NORM, 0>(h4, bc, k, fg, sv, w, live, bad, v2, e2);
-                else if (kind == 1) leaf_pair<NORM, 1>(h4, bc, k, fg, sv, w, live, bad, v2, e2);
-                else leaf_pair<NORM, 2>(h4, bc, k, fg, sv, w, live, bad, v2, e2);
-                x0 = v2[0]; xe0 = e2[0]; x = v2[1]; xe = e2[1];
+                if (kind == 0) leaf_multi<NORM, 0, 4>(h4, bc, k, fg, sv, w, live, bad, y, ye);
+                else leaf_multi<NORM, 1, 4>(h4, bc, k, fg, sv, w, live, bad, y, ye);
             } else {
-                leaf<NORM>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, &x0, &xe0);
-                leaf<NORM>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, &x, &xe);
+                two_points(&y[0], &ye[0]);
+                two_points(&y[2], &ye[2]);
             }
         }
-        halve<NORM>(0, lane, x0, xe0, x, xe, &x, &xe);
-        if (!(q & 2)) { s1 = x; e1 = xe; continue; }
-        halve<NORM>(1, lane, s1, e1, x, xe, &x, &xe);
+        double x, u; int xe, ue;
+        halve<NORM>(0, lane, y[0], ye[0], y[1], ye[1], &u, &ue);
+        halve<NORM>(0, lane, y[2], ye[2], y[3], ye[3], &x, &xe);
+        halve<NORM>(1, lane, u, ue, x, xe, &x, &xe);
         if (!(q & 4)) { s2 = x; e2 = xe; continue; }
         halve<NORM>(2, lane, s2, e2, x, xe, &x, &xe);
         if (!(q & 8)) { s3 = x; e3 = xe; continue; }
