@@ -123,17 +123,28 @@ def build_workload(args, device):
     xn, wn = W.norm_events(cfg, args.n_norm)
     t_gen = time.time() - t0
     model = B.Model(W.DECAY, res)
-    d_x, d_e, d_xn, d_wn = dev(x), dev(eff), dev(xn), dev(wn)
+    # cold start, once: the events as HOST buffers (pinned) -> device -> kinematics cache -> first NLL, by the wall clock
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).pin_memory()
+    h_x, h_e, h_xn, h_wn = pin(x), pin(eff), pin(xn), pin(wn)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    d_x, d_e, d_xn, d_wn = (t.to(device, non_blocking=True) for t in (h_x, h_e, h_xn, h_wn))
     e0.record()
     model.load_events(d_x, d_e)
     model.load_norm(d_xn, d_wn)
     e1.record()
+    cs, mws = step_params(cfg, c, 0)
+    model.set_params(cs, mws)
+    model.nll()
     torch.cuda.synchronize()
+    cold_ms = (time.perf_counter() - t0) * 1e3
     load_ms = e0.elapsed_time(e1)
-    del d_x, d_e, d_xn, d_wn
-    return model, c, {"gen_s": t_gen, "load_ms": load_ms}
+    h2d = sum(t.numel() * 8 for t in (h_x, h_e, h_xn, h_wn))
+    del d_x, d_e, d_xn, d_wn, h_x, h_e, h_xn, h_wn
+    return model, c, {"gen_s": t_gen, "load_ms": load_ms,
+                      "cold_start": {"ms": cold_ms, "h2d_bytes": int(h2d),
+                                     "what": "pinned host events -> H2D -> kinematics cache (k_kinematics) -> amp_set_params + first amp_nll, wall clock"}}
 
 
 def step_params(cfg, c, step):
@@ -256,7 +267,9 @@ def run_own(args):
         "config": {"workload": f"configs[{args.cfg}]: full K*+Z model (R=11, K=27), {args.n_data} data / {args.n_norm} norm events per GPU, "
                                f"P={P}, all lineshapes floating", "n_data": args.n_data, "n_norm": args.n_norm, "P": P,
                    "l2": "inputs (2.1 GB kinematics cache) larger than L2; no flush needed", "parallelism": f"replicas x{world}"},
-        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "note": "host wall clock around amp_set_params (host parameter arrays in) + amp_nll (host NLL out) per step; the events are "
+                        "resident as in a fit (PAPER.md:45) - the one-off upload of the events from host buffers is setup.cold_start"},
         "gpu_launches": int(launches),
         "event_evals_per_s": value * (args.n_data + args.n_norm),
         "phase_ms": {"lineshape": float(np.mean(t_line)), "data": float(np.mean(t_data)), "norm": norm_ms},
@@ -310,7 +323,8 @@ def run_reference(args):
     cfg = args.cfg
     P = 121 if cfg == 4 else 1
     # bounded sample per step so that steps+warmup finish in a few minutes
-    per_step = max(1_200_000 // (P * max(args.steps + args.warmup, 1)), 4000)
+    per_step = max(30_000_000 // (P * max(args.steps + args.warmup, 1)), 4000)
+    per_step = min(per_step, args.n_data + args.n_norm)
     n = max(int(per_step * args.n_data / (args.n_data + args.n_norm)), 500)
     m = max(per_step - n, 2000)
     Mo = O.Model(W.DECAY, W.resonances(cfg))
