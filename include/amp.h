@@ -136,6 +136,13 @@ amp_status amp_eval_lineshape(amp_model* m, int which, int r, double mass, doubl
  * at the lineshapes of point p, so that I(p) = c^H M c (fit fractions of Eq. 13, are ratios
  * of its diagonal blocks).                                                                             */
 amp_status amp_norm_matrix(amp_model* m, int p, double* h_M, void* stream);
+/* h_ff host [R]: fit fraction of every resonance at point p, Eq. 13 (the printed denominator "|S|^2" read
+ * as the integral of the density S):  FF_r = sum_j w_j S_r(x_j) / sum_j w_j S(x_j) over the loaded normalisation sample, S_r
+ * the density with all helicity amplitudes but those of resonance r set to zero.  Evaluated on the device as quadratic
+ * forms c_r^H M c_r / c^H M c of the normalisation matrix (built by the HERK kernel if it is not held).  Load the sample
+ * with unit weights for efficiency-free fractions.  Same call-order requirement as amp_norm_matrix
+ * (amp_set_norm_mode(m, 2) before amp_set_params).                                                                  */
+amp_status amp_fit_fractions(amp_model* m, int p, double* h_ff, void* stream);
 
 /* How the normalisation integral is evaluated: 0 = automatic (default), 1 = always the direct sum over
  * the norm events, 2 = always through the matrix M (rebuilt when a lineshape it depends on changes).   */

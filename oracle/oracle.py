@@ -154,6 +154,22 @@ class Model:
     def norm_integral(self, couplings, xn, wn, mass_width=None, prec=0):
         return self.nll(couplings, np.zeros((4, 0)), None, xn, wn, mass_width, prec, want_nll=False)[1]
 
+    def fit_fractions(self, couplings, xn, wn, mass_width=None, groups=None):
+        """Eq. 13 by its plain definition: FF_j = sum_n w_n S_j(x_n) / sum_n w_n S(x_n), where S_j is the density
+        with every helicity amplitude except those of resonance j set to zero ("setting to zero all the other helicity
+        amplitudes").  groups: optional list of lists of resonance indices (a fraction per group instead of per resonance)."""
+        c = np.asarray(couplings, dtype=np.complex128)
+        assert c.shape == (self.K,)
+        slot_res = []
+        for r in range(self.R):
+            three = self.kinds[r] == ZRES or (self.kinds[r] == KSTAR and self.Js[r] >= 1)
+            slot_res += [r] * (3 if three else 1)
+        slot_res = np.array(slot_res)
+        groups = [[r] for r in range(self.R)] if groups is None else groups
+        mw = None if mass_width is None else np.asarray(mass_width, dtype=np.float64).reshape(1, self.R, 2)
+        total = self.norm_integral(c, xn, wn, mw)[0]
+        return np.array([self.norm_integral(np.where(np.isin(slot_res, g), c, 0.0), xn, wn, mw)[0] / total for g in groups])
+
     def norm_matrix(self, xn, wn):
         xn = _f64(xn)
         kw, pw = _opt(wn)

@@ -19,7 +19,7 @@ AMP_MAX_RESONANCES, AMP_MAX_COUPLINGS, AMP_MAX_POINTS = 16, 48, 256
 SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
     "amp_load_norm", "amp_set_params", "amp_nll", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
-    "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode",
+    "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_fit_fractions", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode",
     "amp_last_call_stats", "amp_last_call_timing", "amp_recent_launch_ms", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
 ]
 
@@ -69,6 +69,7 @@ def lib():
         "amp_cache_column_name": (C.c_char_p, [i]),
         "amp_eval_lineshape": (i, [vp, i, i, d, d, vp, vp]),
         "amp_norm_matrix": (i, [vp, i, vp, vp]),
+        "amp_fit_fractions": (i, [vp, i, vp, vp]),
         "amp_set_norm_mode": (i, [vp, i]),
         "amp_set_lineshape_mode": (i, [vp, i]),
         "amp_set_batch_mode": (i, [vp, i]),
@@ -227,6 +228,11 @@ class Model:
         out = np.empty((self.K, self.K, 2), dtype=np.float64)
         self._check(lib().amp_norm_matrix(self._h, int(p), out.ctypes.data_as(C.c_void_p), _stream_ptr(stream)), "amp_norm_matrix")
         return out[..., 0] + 1j * out[..., 1]
+
+    def fit_fractions(self, p=0, stream=None):
+        out = np.empty(self.R, dtype=np.float64)
+        self._check(lib().amp_fit_fractions(self._h, int(p), out.ctypes.data_as(C.c_void_p), _stream_ptr(stream)), "amp_fit_fractions")
+        return out
 
     def set_norm_mode(self, mode):
         self._check(lib().amp_set_norm_mode(self._h, int(mode)), "amp_set_norm_mode")

@@ -1406,6 +1406,43 @@ amp_status amp_eval_lineshape(amp_model* m, int which, int r, double mass, doubl
     return AMP_OK;
 }
 
+amp_status amp_fit_fractions(amp_model* m, int p, double* h_ff, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
+    if (m->P < 1) return fail(m, AMP_ERR_STATE, "no parameters set (amp_set_params)");
+    if (p < 0 || p >= m->P || !h_ff) return fail(m, AMP_ERR_INVALID, "amp_fit_fractions: bad point index or null output");
+    HerkPlan hp;
+    if (!build_herk_plan(m, &hp, p, 1))
+        return fail(m, AMP_ERR_STATE, "amp_fit_fractions: the lineshape columns of this point are not held; call amp_set_norm_mode(m, 2) before amp_set_params");
+    m->stat_launches = m->stat_columns = 0;
+    amp_status st = ensure_pool(m, 0);
+    if (st != AMP_OK) return st;
+    st = refresh_columns(m, m->norm, true, s);
+    if (st != AMP_OK) return st;
+    // rows of coefficient vectors for the quadratic-form kernel: row 0 = all couplings, row 1 + r = those of resonance r only
+    const int R = m->R, nent = hp.nent;
+    std::vector<double2> C((size_t)(R + 1) * nent, make_double2(0, 0));
+    for (int e = 0; e < nent; ++e) C[e] = hp.C[e];
+    for (int r = 0; r < R; ++r) {
+        const int ns = (m->res[r].kind == AMP_Z || (m->res[r].kind == AMP_KSTAR && m->res[r].J >= 1)) ? 3 : 1;
+        for (int j = 0; j < ns; ++j) C[(size_t)(1 + r) * nent + m->slot0[r] + j] = hp.C[m->slot0[r] + j];   // single point: entry k = slot k
+    }
+    hp.C.swap(C);
+    double* d_tmp = nullptr;
+    CK(cudaMalloc(&d_tmp, sizeof(double) * (R + 1)));
+    st = norm_via_matrix(m, hp, d_tmp, s);
+    std::vector<double> q((size_t)R + 1);
+    cudaError_t e = st == AMP_OK ? cudaMemcpyAsync(q.data(), d_tmp, sizeof(double) * (R + 1), cudaMemcpyDeviceToHost, s) : cudaSuccess;
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(d_tmp);
+    if (st != AMP_OK) return st;
+    if (e != cudaSuccess) return cuda_fail(m, e, "amp_fit_fractions");
+    if (!(q[0] > 0) || !std::isfinite(q[0])) return fail(m, AMP_ERR_DOMAIN, "amp_fit_fractions: the total integral is not positive");
+    for (int r = 0; r < R; ++r) h_ff[r] = q[1 + r] / q[0];
+    return AMP_OK;
+}
+
 amp_status amp_norm_matrix(amp_model* m, int p, double* h_M, void* stream) {
     if (!m) return AMP_ERR_INVALID;
     cudaStream_t s = (cudaStream_t)stream;

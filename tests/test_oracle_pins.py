@@ -420,6 +420,31 @@ def test_mass_width_override_equals_new_model():
     assert a == b
 
 
+# ------------------------------------------------------------------ fit fractions, Eq. 13
+def test_P13_fit_fractions():
+    """Eq. 13.  (i) a model with one resonance has FF = 1; (ii) on a full-angle quadrature grid with
+    eps = 1 the interference between K* of different spin integrates to zero (orthogonality of the d^J, pin P2), so the
+    fractions of the SPIN GROUPS add up to exactly 1 while the per-resonance fractions do not ("the sum of
+    all the fit fractions is not constrained to 100%"); (iii) FF is invariant under a common rescaling of all couplings
+    and linear in |H_j|^2 for the numerator alone."""
+    xq, wq = quadrature_events(24, 6, 4, 8)
+    one = O.Model(DEC, [W.resonances(1)[4]])
+    assert abs(one.fit_fractions(np.array([0.3 + 0.1j, 1.0, -0.7j]), xq, wq)[0] - 1.0) < 1e-14
+    res = W.resonances(1)
+    M = model(1)
+    c = W.couplings(1)
+    ff = M.fit_fractions(c, xq, wq)
+    assert np.all(ff > 0) and abs(ff.sum() - 1.0) > 1e-3                       # interference between same-spin K*
+    groups = [[r for r, rr in enumerate(res) if rr[1] == J] for J in range(5)]
+    ffJ = M.fit_fractions(c, xq, wq, groups=groups)
+    assert abs(ffJ.sum() - 1.0) < 1e-12
+    assert np.max(np.abs(M.fit_fractions((2.0 - 1.5j) * c, xq, wq) - ff)) < 1e-14
+    slots = W.slot_table(res)
+    c2 = np.array([2.0 * v if slots[k][0] == 4 else v for k, v in enumerate(c)])   # K2*(1430) amplitudes doubled
+    I1, I2 = M.norm_integral(c, xq, wq)[0], M.norm_integral(c2, xq, wq)[0]
+    assert abs(M.fit_fractions(c2, xq, wq)[4] * I2 - 4.0 * ff[4] * I1) < 1e-13 * ff[4] * I1
+
+
 # ------------------------------------------------------------------ golden fixtures (tests/golden/)
 GOLDEN = __import__("os").path.join(__import__("os").path.dirname(__import__("os").path.abspath(__file__)), "golden")
 

@@ -351,6 +351,29 @@ def test_norm_matrix_matches_oracle_and_direct_sum():
     assert abs(I_dir - Mo.norm_integral(c, xn, wn)[0]) < 1e-12 * I_dir
 
 
+def test_fit_fractions_match_oracle():
+    """Eq. 13: per-resonance fit fractions from the device quadratic forms against the oracle's plain definition
+    (density with all other helicity amplitudes set to zero, summed over the same sample), configs 1 and 2, also at
+    moved masses and widths."""
+    for cfg in (1, 2):
+        Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+        c = W.couplings(cfg)
+        xn, wn = W.norm_events(cfg, 9001)
+        Mg.load_norm(dev(xn), dev(wn))
+        Mg.set_norm_mode(2)
+        Mg.set_params(c)
+        ff = Mg.fit_fractions(0)
+        ref = Mo.fit_fractions(c, xn, wn)
+        assert ff.shape == (len(W.resonances(cfg)),)
+        assert np.max(np.abs(ff - ref) / ref) < 1e-11, (cfg, ff, ref)
+        mw = W.step_mass_width(3, 2)[:len(W.resonances(cfg))]
+        Mg.set_params(c, mw[None])
+        ff2 = Mg.fit_fractions(0)
+        ref2 = Mo.fit_fractions(c, xn, wn, mass_width=mw)
+        assert np.max(np.abs(ff2 - ref2) / ref2) < 1e-11
+        assert np.max(np.abs(ff2 - ff)) > 1e-9          # the lineshapes did move
+
+
 def test_static_lineshapes_switch_to_the_matrix():
     """cfg 1 call pattern (masses and widths fixed, couplings move): the second call with unchanged lineshapes builds
     M once, later calls only evaluate c^H M c; a moved mass goes back to the direct sum."""
