@@ -33,7 +33,7 @@
 
 namespace {
 
-enum Kind { KSTAR = 0, ZRES = 1, CONSTANT = 2 };
+enum Kind { KSTAR = 0, ZRES = 1, CONSTANT = 2, LASS = 3 };
 
 template <typename T>
 struct Decay {
@@ -92,9 +92,28 @@ inline void orbital_L(int kind, int J, int* LB, int* LR) {
 //   Gamma(m) = Gamma0 (pR/pR0)^(2LR+1) (MR/m) FR^2
 //   A^R(m)   = FB (pB/MB)^LB FR (pR/m)^LR / (MR^2 - m^2 - i MR Gamma(m))
 // m is the running mass of the resonance's daughters: m_Kpi for a K*, m_psipi for the Z.
+// O3b. LASS parametrisation of the K pi S-wave, Eqs. (7)-(8) (readings A21, A22):
+//   A_LASS = (m/q) sin(theta_B) e^{i theta_B} + 2 e^{2 i theta_B} (M0^2/q0) Gamma0 / (M0^2 - m^2 - i M0 Gamma(m))
+//   cot(theta_B) = 1/(a q) + b q / 2,   a = 1.95 GeV^-1, b = 1.76 GeV^-1
+// q = K momentum in the K pi frame at the running mass, q0 at the K0*(1430) mass M0; Gamma(m) is Eq. (3) with L_R = 0.
+template <typename T>
+std::complex<T> lass_lineshape(const Decay<T>& dk, const Resonance<T>& R, T m, T* gamma_out) {
+    const T a = T(1.95e-3L), b = T(1.76e-3L);                 // MeV^-1
+    const T q = breakup_momentum(m, dk.mK, dk.mpi), q0 = breakup_momentum(R.mass, dk.mK, dk.mpi);
+    const T cot = 1 / (a * q) + b * q / 2;                      // Eq. (8)
+    const T theta = std::atan2(T(1), cot);                      // theta_B in (0, pi)
+    const T gamma = R.width * (q / q0) * (R.mass / m);          // Eq. (3), L_R = 0 (F^(0) = 1)
+    if (gamma_out) *gamma_out = gamma;
+    const std::complex<T> first = (m / q) * std::sin(theta) * std::polar(T(1), theta);
+    const std::complex<T> den(R.mass * R.mass - m * m, -R.mass * gamma);
+    const std::complex<T> second = T(2) * std::polar(T(1), 2 * theta) * ((R.mass * R.mass / q0) * R.width) / den;
+    return first + second;                                       // Eq. (7)
+}
+
 template <typename T>
 std::complex<T> lineshape(const Decay<T>& dk, const Resonance<T>& R, T m, T* gamma_out = nullptr) {
     if (R.kind == CONSTANT) { if (gamma_out) *gamma_out = 0; return {T(1), T(0)}; }
+    if (R.kind == LASS) return lass_lineshape(dk, R, m, gamma_out);
     int LB, LR;
     orbital_L(R.kind, R.J, &LB, &LR);
     T pB, pB0, pR, pR0;

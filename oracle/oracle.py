@@ -37,7 +37,7 @@ _lib.orc_nll.restype = _i
 _lib.orc_nll.argtypes = _MODEL + [_i, _pd, _vp, _pd, _vp, _ll, _pd, _vp, _ll, _i, _vp, _vp]
 _lib.orc_norm_matrix.argtypes = _MODEL + [_pd, _vp, _ll, _pd]
 
-KSTAR, ZRES, CONST = 0, 1, 2
+KSTAR, ZRES, CONST, LASS = 0, 1, 2, 3
 
 
 def num_threads():

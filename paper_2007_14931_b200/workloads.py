@@ -16,7 +16,7 @@ SEED = 2007014931
 # m_B0, m_J/psi, m_K+, m_pi- in MeV (BASELINE.json configs[0])
 DECAY = (5279.65, 3096.9, 493.677, 139.570)
 RADIUS = 1.6e-3  # MeV^-1 (1.6 GeV^-1; reading A3)
-KSTAR, ZRES, CONST = 0, 1, 2
+KSTAR, ZRES, CONST, LASS = 0, 1, 2, 3
 
 # (name, kind, J, mass, width) — BASELINE.json configs[1], configs[2] for the Z
 KSTARS = [
@@ -58,6 +58,37 @@ def resonances(cfg):
     if cfg >= 2:
         res.append((ZPLUS[1], ZPLUS[2], ZPLUS[3], ZPLUS[4], RADIUS))
     return res
+
+
+def resonances_lass(with_z=True):
+    """The paper's LASS variant of the model (Eq. 9): the low-mass K pi S-wave — kappa(800) and K0*(1430)
+    — is replaced by ONE LASS term built on the K0*(1430) mass and width (Eq. 7); the other eight K* (and the Z) stay."""
+    k1430 = KSTARS[3]
+    res = [(LASS, 0, k1430[3], k1430[4], RADIUS)]
+    res += [(k[1], k[2], k[3], k[4], RADIUS) for i, k in enumerate(KSTARS) if i not in (0, 3)]
+    if with_z:
+        res.append((ZPLUS[1], ZPLUS[2], ZPLUS[3], ZPLUS[4], RADIUS))
+    return res
+
+
+def couplings_lass(with_z=True):
+    """seeded couplings of the LASS model: as `couplings`, the LASS amplitude scaled to the size of a Breit-Wigner peak
+    (A_LASS is O(1-10), a K* lineshape O(1e-6)), Eq. 6 on K*(892), Eq. 11 on the Z"""
+    res = resonances_lass(with_z)
+    slots = slot_table(res)
+    rng = np.random.default_rng(np.random.SeedSequence([SEED, 7, 0]))
+    c = rng.uniform(0.5, 1.5, len(slots)) * np.exp(1j * rng.uniform(-np.pi, np.pi, len(slots)))
+    for k, (r, lam) in enumerate(slots):
+        if res[r][0] == LASS:
+            c[k] *= 0.3 / (KSTARS[1][3] * KSTARS[1][4])
+        if res[r][0] == KSTAR and abs(res[r][2] - KSTARS[1][3]) < 1e-9 and lam == 0:
+            c[k] = 1.0
+        if res[r][0] == ZRES:
+            c[k] *= Z_COUPLING_SCALE
+    for k, (r, lam) in enumerate(slots):
+        if res[r][0] == ZRES and lam == +1:
+            c[k] = c[k - 2]
+    return c
 
 
 def slot_table(res):

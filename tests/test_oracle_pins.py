@@ -420,6 +420,51 @@ def test_mass_width_override_equals_new_model():
     assert a == b
 
 
+# ------------------------------------------------------------------ LASS S-wave, Eqs. 7-8
+def test_P14_lass_lineshape():
+    """Eqs. 7-8.  The oracle returns the sum of the two terms; they are separated by letting the width
+    go to zero (the resonant term vanishes away from the pole).  Pins: (i) the effective-range term is (m/q) sin(th) e^{i th}
+    with cot(th) = 1/(a q) + b q/2: modulus, phase, and the scattering-length limit A -> a m at threshold; (ii) the resonant
+    term is 2 (m/q) e^{2 i th} sin(dR) e^{i dR} with tan(dR) = M0 Gamma(m)/(M0^2 - m^2) and Gamma(m) = Gamma0 (q/q0)(M0/m):
+    modulus and phase, and its value 2 i e^{2 i th} M0/q0 at the pole; (iii) with the resonant term at HALF its printed
+    strength the sum is the elastic-unitary amplitude (m/q) sin(th + dR) e^{i (th + dR)} — the form the 'similar
+    parametrization' of LASS descends from — which fixes the relative phase e^{2 i th} and the running width together."""
+    a, b = 1.95e-3, 1.76e-3
+    M0, G0 = 1425.0, 270.0
+    lass = O.Model(DEC, [(O.LASS, 0, M0, G0, R16)])
+    bare = O.Model(DEC, [(O.LASS, 0, M0, 1e-30, R16)])
+    q0 = O.breakup_momentum(M0, MK, MPI)
+    assert lass.K == 1
+    for m in (640.0, 700.0, 900.0, 1200.0, 1424.0, 1500.0, 1900.0, 2150.0):
+        q = O.breakup_momentum(m, MK, MPI)
+        th = math.atan2(1.0, 1.0 / (a * q) + 0.5 * b * q)
+        A, gam = lass.lineshape(0, m)
+        A1 = bare.lineshape(0, m)[0]
+        assert abs(gam - G0 * (q / q0) * (M0 / m)) < 1e-12 * gam
+        assert abs(abs(A1) * q / m - math.sin(th)) < 1e-13 and abs(np.angle(A1) - th) < 1e-13
+        dR = math.atan2(M0 * gam, M0 * M0 - m * m)
+        T2 = A - A1
+        ref2 = 2.0 * (m / q) * np.exp(2j * th) * math.sin(dR) * np.exp(1j * dR)
+        assert abs(T2 - ref2) < 1e-12 * abs(ref2)
+        unitary = A1 + 0.5 * T2
+        assert abs(unitary - (m / q) * math.sin(th + dR) * np.exp(1j * (th + dR))) < 1e-12 * abs(unitary)
+        assert abs(unitary) * q / m <= 1.0 + 1e-12
+    m_thr = MK + MPI + 1e-6
+    q_thr = O.breakup_momentum(m_thr, MK, MPI)
+    assert abs(bare.lineshape(0, m_thr)[0] - a * m_thr) < 2.0 * a * q_thr * a * m_thr   # scattering length: A = a m (1 + O(a q))
+    qp = O.breakup_momentum(M0, MK, MPI)
+    thp = math.atan2(1.0, 1.0 / (a * qp) + 0.5 * b * qp)
+    Ap = lass.lineshape(0, M0)[0] - (M0 / qp) * math.sin(thp) * np.exp(1j * thp)   # (at the pole the resonant term survives width -> 0)
+    assert abs(Ap - 2j * np.exp(2j * thp) * M0 / q0) < 1e-12 * abs(Ap)
+    # in the model: one lambda = 0 slot with the J = 0 angular factor d^1_{0 xi}(theta_psi), Eq. 9
+    x = np.array([1000.0, 0.3, -0.4, 1.1])
+    B = lass.basis_terms(x)
+    A1000 = lass.lineshape(0, 1000.0)[0]
+    s = math.sqrt(1 - 0.16) / math.sqrt(2)
+    assert abs(B[0, 0] - A1000 * s) < 1e-14 * abs(A1000) and abs(B[0, 1] + A1000 * s) < 1e-14 * abs(A1000)
+    assert abs(lass.lineshape(0, 1000.0, prec=1)[0] - A1000) < 1e-13 * abs(A1000)
+
+
 # ------------------------------------------------------------------ fit fractions, Eq. 13
 def test_P13_fit_fractions():
     """Eq. 13.  (i) a model with one resonance has FF = 1; (ii) on a full-angle quadrature grid with
