@@ -44,8 +44,12 @@ typedef enum {
 
 /* Resonance kinds.  AMP_KSTAR: K* -> K pi, Eq. 4.  AMP_Z: Z -> J/psi pi evaluated in
  * its own decay frame, Eq. 10; only J^P = 1+ (PAPER.md:171).  AMP_CONST: lineshape == 1,
- * J = 0, angular factor d^1_{0 xi}(theta_psi) (BASELINE.json configs[0], "constant S-wave term").   */
-typedef enum { AMP_KSTAR = 0, AMP_Z = 1, AMP_CONST = 2 } amp_kind;
+ * J = 0, angular factor d^1_{0 xi}(theta_psi) (BASELINE.json configs[0], "constant S-wave term").
+ * AMP_LASS: the LASS parametrisation of the K pi S-wave, Eqs. 7-9: J = 0, one coupling slot,
+ * lineshape A_LASS built on mass = M(K0*(1430)), width = Gamma(K0*(1430)) with the paper's a = 1.95 GeV^-1,
+ * b = 1.76 GeV^-1 (Eq. 8); radius is ignored.  Models with a LASS term run the generic streaming kernel; gradient
+ * batches of such models take the dense path.                                                          */
+typedef enum { AMP_KSTAR = 0, AMP_Z = 1, AMP_CONST = 2, AMP_LASS = 3 } amp_kind;
 
 /* One resonance: spin J (K*: 0..4, Z: 1, CONST: 0), nominal mass M_R and width
  * Gamma_0 [MeV], Blatt-Weisskopf radius r [MeV^-1] used for both F_B and F_R of Eq. 2 (PAPER.md:89,

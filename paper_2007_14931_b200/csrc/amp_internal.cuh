@@ -148,9 +148,28 @@ __device__ __forceinline__ double powi(double x, int n) {   // n in 0..9, warp-u
     return r;
 }
 
+// LASS S-wave, Eqs. 7-8, in rational form (no angle is ever formed): with t = cot(theta_B) =
+// 1/(a q) + b q/2,  sin(th) e^{i th} = (t + i)/(t^2 + 1),  e^{2 i th} = (t + i)^2/(t^2 + 1), and M0 Gamma(m) = kG q/m,
+// kG = M0^2 Gamma0 / q0 (also the numerator constant of the resonant term):
+//   A_LASS = (m/q) (t + i)/(t^2 + 1) + 2 kG (t + i)^2/(t^2 + 1) / (M0^2 - m^2 - i kG q/m)
+__device__ __forceinline__ double2 lass_eval(double M2, double kG, double m2, double invm, double q) {
+    const double a = 1.95e-3, b = 1.76e-3;                    // MeV^-1
+    const double t = fast_rcp(a * q) + 0.5 * b * q;
+    const double n1 = fast_rcp(fma(t, t, 1.0));
+    const double x = q * invm, mq = fast_rcp(x);
+    const double2 s1 = make_double2(t * n1, n1);              // sin(th) e^{i th}
+    const double2 e2 = make_double2(fma(t, t, -1.0) * n1, 2.0 * t * n1);   // e^{2 i th}
+    const double MG = kG * x, dre = M2 - m2;
+    const double r = 2.0 * kG * fast_rcp(fma(dre, dre, MG * MG));
+    const double2 bw = make_double2(r * dre, r * MG);         // 2 kG / (M0^2 - m^2 - i M0 Gamma(m))
+    const double2 second = cmul(e2, bw);
+    return make_double2(fma(mq, s1.x, second.x), fma(mq, s1.y, second.y));
+}
+
 // Lineshape A^R(m) of Eqs. 2-3 from the cached running-mass quantities of its chain.
 __device__ __forceinline__ double2 lineshape_eval(const LineConst& c, double m2, double invm, double pR, double pB) {
     if (c.chain == 2) return make_double2(1.0, 0.0);
+    if (c.kind == AMP_LASS) return lass_eval(c.M2, c.kG, m2, invm, pR);
     const double zR = c.r2 * pR * pR, zB = c.r2 * pB * pB;
     const double DB = bw_poly(c.LB, zB);
     const double rs = rsqrt(bw_poly(c.LR, zR) * DB);
@@ -220,6 +239,7 @@ __device__ __forceinline__ double2 bw_unscaled(const ResEntry& e, double m2, dou
 struct StreamArgs {
     ResEntry ent[AMP_MAX_RESONANCES];
     BarrierGroup grp[AMP_MAX_RESONANCES];
+    int lass0, nlass;               // LASS terms: entries ent[lass0 .. lass0 + nlass) (kG, M2 and c0 used), after the K* and Z entries
     int gstart[7];                  // groups of K* spin J: grp[gstart[J] .. gstart[J+1]), J = 0..4; Z groups: gstart[5] .. gstart[6]
     int shape[6];                   // resonances per K* spin 0..4 and Z's; entries are stored in that order
     int shape_fixed;                // 1: one radius per spin, r2_spin valid: a shape-specialised kernel may run

@@ -132,6 +132,16 @@ bool make_line_const(const amp_model* m, int r, double mass, double width, LineC
     LineConst c{};
     c.kind = R.kind;
     if (R.kind == AMP_CONST) { c.chain = 2; *out = c; return true; }
+    if (R.kind == AMP_LASS) {   // Eq. 7: kG = M0^2 Gamma0 / q0, q0 the K momentum at the K0*(1430) mass
+        const double q0 = h_two_body(mass, m->dk.mK, m->dk.mpi);
+        if (!(q0 > 0) || !(mass > 0) || !(width > 0)) return false;
+        c.chain = 0;
+        c.M2 = mass * mass;
+        c.kG = mass * mass * width / q0;
+        c.kN = 1.0;
+        *out = c;
+        return true;
+    }
     double pR0, pB0;
     if (R.kind == AMP_KSTAR) {
         c.chain = 0;
@@ -245,6 +255,7 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
         if (a.kind == AMP_KSTAR) ok = a.J >= 0 && a.J <= 4;
         else if (a.kind == AMP_Z) ok = a.J == 1;
         else if (a.kind == AMP_CONST) ok = a.J == 0;
+        else if (a.kind == AMP_LASS) ok = a.J == 0;
         else ok = false;
         if (a.kind != AMP_CONST) ok = ok && a.mass > 0 && a.width > 0 && a.radius >= 0 && std::isfinite(a.mass + a.width + a.radius);
         if (!ok) { delete m; return AMP_ERR_INVALID; }
@@ -416,6 +427,8 @@ bool build_delta_plan(amp_model* m) {
     const int P = m->P, R = m->R, K = m->K;
     m->delta_chunks.clear();
     if (P < 2) return false;
+    for (const auto& rs : m->res)
+        if (rs.kind == AMP_LASS) return false;   // LASS terms are not carried by the gradient-batch kernel
     int ent_of_res[AMP_MAX_RESONANCES], grp_of_res[AMP_MAX_RESONANCES];
     {
         StreamArgs tmp;
@@ -704,6 +717,22 @@ void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, Str
     a->gstart[5] = g;
     add_groups(AMP_Z, 1);
     a->gstart[6] = g;
+    a->lass0 = t;
+    for (int r = 0; r < m->R; ++r) {
+        if (m->res[r].kind != AMP_LASS) continue;
+        LineConst lc;
+        make_line_const(m, r, m->mw[((size_t)p * m->R + r) * 2], m->mw[((size_t)p * m->R + r) * 2 + 1], &lc);
+        if (ent_of_res) { ent_of_res[r] = t; grp_of_res[r] = 0; }
+        ResEntry& e = a->ent[t++];
+        e.kN = 1.0; e.kG = lc.kG; e.M2 = lc.M2;
+        const double* cp = &m->couplings[((size_t)p * m->K + m->slot0[r]) * 2];
+        e.c0 = make_double2(cp[0], cp[1]);
+        e.cm = e.cp = make_double2(0, 0);
+        const size_t ci = (size_t)p * m->R + r;
+        const int sidx = ci < m->colidx.size() ? m->colidx[ci] : -1;
+        e.column = (sidx >= 0 && !m->stream_inline) ? sidx : -1;
+    }
+    a->nlass = t - a->lass0;
     for (int sp = 0; sp < 6; ++sp) {
         const int ng = a->gstart[sp + 1] - a->gstart[sp];
         a->shape[sp] = 0;

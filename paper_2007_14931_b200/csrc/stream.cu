@@ -108,6 +108,16 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         AMP_SPIN(3, 2, SH::n3, SH::o3, c * fma(2.5, c2, -1.5), -0.43301270189221932338 * s * fma(5.0, c2, -1.0))            // sqrt(3)/4
         AMP_SPIN(4, 3, SH::n4, SH::o4, fma(fma(4.375, c2, -3.75), c2, 0.375), -0.55901699437494742410 * s * c * fma(7.0, c2, -3.0))   // sqrt(5)/4
 #undef AMP_SPIN
+        if (SH::n0 < 0) {   // LASS S-wave terms (generic kernel only): J = 0, lambda = 0, lineshape of Eq. 7
+            for (int t = a.lass0; t < a.lass0 + a.nlass; ++t) {
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    const double2 bw = a.ent[t].column >= 0 ? a.cols[(size_t)a.ent[t].column * a.npad + i0 + e]
+                                                            : lass_eval(a.ent[t].M2, a.ent[t].kG, m2.v[e], invm.v[e], q.v[e]);
+                    V0[e] = cfma(a.ent[t].c0, bw, V0[e]);
+                }
+            }
+        }
         // A_xi = sum_l e^{i l phi} d^1_{l xi}(theta_psi) V_l ; d^1_{0,+-1} = +-s/sqrt2, d^1_{11} = d^1_{-1-1} = (1+c)/2, d^1_{1-1} = d^1_{-11} = (1-c)/2
         double2 Ap[E], Am[E];
 #pragma unroll
@@ -257,7 +267,8 @@ cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s) {
         return a.shape_fixed && n[0] == a0 && n[1] == a1 && n[2] == a2 && n[3] == a3 && n[4] == a4 && n[5] == az;
     };
     cudaError_t e;
-    if (is(3, 3, 2, 1, 1, 1)) e = launch_shape<Shape<3, 3, 2, 1, 1, 1>>(a, grid, s);
+    if (a.nlass > 0) e = launch_shape<Generic>(a, grid, s);   // LASS terms live in the generic kernel
+    else if (is(3, 3, 2, 1, 1, 1)) e = launch_shape<Shape<3, 3, 2, 1, 1, 1>>(a, grid, s);
     else if (is(3, 3, 2, 1, 1, 0)) e = launch_shape<Shape<3, 3, 2, 1, 1, 0>>(a, grid, s);
     else if (is(0, 1, 0, 0, 0, 0)) e = launch_shape<Shape<0, 1, 0, 0, 0, 0>>(a, grid, s);
     else e = launch_shape<Generic>(a, grid, s);

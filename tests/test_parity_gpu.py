@@ -374,6 +374,59 @@ def test_fit_fractions_match_oracle():
         assert np.max(np.abs(ff2 - ff)) > 1e-9          # the lineshapes did move
 
 
+@pytest.mark.parametrize("with_z", [True, False])
+def test_lass_model_matches_oracle(with_z):
+    """Eqs. 7-9: the model with the LASS S-wave term (replacing kappa(800) and K0*(1430)): lineshape column, per-event density,
+    NLL through the fused launch, the separate launches, the matrix M, and a batch of points through the DMMA contraction
+    with the K0*(1430) mass and width inside the LASS term moving."""
+    from paper_2007_14931_b200 import binding as B
+    res = W.resonances_lass(with_z)
+    c = W.couplings_lass(with_z)
+    Mo, Mg = O.Model(W.DECAY, res), B.Model(W.DECAY, res)
+    assert Mg.K == Mo.K == len(c)
+    xn, wn = W.norm_events(2, 20011)
+    x, eff = W.data_events(2, lambda xx, ee: Mo.eval_events(c, xx, ee), n=5003)
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    col = Mg.eval_lineshape(0, res[0][2], res[0][3]).cpu().numpy()
+    ref = np.array([Mo.lineshape(0, v)[0] for v in x[0]])
+    assert np.max(np.abs(col[:, 0] + 1j * col[:, 1] - ref) / np.abs(ref)) < 5e-13
+    Mg.set_params(c)
+    v = Mg.eval_events(0).cpu().numpy()
+    vref = Mo.eval_events(c, x, eff)
+    assert np.max(np.abs(v - vref) / vref) < RTOL_EVENT
+    only = np.array([c[0]] + [0.0] * (len(c) - 1))               # the LASS term alone
+    Mg.set_params(only)
+    assert np.max(np.abs(Mg.eval_events(0).cpu().numpy() - Mo.eval_events(only, x, eff)) / Mo.eval_events(only, x, eff)) < RTOL_EVENT
+    mw = np.array([[r[2], r[3]] for r in res]) * (1 + 1e-3 * np.linspace(-1, 1, 2 * len(res)).reshape(-1, 2))
+    for fused in (0, 1):
+        mwf = mw * (1 + 1e-4 * fused)                            # (equal masses on successive calls would switch to the matrix)
+        Mg.set_fused_mode(fused)
+        Mg.set_params(c, mwf[None])
+        nll = Mg.nll()[0]
+        assert Mg.last_call_stats()["norm_path"] == (4 if fused == 0 else 1)
+        rn = Mo.nll(c, x, eff, xn, wn, mass_width=mwf[None])[0][0]
+        assert abs(nll - rn) < RTOL_NLL * abs(rn)
+    Mg.set_fused_mode(0)
+    Mg.set_params(c, mwf[None])
+    assert abs(Mg.nll()[0] - rn) < RTOL_NLL * abs(rn)
+    assert Mg.last_call_stats()["norm_path"] == 2             # same masses twice: matrix M
+    # a batch: LASS coupling, LASS mass and width, another coupling, moving point by point -> dense DMMA path
+    P = 30
+    rng = np.random.default_rng(9)
+    cs, mws = np.tile(c, (P, 1)), np.tile(mw, (P, 1, 1))
+    for p in range(1, P):
+        cs[p, p % len(c)] *= 1 + 0.2 * rng.uniform(-1, 1)
+        cs[p, 0] *= 1 + 0.1j * rng.uniform(-1, 1)
+        if p % 3 == 0:
+            mws[p, 0] *= 1 + 1e-2 * rng.uniform(-1, 1, 2)
+    Mg.set_params(cs, mws)
+    nll = Mg.nll()
+    assert Mg.last_call_stats()["norm_path"] in (2, 3)
+    rb, _ = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+    assert np.max(np.abs(nll - rb) / np.abs(rb)) < RTOL_NLL
+
+
 def test_static_lineshapes_switch_to_the_matrix():
     """cfg 1 call pattern (masses and widths fixed, couplings move): the second call with unchanged lineshapes builds
     M once, later calls only evaluate c^H M c; a moved mass goes back to the direct sum."""
