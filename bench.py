@@ -46,6 +46,16 @@ TRAFFIC_NCU_BYTES_CFG4 = 2.192431e9 + 4.04e6  # profiles/r01c_ncu_full_delta_cfg
 DELTA_FLOP_PER_EVENT = 730.0 + 31 * 40.0 + 100 * 25.0 + 20 * 47.0
 
 
+LASS = False   # --lass: the paper's LASS variant of the model (Eq. 9) instead of kappa(800) + K0*(1430)
+
+
+def model_def(cfg):
+    """(resonance list, seeded couplings) of the benchmarked model"""
+    if LASS:
+        return W.resonances_lass(True), W.couplings_lass(True)
+    return W.resonances(cfg), W.couplings(cfg)
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -107,8 +117,7 @@ def build_workload(args, device):
     from paper_2007_14931_b200 import binding as B
 
     cfg = args.cfg
-    res = W.resonances(cfg)
-    c = W.couplings(cfg)
+    res, c = model_def(cfg)
     dev = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=device)
     gen = B.Model(W.DECAY, res)
 
@@ -152,7 +161,11 @@ def step_params(cfg, c, step):
     the couplings rotated by a small seeded amount, so that successive calls genuinely differ."""
     if cfg == 4:
         return W.fit_points(cfg, step)
-    mw = W.step_mass_width(cfg, step)
+    if LASS:
+        mw = np.array([[r[2], r[3]] for r in W.resonances_lass(True)], dtype=np.float64)
+        mw *= 1.0 + 1e-4 * np.random.default_rng(np.random.SeedSequence([W.SEED, 98, int(step)])).uniform(-1, 1, mw.shape)
+    else:
+        mw = W.step_mass_width(cfg, step)
     rng = np.random.default_rng(np.random.SeedSequence([W.SEED, 99, int(step)]))
     cc = c * (1.0 + 1e-3 * rng.uniform(-1, 1, c.size)) * np.exp(1e-3j * rng.uniform(-1, 1, c.size))
     return cc[None], mw[None]
@@ -264,7 +277,7 @@ def run_own(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"configs[{args.cfg}]: full K*+Z model (R=11, K=27), {args.n_data} data / {args.n_norm} norm events per GPU, "
+        "config": {"workload": ("LASS variant (Eq. 9: LASS S-wave + 8 K* + Z, R=10, K=26) of " if LASS else "") + f"configs[{args.cfg}]: full K*+Z model (R=11, K=27), {args.n_data} data / {args.n_norm} norm events per GPU, "
                                f"P={P}, all lineshapes floating", "n_data": args.n_data, "n_norm": args.n_norm, "P": P,
                    "l2": "inputs (2.1 GB kinematics cache) larger than L2; no flush needed", "parallelism": f"replicas x{world}"},
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
@@ -298,8 +311,8 @@ def cpu_baseline(args, target_evals=None):
     n = max(int(args.n_data * frac), 1000)
     m = max(int(args.n_norm * frac), 5000)
     reps = max(1, int(round(target_evals / (P * (n + m)))))
-    Mo = O.Model(W.DECAY, W.resonances(cfg))
-    c = W.couplings(cfg)
+    res, c = model_def(cfg)
+    Mo = O.Model(W.DECAY, res)
     xn, wn = W.norm_events(cfg, m)
     x, eff = W.data_events(cfg, lambda xx, ee: Mo.eval_events(c, xx, ee), n=n)
     dt = 0.0
@@ -327,8 +340,8 @@ def run_reference(args):
     per_step = min(per_step, args.n_data + args.n_norm)
     n = max(int(per_step * args.n_data / (args.n_data + args.n_norm)), 500)
     m = max(per_step - n, 2000)
-    Mo = O.Model(W.DECAY, W.resonances(cfg))
-    c = W.couplings(cfg)
+    res, c = model_def(cfg)
+    Mo = O.Model(W.DECAY, res)
     xn, wn = W.norm_events(cfg, m)
     x, eff = W.data_events(cfg, lambda xx, ee: Mo.eval_events(c, xx, ee), n=n)
     times = []
@@ -362,7 +375,12 @@ def main():
     ap.add_argument("--n-data", type=int, default=2_000_000)
     ap.add_argument("--n-norm", type=int, default=10_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--lass", action="store_true", help="configs[3] call pattern on the LASS variant of the model (Eqs. 7-9; SURVEY.md 8(f)-1)")
     args = ap.parse_args()
+    global LASS
+    LASS = bool(args.lass)
+    if LASS and args.cfg != 3:
+        ap.error("--lass goes with --cfg 3")
     args.warmup = max(args.warmup, 3) if args.impl == "own" else args.warmup
     if args.impl == "reference":
         run_reference(args)
