@@ -427,6 +427,50 @@ def test_lass_model_matches_oracle(with_z):
     assert np.max(np.abs(nll - rb) / np.abs(rb)) < RTOL_NLL
 
 
+def test_two_z_model_matches_oracle():
+    """SURVEY.md 8(f)-3 / PAPER.md:165, 191 ("ten K*s and two Zs"): a second 1+ exotic, Z(4430) (m = 4478, Gamma = 181 MeV), shares
+    the Z(4200)'s decay frame and angular cache; K = 30.  Per-event density, fused NLL with all 12 lineshapes moving, and a
+    gradient batch that moves the couplings, mass and width of both Zs (gradient-batch kernel)."""
+    from paper_2007_14931_b200 import binding as B
+    res = W.resonances(2) + [(W.ZRES, 1, 4478.0, 181.0, W.RADIUS)]
+    rng = np.random.default_rng(21)
+    c = np.concatenate([W.couplings(2), 4.0 * rng.uniform(0.5, 1.5, 3) * np.exp(1j * rng.uniform(-3, 3, 3))])
+    c[-1] = c[-3]                                             # Eq. 11
+    Mo, Mg = O.Model(W.DECAY, res), B.Model(W.DECAY, res)
+    assert Mg.K == 30
+    xn, wn = W.norm_events(2, 20011)
+    x, eff = W.data_events(2, lambda xx, ee: Mo.eval_events(c, xx, ee), n=6007)
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    Mg.set_params(c)
+    v, vref = Mg.eval_events(0).cpu().numpy(), Mo.eval_events(c, x, eff)
+    assert np.max(np.abs(v - vref) / vref) < RTOL_EVENT
+    mw = np.array([[r[2], r[3]] for r in res]) * (1 + 1e-3 * rng.uniform(-1, 1, (len(res), 2)))
+    Mg.set_params(c, mw[None])
+    nll = Mg.nll()[0]
+    assert Mg.last_call_stats()["norm_path"] == 4
+    rn = Mo.nll(c, x, eff, xn, wn, mass_width=mw[None])[0][0]
+    assert abs(nll - rn) < RTOL_NLL * abs(rn)
+    P = 1 + 2 * 12
+    cs, mws = np.tile(c, (P, 1)), np.tile(mw, (P, 1, 1))
+    p = 1
+    for zr, k0 in ((10, 24), (11, 27)):                      # (resonance index, first slot) of the two Zs
+        for sgn in (+1, -1):
+            cs[p, k0] *= 1 + sgn * 1e-3; cs[p, k0 + 2] = cs[p, k0]; p += 1          # |H_-1| = |H_+1| (tied)
+            cs[p, k0 + 1] *= np.exp(sgn * 1e-3j); p += 1                              # arg H_0
+            mws[p, zr, 0] *= 1 + sgn * 1e-4; p += 1                                   # mass
+            mws[p, zr, 1] *= 1 + sgn * 1e-4; p += 1                                   # width
+            cs[p, 3] *= 1 + sgn * 1e-3; p += 1                                        # a K* coupling
+            mws[p, 1, 0] *= 1 + sgn * 1e-5; p += 1                                    # the K*(892) mass
+    assert p == P
+    Mg.set_params(cs, mws)
+    nll = Mg.nll()
+    assert Mg.last_call_stats()["norm_path"] == 5
+    rb, rI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+    assert np.max(np.abs(nll - rb) / np.abs(rb)) < RTOL_NLL
+    assert np.max(np.abs(Mg.norm_integral() - rI) / rI) < 1e-12
+
+
 def test_static_lineshapes_switch_to_the_matrix():
     """cfg 1 call pattern (masses and widths fixed, couplings move): the second call with unchanged lineshapes builds
     M once, later calls only evaluate c^H M c; a moved mass goes back to the direct sum."""
