@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         AMP_SPIN(3, 2, SH::n3, SH::o3, c * fma(2.5, c2, -1.5), -0.43301270189221932338 * s * fma(5.0, c2, -1.0))            // sqrt(3)/4
         AMP_SPIN(4, 3, SH::n4, SH::o4, fma(fma(4.375, c2, -3.75), c2, 0.375), -0.55901699437494742410 * s * c * fma(7.0, c2, -3.0))   // sqrt(5)/4
 #undef AMP_SPIN
-        if (SH::n0 < 0) {   // LASS S-wave terms (generic kernel only): J = 0, lambda = 0, lineshape of Eq. 7
+        if (SH::nl != 0) {   // LASS S-wave terms (shapes compiled with them): J = 0, lambda = 0, lineshape of Eq. 7
             for (int t = a.lass0; t < a.lass0 + a.nlass; ++t) {
 #pragma unroll
                 for (int e = 0; e < E; ++e) {
@@ -267,8 +267,12 @@ cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s) {
         return a.shape_fixed && n[0] == a0 && n[1] == a1 && n[2] == a2 && n[3] == a3 && n[4] == a4 && n[5] == az;
     };
     cudaError_t e;
-    if (a.nlass > 0) e = launch_shape<Generic>(a, grid, s);   // LASS terms live in the generic kernel
+    if (a.nlass > 0) {   // the paper's LASS variant: LASS + K0*(1950) in the S wave, the other eight K*, one Z
+        if (a.nlass == 1 && is(1, 3, 2, 1, 1, 1)) e = launch_shape<Shape<1, 3, 2, 1, 1, 1, 1>>(a, grid, s);
+        else e = launch_shape<Generic>(a, grid, s);
+    }
     else if (is(3, 3, 2, 1, 1, 1)) e = launch_shape<Shape<3, 3, 2, 1, 1, 1>>(a, grid, s);
+    else if (is(3, 3, 2, 1, 1, 2)) e = launch_shape<Shape<3, 3, 2, 1, 1, 2>>(a, grid, s);   // "ten K*s and two Zs"
     else if (is(3, 3, 2, 1, 1, 0)) e = launch_shape<Shape<3, 3, 2, 1, 1, 0>>(a, grid, s);
     else if (is(0, 1, 0, 0, 0, 0)) e = launch_shape<Shape<0, 1, 0, 0, 0, 0>>(a, grid, s);
     else e = launch_shape<Generic>(a, grid, s);

@@ -159,9 +159,10 @@ __device__ __forceinline__ void spin_sum(const StreamArgs& a, long long i0, cons
 }
 
 // Model shape: number of resonances of K* spin 0..4 and of Z's; Generic = runtime loops.
-template <int A0, int A1, int A2, int A3, int A4, int AZ>
+template <int A0, int A1, int A2, int A3, int A4, int AZ, int AL = 0>
 struct Shape {
     static constexpr int n0 = A0, n1 = A1, n2 = A2, n3 = A3, n4 = A4, nz = A4 < 0 ? -1 : AZ;
+    static constexpr int nl = A4 < 0 ? -1 : AL;   // LASS terms (Eq. 7): 0 = none compiled in, -1 = runtime count
     static constexpr int o1 = A0, o2 = A0 + A1, o3 = o2 + A2, o4 = o3 + A3, oz = o4 + A4;
 };
 using Generic = Shape<-1, -1, -1, -1, -1, -1>;
