@@ -154,6 +154,27 @@ class Model:
     def norm_integral(self, couplings, xn, wn, mass_width=None, prec=0):
         return self.nll(couplings, np.zeros((4, 0)), None, xn, wn, mass_width, prec, want_nll=False)[1]
 
+    def nll_background(self, couplings, x, eff, bkg, purity, xn, wn, mass_width=None):
+        """Eq. 14: NLL(p) = -sum_i log f_i, f_i = purity * eps_i S_i / I + (1 - purity) * b_i, with the signal
+        part normalised by the Monte Carlo integral I = sum_j w_j S_j / sum_j w_j and b_i the (normalised) background density
+        at the data events, supplied by the caller.  Plain definition, exact summation (math.fsum).  couplings [P][K] or [K]."""
+        import math
+        cc = np.asarray(couplings)
+        if cc.ndim == 1:
+            cc = cc[None]
+        bkg = _f64(bkg)
+        out = np.zeros(cc.shape[0])
+        for p in range(cc.shape[0]):
+            M = self
+            if mass_width is not None:
+                mw = np.asarray(mass_width, dtype=np.float64).reshape(cc.shape[0], self.R, 2)[p]
+                M = Model(self.decay, [(int(self.kinds[r]), int(self.Js[r]), mw[r, 0], mw[r, 1], self.radius[r]) for r in range(self.R)])
+            I = M.norm_integral(cc[p], xn, wn)[0]
+            v = M.eval_events(cc[p], x, eff)                       # eps_i S_i
+            f = purity * v / I + (1.0 - purity) * bkg
+            out[p] = -math.fsum(np.log(f)) if np.all(f > 0) else np.inf
+        return out
+
     def fit_fractions(self, couplings, xn, wn, mass_width=None, groups=None):
         """Eq. 13 by its plain definition: FF_j = sum_n w_n S_j(x_n) / sum_n w_n S(x_n), where S_j is the density
         with every helicity amplitude except those of resonance j set to zero ("setting to zero all the other helicity

@@ -465,6 +465,37 @@ def test_P14_lass_lineshape():
     assert abs(lass.lineshape(0, 1000.0, prec=1)[0] - A1000) < 1e-13 * abs(A1000)
 
 
+# ------------------------------------------------------------------ background and purity, Eq. 14
+def test_P15_background_and_purity():
+    """Eq. 14.  (i) purity 1 gives the signal-only NLL; (ii) a background with the signal's own shape,
+    b_i = eps_i S_i / I, gives the signal-only NLL at ANY purity (fixes where I divides and that p weights the normalised
+    signal); (iii) purity 0 gives -sum log b_i; (iv) f is linear in purity: exp(-NLL) per event interpolates — checked through
+    the single-event case; (v) the mixture is a normalised density: sum_j w_j f(x_j) / sum_j w_j = 1 on the MC sample when b is
+    normalised on it."""
+    cfg = 2
+    M = model(cfg)
+    c = W.couplings(cfg)
+    xn, wn = W.norm_events(cfg, 4000)
+    x, eff = W.data_events(cfg, lambda xx, ee: M.eval_events(c, xx, ee), n=300)
+    base, I = M.nll(c, x, eff, xn, wn)
+    rng = np.random.default_rng(4)
+    b = rng.uniform(0.2, 2.0, x.shape[1])
+    assert abs(M.nll_background(c, x, eff, b, 1.0, xn, wn)[0] - base[0]) < 1e-12 * abs(base[0])
+    b_sig = M.eval_events(c, x, eff) / I[0]
+    for p in (0.15, 0.85):
+        assert abs(M.nll_background(c, x, eff, b_sig, p, xn, wn)[0] - base[0]) < 1e-12 * abs(base[0])
+    assert abs(M.nll_background(c, x, eff, b, 0.0, xn, wn)[0] + np.sum(np.log(b))) < 1e-12 * abs(np.sum(np.log(b)))
+    x1, e1, b1 = x[:, :1], eff[:1], b[:1]
+    f = lambda p: math.exp(-M.nll_background(c, x1, e1, b1, p, xn, wn)[0])
+    assert abs(f(0.4) - (0.4 * f(1.0) + 0.6 * f(0.0))) < 1e-13 * f(0.4)
+    # normalisation of the mixture on the MC sample: signal part integrates to 1 (pin P12), background given normalised
+    bn = rng.uniform(0.5, 1.5, xn.shape[1])
+    bn /= np.sum(wn * bn / wn) / xn.shape[1]                        # mean of b over the (uniform phase-space) sample = 1
+    sig = M.eval_events(c, xn, None) / I[0]                         # S_j / I ; sum_j w_j S_j / I / sum w = 1
+    mix = 0.85 * np.sum(wn * sig) / np.sum(wn) + 0.15 * np.mean(bn)
+    assert abs(mix - 1.0) < 1e-12
+
+
 # ------------------------------------------------------------------ fit fractions, Eq. 13
 def test_P13_fit_fractions():
     """Eq. 13.  (i) a model with one resonance has FF = 1; (ii) on a full-angle quadrature grid with
