@@ -115,6 +115,14 @@ amp_status amp_set_params(amp_model* m, int P, const double* h_couplings, const 
  * finite and positive: h_nll[p] = +inf for those points, the others are valid.                         */
 amp_status amp_nll(amp_model* m, double* h_nll, void* stream);
 
+/* Background and signal purity, Eq. 14: with a background set, amp_nll returns
+ *   NLL(p) = - sum_i log( purity * eps_i S_i(p) / I(p) + (1 - purity) * b_i ).
+ *   d_bkg device [n]: the normalised background density b(Phi_i) >= 0 at the loaded data events (copied), or NULL to go back
+ *   to the signal-only likelihood; purity in [0, 1] (the paper uses 0.85).  Call after amp_load_events and before
+ *   amp_set_params (loading a new data set drops the background).  Such evaluations run one normalisation launch and one
+ *   data launch per point (path 6); amp_nll_terms is not defined for them (the sums no longer separate).             */
+amp_status amp_set_background(amp_model* m, const double* d_bkg, double purity, void* stream);
+
 /* The two sums behind amp_nll, for callers that shard the events over several devices or processes:
  *   h_sum_log[p] = sum_i log S_i(p) over the loaded data events (without the efficiency), h_sum_wS[p] = sum_j w_j S_j(p)
  * over the loaded normalisation events, host [P] each.  With the constants of amp_dataset_sums summed over the shards,
@@ -168,7 +176,7 @@ amp_status amp_set_batch_mode(amp_model* m, int mode);
 amp_status amp_set_fused_mode(amp_model* m, int mode);
 /* Counters of the last amp_nll / amp_norm_integral call: kernels launched, lineshape columns
  * recomputed (data + norm), which normalisation path ran (1 direct streaming sum, 2 matrix, 3 batched DMMA sum,
- * 4 fused single launch, 5 gradient-batch delta kernel).                         */
+ * 4 fused single launch, 5 gradient-batch delta kernel, 6 background + purity).                         */
 amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_recomputed, int* norm_path);
 
 /* Device time [ms] of the phases of the last amp_nll / amp_norm_integral call, from CUDA events recorded on

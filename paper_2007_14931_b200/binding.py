@@ -18,7 +18,7 @@ AMP_MAX_RESONANCES, AMP_MAX_COUPLINGS, AMP_MAX_POINTS = 16, 48, 256
 # every symbol include/amp.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
-    "amp_load_norm", "amp_set_params", "amp_nll", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
+    "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
     "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_fit_fractions", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode",
     "amp_last_call_stats", "amp_last_call_timing", "amp_recent_launch_ms", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
 ]
@@ -59,6 +59,7 @@ def lib():
         "amp_num_resonances": (i, [vp]),
         "amp_load_events": (i, [vp, vp, vp, ll, vp]),
         "amp_load_norm": (i, [vp, vp, vp, ll, vp]),
+        "amp_set_background": (i, [vp, vp, d, vp]),
         "amp_set_params": (i, [vp, i, vp, vp]),
         "amp_nll": (i, [vp, vp, vp]),
         "amp_nll_terms": (i, [vp, vp, vp, vp]),
@@ -154,6 +155,12 @@ class Model:
         self._check(lib().amp_load_norm(self._h, _dev_ptr(d_x, 4 * n), _dev_ptr(d_w, n if d_w is not None else None), n,
                                         _stream_ptr(stream)), "amp_load_norm")
         self.n_norm = n
+
+    def set_background(self, d_bkg, purity, stream=None):
+        """Eq. 14: background density at the data events (float64 CUDA tensor [n], or None to switch it off) and the purity"""
+        self._check(lib().amp_set_background(self._h, _dev_ptr(d_bkg, self.n) if d_bkg is not None else None, float(purity),
+                                             _stream_ptr(stream)), "amp_set_background")
+        self.P = 0
 
     # --- parameters ------------------------------------------------------------------------------
     def set_params(self, couplings, mass_width=None):

@@ -205,7 +205,8 @@ enum { MAX_LINE_JOBS = 64 };
 cudaError_t launch_lineshape(const Dataset& d, const LineshapeJob* jobs, int njobs, cudaStream_t s);
 
 // Streaming combine + reduce for one parameter point (a3 + a5, P = 1)
-enum StreamMode { MODE_DATA = 0, MODE_NORM = 1, MODE_EVAL = 2, MODE_FUSED = 3 };   // FUSED: data (sum log S) then norm (sum w S) in one launch + final NLL
+enum StreamMode { MODE_DATA = 0, MODE_NORM = 1, MODE_EVAL = 2, MODE_FUSED = 3, MODE_DATA_BKG = 4 };   // FUSED: data (sum log S) then norm (sum w S) in one launch + final NLL;
+                                                                                              // DATA_BKG: sum log(purity eps S / I + (1 - purity) b), Eq. 14
 // One resonance as the streaming kernel sees it: the three per-(mass,width) constants of LineConst,
 // its first coupling slot, and either a pool column to read or -1 = evaluate in registers.
 struct ResEntry {
@@ -260,6 +261,11 @@ struct StreamArgs {
     unsigned int* ticket;           // device counter, 0 between launches
     double* result;                 // [5]: NLL, I, domain flag, sum log S, sum w S
     double sum_log_eff, wsum;
+    // MODE_DATA_BKG (Eq. 14): background density at the data events, signal purity, and the device location of sum_j w_j S_j
+    // of this point (the normalisation pass runs first on the same stream)
+    const double* bkg;
+    const double* sum_wS;
+    double purity;
 };
 cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s);
 int stream_grid(long long n, bool have_z, int mode);

@@ -90,6 +90,9 @@ struct amp_model {
     bool use_delta = false;        // P > 1 and the points are sparse changes of point 0: gradient-batch kernel (delta.cu)
     struct DeltaChunk { int p0, np, nsorted; std::vector<DeltaContrib> contrib; std::vector<double> slots; };
     std::vector<DeltaChunk> delta_chunks;     // compiled program of the last amp_set_params (points p0 .. p0 + np - 1 per launch)
+    double* d_bkg = nullptr;       // [data.npad] background density b_i at the data events (Eq. 14), 1 on padding
+    double purity = 1.0;
+    bool has_bkg = false;
     int fused_mode = 0;            // 0: P == 1 steps with floating lineshapes run as one fused launch; 1: separate launches
     std::string err;
 };
@@ -167,6 +170,10 @@ bool make_line_const(const amp_model* m, int r, double mass, double width, LineC
     return true;
 }
 
+__global__ void k_fill(double* __restrict__ p, long long n, double v) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) p[i] = v;
+}
+
 void free_dataset(Dataset& d) {
     if (d.cache) cudaFree(d.cache);
     if (d.cols) cudaFree(d.cols);
@@ -179,6 +186,7 @@ amp_status load_dataset(amp_model* m, Dataset& d, bool is_norm, const double* d_
     free_dataset(d);
     for (auto& e : m->pool) (is_norm ? e.valid_norm : e.valid_data) = false;
     if (is_norm) m->gram_valid = false;
+    if (!is_norm) { if (m->d_bkg) cudaFree(m->d_bkg); m->d_bkg = nullptr; m->has_bkg = false; m->purity = 1.0; }   // belongs to the old data set
     d.n = n;
     d.npad = stream_pad(n > 0 ? n : 1);
     d.ncache = m->has_z ? NCOL_ALL : NCOL_K;
@@ -298,6 +306,7 @@ amp_status amp_model_destroy(amp_model* m) {
     if (m->d_result) cudaFree(m->d_result);
     if (m->d_flag) cudaFree(m->d_flag);
     if (m->d_ticket) cudaFree(m->d_ticket);
+    if (m->d_bkg) cudaFree(m->d_bkg);
     if (m->h_pinned) cudaFreeHost(m->h_pinned);
     if (m->d_plan) cudaFree(m->d_plan);
     if (m->h_plan) cudaFreeHost(m->h_plan);
@@ -324,6 +333,29 @@ amp_status amp_load_norm(amp_model* m, const double* d_x, const double* d_w, lon
     if (!m) return AMP_ERR_INVALID;
     if (n_norm < 1) return fail(m, AMP_ERR_INVALID, "amp_load_norm: need at least one normalisation event");
     return load_dataset(m, m->norm, true, d_x, d_w, n_norm, (cudaStream_t)stream);
+}
+
+amp_status amp_set_background(amp_model* m, const double* d_bkg, double purity, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!d_bkg) {   // back to the signal-only likelihood
+        if (m->d_bkg) cudaFree(m->d_bkg);
+        m->d_bkg = nullptr; m->has_bkg = false; m->purity = 1.0; m->P = 0;
+        return AMP_OK;
+    }
+    if (!m->data.loaded) return fail(m, AMP_ERR_STATE, "amp_set_background: load the data events first");
+    if (!(purity >= 0.0 && purity <= 1.0)) return fail(m, AMP_ERR_INVALID, "amp_set_background: purity must be in [0, 1]");
+    if (m->d_bkg) cudaFree(m->d_bkg);
+    m->d_bkg = nullptr;
+    CK(cudaMalloc(&m->d_bkg, sizeof(double) * m->data.npad));
+    k_fill<<<148 * 4, 256, 0, s>>>(m->d_bkg, m->data.npad, 1.0);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(m->d_bkg, d_bkg, sizeof(double) * m->data.n, cudaMemcpyDeviceToDevice, s));
+    CK(cudaStreamSynchronize(s));
+    m->purity = purity;
+    m->has_bkg = true;
+    m->P = 0;   // parameters must be set again: the evaluation plan depends on the background
+    return AMP_OK;
 }
 
 amp_status amp_set_norm_mode(amp_model* m, int mode) {
@@ -571,9 +603,10 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
     m->want_matrix = m->norm_mode == 2 || (m->norm_mode == 0 && (P == 1 ? mw_same : (P >= 24 && m->batch_mode != 1)));
     if (P == 1) m->prev_mw = m->mw; else m->prev_mw.clear();
     // P > 1: a batch whose points are sparse changes of point 0 (a gradient step) runs the delta kernel: no column, no matrix
-    m->use_delta = P > 1 && m->batch_mode == 0 && m->lineshape_mode != 1 && m->norm_mode != 2 && build_delta_plan(m);
+    if (m->has_bkg) m->want_matrix = false;   // Eq. 14: the background path streams both samples, point by point
+    m->use_delta = P > 1 && !m->has_bkg && m->batch_mode == 0 && m->lineshape_mode != 1 && m->norm_mode != 2 && build_delta_plan(m);
     if (m->use_delta) m->want_matrix = false;
-    m->stream_inline = (P == 1 || m->use_delta) && m->lineshape_mode != 1;
+    m->stream_inline = (P == 1 || m->use_delta || m->has_bkg) && m->lineshape_mode != 1;
 
     // distinct (resonance, mass, width) keys of this call
     struct Key { int r; double mass, width; };
@@ -771,7 +804,11 @@ __global__ void k_nll_final(const double* __restrict__ sums, int P, double n_dat
     if (p >= P) return;
     const double I = sums[P + p] / wsum;
     result[P + p] = I;
-    if (want_nll) {
+    if (want_nll == 2) {          // Eq. 14: sums[p] = sum_i log f_i already holds efficiency, integral and background
+        double v = -sums[p];
+        if (!isfinite(v) || !(I > 0.0)) v = INFINITY;
+        result[p] = v;
+    } else if (want_nll) {
         double v = -(sums[p] + sum_log_eff) + n_data * log(I);
         if (!isfinite(v) || !(I > 0.0)) v = INFINITY;
         result[p] = v;
@@ -1131,6 +1168,49 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
     amp_status st = ensure_pool(m, 0);
     if (st != AMP_OK) return st;
     m->ev_valid = false;
+    if (m->has_bkg && want_nll) {
+        // Eq. 14: f_i = purity eps_i S_i / I + (1 - purity) b_i needs I before the data pass: per point one
+        // normalisation launch, a fixed-order reduction to sum_j w_j S_j on the device, then the data launch that reads it.
+        if (!m->stream_inline) {
+            st = refresh_columns(m, m->data, false, s); if (st != AMP_OK) return st;
+            st = refresh_columns(m, m->norm, true, s); if (st != AMP_OK) return st;
+        }
+        CK(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
+        const int gd = stream_grid(m->data.n, m->has_z, MODE_DATA), gn = stream_grid(m->norm.n, m->has_z, MODE_NORM);
+        StreamArgs a;
+        for (int p = 0; p < P; ++p) {
+            fill_stream_args(m, m->norm, p, MODE_NORM, &a);
+            a.partial = m->d_partial + (size_t)(P + p) * PARTIAL_STRIDE;
+            CK(launch_stream(a, gn, s));
+        }
+        CK(launch_finalize(m->d_partial + (size_t)P * PARTIAL_STRIDE, gn, PARTIAL_STRIDE, P, m->d_sums + P, s));
+        for (int p = 0; p < P; ++p) {
+            if (m->data.n == 0) { CK(cudaMemsetAsync(m->d_partial + (size_t)p * PARTIAL_STRIDE, 0, sizeof(double), s)); continue; }
+            fill_stream_args(m, m->data, p, MODE_DATA_BKG, &a);
+            a.partial = m->d_partial + (size_t)p * PARTIAL_STRIDE;
+            a.bkg = m->d_bkg; a.purity = m->purity; a.sum_wS = m->d_sums + P + p; a.wsum = m->norm.wsum;
+            CK(launch_stream(a, gd, s));
+        }
+        CK(launch_finalize(m->d_partial, m->data.n > 0 ? gd : 1, PARTIAL_STRIDE, P, m->d_sums, s));
+        k_nll_final<<<(P + 127) / 128, 128, 0, s>>>(m->d_sums, P, (double)m->data.n, 0.0, m->norm.wsum, 2, m->d_result);
+        CK(cudaGetLastError());
+        m->stat_launches = 2 * P + 3;
+        m->stat_norm_path = 6;
+        m->fused_valid = false;
+        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 2 * P, cudaMemcpyDeviceToHost, s));
+        CK(cudaMemcpyAsync(m->h_pinned + 2 * P, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));
+        int flag;
+        std::memcpy(&flag, m->h_pinned + 2 * P, sizeof(int));
+        bool bad = flag != 0;
+        for (int p = 0; p < P; ++p) {
+            h_nll[p] = m->h_pinned[p]; bad |= !std::isfinite(h_nll[p]);
+            if (h_I) h_I[p] = m->h_pinned[P + p];
+        }
+        m->last_slog.assign(P, 0.0); m->last_swS.assign(P, 0.0);
+        if (bad) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
+        return AMP_OK;
+    }
     if (m->use_delta) {
         // Gradient batch: one fused launch per chunk of <= 128 points besides point 0 (delta.cu)
         int ent_of_res[AMP_MAX_RESONANCES], grp_of_res[AMP_MAX_RESONANCES];

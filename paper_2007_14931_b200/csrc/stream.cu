@@ -34,7 +34,9 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     // sum w S (normalisation tiles) lives in `acc`; sum log S (data tiles) as a running product of mantissas in `acc` and a
     // sum of exponents in `accE` (split_exp: integer ops + one multiply per event instead of a ~35-instruction FP64 log)
     const double LN2 = 0.69314718055994530942;
-    double acc = (MODE == MODE_DATA || MODE == MODE_FUSED) ? 1.0 : 0.0;
+    double acc = (MODE == MODE_DATA || MODE == MODE_FUSED || MODE == MODE_DATA_BKG) ? 1.0 : 0.0;
+    // Eq. 14: f = (purity / I) eps S + (1 - purity) b, I = sum_wS / wsum from the normalisation pass that ran before
+    const double bkg_ps = MODE == MODE_DATA_BKG ? a.purity * a.wsum / __ldg(a.sum_wS) : 0.0, bkg_qb = 1.0 - a.purity;
     int accE = 0;
     bool bad = false;
     // One staged tile per CTA, split in two regions with their own mbarrier: the K*-chain columns (+ weight) are
@@ -159,7 +161,15 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         for (int e = 0; e < E; ++e) {
             const double S = fma(Ap[e].x, Ap[e].x, fma(Ap[e].y, Ap[e].y, fma(Am[e].x, Am[e].x, Am[e].y * Am[e].y)));
             const bool live = i0 + e < nlive;   // the last thread may hold padding events (weight 0)
-            if (MODE == MODE_DATA || (MODE == MODE_FUSED && !is_norm)) {
+            if (MODE == MODE_DATA_BKG) {
+                const double f0 = fma(bkg_ps * w.v[e], S, bkg_qb * (live ? a.bkg[i0 + e] : 1.0));
+                const bool ok = f0 > 0.0 && isfinite(f0);
+                bad |= live && !ok;
+                double f; int x;
+                split_exp((live && ok) ? f0 : 1.0, &f, &x);
+                acc *= f;
+                accE += x;
+            } else if (MODE == MODE_DATA || (MODE == MODE_FUSED && !is_norm)) {
                 const bool ok = S > 0.0 && isfinite(S);
                 bad |= live && !ok;
                 double f; int x;
@@ -172,7 +182,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
                 if (live) a.out[i0 + e] = w.v[e] * S;
             }
         }
-        if (MODE == MODE_DATA || (MODE == MODE_FUSED && !is_norm)) {   // running product back to [0.5, 1) once per tile
+        if (MODE == MODE_DATA || MODE == MODE_DATA_BKG || (MODE == MODE_FUSED && !is_norm)) {   // running product back to [0.5, 1) once per tile
             int x;
             split_exp(acc, &acc, &x);
             accE += x;
@@ -181,7 +191,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     if (MODE == MODE_EVAL) return;
     if (bad) atomicOr(a.flag, 2);
     {
-        const bool logs = MODE == MODE_DATA || (MODE == MODE_FUSED && !in_norm);
+        const bool logs = MODE == MODE_DATA || MODE == MODE_DATA_BKG || (MODE == MODE_FUSED && !in_norm);
         const double t = block_sum(logs ? log(acc) + (double)accE * LN2 : acc, sm);
         if (threadIdx.x == 0) {
             if (MODE == MODE_FUSED && !in_norm) { a.partial[blockIdx.x] = t; a.partial2[blockIdx.x] = 0.0; }   // this CTA saw data tiles only
@@ -252,6 +262,7 @@ static cudaError_t launch_shape(const StreamArgs& a, int grid, cudaStream_t s) {
         case MODE_DATA: AMP_LAUNCH(MODE_DATA) break;
         case MODE_NORM: AMP_LAUNCH(MODE_NORM) break;
         case MODE_FUSED: AMP_LAUNCH(MODE_FUSED) break;
+        case MODE_DATA_BKG: AMP_LAUNCH(MODE_DATA_BKG) break;
         default: AMP_LAUNCH(MODE_EVAL) break;
     }
 #undef AMP_LAUNCH

@@ -427,6 +427,42 @@ def test_lass_model_matches_oracle(with_z):
     assert np.max(np.abs(nll - rb) / np.abs(rb)) < RTOL_NLL
 
 
+def test_background_and_purity_match_oracle():
+    """Eq. 14: NLL with a per-event background density and a purity against the oracle's plain definition — one point with
+    all lineshapes moved, a batch of points, purity 1 (= signal only) and switching the background off again."""
+    cfg = 2
+    Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+    c = W.couplings(cfg)
+    x, eff, xn, wn = make_inputs(cfg, 7001, 20011)
+    rng = np.random.default_rng(8)
+    # a smooth seeded background shape at the data events, a few 1e-10 like eps S / I (any positive numbers are valid inputs)
+    I0 = Mo.norm_integral(c, xn, wn)[0]
+    bkg = np.mean(Mo.eval_events(c, x, eff)) / I0 * (1.0 + 0.5 * x[1]) * (1.0 + 0.3 * np.cos(x[3])) * rng.uniform(0.8, 1.2, x.shape[1])
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    Mg.set_params(c)
+    base = Mg.nll()[0]
+    Mg.set_background(dev(bkg), 0.85)
+    mw = W.step_mass_width(3, 4)
+    Mg.set_params(c, mw[None])
+    nll = Mg.nll()[0]
+    assert Mg.last_call_stats()["norm_path"] == 6
+    ref = Mo.nll_background(c, x, eff, bkg, 0.85, xn, wn, mass_width=mw[None])[0]
+    assert abs(nll - ref) < RTOL_NLL * abs(ref), (nll, ref)
+    assert Mg.nll()[0] == nll
+    cs, mws = W.fit_points(4)
+    Mg.set_params(cs[:9], mws[:9])
+    nb = Mg.nll()
+    rb = Mo.nll_background(cs[:9], x, eff, bkg, 0.85, xn, wn, mass_width=mws[:9])
+    assert np.max(np.abs(nb - rb) / np.abs(rb)) < RTOL_NLL
+    Mg.set_background(dev(bkg), 1.0)                       # purity 1: the background drops out
+    Mg.set_params(c)
+    assert abs(Mg.nll()[0] - base) < 1e-12 * abs(base)
+    Mg.set_background(None, 1.0)
+    Mg.set_params(c)
+    assert abs(Mg.nll()[0] - base) < 1e-12 * abs(base) and Mg.last_call_stats()["norm_path"] in (2, 4)   # signal-only paths again
+
+
 def test_two_z_model_matches_oracle():
     """SURVEY.md 8(f)-3 / PAPER.md:165, 191 ("ten K*s and two Zs"): a second 1+ exotic, Z(4430) (m = 4478, Gamma = 181 MeV), shares
     the Z(4200)'s decay frame and angular cache; K = 30.  Per-event density, fused NLL with all 12 lineshapes moving, and a
