@@ -18,13 +18,15 @@
 // the warp's 64 events.  Data side: S = f 2^e is split with integer ops, mantissas are multiplied and exponents
 // added, so the sum of logs takes ONE log per (point, warp) at the very end instead of one per (point, event).
 // Everything is fixed-order: bit-reproducible.  Bound: plain FP64 ALUs.
-// Two events per thread x 256 threads (as k_stream).  Measured alternative: one event per thread x 512 threads (16 warps,
-// 128 registers) hides latency better but pays the warp-uniform per-point overhead twice: 6.20 ms vs 6.12 ms on configs[4].
+// One event per thread x 512 threads (16 warps per SM, 128 registers): the point loop is chains of short dependent FP64
+// sequences and the extra warps hide their latency.  Measured on configs[4] (with the four-point blocks): 5.55 ms, against
+// 5.74 ms for two events per thread x 256 threads (8 warps, 229 registers), which pays the warp-uniform per-point overhead once
+// for two events but stalls more.
 #ifndef AMP_DELTA_E
-#define AMP_DELTA_E 2
+#define AMP_DELTA_E 1
 #endif
 #ifndef AMP_DELTA_THREADS
-#define AMP_DELTA_THREADS 256
+#define AMP_DELTA_THREADS 512
 #endif
 #define AMP_STREAM_E AMP_DELTA_E
 #define AMP_STREAM_THREADS AMP_DELTA_THREADS
