@@ -190,6 +190,9 @@ def run_own(args):
     h2d = sum(a.nbytes for a in (np.zeros((P, model.K, 2)), np.zeros((P, model.R, 2))))
     d2h = 8 * P
 
+    if args.dense:
+        model.set_batch_mode(2)   # configs[4] as the dense DMMA contraction + extended-basis normalisation matrix
+
     def one_step(s):
         cs, mws = params[s]
         model.set_params(cs, mws)
@@ -252,7 +255,14 @@ def run_own(args):
                 "flop_per_event": DELTA_FLOP_PER_EVENT, "flop_per_launch": flop,
                 "hbm_frac": (BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}
     elif args.cfg == 4:
-        roof = None
+        # dense form (--dense): k_batch (data, DMMA contraction) + k_herk (normalisation matrix, DMMA) + k_lineshape
+        tm = model.last_call_timing()
+        flop = 2 * 27 * 8 * 121 * args.n_data     # two helicities x 27 complex multiply-adds x 121 points per data event
+        ach = flop / (tm["data_ms"] * 1e-3) / 1e12
+        roof = {"bound": "tensor", "kernel": "k_batch<14, MODE_DATA> (dense FP64 DMMA contraction points x events, mma.sync.m8n8k4.f64)",
+                "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12, "peak_source": "FP64 tensor peak = FP64 FMA peak on B200, 148 x 64 x 2 x 1.965 GHz "
+                "(the DMMA probe below measures it)", "unit": "TFLOP/s", "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": None,
+                "kernel_ms": tm["data_ms"], "flop_per_launch": flop, "norm_matrix_ms": tm["norm_ms"], "lineshape_ms": tm["lineshape_ms"]}
     elif paths == {4}:
         # one fused launch per step: lineshapes + combine + both reductions over the data tiles then the norm tiles
         k_ms = float(np.mean(t_data))
@@ -375,6 +385,7 @@ def main():
     ap.add_argument("--n-data", type=int, default=2_000_000)
     ap.add_argument("--n-norm", type=int, default=10_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dense", action="store_true", help="--cfg 4 through the dense DMMA contraction instead of the gradient-batch kernel")
     ap.add_argument("--lass", action="store_true", help="configs[3] call pattern on the LASS variant of the model (Eqs. 7-9; SURVEY.md 8(f)-1)")
     args = ap.parse_args()
     global LASS
