@@ -259,7 +259,8 @@ struct StreamArgs {
     long long n2, npad2;
     double* partial2;               // [grid] sum w S
     unsigned int* ticket;           // device counter, 0 between launches
-    double* result;                 // [5]: NLL, I, domain flag, sum log S, sum w S
+    double* result;                 // [6]: NLL, I, domain flag, sum log S, sum w S, sequence stamp; may be mapped HOST memory
+    double seq;                     // written to result[5] after a system-wide fence once the other five are in place
     double sum_log_eff, wsum;
     // MODE_DATA_BKG (Eq. 14): background density at the data events, signal purity, and the device location of sum_j w_j S_j
     // of this point (the normalisation pass runs first on the same stream)

@@ -2,6 +2,8 @@
 // pool (which columns are already held, which must be recomputed), the choice of normalisation path and
 // the launch sequence of one NLL evaluation.  All per-event arithmetic is in the kernels.
 #include <algorithm>
+#include <atomic>
+#include <cstdlib>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -54,6 +56,9 @@ struct amp_model {
     int* d_flag = nullptr;
     unsigned int* d_ticket = nullptr;   // last-CTA ticket of the fused single-launch step (0 between launches)
     double* h_pinned = nullptr;    // same layout
+    double* h_zc = nullptr;        // [8] mapped pinned host memory: the fused step's kernel writes its result block here (zero copy)
+    double zc_seq = 0;             // stamp of the last fused launch
+    bool zero_copy = true;
     std::vector<double> last_slog, last_swS;   // the two sums of the last amp_nll, per point (amp_nll_terms)
 
     // batched (P > 1) plan buffers: coefficient fragments, basis entries, sparse items
@@ -290,6 +295,8 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
     if (e == cudaSuccess) e = cudaMemset(m->d_ticket, 0, sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(m->d_flag, 0, sizeof(int));
     if (e == cudaSuccess) e = cudaMallocHost(&m->h_pinned, sizeof(double) * (4 * AMP_MAX_POINTS + 4));
+    if (e == cudaSuccess) e = cudaHostAlloc(&m->h_zc, sizeof(double) * 8, cudaHostAllocMapped);
+    if (e == cudaSuccess) { std::memset(m->h_zc, 0, sizeof(double) * 8); m->zero_copy = std::getenv("AMP4D_NO_ZERO_COPY") == nullptr; }
     for (int i = 0; i < 5 && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ev[i]);
     for (int i = 0; i < 2 * amp_model::RING && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ring[i]);
     if (e != cudaSuccess) { amp_model_destroy(m); return e == cudaErrorMemoryAllocation ? AMP_ERR_NOMEM : AMP_ERR_CUDA; }
@@ -308,6 +315,7 @@ amp_status amp_model_destroy(amp_model* m) {
     if (m->d_ticket) cudaFree(m->d_ticket);
     if (m->d_bkg) cudaFree(m->d_bkg);
     if (m->h_pinned) cudaFreeHost(m->h_pinned);
+    if (m->h_zc) cudaFreeHost(m->h_zc);
     if (m->d_plan) cudaFree(m->d_plan);
     if (m->h_plan) cudaFreeHost(m->h_plan);
     if (m->d_G) cudaFree(m->d_G);
@@ -394,6 +402,7 @@ amp_status amp_last_call_timing(const amp_model* m, double* ms4) {
     if (!m || !ms4) return AMP_ERR_INVALID;
     if (m->fused_valid) {   // one launch: everything is reported as the combine phase of both samples
         float t = 0;
+        cudaEventSynchronize(m->ring[2 * m->ring_last + 1]);   // (a zero-copy call returns before its end event has landed)
         if (cudaEventElapsedTime(&t, m->ring[2 * m->ring_last], m->ring[2 * m->ring_last + 1]) != cudaSuccess) return AMP_ERR_CUDA;
         ms4[0] = 0; ms4[1] = t; ms4[2] = 0; ms4[3] = 0;
         return AMP_OK;
@@ -414,6 +423,7 @@ amp_status amp_recent_launch_ms(const amp_model* m, int max_calls, double* h_ms,
     for (int i = 0; i < n; ++i) {   // oldest of the n first
         const int slot = ((m->ring_last - (n - 1 - i)) % amp_model::RING + amp_model::RING) % amp_model::RING;
         float t = 0;
+        cudaEventSynchronize(m->ring[2 * slot + 1]);
         if (cudaEventElapsedTime(&t, m->ring[2 * slot], m->ring[2 * slot + 1]) != cudaSuccess) return AMP_ERR_CUDA;
         h_ms[i] = t;
     }
@@ -1291,24 +1301,46 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         a.partial2 = m->d_partial + PARTIAL_STRIDE;
         a.cache2 = m->norm.cache; a.n2 = m->norm.n; a.npad2 = m->norm.npad;
         a.ticket = m->d_ticket;
-        a.result = m->d_result;
         a.sum_log_eff = m->data.wsum;
         a.wsum = m->norm.wsum;
+        // Result block: by default mapped host memory (UVA: same pointer on the device) that the last CTA fills and stamps;
+        // the host spins on the stamp, which saves the D2H copy and the stream-synchronise wake-up of a synchronous call.
+        double* res = m->h_pinned;
+        if (m->zero_copy) {
+            m->zc_seq += 1.0;
+            a.result = m->h_zc;
+            a.seq = m->zc_seq;
+            res = m->h_zc;
+        } else {
+            a.result = m->d_result;
+            a.seq = 0.0;
+        }
         m->ring_last = (m->ring_last + 1) % amp_model::RING;
         m->ring_calls++;
         CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
         CK(launch_stream(a, stream_grid_fused(m->data.n, m->norm.n, m->has_z), s));
         CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
-        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 5, cudaMemcpyDeviceToHost, s));
-        CK(cudaStreamSynchronize(s));
-        m->last_slog.assign(1, m->h_pinned[3]);
-        m->last_swS.assign(1, m->h_pinned[4]);
+        if (m->zero_copy) {
+            volatile double* stamp = m->h_zc + 5;
+            for (unsigned spins = 0; *stamp != m->zc_seq; ++spins) {
+                if ((spins & 0x3fff) == 0x3fff) {   // every 16k spins: has the stream failed or finished without the stamp?
+                    const cudaError_t q = cudaStreamQuery(s);
+                    if (q != cudaErrorNotReady) { if (q != cudaSuccess) return cuda_fail(m, q, "fused step"); if (*stamp == m->zc_seq) break; return fail(m, AMP_ERR_CUDA, "fused step finished without a result"); }
+                }
+            }
+            std::atomic_thread_fence(std::memory_order_acquire);
+        } else {
+            CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 5, cudaMemcpyDeviceToHost, s));
+            CK(cudaStreamSynchronize(s));
+        }
+        m->last_slog.assign(1, res[3]);
+        m->last_swS.assign(1, res[4]);
         m->stat_launches = 1;
         m->stat_norm_path = 4;
         m->fused_valid = true;
-        h_nll[0] = m->h_pinned[0];
-        if (h_I) h_I[0] = m->h_pinned[1];
-        if (m->h_pinned[2] != 0.0 || !std::isfinite(h_nll[0])) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
+        h_nll[0] = res[0];
+        if (h_I) h_I[0] = res[1];
+        if (res[2] != 0.0 || !std::isfinite(h_nll[0])) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
         return AMP_OK;
     }
     m->fused_valid = false;

@@ -221,6 +221,9 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         a.result[4] = swS;
         a.result[2] = (double)atomicExch(a.flag, 0);   // domain flag of this call, cleared for the next one
         *a.ticket = 0u;
+        // the result block may live in mapped host memory: the host spins on the stamp instead of paying a copy + stream sync
+        __threadfence_system();
+        *reinterpret_cast<volatile double*>(a.result + 5) = a.seq;
     }
 }
 
