@@ -464,6 +464,44 @@ int nll_impl(const double* decay, int n_res, const int* kinds, const int* Js, co
     return 0;
 }
 
+// Gradient of the NLL with respect to the complex couplings (the derivative of O9 written out).
+// With A_xi = sum_k c_k B_k,xi and S = sum_xi |A_xi|^2:  dS/dconj(c_k) = sum_xi conj(B_k,xi) A_xi, so
+//   dNLL/dconj(c_k) = - sum_i [sum_xi conj(B_k,xi(i)) A_xi(i)] / S_i  +  N [sum_j w_j sum_xi conj(B_k,xi(j)) A_xi(j)] / [sum_j w_j S_j]
+// and for the real parameters dNLL/dRe(c_k) = 2 Re(.), dNLL/dIm(c_k) = 2 Im(.).  grad_out is [K][2] = (d/dRe, d/dIm).
+template <typename T>
+void nll_gradient_impl(const Model<T>& M, const std::complex<T>* c, const double* x, const double* eff, long long n, const double* xn,
+                       const double* wn, long long mn, double* nll_out, double* grad_out) {
+    using C = std::complex<T>;
+    const int K = M.num_couplings();
+    std::vector<C> B(2 * K), D(K, C(0, 0)), Nk(K, C(0, 0));
+    Neumaier<T> slog, swS, sw;
+    for (long long i = 0; i < n; ++i) {
+        const T xi[4] = {T(x[i]), T(x[n + i]), T(x[2 * n + i]), T(x[3 * n + i])};
+        basis_terms(M, xi, B.data());
+        C A[2] = {C(0, 0), C(0, 0)};
+        for (int k = 0; k < K; ++k) { A[0] += c[k] * B[2 * k]; A[1] += c[k] * B[2 * k + 1]; }
+        const T S = std::norm(A[0]) + std::norm(A[1]);
+        slog.add(std::log((eff ? T(eff[i]) : T(1)) * S));
+        for (int k = 0; k < K; ++k) D[k] += (std::conj(B[2 * k]) * A[0] + std::conj(B[2 * k + 1]) * A[1]) / S;
+    }
+    for (long long j = 0; j < mn; ++j) {
+        const T xj[4] = {T(xn[j]), T(xn[mn + j]), T(xn[2 * mn + j]), T(xn[3 * mn + j])};
+        basis_terms(M, xj, B.data());
+        C A[2] = {C(0, 0), C(0, 0)};
+        for (int k = 0; k < K; ++k) { A[0] += c[k] * B[2 * k]; A[1] += c[k] * B[2 * k + 1]; }
+        const T w = wn ? T(wn[j]) : T(1);
+        swS.add(w * (std::norm(A[0]) + std::norm(A[1])));
+        sw.add(w);
+        for (int k = 0; k < K; ++k) Nk[k] += w * (std::conj(B[2 * k]) * A[0] + std::conj(B[2 * k + 1]) * A[1]);
+    }
+    *nll_out = double(-(slog.value() - T(n) * std::log(swS.value() / sw.value())));
+    for (int k = 0; k < K; ++k) {
+        const C g = -D[k] + T(n) * Nk[k] / swS.value();
+        grad_out[2 * k] = double(2 * g.real());
+        grad_out[2 * k + 1] = double(2 * g.imag());
+    }
+}
+
 // Hermitian normalisation matrix M_kl = sum_j w_j sum_xi conj(B_k xi) B_l xi / sum_j w_j (pin P10,
 // fit fractions Eq. 13).  out is [K][K][2] row-major.
 template <typename T>
@@ -599,6 +637,14 @@ int orc_nll(const double* decay, int n_res, const int* kinds, const int* Js, con
             long long n, const double* xn, const double* wn, long long mn, int prec, double* nll_out, double* integral_out) {
     if (prec) return nll_impl<long double>(decay, n_res, kinds, Js, mass, width, radius, P, couplings, mass_width, x, eff, n, xn, wn, mn, nll_out, integral_out);
     return nll_impl<double>(decay, n_res, kinds, Js, mass, width, radius, P, couplings, mass_width, x, eff, n, xn, wn, mn, nll_out, integral_out);
+}
+
+void orc_nll_gradient(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass, const double* width,
+                      const double* radius, const double* couplings, const double* x, const double* eff, long long n, const double* xn,
+                      const double* wn, long long mn, double* nll_out, double* grad_out) {
+    auto M = make_model<double>(decay, n_res, kinds, Js, mass, width, radius);
+    auto c = make_couplings<double>(couplings, M.num_couplings());
+    nll_gradient_impl(M, c.data(), x, eff, n, xn, wn, mn, nll_out, grad_out);
 }
 
 void orc_norm_matrix(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass, const double* width,

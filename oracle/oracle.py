@@ -36,6 +36,7 @@ _lib.orc_eval_events.argtypes = _MODEL + [_pd, _pd, _vp, _ll, _i, _pd]
 _lib.orc_nll.restype = _i
 _lib.orc_nll.argtypes = _MODEL + [_i, _pd, _vp, _pd, _vp, _ll, _pd, _vp, _ll, _i, _vp, _vp]
 _lib.orc_norm_matrix.argtypes = _MODEL + [_pd, _vp, _ll, _pd]
+_lib.orc_nll_gradient.argtypes = _MODEL + [_pd, _pd, _vp, _ll, _pd, _vp, _ll, _pd, _pd]
 
 KSTAR, ZRES, CONST, LASS = 0, 1, 2, 3
 
@@ -153,6 +154,17 @@ class Model:
 
     def norm_integral(self, couplings, xn, wn, mass_width=None, prec=0):
         return self.nll(couplings, np.zeros((4, 0)), None, xn, wn, mass_width, prec, want_nll=False)[1]
+
+    def nll_gradient(self, couplings, x, eff, xn, wn):
+        """(NLL, grad [K][2]) with grad[k] = (dNLL/dRe c_k, dNLL/dIm c_k): the derivative of the NLL written out event by event."""
+        c = _f64(np.stack([np.real(couplings), np.imag(couplings)], -1))
+        assert c.shape == (self.K, 2)
+        x, xn = _f64(x), _f64(xn)
+        ke, pe = _opt(eff)
+        kw, pw = _opt(wn)
+        nll, grad = np.zeros(1), np.zeros((self.K, 2))
+        _lib.orc_nll_gradient(*self._args(), c, x, pe, x.shape[1], xn, pw, xn.shape[1], nll, grad)
+        return nll[0], grad
 
     def nll_background(self, couplings, x, eff, bkg, purity, xn, wn, mass_width=None):
         """Eq. 14: NLL(p) = -sum_i log f_i, f_i = purity * eps_i S_i / I + (1 - purity) * b_i, with the signal

@@ -465,6 +465,32 @@ def test_P14_lass_lineshape():
     assert abs(lass.lineshape(0, 1000.0, prec=1)[0] - A1000) < 1e-13 * abs(A1000)
 
 
+# ------------------------------------------------------------------ gradient of the NLL in the couplings
+def test_P16_nll_gradient():
+    """(i) central finite differences of the oracle's own NLL (an independent route: no derivative formula involved);
+    (ii) Euler identities from pin P11: the NLL is invariant under c -> s c for any complex s, so
+    sum_k conj(c_k) dNLL/dconj(c_k) = 0 exactly (real part: scale, imaginary part: global phase);
+    (iii) at fixed normalisation events, the data term alone is homogeneous of degree -... checked through (ii) with n_norm >> n."""
+    cfg = 2
+    M = model(cfg)
+    c = W.couplings(cfg)
+    xn, wn = W.norm_events(cfg, 3000)
+    x, eff = W.data_events(cfg, lambda xx, ee: M.eval_events(c, xx, ee), n=400)
+    nll, g = M.nll_gradient(c, x, eff, xn, wn)
+    assert abs(nll - M.nll(c, x, eff, xn, wn)[0][0]) < 1e-12 * abs(nll)
+    gc = 0.5 * (g[:, 0] + 1j * g[:, 1])                       # dNLL/dconj(c_k)
+    euler = np.sum(np.conj(c) * gc)
+    assert abs(euler) < 1e-10 * np.sum(np.abs(c) * np.abs(gc))
+    for k in (0, 4, 11, 24, 26):                              # J = 0 slot, K*(892) lambda = 0, a J = 2 slot, Z lambda' = -1, +1
+        for part, d in ((0, 1.0), (1, 1j)):
+            h = 1e-4 * max(abs(c[k]), 1.0)        # NLL ~ 1e4 to 1e-16 relative: rounding 1e-8, truncation O(h^2)
+            cp, cm = c.copy(), c.copy()
+            cp[k] += h * d
+            cm[k] -= h * d
+            fd = (M.nll(cp, x, eff, xn, wn)[0][0] - M.nll(cm, x, eff, xn, wn)[0][0]) / (2 * h)
+            assert abs(fd - g[k, part]) < 1e-6 * np.abs(g).max(), (k, part, fd, g[k, part])
+
+
 # ------------------------------------------------------------------ background and purity, Eq. 14
 def test_P15_background_and_purity():
     """Eq. 14.  (i) purity 1 gives the signal-only NLL; (ii) a background with the signal's own shape,
