@@ -115,6 +115,15 @@ amp_status amp_set_params(amp_model* m, int P, const double* h_couplings, const 
  * finite and positive: h_nll[p] = +inf for those points, the others are valid.                         */
 amp_status amp_nll(amp_model* m, double* h_nll, void* stream);
 
+/* NLL and its analytic gradient in the couplings at the single point of the last amp_set_params (P = 1), in ONE pass over
+ * the data and normalisation events (one launch):
+ *   h_nll host [1]; h_grad host [K][2] = (dNLL/dRe H_k, dNLL/dIm H_k) in slot order, from
+ *   dNLL/dconj(H_k) = - sum_i [sum_xi conj(B_k,xi) A_xi]_i / S_i + N [sum_j w_j sum_xi conj(B_k,xi) A_xi]_j / [sum_j w_j S_j].
+ * Replaces the 2 K finite-difference points a minimiser would spend on the couplings (masses and widths still go through
+ * a gradient batch).  Constraints such as Eq. 6 / Eq. 11 are the caller's chain rule.  Not available with a background or
+ * for models with a LASS term (AMP_ERR_STATE).  Deterministic.  Path 7 in amp_last_call_stats.                       */
+amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* stream);
+
 /* Background and signal purity, Eq. 14: with a background set, amp_nll returns
  *   NLL(p) = - sum_i log( purity * eps_i S_i(p) / I(p) + (1 - purity) * b_i ).
  *   d_bkg device [n]: the normalised background density b(Phi_i) >= 0 at the loaded data events (copied), or NULL to go back
@@ -176,7 +185,7 @@ amp_status amp_set_batch_mode(amp_model* m, int mode);
 amp_status amp_set_fused_mode(amp_model* m, int mode);
 /* Counters of the last amp_nll / amp_norm_integral call: kernels launched, lineshape columns
  * recomputed (data + norm), which normalisation path ran (1 direct streaming sum, 2 matrix, 3 batched DMMA sum,
- * 4 fused single launch, 5 gradient-batch delta kernel, 6 background + purity).                         */
+ * 4 fused single launch, 5 gradient-batch delta kernel, 6 background + purity, 7 analytic gradient).                         */
 amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_recomputed, int* norm_path);
 
 /* Device time [ms] of the phases of the last amp_nll / amp_norm_integral call, from CUDA events recorded on

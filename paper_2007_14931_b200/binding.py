@@ -18,7 +18,7 @@ AMP_MAX_RESONANCES, AMP_MAX_COUPLINGS, AMP_MAX_POINTS = 16, 48, 256
 # every symbol include/amp.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
-    "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
+    "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_grad", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
     "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_fit_fractions", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode",
     "amp_last_call_stats", "amp_last_call_timing", "amp_recent_launch_ms", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
 ]
@@ -62,6 +62,7 @@ def lib():
         "amp_set_background": (i, [vp, vp, d, vp]),
         "amp_set_params": (i, [vp, i, vp, vp]),
         "amp_nll": (i, [vp, vp, vp]),
+        "amp_nll_grad": (i, [vp, vp, vp, vp]),
         "amp_nll_terms": (i, [vp, vp, vp, vp]),
         "amp_dataset_sums": (i, [vp, C.POINTER(ll), pd, C.POINTER(ll), pd]),
         "amp_eval_events": (i, [vp, i, vp, vp]),
@@ -188,6 +189,12 @@ class Model:
         if not (allow_domain_error and st == AMP_ERR_DOMAIN):
             self._check(st, "amp_nll")
         return out[:self.P]
+
+    def nll_grad(self, stream=None):
+        """(NLL, grad [K][2] = (dNLL/dRe H_k, dNLL/dIm H_k)) at the single point set by set_params"""
+        nll, grad = np.empty(1), np.empty((self.K, 2))
+        self._check(lib().amp_nll_grad(self._h, nll.ctypes.data_as(C.c_void_p), grad.ctypes.data_as(C.c_void_p), _stream_ptr(stream)), "amp_nll_grad")
+        return nll[0], grad
 
     def nll_terms(self, stream=None):
         """(sum_i log S_i(p), sum_j w_j S_j(p)) of this model's own events, [P] each: the per-shard sums behind nll()"""

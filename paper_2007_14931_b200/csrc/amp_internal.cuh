@@ -310,6 +310,25 @@ cudaError_t launch_delta(const DeltaArgs& d, int grid, cudaStream_t s);
 int delta_grid(long long n_data, long long n_norm);
 bool delta_fits(int ngrp);
 
+// Analytic gradient of the NLL in the couplings (grad.cu): one pair of leaves (real, imaginary part) per coupling slot
+enum { GRAD_MAX_PAIRS = 48 };
+struct GradArgs {
+    StreamArgs a;                       // the point, as the streaming kernel sees it (cache/n: data; cache2/n2: norm)
+    int npairs;                         // coupling slots, padded to a multiple of 16 (2 npairs leaves = whole 32-leaf blocks)
+    signed char pair_ent[GRAD_MAX_PAIRS];   // entry of StreamArgs::ent whose lineshape the slot carries; -1: lineshape == 1; -2: padding
+    signed char pair_lam[GRAD_MAX_PAIRS];   // helicity -1, 0, +1
+    signed char pair_J[GRAD_MAX_PAIRS];     // spin of a K* (0 for a constant term); 8: Z
+    signed char pair_grp[GRAD_MAX_PAIRS];   // barrier group of the entry
+    short pair_slot[GRAD_MAX_PAIRS];        // coupling slot k the pair belongs to, -1: padding
+    int K;
+    double* partial;                    // [2][2 + 2 npairs][stride]: per-CTA partials; rows 0, 1 = sum log S / sum w S
+    int stride;
+    double* result;                     // [3 + 2 K]: NLL, I, domain flag, then (dNLL/dRe c_k, dNLL/dIm c_k); may be mapped host memory
+};
+cudaError_t launch_grad(const GradArgs& g, int grid, cudaStream_t s);
+int grad_grid(long long n_data, long long n_norm);
+bool grad_fits(int nent, int ngrp);
+
 // Batched combine (P > 1) on the FP64 tensor cores, see batch.cu
 enum { BATCH_NKT = 14, BATCH_POINTS = 128, BATCH_MAX_COLS = 48 };   // dense k-tiles (2K <= 56 realified rows) and points per launch
 struct BatchArgs {

@@ -1482,6 +1482,65 @@ amp_status amp_dataset_sums(const amp_model* m, long long* n_data, double* sum_l
     return AMP_OK;
 }
 
+amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    if (!h_nll || !h_grad) return fail(m, AMP_ERR_INVALID, "amp_nll_grad: null output");
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
+    if (!m->data.loaded) return fail(m, AMP_ERR_STATE, "no data events loaded (amp_load_events)");
+    if (m->P != 1) return fail(m, AMP_ERR_STATE, "amp_nll_grad: set exactly one parameter point (amp_set_params with P = 1)");
+    if (m->has_bkg) return fail(m, AMP_ERR_STATE, "amp_nll_grad: not available with a background (Eq. 14)");
+    for (const auto& rs : m->res)
+        if (rs.kind == AMP_LASS) return fail(m, AMP_ERR_STATE, "amp_nll_grad: not available for models with a LASS term");
+    if (!m->stream_inline) return fail(m, AMP_ERR_STATE, "amp_nll_grad: needs lineshapes in registers (amp_set_lineshape_mode 0 or 2)");
+    if (m->K > GRAD_MAX_PAIRS) return fail(m, AMP_ERR_INVALID, "amp_nll_grad: too many couplings");
+    int ent_of_res[AMP_MAX_RESONANCES], grp_of_res[AMP_MAX_RESONANCES];
+    GradArgs g{};
+    fill_stream_args(m, m->data, 0, MODE_FUSED, &g.a, ent_of_res, grp_of_res);
+    int nent = 0;
+    for (int sp = 0; sp < 6; ++sp) nent += g.a.shape[sp];
+    if (!grad_fits(nent, g.a.gstart[6])) return fail(m, AMP_ERR_INVALID, "amp_nll_grad: the model does not fit the kernel's shared memory");
+    g.a.cache2 = m->norm.cache; g.a.n2 = m->norm.n; g.a.npad2 = m->norm.npad;
+    g.a.ticket = m->d_ticket;
+    g.a.sum_log_eff = m->data.wsum;
+    g.a.wsum = m->norm.wsum;
+    const int K = m->K;
+    g.K = K;
+    g.npairs = (K + 15) / 16 * 16;
+    for (int p = 0; p < GRAD_MAX_PAIRS; ++p) { g.pair_ent[p] = -2; g.pair_lam[p] = 0; g.pair_J[p] = 0; g.pair_grp[p] = 0; g.pair_slot[p] = -1; }
+    for (int r = 0; r < m->R; ++r) {
+        const amp_resonance& rs = m->res[r];
+        const int ns = (rs.kind == AMP_Z || (rs.kind == AMP_KSTAR && rs.J >= 1)) ? 3 : 1;
+        for (int j = 0; j < ns; ++j) {
+            const int k = m->slot0[r] + j;
+            g.pair_ent[k] = rs.kind == AMP_CONST ? -1 : (signed char)ent_of_res[r];
+            g.pair_lam[k] = (signed char)(ns == 3 ? j - 1 : 0);
+            g.pair_J[k] = rs.kind == AMP_Z ? 8 : (signed char)rs.J;
+            g.pair_grp[k] = rs.kind == AMP_CONST ? 0 : (signed char)grp_of_res[r];
+            g.pair_slot[k] = (short)k;
+        }
+    }
+    g.partial = m->d_partial;
+    g.stride = PARTIAL_STRIDE;
+    g.result = m->d_result;
+    m->ring_last = (m->ring_last + 1) % amp_model::RING;
+    m->ring_calls++;
+    CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
+    CK(launch_grad(g, grad_grid(m->data.n, m->norm.n), s));
+    CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
+    CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (3 + 2 * K), cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    m->stat_launches = 1;
+    m->stat_columns = 0;
+    m->stat_norm_path = 7;
+    m->fused_valid = true;
+    h_nll[0] = m->h_pinned[0];
+    bool bad = m->h_pinned[2] != 0.0 || !std::isfinite(h_nll[0]);
+    for (int i = 0; i < 2 * K; ++i) { h_grad[i] = m->h_pinned[3 + i]; bad |= !std::isfinite(h_grad[i]); }
+    if (bad) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
+    return AMP_OK;
+}
+
 amp_status amp_norm_integral(amp_model* m, double* h_I, void* stream) {
     if (!m) return AMP_ERR_INVALID;
     if (!h_I) return fail(m, AMP_ERR_INVALID, "amp_norm_integral: null output");
