@@ -44,6 +44,8 @@ TRAFFIC_NCU_BYTES_CFG4 = 2.192431e9 + 4.04e6  # profiles/r01c_ncu_full_delta_cfg
 # (Breit-Wigner of point 0 from the saved barrier factors ~20, angular factor ~8, two complex products 12) + 100 coupling
 # points (two complex multiply-adds 16, |A|^2 7, accumulate 2) + 20 mass/width points (perturbed Breit-Wigner ~22, the same 25)
 DELTA_FLOP_PER_EVENT = 730.0 + 31 * 40.0 + 100 * 25.0 + 20 * 47.0
+# analytic gradient: the point (730) + per coupling slot: angular factor ~8, T = sum_xi conj(g) A 16, conj(BW) T 8, weight 2
+GRAD_FLOP_PER_EVENT = 730.0 + 27 * 34.0
 
 
 LASS = False   # --lass: the paper's LASS variant of the model (Eq. 9) instead of kappa(800) + K0*(1430)
@@ -196,6 +198,8 @@ def run_own(args):
     def one_step(s):
         cs, mws = params[s]
         model.set_params(cs, mws)
+        if args.grad:
+            return np.array([model.nll_grad()[0]])   # NLL + its analytic gradient in all K couplings, one launch
         return model.nll()
 
     for s in range(args.warmup):
@@ -224,7 +228,7 @@ def run_own(args):
     # the kernel times come from the library's ring of CUDA event pairs recorded around each launch on its stream
     st = model.last_call_stats()
     launches, paths = st["launches"] * args.steps, {st["norm_path"]}
-    if st["norm_path"] in (4, 5):
+    if st["norm_path"] in (4, 5, 7):
         ring = model.recent_launch_ms(min(args.steps, 256))
         t_data, t_norm, t_line = [float(v) for v in ring], [0.0], [0.0]
     else:
@@ -253,6 +257,15 @@ def run_own(args):
                 "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md 6; the DFMA probe below measures it)", "unit": "TFLOP/s",
                 "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": TRAFFIC_NCU_BYTES_CFG4 if (args.n_data, args.n_norm) == (2_000_000, 10_000_000) else None, "kernel_ms": k_ms,
                 "flop_per_event": DELTA_FLOP_PER_EVENT, "flop_per_launch": flop,
+                "hbm_frac": (BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}
+    elif paths == {7}:
+        # --grad: NLL and analytic gradient in one k_grad launch per step; plain FP64 ALUs
+        k_ms = float(np.mean(t_data))
+        flop = GRAD_FLOP_PER_EVENT * (args.n_data + args.n_norm)
+        ach = flop / (k_ms * 1e-3) / 1e12
+        roof = {"bound": "alu", "kernel": "k_grad (NLL + dNLL/dH_k for all K = 27 couplings, data then norm tiles, one launch)",
+                "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12, "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz", "unit": "TFLOP/s",
+                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": None, "kernel_ms": k_ms, "flop_per_event": GRAD_FLOP_PER_EVENT,
                 "hbm_frac": (BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}
     elif args.cfg == 4:
         # dense form (--dense): k_batch (data, DMMA contraction) + k_herk (normalisation matrix, DMMA) + k_lineshape
@@ -288,7 +301,7 @@ def run_own(args):
         "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": ("LASS variant (Eq. 9: LASS S-wave + 8 K* + Z, R=10, K=26) of " if LASS else "") + f"configs[{args.cfg}]: full K*+Z model (R=11, K=27), {args.n_data} data / {args.n_norm} norm events per GPU, "
-                               f"P={P}, all lineshapes floating", "n_data": args.n_data, "n_norm": args.n_norm, "P": P,
+                               f"P={P}, all lineshapes floating" + (", each step returns the NLL AND its analytic gradient in the 27 couplings" if args.grad else ""), "n_data": args.n_data, "n_norm": args.n_norm, "P": P,
                    "l2": "inputs (2.1 GB kinematics cache) larger than L2; no flush needed", "parallelism": f"replicas x{world}"},
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "note": "host wall clock around amp_set_params (host parameter arrays in) + amp_nll (host NLL out) per step; the events are "
@@ -386,6 +399,7 @@ def main():
     ap.add_argument("--n-norm", type=int, default=10_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--dense", action="store_true", help="--cfg 4 through the dense DMMA contraction instead of the gradient-batch kernel")
+    ap.add_argument("--grad", action="store_true", help="--cfg 3 steps that also return the analytic gradient in all couplings (amp_nll_grad)")
     ap.add_argument("--lass", action="store_true", help="configs[3] call pattern on the LASS variant of the model (Eqs. 7-9; SURVEY.md 8(f)-1)")
     args = ap.parse_args()
     global LASS
