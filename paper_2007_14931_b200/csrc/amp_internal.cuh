@@ -205,8 +205,9 @@ enum { MAX_LINE_JOBS = 64 };
 cudaError_t launch_lineshape(const Dataset& d, const LineshapeJob* jobs, int njobs, cudaStream_t s);
 
 // Streaming combine + reduce for one parameter point (a3 + a5, P = 1)
-enum StreamMode { MODE_DATA = 0, MODE_NORM = 1, MODE_EVAL = 2, MODE_FUSED = 3, MODE_DATA_BKG = 4 };   // FUSED: data (sum log S) then norm (sum w S) in one launch + final NLL;
+enum StreamMode { MODE_DATA = 0, MODE_NORM = 1, MODE_EVAL = 2, MODE_FUSED = 3, MODE_DATA_BKG = 4, MODE_DATA_M = 5 };   // FUSED: data (sum log S) then norm (sum w S) in one launch + final NLL;
                                                                                               // DATA_BKG: sum log(purity eps S / I + (1 - purity) b), Eq. 14
+                                                                                              // DATA_M: data tiles only; the last CTA takes I = c^H M c from the held matrix + final NLL
 // One resonance as the streaming kernel sees it: the three per-(mass,width) constants of LineConst,
 // its first coupling slot, and either a pool column to read or -1 = evaluate in registers.
 struct ResEntry {
@@ -267,6 +268,11 @@ struct StreamArgs {
     const double* bkg;
     const double* sum_wS;
     double purity;
+    // MODE_DATA_M (static lineshapes): the held realified Gram matrix G' [KP][KP] (herk.cu) and the couplings in its entry
+    // order (slot order, zero-padded to qf_nent): the last CTA evaluates sum_j w_j S_j = c^H M c itself
+    const double* qf_G;
+    int qf_KP, qf_nent;
+    double2 qf_c[AMP_MAX_COUPLINGS];
 };
 cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s);
 int stream_grid(long long n, bool have_z, int mode);

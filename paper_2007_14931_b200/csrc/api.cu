@@ -73,6 +73,9 @@ struct amp_model {
     std::vector<int2> gram_tiles;
     bool gram_valid = false;
     int gram_KP = 0;
+    bool gram_p1 = false;          // the held matrix was built for a single-point call whose masses and widths are gram_mw
+    int gram_nent = 0;
+    std::vector<double> gram_mw;
     double* d_G = nullptr;         // [KP][KP] dense symmetric realified Gram matrix (sum_j w_j b' b'^T)
     double* d_gt = nullptr;        // [ntile][64]
     double* d_gpartial = nullptr;  // [148][ntile][64]
@@ -1161,6 +1164,7 @@ amp_status norm_via_matrix(amp_model* m, const HerkPlan& hp, double* d_out, cuda
         m->gram_tiles = hp.tiles;
         m->gram_KP = KP;
         m->gram_valid = true;
+        m->gram_p1 = false;   // (evaluate() marks single-point matrices)
         m->stat_gram_built = 1;
     }
     CK(launch_quadform(m->d_G, KP, reinterpret_cast<const double2*>(m->d_hk + oC), hp.nent, P, d_out, s));
@@ -1290,6 +1294,52 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
             if (h_I) { h_I[p] = m->h_pinned[P + p]; bad |= !(h_I[p] > 0) || !std::isfinite(h_I[p]); }
         }
         if (bad) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
+        return AMP_OK;
+    }
+    if (want_nll && P == 1 && m->stream_inline && m->want_matrix && m->fused_mode == 0 && m->gram_valid && m->gram_p1 && m->gram_mw == m->mw &&
+        m->K <= AMP_MAX_COUPLINGS) {
+        // Static lineshapes (the paper's default: masses and widths fixed) with the matrix M already held: ONE launch
+        // over the data tiles; the last CTA evaluates c^H M c from the device-resident matrix and forms the NLL (MODE_DATA_M).
+        StreamArgs a;
+        fill_stream_args(m, m->data, 0, MODE_DATA_M, &a);
+        a.partial = m->d_partial;
+        a.ticket = m->d_ticket;
+        a.sum_log_eff = m->data.wsum;
+        a.wsum = m->norm.wsum;
+        a.qf_G = m->d_G;
+        a.qf_KP = m->gram_KP;
+        a.qf_nent = m->gram_nent;
+        for (int k = 0; k < AMP_MAX_COUPLINGS; ++k)
+            a.qf_c[k] = k < m->K ? make_double2(m->couplings[2 * k], m->couplings[2 * k + 1]) : make_double2(0, 0);
+        double* res = m->h_pinned;
+        if (m->zero_copy) { m->zc_seq += 1.0; a.result = m->h_zc; a.seq = m->zc_seq; res = m->h_zc; }
+        else { a.result = m->d_result; a.seq = 0.0; }
+        m->ring_last = (m->ring_last + 1) % amp_model::RING;
+        m->ring_calls++;
+        CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
+        CK(launch_stream(a, stream_grid(m->data.n, m->has_z, MODE_DATA), s));
+        CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
+        if (m->zero_copy) {
+            volatile double* stamp = m->h_zc + 5;
+            for (unsigned spins = 0; *stamp != m->zc_seq; ++spins) {
+                if ((spins & 0x3fff) == 0x3fff) {
+                    const cudaError_t q = cudaStreamQuery(s);
+                    if (q != cudaErrorNotReady) { if (q != cudaSuccess) return cuda_fail(m, q, "matrix step"); if (*stamp == m->zc_seq) break; return fail(m, AMP_ERR_CUDA, "matrix step finished without a result"); }
+                }
+            }
+            std::atomic_thread_fence(std::memory_order_acquire);
+        } else {
+            CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * 5, cudaMemcpyDeviceToHost, s));
+            CK(cudaStreamSynchronize(s));
+        }
+        m->last_slog.assign(1, res[3]);
+        m->last_swS.assign(1, res[4]);
+        m->stat_launches = 1;
+        m->stat_norm_path = 2;
+        m->fused_valid = true;
+        h_nll[0] = res[0];
+        if (h_I) h_I[0] = res[1];
+        if (res[2] != 0.0 || !std::isfinite(h_nll[0])) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
         return AMP_OK;
     }
     if (want_nll && P == 1 && m->stream_inline && !m->want_matrix && m->fused_mode == 0) {
@@ -1423,6 +1473,7 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         st = norm_via_matrix(m, hp, m->d_sums + P, s);
         if (st != AMP_OK) return st;
         m->stat_norm_path = 2;
+        if (P == 1) { m->gram_p1 = true; m->gram_nent = hp.nent; m->gram_mw = m->mw; }   // later calls at these masses: one launch
     }
     CK(cudaEventRecord(m->ev[3], s));
     if (want_nll) {

@@ -34,7 +34,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     // sum w S (normalisation tiles) lives in `acc`; sum log S (data tiles) as a running product of mantissas in `acc` and a
     // sum of exponents in `accE` (split_exp: integer ops + one multiply per event instead of a ~35-instruction FP64 log)
     const double LN2 = 0.69314718055994530942;
-    double acc = (MODE == MODE_DATA || MODE == MODE_FUSED || MODE == MODE_DATA_BKG) ? 1.0 : 0.0;
+    double acc = (MODE == MODE_DATA || MODE == MODE_FUSED || MODE == MODE_DATA_BKG || MODE == MODE_DATA_M) ? 1.0 : 0.0;
     // Eq. 14: f = (purity / I) eps S + (1 - purity) b, I = sum_wS / wsum from the normalisation pass that ran before
     const double bkg_ps = MODE == MODE_DATA_BKG ? a.purity * a.wsum / __ldg(a.sum_wS) : 0.0, bkg_qb = 1.0 - a.purity;
     int accE = 0;
@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     // therefore has a whole iteration to arrive, and two CTAs (16 warps) fit on an SM.
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int ncache = have_z ? NCOL_ALL : NCOL_K;
-    const bool with_w = MODE != MODE_DATA;   // the K* region carries the weight column (MODE_FUSED: only for normalisation tiles)
+    const bool with_w = MODE != MODE_DATA && MODE != MODE_DATA_M;   // the K* region carries the weight column (MODE_FUSED: only for normalisation tiles)
     double* stage = reinterpret_cast<double*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)(ncache + 1) * TILE * sizeof(double));   // [0]: K* region, [1]: Z region
     if (threadIdx.x == 0) {
@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
                 split_exp((live && ok) ? f0 : 1.0, &f, &x);
                 acc *= f;
                 accE += x;
-            } else if (MODE == MODE_DATA || (MODE == MODE_FUSED && !is_norm)) {
+            } else if (MODE == MODE_DATA || MODE == MODE_DATA_M || (MODE == MODE_FUSED && !is_norm)) {
                 const bool ok = S > 0.0 && isfinite(S);
                 bad |= live && !ok;
                 double f; int x;
@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
                 if (live) a.out[i0 + e] = w.v[e] * S;
             }
         }
-        if (MODE == MODE_DATA || MODE == MODE_DATA_BKG || (MODE == MODE_FUSED && !is_norm)) {   // running product back to [0.5, 1) once per tile
+        if (MODE == MODE_DATA || MODE == MODE_DATA_BKG || MODE == MODE_DATA_M || (MODE == MODE_FUSED && !is_norm)) {   // running product back to [0.5, 1) once per tile
             int x;
             split_exp(acc, &acc, &x);
             accE += x;
@@ -191,14 +191,14 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     if (MODE == MODE_EVAL) return;
     if (bad) atomicOr(a.flag, 2);
     {
-        const bool logs = MODE == MODE_DATA || MODE == MODE_DATA_BKG || (MODE == MODE_FUSED && !in_norm);
+        const bool logs = MODE == MODE_DATA || MODE == MODE_DATA_BKG || MODE == MODE_DATA_M || (MODE == MODE_FUSED && !in_norm);
         const double t = block_sum(logs ? log(acc) + (double)accE * LN2 : acc, sm);
         if (threadIdx.x == 0) {
             if (MODE == MODE_FUSED && !in_norm) { a.partial[blockIdx.x] = t; a.partial2[blockIdx.x] = 0.0; }   // this CTA saw data tiles only
             else (MODE == MODE_FUSED ? a.partial2 : a.partial)[blockIdx.x] = t;
         }
     }
-    if (MODE != MODE_FUSED) return;
+    if (MODE != MODE_FUSED && MODE != MODE_DATA_M) return;
     // The last CTA to finish (integer ticket) adds the per-CTA partials in a fixed order and forms the NLL: the result
     // does not depend on which CTA that is, so it stays bit-reproducible; no second launch, no host round trip.
     __shared__ bool s_last;
@@ -210,7 +210,23 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     if (!s_last) return;
     __threadfence();
     const double slog = partial_sum(a.partial, gridDim.x, sm);
-    const double swS = partial_sum(a.partial2, gridDim.x, sm);
+    double swS;
+    if (MODE == MODE_DATA_M) {
+        // sum_j w_j S_j = c^H M c from the held matrix (Re M_ef = G'[2e][2f] + G'[2e+1][2f+1], Im M_ef = G'[2e][2f+1] - G'[2e+1][2f]):
+        // K^2 terms, thread t takes idx = t, t + 256, ... in a fixed order
+        double q = 0.0;
+        for (int idx = threadIdx.x; idx < a.qf_nent * a.qf_nent; idx += THREADS) {
+            const int e = idx / a.qf_nent, f = idx % a.qf_nent;
+            const double2 ce = a.qf_c[e], cf = a.qf_c[f];
+            if ((ce.x == 0.0 && ce.y == 0.0) || (cf.x == 0.0 && cf.y == 0.0)) continue;
+            const double* gm = a.qf_G + (size_t)(2 * e) * a.qf_KP + 2 * f;
+            const double mre = gm[0] + gm[a.qf_KP + 1], mim = gm[1] - gm[a.qf_KP];
+            q += ce.x * (mre * cf.x - mim * cf.y) + ce.y * (mre * cf.y + mim * cf.x);
+        }
+        swS = block_sum(q, sm);
+    } else {
+        swS = partial_sum(a.partial2, gridDim.x, sm);
+    }
     if (threadIdx.x == 0) {
         const double I = swS / a.wsum;
         double v = -(slog + a.sum_log_eff) + (double)a.n * log(I);
@@ -266,6 +282,7 @@ static cudaError_t launch_shape(const StreamArgs& a, int grid, cudaStream_t s) {
         case MODE_NORM: AMP_LAUNCH(MODE_NORM) break;
         case MODE_FUSED: AMP_LAUNCH(MODE_FUSED) break;
         case MODE_DATA_BKG: AMP_LAUNCH(MODE_DATA_BKG) break;
+        case MODE_DATA_M: AMP_LAUNCH(MODE_DATA_M) break;
         default: AMP_LAUNCH(MODE_EVAL) break;
     }
 #undef AMP_LAUNCH

@@ -84,7 +84,7 @@ __device__ __forceinline__ void issue_tile(const StreamArgs& a, long long ntd, l
     if (MODE == MODE_FUSED && tile >= ntd)
         issue_cols(a.cache2, a.ncolw, tile - ntd, stage, bar, c0, c1, region_has_w);
     else
-        issue_cols(a.cache, a.ncolw, tile, stage, bar, c0, c1, region_has_w && MODE != MODE_DATA && MODE != MODE_FUSED);
+        issue_cols(a.cache, a.ncolw, tile, stage, bar, c0, c1, region_has_w && MODE != MODE_DATA && MODE != MODE_FUSED && MODE != MODE_DATA_M);
 }
 
 // fixed-order block sum: xor-shuffle tree, then the 8 warp values in warp order; result valid in thread 0

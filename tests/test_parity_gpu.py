@@ -559,6 +559,7 @@ def test_static_lineshapes_switch_to_the_matrix():
         paths.append(st["norm_path"]); launches.append(st["launches"])
     assert paths == [4, 2, 2, 2]      # first call: fused single launch with a direct-sum normalisation; then the matrix
     assert launches[3] < launches[1]          # no lineshape / HERK launches once M is held
+    assert launches[2] == 1 and launches[3] == 1   # ... the step is ONE launch: data tiles + c^H M c + NLL in the last thread block
     mw = W.step_mass_width(3, 5)[:10]
     Mg.set_params(c, mw[None])
     nll = Mg.nll()[0]
