@@ -1555,6 +1555,28 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
     g.a.ticket = m->d_ticket;
     g.a.sum_log_eff = m->data.wsum;
     g.a.wsum = m->norm.wsum;
+    // Static lineshapes (masses and widths as in the previous call): the normalisation side comes from the matrix M —
+    // N_k = (M c)_k, sum w S = c^H M c — so only the data events are walked; M is built here if it is not held yet.
+    if (m->want_matrix && m->K <= AMP_MAX_COUPLINGS) {
+        if (!(m->gram_valid && m->gram_p1 && m->gram_mw == m->mw)) {
+            HerkPlan hp;
+            if (build_herk_plan(m, &hp, 0, 1)) {
+                amp_status st = ensure_pool(m, 0);
+                if (st == AMP_OK) st = refresh_columns(m, m->norm, true, s);
+                if (st == AMP_OK) st = norm_via_matrix(m, hp, m->d_sums, s);
+                if (st != AMP_OK) return st;
+                m->gram_p1 = true; m->gram_nent = hp.nent; m->gram_mw = m->mw;
+            }
+        }
+        if (m->gram_valid && m->gram_p1 && m->gram_mw == m->mw) {
+            g.a.n2 = 0;
+            g.a.qf_G = m->d_G;
+            g.a.qf_KP = m->gram_KP;
+            g.a.qf_nent = m->gram_nent;
+            for (int k = 0; k < AMP_MAX_COUPLINGS; ++k)
+                g.a.qf_c[k] = k < m->K ? make_double2(m->couplings[2 * k], m->couplings[2 * k + 1]) : make_double2(0, 0);
+        }
+    }
     const int K = m->K;
     g.K = K;
     g.npairs = (K + 15) / 16 * 16;
@@ -1577,7 +1599,7 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
     m->ring_last = (m->ring_last + 1) % amp_model::RING;
     m->ring_calls++;
     CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
-    CK(launch_grad(g, grad_grid(m->data.n, m->norm.n), s));
+    CK(launch_grad(g, grad_grid(m->data.n, g.a.n2), s));
     CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
     CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (3 + 2 * K), cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));

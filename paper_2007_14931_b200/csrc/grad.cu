@@ -238,7 +238,37 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
         tot[r] = s;
     }
     __syncthreads();
-    const double swS = tot[1], nd = (double)a.n;
+    const double nd = (double)a.n;
+    if (a.qf_G) {
+        // static lineshapes: no normalisation tile was walked; the held matrix gives N_k = (M c)_k and sum w S = c^H M c
+        // (Re M_kf = G'[2k][2f] + G'[2k+1][2f+1], Im M_kf = G'[2k][2f+1] - G'[2k+1][2f]); one thread per slot, fixed order
+        for (int p = tid; p < g.npairs; p += THREADS) {
+            const int kslot = g.pair_slot[p];
+            double2 acc = make_double2(0.0, 0.0);
+            if (kslot >= 0) {
+                for (int f = 0; f < a.qf_nent; ++f) {
+                    const double2 cf = a.qf_c[f];
+                    const double* gm = a.qf_G + (size_t)(2 * kslot) * a.qf_KP + 2 * f;
+                    const double mre = gm[0] + gm[a.qf_KP + 1], mim = gm[1] - gm[a.qf_KP];
+                    acc.x += mre * cf.x - mim * cf.y;
+                    acc.y += mre * cf.y + mim * cf.x;
+                }
+            }
+            tot[2 + nleaf + 2 * p] = acc.x;
+            tot[2 + nleaf + 2 * p + 1] = acc.y;
+        }
+        __syncthreads();
+        if (tid == 0) {   // c^H M c = sum_k Re(conj(c_k) (M c)_k), slot order
+            double q = 0.0;
+            for (int p = 0; p < g.npairs; ++p) {
+                const int kslot = g.pair_slot[p];
+                if (kslot >= 0) q += a.qf_c[kslot].x * tot[2 + nleaf + 2 * p] + a.qf_c[kslot].y * tot[2 + nleaf + 2 * p + 1];
+            }
+            tot[1] = q;
+        }
+        __syncthreads();
+    }
+    const double swS = tot[1];
     for (int p = tid; p < g.npairs; p += THREADS) {
         const int kslot = g.pair_slot[p];
         if (kslot < 0) continue;

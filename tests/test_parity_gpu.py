@@ -449,6 +449,17 @@ def test_analytic_gradient_matches_oracle(cfg):
     nll2, g2 = Mg.nll_grad()
     assert nll2 == nll and np.array_equal(g2, g)
     assert abs(Mg.nll()[0] - nll) < 1e-13 * abs(nll)
+    # same masses and widths again, other couplings (a fit at fixed lineshapes): the normalisation side comes from the matrix M
+    # ((M c)_k and c^H M c), only the data events are walked
+    c2 = c * (1 + 0.05 * np.cos(np.arange(len(c)))) * np.exp(0.05j * np.sin(np.arange(len(c))))
+    Mg.set_params(c2)
+    nll3, g3 = Mg.nll_grad()
+    rn3, rg3 = Mo.nll_gradient(c2, x, eff, xn, wn)
+    assert abs(nll3 - rn3) < RTOL_NLL * abs(rn3)
+    assert np.max(np.abs(g3 - rg3)) < 1e-9 * np.max(np.abs(rg3)), np.max(np.abs(g3 - rg3)) / np.max(np.abs(rg3))
+    Mg.set_params(c2)
+    nll4, g4 = Mg.nll_grad()
+    assert nll4 == nll3 and np.array_equal(g4, g3)
     if cfg == 2:
         mw = W.step_mass_width(3, 2)
         Mg.set_params(c, mw[None])
