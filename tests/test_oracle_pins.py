@@ -587,3 +587,99 @@ def test_golden_oracle_regression():
         nll, integral = Mo.nll(c, x, eff, xn, wn)
         assert abs(nll[0] - float.fromhex(e["nll"])) < 1e-12 * abs(nll[0])
         assert abs(integral[0] - float.fromhex(e["integral"])) < 1e-13 * integral[0]
+
+
+# ------------------------------------------------------------------ P17-P19: toy generator (oracle/toy.py)
+def test_P17_philox_known_answers():
+    """the counter-based generator against the publication's known-answer vectors (tests/golden/philox4x32_10_kat.txt)"""
+    import os
+    from oracle import toy
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(t, 16) for t in r]
+        out = toy.philox4x32_10(np.array([v[0:4]], dtype=np.uint64), (v[4], v[5]))[0]
+        assert [int(o) for o in out] == v[6:10]
+    # vectorised call = row-by-row calls; distinct counters give distinct outputs
+    ctr = np.array([[i, 7, j, 0] for i in range(5) for j in range(3)], dtype=np.uint64)
+    allr = toy.philox4x32_10(ctr, (123, 456))
+    for k in range(len(ctr)):
+        assert np.array_equal(allr[k], toy.philox4x32_10(ctr[k:k + 1], (123, 456))[0])
+    assert len({tuple(int(v) for v in r) for r in allr}) == len(ctr)
+
+
+def test_P18_uniform53_range_and_resolution():
+    from oracle import toy
+    F = 0xFFFFFFFF
+    assert toy.uniform53([0], [0])[0] == 0.0
+    assert toy.uniform53([F], [F])[0] == 1.0 - 2.0 ** -53          # largest value: strictly below 1
+    assert toy.uniform53([1 << 5], [0])[0] == 2.0 ** -27            # lowest kept bit of the first word
+    assert toy.uniform53([0], [1 << 6])[0] == 2.0 ** -53            # lowest kept bit of the second word
+    assert toy.uniform53([31], [63])[0] == 0.0                      # dropped bits
+    # candidate map: ranges, and the stream does not depend on how it is cut into calls
+    lo, hi, cm = MK + MPI + 1e-3, 2182.0, 1 - 1e-9
+    x, u = toy.candidates(99, 0, 20000, lo, hi, cm)
+    assert x[0].min() >= lo and x[0].max() < hi and np.abs(x[1:3]).max() <= cm and x[3].min() >= -np.pi and x[3].max() < np.pi
+    assert u.min() >= 0 and u.max() < 1
+    x2, u2 = toy.candidates(99, 5000, 100, lo, hi, cm)
+    assert np.array_equal(x2, x[:, 5000:5100]) and np.array_equal(u2, u[5000:5100])
+    xb, _ = toy.candidates(99 + (1 << 32), 0, 100, lo, hi, cm)      # the high seed word is part of the key
+    assert not np.array_equal(xb, x[:, :100])
+    # uniformity of each of the five streams and independence of neighbours (means, variances, lag-1 and cross correlations)
+    U = np.vstack([(x[0] - lo) / (hi - lo), (x[1] / cm + 1) / 2, (x[2] / cm + 1) / 2, (x[3] / np.pi + 1) / 2, u])
+    n = U.shape[1]
+    assert np.all(np.abs(U.mean(1) - 0.5) < 5 * math.sqrt(1 / 12 / n))
+    assert np.all(np.abs(U.var(1) - 1 / 12) < 5 * math.sqrt(1 / 180 / n))
+    cc = np.corrcoef(U)
+    assert np.all(np.abs(cc - np.eye(5)) < 5 / math.sqrt(n))
+    for k in range(5):
+        assert abs(np.corrcoef(U[k, :-1], U[k, 1:])[0, 1]) < 5 / math.sqrt(n)
+
+
+def test_P19_toy_of_constant_spin0_model_follows_phase_space():
+    """one constant spin-0 term: S = |c|^2 sum_xi |d^1_{0 xi}(theta_psi)|^2 = |c|^2 sin^2 theta_psi, so the accepted events follow
+    p_B(m) q(m) in m_Kpi (compared with scipy quadrature of the textbook two-body momenta), (1 - c^2) in cos theta_psi,
+    and are flat in cos theta_K* and phi"""
+    from oracle import toy
+    M = O.Model(DEC, [(W.CONST, 0, 0.0, 0.0, 0.0)])
+    c = np.array([0.7 - 0.4j])
+    lo, hi, cm = MK + MPI + 1e-3, 2182.0, 1 - 1e-9
+
+    def pq(m):
+        pB = math.sqrt((MB * MB - (m + MPSI) ** 2) * (MB * MB - (m - MPSI) ** 2)) / (2 * MB)
+        q = math.sqrt((m * m - (MK + MPI) ** 2) * (m * m - (MK - MPI) ** 2)) / (2 * m)
+        return pB * q
+
+    grid = np.linspace(lo, hi, 20001)
+    fmax = 1.0001 * abs(c[0]) ** 2 * max(pq(m) for m in grid)
+    n = 300_000
+    g = toy.generate(M, c, 4242, 0, n, fmax, lo, hi, cm)
+    assert g["f_seen_max"] <= fmax
+    x = g["x"]
+    nacc = x.shape[1]
+    # acceptance = mean f / f_max;  mean f = |c|^2 <pq> <sin^2> = |c|^2 * (int pq dm / (hi - lo)) * 2/3
+    ipq = integrate.quad(pq, lo, hi, epsabs=0, epsrel=1e-10, limit=200)[0]
+    p_acc = abs(c[0]) ** 2 * ipq / (hi - lo) * (2 / 3) / fmax
+    assert abs(nacc - n * p_acc) < 5 * math.sqrt(n * p_acc * (1 - p_acc)), (nacc, n * p_acc)
+    assert np.array_equal(x, toy.candidates(4242, 0, n, lo, hi, cm)[0][:, g["index"]])
+    # m_Kpi histogram against the integral of p_B q per bin
+    edges = np.linspace(lo, hi, 41)
+    obs = np.histogram(x[0], edges)[0]
+    exp = np.array([integrate.quad(pq, a, b, epsabs=0, epsrel=1e-10)[0] for a, b in zip(edges[:-1], edges[1:])]) / ipq * nacc
+    chi2 = float(np.sum((obs - exp) ** 2 / exp))
+    assert chi2 < 39 + 5 * math.sqrt(2 * 39), chi2
+    # angular moments: <cos^2 theta_psi> = 1/5 for a sin^2 law, 1/3 for a flat one; phi flat
+    assert abs(np.mean(x[2] ** 2) - 0.2) < 5 * math.sqrt((3 / 35 - 1 / 25) / nacc)
+    assert abs(np.mean(x[1] ** 2) - 1 / 3) < 5 * math.sqrt((1 / 5 - 1 / 9) / nacc)
+    assert abs(np.mean(x[1])) < 5 * math.sqrt(1 / 3 / nacc) and abs(np.mean(x[2])) < 5 * math.sqrt(0.2 / nacc)
+    assert abs(np.mean(np.cos(x[3]))) < 5 * math.sqrt(0.5 / nacc) and abs(np.mean(np.cos(2 * x[3]))) < 5 * math.sqrt(0.5 / nacc)
+    # a model WITH structure must not pass the flat-phi test: K*(892) with helicity +-1 couplings modulates cos(2 phi)
+    M2 = O.Model(DEC, W.resonances(0))
+    c2 = W.couplings(0)
+    x2p, _ = toy.candidates(7, 0, 50_000, lo, hi, cm)
+    f2 = toy.weights(M2, c2, x2p)
+    g2 = toy.generate(M2, c2, 7, 0, 50_000, float(f2.max()), lo, hi, cm)
+    assert g2["x"].shape[1] > 300
+    # accepted events are denser where the weight is larger: mean weight of accepted = <f^2>/<f> > <f>
+    assert np.mean(f2[g2["index"]]) > 1.5 * np.mean(f2)
+    assert abs(np.mean(f2[g2["index"]]) / (np.mean(f2 ** 2) / np.mean(f2)) - 1) < 5 * math.sqrt(np.var(f2[g2["index"]]) / g2["x"].shape[1]) / np.mean(f2[g2["index"]])
