@@ -124,6 +124,26 @@ amp_status amp_nll(amp_model* m, double* h_nll, void* stream);
  * for models with a LASS term (AMP_ERR_STATE).  Deterministic.  Path 7 in amp_last_call_stats.                       */
 amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* stream);
 
+/* Accept-reject toy generator ("a distribution according to the fit model is generated through MC techniques";
+ * the recipe the paper leaves open is fixed in DESIGN.md "Toy generator").  For the candidate numbers
+ * first .. first + n_candidates - 1, at the single point of the last amp_set_params (P = 1):
+ *   twelve 32-bit words of Philox4x32-10 (counter (i mod 2^32, i div 2^32, j, 0), key (seed mod 2^32, seed div 2^32), j = 0..2)
+ *   -> five uniforms U = ((w_a >> 5) 2^26 + (w_b >> 6)) 2^-53  ->  the point (Eq. 1)
+ *   x = (m_lo + (m_hi - m_lo) U0, (2 U1 - 1) cos_max, (2 U2 - 1) cos_max, (2 U3 - 1) pi),
+ *   accepted iff  U4 f_max < f(x),  f = p_B(m_Kpi) q(m_Kpi) S(x)  (phase-space density in these variables x Eq. 12).
+ * The accepted points are written in candidate order (independent of scheduling; the candidate stream itself is reproducible
+ * bit for bit): d_x_out DEVICE [4][capacity] SoA (stride = capacity), d_index_out DEVICE [capacity] their candidate numbers
+ * (may be null).  *h_n_accepted = number accepted (points beyond `capacity` are counted, not written); *h_f_seen_max =
+ * largest f among the candidates (if it exceeds f_max the toy is biased: raise f_max and call again; f_max = 0 accepts all).
+ * Efficiency is not applied: thin the toy by eps(x) afterwards, as a detector simulation would.  Needs neither data nor
+ * normalisation events; leaves both untouched.  AMP_ERR_INVALID: mass range not strictly inside (m_K + m_pi, m_B - m_psi),
+ * cos_max outside (0, 1], negative or non-finite f_max, null outputs; AMP_ERR_STATE: no parameters, P != 1, or lineshape
+ * columns forced (amp_set_lineshape_mode 1); AMP_ERR_DOMAIN: a candidate weight is not finite.                              */
+amp_status amp_generate(amp_model* m, unsigned long long seed, unsigned long long first, long long n_candidates,
+                        double f_max, double m_lo, double m_hi, double cos_max,
+                        double* d_x_out, long long* d_index_out, long long capacity,
+                        long long* h_n_accepted, double* h_f_seen_max, void* stream);
+
 /* Background and signal purity, Eq. 14: with a background set, amp_nll returns
  *   NLL(p) = - sum_i log( purity * eps_i S_i(p) / I(p) + (1 - purity) * b_i ).
  *   d_bkg device [n]: the normalised background density b(Phi_i) >= 0 at the loaded data events (copied), or NULL to go back

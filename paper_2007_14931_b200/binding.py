@@ -18,7 +18,7 @@ AMP_MAX_RESONANCES, AMP_MAX_COUPLINGS, AMP_MAX_POINTS = 16, 48, 256
 # every symbol include/amp.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
-    "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_grad", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
+    "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_grad", "amp_generate", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
     "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_fit_fractions", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode",
     "amp_last_call_stats", "amp_last_call_timing", "amp_recent_launch_ms", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
 ]
@@ -63,6 +63,7 @@ def lib():
         "amp_set_params": (i, [vp, i, vp, vp]),
         "amp_nll": (i, [vp, vp, vp]),
         "amp_nll_grad": (i, [vp, vp, vp, vp]),
+        "amp_generate": (i, [vp, C.c_ulonglong, C.c_ulonglong, ll, d, d, d, d, vp, vp, ll, C.POINTER(ll), pd, vp]),
         "amp_nll_terms": (i, [vp, vp, vp, vp]),
         "amp_dataset_sums": (i, [vp, C.POINTER(ll), pd, C.POINTER(ll), pd]),
         "amp_eval_events": (i, [vp, i, vp, vp]),
@@ -195,6 +196,40 @@ class Model:
         nll, grad = np.empty(1), np.empty((self.K, 2))
         self._check(lib().amp_nll_grad(self._h, nll.ctypes.data_as(C.c_void_p), grad.ctypes.data_as(C.c_void_p), _stream_ptr(stream)), "amp_nll_grad")
         return nll[0], grad
+
+    def generate(self, seed, first, n_candidates, f_max, m_lo, m_hi, cos_max, capacity, with_index=False, stream=None):
+        """accept-reject toy block (amp_generate): -> (x_out cuda [4][capacity], index cuda [capacity] or None, n_accepted, f_seen_max);
+        only the first min(n_accepted, capacity) columns are meaningful"""
+        import torch
+        x_out = torch.empty((4, max(capacity, 1)), dtype=torch.float64, device="cuda")[:, :capacity]
+        idx = torch.empty(max(capacity, 1), dtype=torch.int64, device="cuda")[:capacity] if with_index else None
+        nacc, fseen = C.c_longlong(), C.c_double()
+        self._check(lib().amp_generate(self._h, int(seed), int(first), int(n_candidates), float(f_max), float(m_lo), float(m_hi), float(cos_max),
+                                       C.c_void_p(x_out.data_ptr()) if capacity else None, C.c_void_p(idx.data_ptr()) if (with_index and capacity) else None,
+                                       int(capacity), C.byref(nacc), C.byref(fseen), _stream_ptr(stream)), "amp_generate")
+        return x_out, idx, nacc.value, fseen.value
+
+    def generate_toy(self, n_events, seed, m_lo, m_hi, cos_max, f_max=None, block=1 << 22, safety=1.5):
+        """n_events toy events [4][n_events] (cuda), the first n_events accepted candidates of the stream `seed`.
+        f_max None: taken as safety x the largest weight among the first 2^18 candidates (a pilot pass that writes nothing);
+        returns (x, n_candidates_used, f_max, f_seen_max) — f_seen_max > f_max means the envelope was too low"""
+        import torch
+        if f_max is None:
+            _, _, _, fs = self.generate(seed, 0, 1 << 18, 0.0, m_lo, m_hi, cos_max, 0)
+            f_max = safety * fs
+        out = torch.empty((4, n_events), dtype=torch.float64, device="cuda")
+        have, first, fseen = 0, 0, 0.0
+        while have < n_events:
+            x, _, nacc, fs = self.generate(seed, first, block, f_max, m_lo, m_hi, cos_max, n_events - have)
+            take = min(nacc, n_events - have)
+            out[:, have:have + take] = x[:, :take]
+            have += take
+            fseen = max(fseen, fs)
+            if have < n_events:
+                first += block
+            if nacc == 0 and first > (1 << 40):
+                raise AmpError("generate_toy: nothing accepted")
+        return out, first + block, f_max, fseen
 
     def nll_terms(self, stream=None):
         """(sum_i log S_i(p), sum_j w_j S_j(p)) of this model's own events, [P] each: the per-shard sums behind nll()"""

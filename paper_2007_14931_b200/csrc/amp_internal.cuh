@@ -332,6 +332,27 @@ struct GradArgs {
     double* result;                     // [3 + 2 K]: NLL, I, domain flag, then (dNLL/dRe c_k, dNLL/dIm c_k); may be mapped host memory
 };
 cudaError_t launch_grad(const GradArgs& g, int grid, cudaStream_t s);
+
+// toy.cu — accept-reject toy generator: one block of candidates
+struct ToyArgs {
+    unsigned long long seed, first;   // Philox key; number of this block's first candidate
+    long long n;                      // candidates in the block
+    double m_lo, m_span, cos_max, f_max;
+    double* x;                        // [4][n] candidate points (written by k_toy_candidates)
+    double* u;                        // [n] acceptance uniforms
+    const double* S;                  // [n] signal density of the candidates (streaming kernel, MODE_EVAL, weight 1)
+    const double* cache;              // the candidates' kinematics cache (q and p_B columns are read)
+    int ncolw;
+    int* count;                       // [blocks + 1] accepted per block -> exclusive offsets, total last
+    unsigned long long* f_seen;       // bits of the largest weight seen
+    int* flag;
+    double* x_out;                    // [4][capacity] accepted events, candidate order
+    long long* index_out;             // [capacity] their candidate numbers, or null
+    long long capacity, out_base;     // out_base: accepted before this block
+};
+int toy_blocks(long long n);
+cudaError_t launch_toy_candidates(const ToyArgs& t, cudaStream_t s);
+cudaError_t launch_toy_select(const ToyArgs& t, cudaStream_t s);
 int grad_grid(long long n_data, long long n_norm);
 bool grad_fits(int nent, int ngrp);
 

@@ -188,17 +188,24 @@ void free_dataset(Dataset& d) {
     d = Dataset{};
 }
 
-amp_status load_dataset(amp_model* m, Dataset& d, bool is_norm, const double* d_x, const double* d_w, long long n, cudaStream_t s) {
+// `scratch`: d is a private work set of the caller (the toy generator's candidates): the model's own data / normalisation state is
+// left alone and an allocation of the right size is reused
+amp_status load_dataset(amp_model* m, Dataset& d, bool is_norm, const double* d_x, const double* d_w, long long n, cudaStream_t s, bool scratch = false) {
     if (!m) return AMP_ERR_INVALID;
     if (n < 0 || (n > 0 && !d_x)) return fail(m, AMP_ERR_INVALID, "load: null events or negative count");
-    free_dataset(d);
-    for (auto& e : m->pool) (is_norm ? e.valid_norm : e.valid_data) = false;
-    if (is_norm) m->gram_valid = false;
-    if (!is_norm) { if (m->d_bkg) cudaFree(m->d_bkg); m->d_bkg = nullptr; m->has_bkg = false; m->purity = 1.0; }   // belongs to the old data set
+    const long long npad = stream_pad(n > 0 ? n : 1);
+    const bool reuse = scratch && d.cache && d.npad == npad;
+    if (!reuse) free_dataset(d);
+    if (!scratch) {
+        for (auto& e : m->pool) (is_norm ? e.valid_norm : e.valid_data) = false;
+        if (is_norm) m->gram_valid = false;
+        if (!is_norm) { if (m->d_bkg) cudaFree(m->d_bkg); m->d_bkg = nullptr; m->has_bkg = false; m->purity = 1.0; }   // belongs to the old data set
+    }
     d.n = n;
-    d.npad = stream_pad(n > 0 ? n : 1);
+    d.npad = npad;
     d.ncache = m->has_z ? NCOL_ALL : NCOL_K;
-    CK(cudaMalloc(&d.cache, sizeof(double) * (d.ncache + 1) * d.npad));   // tiled: [npad / 512][ncache + 1][512], weight last
+    d.loaded = false;
+    if (!reuse) CK(cudaMalloc(&d.cache, sizeof(double) * (d.ncache + 1) * d.npad));   // tiled: [npad / 512][ncache + 1][512], weight last
     CK(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
     const int grid = kinematics_grid(d.npad);
     KinArgs a{};
@@ -1641,6 +1648,97 @@ amp_status amp_eval_events(amp_model* m, int p, double* d_out, void* stream) {
     m->stat_launches++;
     CK(cudaStreamSynchronize(s));
     return AMP_OK;
+}
+
+amp_status amp_generate(amp_model* m, unsigned long long seed, unsigned long long first, long long n_candidates,
+                        double f_max, double m_lo, double m_hi, double cos_max,
+                        double* d_x_out, long long* d_index_out, long long capacity,
+                        long long* h_n_accepted, double* h_f_seen_max, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (n_candidates < 0 || capacity < 0 || (capacity > 0 && !d_x_out) || !h_n_accepted || !h_f_seen_max)
+        return fail(m, AMP_ERR_INVALID, "amp_generate: negative count or null output");
+    if (!(m_lo > m->dk.mK + m->dk.mpi) || !(m_hi < m->dk.MB - m->dk.mpsi) || !(m_lo < m_hi) || !(cos_max > 0.0 && cos_max <= 1.0) ||
+        !(f_max >= 0.0) || !std::isfinite(f_max))
+        return fail(m, AMP_ERR_INVALID, "amp_generate: mass range outside phase space, cos_max outside (0, 1] or bad f_max");
+    if (m->P != 1) return fail(m, AMP_ERR_STATE, "amp_generate: needs one parameter point (amp_set_params with P = 1)");
+    if (!m->stream_inline) return fail(m, AMP_ERR_STATE, "amp_generate: needs lineshapes in registers (amp_set_lineshape_mode 0 or 2)");
+    *h_n_accepted = 0;
+    *h_f_seen_max = 0.0;
+    if (n_candidates == 0) return AMP_OK;
+    m->stat_launches = m->stat_columns = 0;
+    const long long CH = 1LL << 21;                       // candidates per block of work (a multiple of the selection block)
+    const long long ch = n_candidates < CH ? n_candidates : CH;
+    double *d_x = nullptr, *d_u = nullptr, *d_S = nullptr;
+    int* d_count = nullptr;
+    unsigned long long* d_fseen = nullptr;
+    Dataset tmp{};
+    auto cleanup = [&]() {
+        if (d_x) cudaFree(d_x);
+        if (d_u) cudaFree(d_u);
+        if (d_S) cudaFree(d_S);
+        if (d_count) cudaFree(d_count);
+        if (d_fseen) cudaFree(d_fseen);
+        free_dataset(tmp);
+    };
+    cudaError_t e = cudaMalloc(&d_x, sizeof(double) * 4 * ch);
+    if (e == cudaSuccess) e = cudaMalloc(&d_u, sizeof(double) * ch);
+    if (e == cudaSuccess) e = cudaMalloc(&d_S, sizeof(double) * stream_pad(ch));
+    if (e == cudaSuccess) e = cudaMalloc(&d_count, sizeof(int) * (toy_blocks(ch) + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&d_fseen, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_fseen, 0, sizeof(unsigned long long), s);
+    if (e != cudaSuccess) { cleanup(); return cuda_fail(m, e, "amp_generate"); }
+    long long accepted = 0;
+    amp_status st = AMP_OK;
+    for (long long off = 0; off < n_candidates && st == AMP_OK; off += ch) {
+        const long long nc = n_candidates - off < ch ? n_candidates - off : ch;
+        ToyArgs t{};
+        t.seed = seed;
+        t.first = first + (unsigned long long)off;
+        t.n = nc;
+        t.m_lo = m_lo;
+        t.m_span = m_hi - m_lo;
+        t.cos_max = cos_max;
+        t.f_max = f_max;
+        t.x = d_x;
+        t.u = d_u;
+        t.S = d_S;
+        t.count = d_count;
+        t.f_seen = d_fseen;
+        t.flag = m->d_flag;
+        t.x_out = d_x_out;
+        t.index_out = d_index_out;
+        t.capacity = capacity;
+        t.out_base = accepted;
+        e = launch_toy_candidates(t, s);
+        if (e != cudaSuccess) { st = cuda_fail(m, e, "amp_generate"); break; }
+        st = load_dataset(m, tmp, true, d_x, nullptr, nc, s, true);      // kinematics cache of the candidates, weight 1
+        if (st != AMP_OK) break;
+        StreamArgs a;
+        fill_stream_args(m, tmp, 0, MODE_EVAL, &a);
+        a.out = d_S;
+        e = launch_stream(a, stream_grid(nc, m->has_z, MODE_EVAL), s);
+        t.cache = tmp.cache;
+        t.ncolw = tmp.ncache + 1;
+        if (e == cudaSuccess) e = cudaMemsetAsync(m->d_flag, 0, sizeof(int), s);
+        if (e == cudaSuccess) e = launch_toy_select(t, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(m->h_pinned, d_count + toy_blocks(nc), sizeof(int), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(m->h_pinned + 1, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(m->h_pinned + 2, d_fseen, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) { st = cuda_fail(m, e, "amp_generate"); break; }
+        m->stat_launches += 6;
+        int cnt, flag;
+        std::memcpy(&cnt, m->h_pinned, sizeof(int));
+        std::memcpy(&flag, m->h_pinned + 1, sizeof(int));
+        std::memcpy(h_f_seen_max, m->h_pinned + 2, sizeof(double));
+        if (flag) { st = fail(m, AMP_ERR_DOMAIN, "amp_generate: a candidate weight p_B q S is not finite"); break; }
+        accepted += cnt;
+    }
+    cleanup();
+    CK(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
+    *h_n_accepted = accepted;
+    return st;
 }
 
 static const char* const kColNames[NCOL_ALL] = {"m2", "inv_m", "q", "pB", "cosK", "sinK", "cosPsi", "sinPsi", "cosPhi", "sinPhi",

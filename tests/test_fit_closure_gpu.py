@@ -69,3 +69,49 @@ def test_fit_recovers_generated_couplings(cfg):
     assert np.median(dev_rel) < 0.12, np.median(dev_rel)
     sizeable = np.array([ff_true[slots[k][0]] > 0.05 for k in range(len(c_true))])
     assert np.max(dev_rel[sizeable]) < 0.3, dev_rel[sizeable]
+
+
+def test_generate_on_device_then_fit_one_million_events():
+    """The paper's validation at its own size ("a pseudo-data sample of one million events is generated with the ten
+    K*s ... masses and widths fixed"), generated AND fitted on the device: amp_generate draws the toy from the true couplings,
+    the host thins it by the efficiency (a detector simulation's job), the fit starts from perturbed couplings."""
+    from paper_2007_14931_b200 import binding as B
+    from paper_2007_14931_b200 import fit as F
+    cfg = 1
+    res = W.resonances(cfg)
+    slots = W.slot_table(res)
+    c_true = W.couplings(cfg)
+    lo, hi, cm = W.DECAY[2] + W.DECAY[3] + W.M_LO_MARGIN, W.M_HI, W.COS_MAX
+    Mg = B.Model(W.DECAY, res)
+    Mg.set_params(c_true)
+    xt, used, fmax, fseen = Mg.generate_toy(2_100_000, 20210301, lo, hi, cm)
+    assert fseen <= fmax
+    xt = xt.cpu().numpy()
+    eps = W.efficiency(cfg, xt)
+    keep = np.random.default_rng(11).uniform(0, 1, xt.shape[1]) < eps          # eps <= 1
+    x, eff = xt[:, keep][:, :1_000_000], eps[keep][:1_000_000]
+    assert x.shape[1] == 1_000_000
+    xn, wn = W.norm_events(cfg, 2_000_000)
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    fixed = [k for k, (r, lam) in enumerate(slots) if r == 1 and lam == 0]
+    n_free = 2 * (len(c_true) - len(fixed))
+    Mg.set_params(c_true)
+    nll_true = Mg.nll()[0]
+    rng = np.random.default_rng(6)
+    start = c_true * (1 + 0.3 * rng.uniform(-1, 1, c_true.size)) * np.exp(0.3j * rng.uniform(-1, 1, c_true.size))
+    for k in fixed:
+        start[k] = c_true[k]
+    r = F.fit_couplings(Mg, start, fixed=fixed)
+    assert r.converged, r
+    lr = 2.0 * (nll_true - r.nll)
+    # Wilks: chi2(n_free), plus the bias of a finite normalisation sample (2e6 points for 1e6 events), which the bound leaves room for
+    assert -1e-6 < lr < n_free + 8.0 * np.sqrt(2.0 * n_free) + 40.0, (lr, n_free)
+    Mg.set_norm_mode(2)
+    Mg.set_params(r.couplings)
+    ff_fit = Mg.fit_fractions(0)
+    Mg.set_params(c_true)
+    ff_true = Mg.fit_fractions(0)
+    assert np.max(np.abs(ff_fit - ff_true)) < 0.01, (ff_fit, ff_true)
+    dev_rel = np.abs(r.couplings - c_true) / np.abs(c_true)
+    assert np.median(dev_rel) < 0.06, np.median(dev_rel)
