@@ -33,7 +33,10 @@
 
 namespace {
 
-enum Kind { KSTAR = 0, ZRES = 1, CONSTANT = 2, LASS = 3 };
+enum Kind { KSTAR = 0, ZRES = 1, CONSTANT = 2, LASS = 3, ZNEG = 4 };
+// ZRES: an exotic Z -> J/psi pi of POSITIVE parity (the paper's default 1+; also 2+); ZNEG: of negative parity (0-, 1-, 2-).
+// PAPER.md:171 ("J(Z) is the spin of the Z"), 314 ("any combination of their spin-parity values"); reading A24.
+inline bool is_z(int kind) { return kind == ZRES || kind == ZNEG; }
 
 template <typename T>
 struct Decay {
@@ -81,8 +84,15 @@ T blatt_weisskopf(int L, T p, T p0, T r) {
 
 // ---------------------------------------------------------------------------------
 // Orbital angular momenta ("lowest L_B is taken as the default"; readings A5, A6).
+// Z chain (reading A24): B(0-) -> Z(J) K(0-) has L_B = J (angular momentum alone; the weak decay does not conserve parity);
+// Z(J^P) -> psi(1-) pi(0-) is a strong decay: P = (+1)(-1)^L_R with |L_R - 1| <= J <= L_R + 1, lowest such L_R taken:
+//   1+: 0,  2+: 2,  0-: 1,  1-: 1,  2-: 1   (0+ cannot decay to psi pi).
 inline void orbital_L(int kind, int J, int* LB, int* LR) {
-    if (kind == ZRES) { *LB = 1; *LR = 0; return; }   // 1+ Z: B -> Z K P-wave, Z -> psi pi S-wave
+    if (is_z(kind)) {
+        *LB = J;
+        *LR = (kind == ZRES) ? (J == 1 ? 0 : 2) : 1;
+        return;
+    }
     *LR = J;                                           // K* -> K pi
     *LB = (J == 0) ? 1 : J - 1;                        // B(0-) -> psi(1-) K*(J): lowest allowed
 }
@@ -253,7 +263,7 @@ struct Model {
     std::vector<Resonance<T>> res;
     int num_couplings() const {
         int K = 0;
-        for (auto& r : res) K += (r.kind == ZRES || (r.kind == KSTAR && r.J >= 1)) ? 3 : 1;
+        for (auto& r : res) K += (is_z(r.kind) || (r.kind == KSTAR && r.J >= 1)) ? 3 : 1;
         return K;
     }
 };
@@ -284,7 +294,7 @@ EventAngles<T> event_angles(const Model<T>& M, const T x[4]) {
     const T thK = std::atan2(std::sqrt((1 - cK) * (1 + cK)), cK);
     const T thpsi = std::atan2(std::sqrt((1 - cpsi) * (1 + cpsi)), cpsi);
     for (const auto& R : M.res) {
-        if (R.kind == ZRES) {
+        if (is_z(R.kind)) {
             if (!a.haveZ) {
                 const ZKinematics<T> zk = z_kinematics(M.dk, m, cK, cpsi, phi);
                 const T thT = std::atan2(zk.sinT, zk.cosT);
@@ -317,7 +327,7 @@ void basis_terms(const Model<T>& M, const EventAngles<T>& a, std::complex<T>* ou
     using C = std::complex<T>;
     int k = 0;
     for (const auto& R : M.res) {
-        if (R.kind == ZRES) {
+        if (is_z(R.kind)) {
             const C A = lineshape(M.dk, R, a.mZ);
             for (int lp = -1; lp <= 1; ++lp, ++k)
                 for (int ix = 0; ix < 2; ++ix)
@@ -592,7 +602,7 @@ void orc_z_kinematics(const double* decay, const double* x /*[4]*/, int prec, do
 
 int orc_num_couplings(int n_res, const int* kinds, const int* Js) {
     int K = 0;
-    for (int r = 0; r < n_res; ++r) K += (kinds[r] == ZRES || (kinds[r] == KSTAR && Js[r] >= 1)) ? 3 : 1;
+    for (int r = 0; r < n_res; ++r) K += (is_z(kinds[r]) || (kinds[r] == KSTAR && Js[r] >= 1)) ? 3 : 1;
     return K;
 }
 

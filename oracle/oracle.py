@@ -38,7 +38,7 @@ _lib.orc_nll.argtypes = _MODEL + [_i, _pd, _vp, _pd, _vp, _ll, _pd, _vp, _ll, _i
 _lib.orc_norm_matrix.argtypes = _MODEL + [_pd, _vp, _ll, _pd]
 _lib.orc_nll_gradient.argtypes = _MODEL + [_pd, _pd, _vp, _ll, _pd, _vp, _ll, _pd, _pd]
 
-KSTAR, ZRES, CONST, LASS = 0, 1, 2, 3
+KSTAR, ZRES, CONST, LASS, ZNEG = 0, 1, 2, 3, 4
 
 
 def num_threads():
@@ -195,7 +195,7 @@ class Model:
         assert c.shape == (self.K,)
         slot_res = []
         for r in range(self.R):
-            three = self.kinds[r] == ZRES or (self.kinds[r] == KSTAR and self.Js[r] >= 1)
+            three = self.kinds[r] in (ZRES, ZNEG) or (self.kinds[r] == KSTAR and self.Js[r] >= 1)
             slot_res += [r] * (3 if three else 1)
         slot_res = np.array(slot_res)
         groups = [[r] for r in range(self.R)] if groups is None else groups

@@ -683,3 +683,81 @@ def test_P19_toy_of_constant_spin0_model_follows_phase_space():
     # accepted events are denser where the weight is larger: mean weight of accepted = <f^2>/<f> > <f>
     assert np.mean(f2[g2["index"]]) > 1.5 * np.mean(f2)
     assert abs(np.mean(f2[g2["index"]]) / (np.mean(f2 ** 2) / np.mean(f2)) - 1) < 5 * math.sqrt(np.var(f2[g2["index"]]) / g2["x"].shape[1]) / np.mean(f2[g2["index"]])
+
+
+# ------------------------------------------------------------------ P20: Z of any spin-parity (reading A24)
+Z_CLASSES = [(O.ZRES, 1), (O.ZRES, 2), (O.ZNEG, 0), (O.ZNEG, 1), (O.ZNEG, 2)]
+
+
+def test_P20_z_orbital_momenta_from_selection_rules():
+    """L_B, L_R of each J^P by brute-force enumeration of the selection rules: L_B couples spin J and spin 0 to the B's spin 0;
+    L_R couples the psi's spin 1 to J with parity P = P_psi P_pi (-1)^L = (-1)^L; the lowest allowed value is taken"""
+    for kind, J in Z_CLASSES:
+        P = +1 if kind == O.ZRES else -1
+        LBs = [L for L in range(0, 8) if abs(L - J) <= 0 <= L + J]                     # |L - J| <= 0 <= L + J
+        LRs = [L for L in range(0, 8) if abs(L - 1) <= J <= L + 1 and (-1) ** L == P]
+        assert O.orbital_L(kind, J) == (min(LBs), min(LRs)), (kind, J)
+    assert [L for L in range(0, 8) if abs(L - 1) <= 0 <= L + 1 and (-1) ** L == +1] == []   # 0+ -> psi pi is forbidden
+
+
+@pytest.mark.parametrize("kind,J", Z_CLASSES)
+def test_P20_z_spin_parity_lineshape_and_integral(kind, J):
+    res = [(kind, J, 4196.0, 370.0, R16)]
+    M = O.Model(DEC, res)
+    LB, LR = O.orbital_L(kind, J)
+    # pole: Gamma(M) = Gamma0 and A = (pB0/MB)^LB (pR0/M)^LR i/(M Gamma0) (the barrier factors are 1 at the pole)
+    A, G = M.lineshape(0, 4196.0)
+    pB0, pR0 = O.breakup_momentum(MB, 4196.0, MK), O.breakup_momentum(4196.0, MPSI, MPI)
+    assert abs(G - 370.0) < 1e-12 * 370.0
+    ref = (pB0 / MB) ** LB * (pR0 / 4196.0) ** LR * 1j / (4196.0 * 370.0)
+    assert abs(A - ref) < 1e-13 * abs(ref)
+    # threshold behaviour of the momentum powers: |A| ~ pR^LR near the psi pi threshold
+    m1, m2 = MPSI + MPI + 0.02, MPSI + MPI + 0.08
+    r = abs(M.lineshape(0, m2)[0]) / abs(M.lineshape(0, m1)[0])
+    p1, p2 = O.breakup_momentum(m1, MPSI, MPI), O.breakup_momentum(m2, MPSI, MPI)
+    assert abs(r - (p2 / p1) ** LR) < 2e-3 * r
+    # phase-space integral of the Z-only density: (2/3) (1/(2J+1)) sum_{|l'| <= J} |H_l'|^2 <|A^Z|^2>  (orthogonality of the d's)
+    H = np.array([0.8 * np.exp(0.4j), 1.3 * np.exp(-2.0j), 0.6 * np.exp(1.9j)])
+    x, w = quadrature_events(64, 64, 4, 8)
+    pqZ = lambda mz: O.breakup_momentum(MB, mz, MK) * O.breakup_momentum(mz, MPSI, MPI)
+    lo, hi = MPSI + MPI, MB - MK
+    num = integrate.quad(lambda mz: abs(M.lineshape(0, mz)[0]) ** 2 * pqZ(mz), lo, hi, epsabs=0, epsrel=1e-11, limit=400)[0]
+    den = integrate.quad(pqZ, lo, hi, epsabs=0, epsrel=1e-11, limit=400)[0]
+    for l in range(3):
+        Hl = np.zeros(3, complex)
+        Hl[l] = H[l]
+        Il = M.norm_integral(Hl, x, w)[0]
+        ref = (2.0 / 3.0) / (2 * J + 1) * abs(H[l]) ** 2 * num / den if abs(l - 1) <= J else 0.0
+        assert abs(Il - ref) <= 2e-5 * max(ref, 1e-300), (l, Il, ref)
+    # helicities do not interfere in the integral
+    Iall = M.norm_integral(H, x, w)[0]
+    assert abs(Iall - sum(M.norm_integral(np.where(np.arange(3) == l, H, 0), x, w)[0] for l in range(3))) < 1e-9 * Iall
+
+
+def test_P20_spin0_z_density_closed_form():
+    """0- Z alone: S = |H_0 A^Z(m_psipi)|^2 sin^2(theta~) — no dependence on theta_Z, phi~ or alpha; the lambda' = +-1 slots are inert"""
+    M = O.Model(DEC, [(O.ZNEG, 0, 4196.0, 370.0, R16)])
+    xn, _ = W.norm_events(2, 400)
+    H = np.array([0.3 + 0.2j, 0.9 - 0.5j, -0.7j])
+    S = M.eval_events(H, xn)
+    for i in range(0, 400, 7):
+        zk = M.z_kinematics(xn[:, i])
+        A = M.lineshape(0, zk["mZ"])[0]
+        ref = abs(H[1] * A) ** 2 * zk["sinT"] ** 2
+        assert abs(S[i] - ref) < 1e-12 * ref
+    assert np.array_equal(S, M.eval_events(np.array([0, H[1], 0]), xn))
+    # spin 2: d^2_{00}(theta_Z)^2 sin^2(theta~) for lambda' = 0 alone (sympy value of the d function)
+    from sympy import N
+    from sympy.physics.quantum.spin import Rotation
+    M2 = O.Model(DEC, [(O.ZRES, 2, 4196.0, 370.0, R16)])
+    S2 = M2.eval_events(np.array([0, 1.0, 0]), xn)
+    S2p = M2.eval_events(np.array([0, 0, 1.0]), xn)
+    for i in range(0, 400, 41):
+        zk = M2.z_kinematics(xn[:, i])
+        A = M2.lineshape(0, zk["mZ"])[0]
+        thZ, thT = math.atan2(zk["sinZ"], zk["cosZ"]), math.atan2(zk["sinT"], zk["cosT"])
+        d200 = float(N(Rotation.d(2, 0, 0, thZ).doit(), 30))
+        d201 = float(N(Rotation.d(2, 0, 1, thZ).doit(), 30))
+        assert abs(S2[i] - abs(A) ** 2 * d200 ** 2 * zk["sinT"] ** 2) < 1e-11 * S2[i] + 1e-40
+        d1p = sum(float(N(Rotation.d(1, 1, xi, thT).doit(), 30)) ** 2 for xi in (1, -1))
+        assert abs(S2p[i] - abs(A) ** 2 * d201 ** 2 * d1p) < 1e-11 * S2p[i] + 1e-40
