@@ -43,15 +43,21 @@ typedef enum {
 } amp_status;
 
 /* Resonance kinds.  AMP_KSTAR: K* -> K pi, Eq. 4.  AMP_Z: Z -> J/psi pi evaluated in
- * its own decay frame, Eq. 10; only J^P = 1+ (PAPER.md:171).  AMP_CONST: lineshape == 1,
+ * its own decay frame, Eq. 10, of POSITIVE parity: J^P = 1+ (the paper's default) or 2+;
+ * AMP_ZM: the same of NEGATIVE parity: 0-, 1-, 2- ("any combination of their spin-parity values").  Orbital
+ * momenta of the Z chain: L_B = J; L_R = lowest L with (-1)^L = P and |L - 1| <= J <= L + 1 (1+: 0, 2+: 2, 0-/1-/2-: 1; 0+
+ * does not decay to J/psi pi and is refused).  A Z always has three coupling slots lambda' = -1, 0, +1 (for J = 0 the
+ * lambda' = +-1 slots multiply a zero d function); Eq. 11's relation between them is the caller's.  The fused shape-specialised
+ * kernels and the gradient-batch kernel cover 1+ Zs; other spin-parities run the generic streaming kernel and, for parameter
+ * batches, the dense path.  AMP_CONST: lineshape == 1,
  * J = 0, angular factor d^1_{0 xi}(theta_psi) (BASELINE.json configs[0], "constant S-wave term").
  * AMP_LASS: the LASS parametrisation of the K pi S-wave, Eqs. 7-9: J = 0, one coupling slot,
  * lineshape A_LASS built on mass = M(K0*(1430)), width = Gamma(K0*(1430)) with the paper's a = 1.95 GeV^-1,
  * b = 1.76 GeV^-1 (Eq. 8); radius is ignored.  Models with a LASS term run the generic streaming kernel; gradient
  * batches of such models take the dense path.                                                          */
-typedef enum { AMP_KSTAR = 0, AMP_Z = 1, AMP_CONST = 2, AMP_LASS = 3 } amp_kind;
+typedef enum { AMP_KSTAR = 0, AMP_Z = 1, AMP_CONST = 2, AMP_LASS = 3, AMP_ZM = 4 } amp_kind;
 
-/* One resonance: spin J (K*: 0..4, Z: 1, CONST: 0), nominal mass M_R and width
+/* One resonance: spin J (K*: 0..4, AMP_Z: 1..2, AMP_ZM: 0..2, CONST: 0), nominal mass M_R and width
  * Gamma_0 [MeV], Blatt-Weisskopf radius r [MeV^-1] used for both F_B and F_R of Eq. 2 (PAPER.md:89,
  * 103).  Orbital momenta: K*: L_R = J, L_B = J-1 (J >= 1) or 1 (J = 0), the lowest allowed
  * (PAPER.md:107); Z: L_B = 1, L_R = 0.                                                               */

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("AMP4D_LIB", os.path.join(HERE, "libamp4d.so"))   # override: experiments with kernel variants
 
 AMP_OK, AMP_ERR_INVALID, AMP_ERR_STATE, AMP_ERR_DOMAIN, AMP_ERR_CUDA, AMP_ERR_NOMEM = range(6)
-AMP_KSTAR, AMP_Z, AMP_CONST, AMP_LASS = 0, 1, 2, 3
+AMP_KSTAR, AMP_Z, AMP_CONST, AMP_LASS, AMP_ZM = 0, 1, 2, 3, 4
 AMP_MAX_RESONANCES, AMP_MAX_COUPLINGS, AMP_MAX_POINTS = 16, 48, 256
 
 # every symbol include/amp.h declares (tests/test_abi.py checks the header against this list and the .so)

@@ -51,6 +51,16 @@ struct DecayConst {
 //   F_B F_R          = kF rs                      kF  = sqrt(B_LR(zR0) B_LB(zB0))
 //   numerator        = kN rs pB^LB (pR/m)^LR      kN  = kF / MB^LB
 //   M_R Gamma(m)     = kG pR^(2LR+1) (1/m) rs^2 B_LB(zB),   kG = M_R^2 Gamma0 B_LR(zR0) / pR0^(2LR+1)
+// Spin classes of the streaming kernels: the K* spins J = 0..4, then the Z spin-parities (A24):
+//   class 5: 1+ (the paper's default)   6: 2+   7: 0-   8: 1-   9: 2-
+// B -> Z K has L_B = J; Z -> psi pi takes the lowest L_R with (-1)^L_R = P and |L_R - 1| <= J <= L_R + 1.
+constexpr int NZCLASS = 5, NSPIN = 5 + NZCLASS;
+__host__ __device__ __forceinline__ bool kind_is_z(int kind) { return kind == AMP_Z || kind == AMP_ZM; }
+__host__ __device__ __forceinline__ int z_class(int kind, int J) { return kind == AMP_Z ? (J == 1 ? 0 : 1) : 2 + J; }
+__host__ __device__ __forceinline__ int z_class_kind(int zc) { return zc < 2 ? AMP_Z : AMP_ZM; }
+__host__ __device__ __forceinline__ int z_class_J(int zc) { return zc == 0 ? 1 : (zc == 1 ? 2 : zc - 2); }
+__host__ __device__ __forceinline__ int z_class_LR(int zc) { return zc == 0 ? 0 : (zc == 1 ? 2 : 1); }
+
 struct LineConst {
     int kind, LR, LB, chain;  // chain: 0 = K pi (K*), 1 = psi pi (Z), 2 = constant
     double M2, r2, kN, kG;
@@ -242,10 +252,10 @@ struct StreamArgs {
     ResEntry ent[AMP_MAX_RESONANCES];
     BarrierGroup grp[AMP_MAX_RESONANCES];
     int lass0, nlass;               // LASS terms: entries ent[lass0 .. lass0 + nlass) (kG, M2 and c0 used), after the K* and Z entries
-    int gstart[7];                  // groups of K* spin J: grp[gstart[J] .. gstart[J+1]), J = 0..4; Z groups: gstart[5] .. gstart[6]
-    int shape[6];                   // resonances per K* spin 0..4 and Z's; entries are stored in that order
-    int shape_fixed;                // 1: one radius per spin, r2_spin valid: a shape-specialised kernel may run
-    double r2_spin[6];
+    int gstart[NSPIN + 1];          // groups of spin class sp: grp[gstart[sp] .. gstart[sp+1]); sp = J for the K* (0..4), 5 + z_class for the Z's
+    int shape[NSPIN];               // resonances per spin class; entries are stored in that order
+    int shape_fixed;                // 1: one radius per spin class, r2_spin valid: a shape-specialised kernel may run
+    double r2_spin[NSPIN];
     double2 cconst;                 // sum of the couplings of the constant (lineshape == 1) terms
     const double* cache;            // tiled cache of the (first) sample, ncolw columns per 512-event block
     int ncolw;

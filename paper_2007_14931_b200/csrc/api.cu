@@ -162,8 +162,8 @@ bool make_line_const(const amp_model* m, int r, double mass, double width, LineC
         pB0 = h_two_body(m->dk.MB, mass, m->dk.mpsi);
     } else {
         c.chain = 1;
-        c.LR = 0;                                                // 1+ Z -> psi pi in S wave
-        c.LB = 1;                                                // B -> Z K in P wave
+        c.LR = z_class_LR(z_class(R.kind, R.J));                 // 1+ Z -> psi pi in S wave; the other spin-parities: amp_internal.cuh
+        c.LB = R.J;                                              // B -> Z K: L_B = J (P wave for the 1+)
         pR0 = h_two_body(mass, m->dk.mpsi, m->dk.mpi);
         pB0 = h_two_body(m->dk.MB, mass, m->dk.mK);
     }
@@ -276,7 +276,8 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
         const amp_resonance& a = res[r];
         bool ok = true;
         if (a.kind == AMP_KSTAR) ok = a.J >= 0 && a.J <= 4;
-        else if (a.kind == AMP_Z) ok = a.J == 1;
+        else if (a.kind == AMP_Z) ok = a.J == 1 || a.J == 2;      // 1+, 2+ (0+ cannot decay to psi pi)
+        else if (a.kind == AMP_ZM) ok = a.J >= 0 && a.J <= 2;       // 0-, 1-, 2-
         else if (a.kind == AMP_CONST) ok = a.J == 0;
         else if (a.kind == AMP_LASS) ok = a.J == 0;
         else ok = false;
@@ -284,8 +285,8 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
         if (!ok) { delete m; return AMP_ERR_INVALID; }
         m->res.push_back(a);
         m->slot0[r] = K;
-        K += (a.kind == AMP_Z || (a.kind == AMP_KSTAR && a.J >= 1)) ? 3 : 1;
-        if (a.kind == AMP_Z) m->has_z = true;
+        K += (kind_is_z(a.kind) || (a.kind == AMP_KSTAR && a.J >= 1)) ? 3 : 1;
+        if (kind_is_z(a.kind)) m->has_z = true;
     }
     int nconst = 0;
     for (int r = 0; r < n_res; ++r) nconst += res[r].kind == AMP_CONST;
@@ -485,7 +486,8 @@ bool build_delta_plan(amp_model* m) {
     {
         StreamArgs tmp;
         fill_stream_args(m, m->norm, 0, MODE_FUSED, &tmp, ent_of_res, grp_of_res);
-        if (!delta_fits(tmp.gstart[6])) return false;
+        if (!delta_fits(tmp.gstart[NSPIN])) return false;
+        for (int sp = 6; sp < NSPIN; ++sp) if (tmp.shape[sp]) return false;   // Z's other than 1+: dense path
     }
     size_t total = 0;
     const size_t cap = (size_t)3 * (P - 1) + 8;
@@ -507,7 +509,7 @@ bool build_delta_plan(amp_model* m) {
         int prev_slot = -1;
         auto push = [&](int kind, int slot, int r, double a, double b, double c) {
             DeltaContrib dc{};
-            const bool isz = r >= 0 && m->res[r].kind == AMP_Z;
+            const bool isz = r >= 0 && kind_is_z(m->res[r].kind);
             dc.hdr = kind | (slot != prev_slot ? 8 : 0) | (isz ? 32 : 0) | ((r >= 0 ? grp_of_res[r] : 0) << 8);
             dc.slot = slot;
             dc.a = a; dc.b = b; dc.c = c;
@@ -519,7 +521,7 @@ bool build_delta_plan(amp_model* m) {
             const int p = p0 + q;
             for (int r = 0; q < ch.np && r < R; ++r) {
                 const amp_resonance& rs = m->res[r];
-                const int ns = (rs.kind == AMP_Z || (rs.kind == AMP_KSTAR && rs.J >= 1)) ? 3 : 1;
+                const int ns = (kind_is_z(rs.kind) || (rs.kind == AMP_KSTAR && rs.J >= 1)) ? 3 : 1;
                 const double* c0 = &m->couplings[((size_t)0 * K + m->slot0[r]) * 2];
                 const double* cp = &m->couplings[((size_t)p * K + m->slot0[r]) * 2];
                 bool dcf[3] = {false, false, false}, anyc = false;
@@ -529,7 +531,7 @@ bool build_delta_plan(amp_model* m) {
                 const double* mwp = &m->mw[((size_t)p * R + r) * 2];
                 const bool ls = mwp[0] != mw0[0] || mwp[1] != mw0[1];
                 if (!anyc && !ls) continue;
-                const bool isz = rs.kind == AMP_Z;
+                const bool isz = kind_is_z(rs.kind);
                 const int Jf = isz ? 1 : rs.J;
                 auto term_hdr = [&](int j, bool with_bw, bool unit) {
                     const int l = ns == 3 ? j : 1;   // helicity -1, 0, +1 -> 0, 1, 2
@@ -749,7 +751,7 @@ void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, Str
                 ResEntry& e = a->ent[t++];
                 e.kN = lc.kN; e.kG = lc.kG; e.M2 = lc.M2;
                 const double* cp = &m->couplings[((size_t)p * m->K + m->slot0[r2]) * 2];
-                if (J == 0 && kind == AMP_KSTAR) {
+                if (J == 0 && kind == AMP_KSTAR) {   // one slot (a spin-0 Z keeps three: lambda' = +-1 multiply a zero d function)
                     e.c0 = make_double2(cp[0], cp[1]);
                     e.cm = e.cp = make_double2(0, 0);
                 } else {
@@ -767,9 +769,8 @@ void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, Str
     };
     a->shape_fixed = 1;
     for (int J = 0; J < 5; ++J) { a->gstart[J] = g; add_groups(AMP_KSTAR, J); }
-    a->gstart[5] = g;
-    add_groups(AMP_Z, 1);
-    a->gstart[6] = g;
+    for (int zc = 0; zc < NZCLASS; ++zc) { a->gstart[5 + zc] = g; add_groups(z_class_kind(zc), z_class_J(zc)); }
+    a->gstart[NSPIN] = g;
     a->lass0 = t;
     for (int r = 0; r < m->R; ++r) {
         if (m->res[r].kind != AMP_LASS) continue;
@@ -786,7 +787,7 @@ void fill_stream_args(const amp_model* m, const Dataset& d, int p, int mode, Str
         e.column = (sidx >= 0 && !m->stream_inline) ? sidx : -1;
     }
     a->nlass = t - a->lass0;
-    for (int sp = 0; sp < 6; ++sp) {
+    for (int sp = 0; sp < NSPIN; ++sp) {
         const int ng = a->gstart[sp + 1] - a->gstart[sp];
         a->shape[sp] = 0;
         for (int gg = a->gstart[sp]; gg < a->gstart[sp + 1]; ++gg) a->shape[sp] += a->grp[gg].count;
@@ -854,7 +855,7 @@ bool build_batch_plan(const amp_model* m, int p0, int Pc, BatchPlan* bp) {
     if (2 * K > BATCH_NKT * 4 || Pc > BATCH_POINTS) return false;
     std::vector<int> slot_res(K), slot_lam(K);
     for (int r = 0; r < R; ++r) {
-        const int ns = (m->res[r].kind == AMP_Z || (m->res[r].kind == AMP_KSTAR && m->res[r].J >= 1)) ? 3 : 1;
+        const int ns = (kind_is_z(m->res[r].kind) || (m->res[r].kind == AMP_KSTAR && m->res[r].J >= 1)) ? 3 : 1;
         for (int j = 0; j < ns; ++j) { slot_res[m->slot0[r] + j] = r; slot_lam[m->slot0[r] + j] = ns == 3 ? j - 1 : 0; }
     }
     const int nbase = BATCH_NKT * 2;   // complex base entries incl. padding
@@ -1008,7 +1009,7 @@ bool build_herk_plan(const amp_model* m, HerkPlan* hp, int pbase = 0, int npts =
     const int R = m->R, K = m->K, P = npts < 0 ? m->P : npts;
     std::vector<int> slot_res(K), slot_lam(K);
     for (int r = 0; r < R; ++r) {
-        const int ns = (m->res[r].kind == AMP_Z || (m->res[r].kind == AMP_KSTAR && m->res[r].J >= 1)) ? 3 : 1;
+        const int ns = (kind_is_z(m->res[r].kind) || (m->res[r].kind == AMP_KSTAR && m->res[r].J >= 1)) ? 3 : 1;
         for (int j = 0; j < ns; ++j) { slot_res[m->slot0[r] + j] = r; slot_lam[m->slot0[r] + j] = ns == 3 ? j - 1 : 0; }
     }
     std::vector<int2> ent(K);           // pool column (or -2) and code, base entries
@@ -1556,8 +1557,8 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
     GradArgs g{};
     fill_stream_args(m, m->data, 0, MODE_FUSED, &g.a, ent_of_res, grp_of_res);
     int nent = 0;
-    for (int sp = 0; sp < 6; ++sp) nent += g.a.shape[sp];
-    if (!grad_fits(nent, g.a.gstart[6])) return fail(m, AMP_ERR_INVALID, "amp_nll_grad: the model does not fit the kernel's shared memory");
+    for (int sp = 0; sp < NSPIN; ++sp) nent += g.a.shape[sp];
+    if (!grad_fits(nent, g.a.gstart[NSPIN])) return fail(m, AMP_ERR_INVALID, "amp_nll_grad: the model does not fit the kernel's shared memory");
     g.a.cache2 = m->norm.cache; g.a.n2 = m->norm.n; g.a.npad2 = m->norm.npad;
     g.a.ticket = m->d_ticket;
     g.a.sum_log_eff = m->data.wsum;
@@ -1590,12 +1591,12 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
     for (int p = 0; p < GRAD_MAX_PAIRS; ++p) { g.pair_ent[p] = -2; g.pair_lam[p] = 0; g.pair_J[p] = 0; g.pair_grp[p] = 0; g.pair_slot[p] = -1; }
     for (int r = 0; r < m->R; ++r) {
         const amp_resonance& rs = m->res[r];
-        const int ns = (rs.kind == AMP_Z || (rs.kind == AMP_KSTAR && rs.J >= 1)) ? 3 : 1;
+        const int ns = (kind_is_z(rs.kind) || (rs.kind == AMP_KSTAR && rs.J >= 1)) ? 3 : 1;
         for (int j = 0; j < ns; ++j) {
             const int k = m->slot0[r] + j;
             g.pair_ent[k] = rs.kind == AMP_CONST ? -1 : (signed char)ent_of_res[r];
             g.pair_lam[k] = (signed char)(ns == 3 ? j - 1 : 0);
-            g.pair_J[k] = rs.kind == AMP_Z ? 8 : (signed char)rs.J;
+            g.pair_J[k] = kind_is_z(rs.kind) ? (signed char)(8 + rs.J) : (signed char)rs.J;   // 8 + J: a Z slot of spin J
             g.pair_grp[k] = rs.kind == AMP_CONST ? 0 : (signed char)grp_of_res[r];
             g.pair_slot[k] = (short)k;
         }
@@ -1796,7 +1797,7 @@ amp_status amp_fit_fractions(amp_model* m, int p, double* h_ff, void* stream) {
     std::vector<double2> C((size_t)(R + 1) * nent, make_double2(0, 0));
     for (int e = 0; e < nent; ++e) C[e] = hp.C[e];
     for (int r = 0; r < R; ++r) {
-        const int ns = (m->res[r].kind == AMP_Z || (m->res[r].kind == AMP_KSTAR && m->res[r].J >= 1)) ? 3 : 1;
+        const int ns = (kind_is_z(m->res[r].kind) || (m->res[r].kind == AMP_KSTAR && m->res[r].J >= 1)) ? 3 : 1;
         for (int j = 0; j < ns; ++j) C[(size_t)(1 + r) * nent + m->slot0[r] + j] = hp.C[m->slot0[r] + j];   // single point: entry k = slot k
     }
     hp.C.swap(C);

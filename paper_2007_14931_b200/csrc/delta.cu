@@ -64,7 +64,7 @@ __device__ __forceinline__ void eval_slot(const StreamArgs& a, const double* rec
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             double2 gp, gm;
-            term_angular(J, lam, isz, k[e], zst + e, &gp, &gm);
+            term_angular<true>(J, lam, isz, k[e], zst + e, &gp, &gm);
             if (ent != 255) {
                 const double2 bw = bw_point0(a, ent, grp, isz, k[e], fg + e);
                 gp = cmul(bw, gp);
@@ -272,9 +272,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_delta(const __grid_constant__ De
     const StreamArgs& a = d.a;
     const double RSQRT2 = 0.70710678118654752440;
     const int tid = threadIdx.x, lane = tid & 31;
-    const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[6] > a.gstart[5]);
+    const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[NSPIN] > a.gstart[5]);
     const int ncache = have_z ? NCOL_ALL : NCOL_K;
-    const int ngrp = a.gstart[6];
+    const int ngrp = a.gstart[NSPIN];
     const int nblk = d.nsorted / 32;
 
     // shared memory: staged tile (two regions, as k_stream) | group factors | per-lane point accumulators | the program
@@ -512,8 +512,8 @@ cudaError_t launch_delta_shape(const DeltaArgs& d, int grid, cudaStream_t s) {
     cudaError_t e = cudaSuccess;
     if (!attr_done) { e = cudaFuncSetAttribute(k_delta<SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
     if (e != cudaSuccess) return e;
-    const bool have_z = d.a.gstart[6] > d.a.gstart[5];
-    k_delta<SH><<<grid, THREADS, delta_smem(have_z, d.a.gstart[6]), s>>>(d);
+    const bool have_z = d.a.gstart[NSPIN] > d.a.gstart[5];
+    k_delta<SH><<<grid, THREADS, delta_smem(have_z, d.a.gstart[NSPIN]), s>>>(d);
     return cudaGetLastError();
 }
 

@@ -27,6 +27,8 @@ struct EvK {   // what the point loop keeps of one event in registers
 };
 // Angular factor g_{J,lambda,xi} of one term for one event (Eq. 4 for a K*, Eq. 10 for the Z).
 // zst: this event's element of the staged tile (the Z-chain angles stay there during the point loop).
+// Z1P: every Z of the model is a 1+ (the gradient-batch kernel's plans): d^1_{0 l'} without the spin switch.
+template <bool Z1P = false>
 __device__ __forceinline__ void term_angular(int J, int lam, bool isz, const EvK& k, const double* zst, double2* gp, double2* gm) {
     const double RSQRT2 = 0.70710678118654752440;
     if (!isz) {
@@ -45,10 +47,13 @@ __device__ __forceinline__ void term_angular(int J, int lam, bool isz, const EvK
         }
         return;
     }
-    // d^1_{0 l'}(theta_Z) e^{i l' phi~} d^1_{l' xi}(theta~) e^{i xi alpha}
+    // d^J_{0 l'}(theta_Z) e^{i l' phi~} d^1_{l' xi}(theta~) e^{i xi alpha};  d^J_{0,+1} = -d^J_{+1,0}, d^J_{0,-1} = d^J_{+1,0}
     const double cZ = zst[C_CZ * TILE], sZ = zst[C_SZ * TILE], ct = zst[C_CT * TILE], st = zst[C_ST * TILE];
     const double cpt = zst[C_CPT * TILE], spt = zst[C_SPT * TILE], ca = zst[C_CA * TILE], sa = zst[C_SA * TILE];
-    const double zf = lam == 0 ? cZ : (lam > 0 ? RSQRT2 * sZ : -RSQRT2 * sZ);
+    double z0, z1;
+    if (Z1P) { z0 = cZ; z1 = -RSQRT2 * sZ; }
+    else dJ(J, cZ, sZ, &z0, &z1);
+    const double zf = lam == 0 ? z0 : (lam > 0 ? -z1 : z1);
     const double dp = lam == 0 ? RSQRT2 * st : (lam > 0 ? 0.5 * (1.0 + ct) : 0.5 * (1.0 - ct));
     const double dm = lam == 0 ? -RSQRT2 * st : (lam > 0 ? 0.5 * (1.0 - ct) : 0.5 * (1.0 + ct));
     const double2 eph = lam == 0 ? make_double2(1.0, 0.0) : make_double2(cpt, lam > 0 ? spt : -spt);

@@ -43,10 +43,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
     const StreamArgs& a = g.a;
     const double RSQRT2 = 0.70710678118654752440, LN2 = 0.69314718055994530942;
     const int tid = threadIdx.x, lane = tid & 31;
-    const bool have_z = a.gstart[6] > a.gstart[5];
+    const bool have_z = a.gstart[NSPIN] > a.gstart[5];
     const int ncache = have_z ? NCOL_ALL : NCOL_K;
     int nent = 0;
-    for (int sp = 0; sp < 6; ++sp) nent += a.shape[sp];
+    for (int sp = 0; sp < NSPIN; ++sp) nent += a.shape[sp];
     const int nleaf = 2 * g.npairs, nblk = nleaf / 32;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -131,14 +131,27 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
             mbar_wait(&full[1], parity);
             k.mZ2 = st[C_MZ2 * TILE];
             const double invmZ = st[C_INVMZ * TILE], qZ = st[C_QZ * TILE], pBZ = st[C_PBZ * TILE];
-            double2 Um = make_double2(0, 0), U0 = Um, Up = Um;
-            spin_class<1, 0, 1>(a, 5, k.mZ2, invmZ, qZ, pBZ, bw_rec, Um, U0, Up);
             const double cZ = st[C_CZ * TILE], sZ = st[C_SZ * TILE], ct = st[C_CT * TILE], stt = st[C_ST * TILE];
             const double cpt = st[C_CPT * TILE], spt = st[C_SPT * TILE], ca = st[C_CA * TILE], sa = st[C_SA * TILE];
-            const double z1 = RSQRT2 * sZ;
-            const double2 T0 = cscale(cZ, U0);
-            const double2 Tp = cscale(z1, cmul(make_double2(cpt, spt), Up));
-            const double2 Tm = cscale(-z1, cmul(make_double2(cpt, -spt), Um));
+            // sum over the Z spin classes of d^J_{0 l'}(theta_Z) U_l' (d^J_{0,+1} = -d^J_{+1,0}), then the phi~ phases
+            double2 T0 = make_double2(0, 0), Tp = T0, Tm = T0;
+#define AMP_GZ(ZC, J, LR, LB)                                                                   \
+            if (a.gstart[5 + ZC + 1] > a.gstart[5 + ZC]) {                                        \
+                double2 Um = make_double2(0, 0), U0 = Um, Up = Um;                                \
+                spin_class<J, LR, LB>(a, 5 + ZC, k.mZ2, invmZ, qZ, pBZ, bw_rec, Um, U0, Up);      \
+                double d0, d1;                                                                    \
+                dJ(J, cZ, sZ, &d0, &d1);                                                          \
+                T0 = cadd(T0, cscale(d0, U0));                                                    \
+                if (J) { Tp = cadd(Tp, cscale(-d1, Up)); Tm = cadd(Tm, cscale(d1, Um)); }         \
+            }
+            AMP_GZ(0, 1, 0, 1)   // 1+
+            AMP_GZ(1, 2, 2, 2)   // 2+
+            AMP_GZ(2, 0, 1, 0)   // 0-
+            AMP_GZ(3, 1, 1, 1)   // 1-
+            AMP_GZ(4, 2, 1, 2)   // 2-
+#undef AMP_GZ
+            Tp = cmul(make_double2(cpt, spt), Tp);
+            Tm = cmul(make_double2(cpt, -spt), Tm);
             const double gp = 0.5 * (1.0 + ct), gm = 0.5 * (1.0 - ct), g0 = RSQRT2 * stt;
             const double2 Zp = make_double2(g0 * T0.x + gp * Tp.x + gm * Tm.x, g0 * T0.y + gp * Tp.y + gm * Tm.y);
             const double2 Zm = make_double2(-g0 * T0.x + gm * Tp.x + gp * Tm.x, -g0 * T0.y + gm * Tp.y + gp * Tm.y);
@@ -166,7 +179,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
             if (ent == -2) { *re = 0.0; *im = 0.0; return; }
             const int J = g.pair_J[p];
             double2 gp, gm;
-            term_angular(J == 8 ? 1 : J, g.pair_lam[p], J == 8, k, st, &gp, &gm);
+            term_angular(J >= 8 ? J - 8 : J, g.pair_lam[p], J >= 8, k, st, &gp, &gm);   // 8 + J: a Z slot of spin J
             // T = conj(g+) A+ + conj(g-) A-
             double2 T = make_double2(fma(gp.x, k.Ap.x, gp.y * k.Ap.y), fma(gp.x, k.Ap.y, -gp.y * k.Ap.x));
             T.x = fma(gm.x, k.Am.x, fma(gm.y, k.Am.y, T.x));
@@ -309,8 +322,8 @@ cudaError_t launch_grad(const GradArgs& g, int grid, cudaStream_t s) {
     if (!attr_done) { e = cudaFuncSetAttribute(k_grad, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
     if (e != cudaSuccess) return e;
     int nent = 0;
-    for (int sp = 0; sp < 6; ++sp) nent += g.a.shape[sp];
-    k_grad<<<grid, THREADS, grad_smem(g.a.gstart[6] > g.a.gstart[5], nent), s>>>(g);
+    for (int sp = 0; sp < NSPIN; ++sp) nent += g.a.shape[sp];
+    k_grad<<<grid, THREADS, grad_smem(g.a.gstart[NSPIN] > g.a.gstart[5], nent), s>>>(g);
     return cudaGetLastError();
 }
 

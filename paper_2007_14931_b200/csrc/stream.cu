@@ -30,7 +30,7 @@ namespace amp {
 template <int MODE, class SH>
 __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __grid_constant__ StreamArgs a) {
     const double RSQRT2 = 0.70710678118654752440;
-    const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[6] > a.gstart[5]);
+    const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[NSPIN] > a.gstart[5]);
     // sum w S (normalisation tiles) lives in `acc`; sum log S (data tiles) as a running product of mantissas in `acc` and a
     // sum of exponents in `accE` (split_exp: integer ops + one multiply per event instead of a ~35-instruction FP64 log)
     const double LN2 = 0.69314718055994530942;
@@ -139,20 +139,38 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
             const Ev ca = load_col(stage, C_CA), sa = load_col(stage, C_SA);
             __syncthreads();   // Z region consumed: refill it with the next tile
             if (threadIdx.x == 0 && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[1], NCOL_K, NCOL_ALL, false);
-            double2 Um[E], U0[E], Up[E];
+            // T_l' = sum over the Z spin classes of d^J_{0 l'}(theta_Z) U_l' ; d^J_{0,+1} = -d^J_{+1,0}, d^J_{0,-1} = -d^J_{0,+1}
+            double2 T0[E], Tp[E], Tm[E];
 #pragma unroll
-            for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0);
-            spin_sum<1, 0, 1, SH::nz, SH::oz, 5>(a, i0, mZ2, invmZ, qZ, pBZ, Um, U0, Up);   // 1+ Z: L_R = 0, L_B = 1
+            for (int e = 0; e < E; ++e) T0[e] = Tp[e] = Tm[e] = make_double2(0, 0);
+#define AMP_ZCLASS(ZC, J, LR, LB, CNT, OFF, D0, D1)                                                    \
+            if (CNT != 0 && (CNT > 0 || a.gstart[5 + ZC + 1] > a.gstart[5 + ZC])) {                    \
+                double2 Um[E], U0[E], Up[E];                                                           \
+                _Pragma("unroll") for (int e = 0; e < E; ++e) Um[e] = U0[e] = Up[e] = make_double2(0, 0); \
+                spin_sum<J, LR, LB, CNT, OFF, 5 + ZC>(a, i0, mZ2, invmZ, qZ, pBZ, Um, U0, Up);         \
+                _Pragma("unroll") for (int e = 0; e < E; ++e) {                                        \
+                    const double c = cZ.v[e], s = sZ.v[e], c2 = c * c;                                 \
+                    (void)s; (void)c2;                                                                 \
+                    const double d0 = (D0), d1 = (D1);                                                 \
+                    T0[e] = cadd(T0[e], cscale(d0, U0[e]));                                            \
+                    if (J) { Tp[e] = cadd(Tp[e], cscale(d1, Up[e])); Tm[e] = cadd(Tm[e], cscale(-d1, Um[e])); } \
+                }                                                                                      \
+            }
+            AMP_ZCLASS(0, 1, 0, 1, SH::nz, SH::oz, c, RSQRT2 * s)                                       // 1+ : L_R = 0, L_B = 1
+            if (SH::nz < 0) {   // the other spin-parities run in the generic kernel only
+                AMP_ZCLASS(1, 2, 2, 2, -1, 0, fma(1.5, c2, -0.5), 1.2247448713915890491 * s * c)        // 2+ : 2, 2
+                AMP_ZCLASS(2, 0, 1, 0, -1, 0, 1.0, 0.0)                                                 // 0- : 1, 0
+                AMP_ZCLASS(3, 1, 1, 1, -1, 0, c, RSQRT2 * s)                                            // 1- : 1, 1
+                AMP_ZCLASS(4, 2, 1, 2, -1, 0, fma(1.5, c2, -0.5), 1.2247448713915890491 * s * c)        // 2- : 1, 2
+            }
+#undef AMP_ZCLASS
 #pragma unroll
             for (int e = 0; e < E; ++e) {
-                // T_l' = d^1_{0 l'}(theta_Z) e^{i l' phi~} U_l' ; d^1_{00} = cZ, d^1_{0,+-1} = +-sZ/sqrt2
-                const double z1 = RSQRT2 * sZ.v[e];
-                const double2 T0 = cscale(cZ.v[e], U0[e]);
-                const double2 Tp = cscale(z1, cmul(make_double2(cpt.v[e], spt.v[e]), Up[e]));
-                const double2 Tm = cscale(-z1, cmul(make_double2(cpt.v[e], -spt.v[e]), Um[e]));
+                Tp[e] = cmul(make_double2(cpt.v[e], spt.v[e]), Tp[e]);     // e^{+i phi~}
+                Tm[e] = cmul(make_double2(cpt.v[e], -spt.v[e]), Tm[e]);    // e^{-i phi~}
                 const double gp = 0.5 * (1.0 + ct.v[e]), gm = 0.5 * (1.0 - ct.v[e]), g0 = RSQRT2 * st.v[e];
-                const double2 Zp = make_double2(g0 * T0.x + gp * Tp.x + gm * Tm.x, g0 * T0.y + gp * Tp.y + gm * Tm.y);
-                const double2 Zm = make_double2(-g0 * T0.x + gm * Tp.x + gp * Tm.x, -g0 * T0.y + gm * Tp.y + gp * Tm.y);
+                const double2 Zp = make_double2(g0 * T0[e].x + gp * Tp[e].x + gm * Tm[e].x, g0 * T0[e].y + gp * Tp[e].y + gm * Tm[e].y);
+                const double2 Zm = make_double2(-g0 * T0[e].x + gm * Tp[e].x + gp * Tm[e].x, -g0 * T0[e].y + gm * Tp[e].y + gp * Tm[e].y);
                 Ap[e] = cfma(make_double2(ca.v[e], sa.v[e]), Zp, Ap[e]);    // e^{+i alpha}
                 Am[e] = cfma(make_double2(ca.v[e], -sa.v[e]), Zm, Am[e]);   // e^{-i alpha}
             }
@@ -268,7 +286,7 @@ long long stream_pad(long long n) { return (n + 511) / 512 * 512; }   // whole t
 
 template <class SH>
 static cudaError_t launch_shape(const StreamArgs& a, int grid, cudaStream_t s) {
-    const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[6] > a.gstart[5]);
+    const bool have_z = SH::nz > 0 || (SH::nz < 0 && a.gstart[NSPIN] > a.gstart[5]);
     const size_t smem = stream_smem(have_z, a.mode);
     cudaError_t e = cudaSuccess;
 #define AMP_LAUNCH(M)                                                                                              \
@@ -295,7 +313,8 @@ static cudaError_t launch_shape(const StreamArgs& a, int grid, cudaStream_t s) {
 cudaError_t launch_stream(const StreamArgs& a, int grid, cudaStream_t s) {
     const int* n = a.shape;
     auto is = [&](int a0, int a1, int a2, int a3, int a4, int az) {
-        return a.shape_fixed && n[0] == a0 && n[1] == a1 && n[2] == a2 && n[3] == a3 && n[4] == a4 && n[5] == az;
+        return a.shape_fixed && n[0] == a0 && n[1] == a1 && n[2] == a2 && n[3] == a3 && n[4] == a4 && n[5] == az &&
+               n[6] + n[7] + n[8] + n[9] == 0;   // Z's of another spin-parity than 1+: generic kernel
     };
     cudaError_t e;
     if (a.nlass > 0) {   // the paper's LASS variant: LASS + K0*(1950) in the S wave, the other eight K*, one Z

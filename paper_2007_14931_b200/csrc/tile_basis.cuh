@@ -63,9 +63,12 @@ struct Angles {
 __device__ __forceinline__ void angular_factor(const Angles& g, int code, double2* gp, double2* gm) {
     const double RSQRT2 = 0.70710678118654752440;
     const int kind = code >> 8, J = (code >> 4) & 15, lam = (code & 15) - 1;
-    if (kind == AMP_Z) {
-        // d^1_{0 l'}(theta_Z) e^{i l' phi~} d^1_{l' xi}(theta~) e^{i xi alpha}   (Eq. 10)
-        const double zf = lam == 0 ? g.cZ : (lam > 0 ? RSQRT2 * g.sZ : -RSQRT2 * g.sZ);
+    if (kind_is_z(kind)) {
+        // d^J_{0 l'}(theta_Z) e^{i l' phi~} d^1_{l' xi}(theta~) e^{i xi alpha}   (Eq. 10); J = 0, 1, 2
+        double zf;
+        if (J == 1) zf = lam == 0 ? g.cZ : (lam > 0 ? RSQRT2 * g.sZ : -RSQRT2 * g.sZ);
+        else if (J == 0) zf = lam == 0 ? 1.0 : 0.0;
+        else zf = lam == 0 ? fma(1.5, g.cZ * g.cZ, -0.5) : (lam > 0 ? 1.2247448713915890491 : -1.2247448713915890491) * g.sZ * g.cZ;
         const double dp = lam == 0 ? RSQRT2 * g.st : (lam > 0 ? 0.5 * (1.0 + g.ct) : 0.5 * (1.0 - g.ct));    // d^1_{l',+1}
         const double dm = lam == 0 ? -RSQRT2 * g.st : (lam > 0 ? 0.5 * (1.0 - g.ct) : 0.5 * (1.0 + g.ct));   // d^1_{l',-1}
         const double2 eph = lam == 0 ? make_double2(1.0, 0.0) : make_double2(g.cpt, lam > 0 ? g.spt : -g.spt);

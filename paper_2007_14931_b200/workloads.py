@@ -16,7 +16,7 @@ SEED = 2007014931
 # m_B0, m_J/psi, m_K+, m_pi- in MeV (BASELINE.json configs[0])
 DECAY = (5279.65, 3096.9, 493.677, 139.570)
 RADIUS = 1.6e-3  # MeV^-1 (1.6 GeV^-1; reading A3)
-KSTAR, ZRES, CONST, LASS = 0, 1, 2, 3
+KSTAR, ZRES, CONST, LASS, ZNEG = 0, 1, 2, 3, 4   # ZRES: a Z of positive parity (1+, 2+), ZNEG: of negative parity (0-, 1-, 2-)
 
 # (name, kind, J, mass, width) — BASELINE.json configs[1], configs[2] for the Z
 KSTARS = [
@@ -95,7 +95,7 @@ def slot_table(res):
     """[(resonance index, lambda)] in coupling-slot order (include/amp.h: amp_num_couplings)."""
     slots = []
     for r, (kind, J, *_rest) in enumerate(res):
-        if kind == ZRES or (kind == KSTAR and J >= 1):
+        if kind in (ZRES, ZNEG) or (kind == KSTAR and J >= 1):
             slots += [(r, -1), (r, 0), (r, +1)]
         else:
             slots += [(r, 0)]
