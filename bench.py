@@ -388,6 +388,46 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_pseudo(args):
+    """Context only (not the headline metric): the workload of the paper's one performance figure (Fig. 2, PAPER.md:201,
+    207-209: pseudo-experiments of 10,000 events generated and fitted with models of an increasing number of K*s; the figure's
+    values are not in the text).  Per model: --steps pseudo-experiments are generated on the device (amp_generate), fitted
+    from a perturbed start on the analytic gradient (amp_nll_grad) and given Hessian errors; wall clock around all of it."""
+    import torch
+    from paper_2007_14931_b200 import binding as B
+    from paper_2007_14931_b200 import fit as F
+    torch.cuda.set_device(0)
+    ks = W.KSTARS
+    models = {"3 K*": (1, 3, 4), "6 K*": (1, 2, 3, 4, 5, 6), "10 K*": tuple(range(10))}
+    lo, hi, cm = W.DECAY[2] + W.DECAY[3] + W.M_LO_MARGIN, W.M_HI, W.COS_MAX
+    xn = torch.as_tensor(W.phase_space_events(np.random.default_rng(77), args.n_norm)).cuda()
+    per_model, total_t, total_n = {}, 0.0, 0
+    for name, idx in models.items():
+        res = [(ks[i][1], ks[i][2], ks[i][3], ks[i][4], W.RADIUS) for i in idx]
+        slots = W.slot_table(res)
+        rng = np.random.default_rng(len(idx))
+        c = rng.uniform(0.6, 1.4, len(slots)) * np.exp(1j * rng.uniform(-np.pi, np.pi, len(slots)))
+        fixed = [k for k, (r, lam) in enumerate(slots) if r == 0 and lam == 0]
+        c[fixed[0]] = 1.0
+        M = B.Model(W.DECAY, res)
+        M.load_norm(xn)
+        F.pull_study(M, c, 2, args.pseudo, 1, lo, hi, cm, fixed=fixed)            # warm-up (first launches, the matrix M)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        out = F.pull_study(M, c, args.steps, args.pseudo, 1000, lo, hi, cm, fixed=fixed)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        per_model[name] = {"free_parameters": 2 * (len(slots) - 1), "ms_per_pseudo_experiment": dt / args.steps * 1e3,
+                           "likelihood_calls": float(out["n_calls"].mean()), "converged": float(out["converged"].mean())}
+        total_t += dt
+        total_n += args.steps
+    print(json.dumps({"metric": "pseudo-experiments generated and fitted per second (context: workload of the paper's Fig. 2)", "value": total_n / total_t,
+                      "unit": "pseudo-experiments/s", "n_gpus": 1, "steps": args.steps, "warmup": 2, "higher_is_better": True, "vs_baseline": None,
+                      "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": f"{args.pseudo} events per pseudo-experiment, {args.n_norm} normalisation points, masses and widths fixed, "
+                                             "generate (amp_generate) + BFGS fit on amp_nll_grad + Hessian errors", "models": per_model}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -401,7 +441,13 @@ def main():
     ap.add_argument("--dense", action="store_true", help="--cfg 4 through the dense DMMA contraction instead of the gradient-batch kernel")
     ap.add_argument("--grad", action="store_true", help="--cfg 3 steps that also return the analytic gradient in all couplings (amp_nll_grad)")
     ap.add_argument("--lass", action="store_true", help="configs[3] call pattern on the LASS variant of the model (Eqs. 7-9; SURVEY.md 8(f)-1)")
+    ap.add_argument("--pseudo", type=int, default=0, metavar="N_EVENTS",
+                    help="context mode: generate and fit --steps pseudo-experiments of N_EVENTS each for models of 3, 6 and 10 K*s (the paper's Fig. 2 workload)")
     args = ap.parse_args()
+    if args.pseudo:
+        args.steps = min(args.steps, 50)
+        args.n_norm = min(args.n_norm, 1_000_000)
+        return run_pseudo(args)
     global LASS
     LASS = bool(args.lass)
     if LASS and args.cfg != 3:

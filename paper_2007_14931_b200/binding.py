@@ -18,7 +18,7 @@ AMP_MAX_RESONANCES, AMP_MAX_COUPLINGS, AMP_MAX_POINTS = 16, 48, 256
 # every symbol include/amp.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
-    "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_grad", "amp_generate", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
+    "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_grad", "amp_fit", "amp_generate", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
     "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_fit_fractions", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode",
     "amp_last_call_stats", "amp_last_call_timing", "amp_recent_launch_ms", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
 ]
@@ -63,6 +63,7 @@ def lib():
         "amp_set_params": (i, [vp, i, vp, vp]),
         "amp_nll": (i, [vp, vp, vp]),
         "amp_nll_grad": (i, [vp, vp, vp, vp]),
+        "amp_fit": (i, [vp, vp, vp, vp, i, vp, vp, i, vp, i, d, vp, vp, vp, vp, vp]),
         "amp_generate": (i, [vp, C.c_ulonglong, C.c_ulonglong, ll, d, d, d, d, vp, vp, ll, C.POINTER(ll), pd, vp]),
         "amp_nll_terms": (i, [vp, vp, vp, vp]),
         "amp_dataset_sums": (i, [vp, C.POINTER(ll), pd, C.POINTER(ll), pd]),
@@ -196,6 +197,32 @@ class Model:
         nll, grad = np.empty(1), np.empty((self.K, 2))
         self._check(lib().amp_nll_grad(self._h, nll.ctypes.data_as(C.c_void_p), grad.ctypes.data_as(C.c_void_p), _stream_ptr(stream)), "amp_nll_grad")
         return nll[0], grad
+
+    def fit(self, c_start, fixed=(), ties=(), mass_width=None, scale=None, max_iter=3000, gtol=1e-3, errors=False, stream=None):
+        """native BFGS fit of the couplings (amp_fit) -> dict(couplings [K] complex, nll, grad_max, converged, n_calls, iterations,
+        free (slots), covariance [2F][2F] or None, errors complex [F] or None)"""
+        c = np.asarray(c_start, dtype=np.complex128)
+        assert c.shape == (self.K,)
+        hc = np.ascontiguousarray(np.stack([c.real, c.imag], -1))
+        hmw = None if mass_width is None else np.ascontiguousarray(np.asarray(mass_width, dtype=np.float64).reshape(self.R, 2))
+        fx = np.ascontiguousarray(list(fixed), dtype=np.int32)
+        td = np.ascontiguousarray([t[0] for t in ties], dtype=np.int32)
+        ts = np.ascontiguousarray([t[1] for t in ties], dtype=np.int32)
+        hs = None if scale is None else np.ascontiguousarray(scale, dtype=np.float64)
+        free = [k for k in range(self.K) if k not in set(int(f) for f in fixed) and k not in set(int(t) for t in td)]
+        nf = 2 * len(free)
+        out, nll, info = np.empty((self.K, 2)), np.empty(2), np.zeros(5, dtype=np.int32)
+        cov = np.empty((nf, nf)) if errors else None
+        p = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None and a.size else None
+        self._check(lib().amp_fit(self._h, p(hc), p(hmw), p(fx), len(fx), p(td), p(ts), len(td), p(hs), int(max_iter), float(gtol),
+                                  p(out), p(nll), p(cov), p(info), _stream_ptr(stream)), "amp_fit")
+        self.P = 1
+        res = {"couplings": out[:, 0] + 1j * out[:, 1], "nll": float(nll[0]), "grad_max": float(nll[1]), "converged": bool(info[0]),
+               "n_calls": int(info[1]), "iterations": int(info[2]), "free": free, "covariance": cov, "errors": None}
+        if errors and info[3]:
+            sig = np.sqrt(np.diag(cov)).reshape(-1, 2)
+            res["errors"] = sig[:, 0] + 1j * sig[:, 1]
+        return res
 
     def generate(self, seed, first, n_candidates, f_max, m_lo, m_hi, cos_max, capacity, with_index=False, stream=None):
         """accept-reject toy block (amp_generate): -> (x_out cuda [4][capacity], index cuda [capacity] or None, n_accepted, f_seen_max);

@@ -83,6 +83,11 @@ struct amp_model {
     unsigned char* d_hk = nullptr; // herk plan: entries, tiles, coefficients
     unsigned char* h_hk = nullptr; // pinned
     size_t hk_cap = 0;
+    // scratch of amp_generate, kept between calls (cudaMalloc / cudaFree of ~200 MB per call would cost more than the generation)
+    double *toy_x = nullptr, *toy_u = nullptr, *toy_S = nullptr, *toy_cache = nullptr;
+    int* toy_count = nullptr;
+    unsigned long long* toy_fseen = nullptr;
+    long long toy_cap = 0;         // candidates the scratch holds
     bool stream_inline = true;     // P == 1: streaming launches evaluate lineshapes in registers even if columns exist
     bool want_matrix = false;      // set_params decided that the normalisation should go through the matrix
     std::vector<double> prev_mw;   // masses and widths of the previous single-point call (static-lineshape detection)
@@ -182,6 +187,19 @@ __global__ void k_fill(double* __restrict__ p, long long n, double v) {
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) p[i] = v;
 }
 
+void free_toy_scratch(amp_model* m) {
+    if (m->toy_x) cudaFree(m->toy_x);
+    if (m->toy_u) cudaFree(m->toy_u);
+    if (m->toy_S) cudaFree(m->toy_S);
+    if (m->toy_cache) cudaFree(m->toy_cache);
+    if (m->toy_count) cudaFree(m->toy_count);
+    if (m->toy_fseen) cudaFree(m->toy_fseen);
+    m->toy_x = m->toy_u = m->toy_S = m->toy_cache = nullptr;
+    m->toy_count = nullptr;
+    m->toy_fseen = nullptr;
+    m->toy_cap = 0;
+}
+
 void free_dataset(Dataset& d) {
     if (d.cache) cudaFree(d.cache);
     if (d.cols) cudaFree(d.cols);
@@ -194,7 +212,9 @@ amp_status load_dataset(amp_model* m, Dataset& d, bool is_norm, const double* d_
     if (!m) return AMP_ERR_INVALID;
     if (n < 0 || (n > 0 && !d_x)) return fail(m, AMP_ERR_INVALID, "load: null events or negative count");
     const long long npad = stream_pad(n > 0 ? n : 1);
-    const bool reuse = scratch && d.cache && d.npad == npad;
+    // scratch: the caller's buffer holds at least npad events; otherwise a same-sized reload (pseudo-experiment loops) keeps its
+    // allocations (cache and lineshape pool, whose columns are marked stale below): cudaFree + cudaMalloc cost milliseconds
+    const bool reuse = scratch ? d.cache != nullptr : (d.cache != nullptr && d.npad == npad);
     if (!reuse) free_dataset(d);
     if (!scratch) {
         for (auto& e : m->pool) (is_norm ? e.valid_norm : e.valid_data) = false;
@@ -228,13 +248,13 @@ amp_status load_dataset(amp_model* m, Dataset& d, bool is_norm, const double* d_
     int flag;
     std::memcpy(&flag, m->h_pinned + 1, sizeof(int));
     if (flag) {
-        free_dataset(d);
+        if (!scratch) free_dataset(d);
         return fail(m, AMP_ERR_DOMAIN, is_norm ? "amp_load_norm: event outside phase space or bad weight"
                                                : "amp_load_events: event outside phase space or non-positive efficiency");
     }
     d.wsum = m->h_pinned[0];
     if (is_norm && n > 0 && !(d.wsum > 0)) {
-        free_dataset(d);
+        if (!scratch) free_dataset(d);
         return fail(m, AMP_ERR_DOMAIN, "amp_load_norm: weights sum to zero");
     }
     d.loaded = true;
@@ -325,6 +345,7 @@ amp_status amp_model_destroy(amp_model* m) {
     if (m->d_flag) cudaFree(m->d_flag);
     if (m->d_ticket) cudaFree(m->d_ticket);
     if (m->d_bkg) cudaFree(m->d_bkg);
+    free_toy_scratch(m);
     if (m->h_pinned) cudaFreeHost(m->h_pinned);
     if (m->h_zc) cudaFreeHost(m->h_zc);
     if (m->d_plan) cudaFree(m->d_plan);
@@ -1670,25 +1691,26 @@ amp_status amp_generate(amp_model* m, unsigned long long seed, unsigned long lon
     m->stat_launches = m->stat_columns = 0;
     const long long CH = 1LL << 21;                       // candidates per block of work (a multiple of the selection block)
     const long long ch = n_candidates < CH ? n_candidates : CH;
-    double *d_x = nullptr, *d_u = nullptr, *d_S = nullptr;
-    int* d_count = nullptr;
-    unsigned long long* d_fseen = nullptr;
+    if (m->toy_cap < ch) {
+        free_toy_scratch(m);
+        const int ncolw = (m->has_z ? NCOL_ALL : NCOL_K) + 1;
+        cudaError_t e = cudaMalloc(&m->toy_x, sizeof(double) * 4 * ch);
+        if (e == cudaSuccess) e = cudaMalloc(&m->toy_u, sizeof(double) * ch);
+        if (e == cudaSuccess) e = cudaMalloc(&m->toy_S, sizeof(double) * stream_pad(ch));
+        if (e == cudaSuccess) e = cudaMalloc(&m->toy_cache, sizeof(double) * ncolw * stream_pad(ch));
+        if (e == cudaSuccess) e = cudaMalloc(&m->toy_count, sizeof(int) * (toy_blocks(ch) + 1));
+        if (e == cudaSuccess) e = cudaMalloc(&m->toy_fseen, sizeof(unsigned long long));
+        if (e != cudaSuccess) { free_toy_scratch(m); return cuda_fail(m, e, "amp_generate"); }
+        m->toy_cap = ch;
+    }
+    double *d_x = m->toy_x, *d_u = m->toy_u, *d_S = m->toy_S;
+    int* d_count = m->toy_count;
+    unsigned long long* d_fseen = m->toy_fseen;
     Dataset tmp{};
-    auto cleanup = [&]() {
-        if (d_x) cudaFree(d_x);
-        if (d_u) cudaFree(d_u);
-        if (d_S) cudaFree(d_S);
-        if (d_count) cudaFree(d_count);
-        if (d_fseen) cudaFree(d_fseen);
-        free_dataset(tmp);
-    };
-    cudaError_t e = cudaMalloc(&d_x, sizeof(double) * 4 * ch);
-    if (e == cudaSuccess) e = cudaMalloc(&d_u, sizeof(double) * ch);
-    if (e == cudaSuccess) e = cudaMalloc(&d_S, sizeof(double) * stream_pad(ch));
-    if (e == cudaSuccess) e = cudaMalloc(&d_count, sizeof(int) * (toy_blocks(ch) + 1));
-    if (e == cudaSuccess) e = cudaMalloc(&d_fseen, sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemsetAsync(d_fseen, 0, sizeof(unsigned long long), s);
-    if (e != cudaSuccess) { cleanup(); return cuda_fail(m, e, "amp_generate"); }
+    tmp.cache = m->toy_cache;
+    auto cleanup = [&]() {};
+    cudaError_t e = cudaMemsetAsync(d_fseen, 0, sizeof(unsigned long long), s);
+    if (e != cudaSuccess) return cuda_fail(m, e, "amp_generate");
     long long accepted = 0;
     amp_status st = AMP_OK;
     for (long long off = 0; off < n_candidates && st == AMP_OK; off += ch) {

@@ -90,10 +90,10 @@ def fit_couplings(model, c_start, fixed=(), ties=(), mass_width=None, maxiter=30
     return out
 
 
-def pull_study(model, c_true, n_toys, n_events, seed, m_lo, m_hi, cos_max, fixed=(), ties=(), start_spread=0.1, f_max=None):
+def pull_study(model, c_true, n_toys, n_events, seed, m_lo, m_hi, cos_max, fixed=(), ties=(), start_spread=0.1, f_max=None, native=True):
     """The paper's validation loop: n_toys pseudo-experiments of n_events each are generated from c_true on the
     device (amp_generate; no efficiency: the model's normalisation sample must then be an unweighted phase-space sample), each is
-    fitted from a perturbed start and its pulls (fit - true) / sigma are recorded.
+    fitted from a perturbed start (amp_fit, or scipy's BFGS with native=False) and its pulls (fit - true) / sigma are recorded.
     Returns dict(pulls [n_toys][2 n_free], converged [n_toys], n_calls [n_toys], couplings [n_toys][K]); candidate streams of
     successive toys do not overlap (toy t uses seed + t)."""
     import torch
@@ -117,10 +117,15 @@ def pull_study(model, c_true, n_toys, n_events, seed, m_lo, m_hi, cos_max, fixed
             start[k] = c_true[k]
         for d, s in tied.items():
             start[d] = start[s]
-        r = fit_couplings(model, start, fixed=fixed, ties=ties, scale=np.abs(c_true), errors=True)
-        d = r.couplings[r.free] - c_true[r.free]
-        pulls.append(np.stack([d.real / r.errors.real, d.imag / r.errors.imag], -1).ravel())
-        conv.append(r.converged)
-        ncall.append(r.n_calls)
-        cs.append(r.couplings)
+        if native:      # the minimiser of the library (amp_fit): no interpreter between two launches
+            r = model.fit(start, fixed=fixed, ties=ties, scale=np.abs(c_true), errors=True)
+            cf, free, err, ok, nc = r["couplings"], r["free"], r["errors"], r["converged"] and r["errors"] is not None, r["n_calls"]
+        else:           # scipy's BFGS on the same gradient (cross-check)
+            r = fit_couplings(model, start, fixed=fixed, ties=ties, scale=np.abs(c_true), errors=True)
+            cf, free, err, ok, nc = r.couplings, r.free, r.errors, r.converged, r.n_calls
+        d = cf[free] - c_true[free]
+        pulls.append(np.stack([d.real / err.real, d.imag / err.imag], -1).ravel() if err is not None else np.full(2 * len(free), np.nan))
+        conv.append(ok)
+        ncall.append(nc)
+        cs.append(cf)
     return {"pulls": np.array(pulls), "converged": np.array(conv), "n_calls": np.array(ncall), "couplings": np.array(cs)}

@@ -115,3 +115,60 @@ def test_generate_on_device_then_fit_one_million_events():
     assert np.max(np.abs(ff_fit - ff_true)) < 0.01, (ff_fit, ff_true)
     dev_rel = np.abs(r.couplings - c_true) / np.abs(c_true)
     assert np.median(dev_rel) < 0.06, np.median(dev_rel)
+
+
+def test_native_fit_agrees_with_scipy_bfgs():
+    """amp_fit (BFGS in the library, csrc/minimize.cu) against scipy's BFGS on the same device gradient: same minimum, same
+    covariance; constraints of Eq. 6 (fixed slot) and Eq. 11 (tie) in force"""
+    import time
+    from paper_2007_14931_b200 import binding as B
+    from paper_2007_14931_b200 import fit as F
+    cfg = 2
+    res = W.resonances(cfg)
+    slots = W.slot_table(res)
+    c_true = W.couplings(cfg)
+    Mo = O.Model(W.DECAY, res)
+    xn, wn = W.norm_events(cfg, 400_000)
+    x, eff = W.data_events(cfg, lambda xx, ee: Mo.eval_events(c_true, xx, ee), n=100_000)
+    Mg = B.Model(W.DECAY, res)
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    fixed = [k for k, (r, lam) in enumerate(slots) if r == 1 and lam == 0]
+    ties = [(k, k - 2) for k, (r, lam) in enumerate(slots) if res[r][0] == W.ZRES and lam == +1]
+    rng = np.random.default_rng(8)
+    start = c_true * (1 + 0.3 * rng.uniform(-1, 1, c_true.size)) * np.exp(0.3j * rng.uniform(-1, 1, c_true.size))
+    for k in fixed:
+        start[k] = c_true[k]
+    for d, s in ties:
+        start[d] = start[s]
+    Mg.set_params(start)
+    Mg.nll_grad()
+    t0 = time.perf_counter()
+    rn = Mg.fit(start, fixed=fixed, ties=ties, errors=True, gtol=1e-4)
+    t_native = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    rs = F.fit_couplings(Mg, start, fixed=fixed, ties=ties, errors=True, gtol=1e-4)
+    t_scipy = time.perf_counter() - t0
+    print(f"\nnative: {rn['n_calls']} calls {t_native * 1e3:.1f} ms;  scipy: {rs.n_calls} calls {t_scipy * 1e3:.1f} ms")
+    assert rn["converged"] and rs.converged
+    assert rn["grad_max"] < 1e-4
+    assert abs(rn["nll"] - rs.nll) < 1e-6                                   # same minimum (NLL ~ 1e6; both stop at |g| < 1e-4)
+    assert rn["free"] == rs.free
+    for d, s in ties:
+        assert rn["couplings"][d] == rn["couplings"][s]
+    for k in fixed:
+        assert rn["couplings"][k] == c_true[k]
+    big = np.abs(c_true) > 0
+    assert np.max(np.abs(rn["couplings"] - rs.couplings)[big] / np.abs(c_true)[big]) < 1e-3 * 50      # within a small fraction of the errors
+    err_n, err_s = rn["errors"], rs.errors
+    assert np.max(np.abs(err_n.real - err_s.real) / err_s.real) < 1e-3 and np.max(np.abs(err_n.imag - err_s.imag) / err_s.imag) < 1e-3
+    assert np.max(np.abs(rn["couplings"] - rs.couplings)[rn["free"]] / np.abs(err_s)) < 0.01           # 1 % of a standard deviation
+    # the model is left at the fitted point
+    nll_now, g = Mg.nll_grad()
+    Mg.set_params(rn["couplings"])
+    assert abs(Mg.nll()[0] - rn["nll"]) < 1e-9 * abs(rn["nll"])
+    # bad arguments
+    with pytest.raises(B.AmpError):
+        Mg.fit(start, fixed=[99])
+    with pytest.raises(B.AmpError):
+        Mg.fit(start, ties=[(3, 3)])

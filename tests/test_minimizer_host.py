@@ -1,0 +1,132 @@
+"""Host logic of the native minimiser (csrc/minimize.cu, amp_fit) without a GPU: the file is compiled (host code only) against a
+stand-in likelihood with a known minimum and Hessian (tests/minimize_stub.cu) and compared with the closed form and with scipy."""
+import ctypes as C
+import os
+import shutil
+import subprocess
+
+import numpy as np
+import pytest
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+K = 12
+
+
+def lam(i):
+    return 1e4 ** (i / (2.0 * K - 1))
+
+
+def f_and_grad(h):
+    d = h - (1.0 + 0.1 * np.arange(2 * K))
+    l = lam(np.arange(2 * K))
+    f = np.sum(0.5 * l * d * d + 0.25 * d ** 4) + 0.3 * np.sum(d[:-1] * d[1:])
+    g = l * d + d ** 3
+    g[:-1] += 0.3 * d[1:]
+    g[1:] += 0.3 * d[:-1]
+    return f, g
+
+
+@pytest.fixture(scope="module")
+def stub(tmp_path_factory):
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc not available")
+    out = str(tmp_path_factory.mktemp("minstub") / "libminstub.so")
+    subprocess.check_call([nvcc, "-O2", "-shared", "-Xcompiler", "-fPIC", "-I", os.path.join(HERE, "..", "include"), "-o", out,
+                           os.path.join(HERE, "minimize_stub.cu")])
+    lib = C.CDLL(out)
+    vp, i, d = C.c_void_p, C.c_int, C.c_double
+    lib.amp_fit.restype = i
+    lib.amp_fit.argtypes = [vp, vp, vp, vp, i, vp, vp, i, vp, i, d, vp, vp, vp, vp, vp]
+    return lib
+
+
+def run(lib, start, fixed=(), ties=(), scale=None, max_iter=3000, gtol=1e-7, cov=True):
+    p = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None and a.size else None
+    hs = np.ascontiguousarray(start, dtype=np.float64).reshape(K, 2)
+    fx = np.ascontiguousarray(fixed, dtype=np.int32)
+    td = np.ascontiguousarray([t[0] for t in ties], dtype=np.int32)
+    ts = np.ascontiguousarray([t[1] for t in ties], dtype=np.int32)
+    sc = None if scale is None else np.ascontiguousarray(scale, dtype=np.float64)
+    nfree = K - len(set(fixed)) - len(td)
+    fit, nll, info = np.empty((K, 2)), np.empty(2), np.zeros(5, dtype=np.int32)
+    cv = np.empty((2 * nfree, 2 * nfree)) if cov else None
+    st = lib.amp_fit(C.c_void_p(1), p(hs), None, p(fx), len(fx), p(td), p(ts), len(td), p(sc), max_iter, gtol, p(fit), p(nll), p(cv), p(info), None)
+    return st, fit, nll, cv, info
+
+
+def test_unconstrained_minimum_and_covariance(stub):
+    start = np.full(2 * K, 0.5)
+    st, fit, nll, cov, info = run(stub, start)
+    assert st == 0 and info[0] == 1 and info[3] == 1 and info[4] == 2 * K
+    target = 1.0 + 0.1 * np.arange(2 * K)
+    assert np.max(np.abs(fit.ravel() - target)) < 1e-7          # the known minimum
+    assert nll[0] < 1e-12 and nll[1] < 1e-7
+    # covariance = inverse Hessian; at the minimum the Hessian is diag(lam) + 0.3 (off-diagonals)
+    H = np.diag(lam(np.arange(2 * K))) + 0.3 * (np.eye(2 * K, k=1) + np.eye(2 * K, k=-1))
+    assert np.max(np.abs(cov - np.linalg.inv(H)) / np.abs(np.linalg.inv(H)).max()) < 1e-6
+    # as many likelihood calls as scipy's BFGS needs for the same problem (+ 4 F for the Hessian), within a factor 1.5
+    from scipy.optimize import minimize
+    r = minimize(lambda t: f_and_grad(t), start, jac=True, method="BFGS", options={"gtol": 1e-7})
+    assert info[1] - 4 * K <= 1.5 * r.nfev + 5, (info, r.nfev)
+    # the stand-in model is left at the fitted point
+    cur = np.empty(2 * K)
+    stub.stub_current(cur.ctypes.data_as(C.c_void_p))
+    assert np.array_equal(cur, fit.ravel())
+
+
+def test_fixed_slots_ties_and_scales(stub):
+    start = np.full(2 * K, 0.5)
+    start[2:4] = (0.9, -0.4)                                      # slot 1 fixed at this value
+    fixed, ties = [1], [(5, 3), (7, 3)]                           # H_5 = H_3, H_7 = H_3
+    scale = np.linspace(0.2, 3.0, K)
+    st, fit, nll, cov, info = run(stub, start, fixed=fixed, ties=ties, scale=scale)
+    assert st == 0 and info[0] == 1 and info[4] == 2 * (K - 3)
+    assert tuple(fit[1]) == (0.9, -0.4)
+    assert np.array_equal(fit[5], fit[3]) and np.array_equal(fit[7], fit[3])
+    # reference: scipy on the reduced problem
+    free = [k for k in range(K) if k not in (1, 5, 7)]
+
+    def expand(t):
+        h = start.copy().reshape(K, 2)
+        h[free] = t.reshape(-1, 2)
+        h[5] = h[3]
+        h[7] = h[3]
+        return h
+
+    def red(t):
+        f, g = f_and_grad(expand(t).ravel())
+        g = g.reshape(K, 2).copy()
+        g[3] += g[5] + g[7]
+        return f, g[free].ravel()
+
+    from scipy.optimize import minimize
+    r = minimize(red, start.reshape(K, 2)[free].ravel(), jac=True, method="BFGS", options={"gtol": 1e-9})
+    assert abs(nll[0] - r.fun) < 1e-9 * max(1.0, abs(r.fun))
+    assert np.max(np.abs(fit[free].ravel() - r.x)) < 1e-6
+    # covariance of the free parameters in H units (not in scaled units): finite-difference Hessian of the reduced problem
+    n = 2 * len(free)
+    Hn = np.empty((n, n))
+    for j in range(n):
+        e = np.zeros(n)
+        e[j] = 1e-5
+        Hn[:, j] = (red(r.x + e)[1] - red(r.x - e)[1]) / 2e-5
+    ref = np.linalg.inv(0.5 * (Hn + Hn.T))
+    assert np.max(np.abs(cov - ref)) < 1e-5 * np.abs(ref).max()
+
+
+def test_bad_arguments_and_domain_backoff(stub):
+    start = np.full(2 * K, 0.5)
+    assert run(stub, start, fixed=[K])[0] == 1                    # AMP_ERR_INVALID: slot out of range
+    assert run(stub, start, ties=[(2, 2)])[0] == 1                # tie to itself
+    assert run(stub, start, ties=[(2, 3), (3, 4)])[0] == 1        # chained ties
+    assert run(stub, start, scale=np.zeros(K))[0] == 1            # non-positive scale
+    assert run(stub, start, gtol=0.0)[0] == 1
+    # max_iter = 0: no step, start returned, covariance at the start point still computed
+    st, fit, nll, cov, info = run(stub, start, max_iter=0)
+    assert st == 0 and info[0] == 0 and info[2] == 0 and np.array_equal(fit.ravel(), start)
+    # a start next to a region without a likelihood (the stand-in refuses Re H_0 > 50): the search backs off and still converges
+    far = start.copy()
+    far[0] = 49.9
+    st, fit, nll, cov, info = run(stub, far, cov=False)
+    assert st == 0 and info[0] == 1 and abs(fit[0, 0] - 1.0) < 1e-6
