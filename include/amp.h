@@ -130,24 +130,32 @@ amp_status amp_nll(amp_model* m, double* h_nll, void* stream);
  * for models with a LASS term (AMP_ERR_STATE).  Deterministic.  Path 7 in amp_last_call_stats.                       */
 amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* stream);
 
-/* Fit of the couplings in native code (the paper's MINUIT loop, with the analytic gradient in place of finite
- * differences): BFGS with a strong-Wolfe line search over Re, Im of the free helicity couplings at fixed masses and widths;
- * every iteration is one amp_set_params + one amp_nll_grad.  Needs data and normalisation events loaded.
+/* Fit in native code (the paper's MINUIT loop, with the analytic gradient in place of finite differences for the
+ * couplings): BFGS with a strong-Wolfe line search over Re, Im of the free helicity couplings and, optionally, masses and
+ * widths of chosen resonances ("floating masses/widths").  Every evaluation is one amp_set_params + one
+ * amp_nll_grad; with floating lineshape parameters one more batch of 1 + 2 n_float_mw points (amp_nll; central differences
+ * of the NLL over +- 1 % of the width).  Needs data and normalisation events loaded.
  *   h_start      host [K][2] start values; fixed slots keep them
- *   h_mass_width host [R][2] or NULL (= the values given at amp_model_create)
+ *   h_mass_width host [R][2] start / fixed masses and widths, or NULL (= the values given at amp_model_create; only
+ *                without floating lineshape parameters)
  *   fixed        [n_fixed] slots held constant (Eq. 6: the K*(892) lambda = 0 amplitude)
  *   tie_dst/src  [n_ties] H[dst] = H[src] (Eq. 11); a dst is not free and not a src of another tie
- *   h_scale      host [K] positive parameter scales or NULL (= |start|, floored at 1e-3 of the largest)
- *   max_iter, gtol   iteration cap; converged when max |dNLL/d(H/scale)| < gtol
- *   h_fit        host [K][2] fitted couplings (ties applied);  h_nll host [2]: NLL at the fit, max |gradient| there
- *   h_cov        host [2F][2F] (F = free slots, ascending; order Re, Im per slot) covariance = inverse Hessian of the NLL, the
- *                Hessian from central differences of the analytic gradient (4F more launches); or NULL
- *   h_info       host int[5] or NULL: converged, likelihood calls, iterations, covariance positive definite, 2F
- * The model is left with the fitted point set.  Errors of amp_set_params / amp_nll_grad are passed on; AMP_ERR_INVALID for
- * bad slot indices, chained ties or a non-positive scale; AMP_ERR_DOMAIN if the start point has no finite likelihood.      */
+ *   float_mw     [n_float_mw][2] = (resonance index, 0: its mass / 1: its width) floating lineshape parameters, no duplicates
+ *   h_scale      host [K] positive parameter scales or NULL (= |start|, floored at 1e-3 of the largest); masses and widths
+ *                are scaled by the start width
+ *   max_iter, gtol   iteration cap; converged when max |dNLL/d(parameter / scale)| < gtol
+ *   h_fit        host [K][2] fitted couplings (ties applied);  h_fit_mw host [R][2] fitted masses and widths, or NULL;
+ *   h_nll        host [2]: NLL at the fit, max |gradient| there
+ *   h_cov        host [n][n], n = 2F + n_float_mw (F = free slots, ascending; Re, Im per slot; then float_mw order): covariance
+ *                = inverse Hessian of the NLL, the Hessian from central differences of the gradient (2 n more evaluations); or NULL
+ *   h_info       host int[5] or NULL: converged, likelihood evaluations, iterations, covariance positive definite, n
+ * The model is left with the fitted point set.  Errors of amp_set_params / amp_nll_grad / amp_nll are passed on (a trial point
+ * outside the likelihood's domain makes the line search back off); AMP_ERR_INVALID for bad indices, chained ties, duplicates
+ * or a non-positive scale; AMP_ERR_DOMAIN if the start point has no finite likelihood.                                       */
 amp_status amp_fit(amp_model* m, const double* h_start, const double* h_mass_width, const int* fixed, int n_fixed,
-                   const int* tie_dst, const int* tie_src, int n_ties, const double* h_scale, int max_iter, double gtol,
-                   double* h_fit, double* h_nll, double* h_cov, int* h_info, void* stream);
+                   const int* tie_dst, const int* tie_src, int n_ties, const int* float_mw, int n_float_mw,
+                   const double* h_scale, int max_iter, double gtol,
+                   double* h_fit, double* h_fit_mw, double* h_nll, double* h_cov, int* h_info, void* stream);
 
 /* Accept-reject toy generator ("a distribution according to the fit model is generated through MC techniques";
  * the recipe the paper leaves open is fixed in DESIGN.md "Toy generator").  For the candidate numbers

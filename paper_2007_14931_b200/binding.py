@@ -63,7 +63,7 @@ def lib():
         "amp_set_params": (i, [vp, i, vp, vp]),
         "amp_nll": (i, [vp, vp, vp]),
         "amp_nll_grad": (i, [vp, vp, vp, vp]),
-        "amp_fit": (i, [vp, vp, vp, vp, i, vp, vp, i, vp, i, d, vp, vp, vp, vp, vp]),
+        "amp_fit": (i, [vp, vp, vp, vp, i, vp, vp, i, vp, i, vp, i, d, vp, vp, vp, vp, vp, vp]),
         "amp_generate": (i, [vp, C.c_ulonglong, C.c_ulonglong, ll, d, d, d, d, vp, vp, ll, C.POINTER(ll), pd, vp]),
         "amp_nll_terms": (i, [vp, vp, vp, vp]),
         "amp_dataset_sums": (i, [vp, C.POINTER(ll), pd, C.POINTER(ll), pd]),
@@ -198,9 +198,10 @@ class Model:
         self._check(lib().amp_nll_grad(self._h, nll.ctypes.data_as(C.c_void_p), grad.ctypes.data_as(C.c_void_p), _stream_ptr(stream)), "amp_nll_grad")
         return nll[0], grad
 
-    def fit(self, c_start, fixed=(), ties=(), mass_width=None, scale=None, max_iter=3000, gtol=1e-3, errors=False, stream=None):
-        """native BFGS fit of the couplings (amp_fit) -> dict(couplings [K] complex, nll, grad_max, converged, n_calls, iterations,
-        free (slots), covariance [2F][2F] or None, errors complex [F] or None)"""
+    def fit(self, c_start, fixed=(), ties=(), mass_width=None, float_mw=(), scale=None, max_iter=3000, gtol=1e-3, errors=False, stream=None):
+        """native BFGS fit (amp_fit) of the couplings and, for float_mw = [(resonance, 0 mass | 1 width), ...], of masses and widths
+        -> dict(couplings [K] complex, mass_width [R][2] or None, nll, grad_max, converged, n_calls, iterations, free (slots),
+        covariance [n][n] or None (n = 2 F + len(float_mw)), errors complex [F] or None, mw_errors [len(float_mw)] or None)"""
         c = np.asarray(c_start, dtype=np.complex128)
         assert c.shape == (self.K,)
         hc = np.ascontiguousarray(np.stack([c.real, c.imag], -1))
@@ -208,20 +209,24 @@ class Model:
         fx = np.ascontiguousarray(list(fixed), dtype=np.int32)
         td = np.ascontiguousarray([t[0] for t in ties], dtype=np.int32)
         ts = np.ascontiguousarray([t[1] for t in ties], dtype=np.int32)
+        fm = np.ascontiguousarray([[int(r), int(w)] for r, w in float_mw], dtype=np.int32).reshape(-1, 2)
         hs = None if scale is None else np.ascontiguousarray(scale, dtype=np.float64)
         free = [k for k in range(self.K) if k not in set(int(f) for f in fixed) and k not in set(int(t) for t in td)]
-        nf = 2 * len(free)
+        n = 2 * len(free) + len(fm)
         out, nll, info = np.empty((self.K, 2)), np.empty(2), np.zeros(5, dtype=np.int32)
-        cov = np.empty((nf, nf)) if errors else None
+        out_mw = np.empty((self.R, 2)) if hmw is not None else None
+        cov = np.empty((n, n)) if errors else None
         p = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None and a.size else None
-        self._check(lib().amp_fit(self._h, p(hc), p(hmw), p(fx), len(fx), p(td), p(ts), len(td), p(hs), int(max_iter), float(gtol),
-                                  p(out), p(nll), p(cov), p(info), _stream_ptr(stream)), "amp_fit")
+        self._check(lib().amp_fit(self._h, p(hc), p(hmw), p(fx), len(fx), p(td), p(ts), len(td), p(fm), len(fm), p(hs), int(max_iter), float(gtol),
+                                  p(out), p(out_mw), p(nll), p(cov), p(info), _stream_ptr(stream)), "amp_fit")
         self.P = 1
-        res = {"couplings": out[:, 0] + 1j * out[:, 1], "nll": float(nll[0]), "grad_max": float(nll[1]), "converged": bool(info[0]),
-               "n_calls": int(info[1]), "iterations": int(info[2]), "free": free, "covariance": cov, "errors": None}
+        res = {"couplings": out[:, 0] + 1j * out[:, 1], "mass_width": out_mw, "nll": float(nll[0]), "grad_max": float(nll[1]),
+               "converged": bool(info[0]), "n_calls": int(info[1]), "iterations": int(info[2]), "free": free, "covariance": cov,
+               "errors": None, "mw_errors": None}
         if errors and info[3]:
-            sig = np.sqrt(np.diag(cov)).reshape(-1, 2)
-            res["errors"] = sig[:, 0] + 1j * sig[:, 1]
+            sig = np.sqrt(np.diag(cov))
+            res["errors"] = sig[:2 * len(free):2] + 1j * sig[1:2 * len(free):2]
+            res["mw_errors"] = sig[2 * len(free):]
         return res
 
     def generate(self, seed, first, n_candidates, f_max, m_lo, m_hi, cos_max, capacity, with_index=False, stream=None):

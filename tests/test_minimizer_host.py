@@ -37,11 +37,11 @@ def stub(tmp_path_factory):
     lib = C.CDLL(out)
     vp, i, d = C.c_void_p, C.c_int, C.c_double
     lib.amp_fit.restype = i
-    lib.amp_fit.argtypes = [vp, vp, vp, vp, i, vp, vp, i, vp, i, d, vp, vp, vp, vp, vp]
+    lib.amp_fit.argtypes = [vp, vp, vp, vp, i, vp, vp, i, vp, i, vp, i, d, vp, vp, vp, vp, vp, vp]
     return lib
 
 
-def run(lib, start, fixed=(), ties=(), scale=None, max_iter=3000, gtol=1e-7, cov=True):
+def run(lib, start, fixed=(), ties=(), scale=None, max_iter=3000, gtol=1e-7, cov=True, mw=None, float_mw=()):
     p = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None and a.size else None
     hs = np.ascontiguousarray(start, dtype=np.float64).reshape(K, 2)
     fx = np.ascontiguousarray(fixed, dtype=np.int32)
@@ -49,9 +49,15 @@ def run(lib, start, fixed=(), ties=(), scale=None, max_iter=3000, gtol=1e-7, cov
     ts = np.ascontiguousarray([t[1] for t in ties], dtype=np.int32)
     sc = None if scale is None else np.ascontiguousarray(scale, dtype=np.float64)
     nfree = K - len(set(fixed)) - len(td)
-    fit, nll, info = np.empty((K, 2)), np.empty(2), np.zeros(5, dtype=np.int32)
-    cv = np.empty((2 * nfree, 2 * nfree)) if cov else None
-    st = lib.amp_fit(C.c_void_p(1), p(hs), None, p(fx), len(fx), p(td), p(ts), len(td), p(sc), max_iter, gtol, p(fit), p(nll), p(cv), p(info), None)
+    fm = np.ascontiguousarray(float_mw, dtype=np.int32).reshape(-1, 2)
+    hmw = None if mw is None else np.ascontiguousarray(mw, dtype=np.float64).reshape(1, 2)
+    fit, nll, info, fit_mw = np.empty((K, 2)), np.empty(2), np.zeros(5, dtype=np.int32), np.zeros((1, 2))
+    n = 2 * nfree + len(fm)
+    cv = np.empty((n, n)) if cov else None
+    st = lib.amp_fit(C.c_void_p(1), p(hs), p(hmw), p(fx), len(fx), p(td), p(ts), len(td), p(fm), len(fm), p(sc), max_iter, gtol, p(fit),
+                     p(fit_mw), p(nll), p(cv), p(info), None)
+    if mw is not None:
+        return st, fit, nll, cv, info, fit_mw
     return st, fit, nll, cv, info
 
 
@@ -130,3 +136,45 @@ def test_bad_arguments_and_domain_backoff(stub):
     far[0] = 49.9
     st, fit, nll, cov, info = run(stub, far, cov=False)
     assert st == 0 and info[0] == 1 and abs(fit[0, 0] - 1.0) < 1e-6
+
+
+def test_floating_mass_and_width(stub):
+    """masses and widths as parameters: derivative by central differences of a batch, coupled to the couplings (the stand-in has
+    cross terms M x Re H_0 and M x Gamma); minimum, covariance and the fixed-width variant against the closed form"""
+    MS, GS, QA, QB, QC, QE = 4196.0, 370.0, 0.04, 0.01, 0.1, 0.005
+    start = np.full(2 * K, 0.5)
+    st, fit, nll, cov, info, fmw = run(stub, start, mw=(4230.0, 330.0), float_mw=[(0, 0), (0, 1)], gtol=1e-6)
+    assert st == 0 and info[0] == 1 and info[3] == 1 and info[4] == 2 * K + 2
+    assert abs(fmw[0, 0] - MS) < 1e-4 and abs(fmw[0, 1] - GS) < 1e-4
+    assert np.max(np.abs(fit.ravel() - (1.0 + 0.1 * np.arange(2 * K)))) < 1e-6
+    H = np.zeros((2 * K + 2, 2 * K + 2))
+    H[:2 * K, :2 * K] = np.diag(lam(np.arange(2 * K))) + 0.3 * (np.eye(2 * K, k=1) + np.eye(2 * K, k=-1))
+    H[2 * K, 2 * K], H[2 * K + 1, 2 * K + 1] = QA, QB
+    H[2 * K, 0] = H[0, 2 * K] = QC
+    H[2 * K, 2 * K + 1] = H[2 * K + 1, 2 * K] = QE
+    ref = np.linalg.inv(H)
+    assert np.max(np.abs(cov - ref) / np.sqrt(np.outer(np.diag(ref), np.diag(ref)))) < 1e-4
+    # only the mass floats; the width stays at its (wrong) start value: the minimum in M shifts by -QE (G - G*) / QA (+ the H_0 coupling)
+    st, fit, nll, cov, info, fmw = run(stub, start, mw=(4230.0, 330.0), float_mw=[(0, 0)], gtol=1e-6)
+    assert st == 0 and info[0] == 1 and fmw[0, 1] == 330.0 and info[4] == 2 * K + 1
+    from scipy.optimize import minimize
+
+    def red(t):                                                   # (H, M) at G = 330, the stand-in's formula retyped in numpy
+        f, g = f_and_grad(t[:2 * K])
+        dM, dG, d0 = t[2 * K] * 100.0 - MS, 330.0 - GS, t[0] - 1.0
+        f += 0.5 * QA * dM * dM + 0.5 * QB * dG * dG + QC * dM * d0 + QE * dM * dG
+        g = np.append(g, (QA * dM + QC * d0 + QE * dG) * 100.0)
+        g[0] += QC * dM
+        return f, g
+
+    r = minimize(red, np.append(fit.ravel(), 42.0), jac=True, method="BFGS", options={"gtol": 1e-10})
+    assert abs(fmw[0, 0] - r.x[2 * K] * 100.0) < 1e-3 and abs(fmw[0, 0] - MS) > 1.0
+    assert abs(nll[0] - r.fun) < 1e-8
+    # bad specifications
+    assert run(stub, start, mw=(4230.0, 330.0), float_mw=[(1, 0)])[0] == 1      # resonance index out of range
+    assert run(stub, start, mw=(4230.0, 330.0), float_mw=[(0, 2)])[0] == 1
+    assert run(stub, start, mw=(4230.0, 330.0), float_mw=[(0, 0), (0, 0)])[0] == 1
+    assert run(stub, start, float_mw=[(0, 0)])[0] == 1                            # floating without start values
+    # a start whose first steps would make the width negative: the stand-in refuses, the search backs off and still converges
+    st, fit, nll, cov, info, fmw = run(stub, start, mw=(4230.0, 3.0), float_mw=[(0, 0), (0, 1)], gtol=1e-6, cov=False)
+    assert st == 0 and info[0] == 1 and abs(fmw[0, 1] - GS) < 1e-3
