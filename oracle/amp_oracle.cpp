@@ -512,6 +512,48 @@ void nll_gradient_impl(const Model<T>& M, const std::complex<T>* c, const double
     }
 }
 
+// Gradient with background and purity, Eq. 14: NLL = - sum_i log f_i, f_i = (p / I) eps_i S_i + (1 - p) b_i,
+// I = W / sum_j w_j, W = sum_j w_j S_j.  With u_i = (p / I) eps_i / f_i:
+//   dNLL/dconj(c_k) = - sum_i u_i [sum_xi conj(B_k,xi(i)) A_xi(i)]  +  [sum_i u_i S_i] [sum_j w_j sum_xi conj(B_k,xi(j)) A_xi(j)] / W
+// (the second term is the derivative of 1/I); without background u_i = 1 / S_i and sum_i u_i S_i = N: nll_gradient_impl.
+template <typename T>
+void nll_gradient_bkg_impl(const Model<T>& M, const std::complex<T>* c, const double* x, const double* eff, const double* bkg, double purity,
+                           long long n, const double* xn, const double* wn, long long mn, double* nll_out, double* grad_out) {
+    using C = std::complex<T>;
+    const int K = M.num_couplings();
+    std::vector<C> B(2 * K), D(K, C(0, 0)), Nk(K, C(0, 0));
+    Neumaier<T> slog, swS, sw, suS;
+    for (long long j = 0; j < mn; ++j) {
+        const T xj[4] = {T(xn[j]), T(xn[mn + j]), T(xn[2 * mn + j]), T(xn[3 * mn + j])};
+        basis_terms(M, xj, B.data());
+        C A[2] = {C(0, 0), C(0, 0)};
+        for (int k = 0; k < K; ++k) { A[0] += c[k] * B[2 * k]; A[1] += c[k] * B[2 * k + 1]; }
+        const T w = wn ? T(wn[j]) : T(1);
+        swS.add(w * (std::norm(A[0]) + std::norm(A[1])));
+        sw.add(w);
+        for (int k = 0; k < K; ++k) Nk[k] += w * (std::conj(B[2 * k]) * A[0] + std::conj(B[2 * k + 1]) * A[1]);
+    }
+    const T I = swS.value() / sw.value(), p = T(purity);
+    for (long long i = 0; i < n; ++i) {
+        const T xi[4] = {T(x[i]), T(x[n + i]), T(x[2 * n + i]), T(x[3 * n + i])};
+        basis_terms(M, xi, B.data());
+        C A[2] = {C(0, 0), C(0, 0)};
+        for (int k = 0; k < K; ++k) { A[0] += c[k] * B[2 * k]; A[1] += c[k] * B[2 * k + 1]; }
+        const T S = std::norm(A[0]) + std::norm(A[1]), e = eff ? T(eff[i]) : T(1);
+        const T f = (p / I) * e * S + (1 - p) * T(bkg[i]);
+        slog.add(std::log(f));
+        const T u = (p / I) * e / f;
+        suS.add(u * S);
+        for (int k = 0; k < K; ++k) D[k] += u * (std::conj(B[2 * k]) * A[0] + std::conj(B[2 * k + 1]) * A[1]);
+    }
+    *nll_out = double(-slog.value());
+    for (int k = 0; k < K; ++k) {
+        const C g = -D[k] + suS.value() * Nk[k] / swS.value();
+        grad_out[2 * k] = double(2 * g.real());
+        grad_out[2 * k + 1] = double(2 * g.imag());
+    }
+}
+
 // Hermitian normalisation matrix M_kl = sum_j w_j sum_xi conj(B_k xi) B_l xi / sum_j w_j (pin P10,
 // fit fractions Eq. 13).  out is [K][K][2] row-major.
 template <typename T>
@@ -655,6 +697,14 @@ void orc_nll_gradient(const double* decay, int n_res, const int* kinds, const in
     auto M = make_model<double>(decay, n_res, kinds, Js, mass, width, radius);
     auto c = make_couplings<double>(couplings, M.num_couplings());
     nll_gradient_impl(M, c.data(), x, eff, n, xn, wn, mn, nll_out, grad_out);
+}
+
+void orc_nll_gradient_bkg(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass, const double* width,
+                          const double* radius, const double* couplings, const double* x, const double* eff, const double* bkg,
+                          double purity, long long n, const double* xn, const double* wn, long long mn, double* nll_out, double* grad_out) {
+    auto M = make_model<double>(decay, n_res, kinds, Js, mass, width, radius);
+    auto c = make_couplings<double>(couplings, M.num_couplings());
+    nll_gradient_bkg_impl(M, c.data(), x, eff, bkg, purity, n, xn, wn, mn, nll_out, grad_out);
 }
 
 void orc_norm_matrix(const double* decay, int n_res, const int* kinds, const int* Js, const double* mass, const double* width,

@@ -37,6 +37,7 @@ _lib.orc_nll.restype = _i
 _lib.orc_nll.argtypes = _MODEL + [_i, _pd, _vp, _pd, _vp, _ll, _pd, _vp, _ll, _i, _vp, _vp]
 _lib.orc_norm_matrix.argtypes = _MODEL + [_pd, _vp, _ll, _pd]
 _lib.orc_nll_gradient.argtypes = _MODEL + [_pd, _pd, _vp, _ll, _pd, _vp, _ll, _pd, _pd]
+_lib.orc_nll_gradient_bkg.argtypes = _MODEL + [_pd, _pd, _vp, _pd, _d, _ll, _pd, _vp, _ll, _pd, _pd]
 
 KSTAR, ZRES, CONST, LASS, ZNEG = 0, 1, 2, 3, 4
 
@@ -164,6 +165,17 @@ class Model:
         kw, pw = _opt(wn)
         nll, grad = np.zeros(1), np.zeros((self.K, 2))
         _lib.orc_nll_gradient(*self._args(), c, x, pe, x.shape[1], xn, pw, xn.shape[1], nll, grad)
+        return nll[0], grad
+
+    def nll_gradient_background(self, couplings, x, eff, bkg, purity, xn, wn):
+        """(NLL, grad [K][2]) of Eq. 14 (background + purity), the derivative written out event by event"""
+        c = _f64(np.stack([np.real(couplings), np.imag(couplings)], -1))
+        assert c.shape == (self.K, 2)
+        x, xn, bkg = _f64(x), _f64(xn), _f64(bkg)
+        ke, pe = _opt(eff)
+        kw, pw = _opt(wn)
+        nll, grad = np.zeros(1), np.zeros((self.K, 2))
+        _lib.orc_nll_gradient_bkg(*self._args(), c, x, pe, bkg, float(purity), x.shape[1], xn, pw, xn.shape[1], nll, grad)
         return nll[0], grad
 
     def nll_background(self, couplings, x, eff, bkg, purity, xn, wn, mass_width=None):

@@ -761,3 +761,35 @@ def test_P20_spin0_z_density_closed_form():
         assert abs(S2[i] - abs(A) ** 2 * d200 ** 2 * zk["sinT"] ** 2) < 1e-11 * S2[i] + 1e-40
         d1p = sum(float(N(Rotation.d(1, 1, xi, thT).doit(), 30)) ** 2 for xi in (1, -1))
         assert abs(S2p[i] - abs(A) ** 2 * d201 ** 2 * d1p) < 1e-11 * S2p[i] + 1e-40
+
+
+# ------------------------------------------------------------------ P21: gradient with background and purity (Eq. 14)
+def test_P21_background_gradient():
+    """(i) central finite differences of the plain-definition NLL of Eq. 14 (Model.nll_background: a different code path, python +
+    fsum) in every coupling; (ii) purity 1: the signal-only gradient; (iii) a background of the signal's own shape leaves the NLL
+    stationary in the overall scale of the couplings at any purity (Euler: sum_k conj(c_k) dNLL/dconj(c_k) = 0 still holds, since
+    f is homogeneous of degree 0 in c)"""
+    cfg = 2
+    M = model(cfg)
+    c = W.couplings(cfg)
+    xn, wn = W.norm_events(cfg, 3000)
+    x, eff = W.data_events(cfg, lambda xx, ee: M.eval_events(c, xx, ee), n=250)
+    rng = np.random.default_rng(14)
+    b = rng.uniform(0.2, 2.0, x.shape[1]) * np.mean(M.eval_events(c, x, eff)) / M.norm_integral(c, xn, wn)[0]
+    for purity in (0.85, 0.4):
+        nll, g = M.nll_gradient_background(c, x, eff, b, purity, xn, wn)
+        assert abs(nll - M.nll_background(c, x, eff, b, purity, xn, wn)[0]) < 1e-12 * abs(nll)
+        gmax = np.max(np.abs(g))
+        for k in range(len(c)):
+            for part, d in ((0, 1.0), (1, 1.0j)):
+                h = 1e-4 * max(abs(c[k]), 0.1)
+                cp, cm = c.copy(), c.copy()
+                cp[k] += h * d
+                cm[k] -= h * d
+                fd = (M.nll_background(cp, x, eff, b, purity, xn, wn)[0] - M.nll_background(cm, x, eff, b, purity, xn, wn)[0]) / (2 * h)
+                assert abs(fd - g[k, part]) < 2e-6 * gmax, (purity, k, part, fd, g[k, part])
+        euler = np.sum(np.conj(c) * (g[:, 0] + 1j * g[:, 1]) / 2)
+        assert abs(euler) < 1e-10 * gmax * np.max(np.abs(c))
+    n1, g1 = M.nll_gradient_background(c, x, eff, b, 1.0, xn, wn)
+    n0, g0 = M.nll_gradient(c, x, eff, xn, wn)
+    assert abs(n1 - n0) < 1e-12 * abs(n0) and np.max(np.abs(g1 - g0)) < 1e-11 * np.max(np.abs(g0))
