@@ -646,7 +646,8 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
     m->want_matrix = m->norm_mode == 2 || (m->norm_mode == 0 && (P == 1 ? mw_same : (P >= 24 && m->batch_mode != 1)));
     if (P == 1) m->prev_mw = m->mw; else m->prev_mw.clear();
     // P > 1: a batch whose points are sparse changes of point 0 (a gradient step) runs the delta kernel: no column, no matrix
-    if (m->has_bkg) m->want_matrix = false;   // Eq. 14: the background path streams both samples, point by point
+    if (m->has_bkg && P > 1) m->want_matrix = false;   // Eq. 14: the background path streams both samples, point by point (a single
+                                                          // point at fixed lineshapes may still hold M: amp_nll_grad reads it)
     m->use_delta = P > 1 && !m->has_bkg && m->batch_mode == 0 && m->lineshape_mode != 1 && m->norm_mode != 2 && build_delta_plan(m);
     if (m->use_delta) m->want_matrix = false;
     m->stream_inline = (P == 1 || m->use_delta || m->has_bkg) && m->lineshape_mode != 1;
@@ -1569,7 +1570,6 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
     if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
     if (!m->data.loaded) return fail(m, AMP_ERR_STATE, "no data events loaded (amp_load_events)");
     if (m->P != 1) return fail(m, AMP_ERR_STATE, "amp_nll_grad: set exactly one parameter point (amp_set_params with P = 1)");
-    if (m->has_bkg) return fail(m, AMP_ERR_STATE, "amp_nll_grad: not available with a background (Eq. 14)");
     for (const auto& rs : m->res)
         if (rs.kind == AMP_LASS) return fail(m, AMP_ERR_STATE, "amp_nll_grad: not available for models with a LASS term");
     if (!m->stream_inline) return fail(m, AMP_ERR_STATE, "amp_nll_grad: needs lineshapes in registers (amp_set_lineshape_mode 0 or 2)");
@@ -1606,6 +1606,21 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
                 g.a.qf_c[k] = k < m->K ? make_double2(m->couplings[2 * k], m->couplings[2 * k + 1]) : make_double2(0, 0);
         }
     }
+    int extra_launches = 0;
+    if (m->has_bkg) {   // Eq. 14: the data side needs sum_j w_j S_j before its first event
+        g.a.bkg = m->d_bkg;
+        g.a.purity = m->purity;
+        if (!g.a.qf_G) {   // lineshapes moved: a normalisation launch first (the gradient kernel walks that sample again for N_k)
+            StreamArgs a;
+            fill_stream_args(m, m->norm, 0, MODE_NORM, &a);
+            a.partial = m->d_partial + (size_t)400 * PARTIAL_STRIDE;   // rows the gradient kernel does not use
+            const int gn = stream_grid(m->norm.n, m->has_z, MODE_NORM);
+            CK(launch_stream(a, gn, s));
+            CK(launch_finalize(a.partial, gn, PARTIAL_STRIDE, 1, m->d_sums + 1, s));
+            g.a.sum_wS = m->d_sums + 1;
+            extra_launches = 2;
+        }
+    }
     const int K = m->K;
     g.K = K;
     g.npairs = (K + 15) / 16 * 16;
@@ -1632,7 +1647,7 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
     CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
     CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (3 + 2 * K), cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
-    m->stat_launches = 1;
+    m->stat_launches = 1 + extra_launches;
     m->stat_columns = 0;
     m->stat_norm_path = 7;
     m->fused_valid = true;

@@ -77,9 +77,38 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
         issue(blockIdx.x, 0);
         if (have_z) issue(blockIdx.x, 1);
     }
+    // Eq. 14 (background + purity): f_i = ps eps_i S_i + qb b_i with ps = purity / I, I = W / sum_j w_j, W = sum_j w_j S_j.  W is needed
+    // before the first data event: from the held matrix (c^H M c, every CTA the same fixed-order sum) or from the normalisation
+    // launch the host ran before this one.
+    double bkg_ps = 0.0, bkg_qb = 0.0;
+    if (a.bkg) {
+        __shared__ double s_W;
+        if (a.qf_G) {
+            double r = 0.0;
+            if (tid < a.qf_nent) {
+                double2 acc = make_double2(0.0, 0.0);
+                for (int f = 0; f < a.qf_nent; ++f) {
+                    const double2 cf = a.qf_c[f];
+                    const double* gm = a.qf_G + (size_t)(2 * tid) * a.qf_KP + 2 * f;
+                    const double mre = gm[0] + gm[a.qf_KP + 1], mim = gm[1] - gm[a.qf_KP];
+                    acc.x += mre * cf.x - mim * cf.y;
+                    acc.y += mre * cf.y + mim * cf.x;
+                }
+                r = a.qf_c[tid].x * acc.x + a.qf_c[tid].y * acc.y;
+            }
+            const double t = block_sum(r, sm);
+            if (tid == 0) s_W = t;
+        } else if (tid == 0) {
+            s_W = __ldcg(a.sum_wS);
+        }
+        __syncthreads();
+        bkg_ps = a.purity * a.wsum / s_W;
+        bkg_qb = 1.0 - a.purity;
+    }
     double2* bw_rec = bw_base + tid;
     const double* st = stage + tid;
-    double accF = 1.0, accW = 0.0;   // sum log S as mantissa product / exponent sum; sum w S
+    double accF = 1.0, accW = 0.0;   // sum log S (log f with a background) as mantissa product / exponent sum; sum w S
+    double accT = 0.0;               // background: sum_i u_i S_i, u_i = ps eps_i / f_i (= N without a background)
     int accE = 0;
     bool bad = false;
     uint32_t parity = 0;
@@ -164,6 +193,16 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
             bad |= live && !isfinite(S);
             accW = fma(wgt, S, accW);        // padding events carry w = 0
             u = wgt;
+        } else if (a.bkg) {
+            const double f0 = fma(bkg_ps * wgt, S, bkg_qb * (live ? a.bkg[lt * TILE + tid] : 1.0));
+            const bool ok = f0 > 0.0 && isfinite(f0);
+            bad |= live && !ok;
+            double f; int x1, x2;
+            split_exp((live && ok) ? f0 : 1.0, &f, &x1);
+            split_exp(accF * f, &accF, &x2);
+            accE += x1 + x2;
+            u = (live && ok) ? bkg_ps * wgt / f0 : 0.0;
+            accT = fma(u, S, accT);
         } else {
             const bool ok = S > 0.0 && isfinite(S);
             bad |= live && !ok;
@@ -222,7 +261,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
     {
         const double t0 = block_sum(log(accF) + (double)accE * LN2, sm);
         const double t1 = block_sum(accW, sm);
-        if (tid == 0) { g.partial[(size_t)0 * g.stride + blockIdx.x] = t0; g.partial[(size_t)1 * g.stride + blockIdx.x] = t1; }
+        const double t2 = block_sum(accT, sm);
+        if (tid == 0) {
+            g.partial[(size_t)0 * g.stride + blockIdx.x] = t0;
+            g.partial[(size_t)1 * g.stride + blockIdx.x] = t1;
+            g.partial[(size_t)(2 + 2 * nleaf) * g.stride + blockIdx.x] = t2;
+        }
     }
     __syncthreads();
     for (int idx = tid; idx < nleaf; idx += THREADS) {
@@ -242,8 +286,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    double* tot = accD;   // [2 + 2 nleaf] (<= 194 doubles; the accumulators are dead)
-    const int rows = 2 + 2 * nleaf;
+    double* tot = accD;   // [3 + 2 nleaf] (<= 195 doubles; the accumulators are dead)
+    const int rows = 3 + 2 * nleaf;
     for (int r = tid; r < rows; r += THREADS) {
         const double* p = g.partial + (size_t)r * g.stride;
         double s = 0.0;
@@ -282,16 +326,18 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
         __syncthreads();
     }
     const double swS = tot[1];
+    // with a background (Eq. 14) the data-side weights are u_i = ps eps_i / f_i and N is replaced by T = sum_i u_i S_i
+    const double Tn = a.bkg ? tot[2 + 2 * nleaf] : nd;
     for (int p = tid; p < g.npairs; p += THREADS) {
         const int kslot = g.pair_slot[p];
         if (kslot < 0) continue;
         // dNLL/dconj(c_k) = -D_k + N N_k / sum_j w_j S_j ; (d/dRe, d/dIm) = 2 (Re, Im)
-        g.result[3 + 2 * kslot] = 2.0 * (-tot[2 + 2 * p] + nd * tot[2 + nleaf + 2 * p] / swS);
-        g.result[3 + 2 * kslot + 1] = 2.0 * (-tot[2 + 2 * p + 1] + nd * tot[2 + nleaf + 2 * p + 1] / swS);
+        g.result[3 + 2 * kslot] = 2.0 * (-tot[2 + 2 * p] + Tn * tot[2 + nleaf + 2 * p] / swS);
+        g.result[3 + 2 * kslot + 1] = 2.0 * (-tot[2 + 2 * p + 1] + Tn * tot[2 + nleaf + 2 * p + 1] / swS);
     }
     if (tid == 0) {
         const double I = swS / a.wsum;
-        double v = -(tot[0] + a.sum_log_eff) + nd * log(I);
+        double v = a.bkg ? -tot[0] : -(tot[0] + a.sum_log_eff) + nd * log(I);
         if (!isfinite(v) || !(I > 0.0)) v = INFINITY;
         g.result[0] = v;
         g.result[1] = I;

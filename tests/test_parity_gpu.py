@@ -505,6 +505,54 @@ def test_background_and_purity_match_oracle():
     assert abs(Mg.nll()[0] - base) < 1e-12 * abs(base) and Mg.last_call_stats()["norm_path"] in (2, 4)   # signal-only paths again
 
 
+@pytest.mark.parametrize("cfg,n,m", [(2, 7001, 20011), (1, 513, 1500)])
+def test_analytic_gradient_with_background(cfg, n, m):
+    """amp_nll_grad under Eq. 14 (background + purity): the data-side weights become purity eps / (I f_i) and N becomes
+    sum_i u_i S_i.  Lineshapes just moved (a normalisation launch first, then the gradient kernel over both samples), then
+    fixed (sum w S from the held matrix M inside the kernel); purity 1 gives the signal-only gradient; a fit loop runs on it."""
+    Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+    c = W.couplings(cfg)
+    x, eff, xn, wn = make_inputs(cfg, n, m)
+    rng = np.random.default_rng(9)
+    I0 = Mo.norm_integral(c, xn, wn)[0]
+    bkg = np.mean(Mo.eval_events(c, x, eff)) / I0 * (1.0 + 0.5 * x[1]) * (1.0 + 0.3 * np.cos(x[3])) * rng.uniform(0.8, 1.2, x.shape[1])
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    Mg.set_background(dev(bkg), 0.8)
+    mw = W.step_mass_width(3, 2)[:len(W.resonances(cfg))]
+    res2 = [(r[0], r[1], mw[i, 0], mw[i, 1], r[4]) for i, r in enumerate(W.resonances(cfg))]
+    Mo2 = O.Model(W.DECAY, res2)
+    Mg.set_params(c, mw[None])
+    nll, g = Mg.nll_grad()
+    st = Mg.last_call_stats()
+    assert st["norm_path"] == 7 and st["launches"] == 3
+    rn, rg = Mo2.nll_gradient_background(c, x, eff, bkg, 0.8, xn, wn)
+    assert abs(nll - rn) < RTOL_NLL * abs(rn), (nll, rn)
+    assert np.max(np.abs(g - rg)) < 1e-9 * np.max(np.abs(rg)), np.max(np.abs(g - rg)) / np.max(np.abs(rg))
+    assert abs(Mg.nll()[0] - nll) < 1e-12 * abs(nll)                      # the NLL of amp_nll (path 6) is the same number
+    c2 = c * (1 + 0.05 * np.cos(np.arange(len(c)))) * np.exp(0.05j * np.sin(np.arange(len(c))))
+    Mg.set_params(c2, mw[None])                                           # same lineshapes: matrix M
+    nll2, g2 = Mg.nll_grad()
+    assert Mg.last_call_stats()["launches"] == 1
+    rn2, rg2 = Mo2.nll_gradient_background(c2, x, eff, bkg, 0.8, xn, wn)
+    assert abs(nll2 - rn2) < RTOL_NLL * abs(rn2)
+    assert np.max(np.abs(g2 - rg2)) < 1e-9 * np.max(np.abs(rg2))
+    Mg.set_params(c2, mw[None])
+    nll3, g3 = Mg.nll_grad()
+    assert nll3 == nll2 and np.array_equal(g3, g2)                        # bit-reproducible
+    # purity 1: f = eps S / I, the signal-only likelihood
+    Mg.set_background(dev(bkg), 1.0)
+    Mg.set_params(c2, mw[None])
+    nll4, g4 = Mg.nll_grad()
+    r4, rg4 = Mo2.nll_gradient(c2, x, eff, xn, wn)
+    assert abs(nll4 - r4) < RTOL_NLL * abs(r4) and np.max(np.abs(g4 - rg4)) < 1e-9 * np.max(np.abs(rg4))
+    # the native fit runs on it: the NLL does not go up and the gradient at the result is small
+    Mg.set_background(dev(bkg), 0.8)
+    fixed = [k for k, (r, lam) in enumerate(W.slot_table(W.resonances(cfg))) if r == 1 and lam == 0]
+    r = Mg.fit(c2, fixed=fixed, mass_width=mw, gtol=1e-3, max_iter=400)
+    assert r["nll"] <= nll2 and r["grad_max"] < 0.05 * np.max(np.abs(g2))
+
+
 def test_two_z_model_matches_oracle():
     """SURVEY.md 8(f)-3 / PAPER.md:165, 191 ("ten K*s and two Zs"): a second 1+ exotic, Z(4430) (m = 4478, Gamma = 181 MeV), shares
     the Z(4200)'s decay frame and angular cache; K = 30.  Per-event density, fused NLL with all 12 lineshapes moving, and a
