@@ -126,8 +126,12 @@ amp_status amp_nll(amp_model* m, double* h_nll, void* stream);
  *   h_nll host [1]; h_grad host [K][2] = (dNLL/dRe H_k, dNLL/dIm H_k) in slot order, from
  *   dNLL/dconj(H_k) = - sum_i [sum_xi conj(B_k,xi) A_xi]_i / S_i + N [sum_j w_j sum_xi conj(B_k,xi) A_xi]_j / [sum_j w_j S_j].
  * Replaces the 2 K finite-difference points a minimiser would spend on the couplings (masses and widths still go through
- * a gradient batch).  Constraints such as Eq. 6 / Eq. 11 are the caller's chain rule.  Not available with a background or
- * for models with a LASS term (AMP_ERR_STATE).  Deterministic.  Path 7 in amp_last_call_stats.                       */
+ * a gradient batch; amp_fit does both).  Constraints such as Eq. 6 / Eq. 11 are the caller's chain rule.  With masses and
+ * widths unchanged since the previous amp_set_params the normalisation side comes from the held matrix M ((M c)_k, c^H M c) and
+ * only the data events are walked.  With a background (amp_set_background, Eq. 14) the data-side weights are
+ * purity eps_i / (I f_i) and N becomes sum_i u_i S_i; sum_j w_j S_j is then needed first: from M inside the kernel, or from a
+ * normalisation launch before it (3 launches).  Models with LASS terms and Zs of any spin-parity are covered.
+ * Deterministic.  Path 7 in amp_last_call_stats.                                                                        */
 amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* stream);
 
 /* Fit in native code (the paper's MINUIT loop, with the analytic gradient in place of finite differences for the

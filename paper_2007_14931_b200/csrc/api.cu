@@ -1570,14 +1570,12 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
     if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
     if (!m->data.loaded) return fail(m, AMP_ERR_STATE, "no data events loaded (amp_load_events)");
     if (m->P != 1) return fail(m, AMP_ERR_STATE, "amp_nll_grad: set exactly one parameter point (amp_set_params with P = 1)");
-    for (const auto& rs : m->res)
-        if (rs.kind == AMP_LASS) return fail(m, AMP_ERR_STATE, "amp_nll_grad: not available for models with a LASS term");
     if (!m->stream_inline) return fail(m, AMP_ERR_STATE, "amp_nll_grad: needs lineshapes in registers (amp_set_lineshape_mode 0 or 2)");
     if (m->K > GRAD_MAX_PAIRS) return fail(m, AMP_ERR_INVALID, "amp_nll_grad: too many couplings");
     int ent_of_res[AMP_MAX_RESONANCES], grp_of_res[AMP_MAX_RESONANCES];
     GradArgs g{};
     fill_stream_args(m, m->data, 0, MODE_FUSED, &g.a, ent_of_res, grp_of_res);
-    int nent = 0;
+    int nent = g.a.nlass;
     for (int sp = 0; sp < NSPIN; ++sp) nent += g.a.shape[sp];
     if (!grad_fits(nent, g.a.gstart[NSPIN])) return fail(m, AMP_ERR_INVALID, "amp_nll_grad: the model does not fit the kernel's shared memory");
     g.a.cache2 = m->norm.cache; g.a.n2 = m->norm.n; g.a.npad2 = m->norm.npad;

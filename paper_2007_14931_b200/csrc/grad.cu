@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
     const int tid = threadIdx.x, lane = tid & 31;
     const bool have_z = a.gstart[NSPIN] > a.gstart[5];
     const int ncache = have_z ? NCOL_ALL : NCOL_K;
-    int nent = 0;
+    int nent = a.nlass;   // Breit-Wigner entries of all spin classes + the LASS terms (stored after them)
     for (int sp = 0; sp < NSPIN; ++sp) nent += a.shape[sp];
     const int nleaf = 2 * g.npairs, nblk = nleaf / 32;
 
@@ -143,6 +143,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
         AMP_GSPIN(3, 2)
         AMP_GSPIN(4, 3)
 #undef AMP_GSPIN
+        for (int t = a.lass0; t < a.lass0 + a.nlass; ++t) {   // LASS S-wave terms (Eq. 7): J = 0, lambda = 0, no constant folded in
+            const double2 bw = lass_eval(a.ent[t].M2, a.ent[t].kG, k.m2, invm, q);
+            bw_rec[t * TILE] = bw;
+            V0 = cfma(a.ent[t].c0, bw, V0);
+        }
         {
             const double hp = 0.5 * (1.0 + cpsi), hm = 0.5 * (1.0 - cpsi);
             k.h0 = RSQRT2 * spsi;
@@ -367,7 +372,7 @@ cudaError_t launch_grad(const GradArgs& g, int grid, cudaStream_t s) {
     cudaError_t e = cudaSuccess;
     if (!attr_done) { e = cudaFuncSetAttribute(k_grad, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
     if (e != cudaSuccess) return e;
-    int nent = 0;
+    int nent = g.a.nlass;
     for (int sp = 0; sp < NSPIN; ++sp) nent += g.a.shape[sp];
     k_grad<<<grid, THREADS, grad_smem(g.a.gstart[NSPIN] > g.a.gstart[5], nent), s>>>(g);
     return cudaGetLastError();

@@ -505,6 +505,41 @@ def test_background_and_purity_match_oracle():
     assert abs(Mg.nll()[0] - base) < 1e-12 * abs(base) and Mg.last_call_stats()["norm_path"] in (2, 4)   # signal-only paths again
 
 
+@pytest.mark.parametrize("with_z", [True, False])
+def test_lass_model_gradient_and_fit(with_z):
+    """amp_nll_grad and amp_fit for the paper's LASS variant of the model (Eq. 9): the LASS term is one more slot whose lineshape
+    record is A_LASS; lineshapes moved (both samples walked), fixed (matrix M), and a short fit"""
+    from paper_2007_14931_b200 import binding as B
+    res = W.resonances_lass(with_z)
+    c = W.couplings_lass(with_z)
+    Mo, Mg = O.Model(W.DECAY, res), B.Model(W.DECAY, res)
+    xn, wn = W.norm_events(2, 20011)
+    x, eff = W.data_events(2, lambda xx, ee: Mo.eval_events(c, xx, ee), n=5003)
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    mw = np.array([[r[2], r[3]] for r in res]) * (1 + 1e-3 * np.linspace(-1, 1, 2 * len(res)).reshape(-1, 2))
+    Mo2 = O.Model(W.DECAY, [(r[0], r[1], mw[i, 0], mw[i, 1], r[4]) for i, r in enumerate(res)])
+    Mg.set_params(c, mw[None])
+    nll, g = Mg.nll_grad()
+    rn, rg = Mo2.nll_gradient(c, x, eff, xn, wn)
+    assert abs(nll - rn) < RTOL_NLL * abs(rn)
+    assert np.max(np.abs(g - rg)) < 1e-9 * np.max(np.abs(rg)), np.max(np.abs(g - rg)) / np.max(np.abs(rg))
+    assert np.abs(rg[0]).max() > 1e-3 * np.max(np.abs(rg))                # the LASS slot's derivative is not a trivial zero
+    c2 = c * (1 + 0.04 * np.cos(np.arange(len(c))))
+    Mg.set_params(c2, mw[None])                                           # fixed lineshapes: matrix M
+    nll2, g2 = Mg.nll_grad()
+    rn2, rg2 = Mo2.nll_gradient(c2, x, eff, xn, wn)
+    assert abs(nll2 - rn2) < RTOL_NLL * abs(rn2)
+    assert np.max(np.abs(g2 - rg2)) < 1e-9 * np.max(np.abs(rg2))
+    slots = W.slot_table(res)
+    fixed = [k for k, (r, lam) in enumerate(slots) if res[r][0] == W.KSTAR and abs(res[r][2] - 895.55) < 1e-9 and lam == 0]
+    r = Mg.fit(c2, fixed=fixed, mass_width=mw, gtol=1e-3, max_iter=500)
+    assert r["nll"] < nll2 and r["grad_max"] < 0.02 * np.max(np.abs(g2))
+    # floating K0*(1430) mass and width inside the LASS term: derivative batch through the dense path
+    r3 = Mg.fit(r["couplings"], fixed=fixed, mass_width=mw, float_mw=[(0, 0), (0, 1)], gtol=1e-2, max_iter=60)
+    assert r3["nll"] <= r["nll"] + 1e-9
+
+
 @pytest.mark.parametrize("cfg,n,m", [(2, 7001, 20011), (1, 513, 1500)])
 def test_analytic_gradient_with_background(cfg, n, m):
     """amp_nll_grad under Eq. 14 (background + purity): the data-side weights become purity eps / (I f_i) and N becomes
