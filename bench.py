@@ -38,12 +38,13 @@ FLOP_PER_EVENT = 730.0
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # 148 SMs x 64 DFMA/clk x 2 flop x 1965 MHz
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed `ncu --set full` capture
 # (profiles/): per launch, at the default sizes; None until a capture of the current kernel exists
-TRAFFIC_NCU_BYTES = 2.192192e9 + 3.88e6       # profiles/r01c_ncu_full_stream_fused_cfg3.csv (2M + 10M events)
-TRAFFIC_NCU_BYTES_CFG4 = 2.192431e9 + 4.04e6  # profiles/r01c_ncu_full_delta_cfg4.csv
+TRAFFIC_NCU_BYTES = 2.192192e9 + 4.78e6       # profiles/r01d_ncu_full_stream_fused_cfg3.csv (2M + 10M events)
+TRAFFIC_NCU_BYTES_CFG4 = 2.194401e9 + 7.89e6  # profiles/r01d_ncu_full_delta_cfg4.csv
 # Algorithmic flop per event of the gradient batch of configs[4] in its sparse form: point 0 (730) + 31 slots
-# (Breit-Wigner of point 0 from the saved barrier factors ~20, angular factor ~8, two complex products 12) + 100 coupling
-# points (two complex multiply-adds 16, |A|^2 7, accumulate 2) + 20 mass/width points (perturbed Breit-Wigner ~22, the same 25)
-DELTA_FLOP_PER_EVENT = 730.0 + 31 * 40.0 + 100 * 25.0 + 20 * 47.0
+# (Breit-Wigner of point 0 from the saved barrier factors ~20, angular factor ~8, two complex products 12, and the expansion
+# coefficients T2 = 2 sum conj(A(0)) SLOT, n = sum |SLOT|^2: 25) + 100 coupling points (S(0) + Re(coef T2) + |coef|^2 n: 6, guard 1,
+# accumulate 1) + 20 mass/width points (perturbed Breit-Wigner ~22, difference to point 0 and |coef|^2: 5, expansion 6)
+DELTA_FLOP_PER_EVENT = 730.0 + 31 * 65.0 + 100 * 8.0 + 20 * 33.0
 # analytic gradient: the point (730) + per coupling slot: angular factor ~8, T = sum_xi conj(g) A 16, conj(BW) T 8, weight 2
 GRAD_FLOP_PER_EVENT = 730.0 + 27 * 34.0
 

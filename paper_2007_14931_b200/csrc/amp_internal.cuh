@@ -322,7 +322,7 @@ struct DeltaArgs {
     int want_nll;
     int first_chunk;                // 0: a later launch of the same call: the domain flag adds to the earlier launches'
 };
-cudaError_t launch_delta(const DeltaArgs& d, int grid, cudaStream_t s);
+cudaError_t launch_delta(const DeltaArgs& d, int grid, cudaStream_t s, bool exact = false);
 int delta_grid(long long n_data, long long n_norm);
 bool delta_fits(int ngrp);
 

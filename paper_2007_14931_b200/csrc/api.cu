@@ -88,6 +88,7 @@ struct amp_model {
     int* toy_count = nullptr;
     unsigned long long* toy_fseen = nullptr;
     long long toy_cap = 0;         // candidates the scratch holds
+    long long stat_delta_exact = 0;   // gradient-batch calls repeated without the expansion (guard tripped)
     bool stream_inline = true;     // P == 1: streaming launches evaluate lineshapes in registers even if columns exist
     bool want_matrix = false;      // set_params decided that the normalisation should go through the matrix
     std::vector<double> prev_mw;   // masses and widths of the previous single-point call (static-lineshape detection)
@@ -589,7 +590,7 @@ bool build_delta_plan(amp_model* m) {
                                 ++nt;
                             }
                         rec[0] = word(nt, -1);
-                        push(0, add_slot(rec), r, dre, dim, 0.0);
+                        push(0, add_slot(rec), r, dre, dim, dre * dre + dim * dim);   // third constant of a kind-0 contribution: |coef|^2
                     }
                 } else {
                     LineConst lc;
@@ -602,7 +603,7 @@ bool build_delta_plan(amp_model* m) {
                         const int s1 = weighted_slot(cp, false, -1);          // BW(p) sum_j c_j(p) g_j
                         if (s1 >= 0) push(2, s1, r, lc.kN, lc.kG, lc.M2);
                         const int s0 = weighted_slot(c0, true, -1);           // - sum_j c_j(0) BW(0) g_j
-                        if (s0 >= 0) push(0, s0, r, -1.0, 0.0, 0.0);
+                        if (s0 >= 0) push(0, s0, r, -1.0, 0.0, 1.0);
                     }
                 }
             }
@@ -1298,22 +1299,30 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         m->ring_calls++;
         CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
         CK(cudaMemcpyAsync(m->d_plan, m->h_plan, off, cudaMemcpyHostToDevice, s));
-        for (size_t c = 0; c < m->delta_chunks.size(); ++c) {
-            const auto& ch = m->delta_chunks[c];
-            const size_t bC = al(ch.contrib.size() * sizeof(DeltaContrib)), bS = al(ch.slots.size() * sizeof(double) + 8);
-            d.contrib = reinterpret_cast<const DeltaContrib*>(m->d_plan + offs[c]);
-            d.slots = reinterpret_cast<const double*>(m->d_plan + offs[c] + bC);
-            d.point_of_sorted = reinterpret_cast<const int*>(m->d_plan + offs[c] + bC + bS);
-            d.ncontrib = (int)ch.contrib.size();
-            d.nslotwords = (int)ch.slots.size();
-            d.nsorted = ch.nsorted;
-            d.first_chunk = c == 0 ? 1 : 0;
-            CK(launch_delta(d, delta_grid(d.a.n, d.a.n2), s));
-            m->stat_launches++;
+        // The kernel expands single-contribution points around point 0 (S(0) + Re(coef T2) + |coef|^2 n); if some point's density
+        // falls below 1e-3 S(0) at some event the guard trips (1024 in the flag word) and the call is repeated with the amplitudes
+        // summed term by term.  Gradient steps never trip it; a batch that switches a dominant amplitude off can.
+        for (int exact = 0; exact < 2; ++exact) {
+            for (size_t c = 0; c < m->delta_chunks.size(); ++c) {
+                const auto& ch = m->delta_chunks[c];
+                const size_t bC = al(ch.contrib.size() * sizeof(DeltaContrib)), bS = al(ch.slots.size() * sizeof(double) + 8);
+                d.contrib = reinterpret_cast<const DeltaContrib*>(m->d_plan + offs[c]);
+                d.slots = reinterpret_cast<const double*>(m->d_plan + offs[c] + bC);
+                d.point_of_sorted = reinterpret_cast<const int*>(m->d_plan + offs[c] + bC + bS);
+                d.ncontrib = (int)ch.contrib.size();
+                d.nslotwords = (int)ch.slots.size();
+                d.nsorted = ch.nsorted;
+                d.first_chunk = c == 0 ? 1 : 0;
+                CK(launch_delta(d, delta_grid(d.a.n, d.a.n2), s, exact != 0));
+                m->stat_launches++;
+            }
+            CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
+            CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (4 * P + 1), cudaMemcpyDeviceToHost, s));
+            CK(cudaStreamSynchronize(s));
+            if (m->h_pinned[2 * P] < 1024.0) break;
+            m->h_pinned[2 * P] = std::fmod(m->h_pinned[2 * P], 1024.0);   // (after the repeat: its own flag word)
+            m->stat_delta_exact++;
         }
-        CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
-        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (4 * P + 1), cudaMemcpyDeviceToHost, s));
-        CK(cudaStreamSynchronize(s));
         m->last_slog.assign(m->h_pinned + 2 * P + 1, m->h_pinned + 3 * P + 1);
         m->last_swS.assign(m->h_pinned + 3 * P + 1, m->h_pinned + 4 * P + 1);
         m->stat_norm_path = 5;

@@ -21,6 +21,7 @@ __device__ __forceinline__ void dJ(int J, double c, double s, double* d0, double
 
 struct EvK {   // what the point loop keeps of one event in registers
     double2 Ap, Am;                 // A_xi(0)
+    double S0, Sguard;              // |A_+(0)|^2 + |A_-(0)|^2 (delta.cu: expansion point of the single-contribution points) and its guard level
     double m2, mZ2;
     double cK, sK;
     double h0, a1, a2, a3, a4;      // d^1_{0,+}(theta_psi); hp cos phi, hp sin phi, hm cos phi, hm sin phi

@@ -505,6 +505,41 @@ def test_background_and_purity_match_oracle():
     assert abs(Mg.nll()[0] - base) < 1e-12 * abs(base) and Mg.last_call_stats()["norm_path"] in (2, 4)   # signal-only paths again
 
 
+def test_gradient_batch_guard_repeats_large_cancelling_changes():
+    """The gradient-batch kernel expands single-contribution points around point 0; a point that switches a dominant amplitude
+    off makes S(p) << S(0) at some events, where the expansion would lose digits: the guard trips and the library repeats the call
+    with the amplitudes summed term by term (twice the launches).  Results against the oracle either way; small steps do not trip it."""
+    from paper_2007_14931_b200 import binding as B
+    res = [(W.KSTAR, 1, 895.55, 47.3, W.RADIUS)]                # one resonance: at sin(theta_K*) -> 0 only lambda = 0 is left
+    c = np.array([0.7 * np.exp(0.5j), 1.0, 0.9 * np.exp(-1.1j)])
+    Mo, Mg = O.Model(W.DECAY, res), B.Model(W.DECAY, res)
+    xn, wn = W.norm_events(1, 12000)
+    x, eff = xn[:, :6000].copy(), wn[:6000].copy()
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn[:, 6000:]), dev(wn[6000:]))
+    xn, wn = xn[:, 6000:], wn[6000:]
+    small = np.tile(c, (5, 1))
+    for p in range(1, 5):
+        small[p, (p - 1) % 3] *= 1 + 1e-3 * p
+    Mg.set_params(small)
+    nb = Mg.nll()
+    st = Mg.last_call_stats()
+    assert st["norm_path"] == 5 and st["launches"] == 1
+    rb, rI = Mo.nll(small, x, eff, xn, wn)
+    assert np.max(np.abs(nb - rb) / np.abs(rb)) < RTOL_NLL and np.max(np.abs(Mg.norm_integral() - rI) / rI) < 1e-12
+    big = np.tile(c, (4, 1))
+    big[1, 1] = 1e-7 * c[1]                                      # lambda = 0 switched off: S(p)/S(0) ~ sin^2(theta_K*) at some events
+    big[2, 1] = -c[1]
+    big[3, 0] *= 1.001
+    Mg.set_params(big)
+    nb = Mg.nll()
+    st = Mg.last_call_stats()
+    assert st["norm_path"] == 5 and st["launches"] == 2           # the repeat
+    rb, rI = Mo.nll(big, x, eff, xn, wn)
+    assert np.max(np.abs(nb - rb) / np.abs(rb)) < RTOL_NLL, np.max(np.abs(nb - rb) / np.abs(rb))
+    assert np.max(np.abs(Mg.norm_integral() - rI) / rI) < 1e-12
+
+
 @pytest.mark.parametrize("with_z", [True, False])
 def test_lass_model_gradient_and_fit(with_z):
     """amp_nll_grad and amp_fit for the paper's LASS variant of the model (Eq. 9): the LASS term is one more slot whose lineshape
