@@ -298,9 +298,10 @@ long long stream_pad(long long n);   // events per column rounded up to whole pi
 //   mass/width change of resonance R:       coef = BW_R(p) - BW_R(0),    SLOT = sum_l c_{R,l}(0) g_{R,l}
 //   both at once:                           coef = BW_R(p), SLOT = sum_l c_{R,l}(p) g_{R,l}   and   coef = -1, SLOT = sum_l c_{R,l}(0) BW_R(0) g_{R,l}
 struct DeltaContrib {   // 32 bytes
-    int hdr;            // bits 0-1: coef kind (0 explicit (a, b); 1 BW(kN=a, kG=b, M2=c) - BW_ent(0) of the slot; 2 BW(a, b, c));
+    int hdr;            // bits 0-1: coef kind (0 explicit (a, b), c = a^2 + b^2; 1 BW(kN=a, kG=b, M2=c) - BW_ent(0) of the slot; 2 BW(a, b, c));
                         // bit 2: last contribution of its point; bit 3: slot differs from the previous contribution's;
-                        // bit 4: empty (point equal to point 0 / padding); bit 5: the BW runs on the Z chain; bits 8-11: barrier group
+                        // bit 4: empty (point equal to point 0 / padding); bit 5: the BW runs on the Z chain; bit 6: first of four
+                        // single-contribution points of one kind (0 or 1) on one slot (host-marked); bits 8-11: barrier group
     int slot;           // offset of the slot record in the slot area, in 8-byte words
     double a, b, c;
 };

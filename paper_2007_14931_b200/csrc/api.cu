@@ -538,8 +538,10 @@ bool build_delta_plan(amp_model* m) {
             prev_slot = slot;
             ch.contrib.push_back(dc);
         };
+        std::vector<size_t> first_of(ch.nsorted + 1, 0);
         for (int q = 0; q < ch.nsorted; ++q) {
             const size_t first = ch.contrib.size();
+            first_of[q] = first;
             const int p = p0 + q;
             for (int r = 0; q < ch.np && r < R; ++r) {
                 const amp_resonance& rs = m->res[r];
@@ -611,6 +613,18 @@ bool build_delta_plan(amp_model* m) {
             ch.contrib.back().hdr |= 4;
             if (q < ch.np) total += ch.contrib.size() - first;
             if (total > cap || ch.contrib.size() > DELTA_MAX_CONTRIB || ch.slots.size() > DELTA_MAX_SLOTWORDS) return false;
+        }
+        // Four consecutive points (aligned in the block) that are single contributions of one kind (coupling, or mass / width) on
+        // one slot — the gradient pattern — are marked once here (bit 64 of the first header) instead of being recognised by every thread
+        first_of[ch.nsorted] = ch.contrib.size();
+        for (int q = 0; q + 3 < ch.nsorted; q += 4) {
+            bool quad = true;
+            const int kind = ch.contrib[first_of[q]].hdr & 3;
+            for (int j = 0; j < 4 && quad; ++j) {
+                const int h = ch.contrib[first_of[q + j]].hdr;
+                quad = first_of[q + j + 1] - first_of[q + j] == 1 && (h & (j ? 28 : 20)) == 4 && (h & 3) == kind && kind < 2;
+            }
+            if (quad) ch.contrib[first_of[q]].hdr |= 64;
         }
         m->delta_chunks.push_back(std::move(ch));
     }

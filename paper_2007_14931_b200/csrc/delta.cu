@@ -58,31 +58,70 @@ __device__ __forceinline__ double2 bw_point0(const StreamArgs& a, int ent, int g
     return bw_from_consts(a.ent[ent].kN, a.ent[ent].kG, a.ent[ent].M2, isz ? k.mZ2 : k.m2, f.x, f.y);
 }
 
-// Evaluate the slot record at `rec` (shared memory) for the thread's E events.
+// Evaluate the slot record at `rec` (shared memory) for the thread's E events.  A slot belongs to ONE resonance (its terms are
+// helicities of that resonance): entry, barrier group, spin and chain are decoded once, the Breit-Wigner of point 0 and the
+// d functions are computed once, and only the helicity-dependent factors run per term (at most three).
 template <bool FAST>
 __device__ __forceinline__ void eval_slot(const StreamArgs& a, const double* rec, const EvK (&k)[E], const double2* fg, const double* zst,
                                           SlotVal (&sv)[E]) {
+    const double RSQRT2 = 0.70710678118654752440;
     const int2 h = *reinterpret_cast<const int2*>(rec);
+    const int th0 = *reinterpret_cast<const int*>(rec + 1);
+    const int ent = th0 & 255, grp = (th0 >> 8) & 15, J = (th0 >> 12) & 7;
+    const bool isz = (th0 >> 17) & 1, unit = (th0 >> 18) & 1;
 #pragma unroll
-    for (int e = 0; e < E; ++e) sv[e].Sp = sv[e].Sm = make_double2(0.0, 0.0);
-    for (int t = 0; t < h.x; ++t) {
-        const int th = *reinterpret_cast<const int*>(rec + 1 + 3 * t);
-        const int ent = th & 255, grp = (th >> 8) & 15, J = (th >> 12) & 7, lam = ((th >> 15) & 3) - 1;
-        const bool isz = (th >> 17) & 1, unit = (th >> 18) & 1;
-        const double2 wgt = make_double2(rec[2 + 3 * t], rec[3 + 3 * t]);
+    for (int e = 0; e < E; ++e) {
+        double2 Sp = make_double2(0.0, 0.0), Sm = Sp;
+        if (!isz) {
+            double d0, d1;
+            dJ(J, k[e].cK, k[e].sK, &d0, &d1);
+            const double t0 = d0 * k[e].h0;
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-            double2 gp, gm;
-            term_angular<true>(J, lam, isz, k[e], zst + e, &gp, &gm);
-            if (ent != 255) {
-                const double2 bw = bw_point0(a, ent, grp, isz, k[e], fg + e);
-                gp = cmul(bw, gp);
-                gm = cmul(bw, gm);
+            for (int t = 0; t < 3; ++t) {
+                if (t < h.x) {
+                    const int lam = ((*reinterpret_cast<const int*>(rec + 1 + 3 * t) >> 15) & 3) - 1;
+                    double2 gp, gm;
+                    if (lam == 0) { gp = make_double2(t0, 0.0); gm = make_double2(-t0, 0.0); }
+                    else if (lam > 0) { gp = make_double2(d1 * k[e].a1, d1 * k[e].a2); gm = make_double2(d1 * k[e].a3, d1 * k[e].a4); }
+                    else { gp = make_double2(-d1 * k[e].a3, d1 * k[e].a4); gm = make_double2(-d1 * k[e].a1, d1 * k[e].a2); }
+                    if (!unit) {
+                        const double2 wgt = make_double2(rec[2 + 3 * t], rec[3 + 3 * t]);
+                        gp = cmul(wgt, gp);
+                        gm = cmul(wgt, gm);
+                    }
+                    Sp = cadd(Sp, gp);
+                    Sm = cadd(Sm, gm);
+                }
             }
-            if (!unit) { gp = cmul(wgt, gp); gm = cmul(wgt, gm); }
-            sv[e].Sp = cadd(sv[e].Sp, gp);
-            sv[e].Sm = cadd(sv[e].Sm, gm);
+        } else {
+            // d^1_{0 l'}(theta_Z) e^{i l' phi~} d^1_{l' xi}(theta~) e^{i xi alpha} (the plans of this kernel hold 1+ Zs only)
+            const double* z = zst + e;
+            const double cZ = z[C_CZ * TILE], sZ = z[C_SZ * TILE], ct = z[C_CT * TILE], st = z[C_ST * TILE];
+            const double cpt = z[C_CPT * TILE], spt = z[C_SPT * TILE], ca = z[C_CA * TILE], sa = z[C_SA * TILE];
+            const double z1 = RSQRT2 * sZ, g0 = RSQRT2 * st, gpp = 0.5 * (1.0 + ct), gmm = 0.5 * (1.0 - ct);
+            // T = sum_l' w_l' d^1_{0 l'} e^{i l' phi~} (.)  accumulated per xi before the alpha phase
+            double2 Zp = make_double2(0.0, 0.0), Zm = Zp;
+#pragma unroll
+            for (int t = 0; t < 3; ++t) {
+                if (t < h.x) {
+                    const int lam = ((*reinterpret_cast<const int*>(rec + 1 + 3 * t) >> 15) & 3) - 1;
+                    double2 f = lam == 0 ? make_double2(cZ, 0.0) : (lam > 0 ? make_double2(z1 * cpt, z1 * spt) : make_double2(-z1 * cpt, z1 * spt));
+                    if (!unit) f = cmul(make_double2(rec[2 + 3 * t], rec[3 + 3 * t]), f);
+                    const double dp = lam == 0 ? g0 : (lam > 0 ? gpp : gmm), dm = lam == 0 ? -g0 : (lam > 0 ? gmm : gpp);
+                    Zp = make_double2(fma(dp, f.x, Zp.x), fma(dp, f.y, Zp.y));
+                    Zm = make_double2(fma(dm, f.x, Zm.x), fma(dm, f.y, Zm.y));
+                }
+            }
+            Sp = cmul(make_double2(ca, sa), Zp);
+            Sm = cmul(make_double2(ca, -sa), Zm);
         }
+        if (ent != 255) {
+            const double2 bw = bw_point0(a, ent, grp, isz, k[e], fg + e);
+            Sp = cmul(bw, Sp);
+            Sm = cmul(bw, Sm);
+        }
+        sv[e].Sp = Sp;
+        sv[e].Sm = Sm;
     }
     if (h.y >= 0) {
 #pragma unroll
@@ -194,6 +233,7 @@ __device__ __forceinline__ void leaf_multi(const int4 (&h4)[NP], const double2 (
                                            const SlotVal (&sv)[E], const double (&w)[E], const bool (&live)[E], int& bad, double (&v)[NP],
                                            int (&ex)[NP]) {
     double S[NP][E];
+    bool trip = false;   // (one predicate for the NP x E comparisons, folded into `bad` once)
 #pragma unroll
     for (int j = 0; j < NP; ++j) {
         const double ca = __hiloint2double(h4[j].w, h4[j].z);
@@ -211,7 +251,7 @@ __device__ __forceinline__ void leaf_multi(const int4 (&h4)[NP], const double2 (
                 // nearly cancels A(0) would lose digits here: it trips the guard and the host repeats the call with FAST = false
                 const double c2 = KIND ? fma(coef.x, coef.x, coef.y * coef.y) : bc[j].y;
                 Sv = fma(c2, sv[e].n, fma(coef.x, sv[e].T2.x, fma(-coef.y, sv[e].T2.y, k[e].S0)));
-                bad |= (Sv < k[e].Sguard) ? 2 : 0;
+                trip |= Sv < k[e].Sguard;
             } else {
                 const double2 Ap = cfma(coef, sv[e].Sp, k[e].Ap), Am = cfma(coef, sv[e].Sm, k[e].Am);
                 Sv = fma(Ap.x, Ap.x, Ap.y * Ap.y) + fma(Am.x, Am.x, Am.y * Am.y);
@@ -219,6 +259,7 @@ __device__ __forceinline__ void leaf_multi(const int4 (&h4)[NP], const double2 (
             S[j][e] = Sv;
         }
     }
+    if (FAST && trip) bad |= 2;
 #pragma unroll
     for (int j = 0; j < NP; ++j) leaf_value<NORM>(S[j], w, live, bad, &v[j], &ex[j]);
 }
@@ -265,11 +306,9 @@ __device__ __forceinline__ void eval_block(const StreamArgs& a, const DeltaContr
                 h4[j] = *reinterpret_cast<const int4*>(prog + it + j);
                 bc[j] = *reinterpret_cast<const double2*>(&prog[it + j].b);
             }
-            // four single-contribution points of kind 0 or 1 on one slot (the gradient pattern): one straight-line block
+            // four single-contribution points of kind 0 or 1 on one slot (the gradient pattern, marked by the host): one straight-line block
             const int kind = h4[0].x & 3;
-            bool quad = (h4[0].x & 20) == 4 && kind < 2;
-#pragma unroll
-            for (int j = 1; j < 4; ++j) quad = quad && (h4[j].x & 28) == 4 && ((h4[0].x ^ h4[j].x) & 3) == 0;
+            const bool quad = (h4[0].x & 64) != 0;
             if (quad) {
                 it += 4;
                 if (h4[0].x & 8) eval_slot<FAST>(a, slots + h4[0].y, k, fg, zst, sv);
