@@ -306,7 +306,11 @@ def run_own(args):
                    "l2": "inputs (2.1 GB kinematics cache) larger than L2; no flush needed", "parallelism": f"replicas x{world}"},
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "note": "host wall clock around amp_set_params (host parameter arrays in) + amp_nll (host NLL out) per step; the events are "
-                        "resident as in a fit (PAPER.md:45) - the one-off upload of the events from host buffers is setup.cold_start"},
+                        "resident as in a fit (PAPER.md:45) - the one-off upload of the events from host buffers is setup.cold_start",
+                # the other reading of "host buffers": EVERY evaluation uploads the events again (pinned host -> device -> kinematics
+                # cache -> parameters -> NLL): P evaluations per cold start
+                "value_if_events_uploaded_every_step": P * world / (info["cold_start"]["ms"] * 1e-3),
+                "h2d_bytes_per_step_if_events_uploaded": int(info["cold_start"]["h2d_bytes"] + h2d)},
         "gpu_launches": int(launches),
         "event_evals_per_s": value * (args.n_data + args.n_norm),
         "phase_ms": {"lineshape": float(np.mean(t_line)), "data": float(np.mean(t_data)), "norm": norm_ms},
