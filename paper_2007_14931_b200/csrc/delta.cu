@@ -38,6 +38,10 @@ namespace amp {
 namespace {
 
 constexpr int DBLK = DELTA_MAX_SORTED / 32;
+#ifndef AMP_DELTA_QUNROLL
+#define AMP_DELTA_QUNROLL 2
+#endif
+constexpr int DELTA_QUNROLL = AMP_DELTA_QUNROLL;   // unrolling of the four-point steps of a 32-point block
 
 struct SlotVal {   // the current slot of one event
     double2 Sp, Sm;                 // xi = +1, -1
@@ -295,7 +299,7 @@ __device__ __forceinline__ void eval_block(const StreamArgs& a, const DeltaContr
             leaf<NORM, FAST>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, &y[1], &ye[1]);
         }
     };
-#pragma unroll 1
+#pragma unroll DELTA_QUNROLL
     for (int q = 0; q < 32; q += 4) {
         double y[4]; int ye[4];
         {
