@@ -26,15 +26,12 @@ struct EvK {   // what the point loop keeps of one event in registers
     double cK, sK;
     double h0, a1, a2, a3, a4;      // d^1_{0,+}(theta_psi); hp cos phi, hp sin phi, hm cos phi, hm sin phi
 };
-// Angular factor g_{J,lambda,xi} of one term for one event (Eq. 4 for a K*, Eq. 10 for the Z).
+// Angular factor g_{J,lambda,xi} of one term for one event (Eq. 4 for a K*, Eq. 10 for the Z), given the d functions of the
+// term's spin: (d0, d1) = (d^J_{00}, d^J_{+1,0}) at theta_K* for a K*, at theta_Z for a Z (where d^J_{0,+1} = -d^J_{+1,0}).
 // zst: this event's element of the staged tile (the Z-chain angles stay there during the point loop).
-// Z1P: every Z of the model is a 1+ (the gradient-batch kernel's plans): d^1_{0 l'} without the spin switch.
-template <bool Z1P = false>
-__device__ __forceinline__ void term_angular(int J, int lam, bool isz, const EvK& k, const double* zst, double2* gp, double2* gm) {
+__device__ __forceinline__ void term_angular_d(double d0, double d1, int lam, bool isz, const EvK& k, const double* zst, double2* gp, double2* gm) {
     const double RSQRT2 = 0.70710678118654752440;
     if (!isz) {
-        double d0, d1;
-        dJ(J, k.cK, k.sK, &d0, &d1);
         if (lam == 0) {
             const double t = d0 * k.h0;
             *gp = make_double2(t, 0.0);
@@ -49,17 +46,23 @@ __device__ __forceinline__ void term_angular(int J, int lam, bool isz, const EvK
         return;
     }
     // d^J_{0 l'}(theta_Z) e^{i l' phi~} d^1_{l' xi}(theta~) e^{i xi alpha};  d^J_{0,+1} = -d^J_{+1,0}, d^J_{0,-1} = d^J_{+1,0}
-    const double cZ = zst[C_CZ * TILE], sZ = zst[C_SZ * TILE], ct = zst[C_CT * TILE], st = zst[C_ST * TILE];
+    const double ct = zst[C_CT * TILE], st = zst[C_ST * TILE];
     const double cpt = zst[C_CPT * TILE], spt = zst[C_SPT * TILE], ca = zst[C_CA * TILE], sa = zst[C_SA * TILE];
-    double z0, z1;
-    if (Z1P) { z0 = cZ; z1 = -RSQRT2 * sZ; }
-    else dJ(J, cZ, sZ, &z0, &z1);
-    const double zf = lam == 0 ? z0 : (lam > 0 ? -z1 : z1);
+    const double zf = lam == 0 ? d0 : (lam > 0 ? -d1 : d1);
     const double dp = lam == 0 ? RSQRT2 * st : (lam > 0 ? 0.5 * (1.0 + ct) : 0.5 * (1.0 - ct));
     const double dm = lam == 0 ? -RSQRT2 * st : (lam > 0 ? 0.5 * (1.0 - ct) : 0.5 * (1.0 + ct));
     const double2 eph = lam == 0 ? make_double2(1.0, 0.0) : make_double2(cpt, lam > 0 ? spt : -spt);
     *gp = cscale(zf * dp, cmul(eph, make_double2(ca, sa)));
     *gm = cscale(zf * dm, cmul(eph, make_double2(ca, -sa)));
+}
+// the same with the d functions evaluated here.  Z1P: every Z of the model is a 1+ (the gradient-batch kernel's plans)
+template <bool Z1P = false>
+__device__ __forceinline__ void term_angular(int J, int lam, bool isz, const EvK& k, const double* zst, double2* gp, double2* gm) {
+    double d0, d1;
+    if (!isz) dJ(J, k.cK, k.sK, &d0, &d1);
+    else if (Z1P) { d0 = zst[C_CZ * TILE]; d1 = -0.70710678118654752440 * zst[C_SZ * TILE]; }
+    else dJ(J, zst[C_CZ * TILE], zst[C_SZ * TILE], &d0, &d1);
+    term_angular_d(d0, d1, lam, isz, k, zst, gp, gm);
 }
 
 // Recursive halving over the 32 lanes: `a` belongs to the earlier half of the points, `b` to the later half; lanes with

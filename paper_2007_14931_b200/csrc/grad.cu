@@ -218,12 +218,19 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
             u = (live && ok) ? fast_rcp(S) : 0.0;
         }
         // ---- gradient leaves: slot pair p -> (Re, Im) of u conj(BW) sum_xi conj(g_xi) A_xi
+        int Jc = -1;             // spin code of the d functions held in (d0c, d1c): the slots of one resonance follow each other
+        double d0c = 0.0, d1c = 0.0;
         auto pair_value = [&](int p, double* re, double* im) {
             const int ent = g.pair_ent[p];
             if (ent == -2) { *re = 0.0; *im = 0.0; return; }
-            const int J = g.pair_J[p];
+            const int J = g.pair_J[p];   // 8 + J: a Z slot of spin J
+            if (J != Jc) {
+                if (J >= 8) dJ(J - 8, st[C_CZ * TILE], st[C_SZ * TILE], &d0c, &d1c);
+                else dJ(J, k.cK, k.sK, &d0c, &d1c);
+                Jc = J;
+            }
             double2 gp, gm;
-            term_angular(J >= 8 ? J - 8 : J, g.pair_lam[p], J >= 8, k, st, &gp, &gm);   // 8 + J: a Z slot of spin J
+            term_angular_d(d0c, d1c, g.pair_lam[p], J >= 8, k, st, &gp, &gm);
             // T = conj(g+) A+ + conj(g-) A-
             double2 T = make_double2(fma(gp.x, k.Ap.x, gp.y * k.Ap.y), fma(gp.x, k.Ap.y, -gp.y * k.Ap.x));
             T.x = fma(gm.x, k.Am.x, fma(gm.y, k.Am.y, T.x));
