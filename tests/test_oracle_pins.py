@@ -793,3 +793,73 @@ def test_P21_background_gradient():
     n1, g1 = M.nll_gradient_background(c, x, eff, b, 1.0, xn, wn)
     n0, g0 = M.nll_gradient(c, x, eff, xn, wn)
     assert abs(n1 - n0) < 1e-12 * abs(n0) and np.max(np.abs(g1 - g0)) < 1e-11 * np.max(np.abs(g0))
+
+
+# ------------------------------------------------------------------ P22: orientation of theta_Z (reading A10)
+def _boost(p, v):
+    """4-vector p = (E, px, py, pz) seen from a frame that moves with velocity v (c = 1)"""
+    v = np.asarray(v, float)
+    v2 = v @ v
+    g = 1.0 / math.sqrt(1.0 - v2)
+    vp = v @ p[1:]
+    return np.concatenate([[g * (p[0] - vp)], p[1:] + ((g - 1.0) * vp / v2 - g * p[0]) * v])
+
+
+def test_P22_theta_Z_is_the_helicity_angle_of_the_psi_from_the_Z_line_of_flight():
+    """Eq. 10's d^{J(Z)}_{0 lambda'}(theta_Z) is the Jacob-Wick two-body amplitude of a Z of helicity 0 (B and K are spinless)
+    into a psi of helicity lambda': its angle is the polar angle of the psi, in the Z rest frame, from the Z's line of flight
+    in the B frame.  There p_psi = -p_pi and the Z's line of flight is opposite to p_K, so that angle IS the literal
+    'angle between K and pi momenta in the Z rest frame' and not its supplement."""
+    M = model(2)
+    x = W.phase_space_events(np.random.default_rng(22), 300)
+    for i in range(x.shape[1]):
+        k = M.z_kinematics(x[:, i])
+        Z = k["psi_B"] + k["pi_B"]
+        nZ = Z[1:] / np.linalg.norm(Z[1:])                       # the Z's line of flight in the B rest frame
+        vZ = Z[1:] / Z[0]
+        psi_Z, pi_Z, K_Z = _boost(k["psi_B"], vZ), _boost(k["pi_B"], vZ), _boost(k["K_B"], vZ)
+        assert np.abs(psi_Z[1:] + pi_Z[1:]).max() < 1e-8         # Z rest frame: back to back
+        assert np.linalg.norm(np.cross(K_Z[1:], nZ)) < 1e-9 * np.linalg.norm(K_Z[1:]) and K_Z[1:] @ nZ < 0
+        c_hel = psi_Z[1:] @ nZ / np.linalg.norm(psi_Z[1:])
+        assert abs(c_hel - k["cosZ"]) < 1e-11
+        c_sup = pi_Z[1:] @ nZ / np.linalg.norm(pi_Z[1:])         # the supplement: the pion's polar angle
+        assert abs(c_sup + k["cosZ"]) < 1e-11
+
+
+@pytest.mark.parametrize("kind,J", [(O.ZRES, 1), (O.ZRES, 2), (O.ZNEG, 1), (O.ZNEG, 2)])
+def test_P22_supplement_of_theta_Z_is_a_relabelling_of_the_couplings(kind, J):
+    """Had the paper meant the supplement, d^J_{0 l'}(pi - theta) = (-1)^{J + l'} d^J_{0 l'}(theta): the density with couplings
+    H_l' under one reading is the density with (-1)^{J + l'} H_l' under the other, K* interference included — the two readings
+    span the same family of PDFs, with the same likelihood minimum, fit fractions and significances.  The Z basis terms are
+    rebuilt here from the oracle's separately pinned pieces (lineshape P3/P20, d functions P1, angles P5-P7)."""
+    res = W.resonances(1)[:4] + [(kind, J, 4196.0, 370.0, R16)]
+    M = O.Model(DEC, res)
+    K = M.K
+    rng = np.random.default_rng(220 + J)
+    c = rng.normal(size=K) + 1j * rng.normal(size=K)
+    sign = np.array([(-1.0) ** (J + lp) for lp in (-1, 0, 1)])
+    c_flip = c.copy()
+    c_flip[K - 3:] *= sign
+    x = W.phase_space_events(rng, 60)
+    S, S_flip = M.eval_events(c, x), M.eval_events(c_flip, x)
+    d = O.wigner_d
+    for i in range(x.shape[1]):
+        zk = M.z_kinematics(x[:, i])
+        A = M.lineshape(len(res) - 1, zk["mZ"])[0]
+        thZ, thT = math.atan2(zk["sinZ"], zk["cosZ"]), math.atan2(zk["sinT"], zk["cosT"])
+        B = M.basis_terms(x[:, i])
+
+        def z_terms(theta):
+            return np.array([[A * d(J, 0, lp, theta) * np.exp(1j * lp * zk["phiT"]) * d(1, lp, xi, thT) * np.exp(1j * xi * zk["alpha"])
+                              if abs(lp) <= J else 0.0 for xi in (1, -1)] for lp in (-1, 0, 1)])
+
+        lit, sup = z_terms(thZ), z_terms(math.pi - thZ)
+        scale = np.abs(lit).max()
+        assert np.abs(B[K - 3:] - lit).max() < 1e-12 * scale      # the oracle's terms are Eq. 10 with the literal angle
+        assert np.abs(sup - sign[:, None] * lit).max() < 1e-12 * scale
+        Bs = B.copy()
+        Bs[K - 3:] = sup
+        S_sup = sum(abs(c @ Bs[:, j]) ** 2 for j in range(2))     # supplement reading, couplings c
+        S_sup_flip = sum(abs(c_flip @ Bs[:, j]) ** 2 for j in range(2))
+        assert abs(S_sup - S_flip[i]) < 1e-11 * S[i] and abs(S_sup_flip - S[i]) < 1e-11 * S[i]
+    assert (np.abs(S - S_flip) / S).max() > 1e-3                   # the relabelling is not trivial: the sign matters at fixed H
