@@ -47,6 +47,9 @@ TRAFFIC_NCU_BYTES_CFG4 = 2.194401e9 + 7.89e6  # profiles/r01d_ncu_full_delta_cfg
 DELTA_FLOP_PER_EVENT = 730.0 + 31 * 65.0 + 100 * 8.0 + 20 * 33.0
 # analytic gradient: the point (730) + per coupling slot: angular factor ~8, T = sum_xi conj(g) A 16, conj(BW) T 8, weight 2
 GRAD_FLOP_PER_EVENT = 730.0 + 27 * 34.0
+# its shape-specialised form (gradf.cu): the point (730) + the three W_lambda and three Y_lambda' (u A, conj(g) A:
+# ~110) + one real scaling of them per spin (~30) + per coupling slot conj(BW) X into its register pair (4 FMA = 8)
+GRADF_FLOP_PER_EVENT = 730.0 + 140.0 + 27 * 8.0
 
 
 LASS = False   # --lass: the paper's LASS variant of the model (Eq. 9) instead of kappa(800) + K0*(1430)
@@ -229,7 +232,7 @@ def run_own(args):
     # the kernel times come from the library's ring of CUDA event pairs recorded around each launch on its stream
     st = model.last_call_stats()
     launches, paths = st["launches"] * args.steps, {st["norm_path"]}
-    if st["norm_path"] in (4, 5, 7):
+    if st["norm_path"] in (4, 5, 7, 8):
         ring = model.recent_launch_ms(min(args.steps, 256))
         t_data, t_norm, t_line = [float(v) for v in ring], [0.0], [0.0]
     else:
@@ -259,14 +262,16 @@ def run_own(args):
                 "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": TRAFFIC_NCU_BYTES_CFG4 if (args.n_data, args.n_norm) == (2_000_000, 10_000_000) else None, "kernel_ms": k_ms,
                 "flop_per_event": DELTA_FLOP_PER_EVENT, "flop_per_launch": flop,
                 "hbm_frac": (BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}
-    elif paths == {7}:
-        # --grad: NLL and analytic gradient in one k_grad launch per step; plain FP64 ALUs
+    elif paths == {7} or paths == {8}:
+        # --grad: NLL and analytic gradient in one k_gradf (the paper's resonance lists) or k_grad launch per step; plain FP64 ALUs
         k_ms = float(np.mean(t_data))
-        flop = GRAD_FLOP_PER_EVENT * (args.n_data + args.n_norm)
+        fpe = GRADF_FLOP_PER_EVENT if paths == {8} else GRAD_FLOP_PER_EVENT
+        flop = fpe * (args.n_data + args.n_norm)
         ach = flop / (k_ms * 1e-3) / 1e12
-        roof = {"bound": "alu", "kernel": "k_grad (NLL + dNLL/dH_k for all K = 27 couplings, data then norm tiles, one launch)",
+        roof = {"bound": "alu", "kernel": ("k_gradf (shape-specialised, gradient components in registers" if paths == {8} else "k_grad (generic") +
+                ": NLL + dNLL/dH_k for all K = 27 couplings, data then norm tiles, one launch)",
                 "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12, "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz", "unit": "TFLOP/s",
-                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": None, "kernel_ms": k_ms, "flop_per_event": GRAD_FLOP_PER_EVENT,
+                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": None, "kernel_ms": k_ms, "flop_per_event": fpe,
                 "hbm_frac": (BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}
     elif args.cfg == 4:
         # dense form (--dense): k_batch (data, DMMA contraction) + k_herk (normalisation matrix, DMMA) + k_lineshape

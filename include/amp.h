@@ -240,9 +240,15 @@ amp_status amp_set_batch_mode(amp_model* m, int mode);
  * launch: data tiles, then normalisation tiles, the last thread block forms the NLL), 1 = separate data / normalisation /
  * reduction launches (per-phase timing, parity tests of the two forms against each other).                       */
 amp_status amp_set_fused_mode(amp_model* m, int mode);
+/* Which kernel amp_nll_grad / amp_fit run: 0 = automatic (the paper's resonance lists — ten K* with zero to two 1+ Z's,
+ * one radius per spin, no LASS / constant term, no background — run the shape-specialised kernel that keeps every
+ * gradient component in registers; any other model the generic one), 1 = always the generic kernel (parity tests of the
+ * two against each other).                                                                                        */
+amp_status amp_set_grad_mode(amp_model* m, int mode);
 /* Counters of the last amp_nll / amp_norm_integral call: kernels launched, lineshape columns
  * recomputed (data + norm), which normalisation path ran (1 direct streaming sum, 2 matrix, 3 batched DMMA sum,
- * 4 fused single launch, 5 gradient-batch delta kernel, 6 background + purity, 7 analytic gradient).                         */
+ * 4 fused single launch, 5 gradient-batch delta kernel, 6 background + purity, 7 analytic gradient, generic kernel,
+ * 8 analytic gradient, shape-specialised kernel).                         */
 amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_recomputed, int* norm_path);
 
 /* Device time [ms] of the phases of the last amp_nll / amp_norm_integral call, from CUDA events recorded on

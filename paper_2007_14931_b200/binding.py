@@ -19,7 +19,7 @@ AMP_MAX_RESONANCES, AMP_MAX_COUPLINGS, AMP_MAX_POINTS = 16, 48, 256
 SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
     "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_grad", "amp_fit", "amp_generate", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
-    "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_fit_fractions", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode",
+    "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_fit_fractions", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode", "amp_set_grad_mode",
     "amp_last_call_stats", "amp_last_call_timing", "amp_recent_launch_ms", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
 ]
 
@@ -78,6 +78,7 @@ def lib():
         "amp_set_lineshape_mode": (i, [vp, i]),
         "amp_set_batch_mode": (i, [vp, i]),
         "amp_set_fused_mode": (i, [vp, i]),
+        "amp_set_grad_mode": (i, [vp, i]),
         "amp_last_call_stats": (i, [vp, pi, pi, pi]),
         "amp_last_call_timing": (i, [vp, pd]),
         "amp_recent_launch_ms": (i, [vp, i, pd, pi]),
@@ -326,6 +327,9 @@ class Model:
 
     def set_fused_mode(self, mode):
         self._check(lib().amp_set_fused_mode(self._h, int(mode)), "amp_set_fused_mode")
+
+    def set_grad_mode(self, mode):
+        self._check(lib().amp_set_grad_mode(self._h, int(mode)), "amp_set_grad_mode")
 
     def last_call_stats(self):
         a, b, c = C.c_int(), C.c_int(), C.c_int()

@@ -337,12 +337,17 @@ struct GradArgs {
     signed char pair_J[GRAD_MAX_PAIRS];     // spin of a K* (0 for a constant term); 8: Z
     signed char pair_grp[GRAD_MAX_PAIRS];   // barrier group of the entry
     short pair_slot[GRAD_MAX_PAIRS];        // coupling slot k the pair belongs to, -1: padding
+    signed char acc_pair[GRAD_MAX_PAIRS];   // gradf.cu: pair of accumulator q (entry order; lambda = -1, 0, +1 within an entry of spin >= 1)
     int K;
     double* partial;                    // [2][2 + 2 npairs][stride]: per-CTA partials; rows 0, 1 = sum log S / sum w S
     int stride;
     double* result;                     // [3 + 2 K]: NLL, I, domain flag, then (dNLL/dRe c_k, dNLL/dIm c_k); may be mapped host memory
 };
 cudaError_t launch_grad(const GradArgs& g, int grid, cudaStream_t s);
+// gradf.cu: the shape-specialised form (gradient components in registers)
+bool gradf_supports(const GradArgs& g);
+int gradf_grid(long long n_data, long long n_norm);
+cudaError_t launch_gradf(const GradArgs& g, int grid, cudaStream_t s);
 
 // toy.cu — accept-reject toy generator: one block of candidates
 struct ToyArgs {

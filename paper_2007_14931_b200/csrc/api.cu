@@ -107,6 +107,7 @@ struct amp_model {
     double* d_bkg = nullptr;       // [data.npad] background density b_i at the data events (Eq. 14), 1 on padding
     double purity = 1.0;
     bool has_bkg = false;
+    int grad_mode = 0;             // 0: amp_nll_grad picks the shape-specialised kernel where the model allows; 1: always the generic one
     int fused_mode = 0;            // 0: P == 1 steps with floating lineshapes run as one fused launch; 1: separate launches
     std::string err;
 };
@@ -414,6 +415,12 @@ amp_status amp_set_batch_mode(amp_model* m, int mode) {
 amp_status amp_set_fused_mode(amp_model* m, int mode) {
     if (!m || mode < 0 || mode > 1) return AMP_ERR_INVALID;
     m->fused_mode = mode;
+    return AMP_OK;
+}
+
+amp_status amp_set_grad_mode(amp_model* m, int mode) {
+    if (!m || mode < 0 || mode > 1) return AMP_ERR_INVALID;
+    m->grad_mode = mode;
     return AMP_OK;
 }
 
@@ -1664,13 +1671,24 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
     m->ring_last = (m->ring_last + 1) % amp_model::RING;
     m->ring_calls++;
     CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
-    CK(launch_grad(g, grad_grid(m->data.n, g.a.n2), s));
+    // the paper's resonance lists: every gradient component in a register of the thread that owns the event (gradf.cu)
+    const bool fast = m->grad_mode == 0 && gradf_supports(g);
+    if (fast) {
+        const int n0 = g.a.shape[0];   // accumulators in entry order: one per J = 0 entry, then three (lambda = -1, 0, +1) per entry
+        for (int k = 0; k < K; ++k) {
+            const int t = g.pair_ent[k];
+            g.acc_pair[(t < n0 ? t : n0 + 3 * (t - n0)) + (g.pair_J[k] == 0 ? 0 : g.pair_lam[k] + 1)] = (signed char)k;
+        }
+        CK(launch_gradf(g, gradf_grid(m->data.n, g.a.n2), s));
+    } else {
+        CK(launch_grad(g, grad_grid(m->data.n, g.a.n2), s));
+    }
     CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
     CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (3 + 2 * K), cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
     m->stat_launches = 1 + extra_launches;
     m->stat_columns = 0;
-    m->stat_norm_path = 7;
+    m->stat_norm_path = fast ? 8 : 7;
     m->fused_valid = true;
     h_nll[0] = m->h_pinned[0];
     bool bad = m->h_pinned[2] != 0.0 || !std::isfinite(h_nll[0]);

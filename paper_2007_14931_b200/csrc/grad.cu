@@ -14,6 +14,7 @@
 #define AMP_STREAM_THREADS 512
 #include "stream_core.cuh"
 #include "delta_core.cuh"
+#include "grad_tail.cuh"
 
 namespace amp {
 
@@ -298,64 +299,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_grad(const __grid_constant__ Gra
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    double* tot = accD;   // [3 + 2 nleaf] (<= 195 doubles; the accumulators are dead)
-    const int rows = 3 + 2 * nleaf;
-    for (int r = tid; r < rows; r += THREADS) {
-        const double* p = g.partial + (size_t)r * g.stride;
-        double s = 0.0;
-        for (unsigned c = 0; c < gridDim.x; ++c) s += __ldcg(p + c);
-        tot[r] = s;
-    }
-    __syncthreads();
-    const double nd = (double)a.n;
-    if (a.qf_G) {
-        // static lineshapes: no normalisation tile was walked; the held matrix gives N_k = (M c)_k and sum w S = c^H M c
-        // (Re M_kf = G'[2k][2f] + G'[2k+1][2f+1], Im M_kf = G'[2k][2f+1] - G'[2k+1][2f]); one thread per slot, fixed order
-        for (int p = tid; p < g.npairs; p += THREADS) {
-            const int kslot = g.pair_slot[p];
-            double2 acc = make_double2(0.0, 0.0);
-            if (kslot >= 0) {
-                for (int f = 0; f < a.qf_nent; ++f) {
-                    const double2 cf = a.qf_c[f];
-                    const double* gm = a.qf_G + (size_t)(2 * kslot) * a.qf_KP + 2 * f;
-                    const double mre = gm[0] + gm[a.qf_KP + 1], mim = gm[1] - gm[a.qf_KP];
-                    acc.x += mre * cf.x - mim * cf.y;
-                    acc.y += mre * cf.y + mim * cf.x;
-                }
-            }
-            tot[2 + nleaf + 2 * p] = acc.x;
-            tot[2 + nleaf + 2 * p + 1] = acc.y;
-        }
-        __syncthreads();
-        if (tid == 0) {   // c^H M c = sum_k Re(conj(c_k) (M c)_k), slot order
-            double q = 0.0;
-            for (int p = 0; p < g.npairs; ++p) {
-                const int kslot = g.pair_slot[p];
-                if (kslot >= 0) q += a.qf_c[kslot].x * tot[2 + nleaf + 2 * p] + a.qf_c[kslot].y * tot[2 + nleaf + 2 * p + 1];
-            }
-            tot[1] = q;
-        }
-        __syncthreads();
-    }
-    const double swS = tot[1];
-    // with a background (Eq. 14) the data-side weights are u_i = ps eps_i / f_i and N is replaced by T = sum_i u_i S_i
-    const double Tn = a.bkg ? tot[2 + 2 * nleaf] : nd;
-    for (int p = tid; p < g.npairs; p += THREADS) {
-        const int kslot = g.pair_slot[p];
-        if (kslot < 0) continue;
-        // dNLL/dconj(c_k) = -D_k + N N_k / sum_j w_j S_j ; (d/dRe, d/dIm) = 2 (Re, Im)
-        g.result[3 + 2 * kslot] = 2.0 * (-tot[2 + 2 * p] + Tn * tot[2 + nleaf + 2 * p] / swS);
-        g.result[3 + 2 * kslot + 1] = 2.0 * (-tot[2 + 2 * p + 1] + Tn * tot[2 + nleaf + 2 * p + 1] / swS);
-    }
-    if (tid == 0) {
-        const double I = swS / a.wsum;
-        double v = a.bkg ? -tot[0] : -(tot[0] + a.sum_log_eff) + nd * log(I);
-        if (!isfinite(v) || !(I > 0.0)) v = INFINITY;
-        g.result[0] = v;
-        g.result[1] = I;
-        g.result[2] = (double)atomicExch(a.flag, 0);
-        *a.ticket = 0u;
-    }
+    grad_finish(g, accD, nleaf, tid, THREADS, gridDim.x);   // accD: the accumulators are dead (3 + 2 nleaf <= 195 doubles)
 }
 
 namespace {
