@@ -13,10 +13,10 @@
 // model shape is a template argument and every loop unrolls.  grad.cu reduces every leaf across the warp for every event
 // instead (it cannot index registers at run time); this kernel reduces once per CTA.
 //
-// Thread = one event of a 256-event unit (half a cache block); three units in flight per CTA (cp.async.bulk + mbarrier ring,
-// one 2 KB copy per cache column issued by the lanes of warp 0); the lineshapes of the event are kept in a thread-private
-// shared-memory record between the forward pass and the gradient pass.  One CTA of 256 threads per SM (the accumulators take
-// 108 registers), data units first, then the normalisation units; fixed order everywhere: bit-reproducible.
+// Thread = one event of a 256-event unit (half a cache block); four units in flight per CTA (cp.async.bulk + full / empty
+// mbarrier ring, one 2 KB copy per cache column issued by the lanes of warp 0, no CTA-wide barrier in the loop); the lineshapes
+// of the event stay in registers between the forward pass and the gradient pass.  One CTA of 256 threads per SM (the
+// accumulators take 108 registers), data units first, then the normalisation units; fixed order everywhere: bit-reproducible.
 #define AMP_STREAM_E 2
 #define AMP_STREAM_THREADS 256
 #define AMP_STREAM_MINB 1
@@ -28,8 +28,12 @@ namespace amp {
 namespace {
 
 constexpr int UNIT = THREADS;   // events per pipeline unit (half a cache block)
-constexpr int NSTAGE = 3;
+constexpr int NSTAGE = 4;
 static_assert(2 * UNIT == CACHE_TILE, "two units per cache block");
+
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 
 template <class SH>
 struct Lay {
@@ -38,9 +42,9 @@ struct Lay {
     __host__ __device__ static constexpr int base(int t) { return t < SH::n0 ? t : SH::n0 + 3 * (t - SH::n0); }
 };
 
-// lineshapes of one spin class: U_l += c BW (couplings carry kN), BW / kN into the thread's record
+// lineshapes of one spin class: U_l += c BW (couplings carry kN), BW / kN kept (bwr: registers, every index a constant after unrolling)
 template <int J, int LRv, int LBv, int CNT, int OFF, int SPIN>
-__device__ __forceinline__ void class_forward(const StreamArgs& a, double m2, double invm, double pR, double pB, double2* rec, double2& Um,
+__device__ __forceinline__ void class_forward(const StreamArgs& a, double m2, double invm, double pR, double pB, double2* bwr, double2& Um,
                                               double2& U0, double2& Up) {
     double F, G;
     group_factors<LRv, LBv>(a.r2_spin[SPIN], invm, pR, pB, &F, &G);
@@ -48,7 +52,7 @@ __device__ __forceinline__ void class_forward(const StreamArgs& a, double m2, do
     for (int t = 0; t < CNT; ++t) {
         const ResEntry& en = a.ent[OFF + t];
         const double2 bw = bw_unscaled(en, m2, F, G);
-        rec[(OFF + t) * THREADS] = bw;
+        bwr[OFF + t] = bw;
         U0 = cfma(en.c0, bw, U0);
         if (J) { Um = cfma(en.cm, bw, Um); Up = cfma(en.cp, bw, Up); }
     }
@@ -62,10 +66,10 @@ __device__ __forceinline__ void conj_fma(double2 bw, double2 x, double2& acc) {
 
 // gradient leaves of one spin class: slots (lambda = -1, 0, +1) of entry OFF + t are accumulators base(OFF + t) + 0, 1, 2
 template <class SH, int J, int CNT, int OFF, int NACC>
-__device__ __forceinline__ void class_leaves(const double2* rec, double2 Xm, double2 X0, double2 Xp, double2 (&acc)[NACC]) {
+__device__ __forceinline__ void class_leaves(const double2* bwr, double2 Xm, double2 X0, double2 Xp, double2 (&acc)[NACC]) {
 #pragma unroll
     for (int t = 0; t < CNT; ++t) {
-        const double2 bw = rec[(OFF + t) * THREADS];
+        const double2 bw = bwr[OFF + t];
         const int b = Lay<SH>::base(OFF + t);
         if (J == 0) {
             conj_fma(bw, X0, acc[b]);
@@ -92,13 +96,13 @@ __global__ void __launch_bounds__(THREADS, 1) k_gradf(const __grid_constant__ Gr
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* stage0 = reinterpret_cast<double*>(smem_raw);                                        // [NSTAGE][ncolw][UNIT]
-    double2* rec = reinterpret_cast<double2*>(stage0 + (size_t)NSTAGE * ncolw * UNIT) + tid;     // [NENT][THREADS], this thread's column
-    double* red = reinterpret_cast<double*>(rec - tid);                                          // reused by the flushes: [NWARPS][2 NACC]
-    uint64_t* full = reinterpret_cast<uint64_t*>(reinterpret_cast<double2*>(stage0 + (size_t)NSTAGE * ncolw * UNIT) + (size_t)NENT * THREADS);
+    double* red = stage0 + (size_t)NSTAGE * ncolw * UNIT;                                        // the flushes: [NWARPS][2 NACC]; the finish: 3 + 2 nleaf
+    uint64_t* full = reinterpret_cast<uint64_t*>(red + NWARPS * 2 * NACC);
     __shared__ double sm[NWARPS];
     __shared__ bool s_last;
+    uint64_t* empty = full + NSTAGE;   // a stage is free again once every warp has read its event's columns
     if (tid == 0) {
-        for (int s = 0; s < NSTAGE; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < NSTAGE; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NWARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -126,7 +130,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_gradf(const __grid_constant__ Gr
     // per-CTA partial rows of the leaves held in acc: scaled by kN (the records hold BW / kN), summed over the warp by a fixed
     // xor tree, then over the warps in warp order
     auto flush = [&](int row0) {
-        __syncthreads();   // the lineshape records are dead: their space takes the warp totals
+        __syncthreads();
 #pragma unroll
         for (int t = 0; t < NENT; ++t) {
             const double kN = a.ent[t].kN;
@@ -177,6 +181,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_gradf(const __grid_constant__ Gr
         const double d30 = cK * fma(2.5, cK2, -1.5), d31 = -0.43301270189221932338 * sK * fma(5.0, cK2, -1.0);
         const double d40 = fma(fma(4.375, cK2, -3.75), cK2, 0.375), d41 = -0.55901699437494742410 * sK * cK * fma(7.0, cK2, -3.0);
         double2 V0 = make_double2(0, 0), Vp = V0, Vm = V0;
+        double2 rec[NENT];   // BW_R / kN of this event
 #define AMP_FSPIN(J, LB, CNT, OFF, D0, D1)                                                  \
         if (CNT > 0) {                                                                       \
             double2 Um = make_double2(0, 0), U0 = Um, Up = Um;                               \
@@ -220,10 +225,20 @@ __global__ void __launch_bounds__(THREADS, 1) k_gradf(const __grid_constant__ Gr
             Ap = cfma(make_double2(ca, sa), Zp, Ap);      // e^{+i alpha}
             Am = cfma(make_double2(ca, -sa), Zm, Am);     // e^{-i alpha}
         }
+        const double wgt = st[(ncolw - 1) * UNIT];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[s]);   // this warp has read everything it needs from the stage
+        // Refill the stage of the PREVIOUS unit (every warp released it before its gradient pass, so this rarely waits) with the
+        // unit NSTAGE steps after it.  The warps take turns: a fixed producer warp would fall behind the others by its extra work
+        // until they run into the end of the ring and wait for a whole memory latency every unit.  No CTA-wide barrier in the loop.
+        if (k > 0 && warp == (int)(k & (NWARPS - 1)) && unit + (long long)(NSTAGE - 1) * gridDim.x < nunits) {
+            const int ps = (int)((k - 1) % NSTAGE);
+            mbar_wait(&empty[ps], (uint32_t)(((k - 1) / NSTAGE) & 1));
+            issue(unit + (long long)(NSTAGE - 1) * gridDim.x, ps);
+        }
         const double S = fma(Ap.x, Ap.x, fma(Ap.y, Ap.y, fma(Am.x, Am.x, Am.y * Am.y)));
         double u;   // weight of this event in the gradient sums
         if (is_norm) {
-            const double wgt = st[(ncolw - 1) * UNIT];
             bad |= live && !isfinite(S);
             accW = fma(wgt, S, accW);        // padding events carry w = 0
             u = wgt;
@@ -264,8 +279,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_gradf(const __grid_constant__ Gr
                 class_leaves<SH, 1, SH::nz, SH::oz, NACC>(rec, Ym, Y0, Yp, acc);
             }
         }
-        __syncthreads();   // the unit's stage is consumed: refill it with the unit three steps ahead
-        if (warp == 0 && unit + (long long)NSTAGE * gridDim.x < nunits) issue(unit + (long long)NSTAGE * gridDim.x, s);
     }
     if (bad) atomicOr(a.flag, 2);
 
@@ -295,8 +308,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_gradf(const __grid_constant__ Gr
 
 namespace {
 
-size_t gradf_smem(int ncolw, int nent) {
-    return (size_t)NSTAGE * ncolw * UNIT * sizeof(double) + (size_t)nent * THREADS * sizeof(double2) + NSTAGE * sizeof(uint64_t);
+size_t gradf_smem(int ncolw, int nacc) {
+    return (size_t)NSTAGE * ncolw * UNIT * sizeof(double) + (size_t)NWARPS * 2 * nacc * sizeof(double) + 2 * NSTAGE * sizeof(uint64_t);
 }
 
 template <class SH>
@@ -305,7 +318,7 @@ cudaError_t launch_gradf_shape(const GradArgs& g, int grid, cudaStream_t s) {
     cudaError_t e = cudaSuccess;
     if (!attr_done) { e = cudaFuncSetAttribute(k_gradf<SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
     if (e != cudaSuccess) return e;
-    k_gradf<SH><<<grid, THREADS, gradf_smem(g.a.ncolw, Lay<SH>::NENT), s>>>(g);
+    k_gradf<SH><<<grid, THREADS, gradf_smem(g.a.ncolw, Lay<SH>::NACC), s>>>(g);
     return cudaGetLastError();
 }
 
