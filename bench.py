@@ -302,6 +302,11 @@ def run_own(args):
                 "kernel_ms": norm_ms, "bytes_per_event": BYTES_PER_EVENT_NORM, "flop_per_event": FLOP_PER_EVENT}
     fp64 = {"dfma_tflops_measured": B.probe_fp64(0, 4000) / 1e12, "dmma_tflops_measured": B.probe_fp64(1, 4000) / 1e12,
             "nominal_tflops": FP64_PEAK_NOMINAL / 1e12}
+    if roof["bound"] == "hbm":
+        # the streaming kernels' own TMA tile pipeline with the model arithmetic taken out (amp_probe_hbm_read, after the timed
+        # region): how fast this access pattern reads HBM on this box, next to the copy figure `peak` is
+        roof["read_probe_gbs"] = B.probe_hbm_read(BYTES_PER_EVENT_NORM * 12_000_000)
+        roof["frac_of_read_probe"] = roof["achieved"] / roof["read_probe_gbs"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

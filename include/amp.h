@@ -272,6 +272,13 @@ const char* amp_version(void);
  * and return achieved FLOP/s in *flops (timed with CUDA events on `stream`).                          */
 amp_status amp_probe_fp64(int kind, int iters, double* flops, void* stream);
 
+/* Read-bandwidth probe for the HBM roofline of the streaming kernels: allocates a scratch
+ * buffer of `bytes` (rounded down to whole 512-event blocks of 184 B per event; use more than the 126 MB L2), streams
+ * it through k_stream's own TMA tile pipeline (same grid, block, shared-memory staging; no model arithmetic) and
+ * returns the best of five timed passes in *gbs (GB/s, CUDA events on `stream`).  The buffer is freed before
+ * returning.  AMP_ERR_INVALID: gbs NULL or bytes below one block; AMP_ERR_NOMEM / AMP_ERR_CUDA otherwise.          */
+amp_status amp_probe_hbm_read(long long bytes, double* gbs, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

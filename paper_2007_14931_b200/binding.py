@@ -20,7 +20,7 @@ SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
     "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_grad", "amp_fit", "amp_generate", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
     "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_fit_fractions", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode", "amp_set_grad_mode",
-    "amp_last_call_stats", "amp_last_call_timing", "amp_recent_launch_ms", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64",
+    "amp_last_call_stats", "amp_last_call_timing", "amp_recent_launch_ms", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64", "amp_probe_hbm_read",
 ]
 
 
@@ -86,6 +86,7 @@ def lib():
         "amp_status_string": (C.c_char_p, [i]),
         "amp_version": (C.c_char_p, []),
         "amp_probe_fp64": (i, [i, i, pd, vp]),
+        "amp_probe_hbm_read": (i, [C.c_longlong, pd, vp]),
     }
     for name, (res, args) in sig.items():
         f = getattr(L, name)
@@ -359,6 +360,15 @@ def probe_fp64(kind, iters=2000, stream=None):
     st = lib().amp_probe_fp64(int(kind), int(iters), C.byref(out), _stream_ptr(stream))
     if st != AMP_OK:
         raise AmpError(st, "amp_probe_fp64 failed")
+    return out.value
+
+
+def probe_hbm_read(nbytes=2_208_000_000, stream=None):
+    """GB/s of k_stream's tile pipeline reading `nbytes` of scratch with no model arithmetic (amp_probe_hbm_read)."""
+    out = C.c_double(0)
+    st = lib().amp_probe_hbm_read(int(nbytes), C.byref(out), _stream_ptr(stream))
+    if st != AMP_OK:
+        raise AmpError(st, "amp_probe_hbm_read failed")
     return out.value
 
 

@@ -418,5 +418,6 @@ bool batch_fits(int nent, int ncolu);
 cudaError_t launch_finalize(const double* partial, int nblocks, int stride, int nrows, double* out, cudaStream_t s);
 
 cudaError_t probe_fp64(int kind, int iters, double* flops, cudaStream_t s);
+cudaError_t probe_hbm_read(long long bytes, double* gbs, cudaStream_t s);
 
 }  // namespace amp

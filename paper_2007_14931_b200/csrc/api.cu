@@ -476,6 +476,13 @@ amp_status amp_probe_fp64(int kind, int iters, double* flops, void* stream) {
     return probe_fp64(kind, iters, flops, (cudaStream_t)stream) == cudaSuccess ? AMP_OK : AMP_ERR_CUDA;
 }
 
+amp_status amp_probe_hbm_read(long long bytes, double* gbs, void* stream) {
+    if (!gbs || bytes < (long long)((NCOL_ALL + 1) * CACHE_TILE * sizeof(double))) return AMP_ERR_INVALID;
+    const cudaError_t e = probe_hbm_read(bytes, gbs, (cudaStream_t)stream);
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return AMP_ERR_NOMEM; }
+    return e == cudaSuccess ? AMP_OK : AMP_ERR_CUDA;
+}
+
 }  // extern "C"
 
 // ---------------------------------------------------------------------------------------------------

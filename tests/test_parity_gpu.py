@@ -772,3 +772,11 @@ def test_fp64_probe_runs():
     dfma = B.probe_fp64(0, 500)
     dmma = B.probe_fp64(1, 500)
     assert 1e12 < dfma < 1e14 and 1e11 < dmma < 1e14
+
+
+def test_hbm_read_probe_runs():
+    from paper_2007_14931_b200 import binding as B
+    gbs = B.probe_hbm_read(512 * 1024 * 1024)
+    assert 1e3 < gbs < 1e4                          # a B200 streams several TB/s; the value itself is bench.py's business
+    with pytest.raises(B.AmpError):
+        B.probe_hbm_read(1000)                      # below one 512-event block
