@@ -316,7 +316,22 @@ __device__ __forceinline__ void eval_block(const StreamArgs& a, const DeltaContr
             if (quad) {
                 it += 4;
                 if (h4[0].x & 8) eval_slot<FAST>(a, slots + h4[0].y, k, fg, zst, sv);
-                if (kind == 0) leaf_multi<NORM, 0, 4, FAST>(h4, bc, k, fg, sv, w, live, bad, y, ye);
+                if (NORM && FAST && kind == 0) {
+                    // normalisation side of four coupling points on one slot: their coefficients do not depend on the event, so
+                    //   sum_j w_j S_j(p) = sum w S(0) + Re(coef(p) sum_j w_j T2_j) + |coef(p)|^2 sum_j w_j n_j
+                    // and the three sums of the SLOT take the places of the four points here; the last CTA forms the points
+                    // from them (quad_points_from_slot_sums).  The cancellation guard stays with the data events.
+                    double t0 = 0.0, t1 = 0.0, t2 = 0.0;
+#pragma unroll
+                    for (int e = 0; e < E; ++e) {
+                        t0 = fma(w[e], sv[e].T2.x, t0);
+                        t1 = fma(w[e], sv[e].T2.y, t1);
+                        t2 = fma(w[e], sv[e].n, t2);
+                    }
+                    y[0] = t0; y[1] = t1; y[2] = t2; y[3] = 0.0;
+                    ye[0] = ye[1] = ye[2] = ye[3] = 0;
+                }
+                else if (kind == 0) leaf_multi<NORM, 0, 4, FAST>(h4, bc, k, fg, sv, w, live, bad, y, ye);
                 else leaf_multi<NORM, 1, 4, FAST>(h4, bc, k, fg, sv, w, live, bad, y, ye);
             } else {
                 two_points(&y[0], &ye[0]);
@@ -554,6 +569,29 @@ __global__ void __launch_bounds__(THREADS, 1) k_delta(const __grid_constant__ De
         tot[r] = s;
     }
     __syncthreads();
+    if (FAST) {
+        // quads of coupling points (eval_block): the four normalisation rows hold sum w T2.re, sum w T2.im, sum w n, 0 of the
+        // quad's slot; point j of the quad is sum w S(0) + Re(coef_j T2) + |coef_j|^2 n.  Thread q takes the q-th group of four.
+        __shared__ int s_first[DELTA_MAX_SORTED / 4];   // first contribution of each aligned group of four points
+        if (tid == 0) {
+            int it = 0;
+            for (int idx = 0; idx < d.nsorted; ++idx) {
+                if ((idx & 3) == 0) s_first[idx >> 2] = it;
+                while (!(prog[it++].hdr & 4)) {}
+            }
+        }
+        __syncthreads();
+        if (tid < d.nsorted / 4) {
+            const DeltaContrib* c = prog + s_first[tid];
+            if ((c[0].hdr & 64) && (c[0].hdr & 3) == 0) {
+                double* row = tot + rows + 1 + 4 * tid;
+                const double t2r = row[0], t2i = row[1], nn = row[2], s0 = tot[rows];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) row[j] = fma(c[j].c, nn, fma(c[j].a, t2r, fma(-c[j].b, t2i, s0)));
+            }
+        }
+        __syncthreads();
+    }
     for (int r = tid; r < rows; r += THREADS) {
         const int p = r == 0 ? 0 : d.point_of_sorted[r - 1];
         if (p < 0) continue;

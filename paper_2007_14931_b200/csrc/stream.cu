@@ -27,6 +27,23 @@ namespace amp {
 
 
 
+// A warp has read its part of a staged region into registers.  True in lane 0 of the LAST warp of the CTA to say so for
+// this tile (it resets the count and may overwrite the region): the warps never wait for one another here, and the count
+// cannot be touched again before the refill this warp issues has landed (the next mbarrier phase).
+__device__ __forceinline__ bool region_released(int* count) {
+    __syncwarp();
+    bool last = false;
+    if ((threadIdx.x & 31) == 0) {
+        __threadfence_block();                       // this warp's shared-memory reads are done before the count moves
+        last = atomicAdd(count, 1) == NWARPS - 1;
+        if (last) {
+            *count = 0;
+            __threadfence_block();                   // ... and every other warp's, before the bulk copy is issued
+        }
+    }
+    return last;
+}
+
 template <int MODE, class SH>
 __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __grid_constant__ StreamArgs a) {
     const double RSQRT2 = 0.70710678118654752440;
@@ -48,9 +65,11 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
     const bool with_w = MODE != MODE_DATA && MODE != MODE_DATA_M;   // the K* region carries the weight column (MODE_FUSED: only for normalisation tiles)
     double* stage = reinterpret_cast<double*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)(ncache + 1) * TILE * sizeof(double));   // [0]: K* region, [1]: Z region
+    __shared__ int consumed[2];   // warps that have taken their values of the region's current tile into registers
     if (threadIdx.x == 0) {
         mbar_init(&full[0], 1);
         mbar_init(&full[1], 1);
+        consumed[0] = consumed[1] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -84,8 +103,8 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
         const Ev cphi = load_col(stage, C_CPHI), sphi = load_col(stage, C_SPHI);
         Ev w;
         if (MODE == MODE_FUSED ? is_norm : with_w) w = load_col(stage, ncache);
-        __syncthreads();   // K* region consumed by every thread: stream the next tile into it
-        if (threadIdx.x == 0 && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[0], 0, NCOL_K, true);
+        // K* region consumed by this warp; the last warp to say so streams the next tile into it (no CTA-wide barrier)
+        if (region_released(&consumed[0]) && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[0], 0, NCOL_K, true);
 
         double2 V0[E], Vp[E], Vm[E];
 #pragma unroll
@@ -137,8 +156,8 @@ __global__ void __launch_bounds__(THREADS, AMP_STREAM_MINB) k_stream(const __gri
             const Ev ct = load_col(stage, C_CT), st = load_col(stage, C_ST);
             const Ev cpt = load_col(stage, C_CPT), spt = load_col(stage, C_SPT);
             const Ev ca = load_col(stage, C_CA), sa = load_col(stage, C_SA);
-            __syncthreads();   // Z region consumed: refill it with the next tile
-            if (threadIdx.x == 0 && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[1], NCOL_K, NCOL_ALL, false);
+            // Z region consumed: the last warp refills it with the next tile
+            if (region_released(&consumed[1]) && has_next) issue_tile<MODE>(a, ntd, tile + gridDim.x, stage, &full[1], NCOL_K, NCOL_ALL, false);
             // T_l' = sum over the Z spin classes of d^J_{0 l'}(theta_Z) U_l' ; d^J_{0,+1} = -d^J_{+1,0}, d^J_{0,-1} = -d^J_{0,+1}
             double2 T0[E], Tp[E], Tm[E];
 #pragma unroll
