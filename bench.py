@@ -38,13 +38,16 @@ FLOP_PER_EVENT = 730.0
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # 148 SMs x 64 DFMA/clk x 2 flop x 1965 MHz
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed `ncu --set full` capture
 # (profiles/): per launch, at the default sizes; None until a capture of the current kernel exists
-TRAFFIC_NCU_BYTES = 2.192192e9 + 4.78e6       # profiles/r01d_ncu_full_stream_fused_cfg3.csv (2M + 10M events)
-TRAFFIC_NCU_BYTES_CFG4 = 2.194401e9 + 7.89e6  # profiles/r01d_ncu_full_delta_cfg4.csv
+TRAFFIC_NCU_BYTES = 2.192250e9 + 3.63e6       # profiles/r01g_ncu_full_stream_fused_cfg3.csv (2M + 10M events)
+TRAFFIC_NCU_BYTES_CFG4 = 2.195064e9 + 9.09e6  # profiles/r01g_ncu_full_delta_cfg4.csv
 # Algorithmic flop per event of the gradient batch of configs[4] in its sparse form: point 0 (730) + 31 slots
 # (Breit-Wigner of point 0 from the saved barrier factors ~20, angular factor ~8, two complex products 12, and the expansion
 # coefficients T2 = 2 sum conj(A(0)) SLOT, n = sum |SLOT|^2: 25) + 100 coupling points (S(0) + Re(coef T2) + |coef|^2 n: 6, guard 1,
 # accumulate 1) + 20 mass/width points (perturbed Breit-Wigner ~22, difference to point 0 and |coef|^2: 5, expansion 6)
 DELTA_FLOP_PER_EVENT = 730.0 + 31 * 65.0 + 100 * 8.0 + 20 * 33.0
+# normalisation events: the 100 coupling points cost nothing per point there — three weighted sums per group of four on one slot
+# (25 groups x 3 FMA), the points are formed from them once per launch
+DELTA_FLOP_PER_NORM_EVENT = 730.0 + 31 * 65.0 + 25 * 6.0 + 20 * 33.0
 # analytic gradient: the point (730) + per coupling slot: angular factor ~8, T = sum_xi conj(g) A 16, conj(BW) T 8, weight 2
 GRAD_FLOP_PER_EVENT = 730.0 + 27 * 34.0
 # its shape-specialised form (gradf.cu): the point (730) + the three W_lambda and three Y_lambda' (u A, conj(g) A:
@@ -254,13 +257,13 @@ def run_own(args):
     if args.cfg == 4 and paths == {5}:
         # gradient batch: one fused k_delta launch per step, bound by the plain FP64 ALUs (DESIGN.md 5.6 / 6)
         k_ms = float(np.mean(t_data))
-        flop = DELTA_FLOP_PER_EVENT * (args.n_data + args.n_norm)
+        flop = DELTA_FLOP_PER_EVENT * args.n_data + DELTA_FLOP_PER_NORM_EVENT * args.n_norm
         ach = flop / (k_ms * 1e-3) / 1e12
         roof = {"bound": "alu", "kernel": "k_delta (gradient batch: point 0 + 120 sparse points, data then norm tiles, one launch)",
                 "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12,
                 "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md 6; the DFMA probe below measures it)", "unit": "TFLOP/s",
                 "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": TRAFFIC_NCU_BYTES_CFG4 if (args.n_data, args.n_norm) == (2_000_000, 10_000_000) else None, "kernel_ms": k_ms,
-                "flop_per_event": DELTA_FLOP_PER_EVENT, "flop_per_launch": flop,
+                "flop_per_event": [DELTA_FLOP_PER_EVENT, DELTA_FLOP_PER_NORM_EVENT], "flop_per_launch": flop,
                 "hbm_frac": (BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}
     elif paths == {7} or paths == {8}:
         # --grad: NLL and analytic gradient in one k_gradf (the paper's resonance lists) or k_grad launch per step; plain FP64 ALUs
