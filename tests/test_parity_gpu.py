@@ -291,6 +291,34 @@ def test_delta_batches_general():
         assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
 
 
+def test_gradient_batch_large_coupling_steps_in_groups_of_four():
+    """Groups of four points on one coupling (k_delta takes their normalisation side from three weighted sums of the slot,
+    DESIGN.md 5.6) with LARGE steps, so that the linear and the quadratic term of the expansion both carry weight: every coupling
+    of the full model, 109 points = one launch; then twice that = two launches.  Integrals at 1e-12, NLL at the parity bar."""
+    cfg = 2
+    Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+    x, eff, xn, wn = make_inputs(cfg, 2999, 9001)
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    c0 = W.couplings(cfg)
+    K = len(c0)
+    steps = (1.4, 0.6, 1 + 0.5j, 1 - 0.5j)
+    for reps in (1, 2):
+        P = 1 + 4 * K * reps
+        cs = np.tile(c0, (P, 1))
+        for r in range(reps):
+            for k in range(K):
+                for j, f in enumerate(steps):
+                    cs[1 + 4 * (r * K + k) + j, k] *= f * (1 + 0.1 * r)
+        Mg.set_params(cs)
+        nll = Mg.nll()
+        st = Mg.last_call_stats()
+        assert st["norm_path"] == 5 and st["launches"] == (P - 1 + 127) // 128
+        ref, refI = Mo.nll(cs, x, eff, xn, wn)
+        assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL, reps
+        assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12, reps
+
+
 def test_nll_terms_of_two_shards_add_up():
     """amp_nll_terms / amp_dataset_sums: the per-shard sums of two models that each hold half of the events combine
     (sharded.py's formula, here without a process group) to the oracle's NLL of the whole sample — for the fused
