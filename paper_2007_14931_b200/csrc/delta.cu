@@ -39,9 +39,11 @@ namespace {
 
 constexpr int DBLK = DELTA_MAX_SORTED / 32;
 #ifndef AMP_DELTA_QUNROLL
-#define AMP_DELTA_QUNROLL 2
+#define AMP_DELTA_QUNROLL 1
 #endif
-constexpr int DELTA_QUNROLL = AMP_DELTA_QUNROLL;   // unrolling of the four-point steps of a 32-point block
+// unrolling of the four-point steps of a 32-point block.  Measured on configs[4] with the slot sums on the normalisation tiles:
+// 1: 4.53 ms, 2: 4.63 ms, 4: 4.90 ms (before them 2 was best: 4.82 ms against 4.91 ms) — the loop body is instruction-cache bound
+constexpr int DELTA_QUNROLL = AMP_DELTA_QUNROLL;
 
 struct SlotVal {   // the current slot of one event
     double2 Sp, Sm;                 // xi = +1, -1
