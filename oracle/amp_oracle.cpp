@@ -14,7 +14,9 @@
 // paper's definition written out in the paper's order; where the paper is silent
 // the reading (A1..A18) is the one listed in DESIGN.md §"Readings".
 //
-// Parity pins: every function here is pinned by tests/test_oracle_pins.py (P1-P22).  The orientation
+// Parity pins: every function here is pinned by tests/test_oracle_pins.py (P1-P23), and tests/test_oracle_mutations.py
+// applies the one-line mistakes of tests/oracle_mutants.py to a copy of this file and requires a pin to fail for each.
+// The orientation
 // of theta_Z (reading A10: literal "angle between K and pi momenta in the Z rest frame",
 // PAPER.md:176) is pinned by P22: it is the Jacob-Wick helicity angle of the psi from the Z's line
 // of flight, which Eq. 10's d^{J}_{0 lambda'} requires; its supplement would only relabel the

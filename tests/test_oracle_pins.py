@@ -5,6 +5,7 @@ scipy spherical Bessel / quadrature / Legendre), a closed form, an invariant, or
 dropped term, wrong sign, wrong index or transposed operand breaks.  Pin numbers P1..P12 are those of
 DESIGN.md §"Oracle pins".
 """
+import functools
 import math
 
 import numpy as np
@@ -20,19 +21,26 @@ MB, MPSI, MK, MPI = DEC
 R16 = W.RADIUS
 
 
+@functools.lru_cache(maxsize=None)
+def _sympy_d_function(j, mp, m):
+    import sympy
+    from sympy.physics.quantum.spin import Rotation
+    b = sympy.Symbol("beta", real=True)
+    f = sympy.lambdify(b, Rotation.d(j, mp, m, b).doit(), "math")
+    return lambda beta: float(f(beta))
+
+
 def model(cfg):
     return O.Model(DEC, W.resonances(cfg))
 
 
 # ------------------------------------------------------------------ P1: Wigner d closed forms / library
 def test_P1_wigner_d_matches_sympy_and_tables():
-    from sympy import N
-    from sympy.physics.quantum.spin import Rotation
     for beta in (0.3, 1.1, 2.9):
         for j in (1, 2, 3, 4):
             for mp in range(-j, j + 1):
                 for m in (-1, 0, 1):
-                    ref = complex(N(Rotation.d(j, mp, m, beta).doit(), 30)).real
+                    ref = _sympy_d(j, mp, m, beta)
                     assert abs(O.wigner_d(j, mp, m, beta) - ref) < 2e-15, (j, mp, m, beta)
     # PDG table, j = 1 (valid for any beta, also negative)
     for b in np.linspace(-3.0, 3.0, 13):
@@ -134,6 +142,70 @@ def test_P4_barrier_polynomials_are_spherical_hankel_moduli():
         if L:
             assert O.blatt_weisskopf(L, 400.0, 300.0, R16) < 1.0 < O.blatt_weisskopf(L, 200.0, 300.0, R16)
             assert abs(O.blatt_weisskopf(L, 400.0, 300.0, 1e-9) - 1.0) < 1e-9
+
+
+def _hankel_B(L, x):
+    """x^(2L+2) |h_L^(1)(x)|^2 from scipy's spherical Bessel functions: the Blatt-Weisskopf polynomial B_L(x^2) (pin P4)"""
+    return x ** (2 * L + 2) * (special.spherical_jn(L, x) ** 2 + special.spherical_yn(L, x) ** 2)
+
+
+# ------------------------------------------------------------------ P4b: the barrier FACTOR at r != 0 (square root, normalisation)
+def test_P4b_blatt_weisskopf_factor_at_finite_radius():
+    """F^(L)(p, p0) = sqrt(B_L(z0)/B_L(z)) (reading A2) with B_L from scipy's spherical Hankel functions, at the
+    radii and momenta of the configs; for L = 1 also the textbook closed form sqrt((1 + z0)/(1 + z)).  A missing square root, a
+    swapped (p, p0) or z = r p instead of (r p)^2 fails here (at r = 1.6e-3, p ~ 300-1500 MeV: z = 0.2-6, nowhere near 1)."""
+    for r in (R16, 3.0e-3):
+        for L in range(5):
+            for p, p0 in ((291.0, 642.0), (642.0, 291.0), (1204.0, 88.0), (35.0, 1377.0)):
+                ref = math.sqrt(_hankel_B(L, r * p0) / _hankel_B(L, r * p))
+                got = O.blatt_weisskopf(L, p, p0, r)
+                assert abs(got - ref) < 1e-12 * ref, (L, p, p0, r, got, ref)
+                if L == 1:
+                    z, z0 = (r * p) ** 2, (r * p0) ** 2
+                    assert abs(got - math.sqrt((1 + z0) / (1 + z))) < 1e-14 * got
+                if L:
+                    assert abs(got * got - ref) > 1e-3 * ref          # the square root is not optional at these momenta
+
+
+# ------------------------------------------------------------------ P3c: Eqs. 2-3 at r != 0 from the complex output alone
+@pytest.mark.parametrize("radius", [R16, 3.0e-3])
+def test_P3c_barrier_factors_in_numerator_and_running_width(radius):
+    """A = num / (M^2 - m^2 - i M Gamma(m)) with num real, so 1/A gives both back without any model input:
+    num = (M^2 - m^2)/Re(1/A) and Gamma(m) = -Im(1/A) num / M.  Then, with B_L from scipy's Hankel functions (pin P4),
+        Gamma(m) m / (M Gamma0 (p_R/p_R0)^(2 L_R + 1)) = B_LR(z_R0)/B_LR(z_R)                  [F_R SQUARED in Eq. 3, PAPER.md:94]
+        num / ((p_B/M_B)^L_B (p_R/m)^L_R) = sqrt(B_LB(z_B0)/B_LB(z_B)) sqrt(B_LR(z_R0)/B_LR(z_R)) [F_B F_R in Eq. 2, PAPER.md:89]
+    for every resonance of the full model off the pole.  Dropping F_B or F_R from the numerator, F_R instead of F_R^2 in the
+    width, or a barrier factor without its square root each fail one of the two lines."""
+    res = [(k, J, m, w, radius) for (k, J, m, w, _) in W.resonances(2)]
+    M = O.Model(DEC, res)
+    for r, (kind, J, mass, width, rad) in enumerate(res):
+        LB, LR = O.orbital_L(kind, J)
+        if kind == O.KSTAR:
+            mom = lambda m: (O.breakup_momentum(MB, m, MPSI), O.breakup_momentum(m, MK, MPI))
+            lo, hi = MK + MPI + 5, MB - MPSI - 5
+        else:
+            mom = lambda m: (O.breakup_momentum(MB, m, MK), O.breakup_momentum(m, MPSI, MPI))
+            lo, hi = MPSI + MPI + 5, MB - MK - 5
+        pB0, pR0 = mom(mass)
+        for m in np.linspace(lo, hi, 9):
+            if abs(m - mass) < 1.0:
+                continue
+            A, gam = M.lineshape(r, m)
+            inv = 1.0 / A
+            num = (mass * mass - m * m) / inv.real
+            g = -inv.imag * num / mass
+            assert abs(g - gam) < 1e-9 * abs(gam)
+            pB, pR = mom(m)
+            ratioR = _hankel_B(LR, radius * pR0) / _hankel_B(LR, radius * pR)
+            ratioB = _hankel_B(LB, radius * pB0) / _hankel_B(LB, radius * pB)
+            lhs_w = g * m / (mass * width * (pR / pR0) ** (2 * LR + 1))
+            assert abs(lhs_w - ratioR) < 1e-9 * ratioR, (r, m, lhs_w, ratioR)
+            lhs_n = num / ((pB / MB) ** LB * (pR / m) ** LR)
+            assert abs(lhs_n - math.sqrt(ratioB * ratioR)) < 1e-9 * lhs_n, (r, m, lhs_n, math.sqrt(ratioB * ratioR))
+        # the factors are not trivially 1 for this resonance (else the two lines above pin nothing); L = 0 factors are 1
+        pB, pR = mom(0.5 * (lo + mass) if mass - lo > 50 else 0.5 * (hi + mass))
+        if LB:
+            assert abs(_hankel_B(LB, radius * pB0) / _hankel_B(LB, radius * pB) - 1.0) > 1e-3
 
 
 # ------------------------------------------------------------------ P5: kinematic invariants
@@ -863,3 +935,99 @@ def test_P22_supplement_of_theta_Z_is_a_relabelling_of_the_couplings(kind, J):
         S_sup_flip = sum(abs(c_flip @ Bs[:, j]) ** 2 for j in range(2))
         assert abs(S_sup - S_flip[i]) < 1e-11 * S[i] and abs(S_sup_flip - S[i]) < 1e-11 * S[i]
     assert (np.abs(S - S_flip) / S).max() > 1e-3                   # the relabelling is not trivial: the sign matters at fixed H
+
+
+# ------------------------------------------------------------------ P23: the K* branch of the basis terms (Eq. 4) and its frame relative to the Z's
+def _sympy_d(j, mp, m, beta):
+    """sympy's Wigner small-d (sympy.physics.quantum.spin.Rotation.d), its symbolic form compiled once per (j, m', m)"""
+    return _sympy_d_function(j, mp, m)(beta)
+
+
+def test_P23_kstar_basis_terms_are_eq4_with_library_d_functions():
+    """Eq. 4 (PAPER.md:111): B_(R,lambda),xi = A^R(m) d^J_{lambda 0}(theta_K*) e^{i lambda phi} d^1_{lambda xi}(theta_psi), rebuilt in the
+    test from the separately pinned lineshape (P3, P3c) and sympy's d functions (a few events) / the Legendre forms
+    d^J_{+-1 0} = -+ sin P_J'(cos)/sqrt(J(J+1)), d^J_00 = P_J (numpy, more events), against the oracle's `basis_terms` for the full
+    K* + Z model: slot order, the index order of d^J_{lambda 0}, the sign of the phi phase and the helicity index of d^1."""
+    res = W.resonances(2)
+    M = model(2)
+    slots = W.slot_table(res)
+    x = W.phase_space_events(np.random.default_rng(23), 40)
+    for i in range(x.shape[1]):
+        m, cK, cpsi, phi = x[:, i]
+        thK, thpsi = math.acos(cK), math.acos(cpsi)
+        B = M.basis_terms(x[:, i])
+        for k, (r, lam) in enumerate(slots):
+            kind, J = res[r][0], res[r][1]
+            if kind != O.KSTAR:
+                continue
+            A = M.lineshape(r, m)[0]
+            if i < 4:
+                dJ = _sympy_d(J, lam, 0, thK)
+                d1 = [_sympy_d(1, lam, xi, thpsi) for xi in (1, -1)]
+            else:
+                PJ = npleg.Legendre.basis(J)
+                dJ = PJ(cK) if lam == 0 else -lam * math.sin(thK) * PJ.deriv()(cK) / math.sqrt(J * (J + 1))
+                d1 = [{(1, 1): (1 + cpsi) / 2, (1, -1): (1 - cpsi) / 2, (-1, 1): (1 - cpsi) / 2, (-1, -1): (1 + cpsi) / 2,
+                       (0, 1): math.sin(thpsi) / math.sqrt(2), (0, -1): -math.sin(thpsi) / math.sqrt(2)}[(lam, xi)] for xi in (1, -1)]   # PDG table
+            for ix in range(2):
+                ref = A * dJ * np.exp(1j * lam * phi) * d1[ix]
+                assert abs(B[k, ix] - ref) < 1e-13 * abs(A), (i, k, r, lam, ix, B[k, ix], ref)
+
+
+def test_P23_kstar_and_z_basis_terms_share_one_jpsi_frame():
+    """Pin P7's rotation identity applied to the ORACLE'S OWN basis terms (PAPER.md:111 Eq. 4, :167 Eq. 10): the J/psi-side factor
+    u_{lambda xi} = B_(K*,lambda),xi / (A^K* d^J_{lambda 0}(theta_K*)) of the K* chain, rotated by the spin-1 matrix of the rotation that
+    takes the K* axes (z = n_K*) into the Z axes (z = n_pi), must equal the Z chain's v_{lambda' xi} = B_(Z,lambda'),xi / (A^Z
+    d^1_{0 lambda'}(theta_Z)):   sum_lambda d^1_{lambda lambda'}(beta) u_{lambda xi} = v_{lambda' xi}.
+    Fixes the sign of e^{i lambda phi} and the index order of d^J_{lambda 0} RELATIVE to the Z chain — what decides the K*-Z
+    interference (Eq. 12).  Library d functions throughout (sympy); the oracle supplies only B, A and the angles."""
+    res = [W.resonances(2)[i] for i in (1, 4, 6, 10)]           # K*(892) J=1, K2*(1430) J=2, K3*(1780) J=3, Z(4200)
+    assert [r[1] for r in res] == [1, 2, 3, 1] and res[3][0] == O.ZRES
+    M = O.Model(DEC, res)
+    x = W.phase_space_events(np.random.default_rng(2323), 25)
+    worst, wrong_phi, wrong_idx = 0.0, 0, 0
+    for i in range(x.shape[1]):
+        m, cK, cpsi, phi = x[:, i]
+        zk = M.z_kinematics(x[:, i])
+        B = M.basis_terms(x[:, i])
+        thK, thZ = math.acos(cK), math.atan2(zk["sinZ"], zk["cosZ"])
+        ez = zk["nKst"]
+        ex = zk["nK"] - (zk["nK"] @ ez) * ez
+        ex /= np.linalg.norm(ex)
+        beta = math.atan2(zk["npi"] @ ex, zk["npi"] @ ez)
+        AZ = M.lineshape(3, zk["mZ"])[0]
+        v = np.array([[B[9 + lp + 1, ix] / (AZ * _sympy_d(1, 0, lp, thZ)) for ix in range(2)] for lp in (-1, 0, 1)])
+        D = np.array([[_sympy_d(1, l, lp, beta) for lp in (-1, 0, 1)] for l in (-1, 0, 1)])          # D[l, lp]
+        for r, J in ((0, 1), (1, 2), (2, 3)):
+            A = M.lineshape(r, m)[0]
+            u = np.array([[B[3 * r + l + 1, ix] / (A * _sympy_d(J, l, 0, thK)) for ix in range(2)] for l in (-1, 0, 1)])
+            worst = max(worst, np.abs(D.T @ u - v).max())
+            # what the two plausible mistakes would give: e^{-i lambda phi}, and d^J_{0 lambda} = (-1)^lambda d^J_{lambda 0}
+            u_phi = np.conj(u * np.exp(-1j * np.array([-1, 0, 1])[:, None] * phi)) * np.exp(-1j * np.array([-1, 0, 1])[:, None] * phi)
+            u_idx = u * np.array([-1.0, 1.0, -1.0])[:, None]
+            wrong_phi += np.abs(D.T @ u_phi - v).max() > 1e-2
+            wrong_idx += np.abs(D.T @ u_idx - v).max() > 1e-2
+    assert worst < 1e-12, worst
+    assert wrong_phi > 60 and wrong_idx > 60                      # of 75: either mistake breaks the identity at O(1)
+
+
+def test_P23_kstar_phase_convention_changes_the_density_when_a_z_interferes():
+    """The two K* conventions pinned by P23 are not relabellings once a Z is present at FIXED couplings: S rebuilt with
+    e^{-i lambda phi} (or d^J_{0 lambda}) in the K* terms and the oracle's own Z terms differs from the oracle's S at O(10 %)."""
+    res = W.resonances(2)
+    M = model(2)
+    c = W.couplings(2)
+    slots = W.slot_table(res)
+    x = W.phase_space_events(np.random.default_rng(233), 30)
+    S = M.eval_events(c, x)
+    lam = np.array([l for (_, l) in slots], dtype=float)
+    isK = np.array([res[r][0] == O.KSTAR for (r, _) in slots])
+    dphi, didx = [], []
+    for i in range(x.shape[1]):
+        B = M.basis_terms(x[:, i])
+        assert abs(sum(abs(c @ B[:, j]) ** 2 for j in range(2)) - S[i]) < 1e-13 * S[i]      # Eq. 12 from the basis terms
+        Bp = np.where(isK[:, None], B * np.exp(-2j * lam * x[3, i])[:, None], B)          # e^{i lambda phi} -> e^{-i lambda phi}
+        Bi = np.where(isK[:, None], B * ((-1.0) ** lam)[:, None], B)                        # d^J_{lambda 0} -> d^J_{0 lambda}
+        dphi.append(abs(sum(abs(c @ Bp[:, j]) ** 2 for j in range(2)) / S[i] - 1))
+        didx.append(abs(sum(abs(c @ Bi[:, j]) ** 2 for j in range(2)) / S[i] - 1))
+    assert np.median(dphi) > 1e-2 and np.median(didx) > 1e-2
