@@ -95,7 +95,9 @@ int amp_num_resonances(const amp_model* m);
  *   d_eff device [n] relative efficiency eps_i > 0 (Eq. 14), or NULL (= 1).
  * Replaces a previously loaded data set.  n >= 0 (n == 0: NLL data term is 0).  Synchronises `stream`.
  * AMP_ERR_DOMAIN if any event is outside phase space (m_Kpi not in (m_K+m_pi, m_B-m_psi), |cos| > 1,
- * non-finite input, eps <= 0); the data set is then left unloaded.                                    */
+ * non-finite input, eps <= 0) or, for a model with a Z, has an undefined Z-chain angle (mu+ exactly along the pion in the
+ * J/psi frame — e.g. cos(theta_K*) = +-1 together with cos(theta_J/psi) = +-1 — or m_J/psi pi exactly at a threshold:
+ * PAPER.md:176-179 define the angles between planes that then do not exist); the data set is then left unloaded.     */
 amp_status amp_load_events(amp_model* m, const double* d_x, const double* d_eff, long long n, void* stream);
 
 /* Load the phase-space Monte Carlo sample used for the normalisation integral.
@@ -143,7 +145,10 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
  *   h_mass_width host [R][2] start / fixed masses and widths, or NULL (= the values given at amp_model_create; only
  *                without floating lineshape parameters)
  *   fixed        [n_fixed] slots held constant (Eq. 6: the K*(892) lambda = 0 amplitude)
- *   tie_dst/src  [n_ties] H[dst] = H[src] (Eq. 11); a dst is not free and not a src of another tie
+ *   tie_dst/src  [n_ties] H[dst] = sign * H[src] (Eq. 11); a dst is not free, not fixed, not a src of another tie
+ *                and appears once
+ *   tie_sign     [n_ties] +1 or -1, or NULL (= all +1).  Eq. 11 is H_+1 = H_-1 for the 1+ Z the paper considers; parity
+ *                conservation in Z -> J/psi pi gives H_l' = P (-1)^(1 - J) H_-l' in general (A24), i.e. -1 for 2+ and 1-
  *   float_mw     [n_float_mw][2] = (resonance index, 0: its mass / 1: its width) floating lineshape parameters, no duplicates
  *   h_scale      host [K] positive parameter scales or NULL (= |start|, floored at 1e-3 of the largest); masses and widths
  *                are scaled by the start width
@@ -152,12 +157,13 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
  *   h_nll        host [2]: NLL at the fit, max |gradient| there
  *   h_cov        host [n][n], n = 2F + n_float_mw (F = free slots, ascending; Re, Im per slot; then float_mw order): covariance
  *                = inverse Hessian of the NLL, the Hessian from central differences of the gradient (2 n more evaluations); or NULL
- *   h_info       host int[5] or NULL: converged, likelihood evaluations, iterations, covariance positive definite, n
+ *   h_info       host int[5] or NULL: converged, likelihood evaluations, iterations, covariance valid (Hessian positive definite
+ *                and every evaluation behind it finite; else h_cov is NaN), n
  * The model is left with the fitted point set.  Errors of amp_set_params / amp_nll_grad / amp_nll are passed on (a trial point
  * outside the likelihood's domain makes the line search back off); AMP_ERR_INVALID for bad indices, chained ties, duplicates
  * or a non-positive scale; AMP_ERR_DOMAIN if the start point has no finite likelihood.                                       */
 amp_status amp_fit(amp_model* m, const double* h_start, const double* h_mass_width, const int* fixed, int n_fixed,
-                   const int* tie_dst, const int* tie_src, int n_ties, const int* float_mw, int n_float_mw,
+                   const int* tie_dst, const int* tie_src, const int* tie_sign, int n_ties, const int* float_mw, int n_float_mw,
                    const double* h_scale, int max_iter, double gtol,
                    double* h_fit, double* h_fit_mw, double* h_nll, double* h_cov, int* h_info, void* stream);
 
@@ -193,7 +199,7 @@ amp_status amp_set_background(amp_model* m, const double* d_bkg, double purity, 
  *   h_sum_log[p] = sum_i log S_i(p) over the loaded data events (without the efficiency), h_sum_wS[p] = sum_j w_j S_j(p)
  * over the loaded normalisation events, host [P] each.  With the constants of amp_dataset_sums summed over the shards,
  *   NLL(p) = -( sum_shards sum_log[p] + sum_shards sum_log_eff ) + N_total log( sum_shards sum_wS[p] / sum_shards sum_w ).
- * Same launches, states and errors as amp_nll.                                                                       */
+ * Same launches, states and errors as amp_nll; AMP_ERR_STATE with a background set (Eq. 14 does not separate).       */
 amp_status amp_nll_terms(amp_model* m, double* h_sum_log, double* h_sum_wS, void* stream);
 /* Per-dataset constants fixed at load time: number of data events, sum_i log eps_i, number of normalisation events,
  * sum_j w_j (0 for a sample that is not loaded).  Any output pointer may be NULL.                                     */

@@ -627,6 +627,24 @@ void orc_lineshape(const double* decay, int kind, int J, double mass, double wid
     }
 }
 
+// A^R at an EVENT: the running mass of the resonance's chain (m_Kpi, or m_psipi from O6) is formed from the event in the working
+// precision and handed to O3 without passing through a double — plumbing of z_kinematics + lineshape for the long-double
+// arbitration of the parity tests near the m_psipi thresholds (no arithmetic of its own).  out[0..1] = A^R (re, im), out[2] = running mass
+}  // extern "C"
+template <typename T>
+static void lineshape_at_event_fill(const double* decay, int kind, int J, double mass, double width, double radius, const double* x, double* out) {
+    Decay<T> dk{T(decay[0]), T(decay[1]), T(decay[2]), T(decay[3])};
+    Resonance<T> R{kind, J, T(mass), T(width), T(radius)};
+    const T m = is_z(kind) ? z_kinematics<T>(dk, T(x[0]), T(x[1]), T(x[2]), T(x[3])).mZ : T(x[0]);
+    const std::complex<T> A = lineshape<T>(dk, R, m);
+    out[0] = double(A.real()); out[1] = double(A.imag()); out[2] = double(m);
+}
+extern "C" {
+void orc_lineshape_at_event(const double* decay, int kind, int J, double mass, double width, double radius, const double* x /*[4]*/, int prec, double* out /*[3]*/) {
+    DISPATCH(prec, lineshape_at_event_fill<double>(decay, kind, J, mass, width, radius, x, out),
+             lineshape_at_event_fill<long double>(decay, kind, J, mass, width, radius, x, out));
+}
+
 // out[0..6] = mZ, cosZ, sinZ, cosT, sinT, phiT, alpha; out[7..18] = K_B, pi_B, psi_B (E,px,py,pz);
 // out[19..30] = nK, npi, nKst, nmu (unit 3-vectors in the psi rest frame)
 }  // extern "C"

@@ -28,6 +28,7 @@ _lib.orc_wigner_d.argtypes = [_i, _i, _i, _d, _i]
 _lib.orc_orbital_L.argtypes = [_i, _i, C.POINTER(_i), C.POINTER(_i)]
 _lib.orc_lineshape.argtypes = [_pd, _i, _i, _d, _d, _d, _d, _i, _pd]
 _lib.orc_z_kinematics.argtypes = [_pd, _pd, _i, _pd]
+_lib.orc_lineshape_at_event.argtypes = [_pd, _i, _i, _d, _d, _d, _pd, _i, _pd]
 _lib.orc_num_couplings.restype = _i
 _lib.orc_num_couplings.argtypes = [_i, _pi, _pi]
 _MODEL = [_pd, _i, _pi, _pi, _pd, _pd, _pd]
@@ -107,6 +108,14 @@ class Model:
         _lib.orc_lineshape(self.decay, int(self.kinds[r]), int(self.Js[r]), self.mass[r], self.width[r], self.radius[r],
                            float(m), prec, out)
         return complex(out[0], out[1]), out[2]
+
+    def lineshape_at_event(self, r, x, prec=0):
+        """A^R of resonance r at the event x = (m_Kpi, cosK, cosPsi, phi): its chain's running mass is formed in the working
+        precision (prec=1: long double) and never rounded to double on the way to the lineshape."""
+        out = np.zeros(3)
+        _lib.orc_lineshape_at_event(self.decay, int(self.kinds[r]), int(self.Js[r]), self.mass[r], self.width[r], self.radius[r],
+                                    _f64(x), prec, out)
+        return complex(out[0], out[1])
 
     def z_kinematics(self, x, prec=0):
         out = np.zeros(31)

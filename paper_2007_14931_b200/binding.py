@@ -63,7 +63,7 @@ def lib():
         "amp_set_params": (i, [vp, i, vp, vp]),
         "amp_nll": (i, [vp, vp, vp]),
         "amp_nll_grad": (i, [vp, vp, vp, vp]),
-        "amp_fit": (i, [vp, vp, vp, vp, i, vp, vp, i, vp, i, vp, i, d, vp, vp, vp, vp, vp, vp]),
+        "amp_fit": (i, [vp, vp, vp, vp, i, vp, vp, vp, i, vp, i, vp, i, d, vp, vp, vp, vp, vp, vp]),
         "amp_generate": (i, [vp, C.c_ulonglong, C.c_ulonglong, ll, d, d, d, d, vp, vp, ll, C.POINTER(ll), pd, vp]),
         "amp_nll_terms": (i, [vp, vp, vp, vp]),
         "amp_dataset_sums": (i, [vp, C.POINTER(ll), pd, C.POINTER(ll), pd]),
@@ -211,6 +211,7 @@ class Model:
         fx = np.ascontiguousarray(list(fixed), dtype=np.int32)
         td = np.ascontiguousarray([t[0] for t in ties], dtype=np.int32)
         ts = np.ascontiguousarray([t[1] for t in ties], dtype=np.int32)
+        tg = np.ascontiguousarray([t[2] if len(t) > 2 else 1 for t in ties], dtype=np.int32)   # (dst, src) or (dst, src, +-1)
         fm = np.ascontiguousarray([[int(r), int(w)] for r, w in float_mw], dtype=np.int32).reshape(-1, 2)
         hs = None if scale is None else np.ascontiguousarray(scale, dtype=np.float64)
         free = [k for k in range(self.K) if k not in set(int(f) for f in fixed) and k not in set(int(t) for t in td)]
@@ -219,7 +220,7 @@ class Model:
         out_mw = np.empty((self.R, 2)) if hmw is not None else None
         cov = np.empty((n, n)) if errors else None
         p = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None and a.size else None
-        self._check(lib().amp_fit(self._h, p(hc), p(hmw), p(fx), len(fx), p(td), p(ts), len(td), p(fm), len(fm), p(hs), int(max_iter), float(gtol),
+        self._check(lib().amp_fit(self._h, p(hc), p(hmw), p(fx), len(fx), p(td), p(ts), p(tg), len(td), p(fm), len(fm), p(hs), int(max_iter), float(gtol),
                                   p(out), p(out_mw), p(nll), p(cov), p(info), _stream_ptr(stream)), "amp_fit")
         self.P = 1
         res = {"couplings": out[:, 0] + 1j * out[:, 1], "mass_width": out_mw, "nll": float(nll[0]), "grad_max": float(nll[1]),

@@ -77,6 +77,23 @@ struct Dataset {
 
 static inline long long pad32(long long n) { return (n + 31) / 32 * 32; }
 
+// ---- per-device host state -------------------------------------------------------------------------------
+// One process may drive several devices (one amp_model per device): the SM count that sizes the persistent grids and the
+// opt-in to more than 48 KB of dynamic shared memory (cudaFuncSetAttribute applies to the CURRENT device only) are kept
+// per device, not per process.
+enum { AMP_MAX_DEVICES = 64 };
+static inline int current_device() {
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= AMP_MAX_DEVICES) d = 0;
+    return d;
+}
+int sm_count();   // multiprocessors of the current device (kinematics.cu)
+// first() is true the first time it is called on the current device; one function-local static per kernel instantiation
+struct DeviceOnce {
+    bool seen[AMP_MAX_DEVICES] = {};
+    bool first() { const int d = current_device(); const bool f = !seen[d]; seen[d] = true; return f; }
+};
+
 // ---- tiled cache addressing --------------------------------------------------------------------------
 constexpr int CACHE_TILE = 512;
 // element (col, i) of a cache with ncolw = ncache + 1 columns per block (the weight is column ncache)

@@ -18,6 +18,10 @@ using namespace amp;
 
 namespace {
 
+// values of amp_model::colidx below zero.  The plan builders of the tensor-core paths use -2 for "lineshape == 1" in THEIR entry
+// lists, so the in-register marker must not be -2: a point whose columns are not held has to be refused there, not read as 1.
+enum { COL_NONE = -1, COL_INLINE = -3 };
+
 struct PoolEntry {
     int r = -1;
     double mass = 0, width = 0;
@@ -28,6 +32,7 @@ struct PoolEntry {
 }  // namespace
 
 struct amp_model {
+    int device = 0;                // the device the model was created on and owns its memory on; every call runs there
     DecayConst dk{};
     std::vector<amp_resonance> res;
     int R = 0, K = 0;
@@ -42,7 +47,7 @@ struct amp_model {
     int P = 0;
     std::vector<double> couplings;   // [P][K][2]
     std::vector<double> mw;          // [P][R][2]
-    std::vector<int> colidx;         // [P][R] pool slot, -1 for CONST, -2 for inline evaluation
+    std::vector<int> colidx;         // [P][R] pool slot >= 0, or COL_NONE (constant term: no lineshape) / COL_INLINE (evaluated in registers, no column held)
     int miss_streak[AMP_MAX_RESONANCES]{};
     bool was_inline[AMP_MAX_RESONANCES]{};   // evaluated in registers by the previous call
     long long call_id = 0;
@@ -78,7 +83,7 @@ struct amp_model {
     std::vector<double> gram_mw;
     double* d_G = nullptr;         // [KP][KP] dense symmetric realified Gram matrix (sum_j w_j b' b'^T)
     double* d_gt = nullptr;        // [ntile][64]
-    double* d_gpartial = nullptr;  // [148][ntile][64]
+    double* d_gpartial = nullptr;  // [SMs][ntile][64]
     size_t gram_cap_KP = 0, gram_cap_tiles = 0;
     unsigned char* d_hk = nullptr; // herk plan: entries, tiles, coefficients
     unsigned char* h_hk = nullptr; // pinned
@@ -128,6 +133,17 @@ amp_status cuda_fail(amp_model* m, cudaError_t e, const char* where) {
         cudaError_t e_ = (call);                                  \
         if (e_ != cudaSuccess) return cuda_fail(m, e_, #call);    \
     } while (0)
+
+// Makes the model's device current for the duration of a call (a process may hold one model per device) and restores the
+// caller's device afterwards.
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const amp_model* m) {
+        int cur = 0;
+        if (m && cudaGetDevice(&cur) == cudaSuccess && cur != m->device) { prev = cur; cudaSetDevice(m->device); }
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 double h_two_body(double M, double a, double b) {
     const double s = a + b, d = a - b;
@@ -320,6 +336,7 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
     }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { delete m; return AMP_ERR_CUDA; }
+    if (cudaGetDevice(&m->device) != cudaSuccess) { delete m; return AMP_ERR_CUDA; }
     cudaError_t e = cudaMalloc(&m->d_partial, sizeof(double) * 2 * AMP_MAX_POINTS * PARTIAL_STRIDE);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_sums, sizeof(double) * 2 * AMP_MAX_POINTS);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_result, sizeof(double) * (4 * AMP_MAX_POINTS + 4));
@@ -339,6 +356,7 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
 
 amp_status amp_model_destroy(amp_model* m) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     free_dataset(m->data);
     free_dataset(m->norm);
     if (m->d_partial) cudaFree(m->d_partial);
@@ -368,17 +386,20 @@ int amp_num_resonances(const amp_model* m) { return m ? m->R : -1; }
 
 amp_status amp_load_events(amp_model* m, const double* d_x, const double* d_eff, long long n, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     return load_dataset(m, m->data, false, d_x, d_eff, n, (cudaStream_t)stream);
 }
 
 amp_status amp_load_norm(amp_model* m, const double* d_x, const double* d_w, long long n_norm, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     if (n_norm < 1) return fail(m, AMP_ERR_INVALID, "amp_load_norm: need at least one normalisation event");
     return load_dataset(m, m->norm, true, d_x, d_w, n_norm, (cudaStream_t)stream);
 }
 
 amp_status amp_set_background(amp_model* m, const double* d_bkg, double purity, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     cudaStream_t s = (cudaStream_t)stream;
     if (!d_bkg) {   // back to the signal-only likelihood
         if (m->d_bkg) cudaFree(m->d_bkg);
@@ -390,7 +411,7 @@ amp_status amp_set_background(amp_model* m, const double* d_bkg, double purity, 
     if (m->d_bkg) cudaFree(m->d_bkg);
     m->d_bkg = nullptr;
     CK(cudaMalloc(&m->d_bkg, sizeof(double) * m->data.npad));
-    k_fill<<<148 * 4, 256, 0, s>>>(m->d_bkg, m->data.npad, 1.0);
+    k_fill<<<sm_count() * 4, 256, 0, s>>>(m->d_bkg, m->data.npad, 1.0);
     CK(cudaGetLastError());
     CK(cudaMemcpyAsync(m->d_bkg, d_bkg, sizeof(double) * m->data.n, cudaMemcpyDeviceToDevice, s));
     CK(cudaStreamSynchronize(s));
@@ -440,6 +461,7 @@ amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_r
 
 amp_status amp_last_call_timing(const amp_model* m, double* ms4) {
     if (!m || !ms4) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     if (m->fused_valid) {   // one launch: everything is reported as the combine phase of both samples
         float t = 0;
         cudaEventSynchronize(m->ring[2 * m->ring_last + 1]);   // (a zero-copy call returns before its end event has landed)
@@ -458,6 +480,7 @@ amp_status amp_last_call_timing(const amp_model* m, double* ms4) {
 
 amp_status amp_recent_launch_ms(const amp_model* m, int max_calls, double* h_ms, int* n_out) {
     if (!m || !h_ms || !n_out || max_calls < 0) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     const long long have = std::min<long long>(m->ring_calls, amp_model::RING);
     const int n = (int)std::min<long long>(have, max_calls);
     for (int i = 0; i < n; ++i) {   // oldest of the n first
@@ -744,12 +767,12 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
             keyslot[k] = best;
         }
     }
-    m->colidx.assign((size_t)P * R, -1);
+    m->colidx.assign((size_t)P * R, COL_NONE);
     for (int r = 0; r < R; ++r) m->was_inline[r] = false;
     for (int p = 0; p < P; ++p)
         for (int r = 0; r < R; ++r) {
             const int k = keyidx[(size_t)p * R + r];
-            if (k >= 0) m->colidx[(size_t)p * R + r] = inline_key[k] ? -2 : keyslot[k];
+            if (k >= 0) m->colidx[(size_t)p * R + r] = inline_key[k] ? COL_INLINE : keyslot[k];
             if (k >= 0 && inline_key[k]) m->was_inline[r] = true;
         }
     return AMP_OK;
@@ -914,7 +937,7 @@ bool build_batch_plan(const amp_model* m, int p0, int Pc, BatchPlan* bp) {
     for (int k = 0; k < K; ++k) {
         const int r = slot_res[k];
         const int col = m->res[r].kind == AMP_CONST ? -2 : m->colidx[(size_t)p0 * R + r];
-        if (col == -1 || col < -2) return false;
+        if (col == COL_NONE || col == COL_INLINE) return false;   // no column held for this lineshape: not this path
         bp->entries[k] = make_int2(col, slot_code(m, r, slot_lam[k]));
     }
     bp->Adense.assign((size_t)16 * 2 * BATCH_NKT * 32, 0.0);
@@ -952,7 +975,7 @@ bool build_batch_plan(const amp_model* m, int p0, int Pc, BatchPlan* bp) {
             const int r = slot_res[k];
             const double cre = m->couplings[((size_t)p * K + k) * 2], cim = m->couplings[((size_t)p * K + k) * 2 + 1];
             const int col = m->res[r].kind == AMP_CONST ? -2 : m->colidx[(size_t)p * R + r];
-            if (col == -1 || col < -2) return false;
+            if (col == COL_NONE || col == COL_INLINE) return false;   // no column held for this lineshape: not this path
             int e = k;
             if (col != bp->entries[k].x) {   // this point uses another lineshape column for this slot: extended entry
                 e = -1;
@@ -1067,7 +1090,7 @@ bool build_herk_plan(const amp_model* m, HerkPlan* hp, int pbase = 0, int npts =
     for (int k = 0; k < K; ++k) {
         const int r = slot_res[k];
         const int col = m->res[r].kind == AMP_CONST ? -2 : m->colidx[(size_t)pbase * R + r];
-        if (col == -1 || col < -2) return false;
+        if (col == COL_NONE || col == COL_INLINE) return false;   // no column held for this lineshape: not this path
         ent[k] = make_int2(col, slot_code(m, r, slot_lam[k]));
     }
     std::vector<std::vector<std::pair<int, double2>>> coef(P);
@@ -1076,7 +1099,7 @@ bool build_herk_plan(const amp_model* m, HerkPlan* hp, int pbase = 0, int npts =
             const int p = pbase + q;
             const int r = slot_res[k];
             const int col = m->res[r].kind == AMP_CONST ? -2 : m->colidx[(size_t)p * R + r];
-            if (col == -1 || col < -2) return false;
+            if (col == COL_NONE || col == COL_INLINE) return false;   // no column held for this lineshape: not this path
             int e = k;
             if (col != ent[k].x) {
                 e = -1;
@@ -1193,7 +1216,7 @@ amp_status norm_via_matrix(amp_model* m, const HerkPlan& hp, double* d_out, cuda
         m->gram_cap_tiles = ntile;
         CK(cudaMalloc(&m->d_G, sizeof(double) * (size_t)KP * KP));
         CK(cudaMalloc(&m->d_gt, sizeof(double) * (size_t)ntile * 64));
-        CK(cudaMalloc(&m->d_gpartial, sizeof(double) * (size_t)148 * ntile * 64));
+        CK(cudaMalloc(&m->d_gpartial, sizeof(double) * (size_t)sm_count() * ntile * 64));
     }
     std::memcpy(m->h_hk + oE, hp.entries.data(), bE);
     std::memcpy(m->h_hk + oT, hp.tiles.data(), bT);
@@ -1577,13 +1600,16 @@ extern "C" {
 
 amp_status amp_nll(amp_model* m, double* h_nll, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     if (!h_nll) return fail(m, AMP_ERR_INVALID, "amp_nll: null output");
     return evaluate(m, true, h_nll, nullptr, (cudaStream_t)stream);
 }
 
 amp_status amp_nll_terms(amp_model* m, double* h_sum_log, double* h_sum_wS, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     if (!h_sum_log || !h_sum_wS) return fail(m, AMP_ERR_INVALID, "amp_nll_terms: null output");
+    if (m->has_bkg) return fail(m, AMP_ERR_STATE, "amp_nll_terms: not defined with a background set (Eq. 14 does not separate into the two sums)");
     std::vector<double> nll((size_t)std::max(m->P, 1));
     const amp_status st = evaluate(m, true, nll.data(), nullptr, (cudaStream_t)stream);
     if (st != AMP_OK && st != AMP_ERR_DOMAIN) return st;
@@ -1602,6 +1628,7 @@ amp_status amp_dataset_sums(const amp_model* m, long long* n_data, double* sum_l
 
 amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     if (!h_nll || !h_grad) return fail(m, AMP_ERR_INVALID, "amp_nll_grad: null output");
     cudaStream_t s = (cudaStream_t)stream;
     if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
@@ -1706,12 +1733,14 @@ amp_status amp_nll_grad(amp_model* m, double* h_nll, double* h_grad, void* strea
 
 amp_status amp_norm_integral(amp_model* m, double* h_I, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     if (!h_I) return fail(m, AMP_ERR_INVALID, "amp_norm_integral: null output");
     return evaluate(m, false, nullptr, h_I, (cudaStream_t)stream);
 }
 
 amp_status amp_eval_events(amp_model* m, int p, double* d_out, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     cudaStream_t s = (cudaStream_t)stream;
     if (!m->data.loaded) return fail(m, AMP_ERR_STATE, "no data events loaded (amp_load_events)");
     if (m->P < 1) return fail(m, AMP_ERR_STATE, "no parameters set (amp_set_params)");
@@ -1738,6 +1767,7 @@ amp_status amp_generate(amp_model* m, unsigned long long seed, unsigned long lon
                         double* d_x_out, long long* d_index_out, long long capacity,
                         long long* h_n_accepted, double* h_f_seen_max, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     cudaStream_t s = (cudaStream_t)stream;
     if (n_candidates < 0 || capacity < 0 || (capacity > 0 && !d_x_out) || !h_n_accepted || !h_f_seen_max)
         return fail(m, AMP_ERR_INVALID, "amp_generate: negative count or null output");
@@ -1831,12 +1861,13 @@ const char* amp_cache_column_name(int i) { return (i >= 0 && i < NCOL_ALL) ? kCo
 
 amp_status amp_dump_cache(amp_model* m, int which, double* d_out, int* ncols, void* stream) {
     if (!m || which < 0 || which > 1) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     Dataset& d = which ? m->norm : m->data;
     if (!d.loaded) return fail(m, AMP_ERR_STATE, "amp_dump_cache: dataset not loaded");
     if (ncols) *ncols = d.ncache;
     if (!d_out || d.n == 0) return AMP_OK;
     cudaStream_t s = (cudaStream_t)stream;
-    k_dump_cache<<<148 * 4, 256, 0, s>>>(d.cache, d.ncache + 1, d.ncache, d.n, d_out);
+    k_dump_cache<<<sm_count() * 4, 256, 0, s>>>(d.cache, d.ncache + 1, d.ncache, d.n, d_out);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(s));
     return AMP_OK;
@@ -1844,6 +1875,7 @@ amp_status amp_dump_cache(amp_model* m, int which, double* d_out, int* ncols, vo
 
 amp_status amp_eval_lineshape(amp_model* m, int which, int r, double mass, double width, double* d_out, void* stream) {
     if (!m || which < 0 || which > 1 || r < 0 || r >= m->R || !d_out) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     Dataset& d = which ? m->norm : m->data;
     if (!d.loaded) return fail(m, AMP_ERR_STATE, "amp_eval_lineshape: dataset not loaded");
     cudaStream_t s = (cudaStream_t)stream;
@@ -1863,6 +1895,7 @@ amp_status amp_eval_lineshape(amp_model* m, int which, int r, double mass, doubl
 
 amp_status amp_fit_fractions(amp_model* m, int p, double* h_ff, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     cudaStream_t s = (cudaStream_t)stream;
     if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
     if (m->P < 1) return fail(m, AMP_ERR_STATE, "no parameters set (amp_set_params)");
@@ -1900,6 +1933,7 @@ amp_status amp_fit_fractions(amp_model* m, int p, double* h_ff, void* stream) {
 
 amp_status amp_norm_matrix(amp_model* m, int p, double* h_M, void* stream) {
     if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
     cudaStream_t s = (cudaStream_t)stream;
     if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
     if (m->P < 1) return fail(m, AMP_ERR_STATE, "no parameters set (amp_set_params)");

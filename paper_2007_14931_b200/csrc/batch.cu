@@ -147,7 +147,7 @@ bool batch_fits(int nent, int ncolu) { return ncolu <= BATCH_MAX_COLS && batch_s
 
 int batch_grid(long long n) {
     const long long ntiles = (n + BT_EVENTS - 1) / BT_EVENTS;
-    return (int)(ntiles < 1 ? 1 : (ntiles > 148 ? 148 : ntiles));   // persistent: one CTA per SM
+    return (int)(ntiles < 1 ? 1 : (ntiles > sm_count() ? sm_count() : ntiles));   // persistent: one CTA per SM
 }
 
 cudaError_t launch_batch(const BatchArgs& a, int grid, cudaStream_t s) {
@@ -155,8 +155,8 @@ cudaError_t launch_batch(const BatchArgs& a, int grid, cudaStream_t s) {
     cudaError_t e = cudaSuccess;
 #define AMP_LAUNCH(NKT, M)                                                                                           \
     {                                                                                                                \
-        static bool attr_done = false;                                                                               \
-        if (!attr_done) { e = cudaFuncSetAttribute(k_batch<NKT, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; } \
+        static DeviceOnce attr_done;                                                                               \
+        if (attr_done.first()) { e = cudaFuncSetAttribute(k_batch<NKT, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); } \
         if (e == cudaSuccess) k_batch<NKT, M><<<grid, BT_THREADS, smem, s>>>(a);                                     \
     }
     if (a.nkt != BATCH_NKT) return cudaErrorInvalidValue;

@@ -622,9 +622,9 @@ size_t delta_smem(bool have_z, int ngrp) {
 
 template <class SH, bool FAST>
 cudaError_t launch_delta_shape(const DeltaArgs& d, int grid, cudaStream_t s) {
-    static bool attr_done = false;
+    static DeviceOnce attr_done;
     cudaError_t e = cudaSuccess;
-    if (!attr_done) { e = cudaFuncSetAttribute(k_delta<SH, FAST>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
+    if (attr_done.first()) { e = cudaFuncSetAttribute(k_delta<SH, FAST>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); }
     if (e != cudaSuccess) return e;
     const bool have_z = d.a.gstart[NSPIN] > d.a.gstart[5];
     k_delta<SH, FAST><<<grid, THREADS, delta_smem(have_z, d.a.gstart[NSPIN]), s>>>(d);
@@ -637,7 +637,7 @@ bool delta_fits(int ngrp) { return delta_smem(true, ngrp) <= (size_t)224 * 1024;
 
 int delta_grid(long long n_data, long long n_norm) {
     const long long ntiles = (n_data + TILE - 1) / TILE + (n_norm + TILE - 1) / TILE;
-    return (int)(ntiles < 1 ? 1 : (ntiles > 148 ? 148 : ntiles));   // persistent: one CTA per SM
+    return (int)(ntiles < 1 ? 1 : (ntiles > sm_count() ? sm_count() : ntiles));   // persistent: one CTA per SM
 }
 
 // the paper's model (ten K* + one Z, one radius per spin) runs the unrolled shape; anything else the generic loops.

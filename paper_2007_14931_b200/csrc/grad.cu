@@ -315,13 +315,13 @@ bool grad_fits(int nent, int ngrp) { (void)ngrp; return grad_smem(true, nent) <=
 
 int grad_grid(long long n_data, long long n_norm) {
     const long long ntiles = (n_data + TILE - 1) / TILE + (n_norm + TILE - 1) / TILE;
-    return (int)(ntiles < 1 ? 1 : (ntiles > 148 ? 148 : ntiles));   // persistent: one CTA per SM
+    return (int)(ntiles < 1 ? 1 : (ntiles > sm_count() ? sm_count() : ntiles));   // persistent: one CTA per SM
 }
 
 cudaError_t launch_grad(const GradArgs& g, int grid, cudaStream_t s) {
-    static bool attr_done = false;
+    static DeviceOnce attr_done;
     cudaError_t e = cudaSuccess;
-    if (!attr_done) { e = cudaFuncSetAttribute(k_grad, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
+    if (attr_done.first()) { e = cudaFuncSetAttribute(k_grad, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); }
     if (e != cudaSuccess) return e;
     int nent = g.a.nlass;
     for (int sp = 0; sp < NSPIN; ++sp) nent += g.a.shape[sp];

@@ -314,9 +314,9 @@ size_t gradf_smem(int ncolw, int nacc) {
 
 template <class SH>
 cudaError_t launch_gradf_shape(const GradArgs& g, int grid, cudaStream_t s) {
-    static bool attr_done = false;
+    static DeviceOnce attr_done;
     cudaError_t e = cudaSuccess;
-    if (!attr_done) { e = cudaFuncSetAttribute(k_gradf<SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
+    if (attr_done.first()) { e = cudaFuncSetAttribute(k_gradf<SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); }
     if (e != cudaSuccess) return e;
     k_gradf<SH><<<grid, THREADS, gradf_smem(g.a.ncolw, Lay<SH>::NACC), s>>>(g);
     return cudaGetLastError();
@@ -326,7 +326,7 @@ cudaError_t launch_gradf_shape(const GradArgs& g, int grid, cudaStream_t s) {
 
 int gradf_grid(long long n_data, long long n_norm) {
     const long long nunits = 2 * ((n_data + CACHE_TILE - 1) / CACHE_TILE) + 2 * ((n_norm + CACHE_TILE - 1) / CACHE_TILE);
-    return (int)(nunits < 1 ? 1 : (nunits > 148 ? 148 : nunits));   // persistent: one CTA per SM
+    return (int)(nunits < 1 ? 1 : (nunits > sm_count() ? sm_count() : nunits));   // persistent: one CTA per SM
 }
 
 // 1 if the point is one of the specialised shapes (one radius per spin class, no constant or LASS term, no background, Z's

@@ -137,9 +137,9 @@ int herk_max_runs() { return HERK_MAXRUN; }
 
 template <int NRUN>
 static cudaError_t launch_herk_n(const HerkArgs& h, int grid, cudaStream_t s) {
-    static bool attr_done = false;
+    static DeviceOnce attr_done;
     cudaError_t e = cudaSuccess;
-    if (!attr_done) { e = cudaFuncSetAttribute(k_herk<NRUN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; }
+    if (attr_done.first()) { e = cudaFuncSetAttribute(k_herk<NRUN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); }
     if (e != cudaSuccess) return e;
     k_herk<NRUN><<<grid, BT_THREADS, tile_smem_bytes(h.b.nent, h.b.ncolu), s>>>(h);
     return cudaGetLastError();

@@ -5,10 +5,10 @@
 // need, the sines of the input helicity angles, the phi phase, and the Z-chain
 // variables m_psipi, theta_Z, theta~_psi, phi~, alpha.
 //
-// The Z chain is derived from Lorentz invariants and closed forms,
-// not by boosting 4-vectors: in the J/psi rest frame every hadron lies in the x-z plane (z = K*
-// direction, K on the +x side), so only z components change under the boost along z and the two
-// dihedral angles reduce to ratios of components of the mu+ direction.
+// The Z chain is derived from planar closed forms, not by boosting
+// 3D 4-vectors: in the J/psi rest frame every hadron lies in the x-z plane (z = K* direction, K on the
+// +x side), so only z components change under the boost along z, the two dihedral angles reduce to
+// ratios of components of the mu+ direction, and the Z frame is one more boost along the pion.
 //
 // HBM-bound: reads 32-40 B, writes 88-184 B per event; one thread per event, fully coalesced.  The cache is written in
 // the tiled layout of amp_internal.cuh (blocks of 512 events, one 4 KB column per quantity, the weight last).
@@ -59,18 +59,22 @@ __global__ void __launch_bounds__(256) k_kinematics(const KinArgs a) {
         col[C_SPHI * CACHE_TILE] = sphi;
         if (!a.with_z) continue;
 
-        // B frame, z along the K pi system.  Energies in the K pi frame, then boosted with gamma = E_Kpi/m.
-        const double EKpi = (MB * MB + m2 - mpsi * mpsi) / (2.0 * MB), Epsi = MB - EKpi;
-        const double g = EKpi * invm, bg = pB * invm;
-        const double Epi_r = (m2 - mK * mK + mpi * mpi) * (0.5 * invm);
-        const double Epi = g * Epi_r - bg * q * cK;      // pion energy, B frame
-        const double ppz = bg * Epi_r - g * q * cK;      // pion p_z, B frame (p_x = -q sK)
-        // m_psipi^2 = (P_psi + P_pi)^2, linear in cos theta_K*
-        const double mZ2 = mpsi * mpsi + mpi * mpi + 2.0 * (Epsi * Epi + pB * ppz);
+        // From the K pi rest frame (K along (sK, 0, cK), the J/psi along -z with energy E*_psi and momentum p*_psi = pB MB / m)
+        // straight to the J/psi rest frame, a boost along z: for (E, p_z) there, p_z' = (E*_psi p_z + p*_psi E) / m_psi and
+        // E' = (E*_psi E + p*_psi p_z) / m_psi; p_x is unchanged.  Every hadron stays in the x-z plane.
+        const double Epi_r = (m2 - mK * mK + mpi * mpi) * (0.5 * invm), EK_r = (m2 + mK * mK - mpi * mpi) * (0.5 * invm);
+        const double Eps = (MB * MB - m2 - mpsi * mpsi) * (0.5 * invm), pps = pB * MB * invm;
+        const double qc = q * cK, qs = q * sK, impsi = 1.0 / mpsi;
+        const double pz = (pps * Epi_r - Eps * qc) * impsi, px = -qs;          // pion
+        const double Epi_p = (Eps * Epi_r - pps * qc) * impsi;
+        const double kz = (pps * EK_r + Eps * qc) * impsi, kx = qs;            // kaon
+        const double EK_p = (Eps * EK_r + pps * qc) * impsi;
+        // m_psipi^2 = (P_psi + P_pi)^2 = m_psi^2 + m_pi^2 + 2 m_psi E'_pi, linear in cos theta_K*
+        const double mZ2 = mpsi * mpsi + mpi * mpi + 2.0 * mpsi * Epi_p;
         const double mZ = sqrt(mZ2), invmZ = 1.0 / mZ;
-        // J/psi rest frame: boost along z; pion direction n_pi = (nx, 0, nz)
-        const double pz = (Epsi * ppz + pB * Epi) / mpsi, px = -q * sK;
-        const double inorm = rsqrt(pz * pz + px * px);
+        // pion direction n_pi = (nx, 0, nz) and momentum p' in the J/psi rest frame
+        const double pp2 = pz * pz + px * px;
+        const double inorm = rsqrt(pp2), pp = pp2 * inorm;
         const double nx = px * inorm, nz = pz * inorm;
         // mu+ direction n_mu = (spsi cphi, spsi sphi, cpsi); theta~ = angle(mu+, pi)
         const double ct = spsi * cphi * nx + cpsi * nz;
@@ -81,14 +85,21 @@ __global__ void __launch_bounds__(256) k_kinematics(const KinArgs a) {
         // phi~: azimuth of mu+ about n_pi from the K side; alpha: from the (mu+,pi) to the (mu+,K*) plane about n_mu
         const double cpt = ax * ist, spt = ay * ist;
         const double ca = (spsi * nz - cpsi * cphi * nx) * ist, sa = -sphi * nx * ist;
-        // Z rest frame: theta_Z = angle(K, pi) from invariants; sine from the Gram determinant
-        const double pBZ = two_body(MB, mZ, mK);         // Z (and K) momentum in the B frame
-        const double qZ = two_body(mZ, mpsi, mpi);       // pi momentum in the Z frame
-        const double pKZ = pBZ * MB * invmZ;             // K momentum in the Z frame
-        const double EKZ = (MB * MB - mZ2 - mK * mK) * (0.5 * invmZ), EpiZ = (mZ2 + mpi * mpi - mpsi * mpsi) * (0.5 * invmZ);
-        const double iden = 1.0 / (pKZ * qZ);
-        const double cZ = (EKZ * EpiZ - 0.5 * (m2 - mK * mK - mpi * mpi)) * iden;
-        const double sZ = MB * q * pB * sK * invmZ * iden;
+        // Z rest frame = the J/psi frame boosted along n_pi (gamma = (m_psi + E'_pi)/m_Z, gamma v = p'/m_Z): the pion keeps its
+        // direction, |p_pi^Z| = p' m_psi / m_Z; the kaon's components along and across n_pi give theta_Z = angle(K, pi) and |p_K^Z|
+        // directly.  No momentum is formed from m_psipi minus a threshold: within 1e-3 MeV of m_psi + m_pi or m_B - m_K that
+        // subtraction loses 1e-10 of the angle and of the barrier momenta, these component forms 1e-13.
+        const double nk = nx * kx + nz * kz;
+        const double apar = ((mpsi + Epi_p) * nk - pp * EK_p) * invmZ;
+        const double aperp = fabs(nz * kx - nx * kz);    // (n_pi x p_K)_y > 0: the kaon is on the +x side
+        const double pKZ = sqrt(apar * apar + aperp * aperp), iden = 1.0 / pKZ;
+        const double cZ = apar * iden, sZ = aperp * iden;
+        const double qZ = pp * mpsi * invmZ;             // pi momentum in the Z frame (p_R of the Z)
+        const double pBZ = pKZ * mZ / MB;                // Z (and K) momentum in the B frame (p_B of the Z)
+        // degenerate Z-chain geometry (reading A17): mu+ exactly along the pion (st = 0: phi~ and alpha undefined), m_psipi exactly at
+        // one of its thresholds (theta_Z undefined), the pion at rest in the J/psi frame.  Measure zero; refused at load instead of
+        // caching NaN that would only surface in a later amp_nll.
+        if (!isfinite(ist * iden * inorm * invmZ)) { bad = true; continue; }
         col[C_MZ2 * CACHE_TILE] = mZ2;
         col[C_INVMZ * CACHE_TILE] = invmZ;
         col[C_QZ * CACHE_TILE] = qZ;
@@ -116,9 +127,20 @@ __global__ void __launch_bounds__(256) k_kinematics(const KinArgs a) {
     }
 }
 
+int sm_count() {
+    static int cache[AMP_MAX_DEVICES] = {};
+    const int d = current_device();
+    if (!cache[d]) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, d) != cudaSuccess || v < 1) v = 148;   // B200
+        cache[d] = v;
+    }
+    return cache[d];
+}
+
 int kinematics_grid(long long n) {
     long long blocks = (n + 255) / 256;
-    const long long cap = 148 * 8;
+    const long long cap = (long long)sm_count() * 8;
     return (int)(blocks < 1 ? 1 : (blocks > cap ? cap : blocks));
 }
 

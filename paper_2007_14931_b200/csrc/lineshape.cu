@@ -48,7 +48,7 @@ cudaError_t launch_lineshape(const Dataset& d, const LineshapeJob* jobs, int njo
         a.n = d.n;
         a.npad = d.npad;
         long long blocks = (d.n + 255) / 256;
-        const long long cap = 148 * 8;
+        const long long cap = (long long)sm_count() * 8;
         const int grid = (int)(blocks < 1 ? 1 : (blocks > cap ? cap : blocks));
         k_lineshape<<<grid, 256, 0, s>>>(a);
         cudaError_t e = cudaGetLastError();

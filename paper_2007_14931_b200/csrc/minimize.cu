@@ -25,6 +25,7 @@ struct Problem {
     int K, R, n;                       // n = 2 * number of free slots
     std::vector<int> free_slot;        // free slots
     std::vector<int> tie_dst, tie_src;
+    std::vector<double> tie_sign;      // H[dst] = sign * H[src], sign = +1 or -1 (Eq. 11: the sign depends on the Z's spin-parity)
     std::vector<double> c0;            // [K][2] start (fixed slots stay)
     std::vector<double> scale;         // [K]
     const double* mw;                  // [R][2] or null: what amp_set_params receives (mwv when lineshape parameters float)
@@ -49,8 +50,8 @@ struct Problem {
             c_out[2 * k + 1] = th[2 * i + 1] * scale[k];
         }
         for (size_t t = 0; t < tie_dst.size(); ++t) {
-            c_out[2 * tie_dst[t]] = c_out[2 * tie_src[t]];
-            c_out[2 * tie_dst[t] + 1] = c_out[2 * tie_src[t] + 1];
+            c_out[2 * tie_dst[t]] = tie_sign[t] * c_out[2 * tie_src[t]];
+            c_out[2 * tie_dst[t] + 1] = tie_sign[t] * c_out[2 * tie_src[t] + 1];
         }
     }
     // NLL and its gradient in theta; a domain error (non-finite likelihood) is reported as +inf so that a line search backs off
@@ -80,8 +81,8 @@ struct Problem {
                 g[2 * free_slot.size() + i] = (bnll[1 + 2 * i] - bnll[2 + 2 * i]) / (2.0 * mw_step[i]) * mw_scale[i];
         }
         for (size_t t = 0; t < tie_dst.size(); ++t) {
-            grad[2 * tie_src[t]] += grad[2 * tie_dst[t]];
-            grad[2 * tie_src[t] + 1] += grad[2 * tie_dst[t] + 1];
+            grad[2 * tie_src[t]] += tie_sign[t] * grad[2 * tie_dst[t]];
+            grad[2 * tie_src[t] + 1] += tie_sign[t] * grad[2 * tie_dst[t] + 1];
         }
         for (size_t i = 0; i < free_slot.size(); ++i) {
             const int k = free_slot[i];
@@ -208,7 +209,7 @@ bool spd_inverse(std::vector<double>& A, int n) {
 }  // namespace
 
 extern "C" amp_status amp_fit(amp_model* m, const double* h_start, const double* h_mass_width, const int* fixed, int n_fixed,
-                              const int* tie_dst, const int* tie_src, int n_ties, const int* float_mw, int n_float_mw,
+                              const int* tie_dst, const int* tie_src, const int* tie_sign, int n_ties, const int* float_mw, int n_float_mw,
                               const double* h_scale, int max_iter, double gtol,
                               double* h_fit, double* h_fit_mw, double* h_nll, double* h_cov, int* h_info, void* stream) {
     if (!m || !h_start || !h_fit || !h_nll || n_fixed < 0 || n_ties < 0 || (n_fixed && !fixed) || (n_ties && (!tie_dst || !tie_src)) ||
@@ -228,7 +229,10 @@ extern "C" amp_status amp_fit(amp_model* m, const double* h_start, const double*
     }
     for (int i = 0; i < n_ties; ++i) {
         if (tie_dst[i] < 0 || tie_dst[i] >= P.K || tie_src[i] < 0 || tie_src[i] >= P.K || tie_dst[i] == tie_src[i]) return AMP_ERR_INVALID;
+        if (tie_sign && tie_sign[i] != 1 && tie_sign[i] != -1) return AMP_ERR_INVALID;
+        if (held[tie_dst[i]]) return AMP_ERR_INVALID;   // a destination that is fixed, or tied twice
         held[tie_dst[i]] = 1;
+        P.tie_sign.push_back(tie_sign ? (double)tie_sign[i] : 1.0);
         P.tie_dst.push_back(tie_dst[i]);
         P.tie_src.push_back(tie_src[i]);
     }
@@ -333,6 +337,7 @@ extern "C" amp_status amp_fit(amp_model* m, const double* h_start, const double*
     h_nll[0] = f;
     h_nll[1] = max_abs(g);
     int cov_ok = 0;
+    bool hess_finite = true;   // an evaluation outside the likelihood's domain (f = inf, g = 0) must not enter the covariance
     const int nc = 2 * (int)P.free_slot.size();
     auto par_scale = [&](int i) { return i < nc ? P.scale[P.free_slot[i / 2]] : P.mw_scale[i - nc]; };
     if (h_cov && n > 0) {
@@ -344,12 +349,13 @@ extern "C" amp_status amp_fit(amp_model* m, const double* h_start, const double*
             if (!P.eval(xx.data(), &fp, gp.data())) return P.status;
             xx[j] = x[j] - h;
             if (!P.eval(xx.data(), &fm, gm.data())) return P.status;
+            hess_finite = hess_finite && std::isfinite(fp) && std::isfinite(fm);
             xx[j] = x[j];
             for (int i = 0; i < n; ++i) A[(size_t)i * n + j] = (gp[i] - gm[i]) / (2.0 * h);
         }
         for (int i = 0; i < n; ++i)
             for (int j = 0; j < i; ++j) A[(size_t)i * n + j] = A[(size_t)j * n + i] = 0.5 * (A[(size_t)i * n + j] + A[(size_t)j * n + i]);
-        cov_ok = spd_inverse(A, n) ? 1 : 0;
+        cov_ok = (hess_finite && spd_inverse(A, n)) ? 1 : 0;
         for (int i = 0; i < n; ++i)
             for (int j = 0; j < n; ++j)
                 h_cov[(size_t)i * n + j] = cov_ok ? A[(size_t)i * n + j] * par_scale(i) * par_scale(j) : NAN;

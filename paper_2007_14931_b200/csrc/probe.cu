@@ -49,7 +49,7 @@ cudaError_t probe_fp64(int kind, int iters, double* flops, cudaStream_t s) {
     cudaEvent_t t0, t1;
     cudaEventCreate(&t0);
     cudaEventCreate(&t1);
-    const int grid = 148 * 8, block = 256;
+    const int grid = sm_count() * 8, block = 256;
     double best = 0;
     for (int rep = 0; rep < 4; ++rep) {   // rep 0 is warm-up
         cudaEventRecord(t0, s);
@@ -122,9 +122,7 @@ cudaError_t probe_hbm_read(long long bytes, double* gbs, cudaStream_t s) {
     double* sink = buf + (size_t)ntiles * tile_bytes / sizeof(double);
     e = cudaMemsetAsync(buf, 0, (size_t)ntiles * tile_bytes + 8, s);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_probe_read, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes);
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int sms = sm_count();
     cudaEvent_t t0, t1;
     cudaEventCreate(&t0);
     cudaEventCreate(&t1);

@@ -292,7 +292,7 @@ int stream_grid(long long n, bool have_z, int mode) {
     long long per_sm = (long long)((224 * 1024) / (stream_smem(have_z, mode) + 1024));
     if (per_sm > AMP_STREAM_MINB) per_sm = AMP_STREAM_MINB;
     if (per_sm < 1) per_sm = 1;
-    const long long cap = 148 * per_sm;
+    const long long cap = (long long)sm_count() * per_sm;
     return (int)(ntiles < 1 ? 1 : (ntiles > cap ? cap : ntiles));
 }
 
@@ -310,8 +310,8 @@ static cudaError_t launch_shape(const StreamArgs& a, int grid, cudaStream_t s) {
     cudaError_t e = cudaSuccess;
 #define AMP_LAUNCH(M)                                                                                              \
     {                                                                                                              \
-        static bool attr_done = false;                                                                             \
-        if (!attr_done) { e = cudaFuncSetAttribute(k_stream<M, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); attr_done = true; } \
+        static DeviceOnce attr_done;                                                                             \
+        if (attr_done.first()) { e = cudaFuncSetAttribute(k_stream<M, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); } \
         if (e == cudaSuccess) k_stream<M, SH><<<grid, THREADS, smem, s>>>(a);                                      \
     }
     switch (a.mode) {

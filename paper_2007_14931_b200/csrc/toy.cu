@@ -136,7 +136,7 @@ int toy_blocks(long long n) { return (int)((n + TOY_BLOCK - 1) / TOY_BLOCK); }
 
 cudaError_t launch_toy_candidates(const ToyArgs& t, cudaStream_t s) {
     const long long blocks = (t.n + TOY_THREADS - 1) / TOY_THREADS;
-    k_toy_candidates<<<(int)(blocks < 148 * 8 ? (blocks < 1 ? 1 : blocks) : 148 * 8), TOY_THREADS, 0, s>>>(t);
+    k_toy_candidates<<<(int)(blocks < sm_count() * 8 ? (blocks < 1 ? 1 : blocks) : sm_count() * 8), TOY_THREADS, 0, s>>>(t);
     return cudaGetLastError();
 }
 

@@ -26,7 +26,8 @@ def fit_couplings(model, c_start, fixed=(), ties=(), mass_width=None, maxiter=30
 
     c_start   complex [K] starting values (fixed slots keep these values)
     fixed     slots held constant (e.g. the K*(892) lambda = 0 slot, Eq. 6)
-    ties      (dst, src) pairs with H[dst] = H[src] (Eq. 11); dst is not a free parameter
+    ties      (dst, src) or (dst, src, sign) with H[dst] = sign * H[src], sign = +-1 (Eq. 11, PAPER.md:183: +1 for the 1+ Z;
+              -1 for a 2+ or 1- Z, amp.h); dst is not a free parameter
     scale     optional positive [K] parameter scales (default |c_start|, floored): the fit runs in H / scale
     errors    also return the covariance of the free parameters: inverse of the Hessian of the NLL at the minimum, the Hessian
               from central differences of the ANALYTIC gradient (2 launches per free real parameter) — what the pulls of the
@@ -38,7 +39,7 @@ def fit_couplings(model, c_start, fixed=(), ties=(), mass_width=None, maxiter=30
     c0 = np.asarray(c_start, dtype=np.complex128).copy()
     K = c0.size
     assert K == model.K
-    tied = {int(d): int(s) for d, s in ties}
+    tied = {int(t[0]): (int(t[1]), float(t[2]) if len(t) > 2 else 1.0) for t in ties}
     free = [k for k in range(K) if k not in set(int(f) for f in fixed) and k not in tied]
     sc = np.maximum(np.abs(c0), 1e-3 * np.max(np.abs(c0))) if scale is None else np.asarray(scale, dtype=np.float64)
     mw = None if mass_width is None else np.asarray(mass_width, dtype=np.float64).reshape(1, model.R, 2)
@@ -49,8 +50,8 @@ def fit_couplings(model, c_start, fixed=(), ties=(), mass_width=None, maxiter=30
         t = theta.reshape(-1, 2)
         for i, k in enumerate(free):
             c[k] = (t[i, 0] + 1j * t[i, 1]) * sc[k]
-        for d, s in tied.items():
-            c[d] = c[s]
+        for d, (s, sg) in tied.items():
+            c[d] = sg * c[s]
         return c
 
     def fun(theta):
@@ -59,8 +60,8 @@ def fit_couplings(model, c_start, fixed=(), ties=(), mass_width=None, maxiter=30
         nll, g = model.nll_grad()                 # g[k] = (dNLL/dRe H_k, dNLL/dIm H_k)
         calls[0] += 1
         g = g.copy()
-        for d, s in tied.items():                 # chain rule of H[dst] = H[src]
-            g[s] += g[d]
+        for d, (s, sg) in tied.items():           # chain rule of H[dst] = sign H[src]
+            g[s] += sg * g[d]
         return nll, (g[free] * sc[free, None]).ravel()
 
     theta0 = np.stack([(c0[free] / sc[free]).real, (c0[free] / sc[free]).imag], -1).ravel()
@@ -105,7 +106,7 @@ def pull_study(model, c_true, n_toys, n_events, seed, m_lo, m_hi, cos_max, fixed
     ones = torch.ones(n_events, dtype=torch.float64, device="cuda")
     rng = np.random.default_rng(seed)
     pulls, conv, ncall, cs = [], [], [], []
-    tied = {int(d): int(s) for d, s in ties}
+    tied = {int(t[0]): (int(t[1]), float(t[2]) if len(t) > 2 else 1.0) for t in ties}
     for t in range(n_toys):
         model.set_params(c_true)
         x, _, _, fseen = model.generate_toy(n_events, seed + 1 + t, m_lo, m_hi, cos_max, f_max=f_max, block=1 << 20)
@@ -115,8 +116,8 @@ def pull_study(model, c_true, n_toys, n_events, seed, m_lo, m_hi, cos_max, fixed
         start = c_true * (1 + start_spread * rng.uniform(-1, 1, c_true.size)) * np.exp(1j * start_spread * rng.uniform(-1, 1, c_true.size))
         for k in fixed:
             start[k] = c_true[k]
-        for d, s in tied.items():
-            start[d] = start[s]
+        for d, (s, sg) in tied.items():
+            start[d] = sg * start[s]
         if native:      # the minimiser of the library (amp_fit): no interpreter between two launches
             r = model.fit(start, fixed=fixed, ties=ties, scale=np.abs(c_true), errors=True)
             cf, free, err, ok, nc = r["couplings"], r["free"], r["errors"], r["converged"] and r["errors"] is not None, r["n_calls"]

@@ -37,7 +37,7 @@ def stub(tmp_path_factory):
     lib = C.CDLL(out)
     vp, i, d = C.c_void_p, C.c_int, C.c_double
     lib.amp_fit.restype = i
-    lib.amp_fit.argtypes = [vp, vp, vp, vp, i, vp, vp, i, vp, i, vp, i, d, vp, vp, vp, vp, vp, vp]
+    lib.amp_fit.argtypes = [vp, vp, vp, vp, i, vp, vp, vp, i, vp, i, vp, i, d, vp, vp, vp, vp, vp, vp]
     return lib
 
 
@@ -47,6 +47,7 @@ def run(lib, start, fixed=(), ties=(), scale=None, max_iter=3000, gtol=1e-7, cov
     fx = np.ascontiguousarray(fixed, dtype=np.int32)
     td = np.ascontiguousarray([t[0] for t in ties], dtype=np.int32)
     ts = np.ascontiguousarray([t[1] for t in ties], dtype=np.int32)
+    tg = np.ascontiguousarray([t[2] for t in ties], dtype=np.int32) if ties and all(len(t) > 2 for t in ties) else None
     sc = None if scale is None else np.ascontiguousarray(scale, dtype=np.float64)
     nfree = K - len(set(fixed)) - len(td)
     fm = np.ascontiguousarray(float_mw, dtype=np.int32).reshape(-1, 2)
@@ -54,7 +55,7 @@ def run(lib, start, fixed=(), ties=(), scale=None, max_iter=3000, gtol=1e-7, cov
     fit, nll, info, fit_mw = np.empty((K, 2)), np.empty(2), np.zeros(5, dtype=np.int32), np.zeros((1, 2))
     n = 2 * nfree + len(fm)
     cv = np.empty((n, n)) if cov else None
-    st = lib.amp_fit(C.c_void_p(1), p(hs), p(hmw), p(fx), len(fx), p(td), p(ts), len(td), p(fm), len(fm), p(sc), max_iter, gtol, p(fit),
+    st = lib.amp_fit(C.c_void_p(1), p(hs), p(hmw), p(fx), len(fx), p(td), p(ts), p(tg), len(td), p(fm), len(fm), p(sc), max_iter, gtol, p(fit),
                      p(fit_mw), p(nll), p(cv), p(info), None)
     if mw is not None:
         return st, fit, nll, cv, info, fit_mw
@@ -126,6 +127,9 @@ def test_bad_arguments_and_domain_backoff(stub):
     assert run(stub, start, fixed=[K])[0] == 1                    # AMP_ERR_INVALID: slot out of range
     assert run(stub, start, ties=[(2, 2)])[0] == 1                # tie to itself
     assert run(stub, start, ties=[(2, 3), (3, 4)])[0] == 1        # chained ties
+    assert run(stub, start, ties=[(2, 3), (2, 4)])[0] == 1        # one destination tied twice
+    assert run(stub, start, fixed=[2], ties=[(2, 3)])[0] == 1     # a fixed slot as destination
+    assert run(stub, start, ties=[(2, 3, 0)])[0] == 1             # sign must be +1 or -1
     assert run(stub, start, scale=np.zeros(K))[0] == 1            # non-positive scale
     assert run(stub, start, gtol=0.0)[0] == 1
     # max_iter = 0: no step, start returned, covariance at the start point still computed
@@ -178,3 +182,34 @@ def test_floating_mass_and_width(stub):
     # a start whose first steps would make the width negative: the stand-in refuses, the search backs off and still converges
     st, fit, nll, cov, info, fmw = run(stub, start, mw=(4230.0, 3.0), float_mw=[(0, 0), (0, 1)], gtol=1e-6, cov=False)
     assert st == 0 and info[0] == 1 and abs(fmw[0, 1] - GS) < 1e-3
+
+
+def test_signed_ties_and_hessian_outside_the_domain(stub):
+    """H[dst] = -H[src] (Eq. 11 for a 2+ or 1- Z): minimum of the reduced problem against scipy; a Hessian step that leaves the
+    likelihood's domain (the stand-in refuses Re H_0 > 50) must clear the covariance flag instead of entering the matrix"""
+    start = np.full(2 * K, 0.5)
+    ties = [(5, 3, -1), (7, 2, 1)]
+    st, fit, nll, cov, info = run(stub, start, ties=ties)
+    assert st == 0 and info[0] == 1 and info[3] == 1
+    assert np.array_equal(fit[5], -fit[3]) and np.array_equal(fit[7], fit[2])
+    free = [k for k in range(K) if k not in (5, 7)]
+
+    def red(t):
+        h = np.zeros((K, 2))
+        h[free] = t.reshape(-1, 2)
+        h[5], h[7] = -h[3], h[2]
+        f, g = f_and_grad(h.ravel())
+        g = g.reshape(K, 2).copy()
+        g[3] -= g[5]
+        g[2] += g[7]
+        return f, g[free].ravel()
+
+    from scipy.optimize import minimize
+    r = minimize(red, start.reshape(K, 2)[free].ravel(), jac=True, method="BFGS", options={"gtol": 1e-9})
+    assert abs(nll[0] - r.fun) < 1e-9 * max(1.0, abs(r.fun)) and np.max(np.abs(fit[free].ravel() - r.x)) < 1e-6
+    # at the known minimum with a huge scale on slot 0: the Hessian's +h step puts Re H_0 at 1 + 100 > 50
+    target = 1.0 + 0.1 * np.arange(2 * K)
+    scale = np.ones(K)
+    scale[0] = 1e6
+    st, fit, nll, cov, info = run(stub, target, scale=scale, max_iter=0)
+    assert st == 0 and info[3] == 0 and np.all(np.isnan(cov))

@@ -86,3 +86,36 @@ def test_sharded_nll_two_ranks_gloo(tmp_path):
     world = 2
     mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
     assert all((tmp_path / f"ok{r}").exists() for r in range(world))
+
+
+def test_thread_reducer_two_virtual_ranks():
+    """sharded.ThreadReducer (the exchange step between virtual ranks of one process): two threads form the per-shard sums with
+    the oracle and must both get the oracle's NLL of the whole sample, bit for bit the same"""
+    import threading
+    sys.path.insert(0, ROOT)
+    from oracle import oracle as O
+    from paper_2007_14931_b200 import sharded as S
+    from paper_2007_14931_b200 import workloads as W
+    cfg = 1
+    Mo = O.Model(W.DECAY, W.resonances(cfg))
+    c = W.couplings(cfg)
+    xn, wn = W.norm_events(cfg, 3001)
+    x, eff = W.data_events(cfg, lambda xx, ee: Mo.eval_events(c, xx, ee), n=801)
+    red = S.ThreadReducer(2)
+    out = [None, None]
+
+    def rank_main(r):
+        port = red.port(r)
+        lo, hi = S.shard_bounds(x.shape[1], port.rank, port.world)
+        ln, hn = S.shard_bounds(xn.shape[1], port.rank, port.world)
+        totals = S.combine_constants(hi - lo, float(np.sum(np.log(eff[lo:hi]))), hn - ln, float(np.sum(wn[ln:hn])), reduce=port)
+        sl = np.array([np.sum(np.log(Mo.eval_events(c, x[:, lo:hi], None)))])
+        sw = np.array([np.sum(Mo.eval_events(c, xn[:, ln:hn], wn[ln:hn]))])
+        out[r] = S.combine_terms(sl, sw, totals, reduce=port)
+
+    th = [threading.Thread(target=rank_main, args=(r,)) for r in range(2)]
+    [t.start() for t in th]
+    [t.join() for t in th]
+    ref, ref_I = Mo.nll(c, x, eff, xn, wn)
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    assert abs(out[0][0][0] - ref[0]) < 1e-12 * abs(ref[0]) and abs(out[0][1][0] - ref_I[0]) < 1e-12 * ref_I[0]
