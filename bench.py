@@ -8,11 +8,20 @@ resonances, new couplings) + one `amp_nll` through the C ABI, i.e. one pass of t
 (lineshapes -> combine -> normalisation -> -log L reduction) over the data and the normalisation sample.
 The kinematics cache is built once per dataset (step a1, outside the per-step metric, reported separately).
 
+The default run then times configs[4] (P = 121: the MINUIT-style gradient batch of the fit loop) on the same
+loaded events and prints it inside the same JSON line as "cfg4".
+
 One JSON line on stdout (rank 0).  `--impl reference` times the CPU oracle instead (rank 0 only).
+Multi-GPU: `--gpus N` under torchrun (or alone: bench.py starts the N ranks itself) runs N independent replicas (weak
+scaling, no data-path collective: the paper's validation is hundreds of independent toy fits); `--shard`
+cuts ONE data set N ways (strong scaling) with the 2 P-double all-reduce on NCCL inside every timed step.
 """
 import argparse
+import csv
+import hashlib
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -36,10 +45,6 @@ BYTES_PER_EVENT_DATA = 22 * 8
 BYTES_PER_EVENT_NORM = 23 * 8
 FLOP_PER_EVENT = 730.0
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9   # 148 SMs x 64 DFMA/clk x 2 flop x 1965 MHz
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed `ncu --set full` capture
-# (profiles/): per launch, at the default sizes; None until a capture of the current kernel exists
-TRAFFIC_NCU_BYTES = 2.192250e9 + 3.63e6       # profiles/r01g_ncu_full_stream_fused_cfg3.csv (2M + 10M events)
-TRAFFIC_NCU_BYTES_CFG4 = 2.195064e9 + 9.09e6  # profiles/r01g_ncu_full_delta_cfg4.csv
 # Algorithmic flop per event of the gradient batch of configs[4] in its sparse form: point 0 (730) + 31 slots
 # (Breit-Wigner of point 0 from the saved barrier factors ~20, angular factor ~8, two complex products 12, and the expansion
 # coefficients T2 = 2 sum conj(A(0)) SLOT, n = sum |SLOT|^2: 25) + 100 coupling points (S(0) + Re(coef T2) + |coef|^2 n: 6, guard 1,
@@ -54,6 +59,10 @@ GRAD_FLOP_PER_EVENT = 730.0 + 27 * 34.0
 # ~110) + one real scaling of them per spin (~30) + per coupling slot conj(BW) X into its register pair (4 FMA = 8)
 GRADF_FLOP_PER_EVENT = 730.0 + 140.0 + 27 * 8.0
 
+# `ncu --set full` captures whose DRAM traffic the roofline object quotes: profiles/captures.json lists, per kernel, the CSV
+# (plain `ncu -i <rep> --page raw --csv --metrics ...` output), the sizes it was taken at and the SHA-256 of the kernel's source
+# files at capture time.  `traffic` is null when the sources have changed since (a stale capture is not evidence).
+CAPTURES = os.path.join(ROOT, "profiles", "captures.json")
 
 LASS = False   # --lass: the paper's LASS variant of the model (Eq. 9) instead of kappa(800) + K0*(1430)
 
@@ -71,6 +80,36 @@ def measured_peaks():
         d = json.load(open(p))
         return float(d["hbm_gbs"]), "measured"
     return 6650.0, "fallback"
+
+
+def source_hash(files):
+    h = hashlib.sha256()
+    for f in files:
+        h.update(open(os.path.join(ROOT, f), "rb").read())
+    return h.hexdigest()
+
+
+def traffic_from_profiles(key, n_data, n_norm):
+    """(dram bytes read + written per launch, source) of the committed `ncu --set full` capture of kernel `key`, or (None, why)"""
+    try:
+        cap = json.load(open(CAPTURES))[key]
+    except Exception as e:   # noqa: BLE001
+        return None, f"no capture listed for {key} in profiles/captures.json ({type(e).__name__})"
+    if (cap["n_data"], cap["n_norm"]) != (n_data, n_norm):
+        return None, f"capture {cap['csv']} was taken at {cap['n_data']}/{cap['n_norm']} events"
+    if source_hash(cap["sources"]) != cap["sha256"]:
+        return None, f"kernel sources changed since capture {cap['csv']}"
+    rows = list(csv.reader(open(os.path.join(ROOT, "profiles", cap["csv"]))))
+    hdr, units, data = rows[0], rows[1], [r for r in rows[2:] if r]
+    mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    tot = []
+    for r in data:
+        t = 0.0
+        for name in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            j = hdr.index(name)
+            t += float(r[j]) * mult[units[j]]
+        tot.append(t)
+    return float(np.mean(tot)), f"profiles/{cap['csv']} ({len(tot)} launches, mean)"
 
 
 class ClockSampler:
@@ -103,28 +142,31 @@ class ClockSampler:
                 self.rows.append((time.perf_counter(), sm, rs, pw))
             except Exception:   # noqa: BLE001
                 pass
-            time.sleep(0.002)
+            time.sleep(0.0005)
 
-    def stop(self, t0=None, t1=None):
+    def window(self, t0, t1):
+        """clocks over [t0, t1] of the perf_counter clock (the sampler keeps running)"""
         if not getattr(self, "nv", None):
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable: " + getattr(self, "err", "")]}
-        self.stop_flag = True
-        self.thread.join(timeout=2)
         nv = self.nv
-        rows = [r for r in self.rows if (t0 is None or r[0] >= t0) and (t1 is None or r[0] <= t1)] or self.rows[-3:]
+        rows = [r for r in list(self.rows) if t0 <= r[0] <= t1] or list(self.rows)[-3:]
         names = {"hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown, "hw_thermal_slowdown": nv.nvmlClocksEventReasonHwThermalSlowdown,
                  "sw_thermal_slowdown": nv.nvmlClocksEventReasonSwThermalSlowdown, "sw_power_cap": nv.nvmlClocksEventReasonSwPowerCap}
         reasons = sorted(k for k, bit in names.items() if any(r[2] & bit for r in rows))
         return {"sm_mhz": float(np.median([r[1] for r in rows])) if rows else None, "sm_max_mhz": float(self.smax), "reasons": reasons,
                 "power_w_max": max(r[3] for r in rows) if rows else None, "samples": len(rows)}
 
+    def stop(self):
+        self.stop_flag = True
+        if self.thread:
+            self.thread.join(timeout=2)
 
-def build_workload(args, device):
-    """events on the device, model with data + norm loaded.  Data events: accept-reject driven by the product's
-    own amp_eval_events (toy generation with the fitter itself)."""
+
+def generate_events(args, device):
+    """seeded synthetic events of the workload on the HOST.  Data events: accept-reject driven by the product's own
+    amp_eval_events (toy generation with the fitter itself)."""
     import torch
     from paper_2007_14931_b200 import binding as B
-
     cfg = args.cfg
     res, c = model_def(cfg)
     dev = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=device)
@@ -139,9 +181,17 @@ def build_workload(args, device):
     x, eff = W.data_events(cfg, density, n=args.n_data)
     gen.close()
     xn, wn = W.norm_events(cfg, args.n_norm)
-    t_gen = time.time() - t0
+    return x, eff, xn, wn, time.time() - t0
+
+
+def build_workload(args, device):
+    """events on the device, model with data + norm loaded; the cold start (pinned host events -> device -> kinematics cache ->
+    first NLL) is timed once by the wall clock"""
+    import torch
+    from paper_2007_14931_b200 import binding as B
+    res, c = model_def(args.cfg)
+    x, eff, xn, wn, t_gen = generate_events(args, device)
     model = B.Model(W.DECAY, res)
-    # cold start, once: the events as HOST buffers (pinned) -> device -> kinematics cache -> first NLL, by the wall clock
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).pin_memory()
     h_x, h_e, h_xn, h_wn = pin(x), pin(eff), pin(xn), pin(wn)
     torch.cuda.synchronize()
@@ -152,7 +202,7 @@ def build_workload(args, device):
     model.load_events(d_x, d_e)
     model.load_norm(d_xn, d_wn)
     e1.record()
-    cs, mws = step_params(cfg, c, 0)
+    cs, mws = step_params(args.cfg, c, 0)
     model.set_params(cs, mws)
     model.nll()
     torch.cuda.synchronize()
@@ -180,6 +230,135 @@ def step_params(cfg, c, step):
     return cc[None], mw[None]
 
 
+def timed_steps(step_fn, steps, warmup, world, device, sampler=None):
+    """`warmup` untimed steps, then EXACTLY `steps` timed ones between a barrier + synchronize on both sides: total device
+    time from CUDA events on the launching stream (max over ranks), per-step device and wall times."""
+    import torch
+    import torch.distributed as dist
+    for s in range(warmup):
+        step_fn(s)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    walls, last = [], None
+    t_wall0 = time.perf_counter()
+    ev[0].record()
+    for k in range(steps):
+        t0 = time.perf_counter()
+        last = step_fn(warmup + k)      # nothing else in the timed region: amp_set_params + amp_nll through the C ABI
+        walls.append(time.perf_counter() - t0)
+        ev[k + 1].record()
+    torch.cuda.synchronize()
+    t_wall = time.perf_counter() - t_wall0
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.window(t_wall0, t_wall0 + t_wall) if sampler is not None else None
+    dev_ms = ev[0].elapsed_time(ev[steps])
+    per_step = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
+    if world > 1:
+        t = torch.tensor([dev_ms, t_wall * 1e3], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dev_ms, t_wall = float(t[0]), float(t[1]) / 1e3
+    return {"dev_ms": dev_ms, "wall_s": t_wall, "per_step_ms": per_step, "per_step_wall_ms": [w * 1e3 for w in walls], "last": last, "clocks": clocks}
+
+
+def roofline(model, args, cfg, n_data, n_norm, hbm_peak, peak_kind):
+    """the roofline object of the dominant kernel of the steps just timed (kernel durations: the library's CUDA event pairs)"""
+    st = model.last_call_stats()
+    path = st["norm_path"]
+    if path in (4, 5, 7, 8):
+        t_k = [float(v) for v in model.recent_launch_ms(min(args.steps, 256))]
+        phase = {"lineshape": 0.0, "data": float(np.mean(t_k)), "norm": 0.0}
+    else:
+        tm = model.last_call_timing()
+        t_k = [tm["data_ms"]]
+        phase = {"lineshape": tm["lineshape_ms"], "data": tm["data_ms"], "norm": tm["norm_ms"]}
+    k_ms, k_med = float(np.mean(t_k)), float(np.median(t_k))
+    nbytes = BYTES_PER_EVENT_DATA * n_data + BYTES_PER_EVENT_NORM * n_norm
+    if cfg == 4 and path == 5:
+        # gradient batch: one fused k_delta launch per step, bound by the plain FP64 ALUs (DESIGN.md 5.6 / 6)
+        flop = DELTA_FLOP_PER_EVENT * n_data + DELTA_FLOP_PER_NORM_EVENT * n_norm
+        ach = flop / (k_ms * 1e-3) / 1e12
+        traffic, tsrc = traffic_from_profiles("k_delta_cfg4", n_data, n_norm)
+        roof = {"bound": "alu", "kernel": "k_delta (gradient batch: point 0 + 120 sparse points, data then norm tiles, one launch)",
+                "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12,
+                "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md 6; the DFMA probe below measures it)", "unit": "TFLOP/s",
+                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": traffic, "traffic_source": tsrc, "kernel_ms": k_ms, "kernel_ms_median": k_med,
+                "flop_per_event": [DELTA_FLOP_PER_EVENT, DELTA_FLOP_PER_NORM_EVENT], "flop_per_launch": flop,
+                "hbm_frac": nbytes / (k_ms * 1e-3) / 1e9 / hbm_peak}
+    elif path in (7, 8):
+        # --grad: NLL and analytic gradient in one k_gradf (the paper's resonance lists) or k_grad launch per step; plain FP64 ALUs
+        fpe = GRADF_FLOP_PER_EVENT if path == 8 else GRAD_FLOP_PER_EVENT
+        flop = fpe * (n_data + n_norm)
+        ach = flop / (k_ms * 1e-3) / 1e12
+        traffic, tsrc = traffic_from_profiles("k_gradf_cfg3" if path == 8 else "k_grad_cfg3", n_data, n_norm)
+        roof = {"bound": "alu", "kernel": ("k_gradf (shape-specialised, gradient components in registers" if path == 8 else "k_grad (generic") +
+                ": NLL + dNLL/dH_k for all K = 27 couplings, data then norm tiles, one launch)",
+                "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12, "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz", "unit": "TFLOP/s",
+                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": traffic, "traffic_source": tsrc, "kernel_ms": k_ms, "kernel_ms_median": k_med,
+                "flop_per_event": fpe, "hbm_frac": nbytes / (k_ms * 1e-3) / 1e9 / hbm_peak}
+    elif cfg == 4:
+        # dense form (--dense): k_batch (data, DMMA contraction) + k_herk (normalisation matrix, DMMA) + k_lineshape
+        tm = model.last_call_timing()
+        flop = 2 * 27 * 8 * 121 * n_data     # two helicities x 27 complex multiply-adds x 121 points per data event
+        ach = flop / (tm["data_ms"] * 1e-3) / 1e12
+        roof = {"bound": "tensor", "kernel": "k_batch<14, MODE_DATA> (dense FP64 DMMA contraction points x events, mma.sync.m8n8k4.f64)",
+                "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12, "peak_source": "FP64 tensor peak = FP64 FMA peak on B200, 148 x 64 x 2 x 1.965 GHz "
+                "(the DMMA probe below measures it)", "unit": "TFLOP/s", "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": None,
+                "kernel_ms": tm["data_ms"], "flop_per_launch": flop, "norm_matrix_ms": tm["norm_ms"], "lineshape_ms": tm["lineshape_ms"]}
+    elif path == 4:
+        # one fused launch per step: lineshapes + combine + both reductions over the data tiles then the norm tiles
+        ach = nbytes / (k_ms * 1e-3) / 1e9
+        traffic, tsrc = traffic_from_profiles("k_stream_fused_cfg3", n_data, n_norm)
+        roof = {"bound": "hbm", "kernel": "k_stream<MODE_FUSED> (the whole step: lineshapes + combine + -log L / normalisation reductions, data then norm tiles)",
+                "achieved": ach, "peak": hbm_peak, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})", "unit": "GB/s",
+                "frac": ach / hbm_peak, "traffic": traffic, "traffic_source": tsrc,
+                "alu_frac_nominal": FLOP_PER_EVENT * (n_data + n_norm) / (k_ms * 1e-3) / FP64_PEAK_NOMINAL,
+                "kernel_ms": k_ms, "kernel_ms_median": k_med, "bytes_per_launch": nbytes, "bytes_per_event": [BYTES_PER_EVENT_DATA, BYTES_PER_EVENT_NORM],
+                "flop_per_event": FLOP_PER_EVENT}
+    else:
+        norm_ms = phase["norm"]
+        ach = BYTES_PER_EVENT_NORM * n_norm / (norm_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "k_stream<MODE_NORM> (fused lineshape + combine + reduce over the norm sample)",
+                "achieved": ach, "peak": hbm_peak, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})", "unit": "GB/s",
+                "frac": ach / hbm_peak, "traffic": None,
+                "alu_frac_nominal": FLOP_PER_EVENT * n_norm / (norm_ms * 1e-3) / FP64_PEAK_NOMINAL,
+                "kernel_ms": norm_ms, "bytes_per_event": BYTES_PER_EVENT_NORM, "flop_per_event": FLOP_PER_EVENT}
+    return roof, phase, st
+
+
+def measure(model, args, cfg, c, steps, warmup, world, device, sampler, n_data, n_norm, hbm):
+    """time `steps` steps of configuration `cfg` on the loaded model -> the fields of a bench line"""
+    P = 121 if cfg == 4 else 1
+    params = [step_params(cfg, c, s) for s in range(warmup + steps)]
+
+    def one_step(s):
+        cs, mws = params[s]
+        model.set_params(cs, mws)
+        if args.grad:
+            return np.array([model.nll_grad()[0]])   # NLL + its analytic gradient in all K couplings, one launch
+        return model.nll()
+
+    t = timed_steps(one_step, steps, warmup, world, device, sampler)
+    roof, phase, st = roofline(model, args, cfg, n_data, n_norm, *hbm)
+    evals = P * steps * world          # replicas: every rank evaluates its own data set (DESIGN.md "Multi-GPU")
+    h2d = 8 * (P * model.K * 2 + P * model.R * 2)
+    return {"value": evals / (t["dev_ms"] * 1e-3), "ms_per_step": t["dev_ms"] / steps, "ms_per_step_median": float(np.median(t["per_step_ms"])),
+            "steps": steps, "P": P,
+            "e2e": {"value": evals / t["wall_s"], "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(8 * P),
+                    "ms_per_step_median": float(np.median(t["per_step_wall_ms"]))},
+            "gpu_launches": int(st["launches"] * steps), "phase_ms": phase, "roofline": roof, "clocks": t["clocks"],
+            "nll_last": [float(v) for v in np.atleast_1d(t["last"])[:3]]}
+
+
+def workload_text(cfg, n_data, n_norm, P, grad=False):
+    return (("LASS variant (Eq. 9: LASS S-wave + 8 K* + Z, R=10, K=26) of " if LASS else "") +
+            f"configs[{cfg}]: full K*+Z model (R=11, K=27), {n_data} data / {n_norm} norm events per GPU, P={P}, " +
+            ("all lineshapes floating" if cfg == 3 else "gradient batch of a fit step: 60 free parameters (46 K* moduli/phases, 4 Z, Z mass/width, 4 K* masses/widths) x +-h around a moving central point") +
+            (", each step returns the NLL AND its analytic gradient in the 27 couplings" if grad else ""))
+
+
 def run_own(args):
     import torch
     import torch.distributed as dist
@@ -193,143 +372,65 @@ def run_own(args):
         dist.init_process_group("nccl", device_id=device)
     from paper_2007_14931_b200 import binding as B
 
+    if args.shard:
+        return run_shard(args, world, rank, device)
     model, c, info = build_workload(args, device)
-    P = 121 if args.cfg == 4 else 1
-    params = [step_params(args.cfg, c, s) for s in range(args.warmup + args.steps)]
-    h2d = sum(a.nbytes for a in (np.zeros((P, model.K, 2)), np.zeros((P, model.R, 2))))
-    d2h = 8 * P
-
     if args.dense:
         model.set_batch_mode(2)   # configs[4] as the dense DMMA contraction + extended-basis normalisation matrix
-
-    def one_step(s):
-        cs, mws = params[s]
-        model.set_params(cs, mws)
-        if args.grad:
-            return np.array([model.nll_grad()[0]])   # NLL + its analytic gradient in all K couplings, one launch
-        return model.nll()
-
-    for s in range(args.warmup):
-        one_step(s)
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-        time.sleep(0.02)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    nll_last = None
-    t_wall0 = time.perf_counter()
-    ev0.record()
-    for s in range(args.warmup, args.warmup + args.steps):
-        nll_last = one_step(s)          # nothing else in the timed region: amp_set_params + amp_nll through the C ABI
-    ev1.record()
-    torch.cuda.synchronize()
-    t_wall = time.perf_counter() - t_wall0
-    if world > 1:
-        dist.barrier()
-    clocks = sampler.stop(t_wall0, t_wall0 + t_wall) if rank == 0 else None
-    dev_ms = ev0.elapsed_time(ev1)
-    # per-step launch counts, path and kernel times, read AFTER the timed region: every step of a run takes the same path;
-    # the kernel times come from the library's ring of CUDA event pairs recorded around each launch on its stream
-    st = model.last_call_stats()
-    launches, paths = st["launches"] * args.steps, {st["norm_path"]}
-    if st["norm_path"] in (4, 5, 7, 8):
-        ring = model.recent_launch_ms(min(args.steps, 256))
-        t_data, t_norm, t_line = [float(v) for v in ring], [0.0], [0.0]
-    else:
-        tm = model.last_call_timing()
-        t_data, t_norm, t_line = [tm["data_ms"]], [tm["norm_ms"]], [tm["lineshape_ms"]]
-    if world > 1:
-        t = torch.tensor([dev_ms, t_wall * 1e3], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dev_ms, t_wall = float(t[0]), float(t[1]) / 1e3
+        time.sleep(0.01)
+    hbm = measured_peaks()
+    main = measure(model, args, args.cfg, c, args.steps, args.warmup, world, device, sampler if rank == 0 else None, args.n_data, args.n_norm, hbm)
+    # the default run: configs[4] (P = 121) on the same loaded events, in the same line
+    cfg4 = None
+    if args.cfg == 3 and not (args.grad or args.lass or args.dense or args.no_cfg4):
+        steps4 = max(20, min(args.steps, 50))
+        cfg4 = measure(model, args, 4, W.couplings(4), steps4, 3, world, device, sampler if rank == 0 else None, args.n_data, args.n_norm, hbm)
+    sweep = None
+    if args.sweep and rank == 0:
+        sweep = run_sweep(args, device, sampler, hbm)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    evals = P * args.steps * world          # replicas: every rank evaluates its own data set
-    value = evals / (dev_ms * 1e-3)
-    e2e = evals / t_wall
-    hbm_peak, peak_kind = measured_peaks()
-    norm_ms = float(np.mean(t_norm))
-    if args.cfg == 4 and paths == {5}:
-        # gradient batch: one fused k_delta launch per step, bound by the plain FP64 ALUs (DESIGN.md 5.6 / 6)
-        k_ms = float(np.mean(t_data))
-        flop = DELTA_FLOP_PER_EVENT * args.n_data + DELTA_FLOP_PER_NORM_EVENT * args.n_norm
-        ach = flop / (k_ms * 1e-3) / 1e12
-        roof = {"bound": "alu", "kernel": "k_delta (gradient batch: point 0 + 120 sparse points, data then norm tiles, one launch)",
-                "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12,
-                "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md 6; the DFMA probe below measures it)", "unit": "TFLOP/s",
-                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": TRAFFIC_NCU_BYTES_CFG4 if (args.n_data, args.n_norm) == (2_000_000, 10_000_000) else None, "kernel_ms": k_ms,
-                "flop_per_event": [DELTA_FLOP_PER_EVENT, DELTA_FLOP_PER_NORM_EVENT], "flop_per_launch": flop,
-                "hbm_frac": (BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}
-    elif paths == {7} or paths == {8}:
-        # --grad: NLL and analytic gradient in one k_gradf (the paper's resonance lists) or k_grad launch per step; plain FP64 ALUs
-        k_ms = float(np.mean(t_data))
-        fpe = GRADF_FLOP_PER_EVENT if paths == {8} else GRAD_FLOP_PER_EVENT
-        flop = fpe * (args.n_data + args.n_norm)
-        ach = flop / (k_ms * 1e-3) / 1e12
-        roof = {"bound": "alu", "kernel": ("k_gradf (shape-specialised, gradient components in registers" if paths == {8} else "k_grad (generic") +
-                ": NLL + dNLL/dH_k for all K = 27 couplings, data then norm tiles, one launch)",
-                "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12, "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz", "unit": "TFLOP/s",
-                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": None, "kernel_ms": k_ms, "flop_per_event": fpe,
-                "hbm_frac": (BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}
-    elif args.cfg == 4:
-        # dense form (--dense): k_batch (data, DMMA contraction) + k_herk (normalisation matrix, DMMA) + k_lineshape
-        tm = model.last_call_timing()
-        flop = 2 * 27 * 8 * 121 * args.n_data     # two helicities x 27 complex multiply-adds x 121 points per data event
-        ach = flop / (tm["data_ms"] * 1e-3) / 1e12
-        roof = {"bound": "tensor", "kernel": "k_batch<14, MODE_DATA> (dense FP64 DMMA contraction points x events, mma.sync.m8n8k4.f64)",
-                "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12, "peak_source": "FP64 tensor peak = FP64 FMA peak on B200, 148 x 64 x 2 x 1.965 GHz "
-                "(the DMMA probe below measures it)", "unit": "TFLOP/s", "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": None,
-                "kernel_ms": tm["data_ms"], "flop_per_launch": flop, "norm_matrix_ms": tm["norm_ms"], "lineshape_ms": tm["lineshape_ms"]}
-    elif paths == {4}:
-        # one fused launch per step: lineshapes + combine + both reductions over the data tiles then the norm tiles
-        k_ms = float(np.mean(t_data))
-        nbytes = BYTES_PER_EVENT_DATA * args.n_data + BYTES_PER_EVENT_NORM * args.n_norm
-        ach = nbytes / (k_ms * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": "k_stream<MODE_FUSED> (the whole step: lineshapes + combine + -log L / normalisation reductions, data then norm tiles)",
-                "achieved": ach, "peak": hbm_peak, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})", "unit": "GB/s",
-                "frac": ach / hbm_peak, "traffic": TRAFFIC_NCU_BYTES if (args.n_data, args.n_norm) == (2_000_000, 10_000_000) else None,
-                "alu_frac_nominal": FLOP_PER_EVENT * (args.n_data + args.n_norm) / (k_ms * 1e-3) / FP64_PEAK_NOMINAL,
-                "kernel_ms": k_ms, "bytes_per_launch": nbytes, "bytes_per_event": [BYTES_PER_EVENT_DATA, BYTES_PER_EVENT_NORM],
-                "flop_per_event": FLOP_PER_EVENT}
-    else:
-        ach = BYTES_PER_EVENT_NORM * args.n_norm / (norm_ms * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": "k_stream<MODE_NORM> (fused lineshape + combine + reduce over the norm sample)",
-                "achieved": ach, "peak": hbm_peak, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})", "unit": "GB/s",
-                "frac": ach / hbm_peak, "traffic": None,
-                "alu_frac_nominal": FLOP_PER_EVENT * args.n_norm / (norm_ms * 1e-3) / FP64_PEAK_NOMINAL,
-                "kernel_ms": norm_ms, "bytes_per_event": BYTES_PER_EVENT_NORM, "flop_per_event": FLOP_PER_EVENT}
+    sampler.stop()
     fp64 = {"dfma_tflops_measured": B.probe_fp64(0, 4000) / 1e12, "dmma_tflops_measured": B.probe_fp64(1, 4000) / 1e12,
             "nominal_tflops": FP64_PEAK_NOMINAL / 1e12}
+    roof = main["roofline"]
     if roof["bound"] == "hbm":
         # the streaming kernels' own TMA tile pipeline with the model arithmetic taken out (amp_probe_hbm_read, after the timed
         # region): how fast this access pattern reads HBM on this box, next to the copy figure `peak` is
         roof["read_probe_gbs"] = B.probe_hbm_read(BYTES_PER_EVENT_NORM * 12_000_000)
         roof["frac_of_read_probe"] = roof["achieved"] / roof["read_probe_gbs"]
-    line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": ("LASS variant (Eq. 9: LASS S-wave + 8 K* + Z, R=10, K=26) of " if LASS else "") + f"configs[{args.cfg}]: full K*+Z model (R=11, K=27), {args.n_data} data / {args.n_norm} norm events per GPU, "
-                               f"P={P}, all lineshapes floating" + (", each step returns the NLL AND its analytic gradient in the 27 couplings" if args.grad else ""), "n_data": args.n_data, "n_norm": args.n_norm, "P": P,
-                   "l2": "inputs (2.1 GB kinematics cache) larger than L2; no flush needed", "parallelism": f"replicas x{world}"},
-        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                "note": "host wall clock around amp_set_params (host parameter arrays in) + amp_nll (host NLL out) per step; the events are "
+    P = main["P"]
+    e2e = dict(main["e2e"])
+    e2e.update({"note": "host wall clock around amp_set_params (host parameter arrays in) + amp_nll (host NLL out) per step; the events are "
                         "resident as in a fit (PAPER.md:45) - the one-off upload of the events from host buffers is setup.cold_start",
                 # the other reading of "host buffers": EVERY evaluation uploads the events again (pinned host -> device -> kinematics
                 # cache -> parameters -> NLL): P evaluations per cold start
                 "value_if_events_uploaded_every_step": P * world / (info["cold_start"]["ms"] * 1e-3),
-                "h2d_bytes_per_step_if_events_uploaded": int(info["cold_start"]["h2d_bytes"] + h2d)},
-        "gpu_launches": int(launches),
-        "event_evals_per_s": value * (args.n_data + args.n_norm),
-        "phase_ms": {"lineshape": float(np.mean(t_line)), "data": float(np.mean(t_data)), "norm": norm_ms},
-        "roofline": roof, "fp64_probe": fp64, "clocks": clocks,
-        "setup": info, "nll_last": [float(v) for v in np.atleast_1d(nll_last)[:3]],
+                "h2d_bytes_per_step_if_events_uploaded": int(info["cold_start"]["h2d_bytes"] + e2e["h2d_bytes_per_step"])})
+    line = {
+        "metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": main["ms_per_step"], "ms_per_step_median": main["ms_per_step_median"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_text(args.cfg, args.n_data, args.n_norm, P, args.grad), "n_data": args.n_data, "n_norm": args.n_norm, "P": P,
+                   "l2": "inputs (2.1 GB kinematics cache) larger than L2; no flush needed", "parallelism": f"replicas x{world}"},
+        "e2e": e2e, "gpu_launches": main["gpu_launches"],
+        "event_evals_per_s": main["value"] * (args.n_data + args.n_norm),
+        "phase_ms": main["phase_ms"], "roofline": roof, "fp64_probe": fp64, "clocks": main["clocks"],
+        "setup": info, "nll_last": main["nll_last"],
     }
+    if cfg4 is not None:
+        line["cfg4"] = {"metric": METRIC, "unit": UNIT, "value": cfg4["value"], "ms_per_step": cfg4["ms_per_step"], "ms_per_step_median": cfg4["ms_per_step_median"],
+                        "steps": cfg4["steps"], "warmup": 3, "workload": workload_text(4, args.n_data, args.n_norm, 121),
+                        "e2e": cfg4["e2e"], "gpu_launches": cfg4["gpu_launches"], "roofline": cfg4["roofline"], "clocks": cfg4["clocks"],
+                        "nll_last": cfg4["nll_last"]}
+        line["gpu_launches"] += cfg4["gpu_launches"]
+    if sweep is not None:
+        line["sweep"] = sweep
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args)
     print(json.dumps(line))
@@ -337,11 +438,93 @@ def run_own(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args, device, sampler, hbm):
+    """the six points of BASELINE.json configs[3]: data in {1M, 2M, 8M} x normalisation in {2M, 10M}, each its own loaded model"""
+    out = []
+    for n_norm in (2_000_000, 10_000_000):
+        for n_data in (1_000_000, 2_000_000, 8_000_000):
+            a = argparse.Namespace(**vars(args))
+            a.n_data, a.n_norm = n_data, n_norm
+            model, c, _info = build_workload(a, device)
+            m = measure(model, a, 3, c, a.steps, a.warmup, 1, device, sampler, n_data, n_norm, hbm)
+            out.append({"n_data": n_data, "n_norm": n_norm, "value": m["value"], "ms_per_step": m["ms_per_step"], "ms_per_step_median": m["ms_per_step_median"],
+                        "kernel_ms": m["roofline"]["kernel_ms"], "hbm_gbs": m["roofline"]["achieved"], "frac": m["roofline"]["frac"],
+                        "e2e_value": m["e2e"]["value"], "nll_last": m["nll_last"][0]})
+            model.close()
+    return out
+
+
+def run_shard(args, world, rank, device):
+    """Strong scaling: ONE data set of n_data / n_norm events cut into `world` contiguous shards (ShardedModel); every timed step
+    is amp_set_params + amp_nll_terms on each rank's shard and ONE all-reduce of 2 P doubles on the process group (NCCL over
+    NVLink 5 / NVSwitch), after which every rank holds the NLL of the whole sample."""
+    import torch
+    import torch.distributed as dist
+    from paper_2007_14931_b200 import sharded as S
+    single = world == 1 and not dist.is_initialized()
+    if single:   # one GPU: a one-rank NCCL group, so the same code path (collective included) runs
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", str(port))
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=device)
+    cfg = args.cfg
+    res, c = model_def(cfg)
+    # every rank generates the same seeded events on the host and keeps its own slice (no data-path exchange at load)
+    x, eff, xn, wn, t_gen = generate_events(args, device)
+    sm = S.ShardedModel(W.DECAY, res)
+    sm.load_events(x, eff)
+    sm.load_norm(xn, wn)
+    P = 121 if cfg == 4 else 1
+    params = [step_params(cfg, c, s) for s in range(args.warmup + args.steps)]
+
+    def one_step(s):
+        cs, mws = params[s]
+        sm.set_params(cs, mws)
+        return sm.nll()
+
+    sampler = ClockSampler(device.index)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.01)
+    t = timed_steps(one_step, args.steps, args.warmup, world, device, sampler if rank == 0 else None)
+    st = sm.model.last_call_stats()
+    k_ms = [float(v) for v in sm.model.recent_launch_ms(min(args.steps, 256))] if st["norm_path"] in (4, 5) else [float("nan")]
+    if rank == 0:
+        sampler.stop()
+        hbm_peak, peak_kind = measured_peaks()
+        lo, hi = S.shard_bounds(args.n_data, 0, world)
+        ln, hn = S.shard_bounds(args.n_norm, 0, world)
+        nbytes = BYTES_PER_EVENT_DATA * (hi - lo) + BYTES_PER_EVENT_NORM * (hn - ln)
+        evals = P * args.steps                       # strong scaling: the ranks share ONE evaluation per point
+        kern = float(np.mean(k_ms))
+        line = {"metric": METRIC, "value": evals / (t["dev_ms"] * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": t["dev_ms"] / args.steps, "ms_per_step_median": float(np.median(t["per_step_ms"])), "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": workload_text(cfg, args.n_data, args.n_norm, P).replace(" per GPU", " in total"), "n_data": args.n_data, "n_norm": args.n_norm, "P": P,
+                           "l2": "inputs larger than L2 per rank down to 16 shards; no flush", "parallelism": f"event shards x{world}",
+                           "collective": "one all-reduce (sum) of 2 P float64 per step on the NCCL process group + one of 4 constants at load"},
+                "e2e": {"value": evals / t["wall_s"], "unit": UNIT, "h2d_bytes_per_step": int(8 * (P * sm.K * 2 + P * sm.R * 2) + 16 * P), "d2h_bytes_per_step": int(16 * P + 16 * P),
+                        "ms_per_step_median": float(np.median(t["per_step_wall_ms"])),
+                        "note": "per step and rank: parameters host -> library, the two per-shard sums library -> host -> device tensor, NCCL all-reduce, result -> host"},
+                "gpu_launches": int(st["launches"] * args.steps) * world,
+                "roofline": {"bound": "hbm", "kernel": "k_stream<MODE_FUSED> on one rank's shard", "achieved": nbytes / (kern * 1e-3) / 1e9, "peak": hbm_peak,
+                             "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})", "unit": "GB/s", "frac": nbytes / (kern * 1e-3) / 1e9 / hbm_peak,
+                             "traffic": None, "kernel_ms": kern, "kernel_ms_median": float(np.median(k_ms)),
+                             "exchange_ms_per_step": t["dev_ms"] / args.steps - kern},
+                "clocks": t["clocks"], "setup": {"gen_s": t_gen}, "nll_last": [float(v) for v in np.atleast_1d(t["last"])[:3]]}
+        print(json.dumps(line))
+    if dist.is_initialized():
+        dist.destroy_process_group()
+
+
 def cpu_baseline(args, target_evals=None):
     """The oracle, as it stands, timed on this box's host cores on a bounded sample of the same workload (about 10-30 s
     of CPU work): same model and call pattern, data and norm sizes scaled down by one factor (1 = the full workload) and
     the evaluation repeated so that about `target_evals` event-evaluations are timed; data events drawn by
-    oracle-driven accept-reject (no oracle input comes from the CUDA path)."""
+    oracle-driven accept-reject (no oracle input comes from the CUDA path).  `value_1thread`: the same call with ONE thread on
+    1/8 of that sample's events, scaled linearly to the full sizes."""
     from oracle import oracle as O
     cfg = args.cfg
     P = 121 if cfg == 4 else 1
@@ -363,46 +546,68 @@ def cpu_baseline(args, target_evals=None):
         Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
         dt += time.perf_counter() - t0
     full = dt / reps * total / (n + m)            # time of one full-size call (scaled linearly if the sample is smaller)
-    return {"value": P / full, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+    cores = O.num_threads()
+    n1, m1 = max(n // 8, 500), max(m // 8, 2000)
+    O.set_num_threads(1)
+    cs, mws = step_params(cfg, c, 0)
+    t0 = time.perf_counter()
+    Mo.nll(cs, x[:, :n1], eff[:n1], xn[:, :m1], wn[:m1], mass_width=mws)
+    dt1 = time.perf_counter() - t0
+    O.set_num_threads(cores)
+    full1 = dt1 * total / (n1 + m1)
+    return {"value": P / full, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{reps} x ({n} data + {m} norm events, same model, P={P}), {dt:.2f} s measured"
                       + ("" if n + m == total else f", scaled linearly to {args.n_data}+{args.n_norm}"),
-            "event_evals_per_s": P * (n + m) * reps / dt}
+            "event_evals_per_s": P * (n + m) * reps / dt,
+            "value_1thread": P / full1, "sample_1thread": f"1 x ({n1} data + {m1} norm events), 1 thread, {dt1:.2f} s measured, scaled linearly to {args.n_data}+{args.n_norm}"}
 
 
 def run_reference(args):
+    """The reference arm = the oracle on the host cores.  Every step is the FULL workload (same config as the own arm) unless
+    the first warm-up step shows that steps + warm-up would not end within ~5 minutes; then the sample is cut by a stated factor."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from oracle import oracle as O
     cfg = args.cfg
     P = 121 if cfg == 4 else 1
-    # bounded sample per step so that steps+warmup finish in a few minutes
-    per_step = max(30_000_000 // (P * max(args.steps + args.warmup, 1)), 4000)
-    per_step = min(per_step, args.n_data + args.n_norm)
-    n = max(int(per_step * args.n_data / (args.n_data + args.n_norm)), 500)
-    m = max(per_step - n, 2000)
     res, c = model_def(cfg)
     Mo = O.Model(W.DECAY, res)
+    n, m = args.n_data, args.n_norm
+    t0 = time.perf_counter()
     xn, wn = W.norm_events(cfg, m)
     x, eff = W.data_events(cfg, lambda xx, ee: Mo.eval_events(c, xx, ee), n=n)
+    t_gen = time.perf_counter() - t0
+    # probe: one evaluation of 1/16 of the events decides whether the full workload fits the budget
+    cs, mws = step_params(cfg, c, 0)
+    t0 = time.perf_counter()
+    Mo.nll(cs, x[:, :n // 16], eff[:n // 16], xn[:, :m // 16], wn[:m // 16], mass_width=mws)
+    est_full = (time.perf_counter() - t0) * 16
+    budget = 300.0
+    cut = 1
+    while est_full / cut * (args.steps + args.warmup) > budget and cut < 64:
+        cut *= 2
+    ns, ms = n // cut, m // cut
     times = []
     for s in range(args.warmup + args.steps):
         cs, mws = step_params(cfg, c, s)
         t0 = time.perf_counter()
-        Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+        Mo.nll(cs, x[:, :ns], eff[:ns], xn[:, :ms], wn[:ms], mass_width=mws)
         if s >= args.warmup:
             times.append(time.perf_counter() - t0)
     dt = float(np.sum(times))
-    scale = (args.n_data + args.n_norm) / (n + m)
+    scale = (n + m) / (ns + ms)
     value = P * args.steps / (dt * scale)
-    sample = f"{n} data + {m} norm events per step (same model, P={P}), scaled linearly to {args.n_data}+{args.n_norm}"
+    sample = (f"every step the full workload: {n} data + {m} norm events (same model, P={P})" if cut == 1 else
+              f"{ns} data + {ms} norm events per step (same model, P={P}; 1/{cut} of the workload: the full one would not end within {budget:.0f} s on "
+              f"{O.num_threads()} cores), scaled linearly to {n}+{m}")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * scale / args.steps * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"configs[{cfg}]: full K*+Z model (R=11, K=27), {args.n_data} data / {args.n_norm} norm events, P={P}, "
-                                   "all lineshapes floating", "n_data": args.n_data, "n_norm": args.n_norm, "P": P},
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * scale / args.steps * 1e3, "ms_per_step_median": float(np.median(times)) * scale * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_text(cfg, n, m, P), "n_data": n, "n_norm": m, "P": P, "full_workload_every_step": cut == 1},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
-            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0,
+            "setup": {"gen_s": t_gen}}
     print(json.dumps(line))
 
 
@@ -446,16 +651,29 @@ def run_pseudo(args):
                                              "generate (amp_generate) + BFGS fit on amp_nll_grad + Hessian errors", "models": per_model}}))
 
 
+def spawn_ranks(args):
+    """`--gpus N` without a launcher: start the N ranks the way the driver does (torch.distributed.run, 127.0.0.1)"""
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="own", choices=["own", "reference"])
-    ap.add_argument("--cfg", type=int, default=3, choices=[3, 4], help="3: P=1 all lineshapes floating (headline); 4: P=121 fit-loop pattern")
+    ap.add_argument("--cfg", type=int, default=3, choices=[3, 4], help="3: P=1 all lineshapes floating (headline; the default run adds the cfg 4 timing as \"cfg4\"); 4: P=121 fit-loop pattern only")
     ap.add_argument("--n-data", type=int, default=2_000_000)
     ap.add_argument("--n-norm", type=int, default=10_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cfg4", action="store_true", help="skip the configs[4] timing of the default run")
+    ap.add_argument("--sweep", action="store_true", help="also time the six configs[3] points {1M, 2M, 8M} data x {2M, 10M} normalisation events (\"sweep\" in the line)")
+    ap.add_argument("--shard", action="store_true", help="strong scaling: ONE data set cut over the ranks (ShardedModel), the all-reduce on NCCL inside the timed step")
     ap.add_argument("--dense", action="store_true", help="--cfg 4 through the dense DMMA contraction instead of the gradient-batch kernel")
     ap.add_argument("--grad", action="store_true", help="--cfg 3 steps that also return the analytic gradient in all couplings (amp_nll_grad)")
     ap.add_argument("--lass", action="store_true", help="configs[3] call pattern on the LASS variant of the model (Eqs. 7-9; SURVEY.md 8(f)-1)")
@@ -470,11 +688,15 @@ def main():
     LASS = bool(args.lass)
     if LASS and args.cfg != 3:
         ap.error("--lass goes with --cfg 3")
-    args.warmup = max(args.warmup, 3) if args.impl == "own" else args.warmup
     if args.impl == "reference":
-        run_reference(args)
-    else:
-        run_own(args)
+        return run_reference(args)
+    world = int(os.environ.get("WORLD_SIZE", "0"))
+    if world == 0 and args.gpus > 1:
+        return sys.exit(spawn_ranks(args))
+    if world and world != args.gpus:
+        ap.error(f"--gpus {args.gpus} but the launcher started {world} ranks")
+    args.warmup = max(args.warmup, 3)
+    run_own(args)
 
 
 if __name__ == "__main__":
