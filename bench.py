@@ -53,6 +53,12 @@ DELTA_FLOP_PER_EVENT = 730.0 + 31 * 65.0 + 100 * 8.0 + 20 * 33.0
 # normalisation events: the 100 coupling points cost nothing per point there — three weighted sums per group of four on one slot
 # (25 groups x 3 FMA), the points are formed from them once per launch
 DELTA_FLOP_PER_NORM_EVENT = 730.0 + 31 * 65.0 + 25 * 6.0 + 20 * 33.0
+# The shape-specialised gradient-batch kernel (deltaf.cu), per event: point 0 (730) + the W / Y sums and the per-spin
+# scalings (140 + 50) + the eleven lineshapes evaluated again from the saved barrier factors (11 x 14) + per coupling position in use
+# (25): L = conj(BW) X (6), n (2), data: four points x (3 FMA + the product through the exchange) = 28 + guard 4, normalisation: three
+# sums (3) + per floating lineshape (5): Q (22), G and n_R (44), four points x (BW(p) 12, Delta 4, |Delta|^2 3, x 6, exchange 1)
+DELTAF_FLOP_PER_EVENT = 730.0 + 190.0 + 154.0 + 25 * 40.0 + 5 * 170.0
+DELTAF_FLOP_PER_NORM_EVENT = 730.0 + 190.0 + 154.0 + 25 * 11.0 + 5 * 170.0
 # analytic gradient: the point (730) + per coupling slot: angular factor ~8, T = sum_xi conj(g) A 16, conj(BW) T 8, weight 2
 GRAD_FLOP_PER_EVENT = 730.0 + 27 * 34.0
 # its shape-specialised form (gradf.cu): the point (730) + the three W_lambda and three Y_lambda' (u A, conj(g) A:
@@ -267,7 +273,7 @@ def roofline(model, args, cfg, n_data, n_norm, hbm_peak, peak_kind):
     """the roofline object of the dominant kernel of the steps just timed (kernel durations: the library's CUDA event pairs)"""
     st = model.last_call_stats()
     path = st["norm_path"]
-    if path in (4, 5, 7, 8):
+    if path in (4, 5, 7, 8, 9):
         t_k = [float(v) for v in model.recent_launch_ms(min(args.steps, 256))]
         phase = {"lineshape": 0.0, "data": float(np.mean(t_k)), "norm": 0.0}
     else:
@@ -276,7 +282,19 @@ def roofline(model, args, cfg, n_data, n_norm, hbm_peak, peak_kind):
         phase = {"lineshape": tm["lineshape_ms"], "data": tm["data_ms"], "norm": tm["norm_ms"]}
     k_ms, k_med = float(np.mean(t_k)), float(np.median(t_k))
     nbytes = BYTES_PER_EVENT_DATA * n_data + BYTES_PER_EVENT_NORM * n_norm
-    if cfg == 4 and path == 5:
+    if cfg == 4 and path == 9:
+        # gradient batch of the paper's resonance lists: ONE k_deltaf launch per step, bound by the plain FP64 ALUs
+        flop = DELTAF_FLOP_PER_EVENT * n_data + DELTAF_FLOP_PER_NORM_EVENT * n_norm
+        ach = flop / (k_ms * 1e-3) / 1e12
+        traffic, tsrc = traffic_from_profiles("k_deltaf_cfg4", n_data, n_norm)
+        roof = {"bound": "alu", "kernel": "k_deltaf (shape-specialised gradient batch: point 0 + 100 coupling points + 20 mass/width points, data then norm units, one launch)",
+                "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12,
+                "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md 6; the DFMA probe below measures it)", "unit": "TFLOP/s",
+                "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "traffic": traffic, "traffic_source": tsrc, "kernel_ms": k_ms, "kernel_ms_median": k_med,
+                "flop_per_event": [DELTAF_FLOP_PER_EVENT, DELTAF_FLOP_PER_NORM_EVENT], "flop_per_launch": flop,
+                "flop_note": "algorithmic flop of THIS design; the general kernel (k_delta, --general) needs 4205 / 3555 flop per event for the same batch",
+                "hbm_frac": nbytes / (k_ms * 1e-3) / 1e9 / hbm_peak}
+    elif cfg == 4 and path == 5:
         # gradient batch: one fused k_delta launch per step, bound by the plain FP64 ALUs (DESIGN.md 5.6 / 6)
         flop = DELTA_FLOP_PER_EVENT * n_data + DELTA_FLOP_PER_NORM_EVENT * n_norm
         ach = flop / (k_ms * 1e-3) / 1e12
@@ -377,6 +395,8 @@ def run_own(args):
     model, c, info = build_workload(args, device)
     if args.dense:
         model.set_batch_mode(2)   # configs[4] as the dense DMMA contraction + extended-basis normalisation matrix
+    if args.general:
+        model.set_batch_mode(3)   # configs[4] through the general gradient-batch kernel (k_delta) instead of the shape-specialised one
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -385,7 +405,7 @@ def run_own(args):
     main = measure(model, args, args.cfg, c, args.steps, args.warmup, world, device, sampler if rank == 0 else None, args.n_data, args.n_norm, hbm)
     # the default run: configs[4] (P = 121) on the same loaded events, in the same line
     cfg4 = None
-    if args.cfg == 3 and not (args.grad or args.lass or args.dense or args.no_cfg4):
+    if args.cfg == 3 and not (args.grad or args.lass or args.dense or args.general or args.no_cfg4):
         steps4 = max(20, min(args.steps, 50))
         cfg4 = measure(model, args, 4, W.couplings(4), steps4, 3, world, device, sampler if rank == 0 else None, args.n_data, args.n_norm, hbm)
     sweep = None
@@ -675,6 +695,7 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="also time the six configs[3] points {1M, 2M, 8M} data x {2M, 10M} normalisation events (\"sweep\" in the line)")
     ap.add_argument("--shard", action="store_true", help="strong scaling: ONE data set cut over the ranks (ShardedModel), the all-reduce on NCCL inside the timed step")
     ap.add_argument("--dense", action="store_true", help="--cfg 4 through the dense DMMA contraction instead of the gradient-batch kernel")
+    ap.add_argument("--general", action="store_true", help="configs[4] through the general gradient-batch kernel (k_delta) instead of the shape-specialised k_deltaf")
     ap.add_argument("--grad", action="store_true", help="--cfg 3 steps that also return the analytic gradient in all couplings (amp_nll_grad)")
     ap.add_argument("--lass", action="store_true", help="configs[3] call pattern on the LASS variant of the model (Eqs. 7-9; SURVEY.md 8(f)-1)")
     ap.add_argument("--pseudo", type=int, default=0, metavar="N_EVENTS",

@@ -240,7 +240,12 @@ amp_status amp_set_lineshape_mode(amp_model* m, int mode);
  * launch over data and normalisation events with no lineshape column and no matrix; any other batch with P >= 24, at
  * most 28 couplings and an extended basis that fits in shared memory runs one dense DMMA launch per sample; else as
  * mode 1.  1 = a loop of single-point streaming launches over the stored lineshape columns.  2 = as 0 without the
- * gradient-batch kernel (dense DMMA contraction even for sparse batches).                                        */
+ * gradient-batch kernels (dense DMMA contraction even for sparse batches).  3 = as 0 without the shape-specialised form of the
+ * gradient-batch kernel.  Under 0, a sparse batch of the paper's resonance lists (ten K* with zero to two 1+ Z's, one radius
+ * per spin) in which every point is ONE coupling change (a single slot, or a Z's helicities -1 and +1 moving together, Eq. 11)
+ * or ONE mass / width change, at most four per slot / resonance — MINUIT's gradient step — runs that form: one launch for all
+ * points, exact, S(p) / S(0) formed directly; a step so large that the ratio leaves [0.5, 1.5] at some event repeats the call
+ * through the general kernel.                                                                                       */
 amp_status amp_set_batch_mode(amp_model* m, int mode);
 /* How a P == 1 step with lineshapes in registers and a direct-sum normalisation is launched: 0 = automatic (ONE fused
  * launch: data tiles, then normalisation tiles, the last thread block forms the NLL), 1 = separate data / normalisation /
@@ -254,7 +259,7 @@ amp_status amp_set_grad_mode(amp_model* m, int mode);
 /* Counters of the last amp_nll / amp_norm_integral call: kernels launched, lineshape columns
  * recomputed (data + norm), which normalisation path ran (1 direct streaming sum, 2 matrix, 3 batched DMMA sum,
  * 4 fused single launch, 5 gradient-batch delta kernel, 6 background + purity, 7 analytic gradient, generic kernel,
- * 8 analytic gradient, shape-specialised kernel).                         */
+ * 8 analytic gradient, shape-specialised kernel, 9 gradient batch, shape-specialised kernel).                         */
 amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_recomputed, int* norm_path);
 
 /* Device time [ms] of the phases of the last amp_nll / amp_norm_integral call, from CUDA events recorded on

@@ -344,6 +344,29 @@ cudaError_t launch_delta(const DeltaArgs& d, int grid, cudaStream_t s, bool exac
 int delta_grid(long long n_data, long long n_norm);
 bool delta_fits(int ngrp);
 
+// Gradient batches of the paper's resonance lists, shape-specialised form (deltaf.cu): every point besides point 0 is ONE coupling
+// change (position = a coupling slot, or the tied pair of a Z's helicities +-1) or ONE lineshape change (mass / width of an entry);
+// at most four points per position / entry.  All tables live in kernel parameter space (constant bank operands).
+enum { DELTAF_MAX_POS = 32, DELTAF_MAX_ENT = 12 };
+struct DeltaFArgs {
+    StreamArgs a;                                 // point 0 as the streaming kernel sees it (cache/n: data; cache2/n2: norm)
+    double cq[DELTAF_MAX_POS][4][3];              // coupling points of a position: Re, Im, |.|^2 of (c_k(p) - c_k(0)) kN_R(0)
+    double cmax[DELTAF_MAX_POS][2];               // largest |Re|, |Im| and largest |.|^2 of cq[pos] (the guard on r)
+    double mw[DELTAF_MAX_ENT][4][3];              // lineshape points of an entry: kN(p) / kN(0), kG(p), M2(p)
+    unsigned pos_active, ent_active;              // bit per position / entry with at least one point
+    short val_of_point[AMP_MAX_POINTS];           // point -> value slot 4 quad + j in the kernel's value order (DeltaFLayout); -1: equal to point 0
+    short pos_of_point[AMP_MAX_POINTS];           // point -> its coupling position, -1 for a lineshape point
+    int P;
+    double* partial;                              // [2 + 2 NVAL][stride] per-CTA partials
+    int stride;
+    double* result;                               // [4 P + 1]: NLL[P], I[P], domain flag, sum log S [P], sum w S [P] (as DeltaArgs)
+    int want_nll;
+};
+cudaError_t launch_deltaf(const DeltaFArgs& d, int grid, cudaStream_t s);
+int deltaf_grid(long long n_data, long long n_norm);
+struct DeltaFLayout { int nslot, npos, nent, nquad; int quad_of_pos[DELTAF_MAX_POS], quad_of_ent[DELTAF_MAX_ENT]; };
+bool deltaf_layout(const StreamArgs& a, DeltaFLayout* lay);   // false: not one of the compiled shapes
+
 // Analytic gradient of the NLL in the couplings (grad.cu): one pair of leaves (real, imaginary part) per coupling slot
 enum { GRAD_MAX_PAIRS = 48 };
 struct GradArgs {

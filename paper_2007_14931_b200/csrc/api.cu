@@ -109,6 +109,9 @@ struct amp_model {
     bool use_delta = false;        // P > 1 and the points are sparse changes of point 0: gradient-batch kernel (delta.cu)
     struct DeltaChunk { int p0, np, nsorted; std::vector<DeltaContrib> contrib; std::vector<double> slots; };
     std::vector<DeltaChunk> delta_chunks;     // compiled program of the last amp_set_params (points p0 .. p0 + np - 1 per launch)
+    bool use_deltaf = false;       // ... and every point is ONE coupling or ONE lineshape change of the paper's resonance lists: deltaf.cu
+    DeltaFArgs deltaf{};           // its tables (filled by amp_set_params; pointers and point 0 by evaluate())
+    long long stat_deltaf_guard = 0;   // deltaf calls repeated through delta.cu's exact form (guard on r tripped)
     double* d_bkg = nullptr;       // [data.npad] background density b_i at the data events (Eq. 14), 1 on padding
     double purity = 1.0;
     bool has_bkg = false;
@@ -428,7 +431,7 @@ amp_status amp_set_norm_mode(amp_model* m, int mode) {
 }
 
 amp_status amp_set_batch_mode(amp_model* m, int mode) {
-    if (!m || mode < 0 || mode > 2) return AMP_ERR_INVALID;
+    if (!m || mode < 0 || mode > 3) return AMP_ERR_INVALID;
     m->batch_mode = mode;
     return AMP_OK;
 }
@@ -668,6 +671,92 @@ bool build_delta_plan(amp_model* m) {
     return true;
 }
 
+// The shape-specialised gradient-batch kernel (deltaf.cu): every point 1..P-1 must be ONE coupling change — a single slot, or the
+// helicities -1 and +1 of a Z moving by the same amount (Eq. 11) — or ONE mass / width change of one resonance with its couplings
+// unchanged, at most four points per position / resonance, on one of the compiled model shapes.  Fills m->deltaf's tables.
+bool build_deltaf_plan(amp_model* m) {
+    const int P = m->P, R = m->R, K = m->K;
+    if (P < 2 || !m->norm.loaded) return false;
+    int ent_of_res[AMP_MAX_RESONANCES], grp_of_res[AMP_MAX_RESONANCES];
+    DeltaFArgs& d = m->deltaf;
+    fill_stream_args(m, m->norm, 0, MODE_FUSED, &d.a, ent_of_res, grp_of_res);
+    DeltaFLayout lay;
+    if (!deltaf_layout(d.a, &lay)) return false;
+    const int nslot = lay.nslot, nent = lay.nent;
+    const int n0 = d.a.shape[0];
+    auto base = [&](int t) { return t < n0 ? t : n0 + 3 * (t - n0); };
+    std::memset(d.cq, 0, sizeof(d.cq));
+    std::memset(d.cmax, 0, sizeof(d.cmax));
+    for (auto& e : d.mw) for (auto& q : e) { q[0] = 1.0; q[1] = 1.0; q[2] = 1.0; }
+    d.pos_active = d.ent_active = 0u;
+    for (int p = 0; p < AMP_MAX_POINTS; ++p) d.val_of_point[p] = d.pos_of_point[p] = -1;
+    int used_pos[DELTAF_MAX_POS] = {}, used_ent[DELTAF_MAX_ENT] = {};
+    for (int p = 1; p < P; ++p) {
+        int changed = -1;   // the one resonance that differs from point 0
+        for (int r = 0; r < R; ++r) {
+            bool diff = m->mw[((size_t)p * R + r) * 2] != m->mw[(size_t)r * 2] || m->mw[((size_t)p * R + r) * 2 + 1] != m->mw[(size_t)r * 2 + 1];
+            const int ns = (kind_is_z(m->res[r].kind) || (m->res[r].kind == AMP_KSTAR && m->res[r].J >= 1)) ? 3 : 1;
+            for (int j = 0; j < ns; ++j)
+                for (int c = 0; c < 2; ++c) diff |= m->couplings[((size_t)p * K + m->slot0[r] + j) * 2 + c] != m->couplings[((size_t)(m->slot0[r] + j)) * 2 + c];
+            if (!diff) continue;
+            if (changed >= 0) return false;
+            changed = r;
+        }
+        if (changed < 0) continue;   // equal to point 0
+        const int r = changed, t = ent_of_res[r];
+        const amp_resonance& rs = m->res[r];
+        const bool isz = kind_is_z(rs.kind);
+        const int ns = (isz || (rs.kind == AMP_KSTAR && rs.J >= 1)) ? 3 : 1;
+        const bool ls = m->mw[((size_t)p * R + r) * 2] != m->mw[(size_t)r * 2] || m->mw[((size_t)p * R + r) * 2 + 1] != m->mw[(size_t)r * 2 + 1];
+        double dre[3] = {0, 0, 0}, dim[3] = {0, 0, 0};
+        int nchg = 0, jlast = -1;
+        for (int j = 0; j < ns; ++j) {
+            dre[j] = m->couplings[((size_t)p * K + m->slot0[r] + j) * 2] - m->couplings[(size_t)(m->slot0[r] + j) * 2];
+            dim[j] = m->couplings[((size_t)p * K + m->slot0[r] + j) * 2 + 1] - m->couplings[(size_t)(m->slot0[r] + j) * 2 + 1];
+            if (dre[j] != 0.0 || dim[j] != 0.0) { ++nchg; jlast = j; }
+        }
+        LineConst lc0;
+        make_line_const(m, r, m->mw[(size_t)r * 2], m->mw[(size_t)r * 2 + 1], &lc0);
+        if (ls) {
+            if (nchg) return false;                         // lineshape and couplings at once: delta.cu
+            if (used_ent[t] >= 4) return false;
+            LineConst lcp;
+            make_line_const(m, r, m->mw[((size_t)p * R + r) * 2], m->mw[((size_t)p * R + r) * 2 + 1], &lcp);
+            if (used_ent[t] == 0)   // unused points of an entry in use sit at point 0 (Delta = 0)
+                for (auto& q : d.mw[t]) { q[0] = 1.0; q[1] = lc0.kG; q[2] = lc0.M2; }
+            const int j = used_ent[t]++;
+            d.mw[t][j][0] = lcp.kN / lc0.kN;
+            d.mw[t][j][1] = lcp.kG;
+            d.mw[t][j][2] = lcp.M2;
+            d.ent_active |= 1u << t;
+            d.val_of_point[p] = (short)(4 * lay.quad_of_ent[t] + j);
+            continue;
+        }
+        int pos;
+        if (nchg == 1) {
+            pos = base(t) + (ns == 3 ? jlast : 0);
+        } else if (nchg == 2 && isz && dre[0] == dre[2] && dim[0] == dim[2] && dre[1] == 0.0 && dim[1] == 0.0) {
+            pos = nslot + (t - (nent - d.a.shape[5]));      // tied pair of Z number t - oz
+            jlast = 0;
+        } else {
+            return false;
+        }
+        if (used_pos[pos] >= 4) return false;
+        const int j = used_pos[pos]++;
+        const double are = dre[jlast] * lc0.kN, aim = dim[jlast] * lc0.kN;
+        d.cq[pos][j][0] = are;
+        d.cq[pos][j][1] = aim;
+        d.cq[pos][j][2] = are * are + aim * aim;
+        d.cmax[pos][0] = std::max(d.cmax[pos][0], std::max(std::fabs(are), std::fabs(aim)));
+        d.cmax[pos][1] = std::max(d.cmax[pos][1], d.cq[pos][j][2]);
+        d.pos_active |= 1u << pos;
+        d.val_of_point[p] = (short)(4 * lay.quad_of_pos[pos] + j);
+        d.pos_of_point[p] = (short)pos;
+    }
+    d.P = P;
+    return true;
+}
+
 }  // namespace
 
 extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_couplings, const double* h_mass_width) {
@@ -700,8 +789,10 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
     // P > 1: a batch whose points are sparse changes of point 0 (a gradient step) runs the delta kernel: no column, no matrix
     if (m->has_bkg && P > 1) m->want_matrix = false;   // Eq. 14: the background path streams both samples, point by point (a single
                                                           // point at fixed lineshapes may still hold M: amp_nll_grad reads it)
-    m->use_delta = P > 1 && !m->has_bkg && m->batch_mode == 0 && m->lineshape_mode != 1 && m->norm_mode != 2 && build_delta_plan(m);
+    m->use_delta = P > 1 && !m->has_bkg && (m->batch_mode == 0 || m->batch_mode == 3) && m->lineshape_mode != 1 && m->norm_mode != 2 && build_delta_plan(m);
     if (m->use_delta) m->want_matrix = false;
+    // ... through the shape-specialised kernel where every point is one coupling or one lineshape change (batch mode 3: never)
+    m->use_deltaf = m->use_delta && m->batch_mode == 0 && build_deltaf_plan(m);
     m->stream_inline = (P == 1 || m->use_delta || m->has_bkg) && m->lineshape_mode != 1;
 
     // distinct (resonance, mass, width) keys of this call
@@ -1307,6 +1398,49 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         if (bad) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
         return AMP_OK;
     }
+    bool deltaf_tripped = false;
+    if (m->use_deltaf && (!want_nll || m->data.n <= 600LL * 256 * deltaf_grid(m->data.n, m->norm.n))) {
+        // Gradient batch of the paper's resonance lists: ONE launch of the shape-specialised kernel (deltaf.cu) for all points.
+        // (Per thread the data-side products of r in [0.5, 1.5] run over at most 600 events: far inside the FP64 range.)
+        DeltaFArgs& d = m->deltaf;
+        fill_stream_args(m, m->data, 0, MODE_FUSED, &d.a);
+        d.a.cache2 = m->norm.cache; d.a.n2 = m->norm.n; d.a.npad2 = m->norm.npad;
+        d.a.ticket = m->d_ticket;
+        d.a.sum_log_eff = m->data.loaded ? m->data.wsum : 0.0;
+        d.a.wsum = m->norm.wsum;
+        if (!want_nll) d.a.n = 0;
+        d.P = P;
+        d.partial = m->d_partial;
+        d.stride = PARTIAL_STRIDE;
+        d.result = m->d_result;
+        d.want_nll = want_nll ? 1 : 0;
+        m->ring_last = (m->ring_last + 1) % amp_model::RING;
+        m->ring_calls++;
+        CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
+        CK(launch_deltaf(d, deltaf_grid(d.a.n, d.a.n2), s));
+        CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
+        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (4 * P + 1), cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));
+        m->stat_launches = 1;
+        if (m->h_pinned[2 * P] < 1024.0) {
+            m->last_slog.assign(m->h_pinned + 2 * P + 1, m->h_pinned + 3 * P + 1);
+            m->last_swS.assign(m->h_pinned + 3 * P + 1, m->h_pinned + 4 * P + 1);
+            m->stat_norm_path = 9;
+            m->fused_valid = true;
+            bool bad = m->h_pinned[2 * P] != 0.0;
+            for (int p = 0; p < P; ++p) {
+                if (h_nll) { h_nll[p] = m->h_pinned[p]; bad |= !std::isfinite(h_nll[p]); }
+                if (h_I) { h_I[p] = m->h_pinned[P + p]; bad |= !(h_I[p] > 0) || !std::isfinite(h_I[p]); }
+            }
+            if (bad) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
+            return AMP_OK;
+        }
+        // a step so large that some S(p) / S(0) left [0.5, 1.5]: the general kernel below, amplitudes summed term by term
+        m->stat_deltaf_guard++;
+        deltaf_tripped = true;
+        m->ring_calls--;
+        m->ring_last = (m->ring_last + amp_model::RING - 1) % amp_model::RING;
+    }
     if (m->use_delta) {
         // Gradient batch: one fused launch per chunk of <= 128 points besides point 0 (delta.cu)
         int ent_of_res[AMP_MAX_RESONANCES], grp_of_res[AMP_MAX_RESONANCES];
@@ -1353,7 +1487,7 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         // The kernel expands single-contribution points around point 0 (S(0) + Re(coef T2) + |coef|^2 n); if some point's density
         // falls below 1e-3 S(0) at some event the guard trips (1024 in the flag word) and the call is repeated with the amplitudes
         // summed term by term.  Gradient steps never trip it; a batch that switches a dominant amplitude off can.
-        for (int exact = 0; exact < 2; ++exact) {
+        for (int exact = deltaf_tripped ? 1 : 0; exact < 2; ++exact) {
             for (size_t c = 0; c < m->delta_chunks.size(); ++c) {
                 const auto& ch = m->delta_chunks[c];
                 const size_t bC = al(ch.contrib.size() * sizeof(DeltaContrib)), bS = al(ch.slots.size() * sizeof(double) + 8);

@@ -211,16 +211,27 @@ def test_nll_batched_points_small():
     ref, refI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
     assert nll.shape == (121,)
     st = Mg.last_call_stats()
-    assert st["norm_path"] == 5 and st["launches"] == 1     # gradient-batch kernel: one fused launch, no columns, no matrix
+    assert st["norm_path"] == 9 and st["launches"] == 1     # shape-specialised gradient-batch kernel: one fused launch, no columns, no matrix
     assert st["columns_recomputed"] == 0
     assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
     assert np.array_equal(Mg.nll(), nll)                     # bit-reproducible
     I = Mg.norm_integral()
-    assert Mg.last_call_stats()["norm_path"] == 5
+    assert Mg.last_call_stats()["norm_path"] == 9
     assert np.max(np.abs(I - refI) / refI) < 1e-12
     # the finite differences themselves (what MINUIT uses) agree: compare NLL(p) - NLL(0)
     d, dref = nll[1:] - nll[0], ref[1:] - ref[0]
     assert np.max(np.abs(d - dref)) < 1e-9 * abs(ref[0])
+    # the general gradient-batch kernel (contribution program, delta.cu) on the same batch: another kernel, the same numbers
+    Mg.set_batch_mode(3)
+    Mg.set_params(cs, mws)
+    nll_g = Mg.nll()
+    st = Mg.last_call_stats()
+    assert st["norm_path"] == 5 and st["launches"] == 1
+    assert np.max(np.abs(nll_g - ref) / np.abs(ref)) < RTOL_NLL and np.max(np.abs(nll_g - nll) / np.abs(nll)) < 1e-12
+    assert np.max(np.abs((nll_g[1:] - nll_g[0]) - d)) < 1e-9 * abs(ref[0])
+    assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12 and Mg.last_call_stats()["norm_path"] == 5
+    Mg.set_batch_mode(0)
+    Mg.set_params(cs, mws)
     # per-event density of a perturbed point (lineshapes in registers)
     for p in (0, 5, 97, 120):
         v = Mg.eval_events(p).cpu().numpy()
@@ -254,10 +265,12 @@ def test_nll_batched_points_small():
 def test_delta_batches_general():
     """gradient-batch kernel beyond the cfg 4 pattern: ragged point counts (1, 31, 32, 33, 129, 200 points besides point 0,
     i.e. partial blocks and two launches), points equal to point 0, points that change two resonances at once, a K*-only
-    model, and a dense random batch that must fall back to the DMMA contraction."""
+    model, and a dense random batch that must fall back to the DMMA contraction.  (Batch mode 3: the general kernel even where a
+    batch happens to fit the shape-specialised one.)"""
     rng = np.random.default_rng(5)
     for cfg in (2, 1):
         Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+        Mg.set_batch_mode(3)
         x, eff, xn, wn = make_inputs(cfg, 3001, 7013)
         Mg.load_events(dev(x), dev(eff))
         Mg.load_norm(dev(xn), dev(wn))
@@ -287,6 +300,7 @@ def test_delta_batches_general():
             assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL, (cfg, P)
             assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12, (cfg, P)
         # dense random batch: every coupling differs -> not a gradient batch
+        Mg.set_batch_mode(0)
         P = 40
         cs = c0[None] * (1 + 0.1 * rng.uniform(-1, 1, (P, K)))
         Mg.set_params(cs)
@@ -302,6 +316,7 @@ def test_gradient_batch_large_coupling_steps_in_groups_of_four():
     of the full model, 109 points = one launch; then twice that = two launches.  Integrals at 1e-12, NLL at the parity bar."""
     cfg = 2
     Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+    Mg.set_batch_mode(3)                                      # the general gradient-batch kernel
     x, eff, xn, wn = make_inputs(cfg, 2999, 9001)
     Mg.load_events(dev(x), dev(eff))
     Mg.load_norm(dev(xn), dev(wn))
@@ -324,6 +339,105 @@ def test_gradient_batch_large_coupling_steps_in_groups_of_four():
         assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12, reps
 
 
+def _gradient_points(c0, mw0, couplings, lineshapes, h=1e-4):
+    """a MINUIT-style step: for every listed coupling slot modulus +-h and phase +-h, for every listed (resonance, 0 mass | 1 width) +-h"""
+    pts_c, pts_mw = [c0.copy()], [mw0.copy()]
+    for k in couplings:
+        for f in (1 + h, 1 - h, np.exp(1j * h), np.exp(-1j * h)):
+            c = c0.copy()
+            c[k] *= f
+            pts_c.append(c)
+            pts_mw.append(mw0.copy())
+    for r, which in lineshapes:
+        for sgn in (1, -1):
+            mw = mw0.copy()
+            mw[r, which] *= 1 + sgn * h
+            pts_c.append(c0.copy())
+            pts_mw.append(mw)
+    return np.array(pts_c), np.array(pts_mw)
+
+
+@pytest.mark.parametrize("cfg,n,m", [(1, 3001, 7013), (2, 1, 300), (2, 255, 257), (2, 513, 1025)])
+def test_shape_specialised_gradient_batch(cfg, n, m):
+    """deltaf.cu beyond configs[4]: the K*-only shape (no Z compiled in), every coupling and every mass and width floating, and
+    ragged sizes around the 256-event pipeline unit (a single data event; one event short of / past a unit; past a cache block).
+    NLL, integrals and the finite differences NLL(p) - NLL(0) against the oracle, and against the general kernel."""
+    Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+    c0 = W.couplings(cfg)
+    xn, wn = W.norm_events(cfg, m)
+    x, eff = W.data_events(cfg, lambda xx, ee: Mo.eval_events(c0, xx, ee), n=n)
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    mw0 = np.array([[r[2], r[3]] for r in W.resonances(cfg)]) * (1 + 1e-3 * np.random.default_rng(8).uniform(-1, 1, (len(W.resonances(cfg)), 2)))
+    R = len(mw0)
+    cs, mws = _gradient_points(c0, mw0, range(len(c0)), [(r, w) for r in range(R) for w in (0, 1)])
+    assert len(cs) == 1 + 4 * len(c0) + 4 * R
+    ref, refI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+    out = {}
+    for mode, path in ((0, 9), (3, 5)):
+        Mg.set_batch_mode(mode)
+        Mg.set_params(cs, mws)
+        nll = Mg.nll()
+        st = Mg.last_call_stats()
+        assert st["norm_path"] == path and (path == 5 or st["launches"] == 1), (mode, st)
+        assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
+        assert np.max(np.abs((nll - nll[0]) - (ref - ref[0]))) < 1e-9 * abs(ref[0])
+        assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12
+        assert np.array_equal(Mg.nll(), nll)                    # bit-reproducible
+        out[mode] = nll
+    assert np.max(np.abs(out[0] - out[3]) / np.abs(ref)) < 1e-12
+
+
+def test_shape_specialised_gradient_batch_falls_back():
+    """What deltaf.cu does not take goes to the general kernel with the same results: a fifth point on one coupling, a point that
+    moves a coupling and a mass at once, two resonances at one point; and a step so large that S(p) / S(0) leaves [0.5, 1.5]
+    at some event trips the guard, after which the call is repeated with the amplitudes summed term by term."""
+    cfg = 2
+    Mo, Mg = oracle_model(cfg), gpu_model(cfg)
+    x, eff, xn, wn = make_inputs(cfg, 3001, 7013)
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    c0 = W.couplings(cfg)
+    mw0 = np.array([[r[2], r[3]] for r in W.resonances(cfg)])
+    base_c, base_mw = _gradient_points(c0, mw0, [3, 4, 24, 25], [(10, 0), (1, 1)])
+    assert len(base_c) == 21
+
+    def check(cs, mws, path, launches=None):
+        Mg.set_params(cs, mws)
+        nll = Mg.nll()
+        st = Mg.last_call_stats()
+        assert st["norm_path"] == path and (launches is None or st["launches"] == launches), st
+        ref, refI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+        assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
+        assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12
+
+    check(base_c, base_mw, 9, 1)
+    # a point equal to point 0 and a Z pair moving together (Eq. 11) are still deltaf's
+    cs, mws = np.concatenate([base_c, base_c[:1], base_c[:1]]), np.concatenate([base_mw, base_mw[:1], base_mw[:1]])
+    cs[-1, 24] *= 1.0002
+    assert c0[26] == c0[24]                                    # Eq. 11 in the seeded couplings
+    cs[-1, 26] = cs[-1, 24]                                    # the same delta on l' = -1 and l' = +1
+    check(cs, mws, 9, 1)
+    # a fifth point on slot 3
+    cs, mws = np.concatenate([base_c, base_c[:1]]), np.concatenate([base_mw, base_mw[:1]])
+    cs[-1, 3] *= 1.0003
+    check(cs, mws, 5)
+    # coupling and mass of one resonance at one point
+    cs, mws = base_c.copy(), base_mw.copy()
+    mws[1, 1, 0] *= 1.0001                                     # point 1 already moves slot 3 = K*(892) lambda = -1 (resonance 1)
+    check(cs, mws, 5)
+    # two resonances at one point
+    cs, mws = base_c.copy(), base_mw.copy()
+    cs[2, 12] *= 1.0001
+    check(cs, mws, 5)
+    # the guard: one coupling reversed -> deltaf's launch, then the general kernel's exact form (2 launches in all)
+    cs, mws = base_c.copy(), base_mw.copy()
+    cs[5, 4] = -c0[4]
+    check(cs, mws, 5, 2)
+    # ... and the model returns to deltaf on the next small step
+    check(base_c, base_mw, 9, 1)
+
+
 def test_nll_terms_of_two_shards_add_up():
     """amp_nll_terms / amp_dataset_sums: the per-shard sums of two models that each hold half of the events combine
     (sharded.py's formula, here without a process group) to the oracle's NLL of the whole sample — for the fused
@@ -342,7 +456,7 @@ def test_nll_terms_of_two_shards_add_up():
         shards.append(Mg)
     c = W.couplings(cfg)
     cs4, mws4 = W.fit_points(4)
-    for cs, mws, fused_mode, path in ((c[None], None, 0, 4), (c[None], None, 1, 2), (cs4[:40], mws4[:40], 0, 5)):   # (2: same masses twice -> matrix M)
+    for cs, mws, fused_mode, path in ((c[None], None, 0, 4), (c[None], None, 1, 2), (cs4[:40], mws4[:40], 0, 9)):   # (2: same masses twice -> matrix M; 9: gradient batch)
         tot = np.zeros(4)
         sl, sw = 0.0, 0.0
         for Mg in shards:
@@ -771,12 +885,15 @@ def test_two_z_model_matches_oracle():
             cs[p, 3] *= 1 + sgn * 1e-3; p += 1                                        # a K* coupling
             mws[p, 1, 0] *= 1 + sgn * 1e-5; p += 1                                    # the K*(892) mass
     assert p == P
-    Mg.set_params(cs, mws)
-    nll = Mg.nll()
-    assert Mg.last_call_stats()["norm_path"] == 5
     rb, rI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
-    assert np.max(np.abs(nll - rb) / np.abs(rb)) < RTOL_NLL
-    assert np.max(np.abs(Mg.norm_integral() - rI) / rI) < 1e-12
+    for mode, path in ((0, 9), (3, 5)):                       # the shape-specialised kernel (two Zs compiled in), then the general one
+        Mg.set_batch_mode(mode)
+        Mg.set_params(cs, mws)
+        nll = Mg.nll()
+        assert Mg.last_call_stats()["norm_path"] == path
+        assert np.max(np.abs(nll - rb) / np.abs(rb)) < RTOL_NLL
+        assert np.max(np.abs((nll - nll[0]) - (rb - rb[0]))) < 1e-9 * abs(rb[0])
+        assert np.max(np.abs(Mg.norm_integral() - rI) / rI) < 1e-12
 
 
 def test_static_lineshapes_switch_to_the_matrix():
