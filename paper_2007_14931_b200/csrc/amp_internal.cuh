@@ -450,6 +450,8 @@ cudaError_t launch_herk(const HerkArgs& h, int grid, cudaStream_t s);
 cudaError_t launch_herk_finish(const double* partial, int ncta, int ntile, const int2* tiles, int KP, double* gt, double* G, cudaStream_t s);
 cudaError_t launch_quadform(const double* G, int KP, const double2* C, int nent, int P, double* out, cudaStream_t s);
 int herk_max_runs();
+int herk_grid(long long n, int nent, int ncolu);
+int herk_grid_max();
 cudaError_t launch_batch(const BatchArgs& a, int grid, cudaStream_t s);
 int batch_grid(long long n);
 bool batch_fits(int nent, int ncolu);

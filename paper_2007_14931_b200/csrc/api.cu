@@ -83,7 +83,7 @@ struct amp_model {
     std::vector<double> gram_mw;
     double* d_G = nullptr;         // [KP][KP] dense symmetric realified Gram matrix (sum_j w_j b' b'^T)
     double* d_gt = nullptr;        // [ntile][64]
-    double* d_gpartial = nullptr;  // [SMs][ntile][64]
+    double* d_gpartial = nullptr;  // [CTAs][ntile][64]
     size_t gram_cap_KP = 0, gram_cap_tiles = 0;
     unsigned char* d_hk = nullptr; // herk plan: entries, tiles, coefficients
     unsigned char* h_hk = nullptr; // pinned
@@ -1307,7 +1307,7 @@ amp_status norm_via_matrix(amp_model* m, const HerkPlan& hp, double* d_out, cuda
         m->gram_cap_tiles = ntile;
         CK(cudaMalloc(&m->d_G, sizeof(double) * (size_t)KP * KP));
         CK(cudaMalloc(&m->d_gt, sizeof(double) * (size_t)ntile * 64));
-        CK(cudaMalloc(&m->d_gpartial, sizeof(double) * (size_t)sm_count() * ntile * 64));
+        CK(cudaMalloc(&m->d_gpartial, sizeof(double) * (size_t)herk_grid_max() * ntile * 64));
     }
     std::memcpy(m->h_hk + oE, hp.entries.data(), bE);
     std::memcpy(m->h_hk + oT, hp.tiles.data(), bT);
@@ -1329,7 +1329,7 @@ amp_status norm_via_matrix(amp_model* m, const HerkPlan& hp, double* d_out, cuda
         h.nrun = hp.nrun;
         h.ntile = ntile;
         h.partial = m->d_gpartial;
-        const int grid = batch_grid(d.n);
+        const int grid = herk_grid(d.n, hp.nent, (int)hp.colu.size());
         CK(launch_herk(h, grid, s));
         CK(launch_herk_finish(m->d_gpartial, grid, ntile, reinterpret_cast<const int2*>(m->d_hk + oT), KP, m->d_gt, m->d_G, s));
         m->stat_launches += 3;

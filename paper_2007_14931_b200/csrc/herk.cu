@@ -13,6 +13,12 @@
 
 namespace amp {
 
+#ifndef AMP_HERK_MINB
+#define AMP_HERK_MINB 2
+#endif
+// CTAs per SM: a CTA alternates between building a basis tile (plain ALUs) and multiplying it (tensor pipe) with a barrier in
+// between, so two resident CTAs keep the tensor pipe fed while the other one builds (the tile's shared memory is ~80 KB)
+constexpr int HERK_MINB = AMP_HERK_MINB;
 constexpr int HERK_MAXRUN = 12;   // runs per warp; a run = one row tile I with two column tiles J0, J1 (3 fragment loads, 2 DMMA)
 
 __device__ __forceinline__ double lds_f64(uint32_t addr) {
@@ -24,7 +30,7 @@ __device__ __forceinline__ double lds_f64(uint32_t addr) {
 // The basis tile is built with every event scaled by sqrt(w_j), so G' = sum_j (sqrt(w) b')(sqrt(w) b')^T needs no
 // per-fragment weight and both MMA operands are plain fragment loads of the same tile.
 template <int NRUN>
-__global__ void __launch_bounds__(BT_THREADS, 1) k_herk(const __grid_constant__ HerkArgs h) {
+__global__ void __launch_bounds__(BT_THREADS, (NRUN <= 4 ? HERK_MINB : 1)) k_herk(const __grid_constant__ HerkArgs h) {
     extern __shared__ __align__(16) double smem[];
     const BatchArgs& a = h.b;
     const int KP = a.nent * 2;   // realified rows, multiple of 8
@@ -134,6 +140,17 @@ __global__ void __launch_bounds__(256) k_quadform(const double* __restrict__ G, 
 }
 
 int herk_max_runs() { return HERK_MAXRUN; }
+
+// persistent grid: as many CTAs per SM as the basis tile's shared memory allows, at most HERK_MINB
+int herk_grid(long long n, int nent, int ncolu) {
+    const long long ntiles = (n + BT_EVENTS - 1) / BT_EVENTS;
+    long long per_sm = (long long)((224 * 1024) / (tile_smem_bytes(nent, ncolu) + 1024));
+    if (per_sm > HERK_MINB) per_sm = HERK_MINB;
+    if (per_sm < 1) per_sm = 1;
+    const long long cap = (long long)sm_count() * per_sm;
+    return (int)(ntiles < 1 ? 1 : (ntiles > cap ? cap : ntiles));
+}
+int herk_grid_max() { return sm_count() * HERK_MINB; }
 
 template <int NRUN>
 static cudaError_t launch_herk_n(const HerkArgs& h, int grid, cudaStream_t s) {
