@@ -9,7 +9,7 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("AMP4D_LIB", os.path.join(HERE, "libamp4d.so"))   # override: experiments with kernel variants
+LIB_PATH = os.path.join(HERE, "libamp4d.so")   # built in-tree by paper_2007_14931_b200/build.py
 
 AMP_OK, AMP_ERR_INVALID, AMP_ERR_STATE, AMP_ERR_DOMAIN, AMP_ERR_CUDA, AMP_ERR_NOMEM = range(6)
 AMP_KSTAR, AMP_Z, AMP_CONST, AMP_LASS, AMP_ZM = 0, 1, 2, 3, 4

@@ -349,7 +349,7 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
     if (e == cudaSuccess) e = cudaMemset(m->d_flag, 0, sizeof(int));
     if (e == cudaSuccess) e = cudaMallocHost(&m->h_pinned, sizeof(double) * (4 * AMP_MAX_POINTS + 4));
     if (e == cudaSuccess) e = cudaHostAlloc(&m->h_zc, sizeof(double) * 8, cudaHostAllocMapped);
-    if (e == cudaSuccess) { std::memset(m->h_zc, 0, sizeof(double) * 8); m->zero_copy = std::getenv("AMP4D_NO_ZERO_COPY") == nullptr; }
+    if (e == cudaSuccess) { std::memset(m->h_zc, 0, sizeof(double) * 8); m->zero_copy = true; }
     for (int i = 0; i < 5 && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ev[i]);
     for (int i = 0; i < 2 * amp_model::RING && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ring[i]);
     if (e != cudaSuccess) { amp_model_destroy(m); return e == cudaErrorMemoryAllocation ? AMP_ERR_NOMEM : AMP_ERR_CUDA; }

@@ -22,14 +22,8 @@
 // sequences and the extra warps hide their latency.  Measured on configs[4] (with the four-point blocks): 5.55 ms, against
 // 5.74 ms for two events per thread x 256 threads (8 warps, 229 registers), which pays the warp-uniform per-point overhead once
 // for two events but stalls more.
-#ifndef AMP_DELTA_E
-#define AMP_DELTA_E 1
-#endif
-#ifndef AMP_DELTA_THREADS
-#define AMP_DELTA_THREADS 512
-#endif
-#define AMP_STREAM_E AMP_DELTA_E
-#define AMP_STREAM_THREADS AMP_DELTA_THREADS
+#define AMP_STREAM_E 1
+#define AMP_STREAM_THREADS 512
 #include "stream_core.cuh"
 #include "delta_core.cuh"
 
@@ -38,12 +32,6 @@ namespace amp {
 namespace {
 
 constexpr int DBLK = DELTA_MAX_SORTED / 32;
-#ifndef AMP_DELTA_QUNROLL
-#define AMP_DELTA_QUNROLL 1
-#endif
-// unrolling of the four-point steps of a 32-point block.  Measured on configs[4] with the slot sums on the normalisation tiles:
-// 1: 4.53 ms, 2: 4.63 ms, 4: 4.90 ms (before them 2 was best: 4.82 ms against 4.91 ms) — the loop body is instruction-cache bound
-constexpr int DELTA_QUNROLL = AMP_DELTA_QUNROLL;
 
 struct SlotVal {   // the current slot of one event
     double2 Sp, Sm;                 // xi = +1, -1
@@ -301,7 +289,8 @@ __device__ __forceinline__ void eval_block(const StreamArgs& a, const DeltaContr
             leaf<NORM, FAST>(a, prog, slots, it, k, fg, zst, sv, w, live, bad, &y[1], &ye[1]);
         }
     };
-#pragma unroll DELTA_QUNROLL
+    // (not unrolled: the body is large, and two or four copies of it measured slower)
+#pragma unroll 1
     for (int q = 0; q < 32; q += 4) {
         double y[4]; int ye[4];
         {

@@ -42,13 +42,8 @@ namespace amp {
 namespace {
 
 constexpr int UNIT = THREADS;   // events per pipeline unit (half a cache block)
-#ifndef AMP_DELTAF_NSTAGE
-#define AMP_DELTAF_NSTAGE 2
-#endif
-#ifndef AMP_DELTAF_MINB
-#define AMP_DELTAF_MINB 2
-#endif
-constexpr int NSTAGE = AMP_DELTAF_NSTAGE;
+constexpr int NSTAGE = 2;       // stages per CTA
+constexpr int DELTAF_MINB = 2;  // CTAs per SM
 static_assert(2 * UNIT == CACHE_TILE, "two units per cache block");
 
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
@@ -152,7 +147,7 @@ struct Tree {
 }  // namespace
 
 template <class SH>
-__global__ void __launch_bounds__(THREADS, AMP_DELTAF_MINB) k_deltaf(const __grid_constant__ DeltaFArgs d) {
+__global__ void __launch_bounds__(THREADS, DELTAF_MINB) k_deltaf(const __grid_constant__ DeltaFArgs d) {
     using L = DLay<SH>;
     constexpr int NENT = L::NENT, NSLOT = L::NSLOT, NPOS = L::NPOS, NVAL = L::NVAL, NBLK = L::NBLK;
     constexpr bool have_z = SH::nz > 0;
@@ -319,9 +314,7 @@ __global__ void __launch_bounds__(THREADS, AMP_DELTAF_MINB) k_deltaf(const __gri
         auto position = [&](auto& tree, const bool norm, const int pos, const double2 Lk, const double nk) {
             if (!((d.pos_active >> pos) & 1u)) { tree.push_identity(); return; }
             if (norm) { tree.push3(Lk.x, Lk.y, nk); return; }
-#ifndef AMP_DELTAF_NOGUARD
             if (fma(d.cmax[pos][0], fabs(Lk.x) + fabs(Lk.y), d.cmax[pos][1] * nk) > 0.5) bad |= 2;
-#endif
             double r[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) r[j] = fma(d.cq[pos][j][0], Lk.x, fma(d.cq[pos][j][1], Lk.y, fma(d.cq[pos][j][2], nk, 1.0)));
@@ -338,9 +331,7 @@ __global__ void __launch_bounds__(THREADS, AMP_DELTAF_MINB) k_deltaf(const __gri
                 const double sc = d.mw[t][j][0] * F * fast_rcp(fma(dre, dre, MG * MG));
                 const double Dx = fma(sc, dre, -bw0.x), Dy = fma(sc, MG, -bw0.y);
                 const double x = fma(Dx, Q.x, fma(Dy, Q.y, fma(Dx, Dx, Dy * Dy) * nR));
-#ifndef AMP_DELTAF_NOGUARD
                 if (!norm && !(fabs(x) <= 0.5)) bad |= 2;
-#endif
                 y[j] = norm ? x : 1.0 + x;
             }
             tree.push4(y[0], y[1], y[2], y[3]);
@@ -560,7 +551,7 @@ cudaError_t launch_deltaf_shape(const DeltaFArgs& d, int grid, cudaStream_t s) {
 
 int deltaf_grid(long long n_data, long long n_norm) {
     const long long nunits = 2 * ((n_data + CACHE_TILE - 1) / CACHE_TILE) + 2 * ((n_norm + CACHE_TILE - 1) / CACHE_TILE);
-    const long long cap = (long long)sm_count() * AMP_DELTAF_MINB;
+    const long long cap = (long long)sm_count() * DELTAF_MINB;
     return (int)(nunits < 1 ? 1 : (nunits > cap ? cap : nunits));   // persistent: one CTA per SM
 }
 

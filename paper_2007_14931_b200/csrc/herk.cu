@@ -13,12 +13,9 @@
 
 namespace amp {
 
-#ifndef AMP_HERK_MINB
-#define AMP_HERK_MINB 2
-#endif
 // CTAs per SM: a CTA alternates between building a basis tile (plain ALUs) and multiplying it (tensor pipe) with a barrier in
 // between, so two resident CTAs keep the tensor pipe fed while the other one builds (the tile's shared memory is ~80 KB)
-constexpr int HERK_MINB = AMP_HERK_MINB;
+constexpr int HERK_MINB = 2;
 constexpr int HERK_MAXRUN = 12;   // runs per warp; a run = one row tile I with two column tiles J0, J1 (3 fragment loads, 2 DMMA)
 
 __device__ __forceinline__ double lds_f64(uint32_t addr) {
