@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(BT_THREADS, (NRUN <= 4 ? HERK_MINB : 1)) k_her
         if (tid == 0 && tile + gridDim.x < ntiles) issue_stage(a, tile + gridDim.x, t.scol, t.sang, t.sw, t.full, nang, true);
 #pragma unroll 1
         for (int xi = 0; xi < 2; ++xi) {
-#pragma unroll 1
+#pragma unroll 4   // fragment loads of the next steps issue under the DMMAs of this one (4.2 -> 3.9 ms for K = 27 at 10M events)
             for (int ks = 0; ks < BT_EVENTS / 4; ++ks) {
                 // fragment element of this lane: basis row (tile row lane/4), event 4 ks + lane%4
                 const uint32_t fb = bs32 + (uint32_t)((xi * KP * BT_STRIDE + 4 * ks) * sizeof(double));
