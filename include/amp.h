@@ -123,6 +123,28 @@ amp_status amp_set_params(amp_model* m, int P, const double* h_couplings, const 
  * finite and positive: h_nll[p] = +inf for those points, the others are valid.                         */
 amp_status amp_nll(amp_model* m, double* h_nll, void* stream);
 
+/* amp_nll for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the same one-launch evaluation as amp_nll at a single point with floating lineshapes (k_stream<MODE_FUSED>,
+ * Eqs. 5, 12 and the Monte Carlo integral), one launch per point of the last amp_set_params, with the
+ * kernel's scratch (per-CTA partial sums, the last-CTA ticket, the domain flag) in a file-scope `static __device__` array of
+ * the library instead of the model's buffers.  It calls no cudaMalloc / cudaFree / allocating library routine, copies nothing
+ * and does not synchronise: the launches are enqueued on `stream` and the call returns.
+ *   d_out DEVICE [P][6], caller-owned: per point NLL, I, domain flag (non-zero: some eps_i S_i or I was not finite and positive,
+ *   NLL = +inf), sum_i log S_i, sum_j w_j S_j, and 1.0 (written last: the block is complete).  Same bits as amp_nll for the same
+ *   inputs (same kernel, same grid, same fixed-order sums).
+ * Limits: P <= AMP_STATIC_MAX_POINTS and a persistent grid of at most AMP_STATIC_MAX_CTAS CTAs (2 per SM); beyond them
+ * AMP_ERR_INVALID with a message that names the limit.  AMP_ERR_STATE without data / norm sample / parameters or with a
+ * background set (Eq. 14 needs a second pass over model-owned buffers).  Lineshapes are always evaluated in registers
+ * (amp_set_lineshape_mode is not consulted: pool columns are model-owned buffers).  The array (AMP_STATIC_SCRATCH_BYTES = 133 120 B) is held by every device that loads the library until
+ * the process exits; its address is looked up once per device (cudaGetSymbolAddress, with the model's device current) on the first
+ * call there.  EVERY call on a device shares it and it keeps the last call's contents: the ticket and flag words are cleared on
+ * `stream` before each launch, so calls on ONE stream are safe back to back, while calls that overlap on the GPU (two streams, two
+ * host threads, two models on one device) race on it - serialise them.                                                     */
+#define AMP_STATIC_MAX_POINTS 8
+#define AMP_STATIC_MAX_CTAS 1024
+#define AMP_STATIC_SCRATCH_BYTES (AMP_STATIC_MAX_POINTS * (2 * AMP_STATIC_MAX_CTAS * 8 + 256))
+amp_status amp_nll_static(amp_model* m, double* d_out, void* stream);
+
 /* NLL and its analytic gradient in the couplings at the single point of the last amp_set_params (P = 1), in ONE pass over
  * the data and normalisation events (one launch):
  *   h_nll host [1]; h_grad host [K][2] = (dNLL/dRe H_k, dNLL/dIm H_k) in slot order, from

@@ -14,11 +14,12 @@ LIB_PATH = os.path.join(HERE, "libamp4d.so")   # built in-tree by paper_2007_149
 AMP_OK, AMP_ERR_INVALID, AMP_ERR_STATE, AMP_ERR_DOMAIN, AMP_ERR_CUDA, AMP_ERR_NOMEM = range(6)
 AMP_KSTAR, AMP_Z, AMP_CONST, AMP_LASS, AMP_ZM = 0, 1, 2, 3, 4
 AMP_MAX_RESONANCES, AMP_MAX_COUPLINGS, AMP_MAX_POINTS = 16, 48, 256
+AMP_STATIC_MAX_POINTS, AMP_STATIC_MAX_CTAS = 8, 1024
 
 # every symbol include/amp.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = [
     "amp_model_create", "amp_model_destroy", "amp_num_couplings", "amp_num_resonances", "amp_load_events",
-    "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_grad", "amp_fit", "amp_generate", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
+    "amp_load_norm", "amp_set_background", "amp_set_params", "amp_nll", "amp_nll_static", "amp_nll_grad", "amp_fit", "amp_generate", "amp_nll_terms", "amp_dataset_sums", "amp_eval_events", "amp_norm_integral", "amp_dump_cache",
     "amp_cache_column_name", "amp_eval_lineshape", "amp_norm_matrix", "amp_fit_fractions", "amp_set_norm_mode", "amp_set_lineshape_mode", "amp_set_batch_mode", "amp_set_fused_mode", "amp_set_grad_mode",
     "amp_last_call_stats", "amp_last_call_timing", "amp_recent_launch_ms", "amp_last_error", "amp_status_string", "amp_version", "amp_probe_fp64", "amp_probe_hbm_read",
 ]
@@ -62,6 +63,7 @@ def lib():
         "amp_set_background": (i, [vp, vp, d, vp]),
         "amp_set_params": (i, [vp, i, vp, vp]),
         "amp_nll": (i, [vp, vp, vp]),
+        "amp_nll_static": (i, [vp, vp, vp]),
         "amp_nll_grad": (i, [vp, vp, vp, vp]),
         "amp_fit": (i, [vp, vp, vp, vp, i, vp, vp, vp, i, vp, i, vp, i, d, vp, vp, vp, vp, vp, vp]),
         "amp_generate": (i, [vp, C.c_ulonglong, C.c_ulonglong, ll, d, d, d, d, vp, vp, ll, C.POINTER(ll), pd, vp]),
@@ -193,6 +195,13 @@ class Model:
         if not (allow_domain_error and st == AMP_ERR_DOMAIN):
             self._check(st, "amp_nll")
         return out[:self.P]
+
+    def nll_static(self, out, stream=None):
+        """amp_nll_static: the fused launch(es) with the kernel's scratch in the library's static device array (no allocation, no copy,
+        no synchronisation).  `out`: caller-owned float64 CUDA tensor [P][6] = (NLL, I, domain flag, sum log S, sum w S, 1.0) per point;
+        P <= AMP_STATIC_MAX_POINTS.  Calls that overlap on the GPU race on the shared array."""
+        self._check(lib().amp_nll_static(self._h, _dev_ptr(out, 6 * max(self.P, 1)), _stream_ptr(stream)), "amp_nll_static")
+        return out
 
     def nll_grad(self, stream=None):
         """(NLL, grad [K][2] = (dNLL/dRe H_k, dNLL/dIm H_k)) at the single point set by set_params"""

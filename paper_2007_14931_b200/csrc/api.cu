@@ -1730,6 +1730,31 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
 
 }  // namespace
 
+// ---- amp_nll_static: the fused launch with its scratch in a static device array (include/amp.h) -----------------------
+// Per point a slice of [2][AMP_STATIC_MAX_CTAS] doubles (the CTAs' sum log S and sum w S) and a 256-byte control block
+// (ticket, then flag).  In HOST code the array's name is only a handle for cudaGetSymbolAddress, never a device address.
+constexpr size_t STATIC_SLICE_BYTES = 2 * (size_t)AMP_STATIC_MAX_CTAS * sizeof(double) + 256;
+static_assert(AMP_STATIC_SCRATCH_BYTES == AMP_STATIC_MAX_POINTS * STATIC_SLICE_BYTES, "include/amp.h states the size");
+static __device__ __align__(256) unsigned char g_static_scratch[AMP_STATIC_SCRATCH_BYTES];
+
+// device address of g_static_scratch on the CURRENT device, looked up once per device
+cudaError_t static_scratch_address(unsigned char** out) {
+    static std::atomic<unsigned char*> addr[AMP_MAX_DEVICES];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= AMP_MAX_DEVICES) return cudaErrorInvalidDevice;
+    unsigned char* p = addr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        e = cudaGetSymbolAddress((void**)&p, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        addr[dev].store(p, std::memory_order_release);   // (two threads racing here store the same address)
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
 extern "C" {
 
 amp_status amp_nll(amp_model* m, double* h_nll, void* stream) {
@@ -1737,6 +1762,57 @@ amp_status amp_nll(amp_model* m, double* h_nll, void* stream) {
     DeviceGuard on_device(m);
     if (!h_nll) return fail(m, AMP_ERR_INVALID, "amp_nll: null output");
     return evaluate(m, true, h_nll, nullptr, (cudaStream_t)stream);
+}
+
+amp_status amp_nll_static(amp_model* m, double* d_out, void* stream) {
+    if (!m) return AMP_ERR_INVALID;
+    DeviceGuard on_device(m);
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!d_out) return fail(m, AMP_ERR_INVALID, "amp_nll_static: null output");
+    if (!m->norm.loaded) return fail(m, AMP_ERR_STATE, "no normalisation sample loaded (amp_load_norm)");
+    if (!m->data.loaded) return fail(m, AMP_ERR_STATE, "no data events loaded (amp_load_events)");
+    if (m->P < 1) return fail(m, AMP_ERR_STATE, "no parameters set (amp_set_params)");
+    if (m->has_bkg) return fail(m, AMP_ERR_STATE, "amp_nll_static: not available with a background set (Eq. 14 takes two passes over model-owned buffers)");
+    if (m->P > AMP_STATIC_MAX_POINTS) {
+        char msg[160];
+        std::snprintf(msg, sizeof msg, "amp_nll_static: %d points exceed the static scratch (AMP_STATIC_MAX_POINTS = %d)", m->P, (int)AMP_STATIC_MAX_POINTS);
+        return fail(m, AMP_ERR_INVALID, msg);
+    }
+    const int grid = stream_grid_fused(m->data.n, m->norm.n, m->has_z);
+    if (grid > AMP_STATIC_MAX_CTAS) {
+        char msg[160];
+        std::snprintf(msg, sizeof msg, "amp_nll_static: a grid of %d CTAs exceeds the static scratch (AMP_STATIC_MAX_CTAS = %d)", grid, (int)AMP_STATIC_MAX_CTAS);
+        return fail(m, AMP_ERR_INVALID, msg);
+    }
+    unsigned char* base = nullptr;
+    CK(static_scratch_address(&base));
+    for (int p = 0; p < m->P; ++p) {
+        unsigned char* slice = base + (size_t)p * STATIC_SLICE_BYTES;
+        unsigned char* ctl = slice + 2 * (size_t)AMP_STATIC_MAX_CTAS * sizeof(double);
+        StreamArgs a;
+        fill_stream_args(m, m->data, p, MODE_FUSED, &a);
+        // lineshapes always in registers here (pool columns are model-owned buffers that may not exist yet): fold kN as fill_stream_args does
+        for (int t = 0; t < a.lass0 + a.nlass; ++t) {
+            ResEntry& e = a.ent[t];
+            if (e.column < 0) continue;
+            e.column = -1;
+            if (t < a.lass0) { e.cm.x *= e.kN; e.cm.y *= e.kN; e.c0.x *= e.kN; e.c0.y *= e.kN; e.cp.x *= e.kN; e.cp.y *= e.kN; }
+        }
+        a.cols = nullptr;
+        a.partial = reinterpret_cast<double*>(slice);
+        a.partial2 = a.partial + AMP_STATIC_MAX_CTAS;
+        a.ticket = reinterpret_cast<unsigned int*>(ctl);
+        a.flag = reinterpret_cast<int*>(ctl + 128);
+        a.cache2 = m->norm.cache; a.n2 = m->norm.n; a.npad2 = m->norm.npad;
+        a.sum_log_eff = m->data.wsum;
+        a.wsum = m->norm.wsum;
+        a.result = d_out + (size_t)6 * p;
+        a.seq = 1.0;
+        // the array keeps what the last call (of anyone) left: ticket and flag must start at zero; the partials are overwritten
+        CK(cudaMemsetAsync(ctl, 0, 256, s));
+        CK(launch_stream(a, grid, s));
+    }
+    return AMP_OK;
 }
 
 amp_status amp_nll_terms(amp_model* m, double* h_sum_log, double* h_sum_wS, void* stream) {
