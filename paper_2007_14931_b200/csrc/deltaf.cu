@@ -20,14 +20,15 @@
 // lambda = -1, 0, +1; per Z one more position for the tied pair) and four per entry for its lineshape points — so the code is
 // straight-line: no program decode, no slot records, no per-point branches.  The host fills the coefficient tables of the
 // positions in use (DeltaFArgs, kernel parameter space: operands come from the constant bank) and maps points to value slots.
-// Values are reduced over the warp by the recursive-halving exchange (one shuffle + one add or multiply per value and lane), which
-// leaves lane l of block b with the warp total of value 32 b + l in a register; per-CTA partials, last-CTA finish: bit-reproducible.
+// Values are summed over a warp's 32 events through a per-warp shared-memory tile (struct Tile below: one store, half a 16-byte
+// load and one add or multiply per value and lane), which leaves lane l with the total of value 8 c + l % 8 of chunk c over a
+// quarter of the events in a register; per-CTA partials, last-CTA finish: bit-reproducible.
 // A change so large that r leaves [0.5, 1.5] trips the guard (flag 1024): the host repeats the call with delta.cu's exact form.
 //
 // Pipeline: as gradf.cu (256-event units, a ring of TMA-fed stages with full / empty mbarriers, producer duty rotates over the
-// warps), but TWO CTAs of 256 threads per SM at 128 registers with two stages each: the values pass is long chains of
-// select -> shuffle -> add, and sixteen warps hide them better than eight (measured on configs[4]: 2.53 ms against 2.76 ms for one
-// CTA at 255 registers with four stages).  To fit, the lineshapes of point 0 are not kept across the forward pass (they are
+// warps), but TWO CTAs of 256 threads per SM at 128 registers with two stages each: the values pass is long dependent chains, and
+// sixteen warps hide them better than eight (measured on configs[4]: 2.53 ms against 2.76 ms for one CTA at 255 registers with
+// four stages; four CTAs of 128 threads or one of 512: 2.41 / 2.44 against 2.29 ms).  To fit, the lineshapes of point 0 are not kept across the forward pass (they are
 // re-evaluated class by class from the saved barrier factors) and the Z-chain angles are read again from the stage, which a
 // warp releases only after its values pass.  Bound: plain FP64 ALUs.
 #define AMP_STREAM_E 2
@@ -57,7 +58,7 @@ struct DLay {
     static constexpr int NSLOT = SH::n0 + 3 * (NENT - SH::n0);          // single-slot coupling positions
     static constexpr int NPOS = NSLOT + SH::nz;                         // + one tied-pair position per Z
     static constexpr int NVAL = 4 * (NPOS + NENT);                      // value slots: 4 per coupling position, then 4 per entry (lineshape points)
-    static constexpr int NBLK = (NVAL + 31) / 32;
+    static constexpr int NCH = (NVAL / 4 + 1) / 2;                      // chunks of eight values (two quads)
     __host__ __device__ static constexpr int base(int t) { return t < SH::n0 ? t : SH::n0 + 3 * (t - SH::n0); }
 };
 static_assert(DLay<Shape<3, 3, 2, 1, 1, 2>>::NPOS <= DELTAF_MAX_POS && DLay<Shape<3, 3, 2, 1, 1, 2>>::NENT <= DELTAF_MAX_ENT, "tables of DeltaFArgs");
@@ -81,67 +82,70 @@ __device__ __forceinline__ double2 conj_mul(double2 bw, double2 x) {
     return make_double2(fma(bw.x, x.x, bw.y * x.y), fma(bw.x, x.y, -bw.y * x.x));
 }
 
-// Recursive halving over the 32 lanes without exponents (sums on the normalisation side, products of r ~ 1 on the data side):
-// `a` belongs to the earlier half of the values, `b` to the later half; lanes with bit `level` clear keep the earlier half.
-template <bool NORM>
-__device__ __forceinline__ double halve1(int level, int lane, double a, double b) {
-    const bool up = (lane >> level) & 1;
-    const double send = up ? a : b, keep = up ? b : a;
-    const double recv = __shfl_xor_sync(0xffffffffu, send, 1 << level);
-    return NORM ? keep + recv : keep * recv;
-}
-
-// The values of one event go through a binary-counter merge in groups of four; after 32 values lane l holds the warp total of
-// value l of the block, which is folded into the lane's accumulator of that block.  q (quads pushed so far) only ever changes
-// by constants in straight-line code, so every test on it is resolved at compile time.
-template <bool NORM, int NBLK>
-struct Tree {
-    double s2, s3, s4;
+// The values of one event-row (32 events of a warp, one per lane) are summed over the events through a per-warp shared-memory
+// tile, eight values (two quads) at a time: lane e stores its value v at [v][e] (row stride 256 B: conflict-free), and lane l
+// reads the eight events 8 g .. 8 g + 7 of value v = l % 8 as four 16-byte loads and folds them into its accumulator of the
+// chunk (a register; NORM: sum, DATA: product of r ~ 1).  So that a quarter-warp's 16-byte loads hit eight different banks
+// although every row starts at bank 0, lanes with v >= 4 take the next event group (g = (l / 8 + v / 4) % 4) and every lane
+// walks its four slots rotated by v.  Per value this is one store, half a load and one FP64 operation (the exchange tree of
+// selects and shuffles it replaces took ~8 instructions per value); the order of the sums is fixed, so the result is
+// reproducible.  q (quads pushed so far) only ever changes by constants in straight-line code: every test on it is resolved at
+// compile time.
+constexpr int TILE_ROW_BYTES = 32 * 8;
+constexpr int TILE_BYTES = 8 * TILE_ROW_BYTES;   // per warp
+template <bool NORM, int NCH>
+struct Tile {
+    uint32_t wr;              // shared-space address of [0][lane]
+    uint32_t rd[4];           // ... of the four 16-byte slots this lane reads
+    double x[8];              // the eight values of the chunk whose loads are under way
     int q;
-    int lane;
-    double* acc;              // [NBLK] the lane's block accumulators (registers of the kernel, shared by the two phases): NORM: sums;
-    int* accE;                //        DATA: mantissa of the running product, and [NBLK] its exponent
+    double* acc;              // [NCH] the lane's chunk accumulators (registers of the kernel, shared by the two phases)
+    __device__ __forceinline__ void init(uint32_t tile, int lane) {
+        const int v = lane & 7, g = ((lane >> 3) + (v >> 2)) & 3;
+        wr = tile + lane * 8;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) rd[i] = tile + v * TILE_ROW_BYTES + g * 64 + ((i + v) & 3) * 16;
+    }
     __device__ __forceinline__ void reset_event() { q = 0; }
     __device__ __forceinline__ void push4(double y0, double y1, double y2, double y3) {
-        const double u = halve1<NORM>(0, lane, y0, y1);
-        double x = halve1<NORM>(0, lane, y2, y3);
-        merge(halve1<NORM>(1, lane, u, x));
+        const uint32_t w = wr + (q & 1) * 4 * TILE_ROW_BYTES;
+        asm volatile("st.shared.f64 [%0], %1;" ::"r"(w), "d"(y0) : "memory");
+        asm volatile("st.shared.f64 [%0+256], %1;" ::"r"(w), "d"(y1) : "memory");
+        asm volatile("st.shared.f64 [%0+512], %1;" ::"r"(w), "d"(y2) : "memory");
+        asm volatile("st.shared.f64 [%0+768], %1;" ::"r"(w), "d"(y3) : "memory");
+        if (q & 1) load();             // the chunk is complete: its loads are issued now and used one quad later
+        else if (q > 0) fold(q / 2 - 1);
+        ++q;
     }
     // the three sums of a coupling position on the normalisation side (the fourth value of the quad is zero)
-    __device__ __forceinline__ void push3(double y0, double y1, double y2) {
-        const double u = halve1<NORM>(0, lane, y0, y1);
-        const double r = __shfl_xor_sync(0xffffffffu, y2, 1);
-        merge(halve1<NORM>(1, lane, u, (lane & 1) ? 0.0 : y2 + r));
+    __device__ __forceinline__ void push3(double y0, double y1, double y2) { push4(y0, y1, y2, 0.0); }
+    // a quad that is not in use: neutral values
+    __device__ __forceinline__ void push_identity() { const double id = NORM ? 0.0 : 1.0; push4(id, id, id, id); }
+    // A warp's shared-memory accesses are performed in program order, so the stores of the next quad (rows 0-3 again) cannot
+    // overtake these loads; the four loads are one statement so that they get four register pairs and issue back to back.
+    __device__ __forceinline__ void load() {
+        __syncwarp();
+        asm volatile(
+            "ld.shared.v2.f64 {%0, %1}, [%8];\n\t"
+            "ld.shared.v2.f64 {%2, %3}, [%9];\n\t"
+            "ld.shared.v2.f64 {%4, %5}, [%10];\n\t"
+            "ld.shared.v2.f64 {%6, %7}, [%11];"
+            : "=d"(x[0]), "=d"(x[1]), "=d"(x[2]), "=d"(x[3]), "=d"(x[4]), "=d"(x[5]), "=d"(x[6]), "=d"(x[7])
+            : "r"(rd[0]), "r"(rd[1]), "r"(rd[2]), "r"(rd[3])
+            : "memory");
+        __syncwarp();
     }
-    // a quad that is not in use: neutral values (nothing to exchange at the two lowest levels)
-    __device__ __forceinline__ void push_identity() { merge(NORM ? 0.0 : 1.0); }
-    __device__ __forceinline__ void merge(double x) {
-        const int qq = q & 7, b = q >> 3;
-        ++q;
-        if (!(qq & 1)) { s2 = x; return; }
-        x = halve1<NORM>(2, lane, s2, x);
-        if (!(qq & 2)) { s3 = x; return; }
-        x = halve1<NORM>(3, lane, s3, x);
-        if (!(qq & 4)) { s4 = x; return; }
-        x = halve1<NORM>(4, lane, s4, x);
+    __device__ __forceinline__ void fold(int c) {
 #pragma unroll
-        for (int bb = 0; bb < NBLK; ++bb) {
-            if (bb == b) {
-                if (NORM) {
-                    acc[bb] += x;
-                } else {   // a product of 32 values in [0.5, 1.5]: renormalised once per event and block
-                    double f; int e;
-                    split_exp(acc[bb] * x, &f, &e);
-                    acc[bb] = f;
-                    accE[bb] += e;
-                }
+        for (int cc = 0; cc < NCH; ++cc)
+            if (cc == c) {
+                if (NORM) acc[cc] += ((x[0] + x[1]) + (x[2] + x[3])) + ((x[4] + x[5]) + (x[6] + x[7]));
+                else acc[cc] *= ((x[0] * x[1]) * (x[2] * x[3])) * ((x[4] * x[5]) * (x[6] * x[7]));   // r in [0.5, 1.5]: renormalised every 16 units
             }
-        }
     }
-    __device__ __forceinline__ void pad_block() {   // complete the last block with neutral values
-        const double id = NORM ? 0.0 : 1.0;
-        (void)id;
-        while (q & 7) push_identity();
+    __device__ __forceinline__ void pad_block() {   // complete the last chunk with neutral values and take in the loads still under way
+        if (q & 1) push_identity();
+        fold(q / 2 - 1);
     }
 };
 
@@ -156,7 +160,7 @@ __device__ __forceinline__ void align_warps() { asm volatile("bar.sync 1, %0;" :
 template <class SH>
 __global__ void __launch_bounds__(THREADS, DELTAF_MINB) k_deltaf(const __grid_constant__ DeltaFArgs d) {
     using L = DLay<SH>;
-    constexpr int NENT = L::NENT, NSLOT = L::NSLOT, NPOS = L::NPOS, NVAL = L::NVAL, NBLK = L::NBLK;
+    constexpr int NENT = L::NENT, NSLOT = L::NSLOT, NPOS = L::NPOS, NVAL = L::NVAL, NCH = L::NCH, NVP = 8 * NCH;
     constexpr bool have_z = SH::nz > 0;
     const StreamArgs& a = d.a;
     const double RSQRT2 = 0.70710678118654752440, LN2 = 0.69314718055994530942;
@@ -165,8 +169,8 @@ __global__ void __launch_bounds__(THREADS, DELTAF_MINB) k_deltaf(const __grid_co
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* stage0 = reinterpret_cast<double*>(smem_raw);                                        // [NSTAGE][ncolw][UNIT]
-    double* red = stage0 + (size_t)NSTAGE * ncolw * UNIT;                                        // flush: [NWARPS][32 NBLK]; finish: 2 + 2 NVAL totals
-    uint64_t* full = reinterpret_cast<uint64_t*>(red + NWARPS * 32 * NBLK);
+    double* red = stage0 + (size_t)NSTAGE * ncolw * UNIT;                                        // [NWARPS] value tiles of 2 KB; flush: [NWARPS][NVP]; finish: 2 + 2 NVAL totals
+    uint64_t* full = reinterpret_cast<uint64_t*>(red + NWARPS * (TILE_BYTES / 8));
     __shared__ double sm[NWARPS];
     __shared__ bool s_last;
     uint64_t* empty = full + NSTAGE;   // a stage is free again once every warp has read its event's columns
@@ -189,16 +193,15 @@ __global__ void __launch_bounds__(THREADS, DELTAF_MINB) k_deltaf(const __grid_co
         for (int s = 0; s < NSTAGE; ++s)
             if (blockIdx.x + (long long)s * gridDim.x < nunits) issue(blockIdx.x + (long long)s * gridDim.x, s);
 
-    double accv[NBLK];      // the lane's block accumulators: products of r (data units, with exponents accx), then sums (normalisation units)
-    int accx[NBLK];
-    Tree<false, NBLK> td;   // data side: products of r
-    Tree<true, NBLK> tn;    // normalisation side: sums
-    td.lane = tn.lane = lane;
+    double accv[NCH];       // the lane's chunk accumulators: products of r (data units, with exponents accx), then sums (normalisation units)
+    int accx[NCH];
+    Tile<false, NCH> td;    // data side: products of r
+    Tile<true, NCH> tn;     // normalisation side: sums
+    td.init(smem_u32(red) + warp * TILE_BYTES, lane);
+    tn.init(smem_u32(red) + warp * TILE_BYTES, lane);
     td.acc = tn.acc = accv;
-    td.accE = tn.accE = accx;
-    td.s2 = td.s3 = td.s4 = tn.s2 = tn.s3 = tn.s4 = 0.0;
 #pragma unroll
-    for (int b = 0; b < NBLK; ++b) { accv[b] = 1.0; accx[b] = 0; }
+    for (int c = 0; c < NCH; ++c) { accv[c] = 1.0; accx[c] = 0; }
     double acc0F = 1.0, acc0W = 0.0;   // point 0: sum log S as mantissa product / exponent sum; sum w S
     int acc0E = 0;
     int bad = 0;                       // 1: a density that is not finite and positive; 2: the guard on r tripped
@@ -206,16 +209,21 @@ __global__ void __launch_bounds__(THREADS, DELTAF_MINB) k_deltaf(const __grid_co
 
     // per-CTA partial rows [row0, row0 + NVAL) of the lanes' block accumulators: summed over the warps in warp order
     auto flush = [&](int row0, bool data) {
-        __syncthreads();
+        __syncthreads();   // (every warp is done with its value tile: the flush buffer lies over the tiles)
 #pragma unroll
-        for (int b = 0; b < NBLK; ++b)
-            red[warp * 32 * NBLK + 32 * b + lane] = data ? log(accv[b]) + (double)accx[b] * LN2 : accv[b];
+        for (int c = 0; c < NCH; ++c) {
+            // lane l holds value 8 c + l % 8 over a quarter of the warp's events: the four quarters in a fixed order
+            double t = data ? log(accv[c]) + (double)accx[c] * LN2 : accv[c];
+            t += __shfl_xor_sync(0xffffffffu, t, 8);
+            t += __shfl_xor_sync(0xffffffffu, t, 16);
+            if (lane < 8) red[warp * NVP + 8 * c + lane] = t;
+        }
 #pragma unroll
-        for (int b = 0; b < NBLK; ++b) accv[b] = 0.0;   // (after the data flush: the sums of the normalisation units start)
+        for (int c = 0; c < NCH; ++c) { accv[c] = 0.0; accx[c] = 0; }   // (after the data flush: the sums of the normalisation units start)
         __syncthreads();
         for (int idx = tid; idx < NVAL; idx += THREADS) {
             double s = 0.0;
-            for (int wv = 0; wv < NWARPS; ++wv) s += red[wv * 32 * NBLK + idx];
+            for (int wv = 0; wv < NWARPS; ++wv) s += red[wv * NVP + idx];
             d.partial[(size_t)(row0 + idx) * d.stride + blockIdx.x] = s;
         }
         __syncthreads();
@@ -477,8 +485,15 @@ __global__ void __launch_bounds__(THREADS, DELTAF_MINB) k_deltaf(const __grid_co
             }
             tree.pad_block();
         };
-        if (is_norm) all_values(tn, true);
-        else all_values(td, false);
+        if (is_norm) {
+            all_values(tn, true);
+        } else {
+            all_values(td, false);
+            if ((k & 15) == 15) {   // the products of r in [0.5, 1.5] (eight per unit and chunk) back to [0.5, 1)
+#pragma unroll
+                for (int c = 0; c < NCH; ++c) { int e; split_exp(accv[c], &accv[c], &e); accx[c] += e; }
+            }
+        }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[s]);   // this warp has read everything it needs from the stage
     }
@@ -503,7 +518,7 @@ __global__ void __launch_bounds__(THREADS, DELTAF_MINB) k_deltaf(const __grid_co
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    double* tot = red;   // 2 + 2 NVAL totals (NWARPS * 32 * NBLK >= that)
+    double* tot = red;   // 2 + 2 NVAL totals (the tiles are larger)
     constexpr int ROWS = 2 + 2 * NVAL;
     for (int r = tid; r < ROWS; r += THREADS) {
         const double* p = d.partial + (size_t)r * d.stride;
@@ -543,12 +558,12 @@ namespace {
 
 template <class SH>
 size_t deltaf_smem(int ncolw) {
-    return (size_t)NSTAGE * ncolw * UNIT * sizeof(double) + (size_t)NWARPS * 32 * DLay<SH>::NBLK * sizeof(double) + 2 * NSTAGE * sizeof(uint64_t);
+    return (size_t)NSTAGE * ncolw * UNIT * sizeof(double) + (size_t)NWARPS * TILE_BYTES + 2 * NSTAGE * sizeof(uint64_t);
 }
 
 template <class SH>
 cudaError_t launch_deltaf_shape(const DeltaFArgs& d, int grid, cudaStream_t s) {
-    static_assert(NWARPS * 32 * DLay<SH>::NBLK >= 2 + 2 * DLay<SH>::NVAL, "the finish reuses the flush buffer");
+    static_assert(NWARPS * TILE_BYTES / 8 >= 2 + 2 * DLay<SH>::NVAL && TILE_BYTES / 8 >= 8 * DLay<SH>::NCH, "the flush and the finish reuse the value tiles");
     static DeviceOnce attr_done;
     cudaError_t e = cudaSuccess;
     if (attr_done.first()) { e = cudaFuncSetAttribute(k_deltaf<SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024); }
