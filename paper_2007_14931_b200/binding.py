@@ -177,7 +177,7 @@ class Model:
             c = c[None]
         P = c.shape[0]
         assert c.shape == (P, self.K), f"couplings must be [P][{self.K}]"
-        hc = np.ascontiguousarray(np.stack([c.real, c.imag], -1), dtype=np.float64)
+        hc = np.ascontiguousarray(c, dtype=np.complex128).view(np.float64)      # [P][K][re, im]
         pmw = None
         if mass_width is not None:
             hmw = np.ascontiguousarray(mass_width, dtype=np.float64)

@@ -359,7 +359,8 @@ struct DeltaFArgs {
     int P;
     double* partial;                              // [2 + 2 NVAL][stride] per-CTA partials
     int stride;
-    double* result;                               // [4 P + 1]: NLL[P], I[P], domain flag, sum log S [P], sum w S [P] (as DeltaArgs)
+    double* result;                               // [4 P + 2]: NLL[P], I[P], domain flag, sum log S [P], sum w S [P] (as DeltaArgs), stamp; may be mapped HOST memory
+    double seq;                                   // written to result[4 P + 1] after a system-wide fence once the rest is in place
     int want_nll;
 };
 cudaError_t launch_deltaf(const DeltaFArgs& d, int grid, cudaStream_t s);

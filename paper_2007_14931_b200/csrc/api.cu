@@ -63,6 +63,8 @@ struct amp_model {
     double* h_pinned = nullptr;    // same layout
     double* h_zc = nullptr;        // [8] mapped pinned host memory: the fused step's kernel writes its result block here (zero copy)
     double zc_seq = 0;             // stamp of the last fused launch
+    double* h_zcb = nullptr;       // [4 AMP_MAX_POINTS + 2] the same for the gradient-batch kernel's result block (deltaf.cu)
+    double zcb_seq = 0;
     bool zero_copy = true;
     std::vector<double> last_slog, last_swS;   // the two sums of the last amp_nll, per point (amp_nll_terms)
 
@@ -107,6 +109,8 @@ struct amp_model {
     int ring_last = -1;
     long long ring_calls = 0;      // such evaluations since amp_model_create (amp_recent_launch_ms)
     bool use_delta = false;        // P > 1 and the points are sparse changes of point 0: gradient-batch kernel (delta.cu)
+    bool delta_plan_built = false; // delta_chunks hold the program of the current points (compiled lazily when k_deltaf takes the batch)
+    bool no_deltaf_once = false;   // amp_set_params called again by evaluate(): the specialised kernel is not to be planned
     struct DeltaChunk { int p0, np, nsorted; std::vector<DeltaContrib> contrib; std::vector<double> slots; };
     std::vector<DeltaChunk> delta_chunks;     // compiled program of the last amp_set_params (points p0 .. p0 + np - 1 per launch)
     bool use_deltaf = false;       // ... and every point is ONE coupling or ONE lineshape change of the paper's resonance lists: deltaf.cu
@@ -350,6 +354,8 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
     if (e == cudaSuccess) e = cudaMallocHost(&m->h_pinned, sizeof(double) * (4 * AMP_MAX_POINTS + 4));
     if (e == cudaSuccess) e = cudaHostAlloc(&m->h_zc, sizeof(double) * 8, cudaHostAllocMapped);
     if (e == cudaSuccess) { std::memset(m->h_zc, 0, sizeof(double) * 8); m->zero_copy = true; }
+    if (e == cudaSuccess) e = cudaHostAlloc(&m->h_zcb, sizeof(double) * (4 * AMP_MAX_POINTS + 2), cudaHostAllocMapped);
+    if (e == cudaSuccess) std::memset(m->h_zcb, 0, sizeof(double) * (4 * AMP_MAX_POINTS + 2));
     for (int i = 0; i < 5 && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ev[i]);
     for (int i = 0; i < 2 * amp_model::RING && e == cudaSuccess; ++i) e = cudaEventCreate(&m->ring[i]);
     if (e != cudaSuccess) { amp_model_destroy(m); return e == cudaErrorMemoryAllocation ? AMP_ERR_NOMEM : AMP_ERR_CUDA; }
@@ -371,6 +377,7 @@ amp_status amp_model_destroy(amp_model* m) {
     free_toy_scratch(m);
     if (m->h_pinned) cudaFreeHost(m->h_pinned);
     if (m->h_zc) cudaFreeHost(m->h_zc);
+    if (m->h_zcb) cudaFreeHost(m->h_zcb);
     if (m->d_plan) cudaFree(m->d_plan);
     if (m->h_plan) cudaFreeHost(m->h_plan);
     if (m->d_G) cudaFree(m->d_G);
@@ -768,9 +775,12 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
         for (int r = 0; r < R; ++r) {
             double mass = m->res[r].mass, width = m->res[r].width;
             if (h_mass_width && m->res[r].kind != AMP_CONST) { mass = h_mass_width[((size_t)p * R + r) * 2]; width = h_mass_width[((size_t)p * R + r) * 2 + 1]; }
-            LineConst lc;
-            if (!std::isfinite(mass) || !std::isfinite(width)) return fail(m, AMP_ERR_INVALID, "amp_set_params: non-finite mass or width");
-            if (!make_line_const(m, r, mass, width, &lc)) return fail(m, AMP_ERR_DOMAIN, "amp_set_params: pole mass outside the kinematic range or width <= 0");
+            // (a gradient batch repeats point 0's masses and widths in all but a few points: those are checked once)
+            if (p == 0 || mass != mw[(size_t)r * 2] || width != mw[(size_t)r * 2 + 1]) {
+                LineConst lc;
+                if (!std::isfinite(mass) || !std::isfinite(width)) return fail(m, AMP_ERR_INVALID, "amp_set_params: non-finite mass or width");
+                if (!make_line_const(m, r, mass, width, &lc)) return fail(m, AMP_ERR_DOMAIN, "amp_set_params: pole mass outside the kinematic range or width <= 0");
+            }
             mw[((size_t)p * R + r) * 2] = mass;
             mw[((size_t)p * R + r) * 2 + 1] = width;
         }
@@ -789,10 +799,13 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
     // P > 1: a batch whose points are sparse changes of point 0 (a gradient step) runs the delta kernel: no column, no matrix
     if (m->has_bkg && P > 1) m->want_matrix = false;   // Eq. 14: the background path streams both samples, point by point (a single
                                                           // point at fixed lineshapes may still hold M: amp_nll_grad reads it)
-    m->use_delta = P > 1 && !m->has_bkg && (m->batch_mode == 0 || m->batch_mode == 3) && m->lineshape_mode != 1 && m->norm_mode != 2 && build_delta_plan(m);
+    // ... through the shape-specialised kernel where every point is one coupling or one lineshape change (batch mode 3: never);
+    // the general kernel's program is then compiled only if a call needs it (the guard on r tripped)
+    const bool sparse_ok = P > 1 && !m->has_bkg && (m->batch_mode == 0 || m->batch_mode == 3) && m->lineshape_mode != 1 && m->norm_mode != 2;
+    m->use_deltaf = sparse_ok && m->batch_mode == 0 && !m->no_deltaf_once && build_deltaf_plan(m);
+    m->delta_plan_built = false;
+    m->use_delta = m->use_deltaf || (sparse_ok && (m->delta_plan_built = build_delta_plan(m)));
     if (m->use_delta) m->want_matrix = false;
-    // ... through the shape-specialised kernel where every point is one coupling or one lineshape change (batch mode 3: never)
-    m->use_deltaf = m->use_delta && m->batch_mode == 0 && build_deltaf_plan(m);
     m->stream_inline = (P == 1 || m->use_delta || m->has_bkg) && m->lineshape_mode != 1;
 
     // distinct (resonance, mass, width) keys of this call
@@ -1399,9 +1412,8 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         return AMP_OK;
     }
     bool deltaf_tripped = false;
-    if (m->use_deltaf && (!want_nll || m->data.n <= 600LL * 256 * deltaf_grid(m->data.n, m->norm.n))) {
+    if (m->use_deltaf) {
         // Gradient batch of the paper's resonance lists: ONE launch of the shape-specialised kernel (deltaf.cu) for all points.
-        // (Per thread the data-side products of r in [0.5, 1.5] run over at most 600 events: far inside the FP64 range.)
         DeltaFArgs& d = m->deltaf;
         fill_stream_args(m, m->data, 0, MODE_FUSED, &d.a);
         d.a.cache2 = m->norm.cache; d.a.n2 = m->norm.n; d.a.npad2 = m->norm.npad;
@@ -1412,25 +1424,40 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         d.P = P;
         d.partial = m->d_partial;
         d.stride = PARTIAL_STRIDE;
-        d.result = m->d_result;
         d.want_nll = want_nll ? 1 : 0;
+        // Result block [4 P + 2]: as for the fused step, mapped host memory that the last CTA fills and stamps (the host spins on the
+        // stamp: no D2H copy, no stream-synchronise wake-up)
+        const double* res = m->h_pinned;
+        if (m->zero_copy) { m->zcb_seq += 1.0; d.result = m->h_zcb; d.seq = m->zcb_seq; res = m->h_zcb; }
+        else { d.result = m->d_result; d.seq = 0.0; }
         m->ring_last = (m->ring_last + 1) % amp_model::RING;
         m->ring_calls++;
         CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
         CK(launch_deltaf(d, deltaf_grid(d.a.n, d.a.n2), s));
         CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
-        CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (4 * P + 1), cudaMemcpyDeviceToHost, s));
-        CK(cudaStreamSynchronize(s));
+        if (m->zero_copy) {
+            volatile double* stamp = m->h_zcb + 4 * P + 1;
+            for (unsigned spins = 0; *stamp != m->zcb_seq; ++spins) {
+                if ((spins & 0x3fff) == 0x3fff) {   // every 16k spins: has the stream failed or finished without the stamp?
+                    const cudaError_t q = cudaStreamQuery(s);
+                    if (q != cudaErrorNotReady) { if (q != cudaSuccess) return cuda_fail(m, q, "gradient batch"); if (*stamp == m->zcb_seq) break; return fail(m, AMP_ERR_CUDA, "gradient batch finished without a result"); }
+                }
+            }
+            std::atomic_thread_fence(std::memory_order_acquire);
+        } else {
+            CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (4 * P + 1), cudaMemcpyDeviceToHost, s));
+            CK(cudaStreamSynchronize(s));
+        }
         m->stat_launches = 1;
-        if (m->h_pinned[2 * P] < 1024.0) {
-            m->last_slog.assign(m->h_pinned + 2 * P + 1, m->h_pinned + 3 * P + 1);
-            m->last_swS.assign(m->h_pinned + 3 * P + 1, m->h_pinned + 4 * P + 1);
+        if (res[2 * P] < 1024.0) {
+            m->last_slog.assign(res + 2 * P + 1, res + 3 * P + 1);
+            m->last_swS.assign(res + 3 * P + 1, res + 4 * P + 1);
             m->stat_norm_path = 9;
             m->fused_valid = true;
-            bool bad = m->h_pinned[2 * P] != 0.0;
+            bool bad = res[2 * P] != 0.0;
             for (int p = 0; p < P; ++p) {
-                if (h_nll) { h_nll[p] = m->h_pinned[p]; bad |= !std::isfinite(h_nll[p]); }
-                if (h_I) { h_I[p] = m->h_pinned[P + p]; bad |= !(h_I[p] > 0) || !std::isfinite(h_I[p]); }
+                if (h_nll) { h_nll[p] = res[p]; bad |= !std::isfinite(h_nll[p]); }
+                if (h_I) { h_I[p] = res[P + p]; bad |= !(h_I[p] > 0) || !std::isfinite(h_I[p]); }
             }
             if (bad) return fail(m, AMP_ERR_DOMAIN, "non-finite or non-positive PDF value");
             return AMP_OK;
@@ -1440,6 +1467,19 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         deltaf_tripped = true;
         m->ring_calls--;
         m->ring_last = (m->ring_last + amp_model::RING - 1) % amp_model::RING;
+    }
+    if (m->use_delta && !m->delta_plan_built) {
+        if (build_delta_plan(m)) {
+            m->delta_plan_built = true;
+        } else {
+            // a batch the specialised kernel accepted but the general one cannot compile: plan the call again without the former
+            const std::vector<double> c = m->couplings, w = m->mw;
+            m->no_deltaf_once = true;
+            const amp_status rs = amp_set_params(m, P, c.data(), w.data());
+            m->no_deltaf_once = false;
+            if (rs != AMP_OK) return rs;
+            return evaluate(m, want_nll, h_nll, h_I, s);
+        }
     }
     if (m->use_delta) {
         // Gradient batch: one fused launch per chunk of <= 128 points besides point 0 (delta.cu)

@@ -548,9 +548,14 @@ __global__ void __launch_bounds__(THREADS, DELTAF_MINB) k_deltaf(const __grid_co
         if (!isfinite(nll) || !(I > 0.0)) nll = INFINITY;
         d.result[p] = d.want_nll ? nll : 0.0;
     }
+    // the result block may live in mapped host memory: every writer's values are in place system-wide before the stamp goes out
+    __threadfence_system();
+    __syncthreads();
     if (tid == 0) {
         d.result[2 * d.P] = (double)atomicExch(a.flag, 0);   // domain flag of this launch, cleared for the next one
         *a.ticket = 0u;
+        __threadfence_system();
+        *reinterpret_cast<volatile double*>(d.result + 4 * d.P + 1) = d.seq;
     }
 }
 
