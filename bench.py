@@ -59,6 +59,12 @@ DELTA_FLOP_PER_NORM_EVENT = 730.0 + 31 * 65.0 + 25 * 6.0 + 20 * 33.0
 # sums (3) + per floating lineshape (5): Q (22), G and n_R (44), four points x (BW(p) 12, Delta 4, |Delta|^2 3, x 6, exchange 1)
 DELTAF_FLOP_PER_EVENT = 730.0 + 190.0 + 154.0 + 25 * 40.0 + 5 * 170.0
 DELTAF_FLOP_PER_NORM_EVENT = 730.0 + 190.0 + 154.0 + 25 * 11.0 + 5 * 170.0
+# The same batch as three launches (batch mode 0: deltan.cu pass 0 and pass 1 over the normalisation events, then deltaf.cu over the
+# data events; DESIGN.md 5.6a/5.6b): FP64 operations EXECUTED per event (DFMA = 2, DMUL / DADD / MUFU = 1), read off the instruction
+# counts of the ncu source page of profiles/r02_ncu_full_deltaf3.csv's report — both passes carry the forward pass of point 0.
+DELTAN0_FLOP_PER_NORM_EVENT = 1019.0
+DELTAN1_FLOP_PER_NORM_EVENT = 1705.0
+DELTAF_DATA_FLOP_PER_EVENT = 3136.0
 # analytic gradient: the point (730) + per coupling slot: angular factor ~8, T = sum_xi conj(g) A 16, conj(BW) T 8, weight 2
 GRAD_FLOP_PER_EVENT = 730.0 + 27 * 34.0
 # its shape-specialised form (gradf.cu): the point (730) + the three W_lambda and three Y_lambda' (u A, conj(g) A:
@@ -282,11 +288,40 @@ def roofline(model, args, cfg, n_data, n_norm, hbm_peak, peak_kind):
         phase = {"lineshape": tm["lineshape_ms"], "data": tm["data_ms"], "norm": tm["norm_ms"]}
     k_ms, k_med = float(np.mean(t_k)), float(np.median(t_k))
     nbytes = BYTES_PER_EVENT_DATA * n_data + BYTES_PER_EVENT_NORM * n_norm
-    if cfg == 4 and path == 9:
-        # gradient batch of the paper's resonance lists: ONE k_deltaf launch per step, bound by the plain FP64 ALUs
+    if cfg == 4 and path == 9 and st["launches"] == 3:
+        # gradient batch of the paper's resonance lists: k_deltan pass 0, pass 1 (normalisation events), k_deltaf (data events) per step,
+        # all bound by the plain FP64 ALUs (DESIGN.md 5.6a/b).  The ring times the three together; the last step's event split gives the shares.
+        tm = model.last_call_timing()
+        parts = [("k_deltan<pass 0> (normalisation events: sum w S0 and the 54 sums of L', registers)", tm["norm_ms"], DELTAN0_FLOP_PER_NORM_EVENT, n_norm, "k_deltan0_cfg4"),
+                 ("k_deltan<pass 1> (normalisation events: sums of n' and the lineshape sums, registers; scatters the totals)", tm["final_ms"], DELTAN1_FLOP_PER_NORM_EVENT, n_norm, "k_deltan1_cfg4"),
+                 ("k_deltaf (data events: r = S(p)/S(0) of 120 points through the shared-memory value tile; forms NLL(p), I(p))", tm["data_ms"], DELTAF_DATA_FLOP_PER_EVENT, n_data, "k_deltaf_cfg4")]
+        tsum = sum(p[1] for p in parts)
+        peak = FP64_PEAK_NOMINAL / 1e12
+        launches = []
+        for name, ms, fpe, nev, key in parts:
+            ms_avg = ms / tsum * k_ms                      # this launch's share of the last step x the mean over the timed steps
+            traffic, tsrc = traffic_from_profiles(key, n_data, n_norm)
+            launches.append({"kernel": name, "kernel_ms": ms_avg, "flop_per_event": fpe, "events": nev, "achieved": fpe * nev / (ms_avg * 1e-3) / 1e12,
+                             "frac": fpe * nev / (ms_avg * 1e-3) / 1e12 / peak, "traffic": traffic, "traffic_source": tsrc})
+        dom = max(launches, key=lambda l: l["kernel_ms"])
+        flop = sum(l["flop_per_event"] * l["events"] for l in launches)
+        flop1 = DELTAF_FLOP_PER_EVENT * n_data + DELTAF_FLOP_PER_NORM_EVENT * n_norm
+        roof = {"bound": "alu", "kernel": dom["kernel"], "achieved": dom["achieved"], "peak": peak,
+                "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md 6; the DFMA probe below measures it)", "unit": "TFLOP/s",
+                "frac": dom["frac"], "traffic": dom["traffic"], "traffic_source": dom["traffic_source"], "kernel_ms": dom["kernel_ms"],
+                "flop_per_event": dom["flop_per_event"], "flop_per_launch": dom["flop_per_event"] * dom["events"],
+                "flop_note": "FP64 operations executed per event (DFMA = 2), from the ncu source page; the longest of the step's three launches",
+                "step": {"kernel_ms": k_ms, "kernel_ms_median": k_med, "launches": launches, "flop": flop, "achieved": flop / (k_ms * 1e-3) / 1e12,
+                         "frac": flop / (k_ms * 1e-3) / 1e12 / peak,
+                         "frac_at_one_launch_flop": flop1 / (k_ms * 1e-3) / 1e12 / peak,
+                         "note": "frac: the three launches' executed flop (both normalisation passes carry the forward pass of point 0) over their total time; "
+                                 "frac_at_one_launch_flop: the algorithmic flop of the one-launch form (batch mode 4) over the same time",
+                         "hbm_frac": (nbytes + BYTES_PER_EVENT_NORM * n_norm) / (k_ms * 1e-3) / 1e9 / hbm_peak}}
+    elif cfg == 4 and path == 9:
+        # ... as ONE k_deltaf launch over both samples (batch mode 4)
         flop = DELTAF_FLOP_PER_EVENT * n_data + DELTAF_FLOP_PER_NORM_EVENT * n_norm
         ach = flop / (k_ms * 1e-3) / 1e12
-        traffic, tsrc = traffic_from_profiles("k_deltaf_cfg4", n_data, n_norm)
+        traffic, tsrc = traffic_from_profiles("k_deltaf1_cfg4", n_data, n_norm)
         roof = {"bound": "alu", "kernel": "k_deltaf (shape-specialised gradient batch: point 0 + 100 coupling points + 20 mass/width points, data then norm units, one launch)",
                 "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12,
                 "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md 6; the DFMA probe below measures it)", "unit": "TFLOP/s",
@@ -395,6 +430,8 @@ def run_own(args):
     model, c, info = build_workload(args, device)
     if args.dense:
         model.set_batch_mode(2)   # configs[4] as the dense DMMA contraction + extended-basis normalisation matrix
+    if args.one_launch:
+        model.set_batch_mode(4)   # configs[4] as ONE k_deltaf launch over both samples (the cross-check form of the three-launch default)
     if args.general:
         model.set_batch_mode(3)   # configs[4] through the general gradient-batch kernel (k_delta) instead of the shape-specialised one
     sampler = ClockSampler(local)
@@ -405,7 +442,7 @@ def run_own(args):
     main = measure(model, args, args.cfg, c, args.steps, args.warmup, world, device, sampler if rank == 0 else None, args.n_data, args.n_norm, hbm)
     # the default run: configs[4] (P = 121) on the same loaded events, in the same line
     cfg4 = None
-    if args.cfg == 3 and not (args.grad or args.lass or args.dense or args.general or args.no_cfg4):
+    if args.cfg == 3 and not (args.grad or args.lass or args.dense or args.general or args.one_launch or args.no_cfg4):
         steps4 = max(20, min(args.steps, 50))
         cfg4 = measure(model, args, 4, W.couplings(4), steps4, 3, world, device, sampler if rank == 0 else None, args.n_data, args.n_norm, hbm)
     sweep = None
@@ -695,6 +732,7 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="also time the six configs[3] points {1M, 2M, 8M} data x {2M, 10M} normalisation events (\"sweep\" in the line)")
     ap.add_argument("--shard", action="store_true", help="strong scaling: ONE data set cut over the ranks (ShardedModel), the all-reduce on NCCL inside the timed step")
     ap.add_argument("--dense", action="store_true", help="--cfg 4 through the dense DMMA contraction instead of the gradient-batch kernel")
+    ap.add_argument("--one-launch", action="store_true", help="configs[4] as one k_deltaf launch over both samples instead of k_deltan x 2 + k_deltaf")
     ap.add_argument("--general", action="store_true", help="configs[4] through the general gradient-batch kernel (k_delta) instead of the shape-specialised k_deltaf")
     ap.add_argument("--grad", action="store_true", help="--cfg 3 steps that also return the analytic gradient in all couplings (amp_nll_grad)")
     ap.add_argument("--lass", action="store_true", help="configs[3] call pattern on the LASS variant of the model (Eqs. 7-9; SURVEY.md 8(f)-1)")

@@ -265,9 +265,10 @@ amp_status amp_set_lineshape_mode(amp_model* m, int mode);
  * gradient-batch kernels (dense DMMA contraction even for sparse batches).  3 = as 0 without the shape-specialised form of the
  * gradient-batch kernel.  Under 0, a sparse batch of the paper's resonance lists (ten K* with zero to two 1+ Z's, one radius
  * per spin) in which every point is ONE coupling change (a single slot, or a Z's helicities -1 and +1 moving together, Eq. 11)
- * or ONE mass / width change, at most four per slot / resonance — MINUIT's gradient step — runs that form: one launch for all
- * points, exact, S(p) / S(0) formed directly; a step so large that the ratio leaves [0.5, 1.5] at some event repeats the call
- * through the general kernel.                                                                                       */
+ * or ONE mass / width change, at most four per slot / resonance — MINUIT's gradient step — runs that form: three launches for all
+ * points (two passes over the normalisation events, whose sums do not depend on the point, then the data events), exact, S(p) / S(0) formed
+ * directly; a step so large that the ratio leaves [0.5, 1.5] at some event repeats the call through the general kernel.
+ * 4 = as 0 with that form as ONE launch over both samples (the cross-check of the two-launch form).                   */
 amp_status amp_set_batch_mode(amp_model* m, int mode);
 /* How a P == 1 step with lineshapes in registers and a direct-sum normalisation is launched: 0 = automatic (ONE fused
  * launch: data tiles, then normalisation tiles, the last thread block forms the NLL), 1 = separate data / normalisation /
@@ -287,7 +288,8 @@ amp_status amp_last_call_stats(const amp_model* m, int* launches, int* columns_r
 /* Device time [ms] of the phases of the last amp_nll / amp_norm_integral call, from CUDA events recorded on
  * the call's stream: ms4[0] lineshape columns, ms4[1] data-side combine + reduce, ms4[2] normalisation,
  * ms4[3] final reductions and the copy of the result.  After a fused single launch (path 4): ms4[1] = that launch,
- * the others 0.                                                                                          */
+ * the others 0.  After the three launches of a shape-specialised gradient batch (path 9, batch mode 0): ms4[2], ms4[3] = the
+ * two passes over the normalisation events, ms4[1] = the data events, ms4[0] = 0.                          */
 amp_status amp_last_call_timing(const amp_model* m, double* ms4);
 
 /* Device time [ms] of the launches of the most recent single-launch evaluations (paths 4 and 5), from CUDA event pairs

@@ -362,9 +362,17 @@ struct DeltaFArgs {
     double* result;                               // [4 P + 2]: NLL[P], I[P], domain flag, sum log S [P], sum w S [P] (as DeltaArgs), stamp; may be mapped HOST memory
     double seq;                                   // written to result[4 P + 1] after a system-wide fence once the rest is in place
     int want_nll;
+    // The normalisation events in a kernel of their own (deltan.cu; launched first on the same stream): its per-CTA partials,
+    // the totals its last CTA leaves — [0] sum w S0, [1 + v] the normalisation-side value row v of k_deltaf's layout — and the
+    // layout it scatters them by.  norm_tot == nullptr: k_deltaf walks the normalisation events itself.
+    double* npartial;                             // [1 + 2 NSLOT + 8 NENT][stride]
+    double* norm_tot;                             // [1 + NVAL]
+    short quad_of_pos[DELTAF_MAX_POS], quad_of_ent[DELTAF_MAX_ENT];
 };
 cudaError_t launch_deltaf(const DeltaFArgs& d, int grid, cudaStream_t s);
 int deltaf_grid(long long n_data, long long n_norm);
+cudaError_t launch_deltan(const DeltaFArgs& d, int grid, int pass, cudaStream_t s);
+int deltan_grid(long long n_norm);
 struct DeltaFLayout { int nslot, npos, nent, nquad; int quad_of_pos[DELTAF_MAX_POS], quad_of_ent[DELTAF_MAX_ENT]; };
 bool deltaf_layout(const StreamArgs& a, DeltaFLayout* lay);   // false: not one of the compiled shapes
 

@@ -63,6 +63,8 @@ struct amp_model {
     double* h_pinned = nullptr;    // same layout
     double* h_zc = nullptr;        // [8] mapped pinned host memory: the fused step's kernel writes its result block here (zero copy)
     double zc_seq = 0;             // stamp of the last fused launch
+    double* d_npartial = nullptr;  // [DELTAN_MAX_ROWS][PARTIAL_STRIDE] per-CTA partials of k_deltan (deltan.cu)
+    double* d_ntot = nullptr;      // [1 + NVAL] its totals, read by k_deltaf's finish
     double* h_zcb = nullptr;       // [4 AMP_MAX_POINTS + 2] the same for the gradient-batch kernel's result block (deltaf.cu)
     double zcb_seq = 0;
     bool zero_copy = true;
@@ -103,6 +105,7 @@ struct amp_model {
     int stat_launches = 0, stat_columns = 0, stat_norm_path = 0, stat_batched = 0, stat_gram_built = 0;
     cudaEvent_t ev[5]{};           // phase boundaries of the last evaluation (amp_last_call_timing)
     bool ev_valid = false;
+    bool split_valid = false;      // ... of the gradient batch's three launches: ev[1], ev[2] lie between them
     bool fused_valid = false;      // the last evaluation was one fused launch (or the gradient-batch launches): ring[ring_last] brackets it
     enum { RING = 256 };
     cudaEvent_t ring[2 * RING]{};  // event pairs around the launches of the fused / gradient-batch evaluations, newest at ring_last
@@ -127,6 +130,7 @@ struct amp_model {
 namespace {
 
 enum { PARTIAL_STRIDE = 2048 };
+enum { DELTAN_MAX_ROWS = 1 + 2 * DELTAF_MAX_POS + 8 * DELTAF_MAX_ENT };   // k_deltan: sum w S0, the leaves, eight tile values per entry
 
 amp_status fail(amp_model* m, amp_status s, const std::string& msg) {
     if (m) m->err = msg;
@@ -348,6 +352,8 @@ amp_status amp_model_create(const amp_decay* decay, const amp_resonance* res, in
     if (e == cudaSuccess) e = cudaMalloc(&m->d_sums, sizeof(double) * 2 * AMP_MAX_POINTS);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_result, sizeof(double) * (4 * AMP_MAX_POINTS + 4));
     if (e == cudaSuccess) e = cudaMalloc(&m->d_flag, sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_npartial, sizeof(double) * DELTAN_MAX_ROWS * PARTIAL_STRIDE);
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_ntot, sizeof(double) * (1 + 4 * (DELTAF_MAX_POS + DELTAF_MAX_ENT)));
     if (e == cudaSuccess) e = cudaMalloc(&m->d_ticket, sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(m->d_ticket, 0, sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(m->d_flag, 0, sizeof(int));
@@ -378,6 +384,8 @@ amp_status amp_model_destroy(amp_model* m) {
     if (m->h_pinned) cudaFreeHost(m->h_pinned);
     if (m->h_zc) cudaFreeHost(m->h_zc);
     if (m->h_zcb) cudaFreeHost(m->h_zcb);
+    if (m->d_npartial) cudaFree(m->d_npartial);
+    if (m->d_ntot) cudaFree(m->d_ntot);
     if (m->d_plan) cudaFree(m->d_plan);
     if (m->h_plan) cudaFreeHost(m->h_plan);
     if (m->d_G) cudaFree(m->d_G);
@@ -438,7 +446,7 @@ amp_status amp_set_norm_mode(amp_model* m, int mode) {
 }
 
 amp_status amp_set_batch_mode(amp_model* m, int mode) {
-    if (!m || mode < 0 || mode > 3) return AMP_ERR_INVALID;
+    if (!m || mode < 0 || mode > 4) return AMP_ERR_INVALID;
     m->batch_mode = mode;
     return AMP_OK;
 }
@@ -477,6 +485,13 @@ amp_status amp_last_call_timing(const amp_model* m, double* ms4) {
         cudaEventSynchronize(m->ring[2 * m->ring_last + 1]);   // (a zero-copy call returns before its end event has landed)
         if (cudaEventElapsedTime(&t, m->ring[2 * m->ring_last], m->ring[2 * m->ring_last + 1]) != cudaSuccess) return AMP_ERR_CUDA;
         ms4[0] = 0; ms4[1] = t; ms4[2] = 0; ms4[3] = 0;
+        if (m->split_valid && m->stat_norm_path == 9) {   // normalisation pass 0, pass 1, then the data events
+            float t0 = 0, t1 = 0, t2 = 0;
+            if (cudaEventElapsedTime(&t0, m->ring[2 * m->ring_last], m->ev[1]) != cudaSuccess || cudaEventElapsedTime(&t1, m->ev[1], m->ev[2]) != cudaSuccess ||
+                cudaEventElapsedTime(&t2, m->ev[2], m->ring[2 * m->ring_last + 1]) != cudaSuccess)
+                return AMP_ERR_CUDA;
+            ms4[1] = t2; ms4[2] = t0; ms4[3] = t1;
+        }
         return AMP_OK;
     }
     if (!m->ev_valid) return AMP_ERR_STATE;
@@ -690,6 +705,8 @@ bool build_deltaf_plan(amp_model* m) {
     DeltaFLayout lay;
     if (!deltaf_layout(d.a, &lay)) return false;
     const int nslot = lay.nslot, nent = lay.nent;
+    for (int i = 0; i < DELTAF_MAX_POS; ++i) d.quad_of_pos[i] = (short)(i < lay.npos ? lay.quad_of_pos[i] : 0);
+    for (int i = 0; i < DELTAF_MAX_ENT; ++i) d.quad_of_ent[i] = (short)(i < lay.nent ? lay.quad_of_ent[i] : 0);
     const int n0 = d.a.shape[0];
     auto base = [&](int t) { return t < n0 ? t : n0 + 3 * (t - n0); };
     std::memset(d.cq, 0, sizeof(d.cq));
@@ -801,8 +818,8 @@ extern "C" amp_status amp_set_params(amp_model* m, int P, const double* h_coupli
                                                           // point at fixed lineshapes may still hold M: amp_nll_grad reads it)
     // ... through the shape-specialised kernel where every point is one coupling or one lineshape change (batch mode 3: never);
     // the general kernel's program is then compiled only if a call needs it (the guard on r tripped)
-    const bool sparse_ok = P > 1 && !m->has_bkg && (m->batch_mode == 0 || m->batch_mode == 3) && m->lineshape_mode != 1 && m->norm_mode != 2;
-    m->use_deltaf = sparse_ok && m->batch_mode == 0 && !m->no_deltaf_once && build_deltaf_plan(m);
+    const bool sparse_ok = P > 1 && !m->has_bkg && (m->batch_mode == 0 || m->batch_mode == 3 || m->batch_mode == 4) && m->lineshape_mode != 1 && m->norm_mode != 2;
+    m->use_deltaf = sparse_ok && m->batch_mode != 3 && !m->no_deltaf_once && build_deltaf_plan(m);
     m->delta_plan_built = false;
     m->use_delta = m->use_deltaf || (sparse_ok && (m->delta_plan_built = build_delta_plan(m)));
     if (m->use_delta) m->want_matrix = false;
@@ -1433,8 +1450,22 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
         m->ring_last = (m->ring_last + 1) % amp_model::RING;
         m->ring_calls++;
         CK(cudaEventRecord(m->ring[2 * m->ring_last], s));
+        // The normalisation events in kernels of their own first (deltan.cu: their sums do not depend on the point and live in
+        // registers there, two passes), then the data events; the last launch's last CTA forms NLL(p), I(p) from all.  Batch mode 4: one launch.
+        const bool split = m->batch_mode != 4 && m->norm.n > 0;
+        d.npartial = m->d_npartial;
+        d.norm_tot = split ? m->d_ntot : nullptr;
+        if (split) {
+            CK(launch_deltan(d, deltan_grid(d.a.n2), 0, s));
+            CK(cudaEventRecord(m->ev[1], s));
+            CK(launch_deltan(d, deltan_grid(d.a.n2), 1, s));
+            CK(cudaEventRecord(m->ev[2], s));
+            d.a.n2 = 0;
+        }
         CK(launch_deltaf(d, deltaf_grid(d.a.n, d.a.n2), s));
         CK(cudaEventRecord(m->ring[2 * m->ring_last + 1], s));
+        m->split_valid = split;
+        m->stat_launches = split ? 3 : 1;
         if (m->zero_copy) {
             volatile double* stamp = m->h_zcb + 4 * P + 1;
             for (unsigned spins = 0; *stamp != m->zcb_seq; ++spins) {
@@ -1448,7 +1479,6 @@ amp_status evaluate(amp_model* m, bool want_nll, double* h_nll, double* h_I, cud
             CK(cudaMemcpyAsync(m->h_pinned, m->d_result, sizeof(double) * (4 * P + 1), cudaMemcpyDeviceToHost, s));
             CK(cudaStreamSynchronize(s));
         }
-        m->stat_launches = 1;
         if (res[2 * P] < 1024.0) {
             m->last_slog.assign(res + 2 * P + 1, res + 3 * P + 1);
             m->last_swS.assign(res + 3 * P + 1, res + 4 * P + 1);

@@ -211,7 +211,7 @@ def test_nll_batched_points_small():
     ref, refI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
     assert nll.shape == (121,)
     st = Mg.last_call_stats()
-    assert st["norm_path"] == 9 and st["launches"] == 1     # shape-specialised gradient-batch kernel: one fused launch, no columns, no matrix
+    assert st["norm_path"] == 9 and st["launches"] == 3     # shape-specialised gradient-batch kernels (normalisation events twice, then data events): no columns, no matrix
     assert st["columns_recomputed"] == 0
     assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
     assert np.array_equal(Mg.nll(), nll)                     # bit-reproducible
@@ -374,12 +374,12 @@ def test_shape_specialised_gradient_batch(cfg, n, m):
     assert len(cs) == 1 + 4 * len(c0) + 4 * R
     ref, refI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
     out = {}
-    for mode, path in ((0, 9), (3, 5)):
+    for mode, path in ((0, 9), (4, 9), (3, 5)):     # k_deltan + k_deltaf; k_deltaf alone on both samples; the general kernel
         Mg.set_batch_mode(mode)
         Mg.set_params(cs, mws)
         nll = Mg.nll()
         st = Mg.last_call_stats()
-        assert st["norm_path"] == path and (path == 5 or st["launches"] == 1), (mode, st)
+        assert st["norm_path"] == path and (path == 5 or st["launches"] == (3 if mode == 0 else 1)), (mode, st)
         assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
         assert np.max(np.abs((nll - nll[0]) - (ref - ref[0]))) < 1e-9 * abs(ref[0])
         assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12
@@ -411,13 +411,13 @@ def test_shape_specialised_gradient_batch_falls_back():
         assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
         assert np.max(np.abs(Mg.norm_integral() - refI) / refI) < 1e-12
 
-    check(base_c, base_mw, 9, 1)
+    check(base_c, base_mw, 9, 3)
     # a point equal to point 0 and a Z pair moving together (Eq. 11) are still deltaf's
     cs, mws = np.concatenate([base_c, base_c[:1], base_c[:1]]), np.concatenate([base_mw, base_mw[:1], base_mw[:1]])
     cs[-1, 24] *= 1.0002
     assert c0[26] == c0[24]                                    # Eq. 11 in the seeded couplings
     cs[-1, 26] = cs[-1, 24]                                    # the same delta on l' = -1 and l' = +1
-    check(cs, mws, 9, 1)
+    check(cs, mws, 9, 3)
     # a fifth point on slot 3
     cs, mws = np.concatenate([base_c, base_c[:1]]), np.concatenate([base_mw, base_mw[:1]])
     cs[-1, 3] *= 1.0003
@@ -430,12 +430,12 @@ def test_shape_specialised_gradient_batch_falls_back():
     cs, mws = base_c.copy(), base_mw.copy()
     cs[2, 12] *= 1.0001
     check(cs, mws, 5)
-    # the guard: one coupling reversed -> deltaf's launch, then the general kernel's exact form (2 launches in all)
+    # the guard: one coupling reversed -> deltaf's three launches, then the general kernel's exact form (4 launches in all)
     cs, mws = base_c.copy(), base_mw.copy()
     cs[5, 4] = -c0[4]
-    check(cs, mws, 5, 2)
+    check(cs, mws, 5, 4)
     # ... and the model returns to deltaf on the next small step
-    check(base_c, base_mw, 9, 1)
+    check(base_c, base_mw, 9, 3)
 
 
 def test_nll_terms_of_two_shards_add_up():
