@@ -113,6 +113,10 @@ def traffic_from_profiles(key, n_data, n_norm):
         return None, f"kernel sources changed since capture {cap['csv']}"
     rows = list(csv.reader(open(os.path.join(ROOT, "profiles", cap["csv"]))))
     hdr, units, data = rows[0], rows[1], [r for r in rows[2:] if r]
+    if cap.get("kernel"):   # a capture of several kernels: the rows of this one
+        data = [r for r in data if cap["kernel"] in r[hdr.index("Kernel Name")]]
+        if not data:
+            return None, f"no row of {cap['kernel']} in {cap['csv']}"
     mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
     tot = []
     for r in data:
