@@ -423,6 +423,8 @@ def run_own(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if local >= torch.cuda.device_count():
+        raise SystemExit(f"bench.py: local rank {local} has no GPU (this box has {torch.cuda.device_count()}): --gpus N needs N devices")
     torch.cuda.set_device(local)
     device = torch.device("cuda", local)
     if world > 1:

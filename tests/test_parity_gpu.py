@@ -212,6 +212,9 @@ def test_nll_batched_points_small():
     assert nll.shape == (121,)
     st = Mg.last_call_stats()
     assert st["norm_path"] == 9 and st["launches"] == 3     # shape-specialised gradient-batch kernels (normalisation events twice, then data events): no columns, no matrix
+    tm = Mg.last_call_timing()                                # the three launches: normalisation pass 0, pass 1, then the data events
+    assert tm["lineshape_ms"] == 0.0 and min(tm["norm_ms"], tm["final_ms"], tm["data_ms"]) > 0.0, tm
+    assert abs(tm["norm_ms"] + tm["final_ms"] + tm["data_ms"] - Mg.recent_launch_ms(1)[-1]) < 1e-3, tm
     assert st["columns_recomputed"] == 0
     assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
     assert np.array_equal(Mg.nll(), nll)                     # bit-reproducible
