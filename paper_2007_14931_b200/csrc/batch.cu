@@ -56,6 +56,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_batch(const __grid_constant__
         bmbar_init(full, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    stage_tile_entries(a, t);
     __syncthreads();
     if (tid == 0 && (long long)blockIdx.x < ntiles) issue_stage(a, blockIdx.x, scol, sang, sw, full, nang, with_w);
     uint32_t parity = 0;

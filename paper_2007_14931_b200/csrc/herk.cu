@@ -54,6 +54,7 @@ __global__ void __launch_bounds__(BT_THREADS, (NRUN <= 4 ? HERK_MINB : 1)) k_her
         bmbar_init(t.full, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    stage_tile_entries(a, t);
     __syncthreads();
     if (tid == 0 && (long long)blockIdx.x < ntiles) issue_stage(a, blockIdx.x, t.scol, t.sang, t.sw, t.full, nang, true);
     uint32_t parity = 0;

@@ -39,6 +39,8 @@ __device__ __forceinline__ void bbulk_g2s(void* dst, const void* src, uint32_t b
                  : "memory");
 }
 
+constexpr int BT_NSCAL = 15;  // rows of the scaling table: d^J_{00} (J = 0 .. 4), d^J_{+1,0} (J = 1 .. 4), then per Z spin 0, 1, 2: lambda' = 0, |lambda'| = 1
+constexpr int BT_NBASE = 6;   // rows of the base table: K* lambda = -1, 0, +1, then Z lambda' = -1, 0, +1
 constexpr int BT_NANG = 14;   // staged cache columns: the angular ones (C_CK .. C_SPHI, C_CZ .. C_SA)
 __device__ __forceinline__ int ang_col(int j) { return j < 6 ? C_CK + j : C_CZ + (j - 6); }
 
@@ -55,57 +57,6 @@ __device__ __forceinline__ void issue_stage(const BatchArgs& a, long long tile, 
     if (with_w) bbulk_g2s(sw, a.cache + cache_idx(a.ncolw, a.ncolw - 1, i0), BT_EVENTS * 8, bar);   // (64 divides the 512-event cache block)
 }
 
-// angular factor g_xi (xi = +1, -1) of one basis entry at one event; `code` is warp-uniform
-struct Angles {
-    double cK, sK, cpsi, spsi, cphi, sphi;
-    double cZ, sZ, ct, st, cpt, spt, ca, sa;
-};
-__device__ __forceinline__ void angular_factor(const Angles& g, int code, double2* gp, double2* gm) {
-    const double RSQRT2 = 0.70710678118654752440;
-    const int kind = code >> 8, J = (code >> 4) & 15, lam = (code & 15) - 1;
-    if (kind_is_z(kind)) {
-        // d^J_{0 l'}(theta_Z) e^{i l' phi~} d^1_{l' xi}(theta~) e^{i xi alpha}   (Eq. 10); J = 0, 1, 2
-        double zf;
-        if (J == 1) zf = lam == 0 ? g.cZ : (lam > 0 ? RSQRT2 * g.sZ : -RSQRT2 * g.sZ);
-        else if (J == 0) zf = lam == 0 ? 1.0 : 0.0;
-        else zf = lam == 0 ? fma(1.5, g.cZ * g.cZ, -0.5) : (lam > 0 ? 1.2247448713915890491 : -1.2247448713915890491) * g.sZ * g.cZ;
-        const double dp = lam == 0 ? RSQRT2 * g.st : (lam > 0 ? 0.5 * (1.0 + g.ct) : 0.5 * (1.0 - g.ct));    // d^1_{l',+1}
-        const double dm = lam == 0 ? -RSQRT2 * g.st : (lam > 0 ? 0.5 * (1.0 - g.ct) : 0.5 * (1.0 + g.ct));   // d^1_{l',-1}
-        const double2 eph = lam == 0 ? make_double2(1.0, 0.0) : make_double2(g.cpt, lam > 0 ? g.spt : -g.spt);
-        *gp = cscale(zf * dp, cmul(eph, make_double2(g.ca, g.sa)));
-        *gm = cscale(zf * dm, cmul(eph, make_double2(g.ca, -g.sa)));
-        return;
-    }
-    // d^J_{l 0}(theta_K*) e^{i l phi} d^1_{l xi}(theta_psi)   (Eq. 4); the constant term is J = 0
-    const double c = g.cK, s = g.sK, c2 = c * c;
-    double dj;
-    if (lam == 0) {
-        switch (J) {
-            case 0: dj = 1.0; break;
-            case 1: dj = c; break;
-            case 2: dj = fma(1.5, c2, -0.5); break;
-            case 3: dj = c * fma(2.5, c2, -1.5); break;
-            default: dj = fma(fma(4.375, c2, -3.75), c2, 0.375); break;
-        }
-        const double h0 = RSQRT2 * g.spsi;
-        *gp = make_double2(dj * h0, 0.0);
-        *gm = make_double2(-dj * h0, 0.0);
-        return;
-    }
-    switch (J) {
-        case 1: dj = -RSQRT2 * s; break;
-        case 2: dj = -1.2247448713915890491 * s * c; break;
-        case 3: dj = -0.43301270189221932338 * s * fma(5.0, c2, -1.0); break;
-        default: dj = -0.55901699437494742410 * s * c * fma(7.0, c2, -3.0); break;
-    }
-    if (lam < 0) dj = -dj;                                                 // d^J_{-1,0} = -d^J_{+1,0}
-    const double hp = 0.5 * (1.0 + g.cpsi), hm = 0.5 * (1.0 - g.cpsi);
-    const double2 eph = make_double2(g.cphi, lam > 0 ? g.sphi : -g.sphi);
-    *gp = cscale(dj * (lam > 0 ? hp : hm), eph);
-    *gm = cscale(dj * (lam > 0 ? hm : hp), eph);
-}
-
-
 // shared-memory carve-up common to both kernels
 struct TileSmem {
     double* Bs;      // [2][KP][BT_STRIDE] basis tile, xi = +1 then -1
@@ -114,6 +65,9 @@ struct TileSmem {
     double* sang;    // staging: [BT_NANG][BT_EVENTS] angular cache columns
     double2* scol;   // staging: [ncolu][BT_EVENTS] lineshape columns
     uint64_t* full;  // mbarrier of the staging area
+    double* tabS;    // [BT_NSCAL][BT_EVENTS] the real angular scalings of the tile's events (build_basis_tile)
+    double2* tabB;   // [2 BT_NBASE][BT_EVENTS] their complex angular bases, xi = +1 then -1 per helicity row
+    int2* sent;      // [nent] (staged column, scaling row | base row << 8) per entry, decoded once per CTA
 };
 __device__ __forceinline__ TileSmem carve_tile_smem(double* smem, int KP, int ncolu) {
     TileSmem t;
@@ -123,45 +77,112 @@ __device__ __forceinline__ TileSmem carve_tile_smem(double* smem, int KP, int nc
     t.sang = t.sw + BT_EVENTS;
     t.scol = reinterpret_cast<double2*>(t.sang + BT_NANG * BT_EVENTS);
     t.full = reinterpret_cast<uint64_t*>(t.scol + (size_t)ncolu * BT_EVENTS);
+    t.tabB = reinterpret_cast<double2*>(t.full + 2);
+    t.tabS = reinterpret_cast<double*>(t.tabB + 2 * BT_NBASE * BT_EVENTS);
+    t.sent = reinterpret_cast<int2*>(t.tabS + BT_NSCAL * BT_EVENTS);
     return t;
 }
 static inline size_t tile_smem_bytes(int nent, int ncolu) {
-    return ((size_t)2 * nent * 2 * BT_STRIDE + 2 * BT_EVENTS + BT_NANG * BT_EVENTS + (size_t)ncolu * BT_EVENTS * 2) * sizeof(double) + 16;
+    return ((size_t)2 * nent * 2 * BT_STRIDE + 2 * BT_EVENTS + BT_NANG * BT_EVENTS + (size_t)ncolu * BT_EVENTS * 2) * sizeof(double) + 16 +
+           ((size_t)4 * BT_NBASE + BT_NSCAL) * BT_EVENTS * sizeof(double) + (size_t)nent * sizeof(int2);
 }
 
-// Basis tile from the staged inputs: thread (part, ev) fills entries part, part+4, ... of event ev for both helicities.
+// Once per CTA (before the first tile; all threads, followed by a barrier before the first build): the entries as the build reads
+// them.  An entry's angular factor g_xi (xi = +1, -1; `code` = kind << 8 | J << 4 | lambda + 1) is scaling x base_xi:
+//   K* (Eq. 4):  d^J_{lambda 0}(theta_K*)  x  e^{i lambda phi} d^1_{lambda xi}(theta_psi)        (the constant term is J = 0)
+//   Z (Eq. 10):  d^J_{0 lambda'}(theta_Z)  x  e^{i lambda' phi~} d^1_{lambda' xi}(theta~) e^{i xi alpha}
+// the scaling real and a function of (chain, J, |lambda|), the base complex and a function of (chain, lambda); the signs
+// d^J_{-1,0} = -d^J_{+1,0} and d^J_{0,-1} = -d^J_{0,+1} go into the lambda = -1 bases.
+__device__ __forceinline__ void stage_tile_entries(const BatchArgs& a, const TileSmem& t) {
+    for (int e = threadIdx.x; e < a.nent; e += BT_THREADS) {
+        const int2 en = a.entries[e];
+        const int kind = en.y >> 8, J = (en.y >> 4) & 15, lam = (en.y & 15) - 1;
+        const bool isz = kind_is_z(kind);
+        const int srow = isz ? 9 + 2 * J + (lam != 0) : (lam != 0 ? 4 + J : J);
+        const int brow = (isz ? 3 : 0) + lam + 1;
+        t.sent[e] = make_int2(en.x, srow | (brow << 8));
+    }
+}
+
+// Basis tile from the staged inputs, in two steps with a barrier between them.  (1) The four threads of an event fill its rows of
+// the two angular tables: K* scalings, K* bases, Z scalings, Z bases (the bases carry sqrt(w) for the Gram kernel).  (2) Thread
+// (part, ev) fills entries part, part + 4, ... of event ev for both helicities: B = BW x (scaling x base_xi) — three table loads,
+// one column load, twelve FP64 operations and four stores per entry; no switch on the entry's kind in the loop.
 // Call with all BT_THREADS threads after the staging barrier completed; follow with __syncthreads().
 // scale_sqrt_w: multiply the event's basis by sqrt(w) (Gram kernel) — then ws holds 1 for live events.
 __device__ __forceinline__ void build_basis_tile(const BatchArgs& a, const TileSmem& t, long long tile, int KP, bool with_w,
                                                  bool scale_sqrt_w = false) {
+    const double RSQRT2 = 0.70710678118654752440;
     const int tid = threadIdx.x;
     const int ev = tid & (BT_EVENTS - 1), part = tid / BT_EVENTS;
     const long long i = tile * BT_EVENTS + ev;          // < npad (npad is a multiple of 512)
     const double* sang = t.sang;
-    Angles g;
-    g.cK = sang[0 * BT_EVENTS + ev]; g.sK = sang[1 * BT_EVENTS + ev]; g.cpsi = sang[2 * BT_EVENTS + ev]; g.spsi = sang[3 * BT_EVENTS + ev];
-    g.cphi = sang[4 * BT_EVENTS + ev]; g.sphi = sang[5 * BT_EVENTS + ev];
-    if (a.have_z) {
-        g.cZ = sang[6 * BT_EVENTS + ev]; g.sZ = sang[7 * BT_EVENTS + ev]; g.ct = sang[8 * BT_EVENTS + ev]; g.st = sang[9 * BT_EVENTS + ev];
-        g.cpt = sang[10 * BT_EVENTS + ev]; g.spt = sang[11 * BT_EVENTS + ev]; g.ca = sang[12 * BT_EVENTS + ev]; g.sa = sang[13 * BT_EVENTS + ev];
-    }
     const double sc = scale_sqrt_w ? ((i < a.n) ? sqrt(t.sw[ev]) : 0.0) : 1.0;
+    double* S = t.tabS + ev;
+    double2* Bt = t.tabB + ev;
+    if (part == 0) {            // d^J_{00}(theta_K*), d^J_{+1,0}(theta_K*)
+        const double c = sang[0 * BT_EVENTS + ev], sn = sang[1 * BT_EVENTS + ev], c2 = c * c;
+        S[0 * BT_EVENTS] = 1.0;
+        S[1 * BT_EVENTS] = c;
+        S[2 * BT_EVENTS] = fma(1.5, c2, -0.5);
+        S[3 * BT_EVENTS] = c * fma(2.5, c2, -1.5);
+        S[4 * BT_EVENTS] = fma(fma(4.375, c2, -3.75), c2, 0.375);
+        S[5 * BT_EVENTS] = -RSQRT2 * sn;
+        S[6 * BT_EVENTS] = -1.2247448713915890491 * sn * c;
+        S[7 * BT_EVENTS] = -0.43301270189221932338 * sn * fma(5.0, c2, -1.0);
+        S[8 * BT_EVENTS] = -0.55901699437494742410 * sn * c * fma(7.0, c2, -3.0);
+        t.ws[ev] = (i < a.n) ? (with_w ? t.sw[ev] : 1.0) : 0.0;
+    } else if (part == 1) {     // e^{i lambda phi} d^1_{lambda xi}(theta_psi); d^J_{-1,0} = -d^J_{+1,0} goes into the lambda = -1 row
+        const double cpsi = sang[2 * BT_EVENTS + ev], spsi = sang[3 * BT_EVENTS + ev], cphi = sang[4 * BT_EVENTS + ev], sphi = sang[5 * BT_EVENTS + ev];
+        const double hp = sc * 0.5 * (1.0 + cpsi), hm = sc * 0.5 * (1.0 - cpsi), h0 = sc * RSQRT2 * spsi;
+        Bt[0 * BT_EVENTS] = make_double2(-hm * cphi, hm * sphi);     // lambda = -1, xi = +1: -d^1_{-1,+1} e^{-i phi}
+        Bt[1 * BT_EVENTS] = make_double2(-hp * cphi, hp * sphi);     //              xi = -1
+        Bt[2 * BT_EVENTS] = make_double2(h0, 0.0);                   // lambda = 0
+        Bt[3 * BT_EVENTS] = make_double2(-h0, 0.0);
+        Bt[4 * BT_EVENTS] = make_double2(hp * cphi, hp * sphi);      // lambda = +1
+        Bt[5 * BT_EVENTS] = make_double2(hm * cphi, hm * sphi);
+    } else if (part == 2) {     // d^J_{0 lambda'}(theta_Z): J = 0, 1, 2; lambda' = 0, |lambda'| = 1 (the sign of lambda' < 0 in the base)
+        if (a.have_z) {
+            const double cZ = sang[6 * BT_EVENTS + ev], sZ = sang[7 * BT_EVENTS + ev];
+            S[9 * BT_EVENTS] = 1.0;
+            S[10 * BT_EVENTS] = 0.0;
+            S[11 * BT_EVENTS] = cZ;
+            S[12 * BT_EVENTS] = RSQRT2 * sZ;
+            S[13 * BT_EVENTS] = fma(1.5, cZ * cZ, -0.5);
+            S[14 * BT_EVENTS] = 1.2247448713915890491 * sZ * cZ;
+        }
+    } else {                    // e^{i lambda' phi~} d^1_{lambda' xi}(theta~) e^{i xi alpha}   (Eq. 10)
+        if (a.have_z) {
+            const double ct = sang[8 * BT_EVENTS + ev], st = sang[9 * BT_EVENTS + ev], cpt = sang[10 * BT_EVENTS + ev], spt = sang[11 * BT_EVENTS + ev];
+            const double ca = sang[12 * BT_EVENTS + ev], sa = sang[13 * BT_EVENTS + ev];
+            const double gp = sc * 0.5 * (1.0 + ct), gm = sc * 0.5 * (1.0 - ct), g0 = sc * RSQRT2 * st;
+            const double2 ap = make_double2(ca, sa), am = make_double2(ca, -sa);
+            const double2 ep = cmul(make_double2(cpt, spt), ap), em = cmul(make_double2(cpt, spt), am);       // e^{+i phi~} e^{+-i alpha}
+            const double2 fp = cmul(make_double2(cpt, -spt), ap), fm = cmul(make_double2(cpt, -spt), am);     // e^{-i phi~} e^{+-i alpha}
+            Bt[6 * BT_EVENTS] = cscale(-gm, fp);                     // lambda' = -1: d^1_{-1,+1} = gm, sign of d^J_{0,-1} folded in
+            Bt[7 * BT_EVENTS] = cscale(-gp, fm);
+            Bt[8 * BT_EVENTS] = cscale(g0, ap);                      // lambda' = 0: d^1_{0,+1} = g0, d^1_{0,-1} = -g0
+            Bt[9 * BT_EVENTS] = cscale(-g0, am);
+            Bt[10 * BT_EVENTS] = cscale(gp, ep);                     // lambda' = +1
+            Bt[11 * BT_EVENTS] = cscale(gm, em);
+        }
+    }
+    __syncthreads();
+#pragma unroll 2
     for (int e = part; e < a.nent; e += BT_THREADS / BT_EVENTS) {
-        const int2 en = a.entries[e];                   // (staged column, code); column -1: empty entry, -2: lineshape == 1
+        const int2 en = t.sent[e];                      // (staged column, table rows); column -1: empty entry, -2: lineshape == 1
         double2 bp = make_double2(0, 0), bm = bp;
         if (en.x != -1) {
             const double2 bw = en.x >= 0 ? t.scol[(size_t)en.x * BT_EVENTS + ev] : make_double2(1.0, 0.0);
-            double2 gp, gm;
-            angular_factor(g, en.y, &gp, &gm);
+            const double sv = S[(en.y & 255) * BT_EVENTS];
+            const double2 gp = cscale(sv, Bt[2 * (en.y >> 8) * BT_EVENTS]), gm = cscale(sv, Bt[(2 * (en.y >> 8) + 1) * BT_EVENTS]);
             bp = cmul(bw, gp);
             bm = cmul(bw, gm);
-            if (scale_sqrt_w) { bp = cscale(sc, bp); bm = cscale(sc, bm); }
         }
         double* r0 = t.Bs + (size_t)(2 * e) * BT_STRIDE + ev;
         r0[0] = bp.x; r0[BT_STRIDE] = bp.y;
         r0[(size_t)KP * BT_STRIDE] = bm.x; r0[(size_t)KP * BT_STRIDE + BT_STRIDE] = bm.y;
     }
-    if (part == 0) t.ws[ev] = (i < a.n) ? (with_w ? t.sw[ev] : 1.0) : 0.0;
 }
 
 }  // namespace amp
