@@ -279,12 +279,12 @@ def timed_steps(step_fn, steps, warmup, world, device, sampler=None):
     return {"dev_ms": dev_ms, "wall_s": t_wall, "per_step_ms": per_step, "per_step_wall_ms": [w * 1e3 for w in walls], "last": last, "clocks": clocks}
 
 
-def roofline(model, args, cfg, n_data, n_norm, hbm_peak, peak_kind):
+def roofline(model, args, cfg, n_data, n_norm, hbm_peak, peak_kind, steps):
     """the roofline object of the dominant kernel of the steps just timed (kernel durations: the library's CUDA event pairs)"""
     st = model.last_call_stats()
     path = st["norm_path"]
     if path in (4, 5, 7, 8, 9):
-        t_k = [float(v) for v in model.recent_launch_ms(min(args.steps, 256))]
+        t_k = [float(v) for v in model.recent_launch_ms(min(steps, 256))]   # the launches of the `steps` calls just timed
         phase = {"lineshape": 0.0, "data": float(np.mean(t_k)), "norm": 0.0}
     else:
         tm = model.last_call_timing()
@@ -398,7 +398,7 @@ def measure(model, args, cfg, c, steps, warmup, world, device, sampler, n_data, 
         return model.nll()
 
     t = timed_steps(one_step, steps, warmup, world, device, sampler)
-    roof, phase, st = roofline(model, args, cfg, n_data, n_norm, *hbm)
+    roof, phase, st = roofline(model, args, cfg, n_data, n_norm, *hbm, steps)
     evals = P * steps * world          # replicas: every rank evaluates its own data set
     h2d = 8 * (P * model.K * 2 + P * model.R * 2)
     return {"value": evals / (t["dev_ms"] * 1e-3), "ms_per_step": t["dev_ms"] / steps, "ms_per_step_median": float(np.median(t["per_step_ms"])),
