@@ -64,7 +64,7 @@ DELTAF_FLOP_PER_NORM_EVENT = 730.0 + 190.0 + 154.0 + 25 * 11.0 + 5 * 170.0
 # counts of the ncu source page of profiles/r02_ncu_full_deltaf3.csv's report — both passes carry the forward pass of point 0.
 DELTAN0_FLOP_PER_NORM_EVENT = 1019.0
 DELTAN1_FLOP_PER_NORM_EVENT = 1705.0
-DELTAF_DATA_FLOP_PER_EVENT = 3136.0
+DELTAF_DATA_FLOP_PER_EVENT = 3086.0
 # analytic gradient: the point (730) + per coupling slot: angular factor ~8, T = sum_xi conj(g) A 16, conj(BW) T 8, weight 2
 GRAD_FLOP_PER_EVENT = 730.0 + 27 * 34.0
 # its shape-specialised form (gradf.cu): the point (730) + the three W_lambda and three Y_lambda' (u A, conj(g) A:

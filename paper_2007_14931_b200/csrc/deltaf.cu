@@ -42,10 +42,11 @@ constexpr int DELTAF_MINB = 2;               // CTAs per SM
 
 }  // namespace
 
-// The unrolled body of one phase is ~65 KB of code, twice the SM's 32 KB instruction cache, and sixteen warps drifting apart in it
-// made instruction fetch the bound (I-cache hit rate 77 %, GPC instruction-cache requests at 86 % of peak: 2.57 ms).  A CTA's
-// warps therefore meet at a named barrier at the start of a unit and of every spin class, so that each CTA is ONE stream through
-// the code (hit rate 92 %: 2.28 ms); finer meeting points cost more in waiting than they save in fetches (measured).
+// The unrolled body of one phase is ~50 KB of code, more than the SM's 32 KB instruction cache, and sixteen warps drifting apart in
+// it made instruction fetch the bound (I-cache hit rate 77 %, GPC instruction-cache requests at 86 % of peak).  A CTA's warps
+// therefore meet at a named barrier at the start of every unit, so that each CTA is ONE stream through the code (hit rate > 92 %).
+// With the exchange tree of the first version meeting again at every spin class paid (2.57 -> 2.28 ms); with the shared-memory
+// tile it no longer does (2.29 against 2.20 ms for the unit-only barrier), and finer meeting points never did.
 __device__ __forceinline__ void align_warps() { asm volatile("bar.sync 1, %0;" ::"n"(THREADS) : "memory"); }
 
 template <class SH>
@@ -248,7 +249,6 @@ __global__ void __launch_bounds__(THREADS, DELTAF_MINB) k_deltaf(const __grid_co
                                const double2 Wp, const double2 Wm, const double N0, const double N1) {
             constexpr int J = decltype(Jc)::value, CNT = decltype(CNTc)::value, OFF = decltype(OFFc)::value;
             if (CNT == 0) return;
-            align_warps();
             // the class's d functions and barrier factors again (cheaper than keeping them in registers across the other classes:
             // the kernel runs two CTAs per SM at 128 registers)
             double d0, d1;
@@ -322,7 +322,6 @@ __global__ void __launch_bounds__(THREADS, DELTAF_MINB) k_deltaf(const __grid_co
                 kstar_class(tree, norm, integral_constant<int, 4>{}, integral_constant<int, SH::n4>{}, integral_constant<int, SH::o4>{}, W0, Wp, Wm, N0, N1);
             }
             if (have_z) {
-                align_warps();
                 // the Z chain's angles again from the stage (not kept in registers across the K* classes)
                 const double mZ2 = st[C_MZ2 * UNIT];
                 const double zc0 = st[C_CZ * UNIT], zcp = RSQRT2 * st[C_SZ * UNIT];
