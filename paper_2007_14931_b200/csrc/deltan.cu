@@ -52,7 +52,7 @@ __device__ __forceinline__ void class_forward_keep(const StreamArgs& a, double m
 template <class SH, int PASS>
 __global__ void __launch_bounds__(THREADS, 1) k_deltan(const __grid_constant__ DeltaFArgs d) {
     using L = DLay<SH>;
-    constexpr int NENT = L::NENT, NSLOT = L::NSLOT, NVAL = L::NVAL;
+    constexpr int NENT = L::NENT, NSLOT = L::NSLOT;
     constexpr int NROW = 1 + 2 * NSLOT + 8 * NENT;   // partial rows: sum w S0; the leaves (x, y per slot); eight values per entry
     constexpr bool have_z = SH::nz > 0;
     constexpr int NSTAGE_N = PASS == 0 ? 4 : 2;
@@ -366,7 +366,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_deltan(const __grid_constant__ D
         d.norm_tot[0] = tot[0];
         *a.ticket = 0u;     // (the domain flag stays for the data-side launch, which reports and clears it)
     }
-    (void)NVAL;
 }
 
 namespace {
