@@ -727,6 +727,7 @@ bool build_deltaf_plan(amp_model* m) {
             changed = r;
         }
         if (changed < 0) continue;   // equal to point 0
+        if (m->res[changed].kind == AMP_CONST || m->res[changed].kind == AMP_LASS) return false;   // no entry of the specialised shapes
         const int r = changed, t = ent_of_res[r];
         const amp_resonance& rs = m->res[r];
         const bool isz = kind_is_z(rs.kind);

@@ -391,6 +391,36 @@ def test_shape_specialised_gradient_batch(cfg, n, m):
     assert np.max(np.abs(out[0] - out[3]) / np.abs(ref)) < 1e-12
 
 
+def test_gradient_batch_with_a_silent_constant_term():
+    """The paper's resonance list plus a constant term whose coupling is zero at point 0: the shape-specialised kernels still take
+    batches that leave it alone, and a point that switches it on goes to another kernel — the same numbers as the oracle either way."""
+    from paper_2007_14931_b200 import binding as B
+    cfg = 2
+    res = W.resonances(cfg) + [(W.CONST, 0, 0.0, 0.0, 0.0)]
+    Mo, Mg = O.Model(W.DECAY, res), B.Model(W.DECAY, res)
+    x, eff, xn, wn = make_inputs(cfg, 3001, 7013)
+    Mg.load_events(dev(x), dev(eff))
+    Mg.load_norm(dev(xn), dev(wn))
+    c0 = np.concatenate([W.couplings(cfg), [0.0]])
+    mw0 = np.array([[r[2], r[3]] for r in res])
+    cs = np.stack([c0] * 4)
+    mws = np.stack([mw0] * 4)
+    cs[1, 3] *= 1.001
+    cs[2, 12] *= np.exp(1e-3j)
+    mws[3, 10, 0] *= 1.0001
+    Mg.set_params(cs, mws)
+    nll = Mg.nll()
+    assert Mg.last_call_stats()["norm_path"] == 9
+    ref, _ = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+    assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
+    cs[3, -1] = 0.05 / (W.KSTARS[1][3] * W.KSTARS[1][4])      # the constant term switched on at one point (and the Z mass moved there)
+    Mg.set_params(cs, mws)
+    nll = Mg.nll()
+    assert Mg.last_call_stats()["norm_path"] != 9
+    ref, _ = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
+    assert np.max(np.abs(nll - ref) / np.abs(ref)) < RTOL_NLL
+
+
 def test_shape_specialised_gradient_batch_falls_back():
     """What deltaf.cu does not take goes to the general kernel with the same results: a fifth point on one coupling, a point that
     moves a coupling and a mass at once, two resonances at one point; and a step so large that S(p) / S(0) leaves [0.5, 1.5]
