@@ -919,7 +919,7 @@ def test_two_z_model_matches_oracle():
             mws[p, 1, 0] *= 1 + sgn * 1e-5; p += 1                                    # the K*(892) mass
     assert p == P
     rb, rI = Mo.nll(cs, x, eff, xn, wn, mass_width=mws)
-    for mode, path in ((0, 9), (3, 5)):                       # the shape-specialised kernel (two Zs compiled in), then the general one
+    for mode, path in ((0, 9), (4, 9), (3, 5)):               # the shape-specialised kernels (two Zs compiled in): three launches, one launch; the general one
         Mg.set_batch_mode(mode)
         Mg.set_params(cs, mws)
         nll = Mg.nll()
